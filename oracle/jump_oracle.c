@@ -1,0 +1,1098 @@
+/*
+ * oracle/jump_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, fp64 CPU implementation of the hot path of the Velocity-Jumps
+ * (JUMP) integrator of arXiv 2412.15073, written from /root/reference/PAPER.md
+ * ("P:Lnnn" = line nnn of that file) and the readings R-n listed in DESIGN.md.
+ * It shares no code with the CUDA path (paper_2412_15073_b200/csrc): only
+ * tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * legs may load it.
+ *
+ * What is computed, in the paper's order and notation:
+ *   - Langevin BAOAB splitting                    P:L112-125, eq. (2)
+ *   - force decomposition grad U = F0 + sum F_ij
+ *   - general jump mechanism (6),(7), Theta, f_eta P:L84-98, pairwise P:L338-346
+ *   - BPS mechanism (4),(5) for Lennard-Jones
+ *   - Poisson thinning, Algorithm 4 (step C)
+ *   - ring technique
+ *   - Algorithm 5 (step J, BPS)
+ *   - rejection sampler for G~
+ *   - C'J'AOAJ'C' scheme
+ *   - JUMP-RESPA / BAOAB-RESPA
+ *
+ * Parity pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer
+ * vectors; closed forms of Theta and of the G~ CDF/mean; chi end conditions and
+ * short+long = unsplit; finite differences of U; brute-force O(N^2) sums;
+ * stationarity identity of (6),(7); eps=inf == BPS; eps->0 mean drift == -F/m;
+ * thinning invariance under inflated bounds; OU stationary variance; BAOAB
+ * energy conservation / reversibility; 2-body Boltzmann histogram; degenerate
+ * cases.  "Parity unpinned" by the paper (fixed by DESIGN.md readings only):
+ * the formula of chi, the bound recipe L, r_M, the list policy (skin, order),
+ * the G~ proposal details, the Philox stream layout.
+ *
+ * Sign convention (R-4): every "F" here is a GRADIENT piece (grad U = sum F),
+ * physical force = -F, exactly as in the paper.
+ *
+ * Units (R-1): Angstrom, ps, g/mol; energies kcal/mol at the interface;
+ * 1 kcal/mol = 418.4 g A^2 mol^-1 ps^-2.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_KB 1.987204259e-3 /* kcal/mol/K */
+#define ORC_COULOMB 332.063713 /* kcal A / (mol e^2) */
+#define ORC_KCAL 418.4         /* internal energy units per kcal/mol */
+#define ORC_INV_SQRT_2PI 0.39894228040143267794
+#define ORC_PI 3.14159265358979323846
+
+/* flags (same meaning as the product's header, restated here on purpose) */
+#define ORC_F_COUL_JUMPS 1u
+#define ORC_F_LJ_JUMPS 2u
+#define ORC_F_EVENT_LOG 4u
+#define ORC_F_RESPA_PAPER 8u
+#define ORC_F_RESPA_COMPARATOR 16u
+
+/* weight modes of a pair term */
+enum { W_NONE = 0, W_SHORT = 1, W_LONG = 2, W_FULL = 3 };
+
+typedef struct {
+    int32_t n_atoms, n_inner, eps_mode;
+    uint32_t flags;
+    int32_t nlist_every, pad0;
+    uint64_t seed;
+    double box[3];
+    double r_short, r_switch, r_mid, r_long, ewald_alpha;
+    double dt_fs, gamma_per_ps, temperature_K;
+    double eps_jump, skin, cell_edge;
+} orc_params;
+
+typedef struct {
+    int32_t step, stream, atom, iter;
+    int32_t ring;     /* 0 = M, 1 = L, 2 = V (LJ), -1 = clock expired */
+    int32_t j;        /* partner (original index) or -1 */
+    int32_t accepted; /* 1 if the proposal was accepted */
+    int32_t n_gt;     /* attempts of the G~ rejection sampler */
+    double T, p, U, gt;
+    double margin; /* smallest distance to a discontinuity in this iteration */
+} orc_event;
+
+typedef struct {
+    int64_t proposals, accepts, gt_attempts, rebuilds, expiries;
+    double max_p, max_g_over_L, max_disp, min_margin;
+    int64_t min_margin_step;
+} orc_stats;
+
+typedef struct {
+    orc_params p;
+    int n;
+    double *x, *xu, *v, *m, *q, *sig, *eps;
+    int nb, na;
+    int *bij, *aijk;
+    double *bk, *br0, *ak, *at0;
+    int *excl_ptr, *excl_idx;
+    /* derived */
+    double kT, beta, dt, alpha, rc, h, rM, rE, skin;
+    double *sbm; /* sqrt(beta m_i) in ps/A */
+    double qmax, GM, GL, GV, eps_max, sig_min, sig_max;
+    int gnx, gny, gnz; /* contract grid for the canonical row order */
+    /* rows (CSR) built at x_build */
+    int *ptrM, *idxM, *ptrL, *idxL, *ptrV, *idxV;
+    double *x_build;
+    /* gradient pieces, kcal/mol/A */
+    double *f_bond, *f_nb, *f0, *f_long;
+    int64_t step, outer;
+    /* log + stats */
+    orc_event *ev;
+    int64_t n_ev, cap_ev;
+    orc_stats st;
+} orc_ctx;
+
+/* ------------------------------------------------------------------ */
+/* Philox4x32-10 (R-15).  Salmon et al., SC'11; restated, not copied.  */
+/* ------------------------------------------------------------------ */
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* uniform in (0,1): (2k+1) 2^-24 with k = top 23 bits, so it has 24 significant bits and is
+ * exactly representable in fp32 and fp64 (R-15; the survey's 24-bit variant needs 25 bits) */
+double orc_u01(uint32_t w) { return ((double)(w >> 9) + 0.5) * (1.0 / 8388608.0); }
+
+static void chain_block(const orc_ctx *c, int atom, int64_t step, int stream, uint32_t block, uint32_t w[4]) {
+    uint32_t ctr[4] = {(uint32_t)atom, (uint32_t)step, (uint32_t)stream, block};
+    uint32_t key[2] = {(uint32_t)(c->p.seed & 0xffffffffu), (uint32_t)(c->p.seed >> 32)};
+    orc_philox4x32_10(ctr, key, w);
+}
+
+/* ------------------------------------------------------------------ */
+/* switching function chi (R-3)                                 */
+/* ------------------------------------------------------------------ */
+void orc_chi(double r, double rc, double h, double *chi, double *dchi) {
+    double u = (r - (rc - h)) / h;
+    if (u <= 0.0) { *chi = 1.0; *dchi = 0.0; return; }
+    if (u >= 1.0) { *chi = 0.0; *dchi = 0.0; return; }
+    *chi = 1.0 - u * u * u * (10.0 - 15.0 * u + 6.0 * u * u);
+    *dchi = -30.0 * u * u * (1.0 - u) * (1.0 - u) / h;
+}
+
+/* ------------------------------------------------------------------ */
+/* pair potentials (R-2, R-8): u(r), u'(r)                             */
+/* ------------------------------------------------------------------ */
+void orc_u_coul(double r, double qq, double alpha, double *u, double *du) {
+    /* U_ij = qq erfc(alpha r)/r, qq already holds the Coulomb constant */
+    double e = erfc(alpha * r);
+    *u = qq * e / r;
+    *du = -qq * (e / (r * r) + 2.0 * alpha / sqrt(ORC_PI) * exp(-alpha * alpha * r * r) / r);
+}
+void orc_u_lj(double r, double sig, double eps, double *u, double *du) {
+    /* 4 eps [(s/r)^12 - (s/r)^6]  (P:L441 with the conventional 4, R-8) */
+    double s = sig / r, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
+    *u = 4.0 * eps * (s12 - s6);
+    *du = 4.0 * eps * (-12.0 * s12 + 6.0 * s6) / r;
+}
+/* radial derivative of w(r) u(r) for the weight modes; 0 beyond r_long */
+double orc_weighted_du(int mode, double r, double rc, double h, double rlong, double u, double du) {
+    if (mode == W_NONE || r >= rlong) return 0.0;
+    if (mode == W_FULL) return du;
+    double chi, dchi;
+    orc_chi(r, rc, h, &chi, &dchi);
+    if (mode == W_SHORT) return chi * du + dchi * u;   /* d/dr [chi u] */
+    return (1.0 - chi) * du - dchi * u;                /* d/dr [(1-chi) u] */
+}
+double orc_weighted_u(int mode, double r, double rc, double h, double rlong, double u) {
+    if (mode == W_NONE || r >= rlong) return 0.0;
+    if (mode == W_FULL) return u;
+    double chi, dchi;
+    orc_chi(r, rc, h, &chi, &dchi);
+    return mode == W_SHORT ? chi * u : (1.0 - chi) * u;
+}
+
+/* ------------------------------------------------------------------ */
+/* Theta and the jump mechanism (6),(7)  (R-5)                          */
+/* ------------------------------------------------------------------ */
+double orc_theta(double eta) {
+    /* Theta(eta) = E[(eta+G)_+] = eta Phi(eta) + phi(eta) */
+    double Phi = 0.5 * erfc(-eta / sqrt(2.0));
+    double phi = ORC_INV_SQRT_2PI * exp(-0.5 * eta * eta);
+    return eta * Phi + phi;
+}
+/* rate: lambda_ij = sqrt(beta)/(eps sqrt(m_i)) |F_ij| Theta(eta);  eps=inf -> (4) */
+double orc_jump_rate(double eps, double beta, double sbm, double g, double vn) {
+    if (isinf(eps)) return beta * g * (vn > 0.0 ? vn : 0.0);
+    return beta * g * orc_theta(eps * sbm * vn) / (eps * sbm);
+}
+/* kick (P:L344 / eq.(7)); eps=inf -> reflection (5) */
+void orc_jump_kick(double eps, double sbm, const double n[3], double gt, double v[3]) {
+    double vn = v[0] * n[0] + v[1] * n[1] + v[2] * n[2];
+    double amp;
+    if (isinf(eps)) amp = 2.0 * vn;
+    else {
+        double eta = eps * sbm * vn;
+        amp = 2.0 * eps / ((1.0 + eps * eps) * sbm) * (eta + gt);
+    }
+    v[0] -= amp * n[0]; v[1] -= amp * n[1]; v[2] -= amp * n[2];
+}
+
+/* ------------------------------------------------------------------ */
+/* G~ ~ f_eta by rejection (R-6), proposal family of P:L310.            */
+/* One Philox block per attempt, starting at *block.                    */
+/* ------------------------------------------------------------------ */
+static double upd(double m, double d) { d = fabs(d); return d < m ? d : m; }
+
+double orc_gtilde(const orc_ctx *c, double eta, int atom, int64_t step, int stream,
+                  uint32_t *block, int *attempts, double *margin) {
+    uint32_t w[4];
+    double mg = *margin;
+    int it = 0;
+    double out = 0.0;
+    for (;;) {
+        ++it;
+        chain_block(c, atom, step, stream, (*block)++, w);
+        double u0 = orc_u01(w[0]), u1 = orc_u01(w[1]), u2 = orc_u01(w[2]), u3 = orc_u01(w[3]);
+        if (eta < -2.5) {
+            double z = -(log(u0) + log(u1)) / fabs(eta); /* Gamma(2, |eta|) */
+            double a = exp(-0.5 * z * z);
+            mg = upd(mg, u2 - a);
+            if (u2 <= a) { out = z - eta; break; }
+        } else if (eta < -1.0) {
+            double z = -log(u0) / fabs(eta); /* Exponential(|eta|) */
+            double a = z * exp(0.5 * (1.0 - z * z));
+            mg = upd(mg, u1 - a);
+            if (u1 <= a) { out = z - eta; break; }
+        } else if (eta <= 0.0) {
+            double z = sqrt(-2.0 * log(u0)); /* Rayleigh */
+            double a = exp(eta * z);
+            mg = upd(mg, u1 - a);
+            if (u1 <= a) { out = z - eta; break; }
+        } else {
+            double wR = 1.0 / (1.0 + eta * sqrt(2.0 * ORC_PI)); /* Rayleigh-Gaussian mixture */
+            mg = upd(mg, u0 - wR);
+            if (u0 <= wR) { out = sqrt(-2.0 * log(u1)); break; }
+            double y = sqrt(-2.0 * log(u1)) * cos(2.0 * ORC_PI * u2);
+            mg = upd(mg, y);
+            if (y > 0.0) { out = y; break; }
+            mg = upd(mg, y + eta);
+            if (y > -eta) {
+                double a = (eta + y) / eta;
+                mg = upd(mg, u3 - a);
+                if (u3 <= a) { out = y; break; }
+            }
+        }
+        if (it >= 64) { out = (eta > 0.0) ? 0.0 : -eta + 1.0; break; } /* P < 1e-11 */
+    }
+    *attempts = it;
+    *margin = mg;
+    return out;
+}
+
+/* stand-alone entry for the distribution pins */
+double orc_gtilde_draw(double eta, uint64_t seed, int atom, int64_t step, int *attempts) {
+    orc_ctx c;
+    memset(&c, 0, sizeof c);
+    c.p.seed = seed;
+    uint32_t b = 0;
+    double mg = 1e300;
+    return orc_gtilde(&c, eta, atom, step, 99, &b, attempts, &mg);
+}
+
+/* ------------------------------------------------------------------ */
+/* geometry                                                            */
+/* ------------------------------------------------------------------ */
+static inline void min_image(const orc_ctx *c, const double *xi, const double *xj, double d[3]) {
+    for (int k = 0; k < 3; ++k) {
+        double dx = xi[k] - xj[k];
+        dx -= c->p.box[k] * nearbyint(dx / c->p.box[k]); /* P:L325, minimum image */
+        d[k] = dx;
+    }
+}
+static inline double wrap1(double x, double L) {
+    x -= L * floor(x / L);
+    if (x >= L) x -= L;
+    if (x < 0.0) x = 0.0;
+    return x;
+}
+static int is_excluded(const orc_ctx *c, int i, int j) {
+    if (!c->excl_ptr) return 0;
+    for (int k = c->excl_ptr[i]; k < c->excl_ptr[i + 1]; ++k)
+        if (c->excl_idx[k] == j) return 1;
+    return 0;
+}
+static int contract_key(const orc_ctx *c, const double *x) {
+    int cc[3], nn[3] = {c->gnx, c->gny, c->gnz};
+    for (int k = 0; k < 3; ++k) {
+        double xw = wrap1(x[k], c->p.box[k]);
+        int ci = (int)floor(xw * ((double)nn[k] / c->p.box[k]));
+        if (ci < 0) ci = 0;
+        if (ci > nn[k] - 1) ci = nn[k] - 1;
+        cc[k] = ci;
+    }
+    return (cc[2] * c->gny + cc[1]) * c->gnx + cc[0];
+}
+static int cmp_u64(const void *a, const void *b) {
+    uint64_t x = *(const uint64_t *)a, y = *(const uint64_t *)b;
+    return x < y ? -1 : (x > y ? 1 : 0);
+}
+
+/*
+ * All ordered pairs (i -> j), j != i, not excluded, with minimum-image distance
+ * rmin <= d < rmax at positions x, as CSR.  lj_only: keep eps_i eps_j > 0 only.
+ * Each row in ascending (contract cell key of j, j) order (R-10).  The search
+ * grid below is only an accelerator (checked against brute force in the tests).
+ */
+static void neighbor_csr(const orc_ctx *c, const double *x, double rmin, double rmax, int lj_only,
+                         int brute, int **ptr_out, int **idx_out) {
+    int n = c->n;
+    int ng[3];
+    for (int k = 0; k < 3; ++k) {
+        ng[k] = (int)floor(c->p.box[k] / rmax);
+        if (ng[k] < 1) ng[k] = 1;
+    }
+    int ncell = ng[0] * ng[1] * ng[2];
+    int *cell = malloc(sizeof(int) * n), *start = calloc(ncell + 1, sizeof(int)), *order = malloc(sizeof(int) * n);
+    int *jkey = malloc(sizeof(int) * n);
+    for (int i = 0; i < n; ++i) {
+        int cc[3];
+        for (int k = 0; k < 3; ++k) {
+            double xw = wrap1(x[3 * i + k], c->p.box[k]);
+            cc[k] = (int)floor(xw / c->p.box[k] * ng[k]);
+            if (cc[k] > ng[k] - 1) cc[k] = ng[k] - 1;
+        }
+        cell[i] = (cc[2] * ng[1] + cc[1]) * ng[0] + cc[0];
+        start[cell[i] + 1]++;
+        jkey[i] = contract_key(c, &x[3 * i]);
+    }
+    for (int k = 0; k < ncell; ++k) start[k + 1] += start[k];
+    {
+        int *fill = malloc(sizeof(int) * ncell);
+        memcpy(fill, start, sizeof(int) * ncell);
+        for (int i = 0; i < n; ++i) order[fill[cell[i]]++] = i;
+        free(fill);
+    }
+    int *cnt = calloc(n + 1, sizeof(int));
+    uint64_t **rows = malloc(sizeof(uint64_t *) * n);
+    double r2min = rmin * rmin, r2max = rmax * rmax;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int i = 0; i < n; ++i) {
+        int cap = 64, m = 0;
+        uint64_t *row = malloc(sizeof(uint64_t) * cap);
+        int ci = cell[i];
+        int c3[3] = {ci % ng[0], (ci / ng[0]) % ng[1], ci / (ng[0] * ng[1])};
+        int lo[3], hi[3];
+        for (int k = 0; k < 3; ++k) {
+            if (ng[k] < 3 || brute) { lo[k] = 0; hi[k] = ng[k] - 1; }
+            else { lo[k] = c3[k] - 1; hi[k] = c3[k] + 1; }
+        }
+        for (int z = lo[2]; z <= hi[2]; ++z)
+            for (int y = lo[1]; y <= hi[1]; ++y)
+                for (int xx = lo[0]; xx <= hi[0]; ++xx) {
+                    int zc = (z + ng[2]) % ng[2], yc = (y + ng[1]) % ng[1], xc = (xx + ng[0]) % ng[0];
+                    int cj = (zc * ng[1] + yc) * ng[0] + xc;
+                    for (int s = start[cj]; s < start[cj + 1]; ++s) {
+                        int j = order[s];
+                        if (j == i) continue;
+                        if (lj_only && !(c->eps[i] * c->eps[j] > 0.0)) continue;
+                        double d[3];
+                        min_image(c, &x[3 * i], &x[3 * j], d);
+                        double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+                        if (r2 >= r2max || r2 < r2min) continue;
+                        if (is_excluded(c, i, j)) continue;
+                        if (m == cap) { cap *= 2; row = realloc(row, sizeof(uint64_t) * cap); }
+                        row[m++] = ((uint64_t)(uint32_t)jkey[j] << 32) | (uint32_t)j;
+                    }
+                }
+        qsort(row, m, sizeof(uint64_t), cmp_u64);
+        rows[i] = row;
+        cnt[i + 1] = m;
+    }
+    for (int i = 0; i < n; ++i) cnt[i + 1] += cnt[i];
+    int *idx = malloc(sizeof(int) * (cnt[n] > 0 ? cnt[n] : 1));
+    for (int i = 0; i < n; ++i) {
+        int m = cnt[i + 1] - cnt[i];
+        for (int k = 0; k < m; ++k) idx[cnt[i] + k] = (int)(rows[i][k] & 0xffffffffu);
+        free(rows[i]);
+    }
+    free(rows); free(cell); free(start); free(order); free(jkey);
+    *ptr_out = cnt;
+    *idx_out = idx;
+}
+
+/* exported for the brute-force pin: returns CSR copies */
+int orc_neighbors(orc_ctx *c, double rmin, double rmax, int lj_only, int brute, int *ptr, int *idx, int cap) {
+    int *p, *ix;
+    neighbor_csr(c, c->x, rmin, rmax, lj_only, brute, &p, &ix);
+    int tot = p[c->n];
+    if (ptr) memcpy(ptr, p, sizeof(int) * (c->n + 1));
+    if (idx && tot <= cap) memcpy(idx, ix, sizeof(int) * tot);
+    free(p); free(ix);
+    return tot;
+}
+
+/* ------------------------------------------------------------------ */
+/* forces (gradients) and energies                                     */
+/* ------------------------------------------------------------------ */
+/* gradient w.r.t. x_i of w_C u_C + w_LJ u_LJ for the pair (i,j); returns energy share */
+static double pair_gradient(const orc_ctx *c, int i, int j, int wC, int wLJ, double g[3]) {
+    double d[3];
+    min_image(c, &c->x[3 * i], &c->x[3 * j], d);
+    double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    double fr = 0.0, e = 0.0;
+    if (wC != W_NONE && c->q[i] * c->q[j] != 0.0) {
+        double u, du;
+        orc_u_coul(r, ORC_COULOMB * c->q[i] * c->q[j], c->alpha, &u, &du);
+        fr += orc_weighted_du(wC, r, c->rc, c->h, c->rE, u, du);
+        e += orc_weighted_u(wC, r, c->rc, c->h, c->rE, u);
+    }
+    if (wLJ != W_NONE && c->eps[i] * c->eps[j] > 0.0) {
+        double u, du;
+        orc_u_lj(r, sqrt(c->sig[i] * c->sig[j]), sqrt(c->eps[i] * c->eps[j]), &u, &du); /* R-8 */
+        fr += orc_weighted_du(wLJ, r, c->rc, c->h, c->rE, u, du);
+        e += orc_weighted_u(wLJ, r, c->rc, c->h, c->rE, u);
+    }
+    for (int k = 0; k < 3; ++k) g[k] = fr * d[k] / r;
+    return e;
+}
+
+/* out[3n] += sum_j grad_i; returns the pair energy (each pair counted once) */
+static double pairs_accumulate(const orc_ctx *c, int wC, int wLJ, int brute, double *out) {
+    double rmax = c->rE;
+    if ((wC == W_SHORT || wC == W_NONE) && (wLJ == W_SHORT || wLJ == W_NONE)) rmax = c->rc;
+    int *ptr, *idx;
+    neighbor_csr(c, c->x, 0.0, rmax, 0, brute, &ptr, &idx);
+    double etot = 0.0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : etot)
+    for (int i = 0; i < c->n; ++i) {
+        double acc[3] = {0, 0, 0}, e = 0.0;
+        for (int k = ptr[i]; k < ptr[i + 1]; ++k) {
+            double g[3];
+            e += pair_gradient(c, i, idx[k], wC, wLJ, g);
+            acc[0] += g[0]; acc[1] += g[1]; acc[2] += g[2];
+        }
+        out[3 * i] += acc[0]; out[3 * i + 1] += acc[1]; out[3 * i + 2] += acc[2];
+        etot += 0.5 * e;
+    }
+    free(ptr); free(idx);
+    return etot;
+}
+
+/* harmonic bonds k (r-r0)^2 and angles k (theta-theta0)^2 (R-2); serial, tiny */
+static double bonded_accumulate(const orc_ctx *c, double *out) {
+    double e = 0.0;
+    for (int b = 0; b < c->nb; ++b) {
+        int i = c->bij[2 * b], j = c->bij[2 * b + 1];
+        double d[3];
+        min_image(c, &c->x[3 * i], &c->x[3 * j], d);
+        double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        double dr = r - c->br0[b];
+        e += c->bk[b] * dr * dr;
+        double f = 2.0 * c->bk[b] * dr / r;
+        for (int k = 0; k < 3; ++k) { out[3 * i + k] += f * d[k]; out[3 * j + k] -= f * d[k]; }
+    }
+    for (int a = 0; a < c->na; ++a) {
+        int i = c->aijk[3 * a], j = c->aijk[3 * a + 1], k2 = c->aijk[3 * a + 2]; /* j = vertex */
+        double u[3], w[3];
+        min_image(c, &c->x[3 * i], &c->x[3 * j], u);
+        min_image(c, &c->x[3 * k2], &c->x[3 * j], w);
+        double lu = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
+        double lw = sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+        double ct = (u[0] * w[0] + u[1] * w[1] + u[2] * w[2]) / (lu * lw);
+        if (ct > 1.0) ct = 1.0;
+        if (ct < -1.0) ct = -1.0;
+        double th = acos(ct), st = sqrt(1.0 - ct * ct);
+        if (st < 1e-12) st = 1e-12;
+        double dth = th - c->at0[a];
+        e += c->ak[a] * dth * dth;
+        double dU = 2.0 * c->ak[a] * dth;
+        for (int k = 0; k < 3; ++k) {
+            double gi = -dU * (w[k] / lw - ct * u[k] / lu) / (lu * st);
+            double gk = -dU * (u[k] / lu - ct * w[k] / lw) / (lw * st);
+            out[3 * i + k] += gi;
+            out[3 * k2 + k] += gk;
+            out[3 * j + k] -= gi + gk;
+        }
+    }
+    return e;
+}
+
+/* F0 = bonded + short non-bonded (R-13: LJ tail stays in F0 when LJ jumps are off) */
+static void f0_modes(const orc_ctx *c, int *wC, int *wLJ) {
+    *wC = W_SHORT;
+    *wLJ = (c->p.flags & ORC_F_LJ_JUMPS) ? W_SHORT : W_FULL;
+}
+static void long_modes(const orc_ctx *c, int *wC, int *wLJ) {
+    *wC = W_LONG;
+    *wLJ = (c->p.flags & ORC_F_LJ_JUMPS) ? W_LONG : W_NONE;
+}
+static void compute_f0(orc_ctx *c) {
+    int wC, wLJ;
+    f0_modes(c, &wC, &wLJ);
+    memset(c->f_bond, 0, sizeof(double) * 3 * c->n);
+    memset(c->f_nb, 0, sizeof(double) * 3 * c->n);
+    bonded_accumulate(c, c->f_bond);
+    pairs_accumulate(c, wC, wLJ, 0, c->f_nb);
+    for (int k = 0; k < 3 * c->n; ++k) c->f0[k] = c->f_bond[k] + c->f_nb[k];
+}
+static void compute_bonded_only(orc_ctx *c) {
+    memset(c->f_bond, 0, sizeof(double) * 3 * c->n);
+    bonded_accumulate(c, c->f_bond);
+}
+static void compute_long(orc_ctx *c) {
+    int wC, wLJ;
+    long_modes(c, &wC, &wLJ);
+    memset(c->f_long, 0, sizeof(double) * 3 * c->n);
+    pairs_accumulate(c, wC, wLJ, 0, c->f_long);
+}
+static void compute_full(orc_ctx *c, double *out) { /* BAOAB comparator: unsplit to r_long */
+    memset(out, 0, sizeof(double) * 3 * c->n);
+    bonded_accumulate(c, out);
+    pairs_accumulate(c, W_FULL, W_FULL, 0, out);
+}
+
+/* which: 0 F0, 1 full, 2 long, 3 bonded, 4 short non-bonded; brute != 0 -> O(N^2) sweep */
+void orc_forces(orc_ctx *c, int which, int brute, double *out) {
+    int wC, wLJ;
+    memset(out, 0, sizeof(double) * 3 * c->n);
+    if (which == 0) { f0_modes(c, &wC, &wLJ); bonded_accumulate(c, out); pairs_accumulate(c, wC, wLJ, brute, out); }
+    else if (which == 1) { bonded_accumulate(c, out); pairs_accumulate(c, W_FULL, W_FULL, brute, out); }
+    else if (which == 2) { long_modes(c, &wC, &wLJ); pairs_accumulate(c, wC, wLJ, brute, out); }
+    else if (which == 3) bonded_accumulate(c, out);
+    else if (which == 4) { f0_modes(c, &wC, &wLJ); pairs_accumulate(c, wC, wLJ, brute, out); }
+}
+/* which as above; returns potential energy in kcal/mol */
+double orc_potential(orc_ctx *c, int which) {
+    double *tmp = calloc(3 * c->n, sizeof(double));
+    double e = 0.0;
+    int wC, wLJ;
+    if (which == 0) { f0_modes(c, &wC, &wLJ); e = bonded_accumulate(c, tmp) + pairs_accumulate(c, wC, wLJ, 0, tmp); }
+    else if (which == 1) e = bonded_accumulate(c, tmp) + pairs_accumulate(c, W_FULL, W_FULL, 0, tmp);
+    else if (which == 2) { long_modes(c, &wC, &wLJ); e = pairs_accumulate(c, wC, wLJ, 0, tmp); }
+    else if (which == 3) e = bonded_accumulate(c, tmp);
+    else if (which == 4) { f0_modes(c, &wC, &wLJ); e = pairs_accumulate(c, wC, wLJ, 0, tmp); }
+    free(tmp);
+    return e;
+}
+double orc_kinetic(const orc_ctx *c) {
+    double e = 0.0;
+    for (int i = 0; i < c->n; ++i)
+        e += 0.5 * c->m[i] * (c->v[3 * i] * c->v[3 * i] + c->v[3 * i + 1] * c->v[3 * i + 1] + c->v[3 * i + 2] * c->v[3 * i + 2]);
+    return e / ORC_KCAL;
+}
+
+/* single-pair long-range gradient pieces used by the jump chains */
+static double fij_coul(const orc_ctx *c, int i, int j, double F[3]) {
+    double d[3];
+    min_image(c, &c->x[3 * i], &c->x[3 * j], d);
+    double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    double u, du;
+    orc_u_coul(r, ORC_COULOMB * c->q[i] * c->q[j], c->alpha, &u, &du);
+    double fr = orc_weighted_du(W_LONG, r, c->rc, c->h, c->rE, u, du);
+    for (int k = 0; k < 3; ++k) F[k] = fr * d[k] / r;
+    return fabs(fr);
+}
+static double fij_lj(const orc_ctx *c, int i, int j, double F[3]) {
+    double d[3];
+    min_image(c, &c->x[3 * i], &c->x[3 * j], d);
+    double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+    double u, du;
+    orc_u_lj(r, sqrt(c->sig[i] * c->sig[j]), sqrt(c->eps[i] * c->eps[j]), &u, &du);
+    double fr = orc_weighted_du(W_LONG, r, c->rc, c->h, c->rE, u, du);
+    for (int k = 0; k < 3; ++k) F[k] = fr * d[k] / r;
+    return fabs(fr);
+}
+
+/* ------------------------------------------------------------------ */
+/* bounds L (R-7): sup on a dense grid, times (1 + 1e-6)               */
+/* ------------------------------------------------------------------ */
+static double sup_coul(const orc_ctx *c, double lo, double hi) {
+    if (!(hi > lo)) return 0.0;
+    double best = 0.0;
+    long K = (long)floor((hi - lo) / 1e-4);
+    for (long k = 0; k <= K + 1; ++k) {
+        double r = (k <= K) ? lo + 1e-4 * (double)k : hi;
+        if (r > hi) r = hi;
+        double u, du;
+        orc_u_coul(r, ORC_COULOMB, c->alpha, &u, &du);
+        double chi, dchi;
+        orc_chi(r, c->rc, c->h, &chi, &dchi);
+        double g = fabs((1.0 - chi) * du - dchi * u);
+        if (g > best) best = g;
+    }
+    return best * (1.0 + 1e-6);
+}
+static double sup_lj(const orc_ctx *c, double lo, double hi) { /* 4 eps = 1; sup over sigma range too */
+    if (!(hi > lo) || !(c->sig_max > 0.0)) return 0.0;
+    double best = 0.0;
+    int NS = (c->sig_max > c->sig_min) ? 65 : 1;
+    long K = (long)floor((hi - lo) / 1e-3);
+    for (int s = 0; s < NS; ++s) {
+        double sig = (NS == 1) ? c->sig_min : c->sig_min + (c->sig_max - c->sig_min) * (double)s / (double)(NS - 1);
+        for (long k = 0; k <= K + 1; ++k) {
+            double r = (k <= K) ? lo + 1e-3 * (double)k : hi;
+            if (r > hi) r = hi;
+            double u, du;
+            orc_u_lj(r, sig, 0.25, &u, &du);
+            double chi, dchi;
+            orc_chi(r, c->rc, c->h, &chi, &dchi);
+            double g = fabs((1.0 - chi) * du - dchi * u);
+            if (g > best) best = g;
+        }
+    }
+    return best * (1.0 + 1e-6);
+}
+static double dmin(double a, double b) { return a < b ? a : b; }
+static double dmax(double a, double b) { return a > b ? a : b; }
+
+static void compute_bounds(orc_ctx *c) {
+    c->qmax = 0.0; c->eps_max = 0.0; c->sig_min = 1e300; c->sig_max = 0.0;
+    for (int i = 0; i < c->n; ++i) {
+        c->qmax = dmax(c->qmax, fabs(c->q[i]));
+        if (c->eps[i] > 0.0) {
+            c->eps_max = dmax(c->eps_max, c->eps[i]);
+            c->sig_min = dmin(c->sig_min, c->sig[i]);
+            c->sig_max = dmax(c->sig_max, c->sig[i]);
+        }
+    }
+    if (c->eps_max == 0.0) { c->sig_min = 0.0; c->sig_max = 0.0; }
+    double lo = c->rc - c->h;
+    c->GM = sup_coul(c, lo, dmin(c->rM + c->skin, c->rE));
+    c->GL = sup_coul(c, dmax(c->rM - c->skin, lo), c->rE);
+    c->GV = sup_lj(c, lo, c->rE);
+}
+/* per-atom bounds, uniform in j */
+static double LM_of(const orc_ctx *c, int i) { return fabs(c->q[i]) * c->qmax * c->GM; }
+static double LL_of(const orc_ctx *c, int i) { return fabs(c->q[i]) * c->qmax * c->GL; }
+static double LV_of(const orc_ctx *c, int i) { return 4.0 * sqrt(c->eps[i] * c->eps_max) * c->GV; }
+
+void orc_get_bounds(const orc_ctx *c, double out[8]) {
+    out[0] = c->GM; out[1] = c->GL; out[2] = c->GV; out[3] = c->qmax;
+    out[4] = c->eps_max; out[5] = c->sig_min; out[6] = c->sig_max; out[7] = c->rM;
+}
+
+/* ------------------------------------------------------------------ */
+/* ring rows (R-10)                                         */
+/* ------------------------------------------------------------------ */
+static void rebuild_rows(orc_ctx *c) {
+    free(c->ptrM); free(c->idxM); free(c->ptrL); free(c->idxL); free(c->ptrV); free(c->idxV);
+    double s = c->skin, lo = c->rc - c->h - s;
+    if (lo < 0.0) lo = 0.0;
+    neighbor_csr(c, c->x, lo, c->rM, 0, 0, &c->ptrM, &c->idxM);
+    neighbor_csr(c, c->x, dmax(c->rM, lo), c->rE + s, 0, 0, &c->ptrL, &c->idxL);
+    neighbor_csr(c, c->x, lo, c->rE + s, 1, 0, &c->ptrV, &c->idxV);
+    memcpy(c->x_build, c->x, sizeof(double) * 3 * c->n);
+    c->st.rebuilds++;
+}
+static void check_displacement(orc_ctx *c) {
+    double mx = 0.0;
+    for (int i = 0; i < c->n; ++i) {
+        double d[3];
+        min_image(c, &c->x[3 * i], &c->x_build[3 * i], d);
+        double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        if (r > mx) mx = r;
+    }
+    if (mx > c->st.max_disp) c->st.max_disp = mx;
+}
+void orc_get_row_counts(const orc_ctx *c, int *nM, int *nL, int *nV) {
+    for (int i = 0; i < c->n; ++i) {
+        nM[i] = c->ptrM[i + 1] - c->ptrM[i];
+        nL[i] = c->ptrL[i + 1] - c->ptrL[i];
+        nV[i] = c->ptrV[i + 1] - c->ptrV[i];
+    }
+}
+/* which: 0 M, 1 L, 2 V */
+int orc_get_row(const orc_ctx *c, int which, int i, int *out, int cap) {
+    const int *ptr = which == 0 ? c->ptrM : (which == 1 ? c->ptrL : c->ptrV);
+    const int *idx = which == 0 ? c->idxM : (which == 1 ? c->idxL : c->idxV);
+    int m = ptr[i + 1] - ptr[i];
+    for (int k = 0; k < m && k < cap; ++k) out[k] = idx[ptr[i] + k];
+    return m;
+}
+
+/* ------------------------------------------------------------------ */
+/* event log                                                           */
+/* ------------------------------------------------------------------ */
+static void log_event(orc_ctx *c, const orc_event *e) {
+#pragma omp critical(orc_log)
+    {
+        if (e->margin < c->st.min_margin) { c->st.min_margin = e->margin; c->st.min_margin_step = e->step; }
+        if (c->p.flags & ORC_F_EVENT_LOG) {
+            if (c->n_ev == c->cap_ev) {
+                c->cap_ev = c->cap_ev ? 2 * c->cap_ev : 65536;
+                c->ev = realloc(c->ev, sizeof(orc_event) * c->cap_ev);
+            }
+            c->ev[c->n_ev++] = *e;
+        }
+    }
+}
+static int cmp_event(const void *a, const void *b) {
+    const orc_event *x = a, *y = b;
+    if (x->step != y->step) return x->step < y->step ? -1 : 1;
+    if (x->stream != y->stream) return x->stream < y->stream ? -1 : 1;
+    if (x->atom != y->atom) return x->atom < y->atom ? -1 : 1;
+    return x->iter < y->iter ? -1 : (x->iter > y->iter ? 1 : 0);
+}
+int64_t orc_get_events(orc_ctx *c, orc_event *buf, int64_t cap) {
+    qsort(c->ev, c->n_ev, sizeof(orc_event), cmp_event);
+    int64_t m = c->n_ev < cap ? c->n_ev : cap;
+    if (buf) memcpy(buf, c->ev, sizeof(orc_event) * m);
+    return c->n_ev;
+}
+void orc_clear_events(orc_ctx *c) { c->n_ev = 0; }
+void orc_get_stats(const orc_ctx *c, orc_stats *out) { *out = c->st; }
+void orc_reset_stats(orc_ctx *c) {
+    memset(&c->st, 0, sizeof c->st);
+    c->st.min_margin = 1e300;
+}
+
+/* ------------------------------------------------------------------ */
+/* Step (C'): Algorithm 4 with the ring technique (R-11)               */
+/* P:L352-420.  Position x frozen; one chain per atom.     */
+/* ------------------------------------------------------------------ */
+static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int stream, int64_t step,
+                         int64_t *n_prop, int64_t *n_acc, int64_t *n_gt, int64_t *n_exp, double *max_p, double *max_gl) {
+    double *v = &c->v[3 * i];
+    const double eps = c->p.eps_jump, sbm = c->sbm[i], beta = c->beta;
+    const int bps = isinf(eps);
+    const int NM = c->ptrM[i + 1] - c->ptrM[i], NL = c->ptrL[i + 1] - c->ptrL[i];
+    const double LM = LM_of(c, i), LL = LL_of(c, i);
+    const double SM = (double)NM * LM, S = SM + (double)NL * LL;
+    double t = 0.0;
+    uint32_t block = 0;
+    uint32_t w[4];
+    for (int iter = 0;; ++iter) {
+        orc_event ev;
+        memset(&ev, 0, sizeof ev);
+        ev.step = (int32_t)step; ev.stream = stream; ev.atom = i; ev.iter = iter; ev.ring = -1; ev.j = -1;
+        double mg = 1e300;
+        double tau = H - t;
+        double va = v[0] * a[0] + v[1] * a[1] + v[2] * a[2];
+        double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2], a2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
+        double Bv = sqrt(v2 + tau * tau * a2 + 2.0 * tau * (va > 0.0 ? va : 0.0));
+        double lam = bps ? S * beta * Bv
+                         : S * (beta * Bv + (1.0 / eps) * beta * ORC_INV_SQRT_2PI / sbm);
+        chain_block(c, i, step, stream, block++, w);
+        double E = -log(orc_u01(w[0]));
+        double T = lam > 0.0 ? E / lam : INFINITY;
+        ev.T = T;
+        if (isfinite(T)) mg = upd(mg, (t + T - H) / H);
+        if (t + T > H) {
+            v[0] += tau * a[0]; v[1] += tau * a[1]; v[2] += tau * a[2];
+            ev.margin = mg;
+            (*n_exp)++;
+            log_event(c, &ev);
+            break;
+        }
+        t += T;
+        v[0] += T * a[0]; v[1] += T * a[1]; v[2] += T * a[2];
+        /* ring pick */
+        double ur = orc_u01(w[1]);
+        int ring;
+        if (NM > 0 && NL > 0) mg = upd(mg, ur - SM / S);
+        ring = (ur * S < SM) ? 0 : 1;
+        if (ring == 0 && NM == 0) ring = 1;
+        if (ring == 1 && NL == 0) ring = 0;
+        int cnt = ring == 0 ? NM : NL;
+        int k = (int)(((uint64_t)w[2] * (uint64_t)cnt) >> 32);
+        int j = ring == 0 ? c->idxM[c->ptrM[i] + k] : c->idxL[c->ptrL[i] + k];
+        double LY = ring == 0 ? LM : LL;
+        double U = orc_u01(w[3]);
+        ev.ring = ring; ev.j = j; ev.U = U;
+        (*n_prop)++;
+        double F[3];
+        double g = fij_coul(c, i, j, F);
+        if (g > 0.0) {
+            if (g / LY > *max_gl) *max_gl = g / LY;
+            double n[3] = {F[0] / g, F[1] / g, F[2] / g};
+            double vn = v[0] * n[0] + v[1] * n[1] + v[2] * n[2];
+            double p;
+            if (bps) p = (vn > 0.0 ? vn : 0.0) * g / (LY * Bv);
+            else p = g * orc_theta(eps * sbm * vn) / (LY * (Bv * eps * sbm + ORC_INV_SQRT_2PI)); /* P:L397 + sqrt(beta) */
+            ev.p = p;
+            if (p > *max_p) *max_p = p;
+            mg = upd(mg, U - p);
+            if (U <= p) {
+                double gt = 0.0;
+                int att = 0;
+                if (!bps) gt = orc_gtilde(c, eps * sbm * vn, i, step, stream, &block, &att, &mg);
+                orc_jump_kick(eps, sbm, n, gt, v);
+                ev.accepted = 1; ev.gt = gt; ev.n_gt = att;
+                (*n_acc)++;
+                (*n_gt) += att;
+            }
+        }
+        ev.margin = mg;
+        log_event(c, &ev);
+    }
+}
+
+/* Step (J'): Algorithm 5 (BPS on the long LJ part), exponential clock (R-14). P:L466-505 */
+static void chain_J_atom(orc_ctx *c, int i, double H, int stream, int64_t step,
+                         int64_t *n_prop, int64_t *n_acc, int64_t *n_exp, double *max_p, double *max_gl) {
+    const int NV = c->ptrV[i + 1] - c->ptrV[i];
+    if (!(c->eps[i] > 0.0) || NV == 0) return;
+    double *v = &c->v[3 * i];
+    const double L = LV_of(c, i);
+    double t = 0.0;
+    uint32_t block = 0;
+    uint32_t w[4];
+    for (int iter = 0;; ++iter) {
+        orc_event ev;
+        memset(&ev, 0, sizeof ev);
+        ev.step = (int32_t)step; ev.stream = stream; ev.atom = i; ev.iter = iter; ev.ring = -1; ev.j = -1;
+        double mg = 1e300;
+        double vv = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+        double lam = (double)NV * c->beta * vv * L;
+        chain_block(c, i, step, stream, block++, w);
+        double E = -log(orc_u01(w[0]));
+        double T = lam > 0.0 ? E / lam : INFINITY;
+        ev.T = T;
+        if (isfinite(T)) mg = upd(mg, (t + T - H) / H);
+        if (t + T > H) { ev.margin = mg; (*n_exp)++; log_event(c, &ev); break; }
+        t += T;
+        int k = (int)(((uint64_t)w[1] * (uint64_t)NV) >> 32);
+        int j = c->idxV[c->ptrV[i] + k];
+        double U = orc_u01(w[2]);
+        ev.ring = 2; ev.j = j; ev.U = U;
+        (*n_prop)++;
+        double F[3];
+        double g = fij_lj(c, i, j, F);
+        if (g > 0.0) {
+            if (g / L > *max_gl) *max_gl = g / L;
+            double vF = v[0] * F[0] + v[1] * F[1] + v[2] * F[2];
+            double p = (vF > 0.0 ? vF : 0.0) / (vv * L);
+            ev.p = p;
+            if (p > *max_p) *max_p = p;
+            mg = upd(mg, U - p);
+            if (U <= p) { /* reflection (5) */
+                double n[3] = {F[0] / g, F[1] / g, F[2] / g};
+                orc_jump_kick(INFINITY, c->sbm[i], n, 0.0, v);
+                ev.accepted = 1;
+                (*n_acc)++;
+            }
+        }
+        ev.margin = mg;
+        log_event(c, &ev);
+    }
+}
+
+/* C over all atoms; acc_src: gradient array giving a = -M^-1 F (NULL -> a = 0) */
+static void phase_C(orc_ctx *c, double H, const double *grad, int stream, int64_t step) {
+    int64_t np = 0, nacc = 0, ngt = 0, nexp = 0;
+    double mp = 0.0, mgl = 0.0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : np, nacc, ngt, nexp) reduction(max : mp, mgl)
+    for (int i = 0; i < c->n; ++i) {
+        double a[3] = {0, 0, 0};
+        if (grad)
+            for (int k = 0; k < 3; ++k) a[k] = -(ORC_KCAL / c->m[i]) * grad[3 * i + k];
+        chain_C_atom(c, i, H, a, stream, step, &np, &nacc, &ngt, &nexp, &mp, &mgl);
+    }
+    c->st.proposals += np; c->st.accepts += nacc; c->st.gt_attempts += ngt; c->st.expiries += nexp;
+    if (mp > c->st.max_p) c->st.max_p = mp;
+    if (mgl > c->st.max_g_over_L) c->st.max_g_over_L = mgl;
+}
+static void phase_J(orc_ctx *c, double H, int stream, int64_t step) {
+    int64_t np = 0, nacc = 0, nexp = 0;
+    double mp = 0.0, mgl = 0.0;
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : np, nacc, nexp) reduction(max : mp, mgl)
+    for (int i = 0; i < c->n; ++i) chain_J_atom(c, i, H, stream, step, &np, &nacc, &nexp, &mp, &mgl);
+    c->st.proposals += np; c->st.accepts += nacc; c->st.expiries += nexp;
+    if (mp > c->st.max_p) c->st.max_p = mp;
+    if (mgl > c->st.max_g_over_L) c->st.max_g_over_L = mgl;
+}
+/* plain (B): v <- v - H M^-1 F, written as v += H a so that it is bit-identical to an event-free (C) */
+static void phase_B(orc_ctx *c, double H, const double *grad) {
+    for (int i = 0; i < c->n; ++i)
+        for (int k = 0; k < 3; ++k) {
+            double a = -(ORC_KCAL / c->m[i]) * grad[3 * i + k];
+            c->v[3 * i + k] += H * a;
+        }
+}
+/* C' then J' (fwd) or J' then C' (reverse) over a duration H */
+static void jump_phase(orc_ctx *c, double H, const double *grad, int sC, int sJ, int64_t step, int reverse) {
+    int coul = (c->p.flags & ORC_F_COUL_JUMPS) != 0, lj = (c->p.flags & ORC_F_LJ_JUMPS) != 0;
+    if (reverse && lj) phase_J(c, H, sJ, step);
+    if (coul) phase_C(c, H, grad, sC, step);
+    else if (grad) phase_B(c, H, grad);
+    if (!reverse && lj) phase_J(c, H, sJ, step);
+}
+
+/* (A) P:L119 and (O) P:L121-123 */
+static void phase_A(orc_ctx *c, double H) {
+    for (int k = 0; k < 3 * c->n; ++k) { c->x[k] += H * c->v[k]; c->xu[k] += H * c->v[k]; }
+}
+static void phase_O(orc_ctx *c, double dt, int64_t step) {
+    double c1 = exp(-c->p.gamma_per_ps * dt), c2 = sqrt(1.0 - c1 * c1);
+    for (int i = 0; i < c->n; ++i) {
+        uint32_t w[4];
+        chain_block(c, i, step, 0, 0, w);
+        double r1 = sqrt(-2.0 * log(orc_u01(w[0]))), a1 = 2.0 * ORC_PI * orc_u01(w[1]);
+        double r2 = sqrt(-2.0 * log(orc_u01(w[2]))), a2 = 2.0 * ORC_PI * orc_u01(w[3]);
+        double G[3] = {r1 * cos(a1), r1 * sin(a1), r2 * cos(a2)};
+        for (int k = 0; k < 3; ++k) c->v[3 * i + k] = c1 * c->v[3 * i + k] + c2 / c->sbm[i] * G[k];
+    }
+}
+static void wrap_all(orc_ctx *c) {
+    for (int i = 0; i < c->n; ++i)
+        for (int k = 0; k < 3; ++k) c->x[3 * i + k] = wrap1(c->x[3 * i + k], c->p.box[k]);
+}
+/* A O A, wrap, step counter, scheduled rebuild (steps 3-6 of C.3) */
+static void aoa_and_lists(orc_ctx *c) {
+    phase_A(c, 0.5 * c->dt);
+    phase_O(c, c->dt, c->step);
+    phase_A(c, 0.5 * c->dt);
+    wrap_all(c);
+    c->step++;
+    check_displacement(c);
+    if (c->p.nlist_every > 0 && c->step % c->p.nlist_every == 0) rebuild_rows(c);
+}
+
+/* ------------------------------------------------------------------ */
+/* public steps                                                        */
+/* ------------------------------------------------------------------ */
+/* C'J'AOAJ'C' */
+void orc_jump_step(orc_ctx *c, int nsteps) {
+    for (int s = 0; s < nsteps; ++s) {
+        int64_t st = c->step;
+        jump_phase(c, 0.5 * c->dt, c->f0, 1, 2, st, 0);
+        aoa_and_lists(c);
+        compute_f0(c);
+        jump_phase(c, 0.5 * c->dt, c->f0, 4, 3, st, 1);
+    }
+}
+/* BAOAB with the unsplit force to r_long (P:L112-125 without J) */
+void orc_baoab_step(orc_ctx *c, int nsteps) {
+    double *f = malloc(sizeof(double) * 3 * c->n);
+    compute_full(c, f);
+    for (int s = 0; s < nsteps; ++s) {
+        phase_B(c, 0.5 * c->dt, f);
+        aoa_and_lists(c);
+        compute_full(c, f);
+        phase_B(c, 0.5 * c->dt, f);
+    }
+    free(f);
+    compute_f0(c);
+}
+/* JUMP-RESPA / BAOAB-RESPA (R-12) */
+void orc_jump_respa_step(orc_ctx *c, int nouter) {
+    const int n = c->p.n_inner;
+    const double D = n * c->dt;
+    const int paper = (c->p.flags & ORC_F_RESPA_PAPER) != 0, cmp = (c->p.flags & ORC_F_RESPA_COMPARATOR) != 0;
+    double *fout = malloc(sizeof(double) * 3 * c->n);
+    for (int o = 0; o < nouter; ++o) {
+        for (int half = 0; half < 2; ++half) {
+            if (half == 1) { /* inner loop: n x BAOAB_delta with F_in */
+                for (int s = 0; s < n; ++s) {
+                    const double *fin = paper ? c->f_bond : c->f0;
+                    phase_B(c, 0.5 * c->dt, fin);
+                    aoa_and_lists(c);
+                    if (paper) compute_bonded_only(c); else compute_f0(c);
+                    phase_B(c, 0.5 * c->dt, paper ? c->f_bond : c->f0);
+                }
+                if (paper) compute_f0(c); /* short non-bonded at the new x for the closing outer phase */
+            }
+            if (cmp) {
+                compute_long(c);
+                for (int k = 0; k < 3 * c->n; ++k) fout[k] = c->f_long[k] + (paper ? c->f_nb[k] : 0.0);
+                phase_B(c, 0.5 * D, fout);
+            } else {
+                const double *grad = paper ? c->f_nb : NULL;
+                if (half == 0) jump_phase(c, 0.5 * D, grad, 5, 6, c->outer, 0);
+                else jump_phase(c, 0.5 * D, grad, 8, 7, c->outer, 1);
+            }
+        }
+        c->outer++;
+    }
+    free(fout);
+}
+
+/* ------------------------------------------------------------------ */
+/* life cycle                                                          */
+/* ------------------------------------------------------------------ */
+static void *dup_mem(const void *src, size_t bytes) {
+    void *p = malloc(bytes > 0 ? bytes : 1);
+    if (src && bytes) memcpy(p, src, bytes);
+    return p;
+}
+orc_ctx *orc_create(const orc_params *p, const double *pos, const double *vel, const double *mass,
+                    const double *charge, const double *sigma, const double *eps, int n_bonds, const int *bond_ij,
+                    const double *bond_k, const double *bond_r0, int n_angles, const int *angle_ijk,
+                    const double *angle_k, const double *angle_t0, const int *excl_ptr, const int *excl_idx) {
+    orc_ctx *c = calloc(1, sizeof(orc_ctx));
+    c->p = *p;
+    int n = c->n = p->n_atoms;
+    c->x = dup_mem(pos, sizeof(double) * 3 * n);
+    c->xu = dup_mem(pos, sizeof(double) * 3 * n);
+    c->v = dup_mem(vel, sizeof(double) * 3 * n);
+    c->m = dup_mem(mass, sizeof(double) * n);
+    c->q = dup_mem(charge, sizeof(double) * n);
+    c->sig = dup_mem(sigma, sizeof(double) * n);
+    c->eps = dup_mem(eps, sizeof(double) * n);
+    c->nb = n_bonds; c->na = n_angles;
+    c->bij = dup_mem(bond_ij, sizeof(int) * 2 * n_bonds);
+    c->bk = dup_mem(bond_k, sizeof(double) * n_bonds);
+    c->br0 = dup_mem(bond_r0, sizeof(double) * n_bonds);
+    c->aijk = dup_mem(angle_ijk, sizeof(int) * 3 * n_angles);
+    c->ak = dup_mem(angle_k, sizeof(double) * n_angles);
+    c->at0 = dup_mem(angle_t0, sizeof(double) * n_angles);
+    if (excl_ptr) {
+        c->excl_ptr = dup_mem(excl_ptr, sizeof(int) * (n + 1));
+        c->excl_idx = dup_mem(excl_idx, sizeof(int) * excl_ptr[n]);
+    }
+    c->kT = ORC_KB * p->temperature_K;
+    c->beta = 1.0 / c->kT;
+    c->dt = p->dt_fs * 1e-3;
+    c->rc = p->r_short; c->h = p->r_switch; c->rE = p->r_long; c->skin = p->skin;
+    c->alpha = p->ewald_alpha < 0.0 ? 3.8 / p->r_long : p->ewald_alpha; /* R-2 */
+    /* r_mid <= 0: no ring, M is empty and L covers the whole shell */
+    c->rM = p->r_mid > 0.0 ? p->r_mid : dmax(c->rc - c->h - c->skin, 0.0);
+    c->sbm = malloc(sizeof(double) * n);
+    for (int i = 0; i < n; ++i) c->sbm[i] = sqrt(c->m[i] / (c->kT * ORC_KCAL));
+    double edge = p->cell_edge > 0.0 ? p->cell_edge : (p->r_long + p->skin) / 4.0;
+    c->gnx = (int)floor(p->box[0] / edge); if (c->gnx < 1) c->gnx = 1;
+    c->gny = (int)floor(p->box[1] / edge); if (c->gny < 1) c->gny = 1;
+    c->gnz = (int)floor(p->box[2] / edge); if (c->gnz < 1) c->gnz = 1;
+    c->x_build = malloc(sizeof(double) * 3 * n);
+    c->f_bond = calloc(3 * n, sizeof(double));
+    c->f_nb = calloc(3 * n, sizeof(double));
+    c->f0 = calloc(3 * n, sizeof(double));
+    c->f_long = calloc(3 * n, sizeof(double));
+    orc_reset_stats(c);
+    wrap_all(c);
+    compute_bounds(c);
+    rebuild_rows(c);
+    compute_f0(c);
+    return c;
+}
+void orc_free(orc_ctx *c) {
+    if (!c) return;
+    free(c->x); free(c->xu); free(c->v); free(c->m); free(c->q); free(c->sig); free(c->eps);
+    free(c->bij); free(c->bk); free(c->br0); free(c->aijk); free(c->ak); free(c->at0);
+    free(c->excl_ptr); free(c->excl_idx); free(c->sbm); free(c->x_build);
+    free(c->ptrM); free(c->idxM); free(c->ptrL); free(c->idxL); free(c->ptrV); free(c->idxV);
+    free(c->f_bond); free(c->f_nb); free(c->f0); free(c->f_long); free(c->ev);
+    free(c);
+}
+/* which: 0 wrapped x, 1 v, 2 unwrapped x */
+void orc_get_state(const orc_ctx *c, int which, double *out) {
+    const double *src = which == 0 ? c->x : (which == 1 ? c->v : c->xu);
+    memcpy(out, src, sizeof(double) * 3 * c->n);
+}
+/* overwrite x (and v); rows and F0 are refreshed */
+void orc_set_state(orc_ctx *c, const double *x, const double *v, int rebuild) {
+    if (x) { memcpy(c->x, x, sizeof(double) * 3 * c->n); memcpy(c->xu, x, sizeof(double) * 3 * c->n); wrap_all(c); }
+    if (v) memcpy(c->v, v, sizeof(double) * 3 * c->n);
+    if (rebuild) rebuild_rows(c);
+    compute_f0(c);
+}
+int64_t orc_get_step(const orc_ctx *c) { return c->step; }
+void orc_set_eps(orc_ctx *c, double eps) { c->p.eps_jump = eps; }
+void orc_scale_bounds(orc_ctx *c, double f) { c->GM *= f; c->GL *= f; c->GV *= f; } /* thinning-invariance pin */
+int orc_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+/* run only the C' (and J') half-step at frozen x: used by the rate / drift pins */
+void orc_jump_half(orc_ctx *c, double H_ps, int with_accel, int64_t step) {
+    jump_phase(c, H_ps, with_accel ? c->f0 : NULL, 1, 2, step, 0);
+}
+/* single long-range pair gradient F_ij (kcal/mol/A): which 0 Coulomb, 1 LJ */
+double orc_fij(const orc_ctx *c, int which, int i, int j, double F[3]) {
+    return which == 0 ? fij_coul(c, i, j, F) : fij_lj(c, i, j, F);
+}
+/* many draws of G~ at one eta (distribution pins): out[k], returns total attempts */
+int64_t orc_gtilde_batch(double eta, uint64_t seed, int n, double *out) {
+    orc_ctx c;
+    memset(&c, 0, sizeof c);
+    c.p.seed = seed;
+    int64_t tot = 0;
+    for (int k = 0; k < n; ++k) {
+        uint32_t b = 0;
+        int att = 0;
+        double mg = 1e300;
+        out[k] = orc_gtilde(&c, eta, k, 0, 99, &b, &att, &mg);
+        tot += att;
+    }
+    return tot;
+}
+/* overwrite velocities only (no list or force refresh) */
+void orc_set_vel(orc_ctx *c, const double *v) { memcpy(c->v, v, sizeof(double) * 3 * c->n); }
