@@ -1,0 +1,134 @@
+/*
+ * jump_b200.h -- C ABI of the B200-native JUMP hot path (arXiv 2412.15073).
+ *
+ * "P:Lnnn" = line nnn of the paper text; "R-n" = reading n in DESIGN.md.
+ * Every entry point takes plain pointers and sizes; pointers named d_* are DEVICE
+ * pointers, everything else is HOST memory.  No torch types cross this boundary.
+ *
+ * Sign convention (R-4): every "force" array is a GRADIENT piece, grad U = sum F
+ * (P:L59); the physical force is -F.  Units (R-1): Angstrom, fs for dt_fs, 1/ps for
+ * gamma, K, g/mol, e, kcal/mol; velocities in Angstrom/ps; gradients in kcal/mol/A.
+ *
+ * Errors: every int-returning call gives 0 on success or a negative JUMP_E_* code.
+ * Device-side flags (row overflow, thinning bound violated, displacement beyond
+ * skin/2, non-finite state) are sticky and reported by the next synchronising call
+ * (jump_get_*, jump_sync).  Nothing is printed and nothing calls exit().
+ */
+#ifndef JUMP_B200_H
+#define JUMP_B200_H
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define JUMP_E_ARG (-1)      /* bad argument (n_inner odd, r_short >= r_long, r_long > box/2, ...) */
+#define JUMP_E_CUDA (-2)     /* CUDA runtime error, see jump_last_error */
+#define JUMP_E_OVERFLOW (-3) /* a neighbour/ring row or the event buffer overflowed its capacity */
+#define JUMP_E_BOUND (-4)    /* thinning bound violated: an acceptance probability p > 1 was seen */
+#define JUMP_E_SKIN (-5)     /* an atom moved more than skin/2 since the last list build (only with JUMP_F_STRICT_SKIN;
+                                otherwise jump_stats.max_disp reports it: a hot, far-from-equilibrium start may exceed it) */
+#define JUMP_E_NAN (-6)      /* non-finite position or velocity */
+
+#define JUMP_F_COUL_JUMPS 1u       /* Coulomb tail r_c..r_long by jumps (step C', Alg. 4) */
+#define JUMP_F_LJ_JUMPS 2u         /* LJ tail by BPS jumps (step J', Alg. 5); else LJ tail stays in F0 (R-13) */
+#define JUMP_F_EVENT_LOG 4u        /* record every proposal (R-18) */
+#define JUMP_F_RESPA_PAPER 8u      /* RESPA: bonded inner, short non-bonded + jumps outer */
+#define JUMP_F_RESPA_COMPARATOR 16u /* jump_respa_step runs BAOAB-RESPA: outer kick by the long force */
+
+#define JUMP_F_STRICT_SKIN 32u      /* make a displacement beyond skin/2 between list builds an error (JUMP_E_SKIN) */
+
+typedef struct jump_ctx jump_ctx; /* opaque, owned by the library */
+
+/* Run parameters, copied at init.  Passages: P:L591-643 (simulation details), R-1..R-15. */
+typedef struct {
+    int32_t n_atoms;
+    int32_t n_inner;     /* RESPA: Delta = n_inner * dt, must be even */
+    int32_t eps_mode;    /* 0 = constant epsilon (Alg. 4); others unsupported (NEXT-1) */
+    uint32_t flags;      /* JUMP_F_* */
+    int32_t nlist_every; /* rebuild all lists every this many steps (R-10) */
+    int32_t pad0;
+    uint64_t seed;       /* Philox4x32-10 key (R-15) */
+    double box[3];       /* orthorhombic periodic box edges, A */
+    double r_short;      /* r_c: chi = 0 at and beyond it */
+    double r_switch;     /* h: chi = 1 below r_c - h */
+    double r_mid;        /* r_M ring split; <= 0: no ring */
+    double r_long;       /* r_E: pairs beyond are neglected */
+    double ewald_alpha;  /* alpha of erfc(alpha r)/r; < 0: 3.8 / r_long (R-2) */
+    double dt_fs, gamma_per_ps, temperature_K; /* delta, gamma, T */
+    double eps_jump;     /* epsilon of the general mechanism (6),(7); +inf: BPS */
+    double skin;         /* list skin s (R-10) */
+    double cell_edge;    /* minimum edge of the sort grid; <= 0: (r_long + skin) / 4 (R-10) */
+} jump_params;
+
+/* One proposal of a jump chain (R-18).  ring: 0 = M, 1 = L, 2 = V (LJ), -1 = clock expired. */
+typedef struct {
+    int32_t step, stream, atom, iter;
+    int32_t ring, j, accepted, n_gt;
+    float T, p, U, gt;
+} jump_event;
+
+typedef struct {
+    int64_t proposals, accepts, gt_attempts, rebuilds, expiries;
+    double max_p;        /* largest acceptance probability seen (must stay <= 1) */
+    double max_g_over_L; /* largest |F_ij| / L seen (must stay <= 1) */
+    double max_disp;     /* largest displacement since a list build, A */
+    int32_t max_row[6];  /* largest row length seen: short, M, L, V, full, LJ-tail */
+    int32_t cap_row[6];  /* row capacities */
+    int32_t error;       /* sticky device error (0 or JUMP_E_*) */
+    int32_t pad;
+} jump_stats;
+
+/*
+ * Create a context.  All d_* arrays are device memory owned by the caller and borrowed for the
+ * context's lifetime; d_pos / d_vel (n_atoms x 3, row-major, original atom order) are updated in
+ * place by the step calls, the others are read at init only (copied into the library's own sorted
+ * layout).  lj: 4 eps_ij [(s_ij/r)^12 - (s_ij/r)^6] with geometric mixing (R-8).  Bonds k (r-r0)^2,
+ * angles k (theta-theta0)^2 with the vertex in the middle of each ijk triple (R-2).  Exclusions as
+ * CSR over original indices (R-9); d_excl_ptr may be NULL for none.  cuda_stream: a cudaStream_t
+ * (NULL = default stream); all work is enqueued on it.  Builds the sort, all rows and F0(x0).
+ */
+int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, float *d_vel, const float *d_mass,
+              const float *d_charge, const float *d_lj_sigma, const float *d_lj_eps, int32_t n_bonds,
+              const int32_t *d_bond_ij, const float *d_bond_k, const float *d_bond_r0, int32_t n_angles,
+              const int32_t *d_angle_ijk, const float *d_angle_k, const float *d_angle_t0,
+              const int32_t *d_excl_ptr, const int32_t *d_excl_idx, void *cuda_stream);
+
+/* n_steps of the C'J'AOAJ'C' scheme.  Asynchronous. */
+int jump_step(jump_ctx *c, int32_t n_steps);
+/* n_steps of BAOAB with the unsplit force to r_long.  Asynchronous. */
+int baoab_step(jump_ctx *c, int32_t n_steps);
+/* n_outer outer steps of JUMP-RESPA, or BAOAB-RESPA with JUMP_F_RESPA_COMPARATOR (R-12). */
+int jump_respa_step(jump_ctx *c, int32_t n_outer);
+
+/* Gradient pieces at the current positions, original atom order, kcal/mol/A, into d_out (n x 3).
+ * which: 0 F0 (bonded + short non-bonded), 1 full (unsplit to r_long), 2 long, 3 bonded, 4 short non-bonded. */
+int jump_get_forces(jump_ctx *c, int32_t which, float *d_out);
+/* Kinetic energy and the full unsplit potential to r_long, kcal/mol (host doubles). */
+int jump_get_energy(jump_ctx *c, double *e_kin, double *e_pot_full);
+int jump_get_stats(jump_ctx *c, jump_stats *host_out);
+int jump_reset_stats(jump_ctx *c);
+/* Copy up to cap logged events (unsorted) to host_buf; *n receives the number logged so far. */
+int jump_get_events(jump_ctx *c, jump_event *host_buf, int64_t cap, int64_t *n);
+int jump_clear_events(jump_ctx *c);
+/* Row which (0 short, 1 M, 2 L, 3 V) of original atom i as original indices in canonical order (R-10);
+ * returns the row length (or a negative error); at most cap entries are written to host_out. */
+int jump_get_row(jump_ctx *c, int32_t which, int32_t atom, int32_t *host_out, int32_t cap);
+/* Bounds as used (R-7): GM, GL, GV, qmax, eps_max, sig_min, sig_max, rM. */
+int jump_get_bounds(jump_ctx *c, double out[8]);
+/* Re-read d_pos / d_vel after the caller changed them: re-sort, rebuild rows, recompute F0. */
+int jump_refresh(jump_ctx *c);
+/* Run only the opening jump half-phase C'(H) [then J'(H)] at frozen x with stream ids 1, 2 (pins). */
+int jump_half(jump_ctx *c, double H_ps, int32_t with_accel, int64_t step);
+/* Wait for the stream; returns the sticky device error if any. */
+int jump_sync(jump_ctx *c);
+int64_t jump_get_step(const jump_ctx *c);
+/* Number of kernels this context launched so far (bench.py's gpu_launches). */
+int64_t jump_get_launches(const jump_ctx *c);
+const char *jump_last_error(const jump_ctx *c);
+void jump_free(jump_ctx *c);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

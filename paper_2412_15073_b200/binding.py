@@ -1,0 +1,241 @@
+"""Thin ctypes binding of libjump_b200.so (include/jump_b200.h): argument marshalling only.
+
+PyTorch is used for device memory and streams; every step of the path runs in the library's CUDA
+kernels.  There is no CPU fallback: importing works without a GPU (so that the symbol check can
+run), but creating a context without the built library or without a CUDA device raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libjump_b200.so")
+
+F_COUL_JUMPS, F_LJ_JUMPS, F_EVENT_LOG, F_RESPA_PAPER, F_RESPA_COMPARATOR = 1, 2, 4, 8, 16
+F_STRICT_SKIN = 32
+ERRORS = {-1: "bad argument", -2: "CUDA error", -3: "row/event overflow", -4: "thinning bound violated",
+          -5: "displacement beyond skin/2", -6: "non-finite state"}
+
+EXPORTS = ["jump_init", "jump_step", "baoab_step", "jump_respa_step", "jump_get_forces", "jump_get_energy",
+           "jump_get_stats", "jump_reset_stats", "jump_get_events", "jump_clear_events", "jump_get_row",
+           "jump_get_bounds", "jump_refresh", "jump_half", "jump_sync", "jump_get_step", "jump_get_launches",
+           "jump_last_error", "jump_free"]
+
+
+class jump_params(C.Structure):
+    _fields_ = [
+        ("n_atoms", C.c_int32), ("n_inner", C.c_int32), ("eps_mode", C.c_int32), ("flags", C.c_uint32),
+        ("nlist_every", C.c_int32), ("pad0", C.c_int32), ("seed", C.c_uint64),
+        ("box", C.c_double * 3),
+        ("r_short", C.c_double), ("r_switch", C.c_double), ("r_mid", C.c_double), ("r_long", C.c_double),
+        ("ewald_alpha", C.c_double),
+        ("dt_fs", C.c_double), ("gamma_per_ps", C.c_double), ("temperature_K", C.c_double),
+        ("eps_jump", C.c_double), ("skin", C.c_double), ("cell_edge", C.c_double),
+    ]
+
+
+class jump_event(C.Structure):
+    _fields_ = [("step", C.c_int32), ("stream", C.c_int32), ("atom", C.c_int32), ("iter", C.c_int32),
+                ("ring", C.c_int32), ("j", C.c_int32), ("accepted", C.c_int32), ("n_gt", C.c_int32),
+                ("T", C.c_float), ("p", C.c_float), ("U", C.c_float), ("gt", C.c_float)]
+
+
+EVENT_DTYPE = np.dtype([("step", "i4"), ("stream", "i4"), ("atom", "i4"), ("iter", "i4"), ("ring", "i4"), ("j", "i4"),
+                        ("accepted", "i4"), ("n_gt", "i4"), ("T", "f4"), ("p", "f4"), ("U", "f4"), ("gt", "f4")])
+
+
+class jump_stats(C.Structure):
+    _fields_ = [("proposals", C.c_int64), ("accepts", C.c_int64), ("gt_attempts", C.c_int64), ("rebuilds", C.c_int64),
+                ("expiries", C.c_int64), ("max_p", C.c_double), ("max_g_over_L", C.c_double), ("max_disp", C.c_double),
+                ("max_row", C.c_int32 * 6), ("cap_row", C.c_int32 * 6), ("error", C.c_int32), ("pad", C.c_int32)]
+
+
+_lib = None
+
+
+def build(force=False):
+    from . import build as _b
+    return _b.build(force=force)
+
+
+def lib():
+    """Load the C-ABI library (raises if it has not been built: there is no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("libjump_b200.so is missing: run `python -m paper_2412_15073_b200.build` "
+                               "(or __graft_entry__.build()); the CUDA path has no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, dp = C.c_void_p, C.c_int32, C.c_int64, C.POINTER(C.c_double)
+        L.jump_init.argtypes = [C.POINTER(vp), C.POINTER(jump_params), vp, vp, vp, vp, vp, vp, i32, vp, vp, vp, i32, vp, vp, vp,
+                                vp, vp, vp]
+        L.jump_step.argtypes = [vp, i32]
+        L.baoab_step.argtypes = [vp, i32]
+        L.jump_respa_step.argtypes = [vp, i32]
+        L.jump_get_forces.argtypes = [vp, i32, vp]
+        L.jump_get_energy.argtypes = [vp, dp, dp]
+        L.jump_get_stats.argtypes = [vp, C.POINTER(jump_stats)]
+        L.jump_reset_stats.argtypes = [vp]
+        L.jump_get_events.argtypes = [vp, vp, i64, C.POINTER(i64)]
+        L.jump_clear_events.argtypes = [vp]
+        L.jump_get_row.argtypes = [vp, i32, i32, C.POINTER(i32), i32]
+        L.jump_get_bounds.argtypes = [vp, dp]
+        L.jump_refresh.argtypes = [vp]
+        L.jump_half.argtypes = [vp, C.c_double, i32, i64]
+        L.jump_sync.argtypes = [vp]
+        L.jump_get_step.argtypes = [vp]
+        L.jump_get_step.restype = i64
+        L.jump_get_launches.argtypes = [vp]
+        L.jump_get_launches.restype = i64
+        L.jump_last_error.argtypes = [vp]
+        L.jump_last_error.restype = C.c_char_p
+        L.jump_free.argtypes = [vp]
+        L.jump_free.restype = None
+        _lib = L
+    return _lib
+
+
+def make_params(n_atoms, box, r_short, r_long, r_switch=0.5, r_mid=None, ewald_alpha=-1.0, dt_fs=1.0, gamma_per_ps=1.0,
+                temperature_K=300.0, n_inner=4, eps_jump=1.0, eps_mode=0, flags=F_COUL_JUMPS | F_LJ_JUMPS, skin=1.0,
+                nlist_every=10, seed=0, cell_edge=0.0, **_ignored):
+    p = jump_params()
+    p.n_atoms, p.n_inner, p.eps_mode, p.flags = int(n_atoms), int(n_inner), int(eps_mode), int(flags)
+    p.nlist_every, p.seed = int(nlist_every), int(seed)
+    b = np.broadcast_to(np.asarray(box, dtype=np.float64), (3,))
+    p.box[0], p.box[1], p.box[2] = float(b[0]), float(b[1]), float(b[2])
+    p.r_short, p.r_switch, p.r_long = float(r_short), float(r_switch), float(r_long)
+    p.r_mid = float(r_short + 1.0 if r_mid is None else r_mid)
+    p.ewald_alpha = float(ewald_alpha)
+    p.dt_fs, p.gamma_per_ps, p.temperature_K = float(dt_fs), float(gamma_per_ps), float(temperature_K)
+    p.eps_jump, p.skin, p.cell_edge = float(eps_jump), float(skin), float(cell_edge)
+    return p
+
+
+class JumpError(RuntimeError):
+    pass
+
+
+class JumpSim:
+    """One simulation context on the current CUDA device.  `system` is a dict of numpy arrays as made by
+    paper_2412_15073_b200.workloads (original atom indices throughout); run parameters as keywords."""
+
+    def __init__(self, system, device="cuda:0", stream=None, **params):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2412_15073_b200 needs a CUDA device: there is no CPU fallback")
+        self._torch = torch
+        self._L = lib()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.n = int(system["pos"].shape[0])
+        kw = dict(params)
+        kw.setdefault("box", system["box"])
+        self.params = make_params(self.n, **kw)
+        f32 = lambda k: torch.as_tensor(np.ascontiguousarray(system[k], dtype=np.float32), device=self.device)
+        i32 = lambda k: torch.as_tensor(np.ascontiguousarray(system[k], dtype=np.int32), device=self.device)
+        self.pos, self.vel = f32("pos"), f32("vel")          # updated in place by the library
+        self._keep = [f32("mass"), f32("charge"), f32("lj_sigma"), f32("lj_eps"), i32("bond_ij"), f32("bond_k"),
+                      f32("bond_r0"), i32("angle_ijk"), f32("angle_k"), f32("angle_t0"), i32("excl_ptr"), i32("excl_idx")]
+        k = self._keep
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = C.c_void_p()
+        ptr = lambda t: C.c_void_p(t.data_ptr()) if t.numel() else C.c_void_p(0)
+        torch.cuda.synchronize(self.device)
+        rc = self._L.jump_init(C.byref(h), C.byref(self.params), ptr(self.pos), ptr(self.vel), ptr(k[0]), ptr(k[1]), ptr(k[2]),
+                               ptr(k[3]), int(k[4].shape[0]), ptr(k[4]), ptr(k[5]), ptr(k[6]), int(k[7].shape[0]), ptr(k[7]),
+                               ptr(k[8]), ptr(k[9]), ptr(k[10]), ptr(k[11]), C.c_void_p(self.stream.cuda_stream))
+        self._h = h
+        self._check(rc, "jump_init")
+
+    def _check(self, rc, what):
+        if rc < 0:
+            msg = self._L.jump_last_error(self._h) if self._h else b""
+            raise JumpError("%s failed: %d (%s) %s" % (what, rc, ERRORS.get(rc, "?"), (msg or b"").decode()))
+        return rc
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.jump_free(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- the hot path (asynchronous; same names as the C entry points) -------------------------------
+    def jump_step(self, n=1):
+        self._check(self._L.jump_step(self._h, int(n)), "jump_step")
+
+    def baoab_step(self, n=1):
+        self._check(self._L.baoab_step(self._h, int(n)), "baoab_step")
+
+    def jump_respa_step(self, n=1):
+        self._check(self._L.jump_respa_step(self._h, int(n)), "jump_respa_step")
+
+    def jump_half(self, H_ps, with_accel=True, step=0):
+        self._check(self._L.jump_half(self._h, float(H_ps), int(bool(with_accel)), int(step)), "jump_half")
+
+    def sync(self):
+        self._check(self._L.jump_sync(self._h), "jump_sync")
+
+    def refresh(self):
+        self._check(self._L.jump_refresh(self._h), "jump_refresh")
+
+    # ---- observers -----------------------------------------------------------------------------------
+    def forces(self, which=0):
+        out = self._torch.empty((self.n, 3), dtype=self._torch.float32, device=self.device)
+        self._check(self._L.jump_get_forces(self._h, int(which), C.c_void_p(out.data_ptr())), "jump_get_forces")
+        return out
+
+    def energy(self):
+        ek, ep = C.c_double(), C.c_double()
+        self._check(self._L.jump_get_energy(self._h, C.byref(ek), C.byref(ep)), "jump_get_energy")
+        return ek.value, ep.value
+
+    def temperature(self):
+        ek = C.c_double()
+        self._check(self._L.jump_get_energy(self._h, C.byref(ek), None), "jump_get_energy")
+        return 2.0 * ek.value / (3.0 * self.n * 1.987204259e-3)
+
+    def stats(self):
+        s = jump_stats()
+        self._check(self._L.jump_get_stats(self._h, C.byref(s)), "jump_get_stats")
+        d = {k: getattr(s, k) for k, _ in jump_stats._fields_ if k not in ("max_row", "cap_row", "pad")}
+        d["max_row"], d["cap_row"] = list(s.max_row), list(s.cap_row)
+        return d
+
+    def reset_stats(self):
+        self._check(self._L.jump_reset_stats(self._h), "jump_reset_stats")
+
+    def events(self):
+        n = C.c_int64()
+        self._check(self._L.jump_get_events(self._h, None, 0, C.byref(n)), "jump_get_events")
+        buf = np.zeros(int(n.value), dtype=EVENT_DTYPE)
+        assert buf.itemsize == C.sizeof(jump_event)
+        if n.value:
+            self._check(self._L.jump_get_events(self._h, buf.ctypes.data_as(C.c_void_p), int(n.value), C.byref(n)), "jump_get_events")
+        return np.sort(buf, order=["step", "stream", "atom", "iter"])
+
+    def clear_events(self):
+        self._check(self._L.jump_clear_events(self._h), "jump_clear_events")
+
+    def row(self, which, atom):
+        out = (C.c_int32 * self.n)()
+        m = self._check(self._L.jump_get_row(self._h, int(which), int(atom), out, self.n), "jump_get_row")
+        return np.frombuffer(out, dtype=np.int32, count=m).copy()
+
+    def bounds(self):
+        out = (C.c_double * 8)()
+        self._check(self._L.jump_get_bounds(self._h, out), "jump_get_bounds")
+        return dict(zip(["GM", "GL", "GV", "qmax", "eps_max", "sig_min", "sig_max", "rM"], list(out)))
+
+    @property
+    def step(self):
+        return int(self._L.jump_get_step(self._h))
+
+    @property
+    def launches(self):
+        return int(self._L.jump_get_launches(self._h))

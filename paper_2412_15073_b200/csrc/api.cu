@@ -1,0 +1,671 @@
+// api.cu -- context, host-side step drivers and the C ABI of include/jump_b200.h.
+// The drivers only enqueue kernels on one stream; every arithmetic step of the path runs in the
+// kernels of sort_build.cu, forces.cu and update.cu.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "launch.h"
+
+using namespace jb;
+
+struct jump_ctx {
+    jump_params p;
+    Model m;
+    SortGrid g;
+    cudaStream_t st;
+    int n;
+    double kT, dt, alpha, rM, lo;  // ps; lo = max(r_c - h - skin, 0)
+    double GM, GL, GV, qmax, eps_max, sig_min, sig_max;
+    float c1, c2;
+    float *d_pos, *d_vel;  // caller's
+    // sorted state (cur) and spare buffers (nxt)
+    float4 *xs, *xs_nxt, *vs, *vs_nxt, *x_build;
+    float2 *lj, *lj_nxt, *mi, *mi_nxt;
+    int *orig, *orig_nxt, *sorted_of;
+    int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src;
+    Row rows[N_ROWS];
+    bool row_fresh[N_ROWS];  // built since the last sort
+    float4 *fnb, *fbond, *f0, *ftmp, *ftmp2;
+    double *ke;
+    int *excl_ptr, *excl_idx;
+    Topo topo;
+    std::vector<void *> owned;  // everything to cudaFree
+    Counters *ctr;
+    jump_event *events;
+    long long event_cap;
+    int64_t step, outer, rebuilds, launches;
+    int sticky;
+    std::string err;
+};
+
+#define CK(call)                                                                          \
+    do {                                                                                  \
+        cudaError_t e_ = (call);                                                          \
+        if (e_ != cudaSuccess) {                                                          \
+            c->err = std::string(#call) + ": " + cudaGetErrorString(e_);                  \
+            return JUMP_E_CUDA;                                                           \
+        }                                                                                 \
+    } while (0)
+
+template <class T>
+static int dalloc(jump_ctx *c, T **p, size_t count) {
+    void *q = nullptr;
+    CK(cudaMalloc(&q, std::max<size_t>(count, 1) * sizeof(T)));
+    c->owned.push_back(q);
+    *p = (T *)q;
+    return 0;
+}
+template <class T>
+static int dupload(jump_ctx *c, T **p, const std::vector<T> &h) {
+    int r = dalloc(c, p, h.size());
+    if (r) return r;
+    if (!h.empty()) CK(cudaMemcpyAsync(*p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return 0;
+}
+template <class T>
+static int ddownload(jump_ctx *c, std::vector<T> &h, const T *d, size_t count) {
+    h.resize(count);
+    if (count) CK(cudaMemcpyAsync(h.data(), d, count * sizeof(T), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return 0;
+}
+
+// ---- bounds L (R-7): sup of the long-part radial derivative on a dense grid, times (1 + 1e-6) ---------------
+static void chi_host(double r, double rc, double h, double *chi, double *dchi) {
+    double u = (r - (rc - h)) / h;
+    if (u <= 0.0) { *chi = 1.0; *dchi = 0.0; return; }
+    if (u >= 1.0) { *chi = 0.0; *dchi = 0.0; return; }
+    *chi = 1.0 - u * u * u * (10.0 - 15.0 * u + 6.0 * u * u);
+    *dchi = -30.0 * u * u * (1.0 - u) * (1.0 - u) / h;
+}
+static double sup_long(const jump_ctx *c, double lo, double hi, double step, bool coul, double sig) {
+    if (!(hi > lo)) return 0.0;
+    const double rc = c->p.r_short, h = c->p.r_switch, al = c->alpha;
+    double best = 0.0;
+    long K = (long)std::floor((hi - lo) / step);
+    for (long k = 0; k <= K + 1; ++k) {
+        double r = (k <= K) ? lo + step * (double)k : hi;
+        if (r > hi) r = hi;
+        double u, du;
+        if (coul) {  // unit charges: u = C erfc(alpha r)/r
+            double e = std::erfc(al * r);
+            u = kCoulomb * e / r;
+            du = -kCoulomb * (e / (r * r) + 2.0 * al / std::sqrt(M_PI) * std::exp(-al * al * r * r) / r);
+        } else {  // 4 eps = 1
+            double s = sig / r, s6 = s * s * s * s * s * s, s12 = s6 * s6;
+            u = s12 - s6;
+            du = (-12.0 * s12 + 6.0 * s6) / r;
+        }
+        double chi, dchi;
+        chi_host(r, rc, h, &chi, &dchi);
+        best = std::max(best, std::fabs((1.0 - chi) * du - dchi * u));
+    }
+    return best * (1.0 + 1e-6);
+}
+static void compute_bounds(jump_ctx *c, const std::vector<float> &q, const std::vector<float> &sig,
+                           const std::vector<float> &eps) {
+    c->qmax = 0.0; c->eps_max = 0.0; c->sig_min = 1e300; c->sig_max = 0.0;
+    for (int i = 0; i < c->n; ++i) {
+        c->qmax = std::max(c->qmax, std::fabs((double)q[i]));
+        if (eps[i] > 0.f) {
+            c->eps_max = std::max(c->eps_max, (double)eps[i]);
+            c->sig_min = std::min(c->sig_min, (double)sig[i]);
+            c->sig_max = std::max(c->sig_max, (double)sig[i]);
+        }
+    }
+    if (c->eps_max == 0.0) c->sig_min = c->sig_max = 0.0;
+    const double rlo = c->p.r_short - c->p.r_switch, rE = c->p.r_long, s = c->p.skin;
+    c->GM = sup_long(c, rlo, std::min(c->rM + s, rE), 1e-4, true, 0.0);
+    c->GL = sup_long(c, std::max(c->rM - s, rlo), rE, 1e-4, true, 0.0);
+    c->GV = 0.0;
+    if (c->sig_max > 0.0) {
+        int NS = (c->sig_max > c->sig_min) ? 65 : 1;
+        for (int k = 0; k < NS; ++k) {
+            double sg = NS == 1 ? c->sig_min : c->sig_min + (c->sig_max - c->sig_min) * (double)k / (double)(NS - 1);
+            c->GV = std::max(c->GV, sup_long(c, rlo, rE, 1e-3, false, sg));
+        }
+    }
+}
+
+static int round32(double x) { return (int)(((long long)std::ceil(x) + 31) / 32 * 32); }
+
+static int alloc_row(jump_ctx *c, int k) {
+    Row &R = c->rows[k];
+    if (R.idx) return 0;
+    int r = dalloc(c, &R.idx, (size_t)c->n * R.cap);
+    if (r) return r;
+    r = dalloc(c, &R.cnt, (size_t)c->n);
+    if (r) return r;
+    CK(cudaMemsetAsync(R.cnt, 0, sizeof(int) * c->n, c->st));
+    R.enabled = 1;
+    return 0;
+}
+
+static int build_rows(jump_ctx *c, bool only_missing) {
+    Row sel[N_ROWS];
+    bool any = false;
+    for (int k = 0; k < N_ROWS; ++k) {
+        sel[k] = c->rows[k];
+        if (only_missing && c->row_fresh[k]) sel[k].enabled = 0;
+        if (sel[k].enabled) { any = true; c->row_fresh[k] = true; }
+    }
+    if (!any) return 0;
+    launch_build_rows(c->m, c->g, sel, (float)(c->p.r_long + c->p.skin), c->cell_start, c->xs, c->lj, c->orig,
+                      c->sorted_of, c->excl_ptr, c->excl_idx, c->ctr, c->st, &c->launches);
+    CK(cudaGetLastError());
+    return 0;
+}
+
+static int resort_and_build(jump_ctx *c) {
+    SortArgs a;
+    a.n = c->n; a.grid = c->g;
+    a.xs_in = c->xs; a.vs_in = c->vs; a.lj_in = c->lj; a.mi_in = c->mi; a.orig_in = c->orig;
+    a.xs = c->xs_nxt; a.vs = c->vs_nxt; a.lj = c->lj_nxt; a.mi = c->mi_nxt; a.orig = c->orig_nxt;
+    a.sorted_of = c->sorted_of; a.x_build = c->x_build;
+    a.key = c->key; a.cell_count = c->cell_count; a.cell_fill = c->cell_fill; a.cell_start = c->cell_start;
+    a.tmp_orig = c->tmp_orig; a.tmp_src = c->tmp_src; a.ctr = c->ctr;
+    launch_sort(a, c->st, &c->launches);
+    CK(cudaGetLastError());
+    std::swap(c->xs, c->xs_nxt); std::swap(c->vs, c->vs_nxt); std::swap(c->lj, c->lj_nxt);
+    std::swap(c->mi, c->mi_nxt); std::swap(c->orig, c->orig_nxt);
+    for (int k = 0; k < N_ROWS; ++k) c->row_fresh[k] = false;
+    c->rebuilds++;
+    return build_rows(c, false);
+}
+
+static int need_row(jump_ctx *c, int k) {  // lazily enabled rows (full list of the BAOAB comparator)
+    int r = alloc_row(c, k);
+    if (r) return r;
+    return build_rows(c, true);
+}
+
+static bool lj_jumps(const jump_ctx *c) { return (c->p.flags & JUMP_F_LJ_JUMPS) != 0; }
+static bool coul_jumps(const jump_ctx *c) { return (c->p.flags & JUMP_F_COUL_JUMPS) != 0; }
+
+static int bonded(jump_ctx *c, const float4 *add, float4 *out_sum, float4 *out_bond) {
+    launch_bonded(c->m, c->topo, c->xs, c->orig, c->sorted_of, add, out_sum, out_bond, c->st, &c->launches);
+    CK(cudaGetLastError());
+    return 0;
+}
+// F0 = bonded + short non-bonded (R-13: the LJ tail stays in F0 when LJ jumps are off)
+static int compute_short_nb(jump_ctx *c, float4 *out, bool energy = false) {
+    if (lj_jumps(c)) launch_pair(c->m, c->rows[ROW_S], W_SHORT, W_SHORT, c->xs, c->lj, out, 0, energy, c->st, &c->launches);
+    else {
+        launch_pair(c->m, c->rows[ROW_S], W_SHORT, W_FULL, c->xs, c->lj, out, 0, energy, c->st, &c->launches);
+        launch_pair(c->m, c->rows[ROW_W], W_NONE, W_FULL, c->xs, c->lj, out, 1, energy, c->st, &c->launches);
+    }
+    CK(cudaGetLastError());
+    return 0;
+}
+static int compute_f0(jump_ctx *c) {
+    int r = compute_short_nb(c, c->fnb);
+    if (r) return r;
+    return bonded(c, c->fnb, c->f0, c->fbond);
+}
+static int compute_long(jump_ctx *c, float4 *out) {
+    int wLJ = lj_jumps(c) ? W_LONG : W_NONE;
+    launch_pair(c->m, c->rows[ROW_M], W_LONG, wLJ, c->xs, c->lj, out, 0, false, c->st, &c->launches);
+    launch_pair(c->m, c->rows[ROW_L], W_LONG, wLJ, c->xs, c->lj, out, 1, false, c->st, &c->launches);
+    CK(cudaGetLastError());
+    return 0;
+}
+static int compute_full(jump_ctx *c, float4 *out, bool energy = false) {  // unsplit to r_long + bonded
+    int r = need_row(c, ROW_F);
+    if (r) return r;
+    launch_pair(c->m, c->rows[ROW_F], W_FULL, W_FULL, c->xs, c->lj, c->ftmp2, 0, energy, c->st, &c->launches);
+    CK(cudaGetLastError());
+    return bonded(c, c->ftmp2, out, nullptr);
+}
+
+// ---- step drivers --------------------------------------------------------------------------------------
+static Phase ph_none() { Phase p; memset(&p, 0, sizeof p); return p; }
+static Phase ph_kick(double H) { Phase p = ph_none(); p.kind = 1; p.H = (float)H; p.use_grad = 1; return p; }
+static Phase ph_jump(const jump_ctx *c, double H, bool grad, bool reverse, int sC, int sJ, int64_t step) {
+    Phase p = ph_none();
+    p.kind = 2; p.H = (float)H; p.use_grad = grad ? 1 : 0; p.reverse = reverse ? 1 : 0;
+    p.coul = coul_jumps(c) ? 1 : 0; p.lj = lj_jumps(c) ? 1 : 0;
+    p.streamC = sC; p.streamJ = sJ; p.step = (unsigned)step;
+    return p;
+}
+
+// up to two velocity half-phases, then (aoa) A O A + wrap, step counter and the scheduled rebuild (C.3 steps 3-6)
+static int run_update(jump_ctx *c, const Phase &p0, const float4 *g0, const Phase &p1, const float4 *g1, bool aoa) {
+    UpdateArgs A;
+    memset(&A, 0, sizeof A);
+    A.ph[0] = p0; A.ph[1] = p1; A.grad[0] = g0; A.grad[1] = g1;
+    if (!g0) A.ph[0].use_grad = 0;
+    if (!g1) A.ph[1].use_grad = 0;
+    A.do_aoa = aoa ? 1 : 0;
+    A.half_dt = (float)(0.5 * c->dt); A.c1 = c->c1; A.c2 = c->c2; A.o_step = (unsigned)c->step;
+    A.xs = c->xs; A.xs_out = c->xs_nxt; A.vs = c->vs; A.mi = c->mi; A.lj = c->lj; A.orig = c->orig; A.x_build = c->x_build;
+    A.rowM = c->rows[ROW_M]; A.rowL = c->rows[ROW_L]; A.rowV = c->rows[ROW_V];
+    A.ctr = c->ctr; A.events = (c->p.flags & JUMP_F_EVENT_LOG) ? c->events : nullptr; A.event_cap = c->event_cap;
+    bool jumps = (p0.kind == 2 || p1.kind == 2) && (coul_jumps(c) || lj_jumps(c));
+    launch_update(c->m, A, jumps, c->st, &c->launches);
+    CK(cudaGetLastError());
+    if (aoa) {
+        std::swap(c->xs, c->xs_nxt);
+        c->step++;
+        if (c->p.nlist_every > 0 && c->step % c->p.nlist_every == 0) return resort_and_build(c);
+    }
+    return 0;
+}
+static int writeback(jump_ctx *c) {
+    launch_writeback(c->n, c->xs, c->vs, c->orig, c->d_pos, c->d_vel, c->st, &c->launches);
+    CK(cudaGetLastError());
+    return 0;
+}
+static int poll_error(jump_ctx *c) {  // sticky device flags -> error code
+    Counters h;
+    CK(cudaMemcpyAsync(&h, c->ctr, sizeof h, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    if (h.err & ERR_NAN) c->sticky = JUMP_E_NAN;
+    else if (h.err & (ERR_OVERFLOW | ERR_EVENTS)) c->sticky = JUMP_E_OVERFLOW;
+    else if (h.err & ERR_BOUND) c->sticky = JUMP_E_BOUND;
+    else if ((h.err & ERR_SKIN) && (c->p.flags & JUMP_F_STRICT_SKIN)) c->sticky = JUMP_E_SKIN;
+    if (c->sticky && c->err.empty()) c->err = "device error flags " + std::to_string(h.err);
+    return c->sticky;
+}
+
+extern "C" int jump_step(jump_ctx *c, int32_t n_steps) {
+    if (!c || n_steps < 0) return JUMP_E_ARG;
+    if (n_steps == 0) return 0;
+    const double H = 0.5 * c->dt;
+    for (int s = 0; s < n_steps; ++s) {
+        int64_t st = c->step;
+        Phase open = ph_jump(c, H, true, false, 1, 2, st);
+        Phase close_prev = s > 0 ? ph_jump(c, H, true, true, 4, 3, st - 1) : ph_none();
+        int r = run_update(c, close_prev, c->f0, open, c->f0, true);
+        if (r) return r;
+        r = compute_f0(c);
+        if (r) return r;
+    }
+    int r = run_update(c, ph_jump(c, H, true, true, 4, 3, c->step - 1), c->f0, ph_none(), nullptr, false);
+    if (r) return r;
+    return writeback(c);
+}
+
+extern "C" int baoab_step(jump_ctx *c, int32_t n_steps) {
+    if (!c || n_steps < 0) return JUMP_E_ARG;
+    if (n_steps == 0) return 0;
+    const double H = 0.5 * c->dt;
+    int r = compute_full(c, c->ftmp);
+    if (r) return r;
+    for (int s = 0; s < n_steps; ++s) {
+        r = run_update(c, s > 0 ? ph_kick(H) : ph_none(), c->ftmp, ph_kick(H), c->ftmp, true);
+        if (r) return r;
+        r = compute_full(c, c->ftmp);
+        if (r) return r;
+    }
+    r = run_update(c, ph_kick(H), c->ftmp, ph_none(), nullptr, false);
+    if (r) return r;
+    r = compute_f0(c);
+    if (r) return r;
+    return writeback(c);
+}
+
+extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
+    if (!c || n_outer < 0) return JUMP_E_ARG;
+    const int n = c->p.n_inner;
+    const double D = n * c->dt, H = 0.5 * c->dt;
+    const bool paper = (c->p.flags & JUMP_F_RESPA_PAPER) != 0, cmp = (c->p.flags & JUMP_F_RESPA_COMPARATOR) != 0;
+    int r;
+    for (int o = 0; o < n_outer; ++o) {
+        Phase outer[2];
+        const float4 *gout[2];
+        for (int half = 0; half < 2; ++half) {
+            if (half == 1) {  // inner loop: n x BAOAB_delta with F_in; the first opening kick rides with outer[0]
+                for (int s = 0; s < n; ++s) {
+                    const float4 *fin = paper ? c->fbond : c->f0;
+                    if (s == 0) r = run_update(c, outer[0], gout[0], ph_kick(H), fin, true);
+                    else r = run_update(c, ph_kick(H), fin, ph_kick(H), fin, true);
+                    if (r) return r;
+                    r = paper ? bonded(c, nullptr, nullptr, c->fbond) : compute_f0(c);
+                    if (r) return r;
+                }
+                if (paper) { r = compute_f0(c); if (r) return r; }
+            }
+            if (cmp) {  // BAOAB-RESPA: v <- v - (Delta/2) M^-1 F_long
+                float4 *fl = half == 0 ? c->ftmp : c->ftmp2;
+                r = compute_long(c, fl);
+                if (r) return r;
+                if (paper) {  // + short non-bonded
+                    launch_pair(c->m, c->rows[ROW_S], W_SHORT, lj_jumps(c) ? W_SHORT : W_FULL, c->xs, c->lj, fl, 1, false,
+                                c->st, &c->launches);
+                    if (!lj_jumps(c))
+                        launch_pair(c->m, c->rows[ROW_W], W_NONE, W_FULL, c->xs, c->lj, fl, 1, false, c->st, &c->launches);
+                    CK(cudaGetLastError());
+                }
+                outer[half] = ph_kick(0.5 * D);
+                gout[half] = fl;
+            } else {
+                gout[half] = paper ? c->fnb : nullptr;
+                outer[half] = half == 0 ? ph_jump(c, 0.5 * D, paper, false, 5, 6, c->outer)
+                                        : ph_jump(c, 0.5 * D, paper, true, 8, 7, c->outer);
+            }
+        }
+        const float4 *fin = paper ? c->fbond : c->f0;
+        r = run_update(c, ph_kick(H), fin, outer[1], gout[1], false);
+        if (r) return r;
+        c->outer++;
+    }
+    return writeback(c);
+}
+
+extern "C" int jump_half(jump_ctx *c, double H_ps, int32_t with_accel, int64_t step) {
+    if (!c) return JUMP_E_ARG;
+    int r = run_update(c, ph_jump(c, H_ps, with_accel != 0, false, 1, 2, step), c->f0, ph_none(), nullptr, false);
+    if (r) return r;
+    return writeback(c);
+}
+
+// ---- life cycle ------------------------------------------------------------------------------------------
+static int load_state(jump_ctx *c, const float *d_mass, const float *d_charge, const float *d_sigma, const float *d_eps) {
+    launch_load(c->m, c->d_pos, c->d_vel, d_mass, d_charge, d_sigma, d_eps, c->kT, c->xs, c->vs, c->lj, c->mi, c->orig, c->st,
+                &c->launches);
+    CK(cudaGetLastError());
+    return 0;
+}
+
+static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, const float *d_charge, const float *d_sigma,
+                     const float *d_eps, int n_bonds, const int32_t *d_bond_ij, const float *d_bond_k, const float *d_bond_r0,
+                     int n_angles, const int32_t *d_angle_ijk, const float *d_angle_k, const float *d_angle_t0,
+                     const int32_t *d_excl_ptr, const int32_t *d_excl_idx) {
+    const int n = c->n = p->n_atoms;
+    c->p = *p;
+    c->kT = kKB * p->temperature_K;
+    c->dt = p->dt_fs * 1e-3;
+    c->alpha = p->ewald_alpha < 0.0 ? 3.8 / p->r_long : p->ewald_alpha;  // R-2
+    c->lo = std::max(p->r_short - p->r_switch - p->skin, 0.0);
+    c->rM = p->r_mid > 0.0 ? p->r_mid : c->lo;  // no ring: M empty, L covers the shell
+    double g1 = std::exp(-p->gamma_per_ps * c->dt);
+    c->c1 = (float)g1;
+    c->c2 = (float)std::sqrt(1.0 - g1 * g1);
+    // host copies of the per-atom parameters (bounds) and the topology
+    std::vector<float> hq, hs, he;
+    int r;
+    if ((r = ddownload(c, hq, d_charge, n)) || (r = ddownload(c, hs, d_sigma, n)) || (r = ddownload(c, he, d_eps, n))) return r;
+    compute_bounds(c, hq, hs, he);
+    // model constants
+    Model &m = c->m;
+    memset(&m, 0, sizeof m);
+    m.n = n;
+    for (int k = 0; k < 3; ++k) { m.box[k] = (float)p->box[k]; m.inv_box[k] = (float)(1.0 / p->box[k]); }
+    m.rc = (float)p->r_short; m.h = (float)p->r_switch; m.inv_h = (float)(1.0 / p->r_switch);
+    m.rlo = (float)(p->r_short - p->r_switch);
+    m.rc2 = (float)(p->r_short * p->r_short); m.rlo2 = m.rlo * m.rlo; m.rE2 = (float)(p->r_long * p->r_long);
+    m.alpha = (float)c->alpha; m.alpha2 = (float)(c->alpha * c->alpha);
+    m.beta = (float)(1.0 / c->kT);
+    m.eps_jump = std::isinf(p->eps_jump) ? INFINITY : (float)p->eps_jump;
+    m.qmaxGM = (float)(c->qmax * c->GM); m.qmaxGL = (float)(c->qmax * c->GL);
+    m.GV4se = (float)(4.0 * std::sqrt(c->eps_max) * c->GV);
+    m.half_skin2 = (float)(0.25 * p->skin * p->skin);
+    m.key0 = (unsigned)(p->seed & 0xffffffffu); m.key1 = (unsigned)(p->seed >> 32);
+    // sort grid (R-10)
+    SortGrid &g = c->g;
+    double edge = p->cell_edge > 0.0 ? p->cell_edge : (p->r_long + p->skin) / 4.0;
+    g.ncell = 1;
+    for (int k = 0; k < 3; ++k) {
+        g.gn[k] = std::max(1, (int)std::floor(p->box[k] / edge));
+        g.scale[k] = (double)g.gn[k] / p->box[k];
+        g.reach[k] = (int)std::ceil((p->r_long + p->skin) / (p->box[k] / g.gn[k]) - 1e-12);
+        g.ncell *= g.gn[k];
+    }
+    // buffers
+    if ((r = dalloc(c, &c->xs, n)) || (r = dalloc(c, &c->xs_nxt, n)) || (r = dalloc(c, &c->vs, n)) ||
+        (r = dalloc(c, &c->vs_nxt, n)) || (r = dalloc(c, &c->x_build, n)) || (r = dalloc(c, &c->lj, n)) ||
+        (r = dalloc(c, &c->lj_nxt, n)) || (r = dalloc(c, &c->mi, n)) || (r = dalloc(c, &c->mi_nxt, n)) ||
+        (r = dalloc(c, &c->orig, n)) || (r = dalloc(c, &c->orig_nxt, n)) || (r = dalloc(c, &c->sorted_of, n)) ||
+        (r = dalloc(c, &c->key, n)) || (r = dalloc(c, &c->tmp_orig, n)) || (r = dalloc(c, &c->tmp_src, n)) ||
+        (r = dalloc(c, &c->cell_count, g.ncell + 1)) || (r = dalloc(c, &c->cell_fill, g.ncell + 1)) ||
+        (r = dalloc(c, &c->cell_start, g.ncell + 1)) || (r = dalloc(c, &c->fnb, n)) || (r = dalloc(c, &c->fbond, n)) ||
+        (r = dalloc(c, &c->f0, n)) || (r = dalloc(c, &c->ftmp, n)) || (r = dalloc(c, &c->ftmp2, n)) ||
+        (r = dalloc(c, &c->ke, n)) || (r = dalloc(c, &c->ctr, 1)))
+        return r;
+    CK(cudaMemsetAsync(c->ctr, 0, sizeof(Counters), c->st));
+    c->event_cap = 0; c->events = nullptr;
+    if (p->flags & JUMP_F_EVENT_LOG) {
+        c->event_cap = 1ll << 21;
+        if ((r = dalloc(c, &c->events, (size_t)c->event_cap))) return r;
+    }
+    // exclusions (own copy)
+    c->excl_ptr = nullptr; c->excl_idx = nullptr;
+    if (d_excl_ptr) {
+        std::vector<int> hp;
+        if ((r = ddownload(c, hp, (const int *)d_excl_ptr, n + 1))) return r;
+        int tot = hp[n];
+        if ((r = dalloc(c, &c->excl_ptr, n + 1)) || (r = dalloc(c, &c->excl_idx, tot))) return r;
+        CK(cudaMemcpyAsync(c->excl_ptr, d_excl_ptr, sizeof(int) * (n + 1), cudaMemcpyDeviceToDevice, c->st));
+        if (tot) CK(cudaMemcpyAsync(c->excl_idx, d_excl_idx, sizeof(int) * tot, cudaMemcpyDeviceToDevice, c->st));
+    }
+    // bonded terms as per-atom CSR over original indices
+    {
+        std::vector<int> hb, ha;
+        std::vector<float> hbk, hbr, hak, hat;
+        if ((r = ddownload(c, hb, (const int *)d_bond_ij, 2 * (size_t)n_bonds)) || (r = ddownload(c, hbk, d_bond_k, n_bonds)) ||
+            (r = ddownload(c, hbr, d_bond_r0, n_bonds)) || (r = ddownload(c, ha, (const int *)d_angle_ijk, 3 * (size_t)n_angles)) ||
+            (r = ddownload(c, hak, d_angle_k, n_angles)) || (r = ddownload(c, hat, d_angle_t0, n_angles)))
+            return r;
+        for (int v : hb) if (v < 0 || v >= n) return JUMP_E_ARG;
+        for (int v : ha) if (v < 0 || v >= n) return JUMP_E_ARG;
+        std::vector<int> bptr(n + 1, 0), aptr(n + 1, 0);
+        for (int b = 0; b < n_bonds; ++b) { bptr[hb[2 * b] + 1]++; bptr[hb[2 * b + 1] + 1]++; }
+        for (int a = 0; a < n_angles; ++a) for (int k = 0; k < 3; ++k) aptr[ha[3 * a + k] + 1]++;
+        for (int i = 0; i < n; ++i) { bptr[i + 1] += bptr[i]; aptr[i + 1] += aptr[i]; }
+        std::vector<int> bo(bptr[n]), bfill(bptr.begin(), bptr.end() - 1), ar(aptr[n]), aa(aptr[n]), ab(aptr[n]),
+            afill(aptr.begin(), aptr.end() - 1);
+        std::vector<float> bk(bptr[n]), br(bptr[n]), ak(aptr[n]), at(aptr[n]);
+        for (int b = 0; b < n_bonds; ++b)
+            for (int e = 0; e < 2; ++e) {
+                int me = hb[2 * b + e], s = bfill[me]++;
+                bo[s] = hb[2 * b + 1 - e]; bk[s] = hbk[b]; br[s] = hbr[b];
+            }
+        for (int a = 0; a < n_angles; ++a) {
+            int i = ha[3 * a], j = ha[3 * a + 1], k = ha[3 * a + 2];  // j = vertex
+            int s = afill[i]++; ar[s] = 0; aa[s] = j; ab[s] = k; ak[s] = hak[a]; at[s] = hat[a];
+            s = afill[j]++;     ar[s] = 1; aa[s] = i; ab[s] = k; ak[s] = hak[a]; at[s] = hat[a];
+            s = afill[k]++;     ar[s] = 2; aa[s] = j; ab[s] = i; ak[s] = hak[a]; at[s] = hat[a];
+        }
+        int *dbptr, *dbo, *daptr, *dar, *daa, *dab;
+        float *dbk, *dbr, *dak, *dat;
+        if ((r = dupload(c, &dbptr, bptr)) || (r = dupload(c, &dbo, bo)) || (r = dupload(c, &dbk, bk)) ||
+            (r = dupload(c, &dbr, br)) || (r = dupload(c, &daptr, aptr)) || (r = dupload(c, &dar, ar)) ||
+            (r = dupload(c, &daa, aa)) || (r = dupload(c, &dab, ab)) || (r = dupload(c, &dak, ak)) || (r = dupload(c, &dat, at)))
+            return r;
+        c->topo = Topo{dbptr, dbo, dbk, dbr, daptr, dar, daa, dab, dak, dat};
+    }
+    // rows: windows (R-10) and capacities from the mean density with head-room
+    {
+        const double vol = p->box[0] * p->box[1] * p->box[2], rho = n / vol, s = p->skin, rc = p->r_short, rE = p->r_long;
+        int n_lj = 0;
+        for (int i = 0; i < n; ++i) n_lj += he[i] > 0.f;
+        const double rho_lj = n_lj / vol;
+        struct W { double a, b; int lj; bool on; } w[N_ROWS] = {
+            {0.0, rc + s, 0, true},                              // S short list
+            {c->lo, c->rM, 0, true},                             // M ring
+            {std::max(c->rM, c->lo), rE + s, 0, true},           // L ring
+            {c->lo, rE + s, 1, lj_jumps(c)},                     // V: LJ jump partners
+            {0.0, rE + s, 0, false},                             // F: full list (lazy)
+            {rc + s, rE + s, 1, !lj_jumps(c)}};                  // W: LJ tail kept in F0 (R-13)
+        for (int k = 0; k < N_ROWS; ++k) {
+            Row &R = c->rows[k];
+            memset(&R, 0, sizeof R);
+            double b3 = w[k].b * w[k].b * w[k].b, a3 = w[k].a * w[k].a * w[k].a;
+            double expect = 4.0 / 3.0 * M_PI * std::max(b3 - a3, 0.0) * (w[k].lj ? rho_lj : rho);
+            R.cap = std::min(round32(1.6 * expect + 32.0), round32((double)n));
+            R.lj_only = w[k].lj;
+            R.r2min = (float)(w[k].a * w[k].a);
+            R.r2max = (float)(w[k].b * w[k].b);
+            c->row_fresh[k] = false;
+            if (w[k].on && (r = alloc_row(c, k))) return r;
+        }
+    }
+    if ((r = load_state(c, d_mass, d_charge, d_sigma, d_eps))) return r;
+    if ((r = resort_and_build(c))) return r;
+    c->rebuilds = 1;
+    if ((r = compute_f0(c))) return r;
+    if ((r = writeback(c))) return r;  // wrapped positions
+    return poll_error(c);
+}
+
+extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, float *d_vel, const float *d_mass,
+                         const float *d_charge, const float *d_lj_sigma, const float *d_lj_eps, int32_t n_bonds,
+                         const int32_t *d_bond_ij, const float *d_bond_k, const float *d_bond_r0, int32_t n_angles,
+                         const int32_t *d_angle_ijk, const float *d_angle_k, const float *d_angle_t0,
+                         const int32_t *d_excl_ptr, const int32_t *d_excl_idx, void *cuda_stream) {
+    if (!out || !p || !d_pos || !d_vel || !d_mass || !d_charge || !d_lj_sigma || !d_lj_eps) return JUMP_E_ARG;
+    if (p->n_atoms <= 0 || n_bonds < 0 || n_angles < 0) return JUMP_E_ARG;
+    if (p->n_inner <= 0 || (p->n_inner & 1)) return JUMP_E_ARG;
+    if (!(p->r_switch > 0.0) || !(p->r_short > p->r_switch) || !(p->r_short < p->r_long)) return JUMP_E_ARG;
+    for (int k = 0; k < 3; ++k) if (!(p->box[k] > 0.0) || p->r_long > 0.5 * p->box[k]) return JUMP_E_ARG;
+    if (p->eps_mode != 0 || !(p->eps_jump > 0.0) || !(p->dt_fs > 0.0) || p->gamma_per_ps < 0.0 || !(p->temperature_K > 0.0))
+        return JUMP_E_ARG;
+    if (p->skin < 0.0 || p->nlist_every < 0) return JUMP_E_ARG;
+    if (p->r_mid > 0.0 && (p->r_mid < p->r_short - p->r_switch || p->r_mid > p->r_long)) return JUMP_E_ARG;
+    jump_ctx *c = new jump_ctx();
+    c->st = (cudaStream_t)cuda_stream;
+    c->d_pos = d_pos; c->d_vel = d_vel;
+    c->step = c->outer = c->rebuilds = c->launches = 0;
+    c->sticky = 0;
+    int r = init_impl(c, p, d_mass, d_charge, d_lj_sigma, d_lj_eps, n_bonds, d_bond_ij, d_bond_k, d_bond_r0, n_angles,
+                      d_angle_ijk, d_angle_k, d_angle_t0, d_excl_ptr, d_excl_idx);
+    *out = c;  // returned even on failure so that jump_last_error can be read; free with jump_free
+    return r;
+}
+
+extern "C" void jump_free(jump_ctx *c) {
+    if (!c) return;
+    cudaStreamSynchronize(c->st);
+    for (void *q : c->owned) cudaFree(q);
+    delete c;
+}
+extern "C" const char *jump_last_error(const jump_ctx *c) { return c ? c->err.c_str() : "null context"; }
+extern "C" int64_t jump_get_step(const jump_ctx *c) { return c ? c->step : -1; }
+extern "C" int64_t jump_get_launches(const jump_ctx *c) { return c ? c->launches : -1; }
+extern "C" int jump_sync(jump_ctx *c) { return c ? poll_error(c) : JUMP_E_ARG; }
+
+// ---- observers ---------------------------------------------------------------------------------------------
+extern "C" int jump_get_forces(jump_ctx *c, int32_t which, float *d_out) {
+    if (!c || !d_out) return JUMP_E_ARG;
+    int r = 0;
+    const float4 *src = nullptr;
+    switch (which) {
+        case 0: r = compute_f0(c); src = c->f0; break;
+        case 1: r = compute_full(c, c->ftmp); src = c->ftmp; break;
+        case 2: r = compute_long(c, c->ftmp); src = c->ftmp; break;
+        case 3: r = bonded(c, nullptr, nullptr, c->fbond); src = c->fbond; break;
+        case 4: r = compute_short_nb(c, c->fnb); src = c->fnb; break;
+        default: return JUMP_E_ARG;
+    }
+    if (r) return r;
+    launch_unsort3(c->n, src, c->orig, d_out, c->st, &c->launches);
+    CK(cudaGetLastError());
+    return poll_error(c);
+}
+
+extern "C" int jump_get_energy(jump_ctx *c, double *e_kin, double *e_pot_full) {
+    if (!c) return JUMP_E_ARG;
+    int r;
+    if (e_kin) {
+        launch_kinetic(c->n, c->vs, c->mi, c->ke, c->st, &c->launches);
+        std::vector<double> h;
+        if ((r = ddownload(c, h, c->ke, c->n))) return r;
+        double s = 0.0;
+        for (double v : h) s += v;
+        *e_kin = s;
+    }
+    if (e_pot_full) {
+        if ((r = compute_full(c, c->ftmp, true))) return r;
+        std::vector<float4> h;
+        if ((r = ddownload(c, h, (const float4 *)c->ftmp, c->n))) return r;
+        double s = 0.0;
+        for (const float4 &v : h) s += (double)v.w;
+        *e_pot_full = s;
+    }
+    return poll_error(c);
+}
+
+extern "C" int jump_get_stats(jump_ctx *c, jump_stats *o) {
+    if (!c || !o) return JUMP_E_ARG;
+    Counters h;
+    CK(cudaMemcpyAsync(&h, c->ctr, sizeof h, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    memset(o, 0, sizeof *o);
+    o->proposals = (int64_t)h.proposals; o->accepts = (int64_t)h.accepts; o->gt_attempts = (int64_t)h.gt_attempts;
+    o->expiries = (int64_t)h.expiries; o->rebuilds = c->rebuilds;
+    float f;
+    memcpy(&f, &h.max_p_bits, 4); o->max_p = f;
+    memcpy(&f, &h.max_gl_bits, 4); o->max_g_over_L = f;
+    memcpy(&f, &h.max_disp2_bits, 4); o->max_disp = std::sqrt((double)f);
+    for (int k = 0; k < N_ROWS; ++k) { o->max_row[k] = h.max_row[k]; o->cap_row[k] = c->rows[k].enabled ? c->rows[k].cap : 0; }
+    poll_error(c);
+    o->error = c->sticky;
+    return 0;
+}
+extern "C" int jump_reset_stats(jump_ctx *c) {
+    if (!c) return JUMP_E_ARG;
+    Counters h;
+    CK(cudaMemcpyAsync(&h, c->ctr, sizeof h, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    unsigned long long ne = h.n_events;
+    memset(&h, 0, sizeof h);
+    h.n_events = ne;
+    CK(cudaMemcpyAsync(c->ctr, &h, sizeof h, cudaMemcpyHostToDevice, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    c->sticky = 0; c->err.clear();
+    return 0;
+}
+extern "C" int jump_get_events(jump_ctx *c, jump_event *buf, int64_t cap, int64_t *n) {
+    if (!c || !n) return JUMP_E_ARG;
+    Counters h;
+    CK(cudaMemcpyAsync(&h, c->ctr, sizeof h, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    *n = (int64_t)h.n_events;
+    int64_t m = std::min<int64_t>(std::min<int64_t>(*n, cap), c->event_cap);
+    if (buf && m > 0) {
+        CK(cudaMemcpyAsync(buf, c->events, sizeof(jump_event) * m, cudaMemcpyDeviceToHost, c->st));
+        CK(cudaStreamSynchronize(c->st));
+    }
+    return 0;
+}
+extern "C" int jump_clear_events(jump_ctx *c) {
+    if (!c) return JUMP_E_ARG;
+    CK(cudaMemsetAsync(&c->ctr->n_events, 0, sizeof(unsigned long long), c->st));
+    return 0;
+}
+extern "C" int jump_get_row(jump_ctx *c, int32_t which, int32_t atom, int32_t *host_out, int32_t cap) {
+    if (!c || which < 0 || which >= N_ROWS || atom < 0 || atom >= c->n) return JUMP_E_ARG;
+    const Row &R = c->rows[which];
+    if (!R.enabled) return JUMP_E_ARG;
+    int i = 0, cnt = 0;
+    CK(cudaMemcpyAsync(&i, c->sorted_of + atom, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    CK(cudaMemcpyAsync(&cnt, R.cnt + i, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    std::vector<int> row, orig;
+    int r;
+    if ((r = ddownload(c, row, (const int *)(R.idx + (size_t)i * R.cap), cnt)) || (r = ddownload(c, orig, (const int *)c->orig, c->n)))
+        return r;
+    for (int k = 0; k < cnt && k < cap; ++k) host_out[k] = orig[row[k]];
+    return cnt;
+}
+extern "C" int jump_get_bounds(jump_ctx *c, double out[8]) {
+    if (!c || !out) return JUMP_E_ARG;
+    out[0] = c->GM; out[1] = c->GL; out[2] = c->GV; out[3] = c->qmax;
+    out[4] = c->eps_max; out[5] = c->sig_min; out[6] = c->sig_max; out[7] = c->rM;
+    return 0;
+}
+extern "C" int jump_refresh(jump_ctx *c) {
+    if (!c) return JUMP_E_ARG;
+    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->st, &c->launches);
+    CK(cudaGetLastError());
+    int r = resort_and_build(c);
+    if (r) return r;
+    if ((r = compute_f0(c))) return r;
+    return poll_error(c);
+}

@@ -1,0 +1,134 @@
+// common.cuh -- shared declarations of the CUDA JUMP hot path (sm_100a).
+// P:Lnnn = PAPER.md line, R-n = DESIGN.md reading.  Nothing here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "../../include/jump_b200.h"
+
+namespace jb {
+
+// R-1 constants (restated independently of the oracle)
+constexpr double kKB = 1.987204259e-3;   // kcal/mol/K
+constexpr double kCoulomb = 332.063713;  // kcal A / (mol e^2)
+constexpr double kKcal = 418.4;          // (g/mol) A^2 ps^-2 per kcal/mol
+constexpr float kInvSqrt2Pi = 0.3989422804014327f;
+constexpr float kSqrt2Pi = 2.5066282746310002f;
+constexpr float kTwoOverSqrtPi = 1.1283791670955126f;
+
+// weight of a pair term: none, chi u (short), (1-chi) u (long), u (unsplit)
+enum { W_NONE = 0, W_SHORT = 1, W_LONG = 2, W_FULL = 3 };
+// row kinds
+enum { ROW_S = 0, ROW_M = 1, ROW_L = 2, ROW_V = 3, ROW_F = 4, ROW_W = 5, N_ROWS = 6 };
+// device error bits
+enum { ERR_OVERFLOW = 1, ERR_BOUND = 2, ERR_SKIN = 4, ERR_NAN = 8, ERR_EVENTS = 16 };
+
+struct Row {
+    int *idx;       // [n][cap] sorted indices, canonical order (R-10)
+    int *cnt;       // [n]
+    int cap;        // multiple of 32
+    int lj_only;    // keep eps_i eps_j > 0 only
+    float r2min, r2max;  // build-time window rmin <= d < rmax
+    int enabled;
+};
+
+// device counters (one struct in global memory)
+struct Counters {
+    unsigned long long proposals, accepts, gt_attempts, expiries, n_events;
+    unsigned int max_p_bits, max_gl_bits, max_disp2_bits;  // non-negative floats compared as uints
+    unsigned int err;
+    int max_row[N_ROWS];
+};
+
+// constants of the physical model, passed by value to kernels
+struct Model {
+    int n;
+    float box[3], inv_box[3];
+    float rc, h, inv_h, rlo;      // r_c, h, 1/h, r_c - h
+    float rc2, rlo2, rE2;         // squares
+    float alpha, alpha2;          // Ewald alpha
+    float beta;                   // 1/kT, (kcal/mol)^-1
+    float eps_jump;               // epsilon; +inf -> BPS
+    float qmaxGM, qmaxGL;         // qmax * G_M, qmax * G_L  (L_Y,i = |q_i| * this, R-7)
+    float GV4se;                  // 4 sqrt(eps_max) G_V     (L^vdW_i = sqrt(eps_i) * this)
+    float half_skin2;             // (skin/2)^2
+    unsigned int key0, key1;      // Philox key = seed
+};
+
+// Philox4x32-10 (Salmon et al. SC'11), R-15: counter (atom, step, stream, block), key = seed.
+__host__ __device__ inline void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t out[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+#ifdef __CUDA_ARCH__
+        uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+#else
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t h0 = (uint32_t)(p0 >> 32), l0 = (uint32_t)p0, h1 = (uint32_t)(p1 >> 32), l1 = (uint32_t)p1;
+#endif
+        uint32_t n0 = h1 ^ c1 ^ k0, n2 = h0 ^ c3 ^ k1;
+        c0 = n0; c1 = l1; c2 = n2; c3 = l0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// uniform in (0,1) with 24 significant bits, exact in fp32 and fp64 (R-15)
+__device__ inline float u01(uint32_t w) { return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f); }
+
+__device__ inline float wrap1(float x, float L, float invL) {
+    x -= L * floorf(x * invL);
+    if (x >= L) x -= L;
+    if (x < 0.f) x = 0.f;
+    return x;
+}
+// minimum image of xi - xj, both in [0, L).  The shift (0 or +-L) is applied to xi first:
+// xi - L is exact for xi in [L/2, L) (Sterbenz), so the result carries one rounding of the final
+// difference only -- a plain (xi - xj) - L would carry an absolute error of ulp(L) ~ 2e-6 A.
+__device__ inline float min_image1(float xi, float xj, float L, float invL) {
+    float t = (xi - xj) * invL + 12582912.f;  // round to nearest integer by the 1.5 * 2^23 trick
+    t -= 12582912.f;
+    return fmaf(-L, t, xi) - xj;
+}
+
+// chi (R-3): quintic smootherstep on [rc-h, rc]; returns chi, writes dchi/dr
+__device__ inline float chi_of(float r, const Model &m, float &dchi) {
+    float u = (r - m.rlo) * m.inv_h;
+    if (u <= 0.f) { dchi = 0.f; return 1.f; }
+    if (u >= 1.f) { dchi = 0.f; return 0.f; }
+    float omu = 1.f - u;
+    dchi = -30.f * u * u * omu * omu * m.inv_h;
+    return 1.f - u * u * u * (10.f - 15.f * u + 6.f * u * u);
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-visible launchers (one per .cu file group)
+// ---------------------------------------------------------------------------------------------
+struct SortGrid {
+    int gn[3];
+    double scale[3];  // gn / box (fp64: the cell of an atom is decided in the oracle's precision, R-10)
+    int ncell;
+    int reach[3];     // cells to visit on each side for the largest enabled row
+};
+
+struct Topo {  // per-atom CSR of bonded terms in ORIGINAL indices (device)
+    const int *bptr, *bother;   // bonds: partner atom
+    const float *bk, *br0;
+    const int *aptr, *arole, *aa, *ab;  // angles: my role (0 end i, 1 vertex, 2 end k) and the two other atoms
+    const float *ak, *at0;
+};
+
+struct Phase {      // one half-phase of velocity updates at frozen x
+    int kind;       // 0 none, 1 kick (B), 2 jump chains
+    float H;        // duration, ps
+    int use_grad;   // acceleration a = -M^-1 (ga + gb) else 0
+    int reverse;    // J' before C'
+    int coul, lj;   // which chains run (kind 2)
+    int streamC, streamJ;
+    unsigned int step;
+};
+
+}  // namespace jb

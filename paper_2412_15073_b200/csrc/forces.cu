@@ -1,0 +1,195 @@
+// forces.cu -- bonded gradient and switched pair gradient (a5, a10).
+//
+// Pair term (R-2, R-3, R-8):
+//   u_C(r) = C q_i q_j erfc(alpha r)/r,  u_LJ(r) = 4 eps_ij [(s_ij/r)^12 - (s_ij/r)^6],
+//   short part chi(r) u, long part (1-chi(r)) u, unsplit u; 0 beyond r_long.
+// Every output is a GRADIENT piece (R-4).  One warp per atom over a full (both directions) row:
+// the 32 lanes take 32 consecutive row entries (one coalesced 128-byte index load), gather x_j,
+// accumulate in registers and reduce by shuffles -- no floating-point atomics, deterministic.
+#include "launch.h"
+
+namespace jb {
+
+template <int W>
+__device__ inline float weighted_du(float r, float u, float du, const Model &m) {
+    if (W == W_FULL) return du;
+    float dchi, chi = chi_of(r, m, dchi);
+    if (W == W_SHORT) return chi * du + dchi * u;  // d/dr [chi u]
+    return (1.f - chi) * du - dchi * u;             // d/dr [(1-chi) u]
+}
+template <int W>
+__device__ inline float weighted_u(float r, float u, const Model &m) {
+    if (W == W_FULL) return u;
+    float dchi, chi = chi_of(r, m, dchi);
+    return W == W_SHORT ? chi * u : (1.f - chi) * u;
+}
+
+template <int WC, int WLJ, bool ENERGY>
+__global__ void __launch_bounds__(256) k_pair(Model m, Row row, const float4 *__restrict__ xs,
+                                              const float2 *__restrict__ lj, float4 *__restrict__ out, int accumulate) {
+    const unsigned full = 0xffffffffu;
+    int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (i >= m.n) return;
+    const float4 xi = xs[i];
+    const float qi = (float)kCoulomb * xi.w;
+    const float2 lji = lj[i];
+    const float cutC2 = (WC == W_SHORT) ? m.rc2 : m.rE2, cutL2 = (WLJ == W_SHORT) ? m.rc2 : m.rE2;
+    const float cut2 = (WC == W_NONE) ? cutL2 : ((WLJ == W_NONE) ? cutC2 : fmaxf(cutC2, cutL2));
+    const bool do_lj = (WLJ != W_NONE) && lji.y > 0.f;
+    const int cnt = row.cnt[i];
+    const int *__restrict__ ridx = row.idx + (size_t)i * row.cap;
+    float fx = 0.f, fy = 0.f, fz = 0.f, en = 0.f;
+    for (int k = lane; k < cnt; k += 32) {
+        int j = ridx[k];
+        float4 xj = xs[j];
+        float dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
+        float dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
+        float dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
+        float r2 = dx * dx + dy * dy + dz * dz;
+        if (r2 >= cut2) continue;
+        float rinv = rsqrtf(r2), r = r2 * rinv;
+        float fr = 0.f;
+        if (WC != W_NONE && r2 < cutC2) {
+            float qq = qi * xj.w;
+            float e = erfcf(m.alpha * r), ex = __expf(-m.alpha2 * r2);
+            float u = qq * e * rinv;
+            float du = -(u + qq * kTwoOverSqrtPi * m.alpha * ex) * rinv;  // u'
+            fr += weighted_du<WC>(r, u, du, m);
+            if (ENERGY) en += weighted_u<WC>(r, u, m);
+        }
+        if (do_lj && r2 < cutL2) {
+            float2 ljj = lj[j];
+            if (ljj.y > 0.f) {
+                float s = lji.x * ljj.x * rinv, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
+                float e4 = lji.y * ljj.y;  // 4 eps_ij (R-8: geometric mixing)
+                float u = e4 * (s12 - s6);
+                float du = e4 * (6.f * s6 - 12.f * s12) * rinv;
+                fr += weighted_du<WLJ>(r, u, du, m);
+                if (ENERGY) en += weighted_u<WLJ>(r, u, m);
+            }
+        }
+        float s = fr * rinv;
+        fx += s * dx; fy += s * dy; fz += s * dz;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        fx += __shfl_xor_sync(full, fx, off);
+        fy += __shfl_xor_sync(full, fy, off);
+        fz += __shfl_xor_sync(full, fz, off);
+        if (ENERGY) en += __shfl_xor_sync(full, en, off);
+    }
+    if (lane == 0) {
+        float4 o = make_float4(fx, fy, fz, 0.5f * en);
+        if (accumulate) { float4 p = out[i]; o.x += p.x; o.y += p.y; o.z += p.z; o.w += p.w; }
+        out[i] = o;
+    }
+}
+
+// Harmonic bonds k (r-r0)^2 and angles k (theta-theta0)^2 (R-2), one thread per atom over the terms
+// the atom takes part in; evaluated in fp64 (a few hundred flops per atom) because r - r0 cancels.
+__device__ inline double min_image_d(float xi, float xj, float L) {
+    double d = (double)xi - (double)xj, Ld = (double)L;
+    return d - Ld * rint(d / Ld);
+}
+
+__global__ void k_bonded(Model m, Topo t, const float4 *__restrict__ xs, const int *__restrict__ orig,
+                         const int *__restrict__ sorted_of, const float4 *__restrict__ add,
+                         float4 *__restrict__ out_sum, float4 *__restrict__ out_bond) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m.n) return;
+    const int o = orig[i];
+    const float4 xi = xs[i];
+    double gx = 0., gy = 0., gz = 0., en = 0.;
+    for (int b = t.bptr[o]; b < t.bptr[o + 1]; ++b) {
+        float4 xj = xs[sorted_of[t.bother[b]]];
+        double dx = min_image_d(xi.x, xj.x, m.box[0]);
+        double dy = min_image_d(xi.y, xj.y, m.box[1]);
+        double dz = min_image_d(xi.z, xj.z, m.box[2]);
+        double r = sqrt(dx * dx + dy * dy + dz * dz), dr = r - (double)t.br0[b], k = (double)t.bk[b];
+        double f = 2.0 * k * dr / r;
+        gx += f * dx; gy += f * dy; gz += f * dz;
+        en += 0.5 * k * dr * dr;
+    }
+    for (int a = t.aptr[o]; a < t.aptr[o + 1]; ++a) {
+        // role 1: I am the vertex, (aa, ab) are the ends; else I am an end, aa = vertex, ab = other end
+        const int role = t.arole[a];
+        float4 xa = xs[sorted_of[t.aa[a]]], xb = xs[sorted_of[t.ab[a]]];
+        float4 xv = role == 1 ? xi : xa;             // vertex
+        float4 xe1 = role == 1 ? xa : xi;            // end whose gradient is "gi"
+        float4 xe2 = xb;                             // other end
+        double u[3], w[3];
+        u[0] = min_image_d(xe1.x, xv.x, m.box[0]);
+        u[1] = min_image_d(xe1.y, xv.y, m.box[1]);
+        u[2] = min_image_d(xe1.z, xv.z, m.box[2]);
+        w[0] = min_image_d(xe2.x, xv.x, m.box[0]);
+        w[1] = min_image_d(xe2.y, xv.y, m.box[1]);
+        w[2] = min_image_d(xe2.z, xv.z, m.box[2]);
+        double lu = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]), lw = sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+        double ct = (u[0] * w[0] + u[1] * w[1] + u[2] * w[2]) / (lu * lw);
+        ct = fmin(1.0, fmax(-1.0, ct));
+        double th = acos(ct), st = fmax(sqrt(1.0 - ct * ct), 1e-12);
+        double dth = th - (double)t.at0[a], k = (double)t.ak[a], dU = 2.0 * k * dth;
+        double g[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            double gi = -dU * (w[c] / lw - ct * u[c] / lu) / (lu * st);
+            if (role == 1) {
+                double gk = -dU * (u[c] / lu - ct * w[c] / lw) / (lw * st);
+                g[c] = -(gi + gk);
+            } else g[c] = gi;
+        }
+        gx += g[0]; gy += g[1]; gz += g[2];
+        en += k * dth * dth * (1.0 / 3.0);
+    }
+    float4 fb = make_float4((float)gx, (float)gy, (float)gz, (float)en);
+    if (out_bond) out_bond[i] = fb;
+    if (out_sum) {
+        if (add) { float4 p = add[i]; fb.x += p.x; fb.y += p.y; fb.z += p.z; fb.w += p.w; }
+        out_sum[i] = fb;
+    }
+}
+
+// out[orig[i]] = f[i].xyz  (sorted -> caller order)
+__global__ void k_unsort3(int n, const float4 *__restrict__ f, const int *__restrict__ orig, float *__restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 v = f[i];
+    int o = orig[i];
+    out[3 * o] = v.x; out[3 * o + 1] = v.y; out[3 * o + 2] = v.z;
+}
+
+template <int WC, int WLJ>
+static void pair_dispatch(const Model &m, const Row &row, const float4 *xs, const float2 *lj, float4 *out, int accumulate,
+                          bool energy, cudaStream_t st) {
+    const int B = 256;
+    unsigned grid = (unsigned)(((long long)m.n * 32 + B - 1) / B);
+    if (energy) k_pair<WC, WLJ, true><<<grid, B, 0, st>>>(m, row, xs, lj, out, accumulate);
+    else k_pair<WC, WLJ, false><<<grid, B, 0, st>>>(m, row, xs, lj, out, accumulate);
+}
+
+int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *xs, const float2 *lj, float4 *out,
+                int accumulate, bool energy, cudaStream_t st, int64_t *launches) {
+    *launches += 1;
+#define JB_CASE(a, b) \
+    if (wC == a && wLJ == b) { pair_dispatch<a, b>(m, row, xs, lj, out, accumulate, energy, st); return 0; }
+    JB_CASE(W_SHORT, W_SHORT) JB_CASE(W_SHORT, W_FULL) JB_CASE(W_NONE, W_FULL) JB_CASE(W_FULL, W_FULL)
+    JB_CASE(W_LONG, W_LONG) JB_CASE(W_LONG, W_NONE) JB_CASE(W_SHORT, W_NONE)
+#undef JB_CASE
+    *launches -= 1;
+    return -1;
+}
+
+void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const int *orig, const int *sorted_of,
+                   const float4 *add, float4 *out_sum, float4 *out_bond, cudaStream_t st, int64_t *launches) {
+    const int B = 128;
+    k_bonded<<<(m.n + B - 1) / B, B, 0, st>>>(m, t, xs, orig, sorted_of, add, out_sum, out_bond);
+    *launches += 1;
+}
+
+void launch_unsort3(int n, const float4 *f, const int *orig, float *out, cudaStream_t st, int64_t *launches) {
+    const int B = 256;
+    k_unsort3<<<(n + B - 1) / B, B, 0, st>>>(n, f, orig, out);
+    *launches += 1;
+}
+
+}  // namespace jb

@@ -1,0 +1,57 @@
+// launch.h -- host-side launcher prototypes shared by the .cu files of the CUDA path.
+#pragma once
+#include "common.cuh"
+
+namespace jb {
+
+struct SortArgs {
+    int n;
+    SortGrid grid;
+    const float4 *xs_in, *vs_in;
+    const float2 *lj_in, *mi_in;
+    const int *orig_in;
+    float4 *xs, *vs, *x_build;
+    float2 *lj, *mi;
+    int *orig, *sorted_of;
+    int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src;
+    Counters *ctr;
+};
+
+struct UpdateArgs {
+    Phase ph[2];
+    const float4 *grad[2];
+    int do_aoa;
+    float half_dt, c1, c2;  // delta/2 (ps), exp(-gamma delta), sqrt(1 - c1^2)
+    unsigned o_step;        // Philox step index of the O part
+    const float4 *xs;
+    float4 *xs_out;
+    float4 *vs;
+    const float2 *mi, *lj;
+    const int *orig;
+    const float4 *x_build;
+    Row rowM, rowL, rowV;
+    Counters *ctr;
+    jump_event *events;  // NULL: no log
+    long long event_cap;
+};
+
+void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches);
+void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS], float rmax_all, const int *cell_start,
+                       const float4 *xs, const float2 *lj, const int *orig, const int *sorted_of, const int *excl_ptr,
+                       const int *excl_idx, Counters *ctr, cudaStream_t st, int64_t *launches);
+int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *xs, const float2 *lj, float4 *out,
+                int accumulate, bool energy, cudaStream_t st, int64_t *launches);
+void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const int *orig, const int *sorted_of,
+                   const float4 *add, float4 *out_sum, float4 *out_bond, cudaStream_t st, int64_t *launches);
+void launch_unsort3(int n, const float4 *f, const int *orig, float *out, cudaStream_t st, int64_t *launches);
+void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st, int64_t *launches);
+void launch_writeback(int n, const float4 *xs, const float4 *vs, const int *orig, float *pos, float *vel, cudaStream_t st,
+                      int64_t *launches);
+void launch_load(const Model &m, const float *pos, const float *vel, const float *mass, const float *charge,
+                 const float *sigma, const float *eps, double kT, float4 *xs, float4 *vs, float2 *lj, float2 *mi, int *orig,
+                 cudaStream_t st, int64_t *launches);
+void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
+                   cudaStream_t st, int64_t *launches);
+void launch_kinetic(int n, const float4 *vs, const float2 *mi, double *out, cudaStream_t st, int64_t *launches);
+
+}  // namespace jb

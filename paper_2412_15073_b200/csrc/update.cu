@@ -1,0 +1,398 @@
+// update.cu -- velocity half-phases (B kick / jump chains C', J') and the fused A-O-A drift
+// (SURVEY 8(a) a6, a7, a8).
+//
+// C' : Algorithm 4 with the ring technique, as reconstructed in R-11.
+// J' : Algorithm 5, BPS on the long LJ part, with an exponential clock (R-14).
+// A, O: x += (delta/2) v;  v <- c1 v + c2 m^-1/2 G.
+// Chains of different atoms are independent and a jump of type (i,j) changes v_i only
+// (P:L342): one chain per thread, writing nothing but its own v_i -- no cross-atom conflict; several
+// events on one atom are resolved in time order inside its chain.
+#include "launch.h"
+
+namespace jb {
+
+struct Tally {  // per-thread statistics, reduced once per warp at the end
+    unsigned proposals, accepts, gt_attempts, expiries;
+    float max_p, max_gl;
+};
+
+__device__ inline void log_event(const UpdateArgs &a, unsigned step, int stream, int atom, int iter, int ring, int j,
+                                 int accepted, int n_gt, float T, float p, float U, float gt) {
+    if (!a.events) return;
+    unsigned long long slot = atomicAdd(&a.ctr->n_events, 1ull);
+    if (slot >= (unsigned long long)a.event_cap) { atomicOr(&a.ctr->err, (unsigned)ERR_EVENTS); return; }
+    jump_event e;
+    e.step = (int)step; e.stream = stream; e.atom = atom; e.iter = iter;
+    e.ring = ring; e.j = j; e.accepted = accepted; e.n_gt = n_gt;
+    e.T = T; e.p = p; e.U = U; e.gt = gt;
+    a.events[slot] = e;
+}
+
+// Theta(eta) = E[(eta+G)_+] = eta Phi(eta) + phi(eta)  (R-5)
+__device__ inline float theta_of(float eta) {
+    float Phi = 0.5f * erfcf(-eta * 0.70710678118654752f);
+    float phi = kInvSqrt2Pi * expf(-0.5f * eta * eta);
+    return eta * Phi + phi;
+}
+
+// G~ ~ f_eta by rejection (R-6; proposal family of P:L310).  One Philox block per attempt.
+__device__ inline float gtilde(float eta, unsigned atom, unsigned step, unsigned stream, unsigned &block,
+                               const Model &m, int &attempts) {
+    uint32_t w[4];
+    int it = 0;
+    float out = 0.f;
+    for (;;) {
+        ++it;
+        philox4x32_10(atom, step, stream, block++, m.key0, m.key1, w);
+        float u0 = u01(w[0]), u1 = u01(w[1]), u2 = u01(w[2]), u3 = u01(w[3]);
+        if (eta < -2.5f) {  // Gamma(2, |eta|)
+            float z = -(logf(u0) + logf(u1)) / fabsf(eta);
+            if (u2 <= expf(-0.5f * z * z)) { out = z - eta; break; }
+        } else if (eta < -1.f) {  // Exponential(|eta|)
+            float z = -logf(u0) / fabsf(eta);
+            if (u1 <= z * expf(0.5f * (1.f - z * z))) { out = z - eta; break; }
+        } else if (eta <= 0.f) {  // Rayleigh
+            float z = sqrtf(-2.f * logf(u0));
+            if (u1 <= expf(eta * z)) { out = z - eta; break; }
+        } else {  // Rayleigh-Gaussian mixture
+            float wR = 1.f / (1.f + eta * kSqrt2Pi);
+            if (u0 <= wR) { out = sqrtf(-2.f * logf(u1)); break; }
+            float y = sqrtf(-2.f * logf(u1)) * cospif(2.f * u2);
+            if (y > 0.f) { out = y; break; }
+            if (y > -eta) {
+                if (u3 <= (eta + y) / eta) { out = y; break; }
+            }
+        }
+        if (it >= 64) { out = (eta > 0.f) ? 0.f : -eta + 1.f; break; }
+    }
+    attempts = it;
+    return out;
+}
+
+// kick (7); eps = inf -> reflection (5)
+__device__ inline void jump_kick(float eps, float sbm, float nx, float ny, float nz, float gt, float &vx, float &vy,
+                                 float &vz) {
+    float vn = vx * nx + vy * ny + vz * nz, amp;
+    if (isinf(eps)) amp = 2.f * vn;
+    else amp = 2.f * eps / ((1.f + eps * eps) * sbm) * (eps * sbm * vn + gt);
+    vx -= amp * nx; vy -= amp * ny; vz -= amp * nz;
+}
+
+// long part of the Coulomb pair gradient, F_ij = grad_{x_i} (1-chi) u_C: returns fr = radial
+// derivative, d = minimum-image x_i - x_j, r
+__device__ inline float fij_coul(const Model &m, const float4 &xi, const float4 &xj, float &dx, float &dy, float &dz,
+                                 float &rinv) {
+    dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
+    dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
+    dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
+    float r2 = dx * dx + dy * dy + dz * dz;
+    if (r2 >= m.rE2 || r2 <= m.rlo2) { rinv = 0.f; return 0.f; }
+    rinv = rsqrtf(r2);
+    float r = r2 * rinv;
+    float qq = (float)kCoulomb * xi.w * xj.w;
+    float e = erfcf(m.alpha * r), ex = expf(-m.alpha2 * r2);
+    float u = qq * e * rinv;
+    float du = -(u + qq * kTwoOverSqrtPi * m.alpha * ex) * rinv;
+    float dchi, chi = chi_of(r, m, dchi);
+    return (1.f - chi) * du - dchi * u;
+}
+__device__ inline float fij_lj(const Model &m, const float4 &xi, const float4 &xj, float2 lji, float2 ljj, float &dx,
+                               float &dy, float &dz, float &rinv) {
+    dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
+    dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
+    dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
+    float r2 = dx * dx + dy * dy + dz * dz;
+    if (r2 >= m.rE2 || r2 <= m.rlo2) { rinv = 0.f; return 0.f; }
+    rinv = rsqrtf(r2);
+    float r = r2 * rinv;
+    float s = lji.x * ljj.x * rinv, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
+    float e4 = lji.y * ljj.y;
+    float u = e4 * (s12 - s6), du = e4 * (6.f * s6 - 12.f * s12) * rinv;
+    float dchi, chi = chi_of(r, m, dchi);
+    return (1.f - chi) * du - dchi * u;
+}
+
+// ---- step (C'): Algorithm 4 + ring (R-11).  x frozen; updates (vx,vy,vz) of atom i. -------------------------
+__device__ void chain_C(const Model &m, const UpdateArgs &A, int i, unsigned atom, const float4 &xi, float sbm,
+                        float ax, float ay, float az, float H, unsigned stream, unsigned step, float &vx, float &vy,
+                        float &vz, Tally &tl) {
+    const float eps = m.eps_jump, beta = m.beta;
+    const bool bps = isinf(eps);
+    const int NM = A.rowM.cnt[i], NL = A.rowL.cnt[i];
+    const float aq = fabsf(xi.w);
+    const float LM = aq * m.qmaxGM, LL = aq * m.qmaxGL;
+    const float SM = (float)NM * LM, S = SM + (float)NL * LL;
+    const float lam0 = bps ? 0.f : (1.f / eps) * beta * kInvSqrt2Pi / sbm;
+    const float a2 = ax * ax + ay * ay + az * az;
+    float t = 0.f;
+    unsigned block = 0;
+    uint32_t w[4];
+    for (int iter = 0;; ++iter) {
+        float tau = H - t;
+        float va = vx * ax + vy * ay + vz * az;
+        float v2 = vx * vx + vy * vy + vz * vz;
+        float Bv = sqrtf(v2 + tau * tau * a2 + 2.f * tau * fmaxf(va, 0.f));
+        float lam = S * (beta * Bv + lam0);
+        philox4x32_10(atom, step, stream, block++, m.key0, m.key1, w);
+        float E = -logf(u01(w[0]));
+        float T = lam > 0.f ? E / lam : INFINITY;
+        if (!(t + T <= H)) {
+            vx += tau * ax; vy += tau * ay; vz += tau * az;
+            tl.expiries++;
+            log_event(A, step, stream, atom, iter, -1, -1, 0, 0, T, 0.f, 0.f, 0.f);
+            break;
+        }
+        t += T;
+        vx += T * ax; vy += T * ay; vz += T * az;
+        float ur = u01(w[1]);  // ring pick
+        int ring = (ur * S < SM) ? 0 : 1;
+        if (ring == 0 && NM == 0) ring = 1;
+        if (ring == 1 && NL == 0) ring = 0;
+        const int cnt = ring == 0 ? NM : NL;
+        const int k = (int)__umulhi(w[2], (unsigned)cnt);
+        const int j = ring == 0 ? A.rowM.idx[(size_t)i * A.rowM.cap + k] : A.rowL.idx[(size_t)i * A.rowL.cap + k];
+        const float LY = ring == 0 ? LM : LL;
+        const float U = u01(w[3]);
+        tl.proposals++;
+        float dx, dy, dz, rinv;
+        float fr = fij_coul(m, xi, A.xs[j], dx, dy, dz, rinv);
+        float g = fabsf(fr), p = 0.f, gt = 0.f;
+        int acc = 0, att = 0;
+        if (g > 0.f) {
+            tl.max_gl = fmaxf(tl.max_gl, g / LY);
+            float sg = (fr > 0.f ? rinv : -rinv);  // n = F/|F|
+            float nx = dx * sg, ny = dy * sg, nz = dz * sg;
+            float vn = vx * nx + vy * ny + vz * nz;
+            if (bps) p = fmaxf(vn, 0.f) * g / (LY * Bv);
+            else p = g * theta_of(eps * sbm * vn) / (LY * (Bv * eps * sbm + kInvSqrt2Pi));  // P:L397 with sqrt(beta)
+            tl.max_p = fmaxf(tl.max_p, p);
+            if (U <= p) {
+                if (!bps) gt = gtilde(eps * sbm * vn, atom, step, stream, block, m, att);
+                jump_kick(eps, sbm, nx, ny, nz, gt, vx, vy, vz);
+                acc = 1;
+                tl.accepts++;
+                tl.gt_attempts += att;
+            }
+        }
+        log_event(A, step, stream, atom, iter, ring, A.orig[j], acc, att, T, p, U, gt);
+    }
+}
+
+// ---- step (J'): Algorithm 5 (R-14) ---------------------------------------------------------------------------
+__device__ void chain_J(const Model &m, const UpdateArgs &A, int i, unsigned atom, const float4 &xi, float2 lji,
+                        float sbm, float H, unsigned stream, unsigned step, float &vx, float &vy, float &vz, Tally &tl) {
+    if (!(lji.y > 0.f)) return;
+    const int NV = A.rowV.cnt[i];
+    if (NV == 0) return;
+    const float L = 0.5f * lji.y * m.GV4se;  // 4 sqrt(eps_i eps_max) G_V; lji.y = 2 sqrt(eps_i)
+    float t = 0.f;
+    unsigned block = 0;
+    uint32_t w[4];
+    for (int iter = 0;; ++iter) {
+        float vv = sqrtf(vx * vx + vy * vy + vz * vz);
+        float lam = (float)NV * m.beta * vv * L;
+        philox4x32_10(atom, step, stream, block++, m.key0, m.key1, w);
+        float E = -logf(u01(w[0]));
+        float T = lam > 0.f ? E / lam : INFINITY;
+        if (!(t + T <= H)) {
+            tl.expiries++;
+            log_event(A, step, stream, atom, iter, -1, -1, 0, 0, T, 0.f, 0.f, 0.f);
+            break;
+        }
+        t += T;
+        const int k = (int)__umulhi(w[1], (unsigned)NV);
+        const int j = A.rowV.idx[(size_t)i * A.rowV.cap + k];
+        const float U = u01(w[2]);
+        tl.proposals++;
+        float dx, dy, dz, rinv;
+        float fr = fij_lj(m, xi, A.xs[j], lji, A.lj[j], dx, dy, dz, rinv);
+        float g = fabsf(fr), p = 0.f;
+        int acc = 0;
+        if (g > 0.f) {
+            tl.max_gl = fmaxf(tl.max_gl, g / L);
+            float sg = (fr > 0.f ? rinv : -rinv);
+            float nx = dx * sg, ny = dy * sg, nz = dz * sg;
+            float vF = (vx * nx + vy * ny + vz * nz) * g;
+            p = fmaxf(vF, 0.f) / (vv * L);
+            tl.max_p = fmaxf(tl.max_p, p);
+            if (U <= p) {  // reflection (5)
+                jump_kick(INFINITY, sbm, nx, ny, nz, 0.f, vx, vy, vz);
+                acc = 1;
+                tl.accepts++;
+            }
+        }
+        log_event(A, step, stream, atom, iter, 2, A.orig[j], acc, 0, T, p, U, 0.f);
+    }
+}
+
+// ---- the fused per-atom update: up to two velocity half-phases, then A O A + wrap ----------------------------
+template <bool JUMPS>
+__global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
+    const unsigned full = 0xffffffffu;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool live = i < m.n;
+    Tally tl = {0u, 0u, 0u, 0u, 0.f, 0.f};
+    float disp2 = 0.f;
+    bool bad = false;
+    if (live) {
+        const float4 xi = A.xs[i];
+        float4 v4 = A.vs[i];
+        float vx = v4.x, vy = v4.y, vz = v4.z;
+        const float2 mi = A.mi[i];  // (kcal-scaled 1/m, sqrt(beta m))
+        const unsigned atom = (unsigned)A.orig[i];
+#pragma unroll
+        for (int ph = 0; ph < 2; ++ph) {
+            const Phase &P = A.ph[ph];
+            if (P.kind == 0) continue;
+            float ax = 0.f, ay = 0.f, az = 0.f;
+            if (P.use_grad) {  // a = -M^-1 F
+                float4 g = A.grad[ph][i];
+                ax = -mi.x * g.x; ay = -mi.x * g.y; az = -mi.x * g.z;
+            }
+            if (P.kind == 1 || !JUMPS) {
+                vx += P.H * ax; vy += P.H * ay; vz += P.H * az;
+            } else {
+                const float2 lji = A.lj[i];
+                if (P.reverse && P.lj) chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl);
+                if (P.coul) chain_C(m, A, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl);
+                else if (P.use_grad) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
+                if (!P.reverse && P.lj) chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl);
+            }
+        }
+        if (A.do_aoa) {
+            float x = xi.x, y = xi.y, z = xi.z;
+            x += A.half_dt * vx; y += A.half_dt * vy; z += A.half_dt * vz;  // A
+            uint32_t w[4];                                                  // O
+            philox4x32_10(atom, A.o_step, 0u, 0u, m.key0, m.key1, w);
+            float r1 = sqrtf(-2.f * logf(u01(w[0]))), r2 = sqrtf(-2.f * logf(u01(w[2])));
+            float s1, c1, c2;
+            sincospif(2.f * u01(w[1]), &s1, &c1);
+            c2 = cospif(2.f * u01(w[3]));
+            float sc = A.c2 / mi.y;
+            vx = A.c1 * vx + sc * (r1 * c1);
+            vy = A.c1 * vy + sc * (r1 * s1);
+            vz = A.c1 * vz + sc * (r2 * c2);
+            x += A.half_dt * vx; y += A.half_dt * vy; z += A.half_dt * vz;  // A
+            x = wrap1(x, m.box[0], m.inv_box[0]);
+            y = wrap1(y, m.box[1], m.inv_box[1]);
+            z = wrap1(z, m.box[2], m.inv_box[2]);
+            A.xs_out[i] = make_float4(x, y, z, xi.w);
+            float4 xb = A.x_build[i];
+            float ddx = min_image1(x, xb.x, m.box[0], m.inv_box[0]);
+            float ddy = min_image1(y, xb.y, m.box[1], m.inv_box[1]);
+            float ddz = min_image1(z, xb.z, m.box[2], m.inv_box[2]);
+            disp2 = ddx * ddx + ddy * ddy + ddz * ddz;
+            bad = !(isfinite(x) && isfinite(y) && isfinite(z));
+        }
+        bad = bad || !(isfinite(vx) && isfinite(vy) && isfinite(vz));
+        A.vs[i] = make_float4(vx, vy, vz, v4.w);
+    }
+    // warp-level reduction of the statistics, then a few integer atomics per warp
+    unsigned err = 0;
+    if (bad) err |= ERR_NAN;
+    if (disp2 > m.half_skin2) err |= ERR_SKIN;
+    if (tl.max_p > 1.f + 1e-4f || tl.max_gl > 1.f + 1e-4f) err |= ERR_BOUND;
+    unsigned d2b = __reduce_max_sync(full, __float_as_uint(disp2));
+    err = __reduce_or_sync(full, err);
+    const int lane = threadIdx.x & 31;
+    if (JUMPS) {
+        unsigned np = __reduce_add_sync(full, tl.proposals), na = __reduce_add_sync(full, tl.accepts);
+        unsigned ng = __reduce_add_sync(full, tl.gt_attempts), ne = __reduce_add_sync(full, tl.expiries);
+        unsigned mp = __reduce_max_sync(full, __float_as_uint(tl.max_p));
+        unsigned mg = __reduce_max_sync(full, __float_as_uint(tl.max_gl));
+        if (lane == 0) {
+            if (np) atomicAdd(&A.ctr->proposals, (unsigned long long)np);
+            if (na) atomicAdd(&A.ctr->accepts, (unsigned long long)na);
+            if (ng) atomicAdd(&A.ctr->gt_attempts, (unsigned long long)ng);
+            if (ne) atomicAdd(&A.ctr->expiries, (unsigned long long)ne);
+            if (mp > A.ctr->max_p_bits) atomicMax(&A.ctr->max_p_bits, mp);
+            if (mg > A.ctr->max_gl_bits) atomicMax(&A.ctr->max_gl_bits, mg);
+        }
+    }
+    if (lane == 0) {
+        if (d2b > A.ctr->max_disp2_bits) atomicMax(&A.ctr->max_disp2_bits, d2b);
+        if (err) atomicOr(&A.ctr->err, err);
+    }
+}
+
+// caller arrays (original order, n x 3) <-> sorted float4
+__global__ void k_writeback(int n, const float4 *__restrict__ xs, const float4 *__restrict__ vs,
+                            const int *__restrict__ orig, float *__restrict__ pos, float *__restrict__ vel) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int o = orig[i];
+    float4 x = xs[i], v = vs[i];
+    pos[3 * o] = x.x; pos[3 * o + 1] = x.y; pos[3 * o + 2] = x.z;
+    vel[3 * o] = v.x; vel[3 * o + 1] = v.y; vel[3 * o + 2] = v.z;
+}
+
+// original order in: wrap positions, pack (x, q), (v), (sqrt sigma, 2 sqrt eps), (kcal/m, sqrt(beta m))
+__global__ void k_load(Model m, const float *__restrict__ pos, const float *__restrict__ vel,
+                       const float *__restrict__ mass, const float *__restrict__ charge,
+                       const float *__restrict__ sigma, const float *__restrict__ eps, double kT, float4 *__restrict__ xs,
+                       float4 *__restrict__ vs, float2 *__restrict__ lj, float2 *__restrict__ mi, int *__restrict__ orig) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m.n) return;
+    float x = wrap1(pos[3 * i], m.box[0], m.inv_box[0]);
+    float y = wrap1(pos[3 * i + 1], m.box[1], m.inv_box[1]);
+    float z = wrap1(pos[3 * i + 2], m.box[2], m.inv_box[2]);
+    xs[i] = make_float4(x, y, z, charge[i]);
+    vs[i] = make_float4(vel[3 * i], vel[3 * i + 1], vel[3 * i + 2], 0.f);
+    float e = eps[i];
+    lj[i] = make_float2(e > 0.f ? (float)sqrt((double)sigma[i]) : 0.f, e > 0.f ? (float)(2.0 * sqrt((double)e)) : 0.f);
+    double md = (double)mass[i];
+    mi[i] = make_float2((float)(kKcal / md), (float)sqrt(md / (kT * kKcal)));
+    orig[i] = i;
+}
+
+// re-read the caller's positions (wrapped) and velocities into the current sorted order
+__global__ void k_reload(Model m, const float *__restrict__ pos, const float *__restrict__ vel,
+                         const int *__restrict__ orig, float4 *__restrict__ xs, float4 *__restrict__ vs) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m.n) return;
+    int o = orig[i];
+    float4 x = xs[i];
+    x.x = wrap1(pos[3 * o], m.box[0], m.inv_box[0]);
+    x.y = wrap1(pos[3 * o + 1], m.box[1], m.inv_box[1]);
+    x.z = wrap1(pos[3 * o + 2], m.box[2], m.inv_box[2]);
+    xs[i] = x;
+    vs[i] = make_float4(vel[3 * o], vel[3 * o + 1], vel[3 * o + 2], 0.f);
+}
+
+// kinetic energy per atom into out[i] (kcal/mol), sorted order
+__global__ void k_kinetic(int n, const float4 *__restrict__ vs, const float2 *__restrict__ mi, double *__restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 v = vs[i];
+    double v2 = (double)v.x * v.x + (double)v.y * v.y + (double)v.z * v.z;
+    out[i] = 0.5 * v2 / (double)mi[i].x;  // (1/2) m v^2 / KCAL with mi.x = KCAL / m
+}
+
+void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st, int64_t *launches) {
+    const int B = 128;
+    if (jumps) k_update<true><<<(m.n + B - 1) / B, B, 0, st>>>(m, A);
+    else k_update<false><<<(m.n + B - 1) / B, B, 0, st>>>(m, A);
+    *launches += 1;
+}
+void launch_writeback(int n, const float4 *xs, const float4 *vs, const int *orig, float *pos, float *vel, cudaStream_t st,
+                      int64_t *launches) {
+    k_writeback<<<(n + 255) / 256, 256, 0, st>>>(n, xs, vs, orig, pos, vel);
+    *launches += 1;
+}
+void launch_load(const Model &m, const float *pos, const float *vel, const float *mass, const float *charge,
+                 const float *sigma, const float *eps, double kT, float4 *xs, float4 *vs, float2 *lj, float2 *mi, int *orig,
+                 cudaStream_t st, int64_t *launches) {
+    k_load<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, mass, charge, sigma, eps, kT, xs, vs, lj, mi, orig);
+    *launches += 1;
+}
+void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
+                   cudaStream_t st, int64_t *launches) {
+    k_reload<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, orig, xs, vs);
+    *launches += 1;
+}
+void launch_kinetic(int n, const float4 *vs, const float2 *mi, double *out, cudaStream_t st, int64_t *launches) {
+    k_kinetic<<<(n + 255) / 256, 256, 0, st>>>(n, vs, mi, out);
+    *launches += 1;
+}
+
+}  // namespace jb
