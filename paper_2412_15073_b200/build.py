@@ -38,7 +38,7 @@ def build(force=False, verbose=False):
         for _, log in res:
             sys.stderr.write(log)
     tmp = LIB + ".tmp%d" % os.getpid()
-    cmd = [nvcc, "-shared", "-o", tmp] + [o for o, _ in res]
+    cmd = [nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", tmp] + [o for o, _ in res]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
     return LIB

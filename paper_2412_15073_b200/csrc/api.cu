@@ -23,7 +23,7 @@ struct jump_ctx {
     float c1, c2;
     float *d_pos, *d_vel;  // caller's
     // sorted state (cur) and spare buffers (nxt)
-    float4 *xs, *xs_nxt, *vs, *vs_nxt, *x_build;
+    float4 *xs, *xs_nxt, *vs, *vs_nxt, *xl, *xl_nxt, *x_build;
     float2 *lj, *lj_nxt, *mi, *mi_nxt;
     int *orig, *orig_nxt, *sorted_of;
     int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src;
@@ -164,14 +164,14 @@ static int build_rows(jump_ctx *c, bool only_missing) {
 static int resort_and_build(jump_ctx *c) {
     SortArgs a;
     a.n = c->n; a.grid = c->g;
-    a.xs_in = c->xs; a.vs_in = c->vs; a.lj_in = c->lj; a.mi_in = c->mi; a.orig_in = c->orig;
+    a.xs_in = c->xs; a.vs_in = c->vs; a.xl_in = c->xl; a.xl = c->xl_nxt; a.lj_in = c->lj; a.mi_in = c->mi; a.orig_in = c->orig;
     a.xs = c->xs_nxt; a.vs = c->vs_nxt; a.lj = c->lj_nxt; a.mi = c->mi_nxt; a.orig = c->orig_nxt;
     a.sorted_of = c->sorted_of; a.x_build = c->x_build;
     a.key = c->key; a.cell_count = c->cell_count; a.cell_fill = c->cell_fill; a.cell_start = c->cell_start;
     a.tmp_orig = c->tmp_orig; a.tmp_src = c->tmp_src; a.ctr = c->ctr;
     launch_sort(a, c->st, &c->launches);
     CK(cudaGetLastError());
-    std::swap(c->xs, c->xs_nxt); std::swap(c->vs, c->vs_nxt); std::swap(c->lj, c->lj_nxt);
+    std::swap(c->xs, c->xs_nxt); std::swap(c->vs, c->vs_nxt); std::swap(c->xl, c->xl_nxt); std::swap(c->lj, c->lj_nxt);
     std::swap(c->mi, c->mi_nxt); std::swap(c->orig, c->orig_nxt);
     for (int k = 0; k < N_ROWS; ++k) c->row_fresh[k] = false;
     c->rebuilds++;
@@ -188,7 +188,7 @@ static bool lj_jumps(const jump_ctx *c) { return (c->p.flags & JUMP_F_LJ_JUMPS) 
 static bool coul_jumps(const jump_ctx *c) { return (c->p.flags & JUMP_F_COUL_JUMPS) != 0; }
 
 static int bonded(jump_ctx *c, const float4 *add, float4 *out_sum, float4 *out_bond) {
-    launch_bonded(c->m, c->topo, c->xs, c->orig, c->sorted_of, add, out_sum, out_bond, c->st, &c->launches);
+    launch_bonded(c->m, c->topo, c->xs, c->xl, c->orig, c->sorted_of, add, out_sum, out_bond, c->st, &c->launches);
     CK(cudaGetLastError());
     return 0;
 }
@@ -242,7 +242,7 @@ static int run_update(jump_ctx *c, const Phase &p0, const float4 *g0, const Phas
     if (!g1) A.ph[1].use_grad = 0;
     A.do_aoa = aoa ? 1 : 0;
     A.half_dt = (float)(0.5 * c->dt); A.c1 = c->c1; A.c2 = c->c2; A.o_step = (unsigned)c->step;
-    A.xs = c->xs; A.xs_out = c->xs_nxt; A.vs = c->vs; A.mi = c->mi; A.lj = c->lj; A.orig = c->orig; A.x_build = c->x_build;
+    A.xs = c->xs; A.xs_out = c->xs_nxt; A.vs = c->vs; A.xl = c->xl; A.mi = c->mi; A.lj = c->lj; A.orig = c->orig; A.x_build = c->x_build;
     A.rowM = c->rows[ROW_M]; A.rowL = c->rows[ROW_L]; A.rowV = c->rows[ROW_V];
     A.ctr = c->ctr; A.events = (c->p.flags & JUMP_F_EVENT_LOG) ? c->events : nullptr; A.event_cap = c->event_cap;
     bool jumps = (p0.kind == 2 || p1.kind == 2) && (coul_jumps(c) || lj_jumps(c));
@@ -366,7 +366,7 @@ extern "C" int jump_half(jump_ctx *c, double H_ps, int32_t with_accel, int64_t s
 
 // ---- life cycle ------------------------------------------------------------------------------------------
 static int load_state(jump_ctx *c, const float *d_mass, const float *d_charge, const float *d_sigma, const float *d_eps) {
-    launch_load(c->m, c->d_pos, c->d_vel, d_mass, d_charge, d_sigma, d_eps, c->kT, c->xs, c->vs, c->lj, c->mi, c->orig, c->st,
+    launch_load(c->m, c->d_pos, c->d_vel, d_mass, d_charge, d_sigma, d_eps, c->kT, c->xs, c->vs, c->xl, c->lj, c->mi, c->orig, c->st,
                 &c->launches);
     CK(cudaGetLastError());
     return 0;
@@ -418,7 +418,7 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     }
     // buffers
     if ((r = dalloc(c, &c->xs, n)) || (r = dalloc(c, &c->xs_nxt, n)) || (r = dalloc(c, &c->vs, n)) ||
-        (r = dalloc(c, &c->vs_nxt, n)) || (r = dalloc(c, &c->x_build, n)) || (r = dalloc(c, &c->lj, n)) ||
+        (r = dalloc(c, &c->vs_nxt, n)) || (r = dalloc(c, &c->xl, n)) || (r = dalloc(c, &c->xl_nxt, n)) || (r = dalloc(c, &c->x_build, n)) || (r = dalloc(c, &c->lj, n)) ||
         (r = dalloc(c, &c->lj_nxt, n)) || (r = dalloc(c, &c->mi, n)) || (r = dalloc(c, &c->mi_nxt, n)) ||
         (r = dalloc(c, &c->orig, n)) || (r = dalloc(c, &c->orig_nxt, n)) || (r = dalloc(c, &c->sorted_of, n)) ||
         (r = dalloc(c, &c->key, n)) || (r = dalloc(c, &c->tmp_orig, n)) || (r = dalloc(c, &c->tmp_src, n)) ||
@@ -662,7 +662,7 @@ extern "C" int jump_get_bounds(jump_ctx *c, double out[8]) {
 }
 extern "C" int jump_refresh(jump_ctx *c) {
     if (!c) return JUMP_E_ARG;
-    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->st, &c->launches);
+    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, c->st, &c->launches);
     CK(cudaGetLastError());
     int r = resort_and_build(c);
     if (r) return r;

@@ -87,21 +87,28 @@ __global__ void __launch_bounds__(256) k_pair(Model m, Row row, const float4 *__
 
 // Harmonic bonds k (r-r0)^2 and angles k (theta-theta0)^2 (R-2), one thread per atom over the terms
 // the atom takes part in; evaluated in fp64 (a few hundred flops per atom) because r - r0 cancels.
-__device__ inline double min_image_d(float xi, float xj, float L) {
-    double d = (double)xi - (double)xj, Ld = (double)L;
+__device__ inline double min_image_d(double xi, double xj, float L) {
+    double d = xi - xj, Ld = (double)L;
     return d - Ld * rint(d / Ld);
 }
 
-__global__ void k_bonded(Model m, Topo t, const float4 *__restrict__ xs, const int *__restrict__ orig,
+struct D3 { double x, y, z; };
+__device__ inline D3 full_pos(const float4 *__restrict__ xs, const float4 *__restrict__ xl, int i) {
+    float4 a = xs[i], b = xl[i];  // x = hi + lo (the A steps integrate in fp64, see update.cu)
+    return D3{(double)a.x + (double)b.x, (double)a.y + (double)b.y, (double)a.z + (double)b.z};
+}
+
+__global__ void k_bonded(Model m, Topo t, const float4 *__restrict__ xs, const float4 *__restrict__ xl,
+                         const int *__restrict__ orig,
                          const int *__restrict__ sorted_of, const float4 *__restrict__ add,
                          float4 *__restrict__ out_sum, float4 *__restrict__ out_bond) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
     const int o = orig[i];
-    const float4 xi = xs[i];
+    const D3 xi = full_pos(xs, xl, i);
     double gx = 0., gy = 0., gz = 0., en = 0.;
     for (int b = t.bptr[o]; b < t.bptr[o + 1]; ++b) {
-        float4 xj = xs[sorted_of[t.bother[b]]];
+        D3 xj = full_pos(xs, xl, sorted_of[t.bother[b]]);
         double dx = min_image_d(xi.x, xj.x, m.box[0]);
         double dy = min_image_d(xi.y, xj.y, m.box[1]);
         double dz = min_image_d(xi.z, xj.z, m.box[2]);
@@ -113,10 +120,10 @@ __global__ void k_bonded(Model m, Topo t, const float4 *__restrict__ xs, const i
     for (int a = t.aptr[o]; a < t.aptr[o + 1]; ++a) {
         // role 1: I am the vertex, (aa, ab) are the ends; else I am an end, aa = vertex, ab = other end
         const int role = t.arole[a];
-        float4 xa = xs[sorted_of[t.aa[a]]], xb = xs[sorted_of[t.ab[a]]];
-        float4 xv = role == 1 ? xi : xa;             // vertex
-        float4 xe1 = role == 1 ? xa : xi;            // end whose gradient is "gi"
-        float4 xe2 = xb;                             // other end
+        D3 xa = full_pos(xs, xl, sorted_of[t.aa[a]]), xb = full_pos(xs, xl, sorted_of[t.ab[a]]);
+        D3 xv = role == 1 ? xi : xa;             // vertex
+        D3 xe1 = role == 1 ? xa : xi;            // end whose gradient is "gi"
+        D3 xe2 = xb;                             // other end
         double u[3], w[3];
         u[0] = min_image_d(xe1.x, xv.x, m.box[0]);
         u[1] = min_image_d(xe1.y, xv.y, m.box[1]);
@@ -179,10 +186,10 @@ int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *x
     return -1;
 }
 
-void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const int *orig, const int *sorted_of,
+void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig, const int *sorted_of,
                    const float4 *add, float4 *out_sum, float4 *out_bond, cudaStream_t st, int64_t *launches) {
     const int B = 128;
-    k_bonded<<<(m.n + B - 1) / B, B, 0, st>>>(m, t, xs, orig, sorted_of, add, out_sum, out_bond);
+    k_bonded<<<(m.n + B - 1) / B, B, 0, st>>>(m, t, xs, xl, orig, sorted_of, add, out_sum, out_bond);
     *launches += 1;
 }
 

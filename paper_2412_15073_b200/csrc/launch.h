@@ -7,10 +7,10 @@ namespace jb {
 struct SortArgs {
     int n;
     SortGrid grid;
-    const float4 *xs_in, *vs_in;
+    const float4 *xs_in, *vs_in, *xl_in;
     const float2 *lj_in, *mi_in;
     const int *orig_in;
-    float4 *xs, *vs, *x_build;
+    float4 *xs, *vs, *xl, *x_build;
     float2 *lj, *mi;
     int *orig, *sorted_of;
     int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src;
@@ -26,6 +26,7 @@ struct UpdateArgs {
     const float4 *xs;
     float4 *xs_out;
     float4 *vs;
+    float4 *xl;  // position residuals: x = xs + xl (updated in place)
     const float2 *mi, *lj;
     const int *orig;
     const float4 *x_build;
@@ -41,17 +42,17 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
                        const int *excl_idx, Counters *ctr, cudaStream_t st, int64_t *launches);
 int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *xs, const float2 *lj, float4 *out,
                 int accumulate, bool energy, cudaStream_t st, int64_t *launches);
-void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const int *orig, const int *sorted_of,
+void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig, const int *sorted_of,
                    const float4 *add, float4 *out_sum, float4 *out_bond, cudaStream_t st, int64_t *launches);
 void launch_unsort3(int n, const float4 *f, const int *orig, float *out, cudaStream_t st, int64_t *launches);
 void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st, int64_t *launches);
 void launch_writeback(int n, const float4 *xs, const float4 *vs, const int *orig, float *pos, float *vel, cudaStream_t st,
                       int64_t *launches);
 void launch_load(const Model &m, const float *pos, const float *vel, const float *mass, const float *charge,
-                 const float *sigma, const float *eps, double kT, float4 *xs, float4 *vs, float2 *lj, float2 *mi, int *orig,
+                 const float *sigma, const float *eps, double kT, float4 *xs, float4 *vs, float4 *xl, float2 *lj, float2 *mi, int *orig,
                  cudaStream_t st, int64_t *launches);
 void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
-                   cudaStream_t st, int64_t *launches);
+                   float4 *xl, cudaStream_t st, int64_t *launches);
 void launch_kinetic(int n, const float4 *vs, const float2 *mi, double *out, cudaStream_t st, int64_t *launches);
 
 }  // namespace jb

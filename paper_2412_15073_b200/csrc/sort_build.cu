@@ -88,6 +88,7 @@ __global__ void k_cell_sort(int ncell, const int *__restrict__ cell_start, int *
 
 __global__ void k_permute(int n, const int *__restrict__ src, const int *__restrict__ new_orig,
                           const float4 *__restrict__ xs_in, const float4 *__restrict__ vs_in,
+                          const float4 *__restrict__ xl_in, float4 *__restrict__ xl,
                           const float2 *__restrict__ lj_in, const float2 *__restrict__ mi_in,
                           float4 *__restrict__ xs, float4 *__restrict__ vs, float2 *__restrict__ lj,
                           float2 *__restrict__ mi, int *__restrict__ orig, int *__restrict__ sorted_of,
@@ -99,6 +100,7 @@ __global__ void k_permute(int n, const int *__restrict__ src, const int *__restr
     xs[i] = x;
     x_build[i] = x;
     vs[i] = vs_in[s];
+    xl[i] = xl_in[s];
     lj[i] = lj_in[s];
     mi[i] = mi_in[s];
     int o = new_orig[i];
@@ -242,7 +244,7 @@ void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches) {
     k_scan<<<1, 1024, 0, st>>>(a.grid.ncell, a.cell_count, a.cell_start);
     k_scatter<<<nblk(a.n, B), B, 0, st>>>(a.n, a.key, a.orig_in, a.cell_start, a.cell_fill, a.tmp_orig, a.tmp_src);
     k_cell_sort<<<nblk(a.grid.ncell, B), B, 0, st>>>(a.grid.ncell, a.cell_start, a.tmp_orig, a.tmp_src);
-    k_permute<<<nblk(a.n, B), B, 0, st>>>(a.n, a.tmp_src, a.tmp_orig, a.xs_in, a.vs_in, a.lj_in, a.mi_in, a.xs, a.vs,
+    k_permute<<<nblk(a.n, B), B, 0, st>>>(a.n, a.tmp_src, a.tmp_orig, a.xs_in, a.vs_in, a.xl_in, a.xl, a.lj_in, a.mi_in, a.xs, a.vs,
                                           a.lj, a.mi, a.orig, a.sorted_of, a.x_build);
     *launches += 5;
 }

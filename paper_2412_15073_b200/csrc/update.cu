@@ -225,6 +225,13 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, int i, unsigned ato
     }
 }
 
+__device__ inline double wrap1d(double x, double L) {
+    x -= L * floor(x / L);
+    if (x >= L) x -= L;
+    if (x < 0.0) x = 0.0;
+    return x;
+}
+
 // ---- the fused per-atom update: up to two velocity half-phases, then A O A + wrap ----------------------------
 template <bool JUMPS>
 __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
@@ -260,9 +267,14 @@ __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
             }
         }
         if (A.do_aoa) {
-            float x = xi.x, y = xi.y, z = xi.z;
-            x += A.half_dt * vx; y += A.half_dt * vy; z += A.half_dt * vz;  // A
-            uint32_t w[4];                                                  // O
+            // positions are integrated in fp64 as hi + lo (hi = the fp32 value every pair kernel reads):
+            // fp32 rounding of x (ulp(18 A) = 2e-6 A) through the stiff O-H bonds is otherwise the
+            // largest noise source of the whole step
+            const float4 xlo = A.xl[i];
+            double X = (double)xi.x + (double)xlo.x, Y = (double)xi.y + (double)xlo.y, Z = (double)xi.z + (double)xlo.z;
+            const double hdt = (double)A.half_dt;
+            X += hdt * (double)vx; Y += hdt * (double)vy; Z += hdt * (double)vz;  // A
+            uint32_t w[4];                                                          // O
             philox4x32_10(atom, A.o_step, 0u, 0u, m.key0, m.key1, w);
             float r1 = sqrtf(-2.f * logf(u01(w[0]))), r2 = sqrtf(-2.f * logf(u01(w[2])));
             float s1, c1, c2;
@@ -272,11 +284,11 @@ __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
             vx = A.c1 * vx + sc * (r1 * c1);
             vy = A.c1 * vy + sc * (r1 * s1);
             vz = A.c1 * vz + sc * (r2 * c2);
-            x += A.half_dt * vx; y += A.half_dt * vy; z += A.half_dt * vz;  // A
-            x = wrap1(x, m.box[0], m.inv_box[0]);
-            y = wrap1(y, m.box[1], m.inv_box[1]);
-            z = wrap1(z, m.box[2], m.inv_box[2]);
+            X += hdt * (double)vx; Y += hdt * (double)vy; Z += hdt * (double)vz;  // A
+            X = wrap1d(X, (double)m.box[0]); Y = wrap1d(Y, (double)m.box[1]); Z = wrap1d(Z, (double)m.box[2]);
+            const float x = (float)X, y = (float)Y, z = (float)Z;
             A.xs_out[i] = make_float4(x, y, z, xi.w);
+            A.xl[i] = make_float4((float)(X - (double)x), (float)(Y - (double)y), (float)(Z - (double)z), 0.f);
             float4 xb = A.x_build[i];
             float ddx = min_image1(x, xb.x, m.box[0], m.inv_box[0]);
             float ddy = min_image1(y, xb.y, m.box[1], m.inv_box[1]);
@@ -330,7 +342,8 @@ __global__ void k_writeback(int n, const float4 *__restrict__ xs, const float4 *
 __global__ void k_load(Model m, const float *__restrict__ pos, const float *__restrict__ vel,
                        const float *__restrict__ mass, const float *__restrict__ charge,
                        const float *__restrict__ sigma, const float *__restrict__ eps, double kT, float4 *__restrict__ xs,
-                       float4 *__restrict__ vs, float2 *__restrict__ lj, float2 *__restrict__ mi, int *__restrict__ orig) {
+                       float4 *__restrict__ vs, float4 *__restrict__ xl, float2 *__restrict__ lj, float2 *__restrict__ mi,
+                       int *__restrict__ orig) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
     float x = wrap1(pos[3 * i], m.box[0], m.inv_box[0]);
@@ -338,6 +351,7 @@ __global__ void k_load(Model m, const float *__restrict__ pos, const float *__re
     float z = wrap1(pos[3 * i + 2], m.box[2], m.inv_box[2]);
     xs[i] = make_float4(x, y, z, charge[i]);
     vs[i] = make_float4(vel[3 * i], vel[3 * i + 1], vel[3 * i + 2], 0.f);
+    xl[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     float e = eps[i];
     lj[i] = make_float2(e > 0.f ? (float)sqrt((double)sigma[i]) : 0.f, e > 0.f ? (float)(2.0 * sqrt((double)e)) : 0.f);
     double md = (double)mass[i];
@@ -347,7 +361,8 @@ __global__ void k_load(Model m, const float *__restrict__ pos, const float *__re
 
 // re-read the caller's positions (wrapped) and velocities into the current sorted order
 __global__ void k_reload(Model m, const float *__restrict__ pos, const float *__restrict__ vel,
-                         const int *__restrict__ orig, float4 *__restrict__ xs, float4 *__restrict__ vs) {
+                         const int *__restrict__ orig, float4 *__restrict__ xs, float4 *__restrict__ vs,
+                         float4 *__restrict__ xl) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
     int o = orig[i];
@@ -356,6 +371,7 @@ __global__ void k_reload(Model m, const float *__restrict__ pos, const float *__
     x.y = wrap1(pos[3 * o + 1], m.box[1], m.inv_box[1]);
     x.z = wrap1(pos[3 * o + 2], m.box[2], m.inv_box[2]);
     xs[i] = x;
+    xl[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     vs[i] = make_float4(vel[3 * o], vel[3 * o + 1], vel[3 * o + 2], 0.f);
 }
 
@@ -380,14 +396,14 @@ void launch_writeback(int n, const float4 *xs, const float4 *vs, const int *orig
     *launches += 1;
 }
 void launch_load(const Model &m, const float *pos, const float *vel, const float *mass, const float *charge,
-                 const float *sigma, const float *eps, double kT, float4 *xs, float4 *vs, float2 *lj, float2 *mi, int *orig,
-                 cudaStream_t st, int64_t *launches) {
-    k_load<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, mass, charge, sigma, eps, kT, xs, vs, lj, mi, orig);
+                 const float *sigma, const float *eps, double kT, float4 *xs, float4 *vs, float4 *xl, float2 *lj, float2 *mi,
+                 int *orig, cudaStream_t st, int64_t *launches) {
+    k_load<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, mass, charge, sigma, eps, kT, xs, vs, xl, lj, mi, orig);
     *launches += 1;
 }
 void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
-                   cudaStream_t st, int64_t *launches) {
-    k_reload<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, orig, xs, vs);
+                   float4 *xl, cudaStream_t st, int64_t *launches) {
+    k_reload<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, orig, xs, vs, xl);
     *launches += 1;
 }
 void launch_kinetic(int n, const float4 *vs, const float2 *mi, double *out, cudaStream_t st, int64_t *launches) {
