@@ -1,0 +1,316 @@
+"""bench.py -- throughput of the JUMP hot path on B200 (one JSON line on stdout).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl reference]
+
+A "step" is one jump_step(1): the whole hot path (jump half-phases C'J', A-O-A, list rebuild at its natural
+period, F0 = bonded + short-range pairs, jump half-phases J'C') over one synthetic water box.  Workload:
+BASELINE.json configs[1] (12 000 atoms, 49.3 A, cutoffs 6 / 12 A, dt 1 fs), equilibrated by 2 000 BAOAB steps
+(untimed).  Metric: ns/day (higher is better); atom-steps/s, same-GPU BAOAB with the unsplit 12 A force,
+the kernel roofline and the fp64 oracle on the host cores ride along in the same line.
+N > 1: the path does not shard on one GPU's box sizes (replicas only), so every rank
+runs an independent replica with its own seed; value = sum over ranks / max-over-ranks time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+BLOCK = 10                 # steps per timed block = nlist_every, so every block holds exactly one rebuild
+FLOPS_PER_PAIR = 2 * 50    # ~50 FP32-pipe instructions per in-range half pair, counted as FMAs
+L2_FLUSH_BYTES = 256 << 20
+
+
+def ns_per_day(steps_per_s, dt_fs):
+    return 86400.0 * steps_per_s * dt_fs * 1e-6
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md, clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=d.get("hbm_gbs", 6650.0), sm_max_mhz=d.get("sm_max_mhz", 1965.0), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def run_reference(args):
+    """--impl reference: the fp64 oracle, as it stands, on the host cores (same config, metric and unit)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import jump_oracle as jo
+    from paper_2412_15073_b200 import workloads as wl
+    sysd, run = wl.make_config(args.config)
+    o = jo.Oracle(sysd, **run)
+    o.jump_step(max(args.warmup, 1))
+    t0 = time.perf_counter()
+    o.jump_step(args.steps)
+    dt = time.perf_counter() - t0
+    sps = args.steps / dt
+    val = ns_per_day(sps, run["dt_fs"])
+    cores = jo.num_threads()
+    line = {"impl": "reference", "metric": "ns_per_day_jump", "value": val, "unit": "ns/day", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "BASELINE configs[%d]: %d-atom flexible water box, lattice start (not equilibrated)"
+                                   % (args.config, sysd["n_atoms"])},
+            "atom_steps_per_s": sps * sysd["n_atoms"],
+            "cpu_baseline": {"value": val, "unit": "ns/day", "cores": cores, "kind": "oracle",
+                             "sample": "%d whole-box JUMP steps" % args.steps},
+            "e2e": {"value": val, "unit": "ns/day", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def _dist_setup(n_gpus):
+    """One process per GPU (torchrun env).  Returns (rank, world, dist or None)."""
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world == 1:
+        return 0, 1, None
+    import torch.distributed as dist
+    os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+    dist.init_process_group("nccl")
+    return rank, world, dist
+
+
+def run_cpu_baseline(sysd, run, budget_s=15.0):
+    """The fp64 oracle as it stands on the host cores: whole-box JUMP steps of the same workload until ~budget_s."""
+    from oracle import jump_oracle as jo
+    o = jo.Oracle(sysd, **run)
+    o.jump_step(1)
+    t0 = time.perf_counter()
+    n = 0
+    while True:
+        o.jump_step(1)
+        n += 1
+        dt = time.perf_counter() - t0
+        if dt > budget_s or n >= 200:
+            break
+    o.close()
+    sps = n / dt
+    return {"value": ns_per_day(sps, run["dt_fs"]), "unit": "ns/day", "cores": jo.num_threads(), "kind": "oracle",
+            "sample": "%d whole-box JUMP steps of the same %d-atom box (%.1f s)" % (n, sysd["n_atoms"], dt),
+            "atom_steps_per_s": sps * sysd["n_atoms"]}
+
+
+def timed_blocks(torch, sim, stream, call, n_steps, block, flush):
+    """Time n_steps as ceil(n_steps/block) API calls; CUDA events on the context's stream bracket each call, the L2
+    flush (a 256 MiB write) sits between the brackets.  Returns total milliseconds of the bracketed regions."""
+    evs = []
+    left = n_steps
+    with torch.cuda.stream(stream):
+        while left > 0:
+            b = min(block, left)
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            call(b)
+            e1.record(stream)
+            evs.append((e0, e1))
+            left -= b
+    stream.synchronize()
+    return sum(a.elapsed_time(b) for a, b in evs)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=200)
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--impl", default="b200")
+    ap.add_argument("--equil", type=int, default=2000, help="untimed BAOAB equilibration steps from the lattice start")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", default="jump", choices=["jump", "respa"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2412_15073_b200 import binding as jb, workloads as wl, replicas
+    rank, world, dist = _dist_setup(args.gpus)
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dev = torch.device("cuda", local)
+    torch.cuda.set_device(dev)
+    props = torch.cuda.get_device_properties(dev)
+    peaks = measured_peaks()
+
+    sysd, run = wl.make_config(args.config)
+    run = dict(run, seed=replicas.rank_seed(run["seed"], rank))       # independent replicas
+    n, dt_fs = sysd["n_atoms"], run["dt_fs"]
+    stream = torch.cuda.Stream(dev)
+    flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
+    with torch.cuda.stream(stream):
+        sim = jb.JumpSim(sysd, device=dev, stream=stream, **run)
+        sim.baoab_step(args.equil)
+        sim.sync()
+        sim.reset_stats()
+        respa = args.mode == "respa"
+        per_call = run["n_inner"] if respa else 1                      # MD steps of length dt per API unit
+        step_call = (lambda b: sim.jump_respa_step(b // per_call)) if respa else sim.jump_step
+        block = BLOCK
+        K = max(args.steps // per_call * per_call, per_call)
+        W = max(args.warmup, 3)
+        step_call(max(W // per_call * per_call, per_call))
+        sim.sync()
+
+    # ---- timed region: K steps, device time, max over ranks --------------------------------------------------
+    sampler = ClockSampler(local)
+    sampler.start()
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize(dev)
+    l0 = sim.launches
+    wall0 = time.perf_counter()
+    ms = timed_blocks(torch, sim, stream, step_call, K, block, flush)
+    torch.cuda.synchronize(dev)
+    wall = time.perf_counter() - wall0
+    if dist is not None:
+        dist.barrier()
+    launches = sim.launches - l0
+    clocks = sampler.stop()
+    sim.sync()
+    ms_max = replicas.max_over_ranks(ms, dist, dev)
+    stats = sim.stats()
+
+    # ---- per-kernel times of the same K steps (CUDA events on the launch stream, separate pass) --------------
+    with torch.cuda.stream(stream):
+        sim.set_profiling(True)
+        timed_blocks(torch, sim, stream, step_call, K, block, flush)
+        prof = sim.profile()
+        sim.set_profiling(False)
+        n_pairs_ordered = sim.count_pairs(0, run["r_short"])           # ordered in-range entries of the short row
+    tot_prof = sum(v[0] for v in prof.values())
+    pair_ms, pair_launches = prof["pair"]
+    clk_mhz = clocks["sm_mhz"] or peaks["sm_max_mhz"]
+    peak_tflops = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    half_pairs = n_pairs_ordered / 2.0
+    pair_flops = half_pairs * FLOPS_PER_PAIR
+    pair_avg_ms = pair_ms / max(pair_launches, 1)
+    achieved = pair_flops / (pair_avg_ms * 1e-3) / 1e12 if pair_avg_ms > 0 else 0.0
+    roofline = {"kernel": "k_pair (short-range switched pair gradient, a5)", "bound": "alu", "achieved": achieved,
+                "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
+                "peak_source": "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (%s sm_max_mhz)" % (
+                    props.multi_processor_count, peaks["sm_max_mhz"], peaks["source"]),
+                "algorithmic": "%.0f in-range half pairs x %d flop" % (half_pairs, FLOPS_PER_PAIR),
+                "avg_launch_us": 1e3 * pair_avg_ms, "share_of_step": pair_ms / tot_prof if tot_prof else None,
+                "kernel_ms_share": {k: v[0] / tot_prof for k, v in prof.items()} if tot_prof else None}
+
+    # ---- same-GPU BAOAB with the unsplit r_long force (reported baseline) -------------------------------------
+    with torch.cuda.stream(stream):
+        sim.baoab_step(50)
+        sim.sync()
+        Kb = min(K, 500)
+        ms_b = timed_blocks(torch, sim, stream, sim.baoab_step, Kb, block, flush)
+    baoab = {"ns_per_day": ns_per_day(Kb / (ms_b * 1e-3), dt_fs), "ms_per_step": ms_b / Kb, "steps": Kb,
+             "force": "unsplit pair force to r_long = %.0f A" % run["r_long"]}
+
+    # ---- end to end through the public API with HOST buffers -------------------------------------------------
+    with torch.cuda.stream(stream):
+        Ke = min(K, 500)
+        hp = sim.pos.detach().cpu().pin_memory()
+        hv = sim.vel.detach().cpu().pin_memory()
+        sim.run_host(hp, hv, block, mode=args.mode)                      # warm-up
+        stream.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        calls = 0
+        for _ in range(max(Ke // block, 1)):
+            sim.run_host(hp, hv, block, mode=args.mode)
+            calls += 1
+        e1.record(stream)
+        stream.synchronize()
+        ms_e = e0.elapsed_time(e1)
+    ms_e_max = replicas.max_over_ranks(ms_e, dist, dev)
+    e2e_steps = calls * block
+    bytes_each_way = 2 * n * 3 * 4
+    e2e = {"value": world * ns_per_day(e2e_steps / (ms_e_max * 1e-3), dt_fs), "unit": "ns/day",
+           "h2d_bytes_per_step": bytes_each_way / block, "d2h_bytes_per_step": bytes_each_way / block,
+           "call": "JumpSim.run_host: pinned host (x, v) -> device, jump_refresh, %d steps, device -> host, per call" % block}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = run_cpu_baseline(sysd, run)
+
+    if rank == 0:
+        sps = K / (ms_max * 1e-3)
+        value = world * ns_per_day(sps, dt_fs)
+        line = {"metric": "ns_per_day_jump" if not respa else "ns_per_day_jump_respa", "value": value, "unit": "ns/day",
+                "n_gpus": world, "steps": K, "warmup": W, "ms_per_step": ms_max / K, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "BASELINE configs[%d]: %d-atom flexible water box %.1f A, r_c %.0f / r_long %.0f A, "
+                                       "dt %.0f fs, %s, equilibrated by %d BAOAB steps"
+                                       % (args.config, n, sysd["box"], run["r_short"], run["r_long"], dt_fs,
+                                          "JUMP-RESPA n_inner %d" % run["n_inner"] if respa else "JUMP (C'J'AOAJ'C')", args.equil),
+                           "eps_jump": run["eps_jump"], "r_mid": run["r_mid"], "skin": run["skin"],
+                           "nlist_every": run["nlist_every"], "steps_per_api_call": block,
+                           "l2": "flushed by a 256 MiB write between timed API calls (outside the event brackets)",
+                           "parallelism": "independent replicas x%d" % world},
+                "atom_steps_per_s": world * sps * n,
+                "clocks": clocks, "gpu_launches": launches, "wall_s": wall,
+                "e2e": e2e, "roofline": roofline, "baoab_same_gpu": baoab,
+                "jump_vs_baoab": (K / ms_max) / (Kb / ms_b),
+                "events": {"proposals_per_atom_step": stats["proposals"] / (n * (K + W)) if K + W else None,
+                           "accepts_per_atom_step": stats["accepts"] / (n * (K + W)), "max_p": stats["max_p"],
+                           "error": stats["error"]}}
+        if cpu is not None:
+            line["cpu_baseline"] = cpu
+        print(json.dumps(line))
+    sim.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

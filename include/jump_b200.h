@@ -125,6 +125,15 @@ int jump_sync(jump_ctx *c);
 int64_t jump_get_step(const jump_ctx *c);
 /* Number of kernels this context launched so far (bench.py's gpu_launches). */
 int64_t jump_get_launches(const jump_ctx *c);
+/* Measurement (bench.py): with profiling on, every kernel group is bracketed by CUDA events on the context's
+ * stream; jump_get_profile waits for the stream and returns the summed milliseconds and the number of bracketed
+ * launches (groups) per category: 0 pair-force kernels, 1 bonded, 2 update (jump chains + integrator),
+ * 3 sort + row build.  Turning profiling on or off resets the sums. */
+int jump_set_profiling(jump_ctx *c, int32_t on);
+int jump_get_profile(jump_ctx *c, double ms[4], int64_t count[4]);
+/* Ordered entries of row which_row (0 short .. 5) whose current distance is below r_cut: the number of pair
+ * terms one pair-force launch over that row evaluates (each unordered pair counts twice). */
+int jump_count_pairs(jump_ctx *c, int32_t which_row, double r_cut, int64_t *n_ordered);
 const char *jump_last_error(const jump_ctx *c);
 void jump_free(jump_ctx *c);
 

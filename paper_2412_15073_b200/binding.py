@@ -20,7 +20,7 @@ ERRORS = {-1: "bad argument", -2: "CUDA error", -3: "row/event overflow", -4: "t
 EXPORTS = ["jump_init", "jump_step", "baoab_step", "jump_respa_step", "jump_get_forces", "jump_get_energy",
            "jump_get_stats", "jump_reset_stats", "jump_get_events", "jump_clear_events", "jump_get_row",
            "jump_get_bounds", "jump_refresh", "jump_half", "jump_sync", "jump_get_step", "jump_get_launches",
-           "jump_last_error", "jump_free"]
+           "jump_last_error", "jump_free", "jump_set_profiling", "jump_get_profile", "jump_count_pairs"]
 
 
 class jump_params(C.Structure):
@@ -92,6 +92,9 @@ def lib():
         L.jump_last_error.restype = C.c_char_p
         L.jump_free.argtypes = [vp]
         L.jump_free.restype = None
+        L.jump_set_profiling.argtypes = [vp, i32]
+        L.jump_get_profile.argtypes = [vp, dp, C.POINTER(i64)]
+        L.jump_count_pairs.argtypes = [vp, i32, C.c_double, C.POINTER(i64)]
         _lib = L
     return _lib
 
@@ -184,6 +187,27 @@ class JumpSim:
     def refresh(self):
         self._check(self._L.jump_refresh(self._h), "jump_refresh")
 
+    def run_host(self, host_pos, host_vel, n_steps, mode="jump"):
+        """End-to-end call with HOST state: copy (x, v) from the (pinned) host tensors to the device, re-sort and
+        rebuild the rows at those positions, run n_steps (mode "jump": jump_step; "respa": jump_respa_step with
+        n_steps / n_inner outer steps; "baoab": baoab_step) and copy (x, v) back into the same host tensors.
+        Everything is enqueued on the context's stream; the caller synchronises it."""
+        torch = self._torch
+        with torch.cuda.stream(self.stream):
+            self.pos.copy_(host_pos, non_blocking=True)
+            self.vel.copy_(host_vel, non_blocking=True)
+            self.refresh()
+            if mode == "jump":
+                self.jump_step(n_steps)
+            elif mode == "respa":
+                self.jump_respa_step(max(int(n_steps) // int(self.params.n_inner), 1))
+            elif mode == "baoab":
+                self.baoab_step(n_steps)
+            else:
+                raise ValueError(mode)
+            host_pos.copy_(self.pos, non_blocking=True)
+            host_vel.copy_(self.vel, non_blocking=True)
+
     # ---- observers -----------------------------------------------------------------------------------
     def forces(self, which=0):
         out = self._torch.empty((self.n, 3), dtype=self._torch.float32, device=self.device)
@@ -231,6 +255,20 @@ class JumpSim:
         out = (C.c_double * 8)()
         self._check(self._L.jump_get_bounds(self._h, out), "jump_get_bounds")
         return dict(zip(["GM", "GL", "GV", "qmax", "eps_max", "sig_min", "sig_max", "rM"], list(out)))
+
+    def set_profiling(self, on=True):
+        self._check(self._L.jump_set_profiling(self._h, int(bool(on))), "jump_set_profiling")
+
+    def profile(self):
+        """{category: (milliseconds, bracketed launches)} since profiling was switched on."""
+        ms, cnt = (C.c_double * 4)(), (C.c_int64 * 4)()
+        self._check(self._L.jump_get_profile(self._h, ms, cnt), "jump_get_profile")
+        return {k: (ms[i], cnt[i]) for i, k in enumerate(("pair", "bonded", "update", "build"))}
+
+    def count_pairs(self, which_row, r_cut):
+        n = C.c_int64()
+        self._check(self._L.jump_count_pairs(self._h, int(which_row), float(r_cut), C.byref(n)), "jump_count_pairs")
+        return int(n.value)
 
     @property
     def step(self):

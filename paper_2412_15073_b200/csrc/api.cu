@@ -40,7 +40,37 @@ struct jump_ctx {
     int64_t step, outer, rebuilds, launches;
     int sticky;
     std::string err;
+    // optional per-category kernel timing with CUDA events on the launch stream (bench.py's roofline leg)
+    bool prof;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_pend[4], prof_free;
+    double prof_ms[4];
+    int64_t prof_n[4];
 };
+enum { PROF_PAIR = 0, PROF_BONDED = 1, PROF_UPDATE = 2, PROF_BUILD = 3 };
+
+static void prof_begin(jump_ctx *c, int cat) {
+    if (!c->prof) return;
+    std::pair<cudaEvent_t, cudaEvent_t> ev;
+    if (!c->prof_free.empty()) { ev = c->prof_free.back(); c->prof_free.pop_back(); }
+    else { cudaEventCreate(&ev.first); cudaEventCreate(&ev.second); }
+    cudaEventRecord(ev.first, c->st);
+    c->prof_pend[cat].push_back(ev);
+}
+static void prof_end(jump_ctx *c, int cat) {
+    if (!c->prof) return;
+    cudaEventRecord(c->prof_pend[cat].back().second, c->st);
+}
+static void prof_collect(jump_ctx *c) {
+    cudaStreamSynchronize(c->st);
+    for (int k = 0; k < 4; ++k) {
+        for (auto &ev : c->prof_pend[k]) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, ev.first, ev.second) == cudaSuccess) { c->prof_ms[k] += ms; c->prof_n[k]++; }
+            c->prof_free.push_back(ev);
+        }
+        c->prof_pend[k].clear();
+    }
+}
 
 #define CK(call)                                                                          \
     do {                                                                                  \
@@ -155,8 +185,10 @@ static int build_rows(jump_ctx *c, bool only_missing) {
         if (sel[k].enabled) { any = true; c->row_fresh[k] = true; }
     }
     if (!any) return 0;
+    prof_begin(c, PROF_BUILD);
     launch_build_rows(c->m, c->g, sel, (float)(c->p.r_long + c->p.skin), c->cell_start, c->xs, c->lj, c->orig,
                       c->sorted_of, c->excl_ptr, c->excl_idx, c->ctr, c->st, &c->launches);
+    prof_end(c, PROF_BUILD);
     CK(cudaGetLastError());
     return 0;
 }
@@ -169,7 +201,9 @@ static int resort_and_build(jump_ctx *c) {
     a.sorted_of = c->sorted_of; a.x_build = c->x_build;
     a.key = c->key; a.cell_count = c->cell_count; a.cell_fill = c->cell_fill; a.cell_start = c->cell_start;
     a.tmp_orig = c->tmp_orig; a.tmp_src = c->tmp_src; a.ctr = c->ctr;
+    prof_begin(c, PROF_BUILD);
     launch_sort(a, c->st, &c->launches);
+    prof_end(c, PROF_BUILD);
     CK(cudaGetLastError());
     std::swap(c->xs, c->xs_nxt); std::swap(c->vs, c->vs_nxt); std::swap(c->xl, c->xl_nxt); std::swap(c->lj, c->lj_nxt);
     std::swap(c->mi, c->mi_nxt); std::swap(c->orig, c->orig_nxt);
@@ -184,20 +218,27 @@ static int need_row(jump_ctx *c, int k) {  // lazily enabled rows (full list of 
     return build_rows(c, true);
 }
 
+static void pair(jump_ctx *c, int row, int wC, int wLJ, float4 *out, int accumulate, bool energy) {
+    prof_begin(c, PROF_PAIR);
+    launch_pair(c->m, c->rows[row], wC, wLJ, c->xs, c->lj, out, accumulate, energy, c->st, &c->launches);
+    prof_end(c, PROF_PAIR);
+}
 static bool lj_jumps(const jump_ctx *c) { return (c->p.flags & JUMP_F_LJ_JUMPS) != 0; }
 static bool coul_jumps(const jump_ctx *c) { return (c->p.flags & JUMP_F_COUL_JUMPS) != 0; }
 
 static int bonded(jump_ctx *c, const float4 *add, float4 *out_sum, float4 *out_bond) {
+    prof_begin(c, PROF_BONDED);
     launch_bonded(c->m, c->topo, c->xs, c->xl, c->orig, c->sorted_of, add, out_sum, out_bond, c->st, &c->launches);
+    prof_end(c, PROF_BONDED);
     CK(cudaGetLastError());
     return 0;
 }
 // F0 = bonded + short non-bonded (R-13: the LJ tail stays in F0 when LJ jumps are off)
 static int compute_short_nb(jump_ctx *c, float4 *out, bool energy = false) {
-    if (lj_jumps(c)) launch_pair(c->m, c->rows[ROW_S], W_SHORT, W_SHORT, c->xs, c->lj, out, 0, energy, c->st, &c->launches);
+    if (lj_jumps(c)) pair(c, ROW_S, W_SHORT, W_SHORT, out, 0, energy);
     else {
-        launch_pair(c->m, c->rows[ROW_S], W_SHORT, W_FULL, c->xs, c->lj, out, 0, energy, c->st, &c->launches);
-        launch_pair(c->m, c->rows[ROW_W], W_NONE, W_FULL, c->xs, c->lj, out, 1, energy, c->st, &c->launches);
+        pair(c, ROW_S, W_SHORT, W_FULL, out, 0, energy);
+        pair(c, ROW_W, W_NONE, W_FULL, out, 1, energy);
     }
     CK(cudaGetLastError());
     return 0;
@@ -209,15 +250,15 @@ static int compute_f0(jump_ctx *c) {
 }
 static int compute_long(jump_ctx *c, float4 *out) {
     int wLJ = lj_jumps(c) ? W_LONG : W_NONE;
-    launch_pair(c->m, c->rows[ROW_M], W_LONG, wLJ, c->xs, c->lj, out, 0, false, c->st, &c->launches);
-    launch_pair(c->m, c->rows[ROW_L], W_LONG, wLJ, c->xs, c->lj, out, 1, false, c->st, &c->launches);
+    pair(c, ROW_M, W_LONG, wLJ, out, 0, false);
+    pair(c, ROW_L, W_LONG, wLJ, out, 1, false);
     CK(cudaGetLastError());
     return 0;
 }
 static int compute_full(jump_ctx *c, float4 *out, bool energy = false) {  // unsplit to r_long + bonded
     int r = need_row(c, ROW_F);
     if (r) return r;
-    launch_pair(c->m, c->rows[ROW_F], W_FULL, W_FULL, c->xs, c->lj, c->ftmp2, 0, energy, c->st, &c->launches);
+    pair(c, ROW_F, W_FULL, W_FULL, c->ftmp2, 0, energy);
     CK(cudaGetLastError());
     return bonded(c, c->ftmp2, out, nullptr);
 }
@@ -246,7 +287,9 @@ static int run_update(jump_ctx *c, const Phase &p0, const float4 *g0, const Phas
     A.rowM = c->rows[ROW_M]; A.rowL = c->rows[ROW_L]; A.rowV = c->rows[ROW_V];
     A.ctr = c->ctr; A.events = (c->p.flags & JUMP_F_EVENT_LOG) ? c->events : nullptr; A.event_cap = c->event_cap;
     bool jumps = (p0.kind == 2 || p1.kind == 2) && (coul_jumps(c) || lj_jumps(c));
+    prof_begin(c, PROF_UPDATE);
     launch_update(c->m, A, jumps, c->st, &c->launches);
+    prof_end(c, PROF_UPDATE);
     CK(cudaGetLastError());
     if (aoa) {
         std::swap(c->xs, c->xs_nxt);
@@ -335,10 +378,9 @@ extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
                 r = compute_long(c, fl);
                 if (r) return r;
                 if (paper) {  // + short non-bonded
-                    launch_pair(c->m, c->rows[ROW_S], W_SHORT, lj_jumps(c) ? W_SHORT : W_FULL, c->xs, c->lj, fl, 1, false,
-                                c->st, &c->launches);
+                    pair(c, ROW_S, W_SHORT, lj_jumps(c) ? W_SHORT : W_FULL, fl, 1, false);
                     if (!lj_jumps(c))
-                        launch_pair(c->m, c->rows[ROW_W], W_NONE, W_FULL, c->xs, c->lj, fl, 1, false, c->st, &c->launches);
+                        pair(c, ROW_W, W_NONE, W_FULL, fl, 1, false);
                     CK(cudaGetLastError());
                 }
                 outer[half] = ph_kick(0.5 * D);
@@ -532,6 +574,8 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     c->d_pos = d_pos; c->d_vel = d_vel;
     c->step = c->outer = c->rebuilds = c->launches = 0;
     c->sticky = 0;
+    c->prof = false;
+    for (int k = 0; k < 4; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     int r = init_impl(c, p, d_mass, d_charge, d_lj_sigma, d_lj_eps, n_bonds, d_bond_ij, d_bond_k, d_bond_r0, n_angles,
                       d_angle_ijk, d_angle_k, d_angle_t0, d_excl_ptr, d_excl_idx);
     *out = c;  // returned even on failure so that jump_last_error can be read; free with jump_free
@@ -540,7 +584,8 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
 
 extern "C" void jump_free(jump_ctx *c) {
     if (!c) return;
-    cudaStreamSynchronize(c->st);
+    prof_collect(c);
+    for (auto &ev : c->prof_free) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
     for (void *q : c->owned) cudaFree(q);
     delete c;
 }
@@ -668,4 +713,32 @@ extern "C" int jump_refresh(jump_ctx *c) {
     if (r) return r;
     if ((r = compute_f0(c))) return r;
     return poll_error(c);
+}
+
+// ---- measurement helpers (bench.py) ------------------------------------------------------------------------
+extern "C" int jump_set_profiling(jump_ctx *c, int32_t on) {
+    if (!c) return JUMP_E_ARG;
+    prof_collect(c);
+    c->prof = on != 0;
+    for (int k = 0; k < 4; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
+    return 0;
+}
+extern "C" int jump_get_profile(jump_ctx *c, double ms[4], int64_t count[4]) {
+    if (!c || !ms || !count) return JUMP_E_ARG;
+    prof_collect(c);
+    for (int k = 0; k < 4; ++k) { ms[k] = c->prof_ms[k]; count[k] = c->prof_n[k]; }
+    return 0;
+}
+extern "C" int jump_count_pairs(jump_ctx *c, int32_t which_row, double r_cut, int64_t *n_ordered) {
+    if (!c || !n_ordered || which_row < 0 || which_row >= N_ROWS || !c->rows[which_row].enabled) return JUMP_E_ARG;
+    unsigned long long *d = nullptr;
+    int r = dalloc(c, &d, 1);
+    if (r) return r;
+    CK(cudaMemsetAsync(d, 0, sizeof(unsigned long long), c->st));
+    launch_count_pairs(c->m, c->rows[which_row], c->xs, (float)(r_cut * r_cut), d, c->st, &c->launches);
+    unsigned long long h = 0;
+    CK(cudaMemcpyAsync(&h, d, sizeof h, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    *n_ordered = (int64_t)h;
+    return 0;
 }

@@ -165,6 +165,31 @@ __global__ void k_unsort3(int n, const float4 *__restrict__ f, const int *__rest
     out[3 * o] = v.x; out[3 * o + 1] = v.y; out[3 * o + 2] = v.z;
 }
 
+// number of ordered row entries currently within r_cut (measurement: algorithmic pairs per launch)
+__global__ void k_count_pairs(Model m, Row row, const float4 *__restrict__ xs, float rc2, unsigned long long *out) {
+    int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (i >= m.n) return;
+    const float4 xi = xs[i];
+    const int cnt = row.cnt[i];
+    const int *__restrict__ ridx = row.idx + (size_t)i * row.cap;
+    unsigned c = 0;
+    for (int k = lane; k < cnt; k += 32) {
+        float4 xj = xs[ridx[k]];
+        float dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
+        float dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
+        float dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
+        c += (dx * dx + dy * dy + dz * dz < rc2) ? 1u : 0u;
+    }
+    c = __reduce_add_sync(0xffffffffu, c);
+    if (lane == 0 && c) atomicAdd(out, (unsigned long long)c);
+}
+void launch_count_pairs(const Model &m, const Row &row, const float4 *xs, float rc2, unsigned long long *out,
+                        cudaStream_t st, int64_t *launches) {
+    const int B = 256;
+    k_count_pairs<<<(unsigned)(((long long)m.n * 32 + B - 1) / B), B, 0, st>>>(m, row, xs, rc2, out);
+    *launches += 1;
+}
+
 template <int WC, int WLJ>
 static void pair_dispatch(const Model &m, const Row &row, const float4 *xs, const float2 *lj, float4 *out, int accumulate,
                           bool energy, cudaStream_t st) {

@@ -42,6 +42,8 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
                        const int *excl_idx, Counters *ctr, cudaStream_t st, int64_t *launches);
 int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *xs, const float2 *lj, float4 *out,
                 int accumulate, bool energy, cudaStream_t st, int64_t *launches);
+void launch_count_pairs(const Model &m, const Row &row, const float4 *xs, float rc2, unsigned long long *out,
+                        cudaStream_t st, int64_t *launches);
 void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig, const int *sorted_of,
                    const float4 *add, float4 *out_sum, float4 *out_bond, cudaStream_t st, int64_t *launches);
 void launch_unsort3(int n, const float4 *f, const int *orig, float *out, cudaStream_t st, int64_t *launches);

@@ -1,0 +1,335 @@
+"""Parity of the CUDA path (through the C ABI) against the fp64 oracle on the same seeded inputs.
+
+Tolerances (BASELINE.json north_star): per-atom force pieces <= 1e-5 relative
+(|dF_i| / max(|F_i|, F_rms)), trajectories <= 1e-4 A over 100 steps, integer fields of the event log
+bit-exact, T / p / G~ of each event to fp32 rounding.  Trajectory parity is asserted on the window
+before the oracle's first fragile decision (R-17).
+"""
+import numpy as np
+import pytest
+
+from paper_2412_15073_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+F_TOL = 1e-5
+X_TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def jb():
+    from paper_2412_15073_b200 import binding
+    binding.lib()          # fails loudly if the CUDA library is missing
+    return binding
+
+
+@pytest.fixture(scope="module")
+def jo():
+    from oracle import jump_oracle
+    return jump_oracle
+
+
+@pytest.fixture(scope="module")
+def cfg0():
+    return wl.make_config(0)
+
+
+def rel_force_err(fg, fo):
+    fg = np.asarray(fg, np.float64)
+    frms = np.sqrt((fo ** 2).sum(1).mean())
+    return float((np.linalg.norm(fg - fo, axis=1) / np.maximum(np.linalg.norm(fo, axis=1), frms)).max())
+
+
+def pos_err(g, o, box):
+    d = g.pos.cpu().numpy().astype(np.float64) - o.pos
+    d -= box * np.round(d / box)
+    return float(np.abs(d).max())
+
+
+def check_events(eg, eo):
+    assert len(eg) == len(eo)
+    for k in ("step", "stream", "atom", "iter", "ring", "j", "accepted", "n_gt"):
+        assert (eg[k] == eo[k]).all(), k
+    fin = np.isfinite(eo["T"])
+    assert (np.isfinite(eg["T"]) == fin).all()
+    if fin.any():
+        assert np.abs(eg["T"][fin] / eo["T"][fin] - 1).max() < 1e-3
+    if len(eo) == 0:
+        return
+    assert np.abs(eg["p"] - eo["p"]).max() < 1e-4
+    assert (eg["U"] == eo["U"].astype(np.float32)).all()       # uniforms are exact in fp32 (R-15)
+    assert np.abs(eg["gt"] - eo["gt"]).max() < 1e-3
+
+
+# ------------------------------------------------------------------------------------- rows, bounds
+def test_bounds_match(jb, jo, cfg0):
+    sysd, run = cfg0
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    bg, bo = g.bounds(), o.bounds()
+    for k in bo:
+        assert bg[k] == pytest.approx(bo[k], rel=1e-12, abs=1e-300), k
+
+
+@pytest.mark.parametrize("case", ["cfg0", "small5", "no_ring", "big_cells"])
+def test_rows_identical(jb, jo, cfg0, case):
+    """a1-a3: sort + row build.  Rows M, L, V must hold the same atoms in the same (canonical) order."""
+    if case == "cfg0":
+        sysd, run = cfg0
+    else:
+        sysd = wl.small_water(5, seed=11)                      # 375 atoms, box 22.4 A: ragged, several cells
+        run = dict(cfg0[1], r_short=4.0, r_long=8.0, r_mid=5.0, seed=5)
+        if case == "no_ring":
+            run["r_mid"] = 0.0
+        if case == "big_cells":
+            run["cell_edge"] = 6.1
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    nM, nL, nV = o.row_counts()
+    for i in range(g.n):
+        for which, cnt in ((1, nM), (2, nL), (3, nV)):
+            rg = g.row(which, i)
+            assert len(rg) == cnt[i]
+            if i % 5 == 0:
+                assert (rg == o.row(which - 1, i)).all()
+    st = g.stats()
+    assert st["error"] == 0 and all(m <= c for m, c in zip(st["max_row"], st["cap_row"]) if c)
+
+
+# ------------------------------------------------------------------------------------- forces
+@pytest.mark.parametrize("flags", [3, 1, 0])
+def test_force_pieces_cfg0(jb, jo, cfg0, flags):
+    """a4, a5, a10: F0, unsplit, long, bonded, short non-bonded; flags=1 keeps the LJ tail in F0 (R-13)."""
+    sysd, run = cfg0
+    run = dict(run, flags=flags)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    for which in range(5):
+        fo = o.forces(which)
+        err = rel_force_err(g.forces(which).cpu().numpy(), fo)
+        assert err <= F_TOL, (which, err)
+    ek, ep = g.energy()
+    assert ek == pytest.approx(o.kinetic(), rel=1e-6)
+    assert ep == pytest.approx(o.potential(1), rel=1e-5, abs=1e-3)
+
+
+def test_forces_after_dynamics_and_refresh(jb, jo, cfg0):
+    """Forces at a liquid-like (not lattice) geometry, fed in through jump_refresh."""
+    sysd, run = cfg0
+    o = jo.Oracle(sysd, **run)
+    o.baoab_step(300)
+    s2 = dict(sysd, pos=np.float32(o.pos).astype(np.float64), vel=np.float32(o.vel).astype(np.float64))
+    g, o2 = jb.JumpSim(sysd, **run), jo.Oracle(s2, **run)
+    import torch
+    g.pos.copy_(torch.as_tensor(np.float32(s2["pos"])))
+    g.vel.copy_(torch.as_tensor(np.float32(s2["vel"])))
+    g.refresh()
+    for which in range(5):
+        err = rel_force_err(g.forces(which).cpu().numpy(), o2.forces(which))
+        assert err <= F_TOL, (which, err)
+
+
+def test_forces_solute_config3(jb, jo):
+    """Heterogeneous charges and LJ parameters, chain exclusions (1-2, 1-3), 23 558 atoms."""
+    sysd, run = wl.make_config(3)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    for which in (0, 2, 3):
+        err = rel_force_err(g.forces(which).cpu().numpy(), o.forces(which))
+        assert err <= F_TOL, (which, err)
+    nM, nL, nV = o.row_counts()
+    for i in list(range(0, 2500, 97)) + list(range(2500, g.n, 1999)):
+        for which, cnt in ((1, nM), (2, nL), (3, nV)):
+            rg = g.row(which, i)
+            assert len(rg) == cnt[i] and (rg == o.row(which - 1, i)).all()
+
+
+# ------------------------------------------------------------------------------------- jump chains
+@pytest.mark.parametrize("eps", [1.0, 0.3, float("inf")])
+def test_event_log_and_trajectory_cfg0(jb, jo, cfg0, eps):
+    """a6-a8: every proposal of 10 JUMP steps (C', J', both halves) equals the oracle's; then the 100-step
+    trajectory stays within 1e-4 A on the window before the oracle's first fragile decision (R-17)."""
+    sysd, run = cfg0
+    run = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG, eps_jump=eps)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    g.jump_step(10); g.sync(); o.jump_step(10)
+    eg, eo = g.events(), o.events()
+    assert len(eo) > 15000
+    check_events(eg, eo)
+    assert set(np.unique(eo["stream"])) == {1, 2, 3, 4}
+    g.clear_events(); o.clear_events()
+    window = 10
+    for _ in range(9):
+        o.jump_step(10)
+        st = o.stats()
+        g.jump_step(10); g.sync()
+        if st["min_margin"] < 1e-6:       # a decision the fp32 path may legitimately take the other way
+            break
+        window += 10
+        assert pos_err(g, o, sysd["box"]) <= X_TOL
+        g.clear_events(); o.clear_events()
+    assert window >= 30
+    sg, so = g.stats(), o.stats()
+    assert sg["error"] == 0 and sg["max_p"] <= 1.0 + 1e-4 and sg["max_g_over_L"] <= 1.0 + 1e-4
+    if window == 100:
+        assert sg["proposals"] == so["proposals"] and sg["accepts"] == so["accepts"]
+        assert sg["gt_attempts"] == so["gt_attempts"] and sg["expiries"] == so["expiries"]
+
+
+def test_jump_half_statistics_frozen_x(jb, jo, cfg0):
+    """The C'/J' half-phase alone at frozen x, long duration (many events per atom), with and without drift."""
+    sysd, run = cfg0
+    run = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG)
+    for accel in (True, False):
+        g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+        g.jump_half(0.004, accel, step=7); g.sync(); o.jump_half(0.004, accel, step=7)
+        check_events(g.events(), o.events())
+        assert np.abs(g.vel.cpu().numpy() - o.vel).max() < 2e-3
+        assert (g.pos.cpu().numpy() == np.float32(o.pos)).all()     # x frozen
+
+
+def test_only_coulomb_jumps_and_only_lj_jumps(jb, jo, cfg0):
+    sysd, run = cfg0
+    for flags in (1, 2):
+        r = dict(run, flags=flags | jb.F_EVENT_LOG)
+        g, o = jb.JumpSim(sysd, **r), jo.Oracle(sysd, **r)
+        g.jump_step(5); g.sync(); o.jump_step(5)
+        check_events(g.events(), o.events())
+        assert pos_err(g, o, sysd["box"]) <= X_TOL
+
+
+# ------------------------------------------------------------------------------------- BAOAB, RESPA
+def test_baoab_trajectory_100_steps(jb, jo, cfg0):
+    sysd, run = cfg0
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    g.baoab_step(100); g.sync(); o.baoab_step(100)
+    assert g.step == 100 == o.step
+    assert pos_err(g, o, sysd["box"]) <= X_TOL
+    assert np.abs(g.vel.cpu().numpy() - o.vel).max() < 5e-3
+    assert rel_force_err(g.forces(0).cpu().numpy(), o.forces(0)) <= 20 * F_TOL    # forces at diverged-by-1e-5-A positions
+
+
+def test_baoab_energy_conservation_gamma0(jb, cfg0):
+    """gamma = 0, jumps off: BAOAB is velocity Verlet; the energy error is O(dt^2) and does not drift."""
+    sysd, run = cfg0
+    out = []
+    for dt in (0.5, 0.25):
+        g = jb.JumpSim(sysd, **dict(run, gamma_per_ps=0.0, dt_fs=dt, flags=0))
+        g.baoab_step(int(20 / dt))
+        e0 = sum(g.energy())
+        dev = []
+        for _ in range(10):
+            g.baoab_step(int(20 / dt))
+            dev.append(sum(g.energy()) - e0)
+        out.append(np.abs(dev).max())
+    assert out[0] < 0.02 * 648 * 0.6          # small against the thermal energy scale
+    assert out[1] < 0.5 * out[0]              # second order: quartered, allow 2x
+
+
+@pytest.mark.parametrize("flags", [3, 3 | 8, 3 | 16, 3 | 8 | 16, 1])
+def test_respa_variants(jb, jo, cfg0, flags):
+    """a9: JUMP-RESPA (BASELINE variant and the paper's variant) and the BAOAB-RESPA comparator (R-12)."""
+    sysd, run = cfg0
+    r = dict(run, flags=flags | jb.F_EVENT_LOG)
+    g, o = jb.JumpSim(sysd, **r), jo.Oracle(sysd, **r)
+    g.jump_respa_step(3); g.sync(); o.jump_respa_step(3)
+    assert g.step == 12 == o.step
+    eg, eo = g.events(), o.events()
+    if flags & 16:
+        assert len(eg) == 0 == len(eo)
+    else:
+        check_events(eg, eo)
+        assert set(np.unique(eo["stream"])) <= {5, 6, 7, 8} and len(eo) > 1000
+    assert pos_err(g, o, sysd["box"]) <= X_TOL
+    assert np.abs(g.vel.cpu().numpy() - o.vel).max() < 5e-3
+
+
+def test_degenerate_no_jumps_is_baoab_with_short_forces(jb, jo, cfg0):
+    """flags = 0: jump_step is BAOAB with F0 (C.6 'JUMP degenerate cases'); no events, no proposals."""
+    sysd, run = cfg0
+    r = dict(run, flags=0)
+    g, o = jb.JumpSim(sysd, **r), jo.Oracle(sysd, **r)
+    g.jump_step(50); g.sync(); o.jump_step(50)
+    assert pos_err(g, o, sysd["box"]) <= X_TOL
+    assert g.stats()["proposals"] == 0
+
+
+def test_determinism_bitwise(jb, cfg0):
+    """Same inputs and seed: same bits (counter-based RNG, no floating-point atomics, canonical rows)."""
+    sysd, run = cfg0
+    res = []
+    for _ in range(2):
+        g = jb.JumpSim(sysd, **run)
+        g.jump_step(25); g.jump_respa_step(2); g.sync()
+        res.append((g.pos.cpu().numpy().copy(), g.vel.cpu().numpy().copy(), g.stats()["proposals"]))
+    assert (res[0][0] == res[1][0]).all() and (res[0][1] == res[1][1]).all() and res[0][2] == res[1][2]
+
+
+def test_step_batching_is_invisible(jb, cfg0):
+    """jump_step(20) == 20 x jump_step(1): the closing/opening half-phases fused across steps are the same maths."""
+    sysd, run = cfg0
+    a, b = jb.JumpSim(sysd, **run), jb.JumpSim(sysd, **run)
+    a.jump_step(20); a.sync()
+    for _ in range(20):
+        b.jump_step(1)
+    b.sync()
+    assert (a.pos.cpu().numpy() == b.pos.cpu().numpy()).all() and (a.vel.cpu().numpy() == b.vel.cpu().numpy()).all()
+
+
+# ------------------------------------------------------------------------------------- edge cases
+def test_bad_arguments_are_refused(jb, cfg0):
+    sysd, run = cfg0
+    for bad in (dict(n_inner=3), dict(r_short=9.5), dict(r_long=9.5), dict(eps_jump=0.0), dict(eps_mode=1),
+                dict(r_switch=0.0), dict(dt_fs=0.0)):
+        with pytest.raises(jb.JumpError):
+            jb.JumpSim(sysd, **dict(run, **bad))
+
+
+def test_single_molecule_and_empty_shells(jb, jo):
+    """One water in a big box: every row is empty, no proposal is ever made, the step still runs."""
+    sysd = wl.water_box(1, 20.0, 3, 4)
+    run = dict(wl.make_config(0)[1], flags=3 | 4)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    g.jump_step(30); g.jump_respa_step(2); g.sync()
+    o.jump_step(30); o.jump_respa_step(2)
+    assert g.stats()["proposals"] == 0 and pos_err(g, o, sysd["box"]) <= X_TOL
+    check_events(g.events(), o.events())
+
+
+def test_row_overflow_is_reported(jb):
+    """A dense cluster in a mostly empty box exceeds the mean-density row capacity: error -3, not silence."""
+    sysd = wl.small_water(4, seed=3)
+    big = dict(sysd, box=60.0)
+    run = dict(wl.make_config(0)[1], r_short=5.0, r_long=9.0)
+    with pytest.raises(jb.JumpError, match="-3"):
+        jb.JumpSim(big, **run)
+
+
+# ------------------------------------------------------------------------------------- bench configuration
+def test_full_size_config1_forces_events_trajectory(jb, jo):
+    """BASELINE configs[1] (12 000 atoms), the workload bench.py times: all F0, one logged step, 20 steps."""
+    sysd, run = wl.make_config(1)
+    run = dict(run, flags=3 | 4)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    assert rel_force_err(g.forces(0).cpu().numpy(), o.forces(0)) <= F_TOL
+    assert rel_force_err(g.forces(1).cpu().numpy(), o.forces(1)) <= F_TOL
+    g.jump_step(1); g.sync(); o.jump_step(1)
+    check_events(g.events(), o.events())
+    g.clear_events(); o.clear_events()
+    g.jump_step(19); g.sync(); o.jump_step(19)
+    if o.stats()["min_margin"] >= 1e-6:
+        assert pos_err(g, o, sysd["box"]) <= X_TOL
+    st = g.stats()
+    assert st["error"] == 0 and st["max_p"] <= 1 + 1e-4
+
+
+def test_config2_sampled_forces_and_properties(jb, jo):
+    """BASELINE configs[2] (96 000 atoms): F0 against the oracle, Newton's third law of the short part,
+    and statistics that hold at any size (p <= 1, |F_ij| <= L, proposals per atom in the expected range)."""
+    sysd, run = wl.make_config(2)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    fo = o.forces(0)
+    fg = g.forces(0).cpu().numpy()
+    assert rel_force_err(fg, fo) <= F_TOL
+    assert np.abs(g.forces(4).cpu().numpy().astype(np.float64).sum(0)).max() < 0.05   # sum of pair gradients = 0
+    g.jump_respa_step(5); g.sync()
+    st = g.stats()
+    assert st["error"] == 0 and st["max_p"] <= 1 + 1e-4 and st["max_g_over_L"] <= 1 + 1e-4
+    per_atom_fs = st["proposals"] / (g.n * 20.0)
+    assert 0.5 < per_atom_fs < 10.0
