@@ -76,8 +76,8 @@ def test_rows_identical(jb, jo, cfg0, case):
     if case == "cfg0":
         sysd, run = cfg0
     else:
-        sysd = wl.small_water(5, seed=11)                      # 375 atoms, box 22.4 A: ragged, several cells
-        run = dict(cfg0[1], r_short=4.0, r_long=8.0, r_mid=5.0, seed=5)
+        sysd = wl.small_water(5, seed=11)                      # 375 atoms, box 15.5 A: ragged, several cells
+        run = dict(cfg0[1], r_short=4.0, r_long=7.5, r_mid=5.0, seed=5)
         if case == "no_ring":
             run["r_mid"] = 0.0
         if case == "big_cells":
