@@ -173,6 +173,10 @@ def main():
     ap.add_argument("--equil", type=int, default=2000, help="untimed BAOAB equilibration steps from the lattice start")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--mode", default="jump", choices=["jump", "respa"])
+    ap.add_argument("--r-mid", type=float, default=None, help="ring split r_M (default: the config's)")
+    ap.add_argument("--skin", type=float, default=None)
+    ap.add_argument("--nlist-every", type=int, default=None)
+    ap.add_argument("--eps-jump", type=float, default=None)
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -188,6 +192,9 @@ def main():
 
     sysd, run = wl.make_config(args.config)
     run = dict(run, seed=replicas.rank_seed(run["seed"], rank))       # independent replicas
+    for key, val in (("r_mid", args.r_mid), ("skin", args.skin), ("nlist_every", args.nlist_every), ("eps_jump", args.eps_jump)):
+        if val is not None:
+            run[key] = val
     n, dt_fs = sysd["n_atoms"], run["dt_fs"]
     stream = torch.cuda.Stream(dev)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)

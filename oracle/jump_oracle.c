@@ -86,6 +86,10 @@ typedef struct {
     int64_t proposals, accepts, gt_attempts, rebuilds, expiries;
     double max_p, max_g_over_L, max_disp, min_margin;
     int64_t min_margin_step;
+    /* audit of the list decisions (R-17): smallest |d - window edge| over all candidate pairs of the row builds
+     * and smallest distance of an atom to a contract-grid cell face, in A, and the step of that build */
+    double min_list_margin;
+    int64_t min_list_margin_step;
 } orc_stats;
 
 typedef struct {
@@ -318,9 +322,10 @@ static int cmp_u64(const void *a, const void *b) {
  * Each row in ascending (contract cell key of j, j) order (R-10).  The search
  * grid below is only an accelerator (checked against brute force in the tests).
  */
-static void neighbor_csr(const orc_ctx *c, const double *x, double rmin, double rmax, int lj_only,
-                         int brute, int **ptr_out, int **idx_out) {
+static void neighbor_csr_audit(const orc_ctx *c, const double *x, double rmin, double rmax, int lj_only,
+                               int brute, int **ptr_out, int **idx_out, double *edge_margin) {
     int n = c->n;
+    double emin = 1e300;
     int ng[3];
     for (int k = 0; k < 3; ++k) {
         ng[k] = (int)floor(c->p.box[k] / rmax);
@@ -350,7 +355,7 @@ static void neighbor_csr(const orc_ctx *c, const double *x, double rmin, double 
     int *cnt = calloc(n + 1, sizeof(int));
     uint64_t **rows = malloc(sizeof(uint64_t *) * n);
     double r2min = rmin * rmin, r2max = rmax * rmax;
-#pragma omp parallel for schedule(dynamic, 64)
+#pragma omp parallel for schedule(dynamic, 64) reduction(min : emin)
     for (int i = 0; i < n; ++i) {
         int cap = 64, m = 0;
         uint64_t *row = malloc(sizeof(uint64_t) * cap);
@@ -373,6 +378,12 @@ static void neighbor_csr(const orc_ctx *c, const double *x, double rmin, double 
                         double d[3];
                         min_image(c, &x[3 * i], &x[3 * j], d);
                         double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
+                        if (edge_margin && (fabs(r2 - r2max) < 0.05 || (rmin > 0.0 && fabs(r2 - r2min) < 0.05)) &&
+                            !is_excluded(c, i, j)) { /* audit only: how close is this decision to flipping */
+                            double r = sqrt(r2), e = fabs(r - rmax);
+                            if (rmin > 0.0 && fabs(r - rmin) < e) e = fabs(r - rmin);
+                            if (e < emin) emin = e;
+                        }
                         if (r2 >= r2max || r2 < r2min) continue;
                         if (is_excluded(c, i, j)) continue;
                         if (m == cap) { cap *= 2; row = realloc(row, sizeof(uint64_t) * cap); }
@@ -393,6 +404,11 @@ static void neighbor_csr(const orc_ctx *c, const double *x, double rmin, double 
     free(rows); free(cell); free(start); free(order); free(jkey);
     *ptr_out = cnt;
     *idx_out = idx;
+    if (edge_margin && emin < *edge_margin) *edge_margin = emin;
+}
+static void neighbor_csr(const orc_ctx *c, const double *x, double rmin, double rmax, int lj_only,
+                         int brute, int **ptr_out, int **idx_out) {
+    neighbor_csr_audit(c, x, rmin, rmax, lj_only, brute, ptr_out, idx_out, NULL);
 }
 
 /* exported for the brute-force pin: returns CSR copies */
@@ -653,9 +669,20 @@ static void rebuild_rows(orc_ctx *c) {
     free(c->ptrM); free(c->idxM); free(c->ptrL); free(c->idxL); free(c->ptrV); free(c->idxV);
     double s = c->skin, lo = c->rc - c->h - s;
     if (lo < 0.0) lo = 0.0;
-    neighbor_csr(c, c->x, lo, c->rM, 0, 0, &c->ptrM, &c->idxM);
-    neighbor_csr(c, c->x, dmax(c->rM, lo), c->rE + s, 0, 0, &c->ptrL, &c->idxL);
-    neighbor_csr(c, c->x, lo, c->rE + s, 1, 0, &c->ptrV, &c->idxV);
+    double em = 1e300;
+    neighbor_csr_audit(c, c->x, lo, c->rM, 0, 0, &c->ptrM, &c->idxM, &em);
+    neighbor_csr_audit(c, c->x, dmax(c->rM, lo), c->rE + s, 0, 0, &c->ptrL, &c->idxL, &em);
+    neighbor_csr_audit(c, c->x, lo, c->rE + s, 1, 0, &c->ptrV, &c->idxV, &em);
+    {   /* contract-grid cell faces (the row order depends on the cell of every atom, R-10) */
+        int nn[3] = {c->gnx, c->gny, c->gnz};
+        for (int i = 0; i < c->n; ++i)
+            for (int k = 0; k < 3; ++k) {
+                double w = c->p.box[k] / nn[k], f = wrap1(c->x[3 * i + k], c->p.box[k]) / w;
+                double e = fabs(f - floor(f + 0.5)) * w;
+                if (nn[k] > 1 && e < em) em = e;
+            }
+    }
+    if (em < c->st.min_list_margin) { c->st.min_list_margin = em; c->st.min_list_margin_step = c->step; }
     memcpy(c->x_build, c->x, sizeof(double) * 3 * c->n);
     c->st.rebuilds++;
 }
@@ -719,6 +746,7 @@ void orc_get_stats(const orc_ctx *c, orc_stats *out) { *out = c->st; }
 void orc_reset_stats(orc_ctx *c) {
     memset(&c->st, 0, sizeof c->st);
     c->st.min_margin = 1e300;
+    c->st.min_list_margin = 1e300;
 }
 
 /* ------------------------------------------------------------------ */

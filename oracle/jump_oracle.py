@@ -61,7 +61,7 @@ class Stats(C.Structure):
         ("proposals", C.c_int64), ("accepts", C.c_int64), ("gt_attempts", C.c_int64), ("rebuilds", C.c_int64),
         ("expiries", C.c_int64),
         ("max_p", C.c_double), ("max_g_over_L", C.c_double), ("max_disp", C.c_double), ("min_margin", C.c_double),
-        ("min_margin_step", C.c_int64),
+        ("min_margin_step", C.c_int64), ("min_list_margin", C.c_double), ("min_list_margin_step", C.c_int64),
     ]
 
 

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <initializer_list>
 #include <string>
 #include <vector>
 
@@ -29,6 +30,8 @@ struct jump_ctx {
     int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src;
     Row rows[N_ROWS];
     bool row_fresh[N_ROWS];  // built since the last sort
+    bool row_used[N_ROWS];   // read since the last sort: rebuilt eagerly at the next one (others lazily, on demand)
+    bool f0_valid;           // c->f0 / fnb / fbond hold F0 at the current positions
     float4 *fnb, *fbond, *f0, *ftmp, *ftmp2;
     double *ke;
     int *excl_ptr, *excl_idx;
@@ -176,17 +179,19 @@ static int alloc_row(jump_ctx *c, int k) {
     return 0;
 }
 
-static int build_rows(jump_ctx *c, bool only_missing) {
+// build the given rows (all in one launch) at the current sort
+static int build_rows(jump_ctx *c, const bool want[N_ROWS]) {
     Row sel[N_ROWS];
     bool any = false;
+    double rmax = 0.0;
     for (int k = 0; k < N_ROWS; ++k) {
         sel[k] = c->rows[k];
-        if (only_missing && c->row_fresh[k]) sel[k].enabled = 0;
-        if (sel[k].enabled) { any = true; c->row_fresh[k] = true; }
+        if (!(want[k] && c->rows[k].enabled && !c->row_fresh[k])) sel[k].enabled = 0;
+        if (sel[k].enabled) { any = true; c->row_fresh[k] = true; rmax = std::max(rmax, std::sqrt(sel[k].r2max_d)); }
     }
     if (!any) return 0;
     prof_begin(c, PROF_BUILD);
-    launch_build_rows(c->m, c->g, sel, (float)(c->p.r_long + c->p.skin), c->cell_start, c->xs, c->lj, c->orig,
+    launch_build_rows(c->m, c->g, sel, (float)rmax, c->cell_start, c->xs, c->xl, c->lj, c->orig,
                       c->sorted_of, c->excl_ptr, c->excl_idx, c->ctr, c->st, &c->launches);
     prof_end(c, PROF_BUILD);
     CK(cudaGetLastError());
@@ -207,18 +212,29 @@ static int resort_and_build(jump_ctx *c) {
     CK(cudaGetLastError());
     std::swap(c->xs, c->xs_nxt); std::swap(c->vs, c->vs_nxt); std::swap(c->xl, c->xl_nxt); std::swap(c->lj, c->lj_nxt);
     std::swap(c->mi, c->mi_nxt); std::swap(c->orig, c->orig_nxt);
-    for (int k = 0; k < N_ROWS; ++k) c->row_fresh[k] = false;
+    bool want[N_ROWS];
+    for (int k = 0; k < N_ROWS; ++k) { c->row_fresh[k] = false; want[k] = c->row_used[k]; c->row_used[k] = false; }
     c->rebuilds++;
-    return build_rows(c, false);
+    return build_rows(c, want);
 }
 
-static int need_row(jump_ctx *c, int k) {  // lazily enabled rows (full list of the BAOAB comparator)
-    int r = alloc_row(c, k);
-    if (r) return r;
-    return build_rows(c, true);
+// every read of a row goes through here: allocate on first use, build if stale
+static int need_rows(jump_ctx *c, std::initializer_list<int> ks) {
+    bool want[N_ROWS] = {false, false, false, false, false, false};
+    bool stale = false;
+    for (int k : ks) {
+        int r = alloc_row(c, k);
+        if (r) return r;
+        c->row_used[k] = true;
+        want[k] = true;
+        stale |= !c->row_fresh[k];
+    }
+    return stale ? build_rows(c, want) : 0;
 }
+static int need_row(jump_ctx *c, int k) { return need_rows(c, {k}); }
 
 static void pair(jump_ctx *c, int row, int wC, int wLJ, float4 *out, int accumulate, bool energy) {
+    if (need_row(c, row)) return;
     prof_begin(c, PROF_PAIR);
     launch_pair(c->m, c->rows[row], wC, wLJ, c->xs, c->lj, out, accumulate, energy, c->st, &c->launches);
     prof_end(c, PROF_PAIR);
@@ -246,8 +262,10 @@ static int compute_short_nb(jump_ctx *c, float4 *out, bool energy = false) {
 static int compute_f0(jump_ctx *c) {
     int r = compute_short_nb(c, c->fnb);
     if (r) return r;
+    c->f0_valid = true;
     return bonded(c, c->fnb, c->f0, c->fbond);
 }
+static int ensure_f0(jump_ctx *c) { return c->f0_valid ? 0 : compute_f0(c); }
 static int compute_long(jump_ctx *c, float4 *out) {
     int wLJ = lj_jumps(c) ? W_LONG : W_NONE;
     pair(c, ROW_M, W_LONG, wLJ, out, 0, false);
@@ -256,8 +274,7 @@ static int compute_long(jump_ctx *c, float4 *out) {
     return 0;
 }
 static int compute_full(jump_ctx *c, float4 *out, bool energy = false) {  // unsplit to r_long + bonded
-    int r = need_row(c, ROW_F);
-    if (r) return r;
+    int r;
     pair(c, ROW_F, W_FULL, W_FULL, c->ftmp2, 0, energy);
     CK(cudaGetLastError());
     return bonded(c, c->ftmp2, out, nullptr);
@@ -287,12 +304,19 @@ static int run_update(jump_ctx *c, const Phase &p0, const float4 *g0, const Phas
     A.rowM = c->rows[ROW_M]; A.rowL = c->rows[ROW_L]; A.rowV = c->rows[ROW_V];
     A.ctr = c->ctr; A.events = (c->p.flags & JUMP_F_EVENT_LOG) ? c->events : nullptr; A.event_cap = c->event_cap;
     bool jumps = (p0.kind == 2 || p1.kind == 2) && (coul_jumps(c) || lj_jumps(c));
+    if (jumps) {
+        int r = coul_jumps(c) ? need_rows(c, {ROW_M, ROW_L}) : 0;
+        if (!r && lj_jumps(c)) r = need_row(c, ROW_V);
+        if (r) return r;
+        A.rowM = c->rows[ROW_M]; A.rowL = c->rows[ROW_L]; A.rowV = c->rows[ROW_V];
+    }
     prof_begin(c, PROF_UPDATE);
     launch_update(c->m, A, jumps, c->st, &c->launches);
     prof_end(c, PROF_UPDATE);
     CK(cudaGetLastError());
     if (aoa) {
         std::swap(c->xs, c->xs_nxt);
+        c->f0_valid = false;
         c->step++;
         if (c->p.nlist_every > 0 && c->step % c->p.nlist_every == 0) return resort_and_build(c);
     }
@@ -319,6 +343,8 @@ extern "C" int jump_step(jump_ctx *c, int32_t n_steps) {
     if (!c || n_steps < 0) return JUMP_E_ARG;
     if (n_steps == 0) return 0;
     const double H = 0.5 * c->dt;
+    int r0 = ensure_f0(c);
+    if (r0) return r0;
     for (int s = 0; s < n_steps; ++s) {
         int64_t st = c->step;
         Phase open = ph_jump(c, H, true, false, 1, 2, st);
@@ -347,9 +373,7 @@ extern "C" int baoab_step(jump_ctx *c, int32_t n_steps) {
     }
     r = run_update(c, ph_kick(H), c->ftmp, ph_none(), nullptr, false);
     if (r) return r;
-    r = compute_f0(c);
-    if (r) return r;
-    return writeback(c);
+    return writeback(c);  // F0 is recomputed on demand (f0_valid)
 }
 
 extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
@@ -357,7 +381,8 @@ extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
     const int n = c->p.n_inner;
     const double D = n * c->dt, H = 0.5 * c->dt;
     const bool paper = (c->p.flags & JUMP_F_RESPA_PAPER) != 0, cmp = (c->p.flags & JUMP_F_RESPA_COMPARATOR) != 0;
-    int r;
+    int r = ensure_f0(c);
+    if (r) return r;
     for (int o = 0; o < n_outer; ++o) {
         Phase outer[2];
         const float4 *gout[2];
@@ -401,7 +426,9 @@ extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
 
 extern "C" int jump_half(jump_ctx *c, double H_ps, int32_t with_accel, int64_t step) {
     if (!c) return JUMP_E_ARG;
-    int r = run_update(c, ph_jump(c, H_ps, with_accel != 0, false, 1, 2, step), c->f0, ph_none(), nullptr, false);
+    int r = ensure_f0(c);
+    if (r) return r;
+    r = run_update(c, ph_jump(c, H_ps, with_accel != 0, false, 1, 2, step), c->f0, ph_none(), nullptr, false);
     if (r) return r;
     return writeback(c);
 }
@@ -440,7 +467,8 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     for (int k = 0; k < 3; ++k) { m.box[k] = (float)p->box[k]; m.inv_box[k] = (float)(1.0 / p->box[k]); }
     m.rc = (float)p->r_short; m.h = (float)p->r_switch; m.inv_h = (float)(1.0 / p->r_switch);
     m.rlo = (float)(p->r_short - p->r_switch);
-    m.rc2 = (float)(p->r_short * p->r_short); m.rlo2 = m.rlo * m.rlo; m.rE2 = (float)(p->r_long * p->r_long);
+    m.rc2 = (float)(p->r_short * p->r_short); m.rlo2 = m.rlo * m.rlo;
+    m.rlo2d = (p->r_short - p->r_switch) * (p->r_short - p->r_switch); m.rE2 = (float)(p->r_long * p->r_long);
     m.alpha = (float)c->alpha; m.alpha2 = (float)(c->alpha * c->alpha);
     m.beta = (float)(1.0 / c->kT);
     m.eps_jump = std::isinf(p->eps_jump) ? INFINITY : (float)p->eps_jump;
@@ -455,7 +483,8 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     for (int k = 0; k < 3; ++k) {
         g.gn[k] = std::max(1, (int)std::floor(p->box[k] / edge));
         g.scale[k] = (double)g.gn[k] / p->box[k];
-        g.reach[k] = (int)std::ceil((p->r_long + p->skin) / (p->box[k] / g.gn[k]) - 1e-12);
+        g.reach[k] = (int)std::ceil((p->r_long + p->skin) / (p->box[k] / g.gn[k]));
+        if (g.reach[k] > 8) return JUMP_E_ARG;  // stencil table of the row build (cell_edge too small)
         g.ncell *= g.gn[k];
     }
     // buffers
@@ -472,7 +501,7 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     CK(cudaMemsetAsync(c->ctr, 0, sizeof(Counters), c->st));
     c->event_cap = 0; c->events = nullptr;
     if (p->flags & JUMP_F_EVENT_LOG) {
-        c->event_cap = 1ll << 21;
+        c->event_cap = std::min<long long>(std::max<long long>(1ll << 21, 512ll * n), 1ll << 25);
         if ((r = dalloc(c, &c->events, (size_t)c->event_cap))) return r;
     }
     // exclusions (own copy)
@@ -543,13 +572,20 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
             R.lj_only = w[k].lj;
             R.r2min = (float)(w[k].a * w[k].a);
             R.r2max = (float)(w[k].b * w[k].b);
+            R.r2min_d = w[k].a * w[k].a;
+            R.r2max_d = w[k].b * w[k].b;
             c->row_fresh[k] = false;
-            if (w[k].on && (r = alloc_row(c, k))) return r;
+            c->row_used[k] = false;
         }
     }
     if ((r = load_state(c, d_mass, d_charge, d_sigma, d_eps))) return r;
     if ((r = resort_and_build(c))) return r;
     c->rebuilds = 1;
+    {   // the rows this mode reads on every step, built in one launch
+        bool want[N_ROWS] = {true, coul_jumps(c), coul_jumps(c), lj_jumps(c), false, !lj_jumps(c)};
+        for (int k = 0; k < N_ROWS; ++k) if (want[k] && (r = alloc_row(c, k))) return r;
+        if ((r = build_rows(c, want))) return r;
+    }
     if ((r = compute_f0(c))) return r;
     if ((r = writeback(c))) return r;  // wrapped positions
     return poll_error(c);
@@ -574,6 +610,7 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     c->d_pos = d_pos; c->d_vel = d_vel;
     c->step = c->outer = c->rebuilds = c->launches = 0;
     c->sticky = 0;
+    c->f0_valid = false;
     c->prof = false;
     for (int k = 0; k < 4; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     int r = init_impl(c, p, d_mass, d_charge, d_lj_sigma, d_lj_eps, n_bonds, d_bond_ij, d_bond_k, d_bond_r0, n_angles,
@@ -685,8 +722,8 @@ extern "C" int jump_clear_events(jump_ctx *c) {
 }
 extern "C" int jump_get_row(jump_ctx *c, int32_t which, int32_t atom, int32_t *host_out, int32_t cap) {
     if (!c || which < 0 || which >= N_ROWS || atom < 0 || atom >= c->n) return JUMP_E_ARG;
+    { int r = need_row(c, which); if (r) return r; }
     const Row &R = c->rows[which];
-    if (!R.enabled) return JUMP_E_ARG;
     int i = 0, cnt = 0;
     CK(cudaMemcpyAsync(&i, c->sorted_of + atom, sizeof(int), cudaMemcpyDeviceToHost, c->st));
     CK(cudaStreamSynchronize(c->st));
@@ -730,9 +767,11 @@ extern "C" int jump_get_profile(jump_ctx *c, double ms[4], int64_t count[4]) {
     return 0;
 }
 extern "C" int jump_count_pairs(jump_ctx *c, int32_t which_row, double r_cut, int64_t *n_ordered) {
-    if (!c || !n_ordered || which_row < 0 || which_row >= N_ROWS || !c->rows[which_row].enabled) return JUMP_E_ARG;
+    if (!c || !n_ordered || which_row < 0 || which_row >= N_ROWS) return JUMP_E_ARG;
     unsigned long long *d = nullptr;
-    int r = dalloc(c, &d, 1);
+    int r = need_row(c, which_row);
+    if (r) return r;
+    r = dalloc(c, &d, 1);
     if (r) return r;
     CK(cudaMemsetAsync(d, 0, sizeof(unsigned long long), c->st));
     launch_count_pairs(c->m, c->rows[which_row], c->xs, (float)(r_cut * r_cut), d, c->st, &c->launches);

@@ -30,6 +30,7 @@ struct Row {
     int cap;        // multiple of 32
     int lj_only;    // keep eps_i eps_j > 0 only
     float r2min, r2max;  // build-time window rmin <= d < rmax
+    double r2min_d, r2max_d;  // the same in fp64 (edge decisions, R-17)
     int enabled;
 };
 
@@ -47,6 +48,7 @@ struct Model {
     float box[3], inv_box[3];
     float rc, h, inv_h, rlo;      // r_c, h, 1/h, r_c - h
     float rc2, rlo2, rE2;         // squares
+    double rlo2d;                 // (r_c - h)^2 in fp64 (switching argument, see chi_zone)
     float alpha, alpha2;          // Ewald alpha
     float beta;                   // 1/kT, (kcal/mol)^-1
     float eps_jump;               // epsilon; +inf -> BPS
@@ -85,20 +87,36 @@ __device__ inline float wrap1(float x, float L, float invL) {
     if (x < 0.f) x = 0.f;
     return x;
 }
-// minimum image of xi - xj, both in [0, L).  The shift (0 or +-L) is applied to xi first:
-// xi - L is exact for xi in [L/2, L) (Sterbenz), so the result carries one rounding of the final
-// difference only -- a plain (xi - xj) - L would carry an absolute error of ulp(L) ~ 2e-6 A.
-__device__ inline float min_image1(float xi, float xj, float L, float invL) {
+// Minimum image of xi - xj, both in [0, L).  The periodic shift t L (t = -1, 0, 1) is applied so that it
+// is EXACT: for t = +1 to xi (xi - L with xi in (L/2, L), Sterbenz), for t = -1 to xj (xj - L with xj in
+// (L/2, L)); xi + L would round at ulp(2 L), an absolute error of ~4e-6 A at L = 62 A.  a - b then carries one
+// rounding of the final difference only, and (double)a - (double)b is the exact image difference.
+__device__ inline void image_pair1(float xi, float xj, float L, float invL, float &a, float &b) {
     float t = (xi - xj) * invL + 12582912.f;  // round to nearest integer by the 1.5 * 2^23 trick
     t -= 12582912.f;
-    return fmaf(-L, t, xi) - xj;
+    a = fmaf(-L, fmaxf(t, 0.f), xi);
+    b = fmaf(L, fminf(t, 0.f), xj);
+}
+__device__ inline float min_image1(float xi, float xj, float L, float invL) {
+    float a, b;
+    image_pair1(xi, xj, L, invL, a, b);
+    return a - b;
 }
 
-// chi (R-3): quintic smootherstep on [rc-h, rc]; returns chi, writes dchi/dr
-__device__ inline float chi_of(float r, const Model &m, float &dchi) {
-    float u = (r - m.rlo) * m.inv_h;
-    if (u <= 0.f) { dchi = 0.f; return 1.f; }
-    if (u >= 1.f) { dchi = 0.f; return 0.f; }
+// chi (R-3): quintic smootherstep on [rc-h, rc]; returns chi, writes dchi/dr.
+// Outside the switching zone chi is 0 or 1 and nothing else is computed.  Inside it the argument
+// u = (r - r_lo)/h is formed as (r^2 - r_lo^2) / (h (r + r_lo)) with r^2 - r_lo^2 in fp64 from the exact
+// coordinate differences (a - b of image_pair1): a plain fp32 r - r_lo carries an absolute error
+// of ~3e-7 A that chi'' u_C (~10 kcal/mol/A^2) turns into ~3e-6 per pair -- the largest error of the long
+// force and of the acceptance probabilities p (R-16, R-17).
+__device__ inline float chi_zone(float ax, float ay, float az, float bx, float by, float bz, float r2, float r,
+                                 const Model &m, float &dchi) {
+    if (r2 <= m.rlo2) { dchi = 0.f; return 1.f; }
+    if (r2 >= m.rc2) { dchi = 0.f; return 0.f; }
+    double dx = (double)ax - (double)bx, dy = (double)ay - (double)by, dz = (double)az - (double)bz;
+    double d2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, -m.rlo2d)));
+    float u = (float)d2 * m.inv_h / (r + m.rlo);
+    u = fminf(fmaxf(u, 0.f), 1.f);
     float omu = 1.f - u;
     dchi = -30.f * u * u * omu * omu * m.inv_h;
     return 1.f - u * u * u * (10.f - 15.f * u + 6.f * u * u);

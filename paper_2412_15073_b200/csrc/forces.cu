@@ -11,16 +11,14 @@
 namespace jb {
 
 template <int W>
-__device__ inline float weighted_du(float r, float u, float du, const Model &m) {
+__device__ inline float weighted_du(float chi, float dchi, float u, float du) {
     if (W == W_FULL) return du;
-    float dchi, chi = chi_of(r, m, dchi);
     if (W == W_SHORT) return chi * du + dchi * u;  // d/dr [chi u]
     return (1.f - chi) * du - dchi * u;             // d/dr [(1-chi) u]
 }
 template <int W>
-__device__ inline float weighted_u(float r, float u, const Model &m) {
+__device__ inline float weighted_u(float chi, float u) {
     if (W == W_FULL) return u;
-    float dchi, chi = chi_of(r, m, dchi);
     return W == W_SHORT ? chi * u : (1.f - chi) * u;
 }
 
@@ -42,20 +40,23 @@ __global__ void __launch_bounds__(256) k_pair(Model m, Row row, const float4 *__
     for (int k = lane; k < cnt; k += 32) {
         int j = ridx[k];
         float4 xj = xs[j];
-        float dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
-        float dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
-        float dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
+        float ax, ay, az, bx, by, bz;
+        image_pair1(xi.x, xj.x, m.box[0], m.inv_box[0], ax, bx);
+        image_pair1(xi.y, xj.y, m.box[1], m.inv_box[1], ay, by);
+        image_pair1(xi.z, xj.z, m.box[2], m.inv_box[2], az, bz);
+        float dx = ax - bx, dy = ay - by, dz = az - bz;
         float r2 = dx * dx + dy * dy + dz * dz;
         if (r2 >= cut2) continue;
         float rinv = rsqrtf(r2), r = r2 * rinv;
-        float fr = 0.f;
+        float fr = 0.f, chi = 1.f, dchi = 0.f;
+        if (WC == W_SHORT || WC == W_LONG || WLJ == W_SHORT || WLJ == W_LONG) chi = chi_zone(ax, ay, az, bx, by, bz, r2, r, m, dchi);
         if (WC != W_NONE && r2 < cutC2) {
             float qq = qi * xj.w;
-            float e = erfcf(m.alpha * r), ex = __expf(-m.alpha2 * r2);
+            float e = erfcf(m.alpha * r), ex = expf(-m.alpha2 * r2);
             float u = qq * e * rinv;
             float du = -(u + qq * kTwoOverSqrtPi * m.alpha * ex) * rinv;  // u'
-            fr += weighted_du<WC>(r, u, du, m);
-            if (ENERGY) en += weighted_u<WC>(r, u, m);
+            fr += weighted_du<WC>(chi, dchi, u, du);
+            if (ENERGY) en += weighted_u<WC>(chi, u);
         }
         if (do_lj && r2 < cutL2) {
             float2 ljj = lj[j];
@@ -64,8 +65,8 @@ __global__ void __launch_bounds__(256) k_pair(Model m, Row row, const float4 *__
                 float e4 = lji.y * ljj.y;  // 4 eps_ij (R-8: geometric mixing)
                 float u = e4 * (s12 - s6);
                 float du = e4 * (6.f * s6 - 12.f * s12) * rinv;
-                fr += weighted_du<WLJ>(r, u, du, m);
-                if (ENERGY) en += weighted_u<WLJ>(r, u, m);
+                fr += weighted_du<WLJ>(chi, dchi, u, du);
+                if (ENERGY) en += weighted_u<WLJ>(chi, u);
             }
         }
         float s = fr * rinv;

@@ -7,6 +7,9 @@
 //     fixed-capacity rows.  Because the atom array is sorted by (cell key, original index), rows come
 //     out in the canonical order of R-10 without any per-row sort (rows one can draw
 //     from uniformly, with their counts N_M(i), N_L(i), N_V(i)).
+#include <algorithm>
+#include <cmath>
+
 #include "launch.h"
 
 namespace jb {
@@ -122,115 +125,226 @@ __device__ inline int cyc_off(int val, int c, int gn) {
     return o;
 }
 
-__global__ void __launch_bounds__(256) k_build_rows(Model m, SortGrid g, RowSet rows, float rmax_all,
-                                                    const int *__restrict__ cell_start,
-                                                    const float4 *__restrict__ xs, const float2 *__restrict__ lj,
-                                                    const int *__restrict__ orig, const int *__restrict__ sorted_of,
-                                                    const int *__restrict__ excl_ptr, const int *__restrict__ excl_idx,
-                                                    Counters *ctr) {
+// Row build, one CTA per cell of the contract grid.
+//  1. The candidate set of a cell is the same for all its atoms: the cells of a host-computed stencil (every cell
+//     whose extent comes within rmax of this cell), visited in ascending cell key, i.e. a list of contiguous runs
+//     [seg_beg, seg_beg + seg_len) of the sorted atom array.  The runs are found once per CTA, prefix-summed and
+//     the candidates (x, y, z, q | sorted index + LJ flag) staged in shared memory in canonical order.
+//  2. Each warp takes one atom of the cell and scans the staged candidates 32 at a time: fp32 distance, window
+//     tests of the selected rows, exclusions, ballot compaction into the fixed-capacity rows.
+//  3. A candidate whose fp32 r^2 lies within BUILD_TIE of a window edge is decided again in fp64 from the full
+//     positions x = xs + xl, with the oracle's expression d - L rint(d/L): membership at an edge is a discontinuous
+//     decision (R-17) and the fp32 value of r^2 (error ~1e-5 A^2) would flip it where the fp64 oracle does not.
+constexpr int BUILD_THREADS = 128;
+constexpr int BUILD_WARPS = BUILD_THREADS / 32;
+constexpr int BUILD_CHUNK = 1024;           // candidates staged per pass
+constexpr int BUILD_MAXSEG = 2 * 17 * 17;   // two x-runs per (z, y) cell row of the stencil
+constexpr float BUILD_TIE = 4e-3f;          // A^2
+
+struct Stencil {
+    int R[3];                 // cells on each side, per dimension
+    int n_edge;               // distinct window edges of the selected rows (squared, fp32)
+    float edge2[4];           // padded with a value no r^2 comes near
+    signed char xr[17 * 17];  // [|oz| * 17 + |oy|] -> largest |ox| still within reach, -1: skip the (z, y) cell row
+};
+
+// MASK >= 0: bit k set = row k is built (compile-time row set of the common modes); MASK < 0: rows.r[k].enabled decides
+template <int MASK>
+__global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid g, RowSet rows, Stencil stn, float rmax_all,
+                                                              const int *__restrict__ cell_start,
+                                                              const float4 *__restrict__ xs, const float4 *__restrict__ xl,
+                                                              const float2 *__restrict__ lj,
+                                                              const int *__restrict__ orig, const int *__restrict__ sorted_of,
+                                                              const int *__restrict__ excl_ptr, const int *__restrict__ excl_idx,
+                                                              Counters *ctr) {
+    __shared__ int seg_beg[BUILD_MAXSEG];
+    __shared__ int seg_pre[BUILD_MAXSEG + 1];   // exclusive prefix of the run lengths
+    __shared__ float4 tile_x[BUILD_CHUNK];
+    __shared__ int tile_j[BUILD_CHUNK];         // sorted index | LJ flag in bit 31
+    __shared__ int scan_tmp[BUILD_THREADS];
     const unsigned full = 0xffffffffu;
-    int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (warp >= m.n) return;
-    const int i = warp;
-    const float4 xi = xs[i];
-    const bool lj_i = lj[i].y > 0.f;
-    // my cell (same arithmetic as k_cell_key; x has not moved since)
+    const int cell = blockIdx.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int a_beg = cell_start[cell], a_end = cell_start[cell + 1];
+    if (a_end == a_beg) return;
     int c3[3];
-    c3[0] = min(max((int)floor((double)xi.x * g.scale[0]), 0), g.gn[0] - 1);
-    c3[1] = min(max((int)floor((double)xi.y * g.scale[1]), 0), g.gn[1] - 1);
-    c3[2] = min(max((int)floor((double)xi.z * g.scale[2]), 0), g.gn[2] - 1);
+    c3[0] = cell % g.gn[0];
+    c3[1] = (cell / g.gn[0]) % g.gn[1];
+    c3[2] = cell / (g.gn[0] * g.gn[1]);
     int start[3], cnt[3];
-    float cs[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        cs[k] = m.box[k] / (float)g.gn[k];
-        if (2 * g.reach[k] + 1 >= g.gn[k]) { start[k] = 0; cnt[k] = g.gn[k]; }
-        else { start[k] = (c3[k] - g.reach[k] + g.gn[k]) % g.gn[k]; cnt[k] = 2 * g.reach[k] + 1; }
+        if (2 * stn.R[k] + 1 >= g.gn[k]) { start[k] = 0; cnt[k] = g.gn[k]; }
+        else { start[k] = (c3[k] - stn.R[k] + g.gn[k]) % g.gn[k]; cnt[k] = 2 * stn.R[k] + 1; }
     }
-    // exclusions of atom i (original indices -> sorted), first 32 kept in registers
-    int ex_lo = 0, n_ex = 0;
-    if (excl_ptr) { int o = orig[i]; ex_lo = excl_ptr[o]; n_ex = excl_ptr[o + 1] - ex_lo; }
-    int ex_mine = (lane < n_ex) ? sorted_of[excl_idx[ex_lo + lane]] : -1;
-
-    int count[N_ROWS];
-#pragma unroll
-    for (int k = 0; k < N_ROWS; ++k) count[k] = 0;
+    // ---- 1. runs of the stencil in ascending cell key -------------------------------------------------------
+    const int nzy = cnt[2] * cnt[1], nseg = 2 * nzy;
+    for (int p = tid; p < nzy; p += BUILD_THREADS) {
+        int mz = p / cnt[1], my = p - mz * cnt[1];
+        int zc = cyc_val(mz, start[2], cnt[2], g.gn[2]), yc = cyc_val(my, start[1], cnt[1], g.gn[1]);
+        int oz = abs(cyc_off(zc, c3[2], g.gn[2])), oy = abs(cyc_off(yc, c3[1], g.gn[1]));
+        int xm = stn.xr[oz * 17 + oy];
+        int b0 = 0, n0 = 0, b1 = 0, n1 = 0;
+        if (xm >= 0) {
+            int rowbase = (zc * g.gn[1] + yc) * g.gn[0];
+            if (2 * xm + 1 >= g.gn[0]) {
+                b0 = cell_start[rowbase]; n0 = cell_start[rowbase + g.gn[0]] - b0;
+            } else {
+                int xs0 = (c3[0] - xm + g.gn[0]) % g.gn[0], xc = 2 * xm + 1;
+                int w = max(0, xs0 + xc - g.gn[0]);          // cells wrapped to the low end come first
+                if (w > 0) { b0 = cell_start[rowbase]; n0 = cell_start[rowbase + w] - b0; }
+                b1 = cell_start[rowbase + xs0]; n1 = cell_start[rowbase + xs0 + xc - w] - b1;
+            }
+        }
+        seg_beg[2 * p] = b0; seg_pre[2 * p + 1] = n0;
+        seg_beg[2 * p + 1] = b1; seg_pre[2 * p + 2] = n1;
+    }
+    if (tid == 0) seg_pre[0] = 0;
+    __syncthreads();
+    {   // inclusive scan of seg_pre[1..nseg] (each thread a contiguous slice, then a block scan of the slice sums)
+        int per = (nseg + BUILD_THREADS - 1) / BUILD_THREADS;
+        int lo = min(tid * per, nseg), hi = min(lo + per, nseg);
+        int sum = 0;
+        for (int k = lo; k < hi; ++k) sum += seg_pre[k + 1];
+        scan_tmp[tid] = sum;
+        __syncthreads();
+        for (int off = 1; off < BUILD_THREADS; off <<= 1) {
+            int v = tid >= off ? scan_tmp[tid - off] : 0;
+            __syncthreads();
+            scan_tmp[tid] += v;
+            __syncthreads();
+        }
+        int run = scan_tmp[tid] - sum;
+        for (int k = lo; k < hi; ++k) { run += seg_pre[k + 1]; seg_pre[k + 1] = run; }
+    }
+    __syncthreads();
+    const int total = seg_pre[nseg];
     const float rmax2 = rmax_all * rmax_all;
     const unsigned lt_mask = (1u << lane) - 1u;
 
-    for (int mz = 0; mz < cnt[2]; ++mz) {
-        int zc = cyc_val(mz, start[2], cnt[2], g.gn[2]);
-        float dz = fmaxf(0.f, (float)(abs(cyc_off(zc, c3[2], g.gn[2])) - 1)) * cs[2];
-        for (int my = 0; my < cnt[1]; ++my) {
-            int yc = cyc_val(my, start[1], cnt[1], g.gn[1]);
-            float dy = fmaxf(0.f, (float)(abs(cyc_off(yc, c3[1], g.gn[1])) - 1)) * cs[1];
-            if (dz * dz + dy * dy >= rmax2) continue;
-            int rowbase = (zc * g.gn[1] + yc) * g.gn[0];
-            int w = max(0, start[0] + cnt[0] - g.gn[0]);
-#pragma unroll 1
-            for (int seg = 0; seg < 2; ++seg) {
-                int ca = seg == 0 ? 0 : start[0], cb = seg == 0 ? w : start[0] + cnt[0] - w;
-                if (cb <= ca) continue;
-                int jb = cell_start[rowbase + ca], je = cell_start[rowbase + cb];
-                for (int j0 = jb; j0 < je; j0 += 32) {
-                    int j = j0 + lane;
-                    bool valid = j < je && j != i;
-                    float r2 = 0.f;
-                    bool lj_j = false;
-                    if (valid) {
-                        float4 xj = xs[j];
-                        float dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
-                        float dy2 = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
-                        float dz2 = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
-                        r2 = dx * dx + dy2 * dy2 + dz2 * dz2;
-                        if (lj_i) lj_j = lj[j].y > 0.f;
-                    }
-                    bool pass[N_ROWS];
-                    bool any = false;
+    // ---- 2./3. atoms of the cell, BUILD_WARPS at a time --------------------------------------------------------
+    for (int a0 = a_beg; a0 < a_end; a0 += BUILD_WARPS) {
+        const int i = a0 + warp;
+        const bool have = i < a_end;
+        float4 xi = make_float4(0.f, 0.f, 0.f, 0.f);
+        bool lj_i = false;
+        int ex_lo = 0, n_ex = 0, ex_mine = -1;
+        int ex4[4] = {-1, -1, -1, -1};   // up to four excluded partners held by every lane (water: two)
+        if (have) {
+            xi = xs[i];
+            lj_i = lj[i].y > 0.f;
+            if (excl_ptr) { int o = orig[i]; ex_lo = excl_ptr[o]; n_ex = excl_ptr[o + 1] - ex_lo; }
+            ex_mine = (lane < n_ex) ? sorted_of[excl_idx[ex_lo + lane]] : -1;
 #pragma unroll
-                    for (int k = 0; k < N_ROWS; ++k) {
-                        const Row &R = rows.r[k];
-                        pass[k] = R.enabled && valid && r2 >= R.r2min && r2 < R.r2max && (!R.lj_only || (lj_i && lj_j));
-                        any |= pass[k];
+            for (int e = 0; e < 4; ++e) ex4[e] = __shfl_sync(full, ex_mine, e);
+        }
+#define JB_ROW_ON(k) (MASK >= 0 ? (((MASK) >> (k)) & 1) != 0 : rows.r[k].enabled != 0)
+        int count[N_ROWS];
+        int *rbase[N_ROWS];
+#pragma unroll
+        for (int k = 0; k < N_ROWS; ++k) {
+            count[k] = 0;
+            rbase[k] = JB_ROW_ON(k) ? rows.r[k].idx + (size_t)(have ? i : 0) * rows.r[k].cap : nullptr;
+        }
+        const float e0 = stn.edge2[0], e1 = stn.edge2[1], e2 = stn.edge2[2], e3 = stn.edge2[3];
+
+        for (int c0 = 0; c0 < total; c0 += BUILD_CHUNK) {
+            const int c1 = min(c0 + BUILD_CHUNK, total);
+            __syncthreads();   // the previous chunk has been consumed
+            {   // stage the runs that intersect [c0, c1): first one by bisection, then one run per warp iteration
+                int lo_s = 0, hi_s = nseg;   // first run with seg_pre[s + 1] > c0
+                while (lo_s < hi_s) { int mid = (lo_s + hi_s) >> 1; if (seg_pre[mid + 1] > c0) hi_s = mid; else lo_s = mid + 1; }
+                for (int sgi = lo_s + warp; sgi < nseg; sgi += BUILD_WARPS) {
+                    int p0 = seg_pre[sgi], p1 = seg_pre[sgi + 1];
+                    if (p0 >= c1) break;
+                    int lo = max(p0, c0), hi = min(p1, c1);
+                    for (int q = lo + lane; q < hi; q += 32) {
+                        int j = seg_beg[sgi] + (q - p0);
+                        tile_x[q - c0] = xs[j];
+                        tile_j[q - c0] = j | (lj[j].y > 0.f ? (int)0x80000000 : 0);
                     }
-                    if (n_ex > 0 && __any_sync(full, any)) {  // R-9: excluded pairs are never listed
-                        bool ex = false;
+                }
+            }
+            __syncthreads();
+            if (!have) continue;
+            for (int q0 = c0; q0 < c1; q0 += 32) {
+                const int q = q0 + lane;
+                bool valid = q < c1;
+                float4 xj = make_float4(0.f, 0.f, 0.f, 0.f);
+                int jraw = 0;
+                if (valid) { xj = tile_x[q - c0]; jraw = tile_j[q - c0]; }
+                const int j = jraw & 0x7fffffff;
+                const bool ljp = lj_i && jraw < 0;
+                float dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
+                float dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
+                float dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
+                float r2 = dx * dx + dy * dy + dz * dz;
+                valid = valid && j != i && r2 < rmax2 + BUILD_TIE;
+                if (!__any_sync(full, valid)) continue;
+                if (n_ex > 0) {   // excluded pairs are never listed (R-9)
+                    bool ex = (j == ex4[0]) | (j == ex4[1]) | (j == ex4[2]) | (j == ex4[3]);
+                    if (n_ex > 4) {
                         for (int base = 0; base < n_ex; base += 32) {
                             int mine = ex_mine;
                             if (base > 0) mine = (base + lane < n_ex) ? sorted_of[excl_idx[ex_lo + base + lane]] : -1;
                             int lim = min(32, n_ex - base);
                             for (int e = 0; e < lim; ++e) ex |= (__shfl_sync(full, mine, e) == j);
                         }
-                        if (ex) {
+                    }
+                    valid = valid && !ex;
+                }
+                bool pass[N_ROWS];
 #pragma unroll
-                            for (int k = 0; k < N_ROWS; ++k) pass[k] = false;
-                        }
+                for (int k = 0; k < N_ROWS; ++k) {
+                    pass[k] = false;
+                    if (!JB_ROW_ON(k)) continue;
+                    const Row &R = rows.r[k];
+                    pass[k] = valid && (!R.lj_only || ljp) && r2 >= R.r2min && r2 < R.r2max;
+                }
+                const bool tie = valid && (fabsf(r2 - e0) < BUILD_TIE || fabsf(r2 - e1) < BUILD_TIE ||
+                                           fabsf(r2 - e2) < BUILD_TIE || fabsf(r2 - e3) < BUILD_TIE);
+                if (tie) {   // decide in fp64 from the full positions, like the oracle
+                    float4 li = xl[i], lj4 = xl[j];
+                    double d[3] = {((double)xi.x + (double)li.x) - ((double)xj.x + (double)lj4.x),
+                                   ((double)xi.y + (double)li.y) - ((double)xj.y + (double)lj4.y),
+                                   ((double)xi.z + (double)li.z) - ((double)xj.z + (double)lj4.z)};
+                    double r2d = 0.0;
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) {
+                        double L = (double)m.box[k];
+                        d[k] -= L * rint(d[k] / L);
+                        r2d += d[k] * d[k];
                     }
 #pragma unroll
                     for (int k = 0; k < N_ROWS; ++k) {
+                        if (!JB_ROW_ON(k)) continue;
                         const Row &R = rows.r[k];
-                        if (!R.enabled) continue;
-                        unsigned mask = __ballot_sync(full, pass[k]);
-                        if (pass[k]) {
-                            int pos = count[k] + __popc(mask & lt_mask);
-                            if (pos < R.cap) R.idx[(size_t)i * R.cap + pos] = j;
-                        }
-                        count[k] += __popc(mask);
+                        pass[k] = (!R.lj_only || ljp) && r2d >= R.r2min_d && r2d < R.r2max_d;
                     }
+                }
+#pragma unroll
+                for (int k = 0; k < N_ROWS; ++k) {
+                    if (!JB_ROW_ON(k)) continue;
+                    const unsigned mask = __ballot_sync(full, pass[k]);
+                    if (pass[k]) {
+                        int pos = count[k] + __popc(mask & lt_mask);
+                        if (pos < rows.r[k].cap) rbase[k][pos] = j;
+                    }
+                    count[k] += __popc(mask);
                 }
             }
         }
-    }
-    if (lane == 0) {
+        if (have && lane == 0) {
 #pragma unroll
-        for (int k = 0; k < N_ROWS; ++k) {
-            const Row &R = rows.r[k];
-            if (!R.enabled) continue;
-            R.cnt[i] = min(count[k], R.cap);
-            if (count[k] > R.cap) atomicOr(&ctr->err, (unsigned)ERR_OVERFLOW);
-            if (count[k] > ctr->max_row[k]) atomicMax(&ctr->max_row[k], count[k]);
+            for (int k = 0; k < N_ROWS; ++k) {
+                if (!JB_ROW_ON(k)) continue;
+                const Row &R = rows.r[k];
+                R.cnt[i] = min(count[k], R.cap);
+                if (count[k] > R.cap) atomicOr(&ctr->err, (unsigned)ERR_OVERFLOW);
+                if (count[k] > ctr->max_row[k]) atomicMax(&ctr->max_row[k], count[k]);
+            }
         }
     }
+#undef JB_ROW_ON
 }
 
 // ------------------------------------------------------------------------------------------
@@ -250,14 +364,49 @@ void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches) {
 }
 
 void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS], float rmax_all, const int *cell_start,
-                       const float4 *xs, const float2 *lj, const int *orig, const int *sorted_of, const int *excl_ptr,
-                       const int *excl_idx, Counters *ctr, cudaStream_t st, int64_t *launches) {
+                       const float4 *xs, const float4 *xl, const float2 *lj, const int *orig, const int *sorted_of,
+                       const int *excl_ptr, const int *excl_idx, Counters *ctr, cudaStream_t st, int64_t *launches) {
     RowSet rs;
     for (int k = 0; k < N_ROWS; ++k) rs.r[k] = rows[k];
-    const int B = 256;
-    long long threads = (long long)m.n * 32;
-    k_build_rows<<<(unsigned)((threads + B - 1) / B), B, 0, st>>>(m, g, rs, rmax_all, cell_start, xs, lj, orig, sorted_of,
-                                                                 excl_ptr, excl_idx, ctr);
+    // stencil of cells within reach of a cell: gap between cells at offset o is (|o| - 1)_+ cell edges
+    Stencil stn;
+    double cs[3];
+    for (int k = 0; k < 3; ++k) {
+        cs[k] = (double)m.box[k] / g.gn[k];
+        stn.R[k] = std::min(8, (int)std::ceil((double)rmax_all / cs[k]));  // init refuses grids that need more
+    }
+    stn.n_edge = 0;
+    for (int k = 0; k < N_ROWS; ++k) {
+        if (!rows[k].enabled) continue;
+        for (float e : {rows[k].r2min, rows[k].r2max}) {
+            bool seen = e <= 0.f;
+            for (int q = 0; q < stn.n_edge; ++q) seen |= stn.edge2[q] == e;
+            if (!seen && stn.n_edge < 4) stn.edge2[stn.n_edge++] = e;
+            else if (!seen) stn.n_edge = 5;   // cannot happen with the windows of api.cu (<= 4 distinct edges)
+        }
+    }
+    for (int q = stn.n_edge; q < 4; ++q) stn.edge2[q] = -1e30f;
+    const double r2 = (double)rmax_all * rmax_all;
+    for (int a = 0; a < 17; ++a)
+        for (int b = 0; b < 17; ++b) {
+            double gz = std::max(a - 1, 0) * cs[2], gy = std::max(b - 1, 0) * cs[1];
+            double rem = r2 - gz * gz - gy * gy;
+            int v = -1;
+            if (a <= stn.R[2] && b <= stn.R[1] && rem > 0.0) v = std::min(stn.R[0], (int)std::floor(std::sqrt(rem) / cs[0]) + 1);
+            stn.xr[a * 17 + b] = (signed char)v;
+        }
+    int mask = 0;
+    for (int k = 0; k < N_ROWS; ++k) mask |= rows[k].enabled ? (1 << k) : 0;
+#define JB_BUILD(MASK) k_build_rows<MASK><<<(unsigned)g.ncell, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, cell_start, xs, xl, lj, \
+                                                                                    orig, sorted_of, excl_ptr, excl_idx, ctr)
+    switch (mask) {
+        case 0x0F: JB_BUILD(0x0F); break;   // S M L V   (JUMP with Coulomb and LJ jumps)
+        case 0x27: JB_BUILD(0x27); break;   // S M L W   (Coulomb jumps only, R-13)
+        case 0x10: JB_BUILD(0x10); break;   // F         (BAOAB comparator)
+        case 0x01: JB_BUILD(0x01); break;   // S
+        default: JB_BUILD(-1); break;
+    }
+#undef JB_BUILD
     *launches += 1;
 }
 

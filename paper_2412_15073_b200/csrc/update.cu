@@ -7,6 +7,8 @@
 // Chains of different atoms are independent and a jump of type (i,j) changes v_i only
 // (P:L342): one chain per thread, writing nothing but its own v_i -- no cross-atom conflict; several
 // events on one atom are resolved in time order inside its chain.
+#include <cstdlib>
+
 #include "launch.h"
 
 namespace jb {
@@ -82,9 +84,11 @@ __device__ inline void jump_kick(float eps, float sbm, float nx, float ny, float
 // derivative, d = minimum-image x_i - x_j, r
 __device__ inline float fij_coul(const Model &m, const float4 &xi, const float4 &xj, float &dx, float &dy, float &dz,
                                  float &rinv) {
-    dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
-    dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
-    dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
+    float ax, ay, az, bx, by, bz;
+    image_pair1(xi.x, xj.x, m.box[0], m.inv_box[0], ax, bx);
+    image_pair1(xi.y, xj.y, m.box[1], m.inv_box[1], ay, by);
+    image_pair1(xi.z, xj.z, m.box[2], m.inv_box[2], az, bz);
+    dx = ax - bx; dy = ay - by; dz = az - bz;
     float r2 = dx * dx + dy * dy + dz * dz;
     if (r2 >= m.rE2 || r2 <= m.rlo2) { rinv = 0.f; return 0.f; }
     rinv = rsqrtf(r2);
@@ -93,14 +97,16 @@ __device__ inline float fij_coul(const Model &m, const float4 &xi, const float4 
     float e = erfcf(m.alpha * r), ex = expf(-m.alpha2 * r2);
     float u = qq * e * rinv;
     float du = -(u + qq * kTwoOverSqrtPi * m.alpha * ex) * rinv;
-    float dchi, chi = chi_of(r, m, dchi);
+    float dchi, chi = chi_zone(ax, ay, az, bx, by, bz, r2, r, m, dchi);
     return (1.f - chi) * du - dchi * u;
 }
 __device__ inline float fij_lj(const Model &m, const float4 &xi, const float4 &xj, float2 lji, float2 ljj, float &dx,
                                float &dy, float &dz, float &rinv) {
-    dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
-    dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
-    dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
+    float ax, ay, az, bx, by, bz;
+    image_pair1(xi.x, xj.x, m.box[0], m.inv_box[0], ax, bx);
+    image_pair1(xi.y, xj.y, m.box[1], m.inv_box[1], ay, by);
+    image_pair1(xi.z, xj.z, m.box[2], m.inv_box[2], az, bz);
+    dx = ax - bx; dy = ay - by; dz = az - bz;
     float r2 = dx * dx + dy * dy + dz * dz;
     if (r2 >= m.rE2 || r2 <= m.rlo2) { rinv = 0.f; return 0.f; }
     rinv = rsqrtf(r2);
@@ -108,14 +114,24 @@ __device__ inline float fij_lj(const Model &m, const float4 &xi, const float4 &x
     float s = lji.x * ljj.x * rinv, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
     float e4 = lji.y * ljj.y;
     float u = e4 * (s12 - s6), du = e4 * (6.f * s6 - 12.f * s12) * rinv;
-    float dchi, chi = chi_of(r, m, dchi);
+    float dchi, chi = chi_zone(ax, ay, az, bx, by, bz, r2, r, m, dchi);
     return (1.f - chi) * du - dchi * u;
 }
 
 // ---- step (C'): Algorithm 4 + ring (R-11).  x frozen; updates (vx,vy,vz) of atom i. -------------------------
+// G lanes cooperate on one chain.  What a proposal needs from the random stream and from x -- the exponential
+// E, the ring, the partner j, the uniform U and the pair gradient F_ij(x) (x is frozen) -- does not depend on
+// the chain's state (t, v), so lane l evaluates all of that for the l-th next iteration at once (Philox block
+// b + l, the row and position gathers, erfc/exp).  Only the thinning recurrence itself is sequential
+// (B_v -> lambda-bar -> T -> t, v -> accept test); every lane of the group replays it on the
+// broadcast values, so (t, v) stay replicated in registers.  An accepted jump consumes G~ blocks and thereby
+// shifts the block index of the later iterations (R-15): the speculative tail is then dropped and the batch
+// restarted -- accepted jumps are ~1 % of the proposals.  The arithmetic of every iteration is exactly the
+// sequential algorithm's, so the event log equals the oracle's whatever G is.
+template <int G, bool LOG>
 __device__ void chain_C(const Model &m, const UpdateArgs &A, int i, unsigned atom, const float4 &xi, float sbm,
                         float ax, float ay, float az, float H, unsigned stream, unsigned step, float &vx, float &vy,
-                        float &vz, Tally &tl) {
+                        float &vz, Tally &tl, unsigned gmask, int gl) {
     const float eps = m.eps_jump, beta = m.beta;
     const bool bps = isinf(eps);
     const int NM = A.rowM.cnt[i], NL = A.rowL.cnt[i];
@@ -124,63 +140,101 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, int i, unsigned ato
     const float SM = (float)NM * LM, S = SM + (float)NL * LL;
     const float lam0 = bps ? 0.f : (1.f / eps) * beta * kInvSqrt2Pi / sbm;
     const float a2 = ax * ax + ay * ay + az * az;
+    const bool lead = gl == 0;
     float t = 0.f;
     unsigned block = 0;
-    uint32_t w[4];
-    for (int iter = 0;; ++iter) {
-        float tau = H - t;
-        float va = vx * ax + vy * ay + vz * az;
-        float v2 = vx * vx + vy * vy + vz * vz;
-        float Bv = sqrtf(v2 + tau * tau * a2 + 2.f * tau * fmaxf(va, 0.f));
-        float lam = S * (beta * Bv + lam0);
-        philox4x32_10(atom, step, stream, block++, m.key0, m.key1, w);
-        float E = -logf(u01(w[0]));
-        float T = lam > 0.f ? E / lam : INFINITY;
-        if (!(t + T <= H)) {
-            vx += tau * ax; vy += tau * ay; vz += tau * az;
+    int iter = 0;
+    if (!(S > 0.f)) {  // no partner: lambda-bar = 0, the clock never rings
+        vx += H * ax; vy += H * ay; vz += H * az;
+        if (lead) {
             tl.expiries++;
-            log_event(A, step, stream, atom, iter, -1, -1, 0, 0, T, 0.f, 0.f, 0.f);
-            break;
+            if (LOG) log_event(A, step, stream, atom, 0, -1, -1, 0, 0, INFINITY, 0.f, 0.f, 0.f);
         }
-        t += T;
-        vx += T * ax; vy += T * ay; vz += T * az;
-        float ur = u01(w[1]);  // ring pick
-        int ring = (ur * S < SM) ? 0 : 1;
-        if (ring == 0 && NM == 0) ring = 1;
-        if (ring == 1 && NL == 0) ring = 0;
-        const int cnt = ring == 0 ? NM : NL;
+        return;
+    }
+    for (;;) {
+        // ---- state-independent part of iteration (iter + gl), Philox block (block + gl) ----
+        uint32_t w[4];
+        philox4x32_10(atom, step, stream, block + (unsigned)gl, m.key0, m.key1, w);
+        float E_ = -logf(u01(w[0]));
+        int ring_ = (u01(w[1]) * S < SM) ? 0 : 1;  // ring pick
+        if (ring_ == 0 && NM == 0) ring_ = 1;
+        if (ring_ == 1 && NL == 0) ring_ = 0;
+        const int cnt = ring_ == 0 ? NM : NL;
         const int k = (int)__umulhi(w[2], (unsigned)cnt);
-        const int j = ring == 0 ? A.rowM.idx[(size_t)i * A.rowM.cap + k] : A.rowL.idx[(size_t)i * A.rowL.cap + k];
-        const float LY = ring == 0 ? LM : LL;
-        const float U = u01(w[3]);
-        tl.proposals++;
+        const int j_ = ring_ == 0 ? A.rowM.idx[(size_t)i * A.rowM.cap + k] : A.rowL.idx[(size_t)i * A.rowL.cap + k];
+        const float U_ = u01(w[3]);
         float dx, dy, dz, rinv;
-        float fr = fij_coul(m, xi, A.xs[j], dx, dy, dz, rinv);
-        float g = fabsf(fr), p = 0.f, gt = 0.f;
-        int acc = 0, att = 0;
-        if (g > 0.f) {
-            tl.max_gl = fmaxf(tl.max_gl, g / LY);
-            float sg = (fr > 0.f ? rinv : -rinv);  // n = F/|F|
-            float nx = dx * sg, ny = dy * sg, nz = dz * sg;
-            float vn = vx * nx + vy * ny + vz * nz;
-            if (bps) p = fmaxf(vn, 0.f) * g / (LY * Bv);
-            else p = g * theta_of(eps * sbm * vn) / (LY * (Bv * eps * sbm + kInvSqrt2Pi));  // P:L397 with sqrt(beta)
-            tl.max_p = fmaxf(tl.max_p, p);
-            if (U <= p) {
-                if (!bps) gt = gtilde(eps * sbm * vn, atom, step, stream, block, m, att);
-                jump_kick(eps, sbm, nx, ny, nz, gt, vx, vy, vz);
-                acc = 1;
-                tl.accepts++;
-                tl.gt_attempts += att;
+        float fr = fij_coul(m, xi, A.xs[j_], dx, dy, dz, rinv);
+        float g_ = fabsf(fr);
+        float sg = (fr > 0.f ? rinv : -rinv);  // n = F/|F|
+        float nx_ = dx * sg, ny_ = dy * sg, nz_ = dz * sg;
+        const float LY_ = ring_ == 0 ? LM : LL;
+        float gl_ = g_ / LY_;
+        int jo_ = LOG ? A.orig[j_] : 0;
+        // ---- the thinning recurrence over the G staged iterations ----
+        bool finished = false, restart = false;
+#pragma unroll 1
+        for (int l = 0; l < G; ++l) {
+            float E = __shfl_sync(gmask, E_, l, G);
+            float tau = H - t;
+            float va = vx * ax + vy * ay + vz * az;
+            float v2 = vx * vx + vy * vy + vz * vz;
+            float Bv2 = v2 + tau * tau * a2 + 2.f * tau * fmaxf(va, 0.f);
+            float Bv = Bv2 > 0.f ? Bv2 * rsqrtf(Bv2) : 0.f;
+            float lam = S * (beta * Bv + lam0);
+            float T = __fdividef(E, lam);                                         // P:L379 (lam = 0: +inf)
+            if (!(t + T <= H)) {
+                vx += tau * ax; vy += tau * ay; vz += tau * az;
+                if (lead) {
+                    tl.expiries++;
+                    if (LOG) log_event(A, step, stream, atom, iter, -1, -1, 0, 0, T, 0.f, 0.f, 0.f);
+                }
+                finished = true;
+                break;
             }
+            t += T;
+            vx += T * ax; vy += T * ay; vz += T * az;
+            float g = __shfl_sync(gmask, g_, l, G), goL = __shfl_sync(gmask, gl_, l, G), U = __shfl_sync(gmask, U_, l, G);
+            if (lead) { tl.proposals++; tl.max_gl = fmaxf(tl.max_gl, goL); }
+            float p = 0.f, gt = 0.f;
+            int acc = 0, att = 0;
+            // p <= g / L_Y always (Theta(eta) <= eta_+ + 1/sqrt(2 pi), eta <= eps sqrt(beta m) B_v): most proposals
+            // are rejected on that bound alone; p itself is evaluated when it can matter (or is logged)
+            if (g > 0.f && (LOG || U <= goL * 1.0001f)) {
+                float nx = __shfl_sync(gmask, nx_, l, G), ny = __shfl_sync(gmask, ny_, l, G), nz = __shfl_sync(gmask, nz_, l, G);
+                float LY = __shfl_sync(gmask, LY_, l, G);
+                float vn = vx * nx + vy * ny + vz * nz;
+                if (bps) p = fmaxf(vn, 0.f) * g / (LY * Bv);
+                else p = g * theta_of(eps * sbm * vn) / (LY * (Bv * eps * sbm + kInvSqrt2Pi));  // P:L397 with sqrt(beta)
+                if (lead) tl.max_p = fmaxf(tl.max_p, p);
+                if (U <= p) {
+                    unsigned b2 = block + (unsigned)l + 1u;
+                    if (!bps) gt = gtilde(eps * sbm * vn, atom, step, stream, b2, m, att);
+                    jump_kick(eps, sbm, nx, ny, nz, gt, vx, vy, vz);
+                    acc = 1;
+                    if (lead) { tl.accepts++; tl.gt_attempts += att; }
+                    block = b2;  // the next iteration's block follows the sampler's
+                    restart = true;
+                }
+            }
+            if (LOG) {
+                int ring = __shfl_sync(gmask, ring_, l, G), jo = __shfl_sync(gmask, jo_, l, G);
+                if (lead) log_event(A, step, stream, atom, iter, ring, jo, acc, att, T, p, U, gt);
+            }
+            ++iter;
+            if (restart) break;
         }
-        log_event(A, step, stream, atom, iter, ring, A.orig[j], acc, att, T, p, U, gt);
+        if (finished) break;
+        if (!restart) block += (unsigned)G;
     }
 }
 
 // ---- step (J'): Algorithm 5 (R-14) ---------------------------------------------------------------------------
+// Rare (LJ carriers only, ~0.15 proposals per fs): every lane of the group runs the same sequential chain.
 __device__ void chain_J(const Model &m, const UpdateArgs &A, int i, unsigned atom, const float4 &xi, float2 lji,
-                        float sbm, float H, unsigned stream, unsigned step, float &vx, float &vy, float &vz, Tally &tl) {
+                        float sbm, float H, unsigned stream, unsigned step, float &vx, float &vy, float &vz, Tally &tl,
+                        bool lead) {
     if (!(lji.y > 0.f)) return;
     const int NV = A.rowV.cnt[i];
     if (NV == 0) return;
@@ -195,33 +249,34 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, int i, unsigned ato
         float E = -logf(u01(w[0]));
         float T = lam > 0.f ? E / lam : INFINITY;
         if (!(t + T <= H)) {
-            tl.expiries++;
-            log_event(A, step, stream, atom, iter, -1, -1, 0, 0, T, 0.f, 0.f, 0.f);
+            if (lead) {
+                tl.expiries++;
+                log_event(A, step, stream, atom, iter, -1, -1, 0, 0, T, 0.f, 0.f, 0.f);
+            }
             break;
         }
         t += T;
         const int k = (int)__umulhi(w[1], (unsigned)NV);
         const int j = A.rowV.idx[(size_t)i * A.rowV.cap + k];
         const float U = u01(w[2]);
-        tl.proposals++;
+        if (lead) tl.proposals++;
         float dx, dy, dz, rinv;
         float fr = fij_lj(m, xi, A.xs[j], lji, A.lj[j], dx, dy, dz, rinv);
         float g = fabsf(fr), p = 0.f;
         int acc = 0;
         if (g > 0.f) {
-            tl.max_gl = fmaxf(tl.max_gl, g / L);
             float sg = (fr > 0.f ? rinv : -rinv);
             float nx = dx * sg, ny = dy * sg, nz = dz * sg;
             float vF = (vx * nx + vy * ny + vz * nz) * g;
             p = fmaxf(vF, 0.f) / (vv * L);
-            tl.max_p = fmaxf(tl.max_p, p);
+            if (lead) { tl.max_gl = fmaxf(tl.max_gl, g / L); tl.max_p = fmaxf(tl.max_p, p); }
             if (U <= p) {  // reflection (5)
                 jump_kick(INFINITY, sbm, nx, ny, nz, 0.f, vx, vy, vz);
                 acc = 1;
-                tl.accepts++;
+                if (lead) tl.accepts++;
             }
         }
-        log_event(A, step, stream, atom, iter, 2, A.orig[j], acc, 0, T, p, U, 0.f);
+        if (lead) log_event(A, step, stream, atom, iter, 2, A.orig[j], acc, 0, T, p, U, 0.f);
     }
 }
 
@@ -233,11 +288,16 @@ __device__ inline double wrap1d(double x, double L) {
 }
 
 // ---- the fused per-atom update: up to two velocity half-phases, then A O A + wrap ----------------------------
-template <bool JUMPS>
+// G lanes per atom (a power of two <= 32): they share the jump chains (see chain_C); lane 0 of the group does the
+// A-O-A part and all the stores.
+template <bool JUMPS, int G, bool LOG>
 __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
     const unsigned full = 0xffffffffu;
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const bool live = i < m.n;
+    const int gt_id = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = gt_id / G, gl = gt_id % G;
+    const int lane = threadIdx.x & 31;
+    const unsigned gmask = (G == 32) ? full : (((1u << G) - 1u) << (lane & ~(G - 1)));
+    const bool live = i < m.n, lead = gl == 0;
     Tally tl = {0u, 0u, 0u, 0u, 0.f, 0.f};
     float disp2 = 0.f;
     bool bad = false;
@@ -260,13 +320,13 @@ __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
                 vx += P.H * ax; vy += P.H * ay; vz += P.H * az;
             } else {
                 const float2 lji = A.lj[i];
-                if (P.reverse && P.lj) chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl);
-                if (P.coul) chain_C(m, A, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl);
+                if (P.reverse && P.lj) chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
+                if (P.coul) chain_C<G, LOG>(m, A, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl, gmask, gl);
                 else if (P.use_grad) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
-                if (!P.reverse && P.lj) chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl);
+                if (!P.reverse && P.lj) chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
             }
         }
-        if (A.do_aoa) {
+        if (A.do_aoa && lead) {
             // positions are integrated in fp64 as hi + lo (hi = the fp32 value every pair kernel reads):
             // fp32 rounding of x (ulp(18 A) = 2e-6 A) through the stiff O-H bonds is otherwise the
             // largest noise source of the whole step
@@ -297,7 +357,7 @@ __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
             bad = !(isfinite(x) && isfinite(y) && isfinite(z));
         }
         bad = bad || !(isfinite(vx) && isfinite(vy) && isfinite(vz));
-        A.vs[i] = make_float4(vx, vy, vz, v4.w);
+        if (lead) A.vs[i] = make_float4(vx, vy, vz, v4.w);
     }
     // warp-level reduction of the statistics, then a few integer atomics per warp
     unsigned err = 0;
@@ -306,7 +366,6 @@ __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
     if (tl.max_p > 1.f + 1e-4f || tl.max_gl > 1.f + 1e-4f) err |= ERR_BOUND;
     unsigned d2b = __reduce_max_sync(full, __float_as_uint(disp2));
     err = __reduce_or_sync(full, err);
-    const int lane = threadIdx.x & 31;
     if (JUMPS) {
         unsigned np = __reduce_add_sync(full, tl.proposals), na = __reduce_add_sync(full, tl.accepts);
         unsigned ng = __reduce_add_sync(full, tl.gt_attempts), ne = __reduce_add_sync(full, tl.expiries);
@@ -384,10 +443,36 @@ __global__ void k_kinetic(int n, const float4 *__restrict__ vs, const float2 *__
     out[i] = 0.5 * v2 / (double)mi[i].x;  // (1/2) m v^2 / KCAL with mi.x = KCAL / m
 }
 
-void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st, int64_t *launches) {
+template <int G>
+static void update_dispatch(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st) {
     const int B = 128;
-    if (jumps) k_update<true><<<(m.n + B - 1) / B, B, 0, st>>>(m, A);
-    else k_update<false><<<(m.n + B - 1) / B, B, 0, st>>>(m, A);
+    const unsigned grid = (unsigned)(((long long)m.n * G + B - 1) / B);
+    if (!jumps) k_update<false, 1, false><<<(m.n + B - 1) / B, B, 0, st>>>(m, A);
+    else if (A.events) k_update<true, G, true><<<grid, B, 0, st>>>(m, A);
+    else k_update<true, G, false><<<grid, B, 0, st>>>(m, A);
+}
+// lanes per jump chain: as many as keep the grid within about two full waves of resident threads
+// (148 SMs x 2048); JUMP_B200_LANES overrides (1, 4, 8, 16) for experiments
+static int lanes_per_chain(int n) {
+    static int forced = -1;
+    if (forced < 0) {
+        const char *e = getenv("JUMP_B200_LANES");
+        forced = e ? atoi(e) : 0;
+    }
+    if (forced == 1 || forced == 4 || forced == 8 || forced == 16) return forced;
+    const long long budget = 2ll * 148 * 2048;
+    if ((long long)n * 16 <= budget) return 16;
+    if ((long long)n * 8 <= budget) return 8;
+    if ((long long)n * 4 <= budget) return 4;
+    return 1;
+}
+void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st, int64_t *launches) {
+    switch (jumps ? lanes_per_chain(m.n) : 1) {
+        case 16: update_dispatch<16>(m, A, jumps, st); break;
+        case 8: update_dispatch<8>(m, A, jumps, st); break;
+        case 4: update_dispatch<4>(m, A, jumps, st); break;
+        default: update_dispatch<1>(m, A, jumps, st); break;
+    }
     *launches += 1;
 }
 void launch_writeback(int n, const float4 *xs, const float4 *vs, const int *orig, float *pos, float *vel, cudaStream_t st,
