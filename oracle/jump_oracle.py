@@ -145,7 +145,7 @@ def make_params(n_atoms, box, r_short, r_long, r_switch=0.5, r_mid=None, ewald_a
     b = np.broadcast_to(np.asarray(box, dtype=np.float64), (3,))
     p.box[0], p.box[1], p.box[2] = float(b[0]), float(b[1]), float(b[2])
     p.r_short, p.r_switch, p.r_long = float(r_short), float(r_switch), float(r_long)
-    p.r_mid = float(r_short + 1.0 if r_mid is None else r_mid)
+    p.r_mid = float(r_short + 2.0 if r_mid is None else r_mid)
     p.ewald_alpha = float(ewald_alpha)
     p.dt_fs, p.gamma_per_ps, p.temperature_K = float(dt_fs), float(gamma_per_ps), float(temperature_K)
     p.eps_jump, p.skin, p.cell_edge = float(eps_jump), float(skin), float(cell_edge)

@@ -50,6 +50,9 @@ struct jump_ctx {
     int64_t prof_n[4];
 };
 enum { PROF_PAIR = 0, PROF_BONDED = 1, PROF_UPDATE = 2, PROF_BUILD = 3 };
+// a gradient held as the sum of two arrays (b may be NULL): the fused F0 launch leaves pair and bonded parts apart
+struct GradRef { const float4 *a, *b; };
+static GradRef gr(const float4 *a, const float4 *b = nullptr) { return GradRef{a, b}; }
 
 static void prof_begin(jump_ctx *c, int cat) {
     if (!c->prof) return;
@@ -259,13 +262,37 @@ static int compute_short_nb(jump_ctx *c, float4 *out, bool energy = false) {
     CK(cudaGetLastError());
     return 0;
 }
+static int bonded_only(jump_ctx *c) {  // fbond at the current positions
+    prof_begin(c, PROF_BONDED);
+    launch_bonded_lanes(c->m, c->topo, c->xs, c->xl, c->orig, c->sorted_of, c->fbond, c->st, &c->launches);
+    prof_end(c, PROF_BONDED);
+    CK(cudaGetLastError());
+    return 0;
+}
+// F0 kept as fnb + fbond (the integrator adds the two)
 static int compute_f0(jump_ctx *c) {
+    int r = compute_short_nb(c, c->fnb);
+    if (r) return r;
+    c->f0_valid = true;
+    return bonded_only(c);
+}
+static GradRef gr_f0(const jump_ctx *c) { return gr(c->fnb, c->fbond); }
+static int ensure_f0(jump_ctx *c) { return c->f0_valid ? 0 : compute_f0(c); }
+// F0 materialised in c->f0 (observers only)
+static int compute_f0_sum(jump_ctx *c) {
     int r = compute_short_nb(c, c->fnb);
     if (r) return r;
     c->f0_valid = true;
     return bonded(c, c->fnb, c->f0, c->fbond);
 }
-static int ensure_f0(jump_ctx *c) { return c->f0_valid ? 0 : compute_f0(c); }
+// unsplit force to r_long as ftmp2 + fbond (BAOAB comparator); invalidates F0
+static int compute_full_split(jump_ctx *c) {
+    pair(c, ROW_F, W_FULL, W_FULL, c->ftmp2, 0, false);
+    CK(cudaGetLastError());
+    c->f0_valid = false;
+    return bonded_only(c);
+}
+static GradRef gr_full(const jump_ctx *c) { return gr(c->ftmp2, c->fbond); }
 static int compute_long(jump_ctx *c, float4 *out) {
     int wLJ = lj_jumps(c) ? W_LONG : W_NONE;
     pair(c, ROW_M, W_LONG, wLJ, out, 0, false);
@@ -292,12 +319,12 @@ static Phase ph_jump(const jump_ctx *c, double H, bool grad, bool reverse, int s
 }
 
 // up to two velocity half-phases, then (aoa) A O A + wrap, step counter and the scheduled rebuild (C.3 steps 3-6)
-static int run_update(jump_ctx *c, const Phase &p0, const float4 *g0, const Phase &p1, const float4 *g1, bool aoa) {
+static int run_update(jump_ctx *c, const Phase &p0, GradRef g0, const Phase &p1, GradRef g1, bool aoa) {
     UpdateArgs A;
     memset(&A, 0, sizeof A);
-    A.ph[0] = p0; A.ph[1] = p1; A.grad[0] = g0; A.grad[1] = g1;
-    if (!g0) A.ph[0].use_grad = 0;
-    if (!g1) A.ph[1].use_grad = 0;
+    A.ph[0] = p0; A.ph[1] = p1; A.grad[0] = g0.a; A.grad[1] = g1.a; A.grad_b[0] = g0.b; A.grad_b[1] = g1.b;
+    if (!g0.a) A.ph[0].use_grad = 0;
+    if (!g1.a) A.ph[1].use_grad = 0;
     A.do_aoa = aoa ? 1 : 0;
     A.half_dt = (float)(0.5 * c->dt); A.c1 = c->c1; A.c2 = c->c2; A.o_step = (unsigned)c->step;
     A.xs = c->xs; A.xs_out = c->xs_nxt; A.vs = c->vs; A.xl = c->xl; A.mi = c->mi; A.lj = c->lj; A.orig = c->orig; A.x_build = c->x_build;
@@ -349,12 +376,12 @@ extern "C" int jump_step(jump_ctx *c, int32_t n_steps) {
         int64_t st = c->step;
         Phase open = ph_jump(c, H, true, false, 1, 2, st);
         Phase close_prev = s > 0 ? ph_jump(c, H, true, true, 4, 3, st - 1) : ph_none();
-        int r = run_update(c, close_prev, c->f0, open, c->f0, true);
+        int r = run_update(c, close_prev, gr_f0(c), open, gr_f0(c), true);
         if (r) return r;
         r = compute_f0(c);
         if (r) return r;
     }
-    int r = run_update(c, ph_jump(c, H, true, true, 4, 3, c->step - 1), c->f0, ph_none(), nullptr, false);
+    int r = run_update(c, ph_jump(c, H, true, true, 4, 3, c->step - 1), gr_f0(c), ph_none(), gr(nullptr), false);
     if (r) return r;
     return writeback(c);
 }
@@ -363,15 +390,15 @@ extern "C" int baoab_step(jump_ctx *c, int32_t n_steps) {
     if (!c || n_steps < 0) return JUMP_E_ARG;
     if (n_steps == 0) return 0;
     const double H = 0.5 * c->dt;
-    int r = compute_full(c, c->ftmp);
+    int r = compute_full_split(c);
     if (r) return r;
     for (int s = 0; s < n_steps; ++s) {
-        r = run_update(c, s > 0 ? ph_kick(H) : ph_none(), c->ftmp, ph_kick(H), c->ftmp, true);
+        r = run_update(c, s > 0 ? ph_kick(H) : ph_none(), gr_full(c), ph_kick(H), gr_full(c), true);
         if (r) return r;
-        r = compute_full(c, c->ftmp);
+        r = compute_full_split(c);
         if (r) return r;
     }
-    r = run_update(c, ph_kick(H), c->ftmp, ph_none(), nullptr, false);
+    r = run_update(c, ph_kick(H), gr_full(c), ph_none(), gr(nullptr), false);
     if (r) return r;
     return writeback(c);  // F0 is recomputed on demand (f0_valid)
 }
@@ -385,15 +412,15 @@ extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
     if (r) return r;
     for (int o = 0; o < n_outer; ++o) {
         Phase outer[2];
-        const float4 *gout[2];
+        GradRef gout[2];
         for (int half = 0; half < 2; ++half) {
             if (half == 1) {  // inner loop: n x BAOAB_delta with F_in; the first opening kick rides with outer[0]
                 for (int s = 0; s < n; ++s) {
-                    const float4 *fin = paper ? c->fbond : c->f0;
+                    GradRef fin = paper ? gr(c->fbond) : gr_f0(c);
                     if (s == 0) r = run_update(c, outer[0], gout[0], ph_kick(H), fin, true);
                     else r = run_update(c, ph_kick(H), fin, ph_kick(H), fin, true);
                     if (r) return r;
-                    r = paper ? bonded(c, nullptr, nullptr, c->fbond) : compute_f0(c);
+                    r = paper ? bonded_only(c) : compute_f0(c);
                     if (r) return r;
                 }
                 if (paper) { r = compute_f0(c); if (r) return r; }
@@ -409,14 +436,14 @@ extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
                     CK(cudaGetLastError());
                 }
                 outer[half] = ph_kick(0.5 * D);
-                gout[half] = fl;
+                gout[half] = gr(fl);
             } else {
-                gout[half] = paper ? c->fnb : nullptr;
+                gout[half] = gr(paper ? c->fnb : nullptr);
                 outer[half] = half == 0 ? ph_jump(c, 0.5 * D, paper, false, 5, 6, c->outer)
                                         : ph_jump(c, 0.5 * D, paper, true, 8, 7, c->outer);
             }
         }
-        const float4 *fin = paper ? c->fbond : c->f0;
+        GradRef fin = paper ? gr(c->fbond) : gr_f0(c);
         r = run_update(c, ph_kick(H), fin, outer[1], gout[1], false);
         if (r) return r;
         c->outer++;
@@ -428,7 +455,7 @@ extern "C" int jump_half(jump_ctx *c, double H_ps, int32_t with_accel, int64_t s
     if (!c) return JUMP_E_ARG;
     int r = ensure_f0(c);
     if (r) return r;
-    r = run_update(c, ph_jump(c, H_ps, with_accel != 0, false, 1, 2, step), c->f0, ph_none(), nullptr, false);
+    r = run_update(c, ph_jump(c, H_ps, with_accel != 0, false, 1, 2, step), gr_f0(c), ph_none(), gr(nullptr), false);
     if (r) return r;
     return writeback(c);
 }
@@ -637,7 +664,7 @@ extern "C" int jump_get_forces(jump_ctx *c, int32_t which, float *d_out) {
     int r = 0;
     const float4 *src = nullptr;
     switch (which) {
-        case 0: r = compute_f0(c); src = c->f0; break;
+        case 0: r = compute_f0_sum(c); src = c->f0; break;
         case 1: r = compute_full(c, c->ftmp); src = c->ftmp; break;
         case 2: r = compute_long(c, c->ftmp); src = c->ftmp; break;
         case 3: r = bonded(c, nullptr, nullptr, c->fbond); src = c->fbond; break;

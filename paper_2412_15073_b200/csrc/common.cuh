@@ -103,6 +103,25 @@ __device__ inline float min_image1(float xi, float xj, float L, float invL) {
     return a - b;
 }
 
+// erfc(x) exp(x^2) for 0 <= x <= 4.3 (alpha r never exceeds 3.8 (1 + skin / r_long)): degree-8 polynomial in
+// t = 1 / (1 + x/2), a relative-weighted Chebyshev least-squares fit made for this file (max relative error
+// 6e-8 in exact arithmetic, 2.6e-7 evaluated in fp32 -- the accuracy of erfcf).  erfc(alpha r) is then
+// erfcx_poly(alpha r) * exp(-alpha^2 r^2) with the exponential the Coulomb derivative needs anyway:
+// a third of the pair kernel's instructions were erfcf's.
+__device__ inline float erfcx_poly(float x) {
+    float t = __frcp_rn(fmaf(0.5f, x, 1.f));
+    float p = -4.621402847e-02f;
+    p = fmaf(p, t, 3.202601290e-01f);
+    p = fmaf(p, t, -8.488328818e-01f);
+    p = fmaf(p, t, 9.638187580e-01f);
+    p = fmaf(p, t, -3.656822066e-01f);
+    p = fmaf(p, t, 4.560536203e-01f);
+    p = fmaf(p, t, 2.321311377e-01f);
+    p = fmaf(p, t, 2.888640654e-01f);
+    p = fmaf(p, t, -3.985373802e-04f);
+    return p;
+}
+
 // chi (R-3): quintic smootherstep on [rc-h, rc]; returns chi, writes dchi/dr.
 // Outside the switching zone chi is 0 or 1 and nothing else is computed.  Inside it the argument
 // u = (r - r_lo)/h is formed as (r^2 - r_lo^2) / (h (r + r_lo)) with r^2 - r_lo^2 in fp64 from the exact

@@ -23,11 +23,9 @@ __device__ inline float weighted_u(float chi, float u) {
 }
 
 template <int WC, int WLJ, bool ENERGY>
-__global__ void __launch_bounds__(256) k_pair(Model m, Row row, const float4 *__restrict__ xs,
-                                              const float2 *__restrict__ lj, float4 *__restrict__ out, int accumulate) {
+__device__ inline void pair_warp(const Model &m, const Row &row, const float4 *__restrict__ xs,
+                                 const float2 *__restrict__ lj, float4 *__restrict__ out, int accumulate, int i, int lane) {
     const unsigned full = 0xffffffffu;
-    int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (i >= m.n) return;
     const float4 xi = xs[i];
     const float qi = (float)kCoulomb * xi.w;
     const float2 lji = lj[i];
@@ -52,7 +50,7 @@ __global__ void __launch_bounds__(256) k_pair(Model m, Row row, const float4 *__
         if (WC == W_SHORT || WC == W_LONG || WLJ == W_SHORT || WLJ == W_LONG) chi = chi_zone(ax, ay, az, bx, by, bz, r2, r, m, dchi);
         if (WC != W_NONE && r2 < cutC2) {
             float qq = qi * xj.w;
-            float e = erfcf(m.alpha * r), ex = expf(-m.alpha2 * r2);
+            float ex = expf(-m.alpha2 * r2), e = ex * erfcx_poly(m.alpha * r);
             float u = qq * e * rinv;
             float du = -(u + qq * kTwoOverSqrtPi * m.alpha * ex) * rinv;  // u'
             fr += weighted_du<WC>(chi, dchi, u, du);
@@ -84,6 +82,14 @@ __global__ void __launch_bounds__(256) k_pair(Model m, Row row, const float4 *__
         if (accumulate) { float4 p = out[i]; o.x += p.x; o.y += p.y; o.z += p.z; o.w += p.w; }
         out[i] = o;
     }
+}
+
+template <int WC, int WLJ, bool ENERGY>
+__global__ void __launch_bounds__(256) k_pair(Model m, Row row, const float4 *__restrict__ xs,
+                                              const float2 *__restrict__ lj, float4 *__restrict__ out, int accumulate) {
+    int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (i >= m.n) return;
+    pair_warp<WC, WLJ, ENERGY>(m, row, xs, lj, out, accumulate, i, lane);
 }
 
 // Harmonic bonds k (r-r0)^2 and angles k (theta-theta0)^2 (R-2), one thread per atom over the terms
@@ -157,6 +163,85 @@ __global__ void k_bonded(Model m, Topo t, const float4 *__restrict__ xs, const f
     }
 }
 
+// The same bonded terms with BONDED_LANES lanes per atom (lane l takes the terms l, l + BONDED_LANES, ... of the
+// atom's bond-then-angle list; the partial sums are combined by shuffles in a fixed order: deterministic).
+constexpr int BONDED_LANES = 4;
+__device__ inline void bonded_term(const Model &m, const Topo &t, const float4 *__restrict__ xs, const float4 *__restrict__ xl,
+                                   const int *__restrict__ sorted_of, int o, const D3 &xi, int term, int nb, double &gx,
+                                   double &gy, double &gz, double &en) {
+    if (term < nb) {
+        const int b = t.bptr[o] + term;
+        D3 xj = full_pos(xs, xl, sorted_of[t.bother[b]]);
+        double dx = min_image_d(xi.x, xj.x, m.box[0]);
+        double dy = min_image_d(xi.y, xj.y, m.box[1]);
+        double dz = min_image_d(xi.z, xj.z, m.box[2]);
+        double r = sqrt(dx * dx + dy * dy + dz * dz), dr = r - (double)t.br0[b], k = (double)t.bk[b];
+        double f = 2.0 * k * dr / r;
+        gx += f * dx; gy += f * dy; gz += f * dz;
+        en += 0.5 * k * dr * dr;
+        return;
+    }
+    const int a = t.aptr[o] + (term - nb);
+    const int role = t.arole[a];
+    D3 xa = full_pos(xs, xl, sorted_of[t.aa[a]]), xb = full_pos(xs, xl, sorted_of[t.ab[a]]);
+    D3 xv = role == 1 ? xi : xa;
+    D3 xe1 = role == 1 ? xa : xi;
+    D3 xe2 = xb;
+    double u[3], w[3];
+    u[0] = min_image_d(xe1.x, xv.x, m.box[0]);
+    u[1] = min_image_d(xe1.y, xv.y, m.box[1]);
+    u[2] = min_image_d(xe1.z, xv.z, m.box[2]);
+    w[0] = min_image_d(xe2.x, xv.x, m.box[0]);
+    w[1] = min_image_d(xe2.y, xv.y, m.box[1]);
+    w[2] = min_image_d(xe2.z, xv.z, m.box[2]);
+    double lu = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]), lw = sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
+    double ct = (u[0] * w[0] + u[1] * w[1] + u[2] * w[2]) / (lu * lw);
+    ct = fmin(1.0, fmax(-1.0, ct));
+    double th = acos(ct), st = fmax(sqrt(1.0 - ct * ct), 1e-12);
+    double dth = th - (double)t.at0[a], k = (double)t.ak[a], dU = 2.0 * k * dth;
+    double g[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        double gi = -dU * (w[c] / lw - ct * u[c] / lu) / (lu * st);
+        if (role == 1) {
+            double gk = -dU * (u[c] / lu - ct * w[c] / lw) / (lw * st);
+            g[c] = -(gi + gk);
+        } else g[c] = gi;
+    }
+    gx += g[0]; gy += g[1]; gz += g[2];
+    en += k * dth * dth * (1.0 / 3.0);
+}
+__device__ inline void bonded_lanes(const Model &m, const Topo &t, const float4 *__restrict__ xs, const float4 *__restrict__ xl,
+                                    const int *__restrict__ orig, const int *__restrict__ sorted_of,
+                                    float4 *__restrict__ out_bond, int i, int gl, unsigned gmask) {
+    double gx = 0., gy = 0., gz = 0., en = 0.;
+    if (i < m.n) {
+        const int o = orig[i];
+        const D3 xi = full_pos(xs, xl, i);
+        const int nb = t.bptr[o + 1] - t.bptr[o], nt = nb + t.aptr[o + 1] - t.aptr[o];
+        for (int term = gl; term < nt; term += BONDED_LANES) bonded_term(m, t, xs, xl, sorted_of, o, xi, term, nb, gx, gy, gz, en);
+    }
+#pragma unroll
+    for (int off = 1; off < BONDED_LANES; off <<= 1) {
+        gx += __shfl_xor_sync(gmask, gx, off);
+        gy += __shfl_xor_sync(gmask, gy, off);
+        gz += __shfl_xor_sync(gmask, gz, off);
+        en += __shfl_xor_sync(gmask, en, off);
+    }
+    if (gl == 0 && i < m.n) out_bond[i] = make_float4((float)gx, (float)gy, (float)gz, (float)en);
+}
+
+// bonded gradient alone, BONDED_LANES lanes per atom (a fused pair + bonded launch was tried: the fp64 bonded code
+// raises the register count of the whole kernel and halves the occupancy of the pair warps -- 32 us instead of 20 + 4)
+__global__ void __launch_bounds__(128) k_bonded_lanes(Model m, Topo t, const float4 *__restrict__ xs,
+                                                      const float4 *__restrict__ xl, const int *__restrict__ orig,
+                                                      const int *__restrict__ sorted_of, float4 *__restrict__ out_bond) {
+    const int gt = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    const int i = gt / BONDED_LANES, gl = gt % BONDED_LANES;
+    const unsigned gmask = ((1u << BONDED_LANES) - 1u) << (lane & ~(BONDED_LANES - 1));
+    bonded_lanes(m, t, xs, xl, orig, sorted_of, out_bond, i, gl, gmask);
+}
+
 // out[orig[i]] = f[i].xyz  (sorted -> caller order)
 __global__ void k_unsort3(int n, const float4 *__restrict__ f, const int *__restrict__ orig, float *__restrict__ out) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -210,6 +295,13 @@ int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *x
 #undef JB_CASE
     *launches -= 1;
     return -1;
+}
+
+void launch_bonded_lanes(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig,
+                         const int *sorted_of, float4 *out_bond, cudaStream_t st, int64_t *launches) {
+    const int B = 128;
+    k_bonded_lanes<<<(unsigned)(((long long)m.n * BONDED_LANES + B - 1) / B), B, 0, st>>>(m, t, xs, xl, orig, sorted_of, out_bond);
+    *launches += 1;
 }
 
 void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig, const int *sorted_of,

@@ -19,7 +19,8 @@ struct SortArgs {
 
 struct UpdateArgs {
     Phase ph[2];
-    const float4 *grad[2];
+    const float4 *grad[2];   // gradient of each phase = grad + grad_b (grad_b may be NULL)
+    const float4 *grad_b[2];
     int do_aoa;
     float half_dt, c1, c2;  // delta/2 (ps), exp(-gamma delta), sqrt(1 - c1^2)
     unsigned o_step;        // Philox step index of the O part
@@ -42,6 +43,8 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
                        const int *excl_ptr, const int *excl_idx, Counters *ctr, cudaStream_t st, int64_t *launches);
 int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *xs, const float2 *lj, float4 *out,
                 int accumulate, bool energy, cudaStream_t st, int64_t *launches);
+void launch_bonded_lanes(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig,
+                         const int *sorted_of, float4 *out_bond, cudaStream_t st, int64_t *launches);
 void launch_count_pairs(const Model &m, const Row &row, const float4 *xs, float rc2, unsigned long long *out,
                         cudaStream_t st, int64_t *launches);
 void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig, const int *sorted_of,

@@ -94,7 +94,7 @@ __device__ inline float fij_coul(const Model &m, const float4 &xi, const float4 
     rinv = rsqrtf(r2);
     float r = r2 * rinv;
     float qq = (float)kCoulomb * xi.w * xj.w;
-    float e = erfcf(m.alpha * r), ex = expf(-m.alpha2 * r2);
+    float ex = expf(-m.alpha2 * r2), e = ex * erfcx_poly(m.alpha * r);
     float u = qq * e * rinv;
     float du = -(u + qq * kTwoOverSqrtPi * m.alpha * ex) * rinv;
     float dchi, chi = chi_zone(ax, ay, az, bx, by, bz, r2, r, m, dchi);
@@ -180,10 +180,9 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, int i, unsigned ato
             float tau = H - t;
             float va = vx * ax + vy * ay + vz * az;
             float v2 = vx * vx + vy * vy + vz * vz;
-            float Bv2 = v2 + tau * tau * a2 + 2.f * tau * fmaxf(va, 0.f);
-            float Bv = Bv2 > 0.f ? Bv2 * rsqrtf(Bv2) : 0.f;
+            float Bv = sqrtf(v2 + tau * tau * a2 + 2.f * tau * fmaxf(va, 0.f));
             float lam = S * (beta * Bv + lam0);
-            float T = __fdividef(E, lam);                                         // P:L379 (lam = 0: +inf)
+            float T = E / lam;   // P:L379 (lam = 0: +inf).  IEEE sqrt and division: t + T <= H is a fragile decision (R-17)
             if (!(t + T <= H)) {
                 vx += tau * ax; vy += tau * ay; vz += tau * az;
                 if (lead) {
@@ -314,6 +313,7 @@ __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
             float ax = 0.f, ay = 0.f, az = 0.f;
             if (P.use_grad) {  // a = -M^-1 F
                 float4 g = A.grad[ph][i];
+                if (A.grad_b[ph]) { float4 b = A.grad_b[ph][i]; g.x = b.x + g.x; g.y = b.y + g.y; g.z = b.z + g.z; }
                 ax = -mi.x * g.x; ay = -mi.x * g.y; az = -mi.x * g.z;
             }
             if (P.kind == 1 || !JUMPS) {

@@ -91,4 +91,4 @@ def test_no_gpu_means_a_loud_failure_not_a_fallback(binding):
 
 def test_make_params_defaults(binding):
     p = binding.make_params(648, 18.64, 5.0, 9.0)
-    assert p.r_mid == 6.0 and p.flags == 3 and p.n_inner == 4 and list(p.box) == [18.64] * 3
+    assert p.r_mid == 7.0 and p.flags == 3 and p.n_inner == 4 and list(p.box) == [18.64] * 3
