@@ -762,19 +762,28 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
     const double LM = LM_of(c, i), LL = LL_of(c, i);
     const double SM = (double)NM * LM, S = SM + (double)NL * LL; /* P:L424 */
     double t = 0.0;
-    uint32_t block = 0;
+    uint32_t block = 0;  /* proposal k of the chain draws Philox block k of its stream ...                     */
+    uint32_t gblock = 0; /* ... and the G~ attempts draw blocks 0, 1, ... of stream + 16 (R-15)                 */
     uint32_t w[4];
+    /* R-11: the bound is "re-evaluated after each jump" (P:L161): B_v bounds |v_i| on the whole of [t, delta/2]
+     * (P:L373), so it and lambda-bar are evaluated at t = 0 and after every ACCEPTED jump and held in between. */
+    int fresh = 1;
+    double Bv = 0.0, lam = 0.0;
+    const double a2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
     for (int iter = 0;; ++iter) {
         orc_event ev;
         memset(&ev, 0, sizeof ev);
         ev.step = (int32_t)step; ev.stream = stream; ev.atom = i; ev.iter = iter; ev.ring = -1; ev.j = -1;
         double mg = 1e300;
         double tau = H - t;
-        double va = v[0] * a[0] + v[1] * a[1] + v[2] * a[2];
-        double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2], a2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
-        double Bv = sqrt(v2 + tau * tau * a2 + 2.0 * tau * (va > 0.0 ? va : 0.0)); /* P:L373 */
-        double lam = bps ? S * beta * Bv
-                         : S * (beta * Bv + (1.0 / eps) * beta * ORC_INV_SQRT_2PI / sbm); /* P:L374 */
+        if (fresh) {
+            double va = v[0] * a[0] + v[1] * a[1] + v[2] * a[2];
+            double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
+            Bv = sqrt(v2 + tau * tau * a2 + 2.0 * tau * (va > 0.0 ? va : 0.0)); /* P:L373 */
+            lam = bps ? S * beta * Bv
+                      : S * (beta * Bv + (1.0 / eps) * beta * ORC_INV_SQRT_2PI / sbm); /* P:L374 */
+            fresh = 0;
+        }
         chain_block(c, i, step, stream, block++, w);
         double E = -log(orc_u01(w[0]));
         double T = lam > 0.0 ? E / lam : INFINITY; /* P:L379 */
@@ -818,11 +827,12 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
             if (U <= p) { /* P:L401 */
                 double gt = 0.0;
                 int att = 0;
-                if (!bps) gt = orc_gtilde(c, eps * sbm * vn, i, step, stream, &block, &att, &mg);
+                if (!bps) gt = orc_gtilde(c, eps * sbm * vn, i, step, stream + 16, &gblock, &att, &mg);
                 orc_jump_kick(eps, sbm, n, gt, v); /* P:L406 */
                 ev.accepted = 1; ev.gt = gt; ev.n_gt = att;
                 (*n_acc)++;
                 (*n_gt) += att;
+                fresh = 1;
             }
         }
         ev.margin = mg;
