@@ -26,6 +26,8 @@ import numpy as np
 
 BLOCK = 10                 # steps per timed block = nlist_every, so every block holds exactly one rebuild
 FLOPS_PER_PAIR = 2 * 50    # ~50 FP32-pipe instructions per in-range half pair, counted as FMAs
+PROPOSAL_INSTR = 250       # ~150 FP32-pipe + ~100 INT-pipe (one Philox block) instructions per proposal
+CHAIN_INSTR = 60           # chain set-up + expiry per half-phase chain
 L2_FLUSH_BYTES = 256 << 20
 
 
@@ -233,26 +235,50 @@ def main():
 
     # ---- per-kernel times of the same K steps (CUDA events on the launch stream, separate pass) --------------
     with torch.cuda.stream(stream):
+        sim.reset_stats()
         sim.set_profiling(True)
         timed_blocks(torch, sim, stream, step_call, K, block, flush)
         prof = sim.profile()
         sim.set_profiling(False)
+        pstats = sim.stats()
         n_pairs_ordered = sim.count_pairs(0, run["r_short"])           # ordered in-range entries of the short row
+        row_entries = sum(sim.count_pairs(k, 1e3) for k in (0, 1, 2, 3) if stats["cap_row"][k])
     tot_prof = sum(v[0] for v in prof.values())
-    pair_ms, pair_launches = prof["pair"]
-    clk_mhz = clocks["sm_mhz"] or peaks["sm_max_mhz"]
+    share = {k: (v[0] / tot_prof if tot_prof else 0.0) for k, v in prof.items()}
     peak_tflops = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    alu_src = "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (%s sm_max_mhz)" % (props.multi_processor_count, peaks["sm_max_mhz"],
+                                                                      peaks["source"])
+
+    def avg_ms(cat):
+        return prof[cat][0] / max(prof[cat][1], 1)
+
+    def alu_line(kernel, flops, what, cat):
+        ach = flops / (avg_ms(cat) * 1e-3) / 1e12 if avg_ms(cat) > 0 else 0.0
+        return {"kernel": kernel, "bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": ach / peak_tflops, "traffic": None, "peak_source": alu_src, "algorithmic": what,
+                "avg_launch_us": 1e3 * avg_ms(cat), "share_of_step": share[cat]}
+
     half_pairs = n_pairs_ordered / 2.0
-    pair_flops = half_pairs * FLOPS_PER_PAIR
-    pair_avg_ms = pair_ms / max(pair_launches, 1)
-    achieved = pair_flops / (pair_avg_ms * 1e-3) / 1e12 if pair_avg_ms > 0 else 0.0
-    roofline = {"kernel": "k_pair (short-range switched pair gradient, a5)", "bound": "alu", "achieved": achieved,
-                "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": None,
-                "peak_source": "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (%s sm_max_mhz)" % (
-                    props.multi_processor_count, peaks["sm_max_mhz"], peaks["source"]),
-                "algorithmic": "%.0f in-range half pairs x %d flop" % (half_pairs, FLOPS_PER_PAIR),
-                "avg_launch_us": 1e3 * pair_avg_ms, "share_of_step": pair_ms / tot_prof if tot_prof else None,
-                "kernel_ms_share": {k: v[0] / tot_prof for k, v in prof.items()} if tot_prof else None}
+    n_upd = max(prof["update"][1], 1)
+    chains = 2.0 * n * (2 if run["flags"] & 2 else 1)                  # half-phases x (C' [+ J']) per update launch
+    upd_instr = pstats["proposals"] / n_upd * PROPOSAL_INSTR + chains * CHAIN_INSTR
+    build_bytes = row_entries * 4.0 + n * 48.0
+    build_ach = build_bytes / (avg_ms("build") * 1e-3) / 1e9 if avg_ms("build") > 0 else 0.0
+    lines = {
+        "pair": alu_line("k_pair (short-range switched pair gradient, a5)", half_pairs * FLOPS_PER_PAIR,
+                         "%.0f in-range half pairs x %d flop" % (half_pairs, FLOPS_PER_PAIR), "pair"),
+        "update": alu_line("k_update (jump chains C'J' of two half-phases + A-O-A, a6-a8)", 2.0 * upd_instr,
+                           "%.0f proposals x %d + %.0f chains x %d FP32/INT-pipe instructions, x 2 flop"
+                           % (pstats["proposals"] / n_upd, PROPOSAL_INSTR, chains, CHAIN_INSTR), "update"),
+        "build": {"kernel": "sort + k_build_rows (a1-a3), one group per rebuild", "bound": "hbm", "achieved": build_ach,
+                  "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": build_ach / peaks["hbm_gbs"], "traffic": None,
+                  "peak_source": "%s HBM copy bandwidth" % peaks["source"],
+                  "algorithmic": "%.0f row entries x 4 B + %d atoms x 48 B" % (row_entries, n),
+                  "avg_launch_us": 1e3 * avg_ms("build"), "share_of_step": share["build"]},
+    }
+    dominant = max(("pair", "update", "build"), key=lambda k: share[k])
+    roofline = dict(lines[dominant], kernel_ms_share=share)
+    roofline_other = {k: v for k, v in lines.items() if k != dominant}
 
     # ---- same-GPU BAOAB with the unsplit r_long force (reported baseline) -------------------------------------
     with torch.cuda.stream(stream):
@@ -306,7 +332,7 @@ def main():
                            "parallelism": "independent replicas x%d" % world},
                 "atom_steps_per_s": world * sps * n,
                 "clocks": clocks, "gpu_launches": launches, "wall_s": wall,
-                "e2e": e2e, "roofline": roofline, "baoab_same_gpu": baoab,
+                "e2e": e2e, "roofline": roofline, "roofline_other": roofline_other, "baoab_same_gpu": baoab,
                 "jump_vs_baoab": (K / ms_max) / (Kb / ms_b),
                 "events": {"proposals_per_atom_step": stats["proposals"] / (n * (K + W)) if K + W else None,
                            "accepts_per_atom_step": stats["accepts"] / (n * (K + W)), "max_p": stats["max_p"],

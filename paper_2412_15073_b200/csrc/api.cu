@@ -33,6 +33,7 @@ struct jump_ctx {
     bool row_used[N_ROWS];   // read since the last sort: rebuilt eagerly at the next one (others lazily, on demand)
     bool f0_valid;           // c->f0 / fnb / fbond hold F0 at the current positions
     float4 *fnb, *fbond, *f0, *ftmp, *ftmp2;
+
     double *ke;
     int *excl_ptr, *excl_idx;
     Topo topo;

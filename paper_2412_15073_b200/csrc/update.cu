@@ -30,11 +30,16 @@ __device__ inline void log_event(const UpdateArgs &a, unsigned step, int stream,
     a.events[slot] = e;
 }
 
-// Theta(eta) = E[(eta+G)_+] = eta Phi(eta) + phi(eta)  (R-5)
+// Theta(eta) = E[(eta+G)_+] = eta Phi(eta) + phi(eta)  (R-5).  With x = |eta| / sqrt 2 both terms share
+// e^{-x^2}: erfc(x) = e^{-x^2} erfcx_poly(x), phi = e^{-x^2} / sqrt(2 pi).  Beyond the polynomial's range
+// (|eta| > 6.08) Theta is eta_+ to 1e-10, far below the smallest uniform (2^-24).
 __device__ inline float theta_of(float eta) {
-    float Phi = 0.5f * erfcf(-eta * 0.70710678118654752f);
-    float phi = kInvSqrt2Pi * expf(-0.5f * eta * eta);
-    return eta * Phi + phi;
+    const float x = fabsf(eta) * 0.70710678118654752f;
+    if (x > 4.3f) return fmaxf(eta, 0.f);
+    const float ex = expf(-x * x);
+    const float half_erfc = 0.5f * ex * erfcx_poly(x);            // Phi(-|eta|)
+    const float Phi = eta > 0.f ? 1.f - half_erfc : half_erfc;
+    return fmaf(eta, Phi, kInvSqrt2Pi * ex);
 }
 
 // G~ ~ f_eta by rejection (R-6; proposal family of P:L310).  One Philox block per attempt.
@@ -118,32 +123,63 @@ __device__ inline float fij_lj(const Model &m, const float4 &xi, const float4 &x
     return (1.f - chi) * du - dchi * u;
 }
 
-// ---- step (C'): Algorithm 4 + ring (R-11).  x frozen; updates (vx,vy,vz) of atom i. -------------------------
-// G lanes cooperate on one chain.  What a proposal needs from the random stream and from x -- the exponential
-// E, the ring, the partner j, the uniform U and the pair gradient F_ij(x) (x is frozen) -- does not depend on
-// the chain's state (t, v), so lane l evaluates all of that for the l-th next iteration at once (Philox block
-// b + l, the row and position gathers, erfc/exp).  Only the thinning recurrence itself is sequential
-// (B_v -> lambda-bar -> T -> t, v -> accept test); every lane of the group replays it on the
-// broadcast values, so (t, v) stay replicated in registers.  An accepted jump consumes G~ blocks and thereby
-// shifts the block index of the later iterations (R-15): the speculative tail is then dropped and the batch
-// restarted -- accepted jumps are ~1 % of the proposals.  The arithmetic of every iteration is exactly the
-// sequential algorithm's, so the event log equals the oracle's whatever G is.
+// ---- step (C'): Algorithm 4 + ring (R-11) --------------------------------------------------------------------
+// G lanes cooperate on one chain, and nothing in the common case is sequential:
+//  * what proposal k needs from the random stream and from x -- the exponential E_k, the ring, the partner j, the
+//    uniform U_k and the pair gradient F_ij(x) -- depends neither on the chain's state nor on the other
+//    proposals (x is frozen during a jump phase; proposal k draws Philox block k of its stream, the G~ attempts
+//    have a stream of their own, R-15): lane l evaluates proposal kb + l;
+//  * the bound lambda-bar is re-evaluated after each ACCEPTED jump only (R-11), so between two accepted
+//    jumps the proposal times are a running sum of E_k / lambda-bar and v(t) = v_e + (t - t_e) a in closed form:
+//    every lane gets its own proposal time (summed in the sequential order, so the value is the sequential
+//    algorithm's bit for bit), its expiry test, its acceptance probability and its accept test at once;
+//  * the first accepting lane (a ballot) ends the epoch: kick, new bound, the later lanes are dropped and the
+//    batch restarts after it -- accepted jumps are ~1-2 % of the proposals.
+struct ChainConst {   // per-atom constants of a C' chain
+    int NM, NL;
+    float LM, LL, SM, S;
+};
+__device__ inline ChainConst chain_const(const Model &m, const Row &rowM, const Row &rowL, int i, float qi) {
+    ChainConst c;
+    c.NM = rowM.cnt[i]; c.NL = rowL.cnt[i];
+    const float aq = fabsf(qi);
+    c.LM = aq * m.qmaxGM; c.LL = aq * m.qmaxGL;
+    c.SM = (float)c.NM * c.LM; c.S = c.SM + (float)c.NL * c.LL;
+    return c;
+}
+// proposal `block` of a chain: sa = (E, U, |F_ij| / L_Y, ring << 31 | j_orig), sb = (n_x, n_y, n_z, -), n = F_ij / |F_ij|
+template <bool WANT_J>
+__device__ inline void propose(const Model &m, const Row &rowM, const Row &rowL, const float4 *__restrict__ xs,
+                               const int *__restrict__ orig, const ChainConst &c, int i, unsigned atom, const float4 &xi,
+                               unsigned step, unsigned stream, unsigned block, float4 &sa, float4 &sb) {
+    uint32_t w[4];
+    philox4x32_10(atom, step, stream, block, m.key0, m.key1, w);
+    const float E = -logf(u01(w[0]));
+    int ring = (u01(w[1]) * c.S < c.SM) ? 0 : 1;  // ring pick
+    if (ring == 0 && c.NM == 0) ring = 1;
+    if (ring == 1 && c.NL == 0) ring = 0;
+    const int cnt = ring == 0 ? c.NM : c.NL;
+    const int k = (int)__umulhi(w[2], (unsigned)cnt);
+    const int j = ring == 0 ? rowM.idx[(size_t)i * rowM.cap + k] : rowL.idx[(size_t)i * rowL.cap + k];
+    const float U = u01(w[3]);
+    float dx, dy, dz, rinv;
+    const float fr = fij_coul(m, xi, xs[j], dx, dy, dz, rinv);
+    const float sg = (fr > 0.f ? rinv : -rinv);  // n = F/|F|
+    const float LY = ring == 0 ? c.LM : c.LL;
+    int tag = 0;
+    if (WANT_J) tag = orig[j] | (ring << 31);
+    sa = make_float4(E, U, fabsf(fr) / LY, __int_as_float(tag));
+    sb = make_float4(dx * sg, dy * sg, dz * sg, 0.f);
+}
+
 template <int G, bool LOG>
 __device__ void chain_C(const Model &m, const UpdateArgs &A, int i, unsigned atom, const float4 &xi, float sbm,
                         float ax, float ay, float az, float H, unsigned stream, unsigned step, float &vx, float &vy,
-                        float &vz, Tally &tl, unsigned gmask, int gl) {
+                        float &vz, Tally &tl, unsigned gmask, int gl, int gshift) {
     const float eps = m.eps_jump, beta = m.beta;
-    const bool bps = isinf(eps);
-    const int NM = A.rowM.cnt[i], NL = A.rowL.cnt[i];
-    const float aq = fabsf(xi.w);
-    const float LM = aq * m.qmaxGM, LL = aq * m.qmaxGL;
-    const float SM = (float)NM * LM, S = SM + (float)NL * LL;
-    const float lam0 = bps ? 0.f : (1.f / eps) * beta * kInvSqrt2Pi / sbm;
-    const float a2 = ax * ax + ay * ay + az * az;
-    const bool lead = gl == 0;
-    float t = 0.f;
-    unsigned block = 0;
-    int iter = 0;
+    const bool bps = isinf(eps), lead = gl == 0;
+    const ChainConst c = chain_const(m, A.rowM, A.rowL, i, xi.w);
+    const float S = c.S;
     if (!(S > 0.f)) {  // no partner: lambda-bar = 0, the clock never rings
         vx += H * ax; vy += H * ay; vz += H * az;
         if (lead) {
@@ -152,81 +188,84 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, int i, unsigned ato
         }
         return;
     }
+    const float lam0 = bps ? 0.f : (1.f / eps) * beta * kInvSqrt2Pi / sbm;
+    const float a2 = ax * ax + ay * ay + az * az, esb = eps * sbm;
+    const unsigned gbits = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
+    float vex = vx, vey = vy, vez = vz, te = 0.f;   // epoch start: velocity and time after the last accepted jump
+    float t_run = 0.f;                              // time of the last proposal so far
+    float Bv = 0.f, lam = 0.f, den = 1.f;
+    bool fresh = true;
+    unsigned kb = 0, gblock = 0;
     for (;;) {
-        // ---- state-independent part of iteration (iter + gl), Philox block (block + gl) ----
-        uint32_t w[4];
-        philox4x32_10(atom, step, stream, block + (unsigned)gl, m.key0, m.key1, w);
-        float E_ = -logf(u01(w[0]));
-        int ring_ = (u01(w[1]) * S < SM) ? 0 : 1;  // ring pick
-        if (ring_ == 0 && NM == 0) ring_ = 1;
-        if (ring_ == 1 && NL == 0) ring_ = 0;
-        const int cnt = ring_ == 0 ? NM : NL;
-        const int k = (int)__umulhi(w[2], (unsigned)cnt);
-        const int j_ = ring_ == 0 ? A.rowM.idx[(size_t)i * A.rowM.cap + k] : A.rowL.idx[(size_t)i * A.rowL.cap + k];
-        const float U_ = u01(w[3]);
-        float dx, dy, dz, rinv;
-        float fr = fij_coul(m, xi, A.xs[j_], dx, dy, dz, rinv);
-        float g_ = fabsf(fr);
-        float sg = (fr > 0.f ? rinv : -rinv);  // n = F/|F|
-        float nx_ = dx * sg, ny_ = dy * sg, nz_ = dz * sg;
-        const float LY_ = ring_ == 0 ? LM : LL;
-        float gl_ = g_ / LY_;
-        int jo_ = LOG ? A.orig[j_] : 0;
-        // ---- the thinning recurrence over the G staged iterations ----
-        bool finished = false, restart = false;
-#pragma unroll 1
-        for (int l = 0; l < G; ++l) {
-            float E = __shfl_sync(gmask, E_, l, G);
-            float tau = H - t;
-            float va = vx * ax + vy * ay + vz * az;
-            float v2 = vx * vx + vy * vy + vz * vz;
-            float Bv = sqrtf(v2 + tau * tau * a2 + 2.f * tau * fmaxf(va, 0.f));
-            float lam = S * (beta * Bv + lam0);
-            float T = E / lam;   // P:L379 (lam = 0: +inf).  IEEE sqrt and division: t + T <= H is a fragile decision (R-17)
-            if (!(t + T <= H)) {
-                vx += tau * ax; vy += tau * ay; vz += tau * az;
-                if (lead) {
-                    tl.expiries++;
-                    if (LOG) log_event(A, step, stream, atom, iter, -1, -1, 0, 0, T, 0.f, 0.f, 0.f);
-                }
-                finished = true;
-                break;
-            }
-            t += T;
-            vx += T * ax; vy += T * ay; vz += T * az;
-            float g = __shfl_sync(gmask, g_, l, G), goL = __shfl_sync(gmask, gl_, l, G), U = __shfl_sync(gmask, U_, l, G);
-            if (lead) { tl.proposals++; tl.max_gl = fmaxf(tl.max_gl, goL); }
-            float p = 0.f, gt = 0.f;
-            int acc = 0, att = 0;
-            // p <= g / L_Y always (Theta(eta) <= eta_+ + 1/sqrt(2 pi), eta <= eps sqrt(beta m) B_v): most proposals
-            // are rejected on that bound alone; p itself is evaluated when it can matter (or is logged)
-            if (g > 0.f && (LOG || U <= goL * 1.0001f)) {
-                float nx = __shfl_sync(gmask, nx_, l, G), ny = __shfl_sync(gmask, ny_, l, G), nz = __shfl_sync(gmask, nz_, l, G);
-                float LY = __shfl_sync(gmask, LY_, l, G);
-                float vn = vx * nx + vy * ny + vz * nz;
-                if (bps) p = fmaxf(vn, 0.f) * g / (LY * Bv);
-                else p = g * theta_of(eps * sbm * vn) / (LY * (Bv * eps * sbm + kInvSqrt2Pi));  // P:L397 with sqrt(beta)
-                if (lead) tl.max_p = fmaxf(tl.max_p, p);
-                if (U <= p) {
-                    unsigned b2 = block + (unsigned)l + 1u;
-                    if (!bps) gt = gtilde(eps * sbm * vn, atom, step, stream, b2, m, att);
-                    jump_kick(eps, sbm, nx, ny, nz, gt, vx, vy, vz);
-                    acc = 1;
-                    if (lead) { tl.accepts++; tl.gt_attempts += att; }
-                    block = b2;  // the next iteration's block follows the sampler's
-                    restart = true;
-                }
-            }
-            if (LOG) {
-                int ring = __shfl_sync(gmask, ring_, l, G), jo = __shfl_sync(gmask, jo_, l, G);
-                if (lead) log_event(A, step, stream, atom, iter, ring, jo, acc, att, T, p, U, gt);
-            }
-            ++iter;
-            if (restart) break;
+        if (fresh) {   // the bound of this epoch, P:L373-374 (R-11)
+            const float tau = H - te;
+            const float va = vex * ax + vey * ay + vez * az, v2 = vex * vex + vey * vey + vez * vez;
+            Bv = sqrtf(v2 + tau * tau * a2 + 2.f * tau * fmaxf(va, 0.f));
+            lam = S * (beta * Bv + lam0);
+            den = bps ? Bv : fmaf(Bv, esb, kInvSqrt2Pi);
+            fresh = false;
         }
-        if (finished) break;
-        if (!restart) block += (unsigned)G;
+        float4 sa, sb;
+        propose<LOG>(m, A.rowM, A.rowL, A.xs, A.orig, c, i, atom, xi, step, stream, kb + (unsigned)gl, sa, sb);
+        const float T_ = sa.x / lam;   // P:L379 (lam = 0: +inf)
+        float tk = t_run;              // time of my proposal: ((t_run + T_0) + T_1) + ... + T_gl, the sequential order
+#pragma unroll
+        for (int q = 0; q < G; ++q) {
+            const float Tq = __shfl_sync(gmask, T_, q, G);
+            if (q <= gl) tk += Tq;
+        }
+        const bool alive = tk <= H;    // the chain expires at the first proposal with t + T > delta/2
+        const float U = sa.y, goL = sa.z;
+        float p = 0.f, vn = 0.f;
+        bool acc = false;
+        // p <= |F_ij| / L_Y always (Theta(eta) <= eta_+ + 1/sqrt(2 pi), eta <= eps sqrt(beta m) B_v): most proposals
+        // are rejected on that bound alone; p itself is evaluated when it can matter (or is logged)
+        if (alive && goL > 0.f && (LOG || U <= goL * 1.0001f)) {
+            const float s = tk - te;
+            const float cx = fmaf(s, ax, vex), cy = fmaf(s, ay, vey), cz = fmaf(s, az, vez);  // the advanced v
+            vn = cx * sb.x + cy * sb.y + cz * sb.z;
+            const float pub = bps ? goL * fmaxf(vn, 0.f) / den : goL * (fmaxf(esb * vn, 0.f) + kInvSqrt2Pi) / den;
+            if (LOG || U <= pub * 1.0001f) {
+                p = bps ? fmaxf(vn, 0.f) * goL / den : goL * theta_of(esb * vn) / den;  // P:L397 with sqrt(beta)
+                acc = U <= p;
+            }
+        }
+        const unsigned alive_m = (__ballot_sync(gmask, alive) >> gshift) & gbits;
+        const unsigned acc_m = (__ballot_sync(gmask, acc) >> gshift) & gbits;
+        const int n_alive = __popc(alive_m);
+        const int f = acc_m ? __ffs(acc_m) - 1 : -1;   // first accepted proposal of the batch
+        const int n_used = f >= 0 ? f + 1 : n_alive;
+        if (gl < n_used) { tl.max_gl = fmaxf(tl.max_gl, goL); tl.max_p = fmaxf(tl.max_p, p); }
+        if (lead) tl.proposals += (unsigned)n_used;
+        float gt = 0.f;
+        int att = 0;
+        if (f >= 0) {   // kick (7) on the velocity at the time of proposal f; a new epoch starts there
+            const float tf = __shfl_sync(gmask, tk, f, G), vnf = __shfl_sync(gmask, vn, f, G);
+            const float nx = __shfl_sync(gmask, sb.x, f, G), ny = __shfl_sync(gmask, sb.y, f, G), nz = __shfl_sync(gmask, sb.z, f, G);
+            if (!bps) gt = gtilde(esb * vnf, atom, step, stream + 16u, gblock, m, att);
+            const float s = tf - te;
+            float cx = fmaf(s, ax, vex), cy = fmaf(s, ay, vey), cz = fmaf(s, az, vez);
+            jump_kick(eps, sbm, nx, ny, nz, gt, cx, cy, cz);
+            vex = cx; vey = cy; vez = cz; te = tf; t_run = tf;
+            fresh = true;
+            if (lead) { tl.accepts++; tl.gt_attempts += att; }
+        }
+        if (LOG) {
+            const int tag = __float_as_int(sa.w);
+            if (gl < n_used)
+                log_event(A, step, stream, atom, (int)kb + gl, (int)((unsigned)tag >> 31), tag & 0x7fffffff, gl == f ? 1 : 0,
+                          gl == f ? att : 0, T_, p, U, gl == f ? gt : 0.f);
+            else if (f < 0 && gl == n_alive)
+                log_event(A, step, stream, atom, (int)kb + gl, -1, -1, 0, 0, T_, 0.f, 0.f, 0.f);
+        }
+        if (f >= 0) { kb += (unsigned)(f + 1); continue; }
+        if (n_alive < G) break;   // expired inside this batch
+        t_run = __shfl_sync(gmask, tk, G - 1, G);
+        kb += (unsigned)G;
     }
+    if (lead) tl.expiries++;
+    const float s_end = H - te;   // drift to the end of the half-step
+    vx = fmaf(s_end, ax, vex); vy = fmaf(s_end, ay, vey); vz = fmaf(s_end, az, vez);
 }
 
 // ---- step (J'): Algorithm 5 (R-14) ---------------------------------------------------------------------------
@@ -287,15 +326,14 @@ __device__ inline double wrap1d(double x, double L) {
 }
 
 // ---- the fused per-atom update: up to two velocity half-phases, then A O A + wrap ----------------------------
-// G lanes per atom (a power of two <= 32): they share the jump chains (see chain_C); lane 0 of the group does the
-// A-O-A part and all the stores.
+// G lanes per atom (a power of two <= 32) share the atom's jump chains; lane 0 of the group does A-O-A and the stores.
 template <bool JUMPS, int G, bool LOG>
-__global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
+__global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
     const unsigned full = 0xffffffffu;
     const int gt_id = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gt_id / G, gl = gt_id % G;
-    const int lane = threadIdx.x & 31;
-    const unsigned gmask = (G == 32) ? full : (((1u << G) - 1u) << (lane & ~(G - 1)));
+    const int lane = threadIdx.x & 31, gshift = lane & ~(G - 1);
+    const unsigned gmask = (G == 32) ? full : (((1u << G) - 1u) << gshift);
     const bool live = i < m.n, lead = gl == 0;
     Tally tl = {0u, 0u, 0u, 0u, 0.f, 0.f};
     float disp2 = 0.f;
@@ -321,7 +359,7 @@ __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
             } else {
                 const float2 lji = A.lj[i];
                 if (P.reverse && P.lj) chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
-                if (P.coul) chain_C<G, LOG>(m, A, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl, gmask, gl);
+                if (P.coul) chain_C<G, LOG>(m, A, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl, gmask, gl, gshift);
                 else if (P.use_grad) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
                 if (!P.reverse && P.lj) chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
             }
@@ -359,7 +397,11 @@ __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
         bad = bad || !(isfinite(vx) && isfinite(vy) && isfinite(vz));
         if (lead) A.vs[i] = make_float4(vx, vy, vz, v4.w);
     }
-    // warp-level reduction of the statistics, then a few integer atomics per warp
+    // statistics: warp reduction -> shared-memory atomics -> one set of global atomics per CTA (thousands of warps
+    // hitting the same few global counters serialise at one L2 slice)
+    __shared__ unsigned s_stat[8];   // proposals, accepts, gt_attempts, expiries, max_p, max_gl, max_disp2, err
+    if (threadIdx.x < 8) s_stat[threadIdx.x] = 0u;
+    __syncthreads();
     unsigned err = 0;
     if (bad) err |= ERR_NAN;
     if (disp2 > m.half_skin2) err |= ERR_SKIN;
@@ -372,17 +414,30 @@ __global__ void __launch_bounds__(128) k_update(Model m, UpdateArgs A) {
         unsigned mp = __reduce_max_sync(full, __float_as_uint(tl.max_p));
         unsigned mg = __reduce_max_sync(full, __float_as_uint(tl.max_gl));
         if (lane == 0) {
-            if (np) atomicAdd(&A.ctr->proposals, (unsigned long long)np);
-            if (na) atomicAdd(&A.ctr->accepts, (unsigned long long)na);
-            if (ng) atomicAdd(&A.ctr->gt_attempts, (unsigned long long)ng);
-            if (ne) atomicAdd(&A.ctr->expiries, (unsigned long long)ne);
-            if (mp > A.ctr->max_p_bits) atomicMax(&A.ctr->max_p_bits, mp);
-            if (mg > A.ctr->max_gl_bits) atomicMax(&A.ctr->max_gl_bits, mg);
+            if (np) atomicAdd(&s_stat[0], np);
+            if (na) atomicAdd(&s_stat[1], na);
+            if (ng) atomicAdd(&s_stat[2], ng);
+            if (ne) atomicAdd(&s_stat[3], ne);
+            atomicMax(&s_stat[4], mp);
+            atomicMax(&s_stat[5], mg);
         }
     }
     if (lane == 0) {
-        if (d2b > A.ctr->max_disp2_bits) atomicMax(&A.ctr->max_disp2_bits, d2b);
-        if (err) atomicOr(&A.ctr->err, err);
+        atomicMax(&s_stat[6], d2b);
+        if (err) atomicOr(&s_stat[7], err);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (JUMPS) {
+            if (s_stat[0]) atomicAdd(&A.ctr->proposals, (unsigned long long)s_stat[0]);
+            if (s_stat[1]) atomicAdd(&A.ctr->accepts, (unsigned long long)s_stat[1]);
+            if (s_stat[2]) atomicAdd(&A.ctr->gt_attempts, (unsigned long long)s_stat[2]);
+            if (s_stat[3]) atomicAdd(&A.ctr->expiries, (unsigned long long)s_stat[3]);
+            if (s_stat[4] > A.ctr->max_p_bits) atomicMax(&A.ctr->max_p_bits, s_stat[4]);
+            if (s_stat[5] > A.ctr->max_gl_bits) atomicMax(&A.ctr->max_gl_bits, s_stat[5]);
+        }
+        if (s_stat[6] > A.ctr->max_disp2_bits) atomicMax(&A.ctr->max_disp2_bits, s_stat[6]);
+        if (s_stat[7]) atomicOr(&A.ctr->err, s_stat[7]);
     }
 }
 
@@ -444,15 +499,14 @@ __global__ void k_kinetic(int n, const float4 *__restrict__ vs, const float2 *__
 }
 
 template <int G>
-static void update_dispatch(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st) {
+static void update_dispatch(const Model &m, const UpdateArgs &A, cudaStream_t st) {
     const int B = 128;
     const unsigned grid = (unsigned)(((long long)m.n * G + B - 1) / B);
-    if (!jumps) k_update<false, 1, false><<<(m.n + B - 1) / B, B, 0, st>>>(m, A);
-    else if (A.events) k_update<true, G, true><<<grid, B, 0, st>>>(m, A);
+    if (A.events) k_update<true, G, true><<<grid, B, 0, st>>>(m, A);
     else k_update<true, G, false><<<grid, B, 0, st>>>(m, A);
 }
-// lanes per jump chain: as many as keep the grid within about two full waves of resident threads
-// (148 SMs x 2048); JUMP_B200_LANES overrides (1, 4, 8, 16) for experiments
+// lanes per jump chain: as many as keep the whole grid resident at once (148 SMs x 6 CTAs of 128 threads, the
+// register-limited occupancy of k_update); JUMP_B200_LANES overrides (1, 4, 8, 16) for experiments
 static int lanes_per_chain(int n) {
     static int forced = -1;
     if (forced < 0) {
@@ -460,18 +514,23 @@ static int lanes_per_chain(int n) {
         forced = e ? atoi(e) : 0;
     }
     if (forced == 1 || forced == 4 || forced == 8 || forced == 16) return forced;
-    const long long budget = 2ll * 148 * 2048;
+    const long long budget = 148ll * 6 * 128;
     if ((long long)n * 16 <= budget) return 16;
     if ((long long)n * 8 <= budget) return 8;
     if ((long long)n * 4 <= budget) return 4;
     return 1;
 }
 void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st, int64_t *launches) {
-    switch (jumps ? lanes_per_chain(m.n) : 1) {
-        case 16: update_dispatch<16>(m, A, jumps, st); break;
-        case 8: update_dispatch<8>(m, A, jumps, st); break;
-        case 4: update_dispatch<4>(m, A, jumps, st); break;
-        default: update_dispatch<1>(m, A, jumps, st); break;
+    if (!jumps) {
+        const int B = 128;
+        k_update<false, 1, false><<<(unsigned)((m.n + B - 1) / B), B, 0, st>>>(m, A);
+    } else {
+        switch (lanes_per_chain(m.n)) {
+            case 16: update_dispatch<16>(m, A, st); break;
+            case 8: update_dispatch<8>(m, A, st); break;
+            case 4: update_dispatch<4>(m, A, st); break;
+            default: update_dispatch<1>(m, A, st); break;
+        }
     }
     *launches += 1;
 }
