@@ -125,20 +125,34 @@ __device__ inline int cyc_off(int val, int c, int gn) {
     return o;
 }
 
+// d wrapped to the periodic image nearest to 0
+__device__ inline float near_image1(float d, float L, float invL) {
+    float t = d * invL + 12582912.f;   // round to nearest integer by the 1.5 * 2^23 trick
+    t -= 12582912.f;
+    return fmaf(-L, t, d);
+}
+
 // Row build, one CTA per cell of the contract grid.
 //  1. The candidate set of a cell is the same for all its atoms: the cells of a host-computed stencil (every cell
 //     whose extent comes within rmax of this cell), visited in ascending cell key, i.e. a list of contiguous runs
 //     [seg_beg, seg_beg + seg_len) of the sorted atom array.  The runs are found once per CTA, prefix-summed and
-//     the candidates (x, y, z, q | sorted index + LJ flag) staged in shared memory in canonical order.
-//  2. Each warp takes one atom of the cell and scans the staged candidates 32 at a time: fp32 distance, window
-//     tests of the selected rows, exclusions, ballot compaction into the fixed-capacity rows.
+//     the candidates staged in shared memory in canonical order, BUILD_CHUNK at a time, ONCE for all atoms of the
+//     cell.  A staged entry is (x, y, z | sorted index + LJ flag): in the FAST variant the coordinates are taken
+//     relative to the cell centre and wrapped to the image nearest to it, so that the inner loop needs no minimum
+//     image at all (valid when rmax + cell/2 <= box/2 in every dimension: then for every pair closer than rmax the
+//     staged image IS the minimum image, and any other image is farther than rmax anyway).
+//  2. Each warp takes the atoms a_beg + warp, + BUILD_WARPS, ... of the cell and scans the staged candidates 32 at
+//     a time: distance, window tests of the selected rows, ballot compaction into the fixed-capacity rows (running
+//     counts live in shared memory between chunks).  Exclusions and the atom itself are looked at only for
+//     candidates closer than the atom's farthest excluded partner.
 //  3. A candidate whose fp32 r^2 lies within BUILD_TIE of a window edge is decided again in fp64 from the full
 //     positions x = xs + xl, with the oracle's expression d - L rint(d/L): membership at an edge is a discontinuous
-//     decision (R-17) and the fp32 value of r^2 (error ~1e-5 A^2) would flip it where the fp64 oracle does not.
+//     decision (R-17) and the fp32 value of r^2 (error < 1e-3 A^2) would flip it where the fp64 oracle does not.
 constexpr int BUILD_THREADS = 128;
 constexpr int BUILD_WARPS = BUILD_THREADS / 32;
 constexpr int BUILD_CHUNK = 1024;           // candidates staged per pass
 constexpr int BUILD_MAXSEG = 2 * 17 * 17;   // two x-runs per (z, y) cell row of the stencil
+constexpr int BUILD_MAXATOMS = 32;          // atoms of a cell whose running counts are held at once
 constexpr float BUILD_TIE = 4e-3f;          // A^2
 
 struct Stencil {
@@ -149,7 +163,7 @@ struct Stencil {
 };
 
 // MASK >= 0: bit k set = row k is built (compile-time row set of the common modes); MASK < 0: rows.r[k].enabled decides
-template <int MASK>
+template <int MASK, bool FAST>
 __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid g, RowSet rows, Stencil stn, float rmax_all,
                                                               const int *__restrict__ cell_start,
                                                               const float4 *__restrict__ xs, const float4 *__restrict__ xl,
@@ -159,9 +173,9 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                                                               Counters *ctr) {
     __shared__ int seg_beg[BUILD_MAXSEG];
     __shared__ int seg_pre[BUILD_MAXSEG + 1];   // exclusive prefix of the run lengths
-    __shared__ float4 tile_x[BUILD_CHUNK];
-    __shared__ int tile_j[BUILD_CHUNK];         // sorted index | LJ flag in bit 31
+    __shared__ float4 tile[BUILD_CHUNK];        // (x, y, z, sorted index | LJ flag in bit 31)
     __shared__ int scan_tmp[BUILD_THREADS];
+    __shared__ int s_count[BUILD_MAXATOMS][N_ROWS];
     const unsigned full = 0xffffffffu;
     const int cell = blockIdx.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int a_beg = cell_start[cell], a_end = cell_start[cell + 1];
@@ -170,9 +184,11 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
     c3[0] = cell % g.gn[0];
     c3[1] = (cell / g.gn[0]) % g.gn[1];
     c3[2] = cell / (g.gn[0] * g.gn[1]);
+    float ctr3[3];   // cell centre (FAST: origin of the staged coordinates)
     int start[3], cnt[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
+        ctr3[k] = ((float)c3[k] + 0.5f) * (m.box[k] / (float)g.gn[k]);
         if (2 * stn.R[k] + 1 >= g.gn[k]) { start[k] = 0; cnt[k] = g.gn[k]; }
         else { start[k] = (c3[k] - stn.R[k] + g.gn[k]) % g.gn[k]; cnt[k] = 2 * stn.R[k] + 1; }
     }
@@ -218,39 +234,17 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
     }
     __syncthreads();
     const int total = seg_pre[nseg];
-    const float rmax2 = rmax_all * rmax_all;
+    const float rmax2t = rmax_all * rmax_all + BUILD_TIE;
     const unsigned lt_mask = (1u << lane) - 1u;
-
-    // ---- 2./3. atoms of the cell, BUILD_WARPS at a time --------------------------------------------------------
-    for (int a0 = a_beg; a0 < a_end; a0 += BUILD_WARPS) {
-        const int i = a0 + warp;
-        const bool have = i < a_end;
-        float4 xi = make_float4(0.f, 0.f, 0.f, 0.f);
-        bool lj_i = false;
-        int ex_lo = 0, n_ex = 0, ex_mine = -1;
-        int ex4[4] = {-1, -1, -1, -1};   // up to four excluded partners held by every lane (water: two)
-        if (have) {
-            xi = xs[i];
-            lj_i = lj[i].y > 0.f;
-            if (excl_ptr) { int o = orig[i]; ex_lo = excl_ptr[o]; n_ex = excl_ptr[o + 1] - ex_lo; }
-            ex_mine = (lane < n_ex) ? sorted_of[excl_idx[ex_lo + lane]] : -1;
-#pragma unroll
-            for (int e = 0; e < 4; ++e) ex4[e] = __shfl_sync(full, ex_mine, e);
-        }
 #define JB_ROW_ON(k) (MASK >= 0 ? (((MASK) >> (k)) & 1) != 0 : rows.r[k].enabled != 0)
-        int count[N_ROWS];
-        int *rbase[N_ROWS];
-#pragma unroll
-        for (int k = 0; k < N_ROWS; ++k) {
-            count[k] = 0;
-            rbase[k] = JB_ROW_ON(k) ? rows.r[k].idx + (size_t)(have ? i : 0) * rows.r[k].cap : nullptr;
-        }
-        const float e0 = stn.edge2[0], e1 = stn.edge2[1], e2 = stn.edge2[2], e3 = stn.edge2[3];
-
-        for (int c0 = 0; c0 < total; c0 += BUILD_CHUNK) {
+    for (int g0 = a_beg; g0 < a_end; g0 += BUILD_MAXATOMS) {   // one pass unless a cell holds > BUILD_MAXATOMS atoms
+        const int g1 = min(g0 + BUILD_MAXATOMS, a_end);
+        for (int t = tid; t < BUILD_MAXATOMS * N_ROWS; t += BUILD_THREADS) (&s_count[0][0])[t] = 0;
+        for (int c0 = 0; c0 < total || c0 == 0; c0 += BUILD_CHUNK) {
             const int c1 = min(c0 + BUILD_CHUNK, total);
-            __syncthreads();   // the previous chunk has been consumed
-            {   // stage the runs that intersect [c0, c1): first one by bisection, then one run per warp iteration
+            const int npad = (c1 - c0 + 31) & ~31;
+            __syncthreads();   // the previous chunk has been consumed (and s_count is zeroed)
+            {   // ---- stage the runs that intersect [c0, c1): first one by bisection, then one run per warp iteration
                 int lo_s = 0, hi_s = nseg;   // first run with seg_pre[s + 1] > c0
                 while (lo_s < hi_s) { int mid = (lo_s + hi_s) >> 1; if (seg_pre[mid + 1] > c0) hi_s = mid; else lo_s = mid + 1; }
                 for (int sgi = lo_s + warp; sgi < nseg; sgi += BUILD_WARPS) {
@@ -259,90 +253,143 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                     int lo = max(p0, c0), hi = min(p1, c1);
                     for (int q = lo + lane; q < hi; q += 32) {
                         int j = seg_beg[sgi] + (q - p0);
-                        tile_x[q - c0] = xs[j];
-                        tile_j[q - c0] = j | (lj[j].y > 0.f ? (int)0x80000000 : 0);
+                        float4 x = xs[j];
+                        if (FAST) {
+                            x.x = near_image1(x.x - ctr3[0], m.box[0], m.inv_box[0]);
+                            x.y = near_image1(x.y - ctr3[1], m.box[1], m.inv_box[1]);
+                            x.z = near_image1(x.z - ctr3[2], m.box[2], m.inv_box[2]);
+                        }
+                        x.w = __int_as_float(j | (lj[j].y > 0.f ? (int)0x80000000 : 0));
+                        tile[q - c0] = x;
                     }
                 }
+                for (int q = (c1 - c0) + tid; q < npad; q += BUILD_THREADS) tile[q] = make_float4(nanf(""), 0.f, 0.f, 0.f);   // padding: r^2 = NaN fails every test
             }
             __syncthreads();
-            if (!have) continue;
-            for (int q0 = c0; q0 < c1; q0 += 32) {
-                const int q = q0 + lane;
-                bool valid = q < c1;
-                float4 xj = make_float4(0.f, 0.f, 0.f, 0.f);
-                int jraw = 0;
-                if (valid) { xj = tile_x[q - c0]; jraw = tile_j[q - c0]; }
-                const int j = jraw & 0x7fffffff;
-                const bool ljp = lj_i && jraw < 0;
-                float dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
-                float dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
-                float dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
-                float r2 = dx * dx + dy * dy + dz * dz;
-                valid = valid && j != i && r2 < rmax2 + BUILD_TIE;
-                if (!__any_sync(full, valid)) continue;
-                if (n_ex > 0) {   // excluded pairs are never listed (R-9)
-                    bool ex = (j == ex4[0]) | (j == ex4[1]) | (j == ex4[2]) | (j == ex4[3]);
-                    if (n_ex > 4) {
-                        for (int base = 0; base < n_ex; base += 32) {
-                            int mine = ex_mine;
-                            if (base > 0) mine = (base + lane < n_ex) ? sorted_of[excl_idx[ex_lo + base + lane]] : -1;
-                            int lim = min(32, n_ex - base);
-                            for (int e = 0; e < lim; ++e) ex |= (__shfl_sync(full, mine, e) == j);
-                        }
-                    }
-                    valid = valid && !ex;
+            // ---- 2./3. the atoms of the cell against the staged chunk ---------------------------------------------
+            for (int i = g0 + warp; i < g1; i += BUILD_WARPS) {
+                const float4 xi4 = xs[i];
+                float xi = xi4.x, yi = xi4.y, zi = xi4.z;
+                if (FAST) {
+                    xi = near_image1(xi - ctr3[0], m.box[0], m.inv_box[0]);
+                    yi = near_image1(yi - ctr3[1], m.box[1], m.inv_box[1]);
+                    zi = near_image1(zi - ctr3[2], m.box[2], m.inv_box[2]);
                 }
-                bool pass[N_ROWS];
+                const bool lj_i = lj[i].y > 0.f;
+                // excluded partners (R-9): the first four in every lane, and the largest distance to any of them
+                int ex_lo = 0, n_ex = 0;
+                if (excl_ptr) { int o = orig[i]; ex_lo = excl_ptr[o]; n_ex = excl_ptr[o + 1] - ex_lo; }
+                float exr2 = 0.f;
+                int ex_mine = -1;
+                for (int base = 0; base < n_ex; base += 32) {
+                    int p = (base + lane < n_ex) ? sorted_of[excl_idx[ex_lo + base + lane]] : -1;
+                    if (base == 0) ex_mine = p;
+                    if (p >= 0) {
+                        float4 xp = xs[p];
+                        float ddx = min_image1(xi4.x, xp.x, m.box[0], m.inv_box[0]);
+                        float ddy = min_image1(xi4.y, xp.y, m.box[1], m.inv_box[1]);
+                        float ddz = min_image1(xi4.z, xp.z, m.box[2], m.inv_box[2]);
+                        exr2 = fmaxf(exr2, ddx * ddx + ddy * ddy + ddz * ddz);
+                    }
+                }
+                exr2 = __uint_as_float(__reduce_max_sync(full, __float_as_uint(exr2)));   // non-negative floats order as uints
+                exr2 = exr2 * 1.0001f + 2e-3f;   // also catches the atom itself (r^2 = 0)
+                int ex4[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) ex4[e] = __shfl_sync(full, ex_mine, e);
+                int count[N_ROWS];
+                int *rbase[N_ROWS];
 #pragma unroll
                 for (int k = 0; k < N_ROWS; ++k) {
-                    pass[k] = false;
-                    if (!JB_ROW_ON(k)) continue;
-                    const Row &R = rows.r[k];
-                    pass[k] = valid && (!R.lj_only || ljp) && r2 >= R.r2min && r2 < R.r2max;
+                    count[k] = JB_ROW_ON(k) ? s_count[i - g0][k] : 0;
+                    rbase[k] = JB_ROW_ON(k) ? rows.r[k].idx + (size_t)i * rows.r[k].cap : nullptr;
                 }
-                const bool tie = valid && (fabsf(r2 - e0) < BUILD_TIE || fabsf(r2 - e1) < BUILD_TIE ||
-                                           fabsf(r2 - e2) < BUILD_TIE || fabsf(r2 - e3) < BUILD_TIE);
-                if (tie) {   // decide in fp64 from the full positions, like the oracle
-                    float4 li = xl[i], lj4 = xl[j];
-                    double d[3] = {((double)xi.x + (double)li.x) - ((double)xj.x + (double)lj4.x),
-                                   ((double)xi.y + (double)li.y) - ((double)xj.y + (double)lj4.y),
-                                   ((double)xi.z + (double)li.z) - ((double)xj.z + (double)lj4.z)};
-                    double r2d = 0.0;
+                const float e0 = stn.edge2[0], e1 = stn.edge2[1], e2 = stn.edge2[2], e3 = stn.edge2[3];
+                for (int q0 = 0; q0 < npad; q0 += 32) {
+                    const float4 xj = tile[q0 + lane];
+                    const int jraw = __float_as_int(xj.w);
+                    const int j = jraw & 0x7fffffff;
+                    float dx, dy, dz;
+                    if (FAST) { dx = xi - xj.x; dy = yi - xj.y; dz = zi - xj.z; }
+                    else {
+                        dx = min_image1(xi, xj.x, m.box[0], m.inv_box[0]);
+                        dy = min_image1(yi, xj.y, m.box[1], m.inv_box[1]);
+                        dz = min_image1(zi, xj.z, m.box[2], m.inv_box[2]);
+                    }
+                    const float r2 = dx * dx + dy * dy + dz * dz;
+                    bool valid = r2 < rmax2t;   // false for the NaN of a padding entry
+                    if (!__any_sync(full, valid)) continue;
+                    const bool nearby = valid && r2 <= exr2;
+                    if (__any_sync(full, nearby)) {   // the atom itself and excluded pairs are never listed (R-9)
+                        bool ex = (j == i) | (j == ex4[0]) | (j == ex4[1]) | (j == ex4[2]) | (j == ex4[3]);
+                        if (n_ex > 4) {
+                            for (int base = 0; base < n_ex; base += 32) {
+                                int mine = (base + lane < n_ex) ? sorted_of[excl_idx[ex_lo + base + lane]] : -1;
+                                int lim = min(32, n_ex - base);
+                                for (int e = 0; e < lim; ++e) ex |= (__shfl_sync(full, mine, e) == j);
+                            }
+                        }
+                        valid = valid && !ex;
+                    }
+                    const bool ljp = lj_i && jraw < 0;
+                    bool pass[N_ROWS];
 #pragma unroll
-                    for (int k = 0; k < 3; ++k) {
-                        double L = (double)m.box[k];
-                        d[k] -= L * rint(d[k] / L);
-                        r2d += d[k] * d[k];
+                    for (int k = 0; k < N_ROWS; ++k) {
+                        pass[k] = false;
+                        if (!JB_ROW_ON(k)) continue;
+                        const Row &R = rows.r[k];
+                        pass[k] = valid && (!R.lj_only || ljp) && r2 >= R.r2min && r2 < R.r2max;
+                    }
+                    const bool tie = valid && (fabsf(r2 - e0) < BUILD_TIE || fabsf(r2 - e1) < BUILD_TIE ||
+                                               fabsf(r2 - e2) < BUILD_TIE || fabsf(r2 - e3) < BUILD_TIE);
+                    if (tie) {   // decide in fp64 from the full positions, like the oracle
+                        float4 hi_j = xs[j], li = xl[i], lo_j = xl[j];
+                        double d[3] = {((double)xi4.x + (double)li.x) - ((double)hi_j.x + (double)lo_j.x),
+                                       ((double)xi4.y + (double)li.y) - ((double)hi_j.y + (double)lo_j.y),
+                                       ((double)xi4.z + (double)li.z) - ((double)hi_j.z + (double)lo_j.z)};
+                        double r2d = 0.0;
+#pragma unroll
+                        for (int k = 0; k < 3; ++k) {
+                            double L = (double)m.box[k];
+                            d[k] -= L * rint(d[k] / L);
+                            r2d += d[k] * d[k];
+                        }
+#pragma unroll
+                        for (int k = 0; k < N_ROWS; ++k) {
+                            if (!JB_ROW_ON(k)) continue;
+                            const Row &R = rows.r[k];
+                            pass[k] = (!R.lj_only || ljp) && r2d >= R.r2min_d && r2d < R.r2max_d;
+                        }
                     }
 #pragma unroll
                     for (int k = 0; k < N_ROWS; ++k) {
                         if (!JB_ROW_ON(k)) continue;
-                        const Row &R = rows.r[k];
-                        pass[k] = (!R.lj_only || ljp) && r2d >= R.r2min_d && r2d < R.r2max_d;
+                        const unsigned mask = __ballot_sync(full, pass[k]);
+                        if (pass[k]) {
+                            int pos = count[k] + __popc(mask & lt_mask);
+                            if (pos < rows.r[k].cap) rbase[k][pos] = j;
+                        }
+                        count[k] += __popc(mask);
                     }
                 }
+                if (c1 >= total) {   // last chunk: publish the counts
+                    if (lane == 0) {
 #pragma unroll
-                for (int k = 0; k < N_ROWS; ++k) {
-                    if (!JB_ROW_ON(k)) continue;
-                    const unsigned mask = __ballot_sync(full, pass[k]);
-                    if (pass[k]) {
-                        int pos = count[k] + __popc(mask & lt_mask);
-                        if (pos < rows.r[k].cap) rbase[k][pos] = j;
+                        for (int k = 0; k < N_ROWS; ++k) {
+                            if (!JB_ROW_ON(k)) continue;
+                            const Row &R = rows.r[k];
+                            R.cnt[i] = min(count[k], R.cap);
+                            if (count[k] > R.cap) atomicOr(&ctr->err, (unsigned)ERR_OVERFLOW);
+                            if (count[k] > ctr->max_row[k]) atomicMax(&ctr->max_row[k], count[k]);
+                        }
                     }
-                    count[k] += __popc(mask);
+                } else if (lane == 0) {
+#pragma unroll
+                    for (int k = 0; k < N_ROWS; ++k) if (JB_ROW_ON(k)) s_count[i - g0][k] = count[k];
                 }
             }
         }
-        if (have && lane == 0) {
-#pragma unroll
-            for (int k = 0; k < N_ROWS; ++k) {
-                if (!JB_ROW_ON(k)) continue;
-                const Row &R = rows.r[k];
-                R.cnt[i] = min(count[k], R.cap);
-                if (count[k] > R.cap) atomicOr(&ctr->err, (unsigned)ERR_OVERFLOW);
-                if (count[k] > ctr->max_row[k]) atomicMax(&ctr->max_row[k], count[k]);
-            }
-        }
+        __syncthreads();   // before s_count is zeroed for the next group of atoms
     }
 #undef JB_ROW_ON
 }
@@ -397,8 +444,16 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
         }
     int mask = 0;
     for (int k = 0; k < N_ROWS; ++k) mask |= rows[k].enabled ? (1 << k) : 0;
-#define JB_BUILD(MASK) k_build_rows<MASK><<<(unsigned)g.ncell, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, cell_start, xs, xl, lj, \
-                                                                                    orig, sorted_of, excl_ptr, excl_idx, ctr)
+    // FAST: staged coordinates relative to the cell centre, no minimum image in the inner loop (see k_build_rows)
+    bool fast = true;
+    for (int k = 0; k < 3; ++k) fast = fast && ((double)rmax_all + 0.5 * cs[k] <= 0.5 * (double)m.box[k]) && m.box[k] <= 512.f;
+#define JB_BUILD(MASK)                                                                                                        \
+    do {                                                                                                                      \
+        if (fast) k_build_rows<MASK, true><<<(unsigned)g.ncell, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, cell_start, xs, xl, lj, \
+                                                                                       orig, sorted_of, excl_ptr, excl_idx, ctr);         \
+        else k_build_rows<MASK, false><<<(unsigned)g.ncell, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, cell_start, xs, xl, lj,      \
+                                                                                    orig, sorted_of, excl_ptr, excl_idx, ctr);            \
+    } while (0)
     switch (mask) {
         case 0x0F: JB_BUILD(0x0F); break;   // S M L V   (JUMP with Coulomb and LJ jumps)
         case 0x27: JB_BUILD(0x27); break;   // S M L W   (Coulomb jumps only, R-13)
