@@ -147,56 +147,56 @@ __device__ inline ChainConst chain_const(const Model &m, const Row &rowM, const 
     c.SM = (float)c.NM * c.LM; c.S = c.SM + (float)c.NL * c.LL;
     return c;
 }
-// proposal `block` of a chain: sa = (E, U, |F_ij| / L_Y, ring << 31 | j_orig), sb = (n_x, n_y, n_z, -), n = F_ij / |F_ij|
+// state-independent part of a proposal, from its Philox block w: ring pick and partner, then
+// goL = |F_ij| / L_Y and n = F_ij / |F_ij|; tag = ring << 31 | j_orig (event log only)
 template <bool WANT_J>
-__device__ inline void propose(const Model &m, const Row &rowM, const Row &rowL, const float4 *__restrict__ xs,
-                               const int *__restrict__ orig, const ChainConst &c, int i, unsigned atom, const float4 &xi,
-                               unsigned step, unsigned stream, unsigned block, float4 &sa, float4 &sb) {
-    uint32_t w[4];
-    philox4x32_10(atom, step, stream, block, m.key0, m.key1, w);
-    const float E = -logf(u01(w[0]));
-    int ring = (u01(w[1]) * c.S < c.SM) ? 0 : 1;  // ring pick
+__device__ inline void propose_pair(const Model &m, const Row &rowM, const Row &rowL, const float4 *__restrict__ xs,
+                                    const int *__restrict__ orig, const ChainConst &c, int i, const float4 &xi,
+                                    const uint32_t w[4], float &goL, float &nx, float &ny, float &nz, int &tag) {
+    int ring = (u01(w[1]) * c.S < c.SM) ? 0 : 1;
     if (ring == 0 && c.NM == 0) ring = 1;
     if (ring == 1 && c.NL == 0) ring = 0;
     const int cnt = ring == 0 ? c.NM : c.NL;
     const int k = (int)__umulhi(w[2], (unsigned)cnt);
     const int j = ring == 0 ? rowM.idx[(size_t)i * rowM.cap + k] : rowL.idx[(size_t)i * rowL.cap + k];
-    const float U = u01(w[3]);
     float dx, dy, dz, rinv;
     const float fr = fij_coul(m, xi, xs[j], dx, dy, dz, rinv);
     const float sg = (fr > 0.f ? rinv : -rinv);  // n = F/|F|
     const float LY = ring == 0 ? c.LM : c.LL;
-    int tag = 0;
+    goL = fabsf(fr) / LY;
+    nx = dx * sg; ny = dy * sg; nz = dz * sg;
+    tag = 0;
     if (WANT_J) tag = orig[j] | (ring << 31);
-    sa = make_float4(E, U, fabsf(fr) / LY, __int_as_float(tag));
-    sb = make_float4(dx * sg, dy * sg, dz * sg, 0.f);
 }
 
+// The chain of one atom, run by the G lanes of its group.  The whole warp executes the loop together (while any
+// of its 32 / G groups still has a live chain, finished groups predicated off): groups of one warp never run one
+// after the other, and every shuffle and ballot is a full-warp one.  `on` = this lane's atom exists and runs C'.
 template <int G, bool LOG>
-__device__ void chain_C(const Model &m, const UpdateArgs &A, int i, unsigned atom, const float4 &xi, float sbm,
+__device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, int i, unsigned atom, const float4 &xi, float sbm,
                         float ax, float ay, float az, float H, unsigned stream, unsigned step, float &vx, float &vy,
-                        float &vz, Tally &tl, unsigned gmask, int gl, int gshift) {
+                        float &vz, Tally &tl, int gl, int gshift) {
+    const unsigned full = 0xffffffffu;
     const float eps = m.eps_jump, beta = m.beta;
     const bool bps = isinf(eps), lead = gl == 0;
-    const ChainConst c = chain_const(m, A.rowM, A.rowL, i, xi.w);
+    ChainConst c;
+    c.NM = c.NL = 0; c.LM = c.LL = c.SM = c.S = 0.f;
+    if (on) c = chain_const(m, A.rowM, A.rowL, i, xi.w);
     const float S = c.S;
-    if (!(S > 0.f)) {  // no partner: lambda-bar = 0, the clock never rings
-        vx += H * ax; vy += H * ay; vz += H * az;
-        if (lead) {
-            tl.expiries++;
-            if (LOG) log_event(A, step, stream, atom, 0, -1, -1, 0, 0, INFINITY, 0.f, 0.f, 0.f);
-        }
-        return;
+    bool done = !(on && S > 0.f);
+    if (on && done && lead) {  // no partner: lambda-bar = 0, the clock never rings; v drifts to the end below
+        tl.expiries++;
+        if (LOG) log_event(A, step, stream, atom, 0, -1, -1, 0, 0, INFINITY, 0.f, 0.f, 0.f);
     }
     const float lam0 = bps ? 0.f : (1.f / eps) * beta * kInvSqrt2Pi / sbm;
     const float a2 = ax * ax + ay * ay + az * az, esb = eps * sbm;
     const unsigned gbits = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
     float vex = vx, vey = vy, vez = vz, te = 0.f;   // epoch start: velocity and time after the last accepted jump
     float t_run = 0.f;                              // time of the last proposal so far
-    float Bv = 0.f, lam = 0.f, den = 1.f;
+    float Bv = 0.f, lam = 1.f, den = 1.f;
     bool fresh = true;
     unsigned kb = 0, gblock = 0;
-    for (;;) {
+    while (__any_sync(full, !done)) {
         if (fresh) {   // the bound of this epoch, P:L373-374 (R-11)
             const float tau = H - te;
             const float va = vex * ax + vey * ay + vez * az, v2 = vex * vex + vey * vey + vez * vez;
@@ -205,17 +205,24 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, int i, unsigned ato
             den = bps ? Bv : fmaf(Bv, esb, kInvSqrt2Pi);
             fresh = false;
         }
-        float4 sa, sb;
-        propose<LOG>(m, A.rowM, A.rowL, A.xs, A.orig, c, i, atom, xi, step, stream, kb + (unsigned)gl, sa, sb);
-        const float T_ = sa.x / lam;   // P:L379 (lam = 0: +inf)
+        // lane gl draws Philox block kb + gl of the chain's stream: (E, ring, j, U) of proposal kb + gl (R-15)
+        uint32_t w[4];
+        philox4x32_10(atom, step, stream, kb + (unsigned)gl, m.key0, m.key1, w);
+        const float T_ = done ? INFINITY : -logf(u01(w[0])) / lam;   // P:L379 (lam = 0: +inf)
         float tk = t_run;              // time of my proposal: ((t_run + T_0) + T_1) + ... + T_gl, the sequential order
+        if (G == 1) tk += T_;
+        else {
 #pragma unroll
-        for (int q = 0; q < G; ++q) {
-            const float Tq = __shfl_sync(gmask, T_, q, G);
-            if (q <= gl) tk += Tq;
+            for (int q = 0; q < G; ++q) {
+                const float Tq = __shfl_sync(full, T_, q, G);
+                if (q <= gl) tk += Tq;
+            }
         }
-        const bool alive = tk <= H;    // the chain expires at the first proposal with t + T > delta/2
-        const float U = sa.y, goL = sa.z;
+        const bool alive = !done && tk <= H;   // the chain expires at the first proposal with t + T > delta/2
+        const float U = u01(w[3]);
+        float goL = 0.f, nx = 0.f, ny = 0.f, nz = 0.f;
+        int tag = 0;
+        if (alive) propose_pair<LOG>(m, A.rowM, A.rowL, A.xs, A.orig, c, i, xi, w, goL, nx, ny, nz, tag);
         float p = 0.f, vn = 0.f;
         bool acc = false;
         // p <= |F_ij| / L_Y always (Theta(eta) <= eta_+ + 1/sqrt(2 pi), eta <= eps sqrt(beta m) B_v): most proposals
@@ -223,49 +230,53 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, int i, unsigned ato
         if (alive && goL > 0.f && (LOG || U <= goL * 1.0001f)) {
             const float s = tk - te;
             const float cx = fmaf(s, ax, vex), cy = fmaf(s, ay, vey), cz = fmaf(s, az, vez);  // the advanced v
-            vn = cx * sb.x + cy * sb.y + cz * sb.z;
+            vn = cx * nx + cy * ny + cz * nz;
             const float pub = bps ? goL * fmaxf(vn, 0.f) / den : goL * (fmaxf(esb * vn, 0.f) + kInvSqrt2Pi) / den;
             if (LOG || U <= pub * 1.0001f) {
                 p = bps ? fmaxf(vn, 0.f) * goL / den : goL * theta_of(esb * vn) / den;  // P:L397 with sqrt(beta)
                 acc = U <= p;
             }
         }
-        const unsigned alive_m = (__ballot_sync(gmask, alive) >> gshift) & gbits;
-        const unsigned acc_m = (__ballot_sync(gmask, acc) >> gshift) & gbits;
+        const unsigned alive_m = (__ballot_sync(full, alive) >> gshift) & gbits;
+        const unsigned acc_m = (__ballot_sync(full, acc) >> gshift) & gbits;
         const int n_alive = __popc(alive_m);
         const int f = acc_m ? __ffs(acc_m) - 1 : -1;   // first accepted proposal of the batch
         const int n_used = f >= 0 ? f + 1 : n_alive;
+        const int fs = f >= 0 ? f : 0;
+        const float tf = __shfl_sync(full, tk, fs, G), vnf = __shfl_sync(full, vn, fs, G);
+        const float fnx = __shfl_sync(full, nx, fs, G), fny = __shfl_sync(full, ny, fs, G), fnz = __shfl_sync(full, nz, fs, G);
+        const float t_last = __shfl_sync(full, tk, G - 1, G);
+        if (done) continue;
         if (gl < n_used) { tl.max_gl = fmaxf(tl.max_gl, goL); tl.max_p = fmaxf(tl.max_p, p); }
         if (lead) tl.proposals += (unsigned)n_used;
         float gt = 0.f;
         int att = 0;
         if (f >= 0) {   // kick (7) on the velocity at the time of proposal f; a new epoch starts there
-            const float tf = __shfl_sync(gmask, tk, f, G), vnf = __shfl_sync(gmask, vn, f, G);
-            const float nx = __shfl_sync(gmask, sb.x, f, G), ny = __shfl_sync(gmask, sb.y, f, G), nz = __shfl_sync(gmask, sb.z, f, G);
             if (!bps) gt = gtilde(esb * vnf, atom, step, stream + 16u, gblock, m, att);
             const float s = tf - te;
             float cx = fmaf(s, ax, vex), cy = fmaf(s, ay, vey), cz = fmaf(s, az, vez);
-            jump_kick(eps, sbm, nx, ny, nz, gt, cx, cy, cz);
+            jump_kick(eps, sbm, fnx, fny, fnz, gt, cx, cy, cz);
             vex = cx; vey = cy; vez = cz; te = tf; t_run = tf;
             fresh = true;
             if (lead) { tl.accepts++; tl.gt_attempts += att; }
         }
         if (LOG) {
-            const int tag = __float_as_int(sa.w);
             if (gl < n_used)
                 log_event(A, step, stream, atom, (int)kb + gl, (int)((unsigned)tag >> 31), tag & 0x7fffffff, gl == f ? 1 : 0,
                           gl == f ? att : 0, T_, p, U, gl == f ? gt : 0.f);
             else if (f < 0 && gl == n_alive)
                 log_event(A, step, stream, atom, (int)kb + gl, -1, -1, 0, 0, T_, 0.f, 0.f, 0.f);
         }
-        if (f >= 0) { kb += (unsigned)(f + 1); continue; }
-        if (n_alive < G) break;   // expired inside this batch
-        t_run = __shfl_sync(gmask, tk, G - 1, G);
-        kb += (unsigned)G;
+        if (f >= 0) kb += (unsigned)(f + 1);
+        else if (n_alive < G) {   // expired inside this batch
+            done = true;
+            if (lead) tl.expiries++;
+        } else { t_run = t_last; kb += (unsigned)G; }
     }
-    if (lead) tl.expiries++;
-    const float s_end = H - te;   // drift to the end of the half-step
-    vx = fmaf(s_end, ax, vex); vy = fmaf(s_end, ay, vey); vz = fmaf(s_end, az, vez);
+    if (on) {   // drift to the end of the half-step
+        const float s_end = H - te;
+        vx = fmaf(s_end, ax, vex); vy = fmaf(s_end, ay, vey); vz = fmaf(s_end, az, vez);
+    }
 }
 
 // ---- step (J'): Algorithm 5 (R-14) ---------------------------------------------------------------------------
@@ -333,37 +344,46 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
     const int gt_id = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gt_id / G, gl = gt_id % G;
     const int lane = threadIdx.x & 31, gshift = lane & ~(G - 1);
-    const unsigned gmask = (G == 32) ? full : (((1u << G) - 1u) << gshift);
     const bool live = i < m.n, lead = gl == 0;
     Tally tl = {0u, 0u, 0u, 0u, 0.f, 0.f};
     float disp2 = 0.f;
     bool bad = false;
-    if (live) {
-        const float4 xi = A.xs[i];
-        float4 v4 = A.vs[i];
-        float vx = v4.x, vy = v4.y, vz = v4.z;
-        const float2 mi = A.mi[i];  // (kcal-scaled 1/m, sqrt(beta m))
-        const unsigned atom = (unsigned)A.orig[i];
-#pragma unroll
-        for (int ph = 0; ph < 2; ++ph) {
-            const Phase &P = A.ph[ph];
-            if (P.kind == 0) continue;
-            float ax = 0.f, ay = 0.f, az = 0.f;
-            if (P.use_grad) {  // a = -M^-1 F
-                float4 g = A.grad[ph][i];
-                if (A.grad_b[ph]) { float4 b = A.grad_b[ph][i]; g.x = b.x + g.x; g.y = b.y + g.y; g.z = b.z + g.z; }
-                ax = -mi.x * g.x; ay = -mi.x * g.y; az = -mi.x * g.z;
-            }
-            if (P.kind == 1 || !JUMPS) {
-                vx += P.H * ax; vy += P.H * ay; vz += P.H * az;
-            } else {
-                const float2 lji = A.lj[i];
-                if (P.reverse && P.lj) chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
-                if (P.coul) chain_C<G, LOG>(m, A, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl, gmask, gl, gshift);
-                else if (P.use_grad) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
-                if (!P.reverse && P.lj) chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
+    float4 xi = make_float4(0.f, 0.f, 0.f, 0.f), v4 = xi;
+    float2 mi = make_float2(1.f, 1.f);   // (kcal-scaled 1/m, sqrt(beta m))
+    unsigned atom = 0u;
+    if (live) { xi = A.xs[i]; v4 = A.vs[i]; mi = A.mi[i]; atom = (unsigned)A.orig[i]; }
+    float vx = v4.x, vy = v4.y, vz = v4.z;
+    // the velocity half-phases: every lane of the warp walks through them together (chain_C is a warp-wide loop)
+    // (not unrolled, and each chain routine appears once: the kernel's code stays small enough for the
+    // instruction cache -- "no instruction" was the second largest stall of the unrolled version)
+#pragma unroll 1
+    for (int ph = 0; ph < 2; ++ph) {
+        const Phase P = A.ph[ph];
+        if (P.kind == 0) continue;
+        float ax = 0.f, ay = 0.f, az = 0.f;
+        if (P.use_grad && live) {  // a = -M^-1 F
+            float4 g = A.grad[ph][i];
+            if (A.grad_b[ph]) { float4 b = A.grad_b[ph][i]; g.x = b.x + g.x; g.y = b.y + g.y; g.z = b.z + g.z; }
+            ax = -mi.x * g.x; ay = -mi.x * g.y; az = -mi.x * g.z;
+        }
+        if (P.kind == 1 || !JUMPS) {
+            vx += P.H * ax; vy += P.H * ay; vz += P.H * az;
+        } else {
+            float2 lji = make_float2(0.f, 0.f);
+            if (live && P.lj) lji = A.lj[i];
+            // slots: J' if the phase is a closing one (J'C'), then C', then J' if it is an opening one (C'J')
+#pragma unroll 1
+            for (int slot = 0; slot < 3; ++slot) {
+                if (slot == 1) {
+                    if (P.coul) chain_C<G, LOG>(m, A, live, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl, gl, gshift);
+                    else if (P.use_grad) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
+                } else if (P.lj && live && (slot == 0) == (P.reverse != 0)) {
+                    chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
+                }
             }
         }
+    }
+    if (live) {
         if (A.do_aoa && lead) {
             // positions are integrated in fp64 as hi + lo (hi = the fp32 value every pair kernel reads):
             // fp32 rounding of x (ulp(18 A) = 2e-6 A) through the stiff O-H bonds is otherwise the
