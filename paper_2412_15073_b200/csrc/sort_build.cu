@@ -171,8 +171,10 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                                                               const int *__restrict__ orig, const int *__restrict__ sorted_of,
                                                               const int *__restrict__ excl_ptr, const int *__restrict__ excl_idx,
                                                               Counters *ctr) {
-    __shared__ int seg_beg[BUILD_MAXSEG];
-    __shared__ int seg_pre[BUILD_MAXSEG + 1];   // exclusive prefix of the run lengths
+    __shared__ int seg_beg[BUILD_MAXSEG];       // stencil runs in ascending cell key (many are empty) ...
+    __shared__ int seg_pre[BUILD_MAXSEG + 1];   // ... their lengths, then (length << 10 | non-empty) prefix sums
+    __shared__ int run_beg[BUILD_MAXSEG];       // the non-empty runs, compacted: first atom ...
+    __shared__ int run_pre[BUILD_MAXSEG + 1];   // ... and exclusive prefix of the lengths
     __shared__ float4 tile[BUILD_CHUNK];        // (x, y, z, sorted index | LJ flag in bit 31)
     __shared__ int scan_tmp[BUILD_THREADS];
     __shared__ int s_count[BUILD_MAXATOMS][N_ROWS];
@@ -216,11 +218,12 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
     }
     if (tid == 0) seg_pre[0] = 0;
     __syncthreads();
-    {   // inclusive scan of seg_pre[1..nseg] (each thread a contiguous slice, then a block scan of the slice sums)
+    {   // inclusive scan of (length << 10 | non-empty) over seg_pre[1..nseg] (each thread a contiguous slice, then a
+        // block scan of the slice sums): one pass gives the candidate offsets and the compacted run indices
         int per = (nseg + BUILD_THREADS - 1) / BUILD_THREADS;
         int lo = min(tid * per, nseg), hi = min(lo + per, nseg);
         int sum = 0;
-        for (int k = lo; k < hi; ++k) sum += seg_pre[k + 1];
+        for (int k = lo; k < hi; ++k) { int len = seg_pre[k + 1]; sum += (len << 10) | (len > 0 ? 1 : 0); }
         scan_tmp[tid] = sum;
         __syncthreads();
         for (int off = 1; off < BUILD_THREADS; off <<= 1) {
@@ -230,10 +233,15 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
             __syncthreads();
         }
         int run = scan_tmp[tid] - sum;
-        for (int k = lo; k < hi; ++k) { run += seg_pre[k + 1]; seg_pre[k + 1] = run; }
+        for (int k = lo; k < hi; ++k) {
+            int len = seg_pre[k + 1];
+            if (len > 0) { run_beg[run & 1023] = seg_beg[k]; run_pre[run & 1023] = run >> 10; }
+            run += (len << 10) | (len > 0 ? 1 : 0);
+        }
+        if (tid == BUILD_THREADS - 1) { seg_pre[0] = run; run_pre[run & 1023] = run >> 10; }
     }
     __syncthreads();
-    const int total = seg_pre[nseg];
+    const int total = seg_pre[0] >> 10, nrun = seg_pre[0] & 1023;
     const float rmax2t = rmax_all * rmax_all + BUILD_TIE;
     const unsigned lt_mask = (1u << lane) - 1u;
 #define JB_ROW_ON(k) (MASK >= 0 ? (((MASK) >> (k)) & 1) != 0 : rows.r[k].enabled != 0)
@@ -244,24 +252,24 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
             const int c1 = min(c0 + BUILD_CHUNK, total);
             const int npad = (c1 - c0 + 31) & ~31;
             __syncthreads();   // the previous chunk has been consumed (and s_count is zeroed)
-            {   // ---- stage the runs that intersect [c0, c1): first one by bisection, then one run per warp iteration
-                int lo_s = 0, hi_s = nseg;   // first run with seg_pre[s + 1] > c0
-                while (lo_s < hi_s) { int mid = (lo_s + hi_s) >> 1; if (seg_pre[mid + 1] > c0) hi_s = mid; else lo_s = mid + 1; }
-                for (int sgi = lo_s + warp; sgi < nseg; sgi += BUILD_WARPS) {
-                    int p0 = seg_pre[sgi], p1 = seg_pre[sgi + 1];
-                    if (p0 >= c1) break;
-                    int lo = max(p0, c0), hi = min(p1, c1);
-                    for (int q = lo + lane; q < hi; q += 32) {
-                        int j = seg_beg[sgi] + (q - p0);
-                        float4 x = xs[j];
-                        if (FAST) {
-                            x.x = near_image1(x.x - ctr3[0], m.box[0], m.inv_box[0]);
-                            x.y = near_image1(x.y - ctr3[1], m.box[1], m.inv_box[1]);
-                            x.z = near_image1(x.z - ctr3[2], m.box[2], m.inv_box[2]);
-                        }
-                        x.w = __int_as_float(j | (lj[j].y > 0.f ? (int)0x80000000 : 0));
-                        tile[q - c0] = x;
+            {   // ---- stage [c0, c1): thread t takes the candidates c0 + t, + BUILD_THREADS, ...; its run is found by one
+                // bisection and then advanced linearly
+                int q = c0 + tid, r = 0;
+                if (q < c1) {
+                    int hi_r = nrun - 1;   // last run with run_pre[r] <= q
+                    while (r < hi_r) { int mid = (r + hi_r + 1) >> 1; if (run_pre[mid] <= q) r = mid; else hi_r = mid - 1; }
+                }
+                for (; q < c1; q += BUILD_THREADS) {
+                    while (run_pre[r + 1] <= q) ++r;
+                    const int j = run_beg[r] + (q - run_pre[r]);
+                    float4 x = xs[j];
+                    if (FAST) {
+                        x.x = near_image1(x.x - ctr3[0], m.box[0], m.inv_box[0]);
+                        x.y = near_image1(x.y - ctr3[1], m.box[1], m.inv_box[1]);
+                        x.z = near_image1(x.z - ctr3[2], m.box[2], m.inv_box[2]);
                     }
+                    x.w = __int_as_float(j | (lj[j].y > 0.f ? (int)0x80000000 : 0));
+                    tile[q - c0] = x;
                 }
                 for (int q = (c1 - c0) + tid; q < npad; q += BUILD_THREADS) tile[q] = make_float4(nanf(""), 0.f, 0.f, 0.f);   // padding: r^2 = NaN fails every test
             }
@@ -340,8 +348,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                         const Row &R = rows.r[k];
                         pass[k] = valid && (!R.lj_only || ljp) && r2 >= R.r2min && r2 < R.r2max;
                     }
-                    const bool tie = valid && (fabsf(r2 - e0) < BUILD_TIE || fabsf(r2 - e1) < BUILD_TIE ||
-                                               fabsf(r2 - e2) < BUILD_TIE || fabsf(r2 - e3) < BUILD_TIE);
+                    const bool tie = valid && fminf(fminf(fabsf(r2 - e0), fabsf(r2 - e1)), fminf(fabsf(r2 - e2), fabsf(r2 - e3))) < BUILD_TIE;
                     if (tie) {   // decide in fp64 from the full positions, like the oracle
                         float4 hi_j = xs[j], li = xl[i], lo_j = xl[j];
                         double d[3] = {((double)xi4.x + (double)li.x) - ((double)hi_j.x + (double)lo_j.x),
