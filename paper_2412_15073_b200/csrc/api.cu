@@ -18,6 +18,9 @@ struct jump_ctx {
     Model m;
     SortGrid g;
     cudaStream_t st;
+    cudaStream_t st2;            // side stream: the bonded kernel runs beside the pair kernel (fork / join by events)
+    cudaEvent_t ev_fork, ev_join;
+    bool bonded_in_flight;
     int n;
     double kT, dt, alpha, rM, lo;  // ps; lo = max(r_c - h - skin, 0)
     double GM, GL, GV, qmax, eps_max, sig_min, sig_max;
@@ -270,12 +273,39 @@ static int bonded_only(jump_ctx *c) {  // fbond at the current positions
     CK(cudaGetLastError());
     return 0;
 }
+// the same on the side stream: fork after everything enqueued so far, join_bonded() before fbond is read.
+// The bonded kernel (a few thousand latency-bound threads) then overlaps the pair kernel instead of preceding it.
+static int bonded_fork(jump_ctx *c) {
+    CK(cudaEventRecord(c->ev_fork, c->st));
+    CK(cudaStreamWaitEvent(c->st2, c->ev_fork, 0));
+    if (c->prof) {   // bracket on the side stream (the categories then overlap in time)
+        std::pair<cudaEvent_t, cudaEvent_t> ev;
+        if (!c->prof_free.empty()) { ev = c->prof_free.back(); c->prof_free.pop_back(); }
+        else { cudaEventCreate(&ev.first); cudaEventCreate(&ev.second); }
+        cudaEventRecord(ev.first, c->st2);
+        c->prof_pend[PROF_BONDED].push_back(ev);
+    }
+    launch_bonded_lanes(c->m, c->topo, c->xs, c->xl, c->orig, c->sorted_of, c->fbond, c->st2, &c->launches);
+    if (c->prof) cudaEventRecord(c->prof_pend[PROF_BONDED].back().second, c->st2);
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(c->ev_join, c->st2));
+    c->bonded_in_flight = true;
+    return 0;
+}
+static int bonded_join(jump_ctx *c) {
+    if (!c->bonded_in_flight) return 0;
+    CK(cudaStreamWaitEvent(c->st, c->ev_join, 0));
+    c->bonded_in_flight = false;
+    return 0;
+}
 // F0 kept as fnb + fbond (the integrator adds the two)
 static int compute_f0(jump_ctx *c) {
-    int r = compute_short_nb(c, c->fnb);
+    int r = bonded_fork(c);
+    if (r) return r;
+    r = compute_short_nb(c, c->fnb);
     if (r) return r;
     c->f0_valid = true;
-    return bonded_only(c);
+    return bonded_join(c);
 }
 static GradRef gr_f0(const jump_ctx *c) { return gr(c->fnb, c->fbond); }
 static int ensure_f0(jump_ctx *c) { return c->f0_valid ? 0 : compute_f0(c); }
@@ -288,10 +318,12 @@ static int compute_f0_sum(jump_ctx *c) {
 }
 // unsplit force to r_long as ftmp2 + fbond (BAOAB comparator); invalidates F0
 static int compute_full_split(jump_ctx *c) {
+    int r = bonded_fork(c);
+    if (r) return r;
     pair(c, ROW_F, W_FULL, W_FULL, c->ftmp2, 0, false);
     CK(cudaGetLastError());
     c->f0_valid = false;
-    return bonded_only(c);
+    return bonded_join(c);
 }
 static GradRef gr_full(const jump_ctx *c) { return gr(c->ftmp2, c->fbond); }
 static int compute_long(jump_ctx *c, float4 *out) {
@@ -635,6 +667,12 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     if (p->r_mid > 0.0 && (p->r_mid < p->r_short - p->r_switch || p->r_mid > p->r_long)) return JUMP_E_ARG;
     jump_ctx *c = new jump_ctx();
     c->st = (cudaStream_t)cuda_stream;
+    c->st2 = nullptr; c->ev_fork = c->ev_join = nullptr; c->bonded_in_flight = false;
+    if (cudaStreamCreateWithFlags(&c->st2, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        c->err = "side stream / events"; *out = c; return JUMP_E_CUDA;
+    }
     c->d_pos = d_pos; c->d_vel = d_vel;
     c->step = c->outer = c->rebuilds = c->launches = 0;
     c->sticky = 0;
@@ -650,7 +688,11 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
 extern "C" void jump_free(jump_ctx *c) {
     if (!c) return;
     prof_collect(c);
+    if (c->st2) cudaStreamSynchronize(c->st2);
     for (auto &ev : c->prof_free) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
+    if (c->ev_fork) cudaEventDestroy(c->ev_fork);
+    if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->st2) cudaStreamDestroy(c->st2);
     for (void *q : c->owned) cudaFree(q);
     delete c;
 }
