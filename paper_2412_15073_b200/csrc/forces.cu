@@ -35,9 +35,16 @@ __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *_
     const int cnt = row.cnt[i];
     const int *__restrict__ ridx = row.idx + (size_t)i * row.cap;
     float fx = 0.f, fy = 0.f, fz = 0.f, en = 0.f;
+    // software pipeline: the index two iterations ahead and the position one iteration ahead are in flight while
+    // the current entry is evaluated (the gathers' L1/L2 latency was the kernel's largest stall)
+    int j1 = lane < cnt ? ridx[lane] : 0, j2 = lane + 32 < cnt ? ridx[lane + 32] : 0;
+    float4 x1 = xs[j1];
     for (int k = lane; k < cnt; k += 32) {
-        int j = ridx[k];
-        float4 xj = xs[j];
+        const int j = j1;
+        const float4 xj = x1;
+        j1 = j2;
+        x1 = xs[j1];
+        j2 = k + 64 < cnt ? ridx[k + 64] : 0;
         float ax, ay, az, bx, by, bz;
         image_pair1(xi.x, xj.x, m.box[0], m.inv_box[0], ax, bx);
         image_pair1(xi.y, xj.y, m.box[1], m.inv_box[1], ay, by);
