@@ -165,6 +165,86 @@ def timed_blocks(torch, sim, stream, call, n_steps, block, flush):
     return sum(a.elapsed_time(b) for a, b in evs)
 
 
+def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, props, peaks):
+    """Per-kernel device times of K more steps (CUDA events on the streams the kernels are launched on, recorded by
+    the library around each kernel group) against each kernel's roofline.  Returns (dominant line, other lines)."""
+    with torch.cuda.stream(stream):
+        sim.reset_stats()
+        r0 = sim.stats()["rebuilds"]
+        sim.set_profiling(True)
+        timed_blocks(torch, sim, stream, step_call, K, block, flush)
+        prof = sim.profile()
+        sim.set_profiling(False)
+        pstats = sim.stats()
+        n_pairs_ordered = sim.count_pairs(0, run["r_short"])           # ordered in-range entries of the short row
+        row_entries = sum(sim.count_pairs(k, 1e3) for k in (0, 1, 2, 3) if pstats["cap_row"][k])
+    rebuilds = max(pstats["rebuilds"] - r0, 1)
+    tot_prof = sum(v[0] for v in prof.values())
+    share = {k: (v[0] / tot_prof if tot_prof else 0.0) for k, v in prof.items()}
+    peak_tflops = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+    alu_src = "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (%s sm_max_mhz)" % (props.multi_processor_count, peaks["sm_max_mhz"],
+                                                                      peaks["source"])
+
+    def avg_ms(cat):
+        return prof[cat][0] / max(prof[cat][1], 1)
+
+    def alu_line(kernel, flops, what, cat):
+        ach = flops / (avg_ms(cat) * 1e-3) / 1e12 if avg_ms(cat) > 0 else 0.0
+        return {"kernel": kernel, "bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s",
+                "frac": ach / peak_tflops, "traffic": None, "peak_source": alu_src, "algorithmic": what,
+                "avg_launch_us": 1e3 * avg_ms(cat), "share_of_step": share[cat]}
+
+    half_pairs = n_pairs_ordered / 2.0
+    n_upd = max(prof["update"][1], 1)
+    chains = 2.0 * n * (2 if run["flags"] & 2 else 1)                  # half-phases x (C' [+ J']) per update launch
+    upd_instr = pstats["proposals"] / n_upd * PROPOSAL_INSTR + chains * CHAIN_INSTR
+    build_ms = prof["build"][0] / rebuilds                             # sort (5 kernels) + k_build_rows, per rebuild
+    build_bytes = row_entries * 4.0 + n * 48.0
+    build_ach = build_bytes / (build_ms * 1e-3) / 1e9 if build_ms > 0 else 0.0
+    lines = {
+        "pair": alu_line("k_pair (short-range switched pair gradient, a5)", half_pairs * FLOPS_PER_PAIR,
+                         "%.0f in-range half pairs x %d flop" % (half_pairs, FLOPS_PER_PAIR), "pair"),
+        "update": alu_line("k_update (jump chains C'J' of two half-phases + A-O-A, a6-a8)", 2.0 * upd_instr,
+                           "%.0f proposals x %d + %.0f chains x %d FP32/INT-pipe instructions, x 2 flop"
+                           % (pstats["proposals"] / n_upd, PROPOSAL_INSTR, chains, CHAIN_INSTR), "update"),
+        "build": {"kernel": "sort + k_build_rows (a1-a3), one group per rebuild", "bound": "hbm", "achieved": build_ach,
+                  "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": build_ach / peaks["hbm_gbs"], "traffic": None,
+                  "peak_source": "%s HBM copy bandwidth" % peaks["source"],
+                  "algorithmic": "%.0f row entries x 4 B + %d atoms x 48 B" % (row_entries, n),
+                  "avg_launch_us": 1e3 * build_ms, "share_of_step": share["build"]},
+    }
+    share_note = "device time per kernel group / sum over groups; k_bonded runs on a side stream beside k_pair, so the groups overlap"
+    dominant = max(("pair", "update", "build"), key=lambda k: share[k])
+    roofline = dict(lines[dominant], kernel_ms_share=share, share_note=share_note)
+    return roofline, {k: v for k, v in lines.items() if k != dominant}
+
+
+def large_box_rooflines(torch, jb, wl, dev, stream, flush, props, peaks, config, steps):
+    """The same kernel lines on a box large enough to fill the GPU (BASELINE configs[4], ~1e6 atoms: 'throughput and
+    roofline at 1 B200'); the configs[1] box of the headline metric leaves every kernel latency-bound."""
+    sysd, run = wl.make_config(config)
+    n = sysd["n_atoms"]
+    with torch.cuda.stream(stream):
+        sim = jb.JumpSim(sysd, device=dev, stream=stream, **run)
+        sim.baoab_step(300)
+        sim.jump_step(30)
+        sim.sync()
+        ms = timed_blocks(torch, sim, stream, sim.jump_step, steps, BLOCK, flush)
+        line, other = kernel_rooflines(torch, sim, stream, sim.jump_step, steps, BLOCK, flush, run, n, props, peaks)
+        sim.baoab_step(20)
+        sim.sync()
+        ms_b = timed_blocks(torch, sim, stream, sim.baoab_step, steps, BLOCK, flush)
+        err = sim.stats()["error"]
+    sim.close()
+    lines = dict(other)
+    lines["dominant"] = line
+    return {"workload": "BASELINE configs[%d]: %d-atom flexible water box %.1f A, JUMP, equilibrated by 300 BAOAB steps"
+                        % (config, n, sysd["box"]),
+            "steps": steps, "ms_per_step": ms / steps, "ns_per_day": ns_per_day(steps / (ms * 1e-3), run["dt_fs"]),
+            "atom_steps_per_s": n * steps / (ms * 1e-3), "baoab_ms_per_step": ms_b / steps,
+            "jump_vs_baoab": ms_b / ms, "error": err, "kernels": lines}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -174,6 +254,8 @@ def main():
     ap.add_argument("--impl", default="b200")
     ap.add_argument("--equil", type=int, default=2000, help="untimed BAOAB equilibration steps from the lattice start")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--large-config", type=int, default=4,
+                    help="also report the kernel rooflines on this (GPU-filling) config, N=1 only; -1: skip")
     ap.add_argument("--mode", default="jump", choices=["jump", "respa"])
     ap.add_argument("--r-mid", type=float, default=None, help="ring split r_M (default: the config's)")
     ap.add_argument("--skin", type=float, default=None)
@@ -234,51 +316,7 @@ def main():
     stats = sim.stats()
 
     # ---- per-kernel times of the same K steps (CUDA events on the launch stream, separate pass) --------------
-    with torch.cuda.stream(stream):
-        sim.reset_stats()
-        sim.set_profiling(True)
-        timed_blocks(torch, sim, stream, step_call, K, block, flush)
-        prof = sim.profile()
-        sim.set_profiling(False)
-        pstats = sim.stats()
-        n_pairs_ordered = sim.count_pairs(0, run["r_short"])           # ordered in-range entries of the short row
-        row_entries = sum(sim.count_pairs(k, 1e3) for k in (0, 1, 2, 3) if stats["cap_row"][k])
-    tot_prof = sum(v[0] for v in prof.values())
-    share = {k: (v[0] / tot_prof if tot_prof else 0.0) for k, v in prof.items()}
-    peak_tflops = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-    alu_src = "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (%s sm_max_mhz)" % (props.multi_processor_count, peaks["sm_max_mhz"],
-                                                                      peaks["source"])
-
-    def avg_ms(cat):
-        return prof[cat][0] / max(prof[cat][1], 1)
-
-    def alu_line(kernel, flops, what, cat):
-        ach = flops / (avg_ms(cat) * 1e-3) / 1e12 if avg_ms(cat) > 0 else 0.0
-        return {"kernel": kernel, "bound": "alu", "achieved": ach, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": ach / peak_tflops, "traffic": None, "peak_source": alu_src, "algorithmic": what,
-                "avg_launch_us": 1e3 * avg_ms(cat), "share_of_step": share[cat]}
-
-    half_pairs = n_pairs_ordered / 2.0
-    n_upd = max(prof["update"][1], 1)
-    chains = 2.0 * n * (2 if run["flags"] & 2 else 1)                  # half-phases x (C' [+ J']) per update launch
-    upd_instr = pstats["proposals"] / n_upd * PROPOSAL_INSTR + chains * CHAIN_INSTR
-    build_bytes = row_entries * 4.0 + n * 48.0
-    build_ach = build_bytes / (avg_ms("build") * 1e-3) / 1e9 if avg_ms("build") > 0 else 0.0
-    lines = {
-        "pair": alu_line("k_pair (short-range switched pair gradient, a5)", half_pairs * FLOPS_PER_PAIR,
-                         "%.0f in-range half pairs x %d flop" % (half_pairs, FLOPS_PER_PAIR), "pair"),
-        "update": alu_line("k_update (jump chains C'J' of two half-phases + A-O-A, a6-a8)", 2.0 * upd_instr,
-                           "%.0f proposals x %d + %.0f chains x %d FP32/INT-pipe instructions, x 2 flop"
-                           % (pstats["proposals"] / n_upd, PROPOSAL_INSTR, chains, CHAIN_INSTR), "update"),
-        "build": {"kernel": "sort + k_build_rows (a1-a3), one group per rebuild", "bound": "hbm", "achieved": build_ach,
-                  "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": build_ach / peaks["hbm_gbs"], "traffic": None,
-                  "peak_source": "%s HBM copy bandwidth" % peaks["source"],
-                  "algorithmic": "%.0f row entries x 4 B + %d atoms x 48 B" % (row_entries, n),
-                  "avg_launch_us": 1e3 * avg_ms("build"), "share_of_step": share["build"]},
-    }
-    dominant = max(("pair", "update", "build"), key=lambda k: share[k])
-    roofline = dict(lines[dominant], kernel_ms_share=share)
-    roofline_other = {k: v for k, v in lines.items() if k != dominant}
+    roofline, roofline_other = kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, props, peaks)
 
     # ---- same-GPU BAOAB with the unsplit r_long force (reported baseline) -------------------------------------
     with torch.cuda.stream(stream):
@@ -312,6 +350,10 @@ def main():
            "h2d_bytes_per_step": bytes_each_way / block, "d2h_bytes_per_step": bytes_each_way / block,
            "call": "JumpSim.run_host: pinned host (x, v) -> device, jump_refresh, %d steps, device -> host, per call" % block}
 
+    large = None
+    if rank == 0 and world == 1 and args.large_config >= 0:
+        large = large_box_rooflines(torch, jb, wl, dev, stream, flush, props, peaks, args.large_config, 100)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = run_cpu_baseline(sysd, run)
@@ -337,6 +379,8 @@ def main():
                 "events": {"proposals_per_atom_step": stats["proposals"] / (n * (K + W)) if K + W else None,
                            "accepts_per_atom_step": stats["accepts"] / (n * (K + W)), "max_p": stats["max_p"],
                            "error": stats["error"]}}
+        if large is not None:
+            line["roofline_large_box"] = large
         if cpu is not None:
             line["cpu_baseline"] = cpu
         print(json.dumps(line))
