@@ -173,15 +173,12 @@ __device__ inline void propose_pair(const Model &m, const Row &rowM, const Row &
 // of its 32 / G groups still has a live chain, finished groups predicated off): groups of one warp never run one
 // after the other, and every shuffle and ballot is a full-warp one.  `on` = this lane's atom exists and runs C'.
 template <int G, bool LOG>
-__device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, int i, unsigned atom, const float4 &xi, float sbm,
-                        float ax, float ay, float az, float H, unsigned stream, unsigned step, float &vx, float &vy,
+__device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const ChainConst &c, int i, unsigned atom, const float4 &xi,
+                        float sbm, float ax, float ay, float az, float H, unsigned stream, unsigned step, float &vx, float &vy,
                         float &vz, Tally &tl, int gl, int gshift) {
     const unsigned full = 0xffffffffu;
     const float eps = m.eps_jump, beta = m.beta;
     const bool bps = isinf(eps), lead = gl == 0;
-    ChainConst c;
-    c.NM = c.NL = 0; c.LM = c.LL = c.SM = c.S = 0.f;
-    if (on) c = chain_const(m, A.rowM, A.rowL, i, xi.w);
     const float S = c.S;
     bool done = !(on && S > 0.f);
     if (on && done && lead) {  // no partner: lambda-bar = 0, the clock never rings; v drifts to the end below
@@ -281,12 +278,10 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, int i, uns
 
 // ---- step (J'): Algorithm 5 (R-14) ---------------------------------------------------------------------------
 // Rare (LJ carriers only, ~0.15 proposals per fs): every lane of the group runs the same sequential chain.
-__device__ void chain_J(const Model &m, const UpdateArgs &A, int i, unsigned atom, const float4 &xi, float2 lji,
+__device__ void chain_J(const Model &m, const UpdateArgs &A, int NV, int i, unsigned atom, const float4 &xi, float2 lji,
                         float sbm, float H, unsigned stream, unsigned step, float &vx, float &vy, float &vz, Tally &tl,
                         bool lead) {
-    if (!(lji.y > 0.f)) return;
-    const int NV = A.rowV.cnt[i];
-    if (NV == 0) return;
+    if (!(lji.y > 0.f) || NV == 0) return;
     const float L = 0.5f * lji.y * m.GV4se;  // 4 sqrt(eps_i eps_max) G_V; lji.y = 2 sqrt(eps_i)
     float t = 0.f;
     unsigned block = 0;
@@ -351,7 +346,29 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
     float4 xi = make_float4(0.f, 0.f, 0.f, 0.f), v4 = xi;
     float2 mi = make_float2(1.f, 1.f);   // (kcal-scaled 1/m, sqrt(beta m))
     unsigned atom = 0u;
-    if (live) { xi = A.xs[i]; v4 = A.vs[i]; mi = A.mi[i]; atom = (unsigned)A.orig[i]; }
+    // everything the phases read from global memory is requested up front, in one batch of independent loads:
+    // state, the accelerations of both phases, the ring counts (the per-phase dependent loads were a visible
+    // part of a warp's latency chain)
+    const bool jumpy0 = JUMPS && A.ph[0].kind == 2, jumpy1 = JUMPS && A.ph[1].kind == 2;
+    const bool any_coul = (jumpy0 && A.ph[0].coul) || (jumpy1 && A.ph[1].coul);
+    const bool any_lj = (jumpy0 && A.ph[0].lj) || (jumpy1 && A.ph[1].lj);
+    float a0x = 0.f, a0y = 0.f, a0z = 0.f, a1x = 0.f, a1y = 0.f, a1z = 0.f;   // accelerations of the two phases
+    ChainConst cc;
+    cc.NM = cc.NL = 0; cc.LM = cc.LL = cc.SM = cc.S = 0.f;
+    float2 lji = make_float2(0.f, 0.f);
+    int NV = 0;
+    if (live) {
+        xi = A.xs[i]; v4 = A.vs[i]; mi = A.mi[i]; atom = (unsigned)A.orig[i];
+        const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        float4 g0 = z4, g1 = z4, b0 = z4, b1 = z4;
+        if (A.ph[0].kind != 0 && A.ph[0].use_grad) { g0 = A.grad[0][i]; if (A.grad_b[0]) b0 = A.grad_b[0][i]; }
+        if (A.ph[1].kind != 0 && A.ph[1].use_grad) { g1 = A.grad[1][i]; if (A.grad_b[1]) b1 = A.grad_b[1][i]; }
+        if (any_coul) cc = chain_const(m, A.rowM, A.rowL, i, xi.w);
+        if (any_lj) { lji = A.lj[i]; if (lji.y > 0.f) NV = A.rowV.cnt[i]; }
+        // a = -M^-1 F
+        a0x = -mi.x * (b0.x + g0.x); a0y = -mi.x * (b0.y + g0.y); a0z = -mi.x * (b0.z + g0.z);
+        a1x = -mi.x * (b1.x + g1.x); a1y = -mi.x * (b1.y + g1.y); a1z = -mi.x * (b1.z + g1.z);
+    }
     float vx = v4.x, vy = v4.y, vz = v4.z;
     // the velocity half-phases: every lane of the warp walks through them together (chain_C is a warp-wide loop)
     // (not unrolled, and each chain routine appears once: the kernel's code stays small enough for the
@@ -360,25 +377,18 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
     for (int ph = 0; ph < 2; ++ph) {
         const Phase P = A.ph[ph];
         if (P.kind == 0) continue;
-        float ax = 0.f, ay = 0.f, az = 0.f;
-        if (P.use_grad && live) {  // a = -M^-1 F
-            float4 g = A.grad[ph][i];
-            if (A.grad_b[ph]) { float4 b = A.grad_b[ph][i]; g.x = b.x + g.x; g.y = b.y + g.y; g.z = b.z + g.z; }
-            ax = -mi.x * g.x; ay = -mi.x * g.y; az = -mi.x * g.z;
-        }
+        const float ax = ph == 0 ? a0x : a1x, ay = ph == 0 ? a0y : a1y, az = ph == 0 ? a0z : a1z;
         if (P.kind == 1 || !JUMPS) {
             vx += P.H * ax; vy += P.H * ay; vz += P.H * az;
         } else {
-            float2 lji = make_float2(0.f, 0.f);
-            if (live && P.lj) lji = A.lj[i];
             // slots: J' if the phase is a closing one (J'C'), then C', then J' if it is an opening one (C'J')
 #pragma unroll 1
             for (int slot = 0; slot < 3; ++slot) {
                 if (slot == 1) {
-                    if (P.coul) chain_C<G, LOG>(m, A, live, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl, gl, gshift);
+                    if (P.coul) chain_C<G, LOG>(m, A, live, cc, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl, gl, gshift);
                     else if (P.use_grad) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
                 } else if (P.lj && live && (slot == 0) == (P.reverse != 0)) {
-                    chain_J(m, A, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
+                    chain_J(m, A, NV, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
                 }
             }
         }
