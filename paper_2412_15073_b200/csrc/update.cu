@@ -131,8 +131,8 @@ __device__ inline float fij_lj(const Model &m, const float4 &xi, const float4 &x
 //    have a stream of their own, R-15): lane l evaluates proposal kb + l;
 //  * the bound lambda-bar is re-evaluated after each ACCEPTED jump only (R-11), so between two accepted
 //    jumps the proposal times are a running sum of E_k / lambda-bar and v(t) = v_e + (t - t_e) a in closed form:
-//    every lane gets its own proposal time (summed in the sequential order, so the value is the sequential
-//    algorithm's bit for bit), its expiry test, its acceptance probability and its accept test at once;
+//    every lane gets its own proposal time (an inclusive scan over the group), its expiry test, its acceptance
+//    probability and its accept test at once;
 //  * the first accepting lane (a ballot) ends the epoch: kick, new bound, the later lanes are dropped and the
 //    batch restarts after it -- accepted jumps are ~1-2 % of the proposals.
 struct ChainConst {   // per-atom constants of a C' chain
@@ -206,15 +206,16 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
         uint32_t w[4];
         philox4x32_10(atom, step, stream, kb + (unsigned)gl, m.key0, m.key1, w);
         const float T_ = done ? INFINITY : -logf(u01(w[0])) / lam;   // P:L379 (lam = 0: +inf)
-        float tk = t_run;              // time of my proposal: ((t_run + T_0) + T_1) + ... + T_gl, the sequential order
-        if (G == 1) tk += T_;
-        else {
+        // time of my proposal: t_run + (T_0 + ... + T_gl), an inclusive scan over the group in log2 G shuffle steps
+        // (the fp32 sum is associated differently from a sequential chain's: 1e-7 relative, far inside the
+        // margins of R-17)
+        float tk = T_;
 #pragma unroll
-            for (int q = 0; q < G; ++q) {
-                const float Tq = __shfl_sync(full, T_, q, G);
-                if (q <= gl) tk += Tq;
-            }
+        for (int off = 1; off < G; off <<= 1) {
+            const float up = __shfl_up_sync(full, tk, off, G);
+            if (gl >= off) tk += up;
         }
+        tk += t_run;
         const bool alive = !done && tk <= H;   // the chain expires at the first proposal with t + T > delta/2
         const float U = u01(w[3]);
         float goL = 0.f, nx = 0.f, ny = 0.f, nz = 0.f;
