@@ -132,7 +132,7 @@ __device__ inline float near_image1(float d, float L, float invL) {
     return fmaf(-L, t, d);
 }
 
-// Row build, one CTA per cell of the contract grid.
+// Row build, one CTA per cell of the contract grid (per CX consecutive cells along x when the grid is large).
 //  1. The candidate set of a cell is the same for all its atoms: the cells of a host-computed stencil (every cell
 //     whose extent comes within rmax of this cell), visited in ascending cell key, i.e. a list of contiguous runs
 //     [seg_beg, seg_beg + seg_len) of the sorted atom array.  The runs are found once per CTA, prefix-summed and
@@ -150,6 +150,7 @@ __device__ inline float near_image1(float d, float L, float invL) {
 //     decision (R-17) and the fp32 value of r^2 (error < 1e-3 A^2) would flip it where the fp64 oracle does not.
 constexpr int BUILD_THREADS = 128;
 constexpr int BUILD_WARPS = BUILD_THREADS / 32;
+constexpr int BUILD_CX_MAX = 2;            // home cells per CTA (consecutive along x): 1 on small grids, more when the grid is large
 constexpr int BUILD_CHUNK = 1024;           // candidates staged per pass
 constexpr int BUILD_MAXSEG = 2 * 17 * 17;   // two x-runs per (z, y) cell row of the stencil
 constexpr int BUILD_MAXATOMS = 32;          // atoms of a cell whose running counts are held at once
@@ -164,7 +165,7 @@ struct Stencil {
 
 // MASK >= 0: bit k set = row k is built (compile-time row set of the common modes); MASK < 0: rows.r[k].enabled decides
 template <int MASK, bool FAST>
-__global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid g, RowSet rows, Stencil stn, float rmax_all,
+__global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid g, RowSet rows, Stencil stn, float rmax_all, int CX,
                                                               const int *__restrict__ cell_start,
                                                               const float4 *__restrict__ xs, const float4 *__restrict__ xl,
                                                               const float2 *__restrict__ lj,
@@ -179,18 +180,22 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
     __shared__ int scan_tmp[BUILD_THREADS];
     __shared__ int s_count[BUILD_MAXATOMS][N_ROWS];
     const unsigned full = 0xffffffffu;
-    const int cell = blockIdx.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int a_beg = cell_start[cell], a_end = cell_start[cell + 1];
-    if (a_end == a_beg) return;
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // the CTA's home: CX consecutive cells along x (their atoms are contiguous in the sorted array)
+    const int nbx = (g.gn[0] + CX - 1) / CX;
     int c3[3];
-    c3[0] = cell % g.gn[0];
-    c3[1] = (cell / g.gn[0]) % g.gn[1];
-    c3[2] = cell / (g.gn[0] * g.gn[1]);
-    float ctr3[3];   // cell centre (FAST: origin of the staged coordinates)
+    c3[0] = (blockIdx.x % nbx) * CX;
+    c3[1] = (blockIdx.x / nbx) % g.gn[1];
+    c3[2] = blockIdx.x / (nbx * g.gn[1]);
+    const int ncx = min(CX, g.gn[0] - c3[0]);
+    const int cell0 = (c3[2] * g.gn[1] + c3[1]) * g.gn[0] + c3[0];
+    const int a_beg = cell_start[cell0], a_end = cell_start[cell0 + ncx];
+    if (a_end == a_beg) return;
+    float ctr3[3];   // centre of the home cells (FAST: origin of the staged coordinates)
     int start[3], cnt[3];
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-        ctr3[k] = ((float)c3[k] + 0.5f) * (m.box[k] / (float)g.gn[k]);
+        ctr3[k] = ((float)c3[k] + (k == 0 ? 0.5f * (float)ncx : 0.5f)) * (m.box[k] / (float)g.gn[k]);
         if (2 * stn.R[k] + 1 >= g.gn[k]) { start[k] = 0; cnt[k] = g.gn[k]; }
         else { start[k] = (c3[k] - stn.R[k] + g.gn[k]) % g.gn[k]; cnt[k] = 2 * stn.R[k] + 1; }
     }
@@ -204,10 +209,10 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
         int b0 = 0, n0 = 0, b1 = 0, n1 = 0;
         if (xm >= 0) {
             int rowbase = (zc * g.gn[1] + yc) * g.gn[0];
-            if (2 * xm + 1 >= g.gn[0]) {
+            if (2 * xm + ncx >= g.gn[0]) {
                 b0 = cell_start[rowbase]; n0 = cell_start[rowbase + g.gn[0]] - b0;
             } else {
-                int xs0 = (c3[0] - xm + g.gn[0]) % g.gn[0], xc = 2 * xm + 1;
+                int xs0 = (c3[0] - xm + g.gn[0]) % g.gn[0], xc = 2 * xm + ncx;
                 int w = max(0, xs0 + xc - g.gn[0]);          // cells wrapped to the low end come first
                 if (w > 0) { b0 = cell_start[rowbase]; n0 = cell_start[rowbase + w] - b0; }
                 b1 = cell_start[rowbase + xs0]; n1 = cell_start[rowbase + xs0 + xc - w] - b1;
@@ -451,14 +456,18 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
         }
     int mask = 0;
     for (int k = 0; k < N_ROWS; ++k) mask |= rows[k].enabled ? (1 << k) : 0;
+    // home cells per CTA: staging is shared by more atoms and the warps are better balanced, as long as the grid
+    // still gives every SM several waves of CTAs
+    const int CX = std::max(1, std::min(BUILD_CX_MAX, g.ncell / 4000));
     // FAST: staged coordinates relative to the cell centre, no minimum image in the inner loop (see k_build_rows)
     bool fast = true;
-    for (int k = 0; k < 3; ++k) fast = fast && ((double)rmax_all + 0.5 * cs[k] <= 0.5 * (double)m.box[k]) && m.box[k] <= 512.f;
+    for (int k = 0; k < 3; ++k) fast = fast && ((double)rmax_all + 0.5 * cs[k] * (k == 0 ? CX : 1) <= 0.5 * (double)m.box[k]) && m.box[k] <= 512.f;
+    const unsigned nblocks = (unsigned)(((g.gn[0] + CX - 1) / CX) * g.gn[1] * g.gn[2]);
 #define JB_BUILD(MASK)                                                                                                        \
     do {                                                                                                                      \
-        if (fast) k_build_rows<MASK, true><<<(unsigned)g.ncell, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, cell_start, xs, xl, lj, \
+        if (fast) k_build_rows<MASK, true><<<nblocks, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, \
                                                                                        orig, sorted_of, excl_ptr, excl_idx, ctr);         \
-        else k_build_rows<MASK, false><<<(unsigned)g.ncell, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, cell_start, xs, xl, lj,      \
+        else k_build_rows<MASK, false><<<nblocks, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, \
                                                                                     orig, sorted_of, excl_ptr, excl_idx, ctr);            \
     } while (0)
     switch (mask) {
