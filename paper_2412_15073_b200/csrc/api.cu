@@ -30,7 +30,7 @@ struct jump_ctx {
     float4 *xs, *xs_nxt, *vs, *vs_nxt, *xl, *xl_nxt, *x_build;
     float2 *lj, *lj_nxt, *mi, *mi_nxt;
     int *orig, *orig_nxt, *sorted_of;
-    int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src;
+    int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src, *scan_sums, *scan_offs;
     Row rows[N_ROWS];
     bool row_fresh[N_ROWS];  // built since the last sort
     bool row_used[N_ROWS];   // read since the last sort: rebuilt eagerly at the next one (others lazily, on demand)
@@ -212,7 +212,7 @@ static int resort_and_build(jump_ctx *c) {
     a.xs = c->xs_nxt; a.vs = c->vs_nxt; a.lj = c->lj_nxt; a.mi = c->mi_nxt; a.orig = c->orig_nxt;
     a.sorted_of = c->sorted_of; a.x_build = c->x_build;
     a.key = c->key; a.cell_count = c->cell_count; a.cell_fill = c->cell_fill; a.cell_start = c->cell_start;
-    a.tmp_orig = c->tmp_orig; a.tmp_src = c->tmp_src; a.ctr = c->ctr;
+    a.tmp_orig = c->tmp_orig; a.tmp_src = c->tmp_src; a.scan_sums = c->scan_sums; a.scan_offs = c->scan_offs; a.ctr = c->ctr;
     prof_begin(c, PROF_BUILD);
     launch_sort(a, c->st, &c->launches);
     prof_end(c, PROF_BUILD);
@@ -554,7 +554,8 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
         (r = dalloc(c, &c->orig, n)) || (r = dalloc(c, &c->orig_nxt, n)) || (r = dalloc(c, &c->sorted_of, n)) ||
         (r = dalloc(c, &c->key, n)) || (r = dalloc(c, &c->tmp_orig, n)) || (r = dalloc(c, &c->tmp_src, n)) ||
         (r = dalloc(c, &c->cell_count, g.ncell + 1)) || (r = dalloc(c, &c->cell_fill, g.ncell + 1)) ||
-        (r = dalloc(c, &c->cell_start, g.ncell + 1)) || (r = dalloc(c, &c->fnb, n)) || (r = dalloc(c, &c->fbond, n)) ||
+        (r = dalloc(c, &c->cell_start, g.ncell + 1)) || (r = dalloc(c, &c->scan_sums, g.ncell / 4096 + 2)) ||
+        (r = dalloc(c, &c->scan_offs, g.ncell / 4096 + 2)) || (r = dalloc(c, &c->fnb, n)) || (r = dalloc(c, &c->fbond, n)) ||
         (r = dalloc(c, &c->f0, n)) || (r = dalloc(c, &c->ftmp, n)) || (r = dalloc(c, &c->ftmp2, n)) ||
         (r = dalloc(c, &c->ke, n)) || (r = dalloc(c, &c->ctr, 1)))
         return r;

@@ -14,6 +14,7 @@ struct SortArgs {
     float2 *lj, *mi;
     int *orig, *sorted_of;
     int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src;
+    int *scan_sums, *scan_offs;   // scratch of the multi-block scan (ncell / 4096 + 2 each)
     Counters *ctr;
 };
 

@@ -59,6 +59,48 @@ __global__ void k_scan(int ncell, const int *__restrict__ cell_count, int *__res
     if (t == nt - 1) cell_start[ncell] = part[t];
 }
 
+// the same scan for large grids, in three small launches: per-block sums of 4096-cell slices, a scan of the
+// sums (k_scan on them), then each block scans its slice from its offset
+constexpr int SCAN_SLICE = 4096;
+__global__ void k_scan_sums(int ncell, const int *__restrict__ cell_count, int *__restrict__ sums) {
+    __shared__ int part[32];
+    const int lo = blockIdx.x * SCAN_SLICE, hi = min(lo + SCAN_SLICE, ncell);
+    int s = 0;
+    for (int k = lo + threadIdx.x; k < hi; k += blockDim.x) s += cell_count[k];
+    s = __reduce_add_sync(0xffffffffu, s);
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        int v = threadIdx.x < (blockDim.x >> 5) ? part[threadIdx.x] : 0;
+        v = __reduce_add_sync(0xffffffffu, v);
+        if (threadIdx.x == 0) sums[blockIdx.x] = v;
+    }
+}
+__global__ void k_scan_slices(int ncell, const int *__restrict__ cell_count, const int *__restrict__ offs,
+                              int *__restrict__ cell_start) {
+    __shared__ int part[1024];
+    const int t = threadIdx.x, nt = blockDim.x;   // nt * 4 = SCAN_SLICE
+    const int lo = blockIdx.x * SCAN_SLICE + 4 * t;
+    int c[4], s = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { c[k] = lo + k < ncell ? cell_count[lo + k] : 0; s += c[k]; }
+    part[t] = s;
+    __syncthreads();
+    for (int off = 1; off < nt; off <<= 1) {
+        int v = (t >= off) ? part[t - off] : 0;
+        __syncthreads();
+        part[t] += v;
+        __syncthreads();
+    }
+    int run = offs[blockIdx.x] + part[t] - s;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        if (lo + k < ncell) cell_start[lo + k] = run;
+        run += c[k];
+    }
+    if (lo <= ncell - 1 && ncell - 1 < lo + 4) cell_start[ncell] = run;
+}
+
 __global__ void k_scatter(int n, const int *__restrict__ key, const int *__restrict__ orig,
                           const int *__restrict__ cell_start, int *__restrict__ cell_fill,
                           int *__restrict__ tmp_orig, int *__restrict__ tmp_src) {
@@ -414,7 +456,15 @@ void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches) {
     cudaMemsetAsync(a.cell_count, 0, sizeof(int) * (a.grid.ncell + 1), st);
     cudaMemsetAsync(a.cell_fill, 0, sizeof(int) * (a.grid.ncell + 1), st);
     k_cell_key<<<nblk(a.n, B), B, 0, st>>>(a.n, a.xs_in, a.grid, a.key, a.cell_count, a.ctr);
-    k_scan<<<1, 1024, 0, st>>>(a.grid.ncell, a.cell_count, a.cell_start);
+    if (a.grid.ncell <= 4 * SCAN_SLICE) {
+        k_scan<<<1, 1024, 0, st>>>(a.grid.ncell, a.cell_count, a.cell_start);
+    } else {
+        const int nb = nblk(a.grid.ncell, SCAN_SLICE);
+        k_scan_sums<<<nb, 256, 0, st>>>(a.grid.ncell, a.cell_count, a.scan_sums);
+        k_scan<<<1, 1024, 0, st>>>(nb, a.scan_sums, a.scan_offs);
+        k_scan_slices<<<nb, SCAN_SLICE / 4, 0, st>>>(a.grid.ncell, a.cell_count, a.scan_offs, a.cell_start);
+        *launches += 2;
+    }
     k_scatter<<<nblk(a.n, B), B, 0, st>>>(a.n, a.key, a.orig_in, a.cell_start, a.cell_fill, a.tmp_orig, a.tmp_src);
     k_cell_sort<<<nblk(a.grid.ncell, B), B, 0, st>>>(a.grid.ncell, a.cell_start, a.tmp_orig, a.tmp_src);
     k_permute<<<nblk(a.n, B), B, 0, st>>>(a.n, a.tmp_src, a.tmp_orig, a.xs_in, a.vs_in, a.xl_in, a.xl, a.lj_in, a.mi_in, a.xs, a.vs,

@@ -316,6 +316,17 @@ def test_row_overflow_is_reported(jb):
 
 
 # ------------------------------------------------------------------------------------- bench configuration
+def check_sampled_rows(g, o, n_sample):
+    """Rows M, L, V of a seeded sample of atoms: same atoms, same (canonical) order as the oracle's (bit-exact)."""
+    nM, nL, nV = o.row_counts()
+    rng = np.random.default_rng(7)
+    for i in rng.choice(g.n, size=n_sample, replace=False):
+        for which, cnt in ((1, nM), (2, nL), (3, nV)):
+            rg = g.row(which, int(i))
+            assert len(rg) == cnt[i]
+            assert (rg == o.row(which - 1, int(i))).all()
+
+
 def test_full_size_config1_forces_events_trajectory(jb, jo):
     """BASELINE configs[1] (12 000 atoms), the workload bench.py times: all F0, one logged step, 20 steps."""
     sysd, run = wl.make_config(1)
@@ -323,6 +334,7 @@ def test_full_size_config1_forces_events_trajectory(jb, jo):
     g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
     assert rel_force_err(g.forces(0).cpu().numpy(), o.forces(0)) <= F_TOL
     assert rel_force_err(g.forces(1).cpu().numpy(), o.forces(1)) <= F_TOL
+    check_sampled_rows(g, o, 48)
     g.jump_step(1); g.sync(); o.jump_step(1)
     check_events(g.events(), o.events())
     g.clear_events(); o.clear_events()
@@ -344,6 +356,7 @@ def test_config2_sampled_forces_and_properties(jb, jo):
     fg = g.forces(0).cpu().numpy()
     assert rel_force_err(fg, fo) <= F_TOL
     assert np.abs(g.forces(4).cpu().numpy().astype(np.float64).sum(0)).max() < 0.05   # sum of pair gradients = 0
+    check_sampled_rows(g, o, 48)   # large grid: multi-block cell scan, two home cells per CTA, cell-centred staging
     g.jump_respa_step(5); g.sync()
     st = g.stats()
     assert st["error"] == 0 and st["max_p"] <= 1 + 1e-4 and st["max_g_over_L"] <= 1 + 1e-4
