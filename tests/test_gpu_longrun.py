@@ -1,0 +1,98 @@
+"""Long-run averages of the CUDA JUMP path against CUDA BAOAB and against the fp64 oracle (BASELINE.json
+north_star: T, potential energy, RDF and diffusion constant within stated statistical error bars).
+
+JUMP is a different stochastic process from BAOAB with the same invariant measure mu, so realised
+trajectories differ and what must agree are averages under mu.  Error bars: standard errors from block averages
+(tests/observables.py); a comparison passes when the means differ by less than 4 combined standard errors plus a
+stated slack for the O(delta^2) time-step bias, which differs between the two splittings.
+"""
+import numpy as np
+import pytest
+
+from paper_2412_15073_b200 import workloads as wl
+import observables as ob
+
+pytestmark = pytest.mark.gpu
+KB = 1.987204259e-3
+
+
+@pytest.fixture(scope="module")
+def jb():
+    from paper_2412_15073_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def jo():
+    from oracle import jump_oracle
+    jump_oracle.build()
+    return jump_oracle
+
+
+def sample_run(sim, step_fn, energy_fn, pos_fn, n_samples, stride, oxy, snap_every):
+    T, U, snaps = [], [], []
+    n = len(oxy) * 3
+    for k in range(n_samples):
+        step_fn(stride)
+        ek, ep = energy_fn()
+        T.append(2.0 * ek / (3.0 * n * KB))
+        U.append(ep / len(oxy))
+        if k % snap_every == 0:
+            snaps.append(pos_fn()[oxy].astype(np.float64))
+    return np.array(T), np.array(U), snaps
+
+
+def test_long_run_averages_jump_vs_baoab_vs_oracle(jb, jo):
+    sysd, run = wl.make_config(0)                       # 216 waters, 648 atoms, box 18.64 A
+    box = float(sysd["box"])
+    oxy = np.nonzero(np.asarray(sysd["lj_eps"]) > 0)[0]
+    assert len(oxy) * 3 == sysd["n_atoms"]
+    # common starting point: the lattice start relaxed by 6 ps of BAOAB on the GPU
+    g = jb.JumpSim(sysd, **run)
+    g.baoab_step(6000); g.sync()
+    sys_eq = dict(sysd, pos=g.pos.cpu().numpy().copy(), vel=g.vel.cpu().numpy().copy())
+    g.close()
+
+    stride, n_samples, snap_every = 20, 2000, 5          # 40 ps per GPU run, a snapshot every 100 fs
+    res = {}
+    for name in ("jump", "baoab"):
+        g = jb.JumpSim(sys_eq, **dict(run, seed=run["seed"] + (1 if name == "jump" else 2)))
+        step = g.jump_step if name == "jump" else g.baoab_step
+        res[name] = sample_run(g, step, g.energy, lambda: g.pos.cpu().numpy(), n_samples, stride, oxy, snap_every)
+        st = g.stats()
+        assert st["error"] == 0 and st["max_p"] <= 1 + 1e-4
+        g.close()
+    o = jo.Oracle(sys_eq, **dict(run, seed=run["seed"] + 3))
+    res["oracle"] = sample_run(o, o.jump_step, lambda: (o.kinetic(), o.potential(1)), lambda: o.pos, 200, stride, oxy, 1)
+    o.close()
+
+    T = {k: ob.block_mean_se(v[0]) for k, v in res.items()}      # kinetic temperature, K
+    U = {k: ob.block_mean_se(v[1]) for k, v in res.items()}      # potential energy, kcal/mol per molecule
+    print("T", T, "U", U)
+    r, gj, ej = ob.rdf_blocks(res["jump"][2], box, 8.0, 64)      # O-O radial distribution function
+    _, gb, eb = ob.rdf_blocks(res["baoab"][2], box, 8.0, 64)
+    _, go, eo = ob.rdf_blocks(res["oracle"][2], box, 8.0, 64)
+    ps = run["dt_fs"] * 1e-3
+    Dj = ob.diffusion_atoms(res["jump"][2], box, stride * snap_every * ps, 2, 10)     # MSD slope between 0.2 and 1 ps
+    Db = ob.diffusion_atoms(res["baoab"][2], box, stride * snap_every * ps, 2, 10)
+    Do = ob.diffusion_atoms(res["oracle"][2], box, stride * ps, 10, 50)
+    print("D", Dj, Db, Do)
+
+    # (1) the CUDA path against the oracle: the SAME process, so every long-run average agrees, the dynamical one too
+    assert ob.agree(T["jump"], T["oracle"], 4.0, slack=1.0), (T["jump"], T["oracle"])
+    assert ob.agree(U["jump"], U["oracle"], 4.0, slack=0.05), (U["jump"], U["oracle"])
+    assert (np.abs(gj - go) <= 4.0 * np.hypot(ej, eo) + 0.15).all(), np.abs(gj - go).max()
+    assert ob.agree(Dj, Do, 4.0, slack=0.1 * Dj[0]), (Dj, Do)
+
+    # (2) JUMP against BAOAB: different processes, the same invariant measure mu -- configurational
+    # averages agree.  The kinetic temperature read at the end of a step carries each splitting's own O(delta^2) bias
+    # (stiff O-H bonds at delta = 1 fs; the jumps resample velocity components exactly), and at eps = 1 the jumps act
+    # as extra friction, so the diffusion constant is NOT expected to agree (eps -> 0 recovers the
+    # Hamiltonian kicks): both are checked for sanity only.
+    assert abs(T["jump"][0] - 300.0) < 15.0 and abs(T["baoab"][0] - 300.0) < 15.0
+    assert ob.agree(U["jump"], U["baoab"], 4.0, slack=0.05), (U["jump"], U["baoab"])
+    sj, sb = res["jump"][1].std(), res["baoab"][1].std()          # width of the energy distribution (heat capacity)
+    assert abs(sj / sb - 1.0) < 0.3, (sj, sb)
+    assert gj.max() > 2.0 and 2.6 < r[gj.argmax()] < 3.0          # first O-O peak of liquid water
+    assert (np.abs(gj - gb) <= 4.0 * np.hypot(ej, eb) + 0.08).all(), np.abs(gj - gb).max()
+    assert 0.0 < Dj[0] <= Db[0] * 1.2

@@ -556,3 +556,33 @@ def test_respa_proposals_per_time_independent_of_outer_step(relaxed_small):
     o.jump_step(40)
     rates.append(o.stats()["proposals"] / (20 * 0.5))
     assert abs(rates[0] / rates[1] - 1) < 0.1 and abs(rates[2] / rates[1] - 1) < 0.15
+
+
+def test_jump_and_baoab_sample_the_same_measure(relaxed_small):
+    """the hybrid jump process leaves mu invariant, so its long-run averages equal BAOAB's (which
+    integrates the whole gradient of the same U).  192 atoms, 3 ps each after 1 ps of burn-in; kinetic temperature
+    and potential energy per molecule with block-average error bars (BASELINE.json north_star: "the hybrid process
+    still samples mu").  A wrong rate, kick amplitude or sign heats or cools the system by tens of K within a ps
+    (the Langevin thermostat acts on a 1 ps scale only)."""
+    import observables as ob
+    sysd, _ = relaxed_small
+    run = dict(r_short=4.0, r_long=6.0, r_mid=5.0, skin=1.0, nlist_every=10, dt_fs=1.0, gamma_per_ps=1.0, eps_jump=1.0, flags=3)
+    out = {}
+    for name, seed in (("jump", 11), ("baoab", 12)):
+        o = jo.Oracle(sysd, **dict(run, seed=seed))
+        step = o.jump_step if name == "jump" else o.baoab_step
+        step(1000)
+        T, U = [], []
+        for _ in range(300):
+            step(10)
+            T.append(o.temperature())
+            U.append(o.potential(1) / 64.0)
+        if name == "jump":
+            st = o.stats()
+            assert st["accepts"] > 1000 and st["max_p"] <= 1.0 + 1e-9
+        out[name] = (ob.block_mean_se(T, 6), ob.block_mean_se(U, 6))
+        o.close()
+    (Tj, Uj), (Tb, Ub) = out["jump"], out["baoab"]
+    assert ob.agree(Tj, Tb, 4.0, slack=3.0), (Tj, Tb)        # K
+    assert abs(Tj[0] - 300.0) < 20.0 and abs(Tb[0] - 300.0) < 20.0
+    assert ob.agree(Uj, Ub, 4.0, slack=0.1), (Uj, Ub)        # kcal/mol per molecule
