@@ -758,6 +758,11 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
     double *v = &c->v[3 * i];
     const double eps = c->p.eps_jump, sbm = c->sbm[i], beta = c->beta;
     const int bps = isinf(eps);
+    /* R-19 (NEXT-1): eps_mode 1 = adaptive eps(x) = eps0 |F_ij(x)|, eps0 = eps_jump.  With
+     * g = |F_ij| <= L_Y, eta = eps0 g sqrt(beta m)(v.n) and Theta(eta) <= eta_+ + 1/sqrt(2 pi) the pair rate
+     * lambda_ij = sqrt(beta) Theta(eta) / (eps0 sqrt(m)) (P:L340 with eps = eps0 g) is bounded, uniformly in j, by
+     * lambda*_Y = beta L_Y B_v + (1/eps0) sqrt(beta / (2 pi m)); p = lambda_ij / lambda*_Y. */
+    const int adaptive = c->p.eps_mode == 1 && !bps;
     const int NM = c->ptrM[i + 1] - c->ptrM[i], NL = c->ptrL[i + 1] - c->ptrL[i];
     const double LM = LM_of(c, i), LL = LL_of(c, i);
     const double SM = (double)NM * LM, S = SM + (double)NL * LL; /* P:L424 */
@@ -769,6 +774,8 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
      * (P:L373), so it and lambda-bar are evaluated at t = 0 and after every ACCEPTED jump and held in between. */
     int fresh = 1;
     double Bv = 0.0, lam = 0.0;
+    double ringM = SM, ringS = S; /* ring M is picked with probability ringM / ringS */
+    const double lam0 = bps ? 0.0 : (1.0 / eps) * beta * ORC_INV_SQRT_2PI / sbm; /* (1/eps) sqrt(beta/(2 pi m)) */
     const double a2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
     for (int iter = 0;; ++iter) {
         orc_event ev;
@@ -780,8 +787,12 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
             double va = v[0] * a[0] + v[1] * a[1] + v[2] * a[2];
             double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
             Bv = sqrt(v2 + tau * tau * a2 + 2.0 * tau * (va > 0.0 ? va : 0.0)); /* P:L373 */
-            lam = bps ? S * beta * Bv
-                      : S * (beta * Bv + (1.0 / eps) * beta * ORC_INV_SQRT_2PI / sbm); /* P:L374 */
+            if (!(S > 0.0)) lam = 0.0; /* no partner, or an uncharged atom: no mechanism */
+            else if (adaptive) {        /* sum over the listed pairs of lambda*_Y (R-19) */
+                ringM = (double)NM * (beta * LM * Bv + lam0);
+                lam = ringM + (double)NL * (beta * LL * Bv + lam0);
+                ringS = lam;
+            } else lam = S * (beta * Bv + lam0); /* P:L374 */
             fresh = 0;
         }
         chain_block(c, i, step, stream, block++, w);
@@ -801,8 +812,8 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
         /* ring pick */
         double ur = orc_u01(w[1]);
         int ring;
-        if (NM > 0 && NL > 0) mg = upd(mg, ur - SM / S);
-        ring = (ur * S < SM) ? 0 : 1;
+        if (NM > 0 && NL > 0) mg = upd(mg, ur - ringM / ringS);
+        ring = (ur * ringS < ringM) ? 0 : 1;
         if (ring == 0 && NM == 0) ring = 1;
         if (ring == 1 && NL == 0) ring = 0;
         int cnt = ring == 0 ? NM : NL;
@@ -819,7 +830,9 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
             double n[3] = {F[0] / g, F[1] / g, F[2] / g};
             double vn = v[0] * n[0] + v[1] * n[1] + v[2] * n[2];
             double p;
+            const double eps_ij = adaptive ? eps * g : eps; /* eps(x) = eps0 |F_ij(x)| */
             if (bps) p = (vn > 0.0 ? vn : 0.0) * g / (LY * Bv);
+            else if (adaptive) p = orc_theta(eps_ij * sbm * vn) / (eps * sbm * LY * Bv + ORC_INV_SQRT_2PI); /* R-19 */
             else p = g * orc_theta(eps * sbm * vn) / (LY * (Bv * eps * sbm + ORC_INV_SQRT_2PI)); /* P:L397 + sqrt(beta) */
             ev.p = p;
             if (p > *max_p) *max_p = p;
@@ -827,8 +840,8 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
             if (U <= p) { /* P:L401 */
                 double gt = 0.0;
                 int att = 0;
-                if (!bps) gt = orc_gtilde(c, eps * sbm * vn, i, step, stream + 16, &gblock, &att, &mg);
-                orc_jump_kick(eps, sbm, n, gt, v); /* P:L406 */
+                if (!bps) gt = orc_gtilde(c, eps_ij * sbm * vn, i, step, stream + 16, &gblock, &att, &mg);
+                orc_jump_kick(eps_ij, sbm, n, gt, v); /* P:L406 */
                 ev.accepted = 1; ev.gt = gt; ev.n_gt = att;
                 (*n_acc)++;
                 (*n_gt) += att;

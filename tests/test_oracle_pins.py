@@ -430,8 +430,9 @@ def _frozen(relaxed_small, **over):
     return sysd, kw
 
 
-def test_event_log_invariants(relaxed_small):
-    sysd, kw = _frozen(relaxed_small, flags=1 | 2 | 4, eps_jump=1.0)
+@pytest.mark.parametrize("mode", [0, 1])
+def test_event_log_invariants(relaxed_small, mode):
+    sysd, kw = _frozen(relaxed_small, flags=1 | 2 | 4, eps_jump=1.0, eps_mode=mode)
     o = jo.Oracle(sysd, **kw)
     o.jump_step(3)
     ev = o.events()
@@ -466,17 +467,24 @@ def _two_atoms(d=5.0, q=0.5):
                 excl_ptr=np.zeros(3, dtype=np.int32), excl_idx=np.zeros(0, dtype=np.int32))
 
 
-@pytest.mark.parametrize("eps", [0.3, 2.0])
-def test_mean_drift_of_jump_process_is_minus_F_over_m(eps):
+@pytest.mark.parametrize("eps,mode", [(0.3, 0), (2.0, 0), (15.0, 1)])
+def test_mean_drift_of_jump_process_is_minus_F_over_m(eps, mode):
     """Averaged over Maxwellian velocities, rate (6) x mean kick (7) (E[G~] = Phi/Theta) gives exactly
     dE[v]/dt = -M^-1 F_ij for every eps -- the drift of the Hamiltonian flow the process replaces
-    (P:L100-104).  Pins the sign convention R-4 and every factor of (6), (7)."""
+    (P:L100-104).  Pins the sign convention R-4 and every factor of (6), (7).
+    mode 1: adaptive eps(x) = eps0 |F_ij(x)| (R-19) -- at frozen x that is the constant eps0 g, so
+    the same identity pins its rate, its bound (a p whose denominator were not the bound the clock runs on would
+    change the effective rate) and its kernel."""
     sysd = _two_atoms()
-    o = jo.Oracle(sysd, r_short=4.0, r_long=8.0, r_mid=6.0, skin=0.5, flags=1, eps_jump=eps, nlist_every=10 ** 9, seed=77)
+    o = jo.Oracle(sysd, r_short=4.0, r_long=8.0, r_mid=6.0, skin=0.5, flags=1, eps_jump=eps, eps_mode=mode,
+                  nlist_every=10 ** 9, seed=77)
     F = o.forces(2)
     assert np.abs(F[:, 0]).min() > 1e-3 and np.abs(F[:, 1:]).max() < 1e-12
     kT = KB * 300
     sbm = np.sqrt(sysd["mass"] / (kT * KCAL))
+    if mode == 1:
+        eps = eps * abs(F[0, 0])                              # the effective epsilon of the one pair (same |F| on both atoms)
+        assert 0.2 < eps < 5.0
     rate0 = max(jo.jump_rate(eps, 1 / kT, sbm[i], abs(F[i, 0]), 0.0) for i in range(2))
     # mean rate over Maxwellian v is sqrt(1+eps^2) x the v = 0 rate; keep second events (bias) rare
     H = 0.02 / (rate0 * math.sqrt(1 + eps * eps))
@@ -496,9 +504,11 @@ def test_mean_drift_of_jump_process_is_minus_F_over_m(eps):
         assert np.abs(mean[i, 1:]).max() < 0.05 * abs(pred[i, 0])
 
 
-def test_thinning_is_invariant_under_looser_bounds(relaxed_small):
-    # doubling every L doubles proposals and leaves the accepted-jump statistics unchanged
-    sysd, kw = _frozen(relaxed_small, flags=1 | 2, eps_jump=1.0)
+@pytest.mark.parametrize("mode", [0, 1])
+def test_thinning_is_invariant_under_looser_bounds(relaxed_small, mode):
+    # doubling every L doubles proposals and leaves the accepted-jump statistics unchanged; with the
+    # adaptive eps (mode 1, R-19) only the beta L B_v part of the bound doubles, the accepted jumps still do not move
+    sysd, kw = _frozen(relaxed_small, flags=1 | 2, eps_jump=1.0 if mode == 0 else 0.5, eps_mode=mode)
     res = []
     R = 1500
     for f in (1.0, 2.0):
@@ -513,7 +523,10 @@ def test_thinning_is_invariant_under_looser_bounds(relaxed_small):
         st = o.stats()
         res.append((st["proposals"] / R, st["accepts"] / R, dv / R))
     (p1, a1, d1), (p2, a2, d2) = res
-    assert abs(p2 / p1 - 2.0) < 5 * 2.0 * math.sqrt(1 / (p1 * R) + 1 / (p2 * R)) + 0.01
+    if mode == 0:
+        assert abs(p2 / p1 - 2.0) < 5 * 2.0 * math.sqrt(1 / (p1 * R) + 1 / (p2 * R)) + 0.01
+    else:
+        assert 1.02 < p2 / p1 < 2.0
     assert abs(a2 / a1 - 1.0) < 5 * math.sqrt(2 / (a1 * R))
     o = jo.Oracle(sysd, **kw)
     pred = -5e-4 * KCAL * o.forces(2) / sysd["mass"][:, None]      # direction of the mean kick
@@ -568,16 +581,19 @@ def test_jump_and_baoab_sample_the_same_measure(relaxed_small):
     sysd, _ = relaxed_small
     run = dict(r_short=4.0, r_long=6.0, r_mid=5.0, skin=1.0, nlist_every=10, dt_fs=1.0, gamma_per_ps=1.0, eps_jump=1.0, flags=3)
     out = {}
-    for name, seed in (("jump", 11), ("baoab", 12)):
-        o = jo.Oracle(sysd, **dict(run, seed=seed))
-        step = o.jump_step if name == "jump" else o.baoab_step
+    for name, seed in (("jump", 11), ("baoab", 12), ("adaptive", 13)):
+        kw = dict(run, seed=seed)
+        if name == "adaptive":                                 # eps(x) = eps0 |F_ij(x)| (R-19)
+            kw.update(eps_mode=1, eps_jump=0.5)
+        o = jo.Oracle(sysd, **kw)
+        step = o.baoab_step if name == "baoab" else o.jump_step
         step(1000)
         T, U = [], []
         for _ in range(300):
             step(10)
             T.append(o.temperature())
             U.append(o.potential(1) / 64.0)
-        if name == "jump":
+        if name != "baoab":
             st = o.stats()
             assert st["accepts"] > 1000 and st["max_p"] <= 1.0 + 1e-9
         out[name] = (ob.block_mean_se(T, 6), ob.block_mean_se(U, 6))
@@ -586,3 +602,6 @@ def test_jump_and_baoab_sample_the_same_measure(relaxed_small):
     assert ob.agree(Tj, Tb, 4.0, slack=3.0), (Tj, Tb)        # K
     assert abs(Tj[0] - 300.0) < 20.0 and abs(Tb[0] - 300.0) < 20.0
     assert ob.agree(Uj, Ub, 4.0, slack=0.1), (Uj, Ub)        # kcal/mol per molecule
+    Ta, Ua = out["adaptive"]
+    assert ob.agree(Ta, Tb, 4.0, slack=3.0) and abs(Ta[0] - 300.0) < 20.0, (Ta, Tb)
+    assert ob.agree(Ua, Ub, 4.0, slack=0.1), (Ua, Ub)
