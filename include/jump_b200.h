@@ -44,7 +44,8 @@ typedef struct jump_ctx jump_ctx; /* opaque, owned by the library */
 typedef struct {
     int32_t n_atoms;
     int32_t n_inner;     /* RESPA: Delta = n_inner * dt, must be even */
-    int32_t eps_mode;    /* 0 = constant epsilon (Alg. 4); others unsupported (NEXT-1) */
+    int32_t eps_mode;    /* 0 = constant epsilon = eps_jump (Alg. 4); 1 = adaptive eps(x) = eps_jump |F_ij(x)| (
+                            DESIGN.md R-19), eps_jump finite, in A mol/kcal */
     uint32_t flags;      /* JUMP_F_* */
     int32_t nlist_every; /* rebuild all lists every this many steps (R-10) */
     int32_t pad0;

@@ -532,6 +532,7 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     m.alpha = (float)c->alpha; m.alpha2 = (float)(c->alpha * c->alpha);
     m.beta = (float)(1.0 / c->kT);
     m.eps_jump = std::isinf(p->eps_jump) ? INFINITY : (float)p->eps_jump;
+    m.eps_adaptive = p->eps_mode == 1 ? 1 : 0;
     m.qmaxGM = (float)(c->qmax * c->GM); m.qmaxGL = (float)(c->qmax * c->GL);
     m.GV4se = (float)(4.0 * std::sqrt(c->eps_max) * c->GV);
     m.half_skin2 = (float)(0.25 * p->skin * p->skin);
@@ -662,7 +663,7 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     if (p->n_inner <= 0 || (p->n_inner & 1)) return JUMP_E_ARG;
     if (!(p->r_switch > 0.0) || !(p->r_short > p->r_switch) || !(p->r_short < p->r_long)) return JUMP_E_ARG;
     for (int k = 0; k < 3; ++k) if (!(p->box[k] > 0.0) || p->r_long > 0.5 * p->box[k]) return JUMP_E_ARG;
-    if (p->eps_mode != 0 || !(p->eps_jump > 0.0) || !(p->dt_fs > 0.0) || p->gamma_per_ps < 0.0 || !(p->temperature_K > 0.0))
+    if ((p->eps_mode != 0 && p->eps_mode != 1) || (p->eps_mode == 1 && std::isinf(p->eps_jump)) || !(p->eps_jump > 0.0) || !(p->dt_fs > 0.0) || p->gamma_per_ps < 0.0 || !(p->temperature_K > 0.0))
         return JUMP_E_ARG;
     if (p->skin < 0.0 || p->nlist_every < 0) return JUMP_E_ARG;
     if (p->r_mid > 0.0 && (p->r_mid < p->r_short - p->r_switch || p->r_mid > p->r_long)) return JUMP_E_ARG;

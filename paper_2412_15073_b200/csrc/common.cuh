@@ -52,6 +52,7 @@ struct Model {
     float alpha, alpha2;          // Ewald alpha
     float beta;                   // 1/kT, (kcal/mol)^-1
     float eps_jump;               // epsilon; +inf -> BPS
+    int eps_adaptive;             // eps(x) = eps_jump |F_ij(x)| (R-19)
     float qmaxGM, qmaxGL;         // qmax * G_M, qmax * G_L  (L_Y,i = |q_i| * this, R-7)
     float GV4se;                  // 4 sqrt(eps_max) G_V     (L^vdW_i = sqrt(eps_i) * this)
     float half_skin2;             // (skin/2)^2

@@ -151,9 +151,10 @@ __device__ inline ChainConst chain_const(const Model &m, const Row &rowM, const 
 // goL = |F_ij| / L_Y and n = F_ij / |F_ij|; tag = ring << 31 | j_orig (event log only)
 template <bool WANT_J>
 __device__ inline void propose_pair(const Model &m, const Row &rowM, const Row &rowL, const float4 *__restrict__ xs,
-                                    const int *__restrict__ orig, const ChainConst &c, int i, const float4 &xi,
-                                    const uint32_t w[4], float &goL, float &nx, float &ny, float &nz, int &tag) {
-    int ring = (u01(w[1]) * c.S < c.SM) ? 0 : 1;
+                                    const int *__restrict__ orig, const ChainConst &c, float ringS, float ringM, int i,
+                                    const float4 &xi, const uint32_t w[4], float &g, float &LY, float &nx, float &ny,
+                                    float &nz, int &tag) {
+    int ring = (u01(w[1]) * ringS < ringM) ? 0 : 1;   // ring M with probability ringM / ringS
     if (ring == 0 && c.NM == 0) ring = 1;
     if (ring == 1 && c.NL == 0) ring = 0;
     const int cnt = ring == 0 ? c.NM : c.NL;
@@ -162,8 +163,8 @@ __device__ inline void propose_pair(const Model &m, const Row &rowM, const Row &
     float dx, dy, dz, rinv;
     const float fr = fij_coul(m, xi, xs[j], dx, dy, dz, rinv);
     const float sg = (fr > 0.f ? rinv : -rinv);  // n = F/|F|
-    const float LY = ring == 0 ? c.LM : c.LL;
-    goL = fabsf(fr) / LY;
+    LY = ring == 0 ? c.LM : c.LL;
+    g = fabsf(fr);
     nx = dx * sg; ny = dy * sg; nz = dz * sg;
     tag = 0;
     if (WANT_J) tag = orig[j] | (ring << 31);
@@ -172,7 +173,9 @@ __device__ inline void propose_pair(const Model &m, const Row &rowM, const Row &
 // The chain of one atom, run by the G lanes of its group.  The whole warp executes the loop together (while any
 // of its 32 / G groups still has a live chain, finished groups predicated off): groups of one warp never run one
 // after the other, and every shuffle and ballot is a full-warp one.  `on` = this lane's atom exists and runs C'.
-template <int G, bool LOG>
+// ADAPT: eps(x) = eps0 |F_ij(x)| (R-19): per-pair bound beta L_Y B_v + lam0, p = Theta(eta) / (eps0
+// sqrt(beta m) L_Y B_v + 1/sqrt(2 pi)), G~ and the kick (7) with eps = eps0 |F_ij|.
+template <int G, bool LOG, bool ADAPT>
 __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const ChainConst &c, int i, unsigned atom, const float4 &xi,
                         float sbm, float ax, float ay, float az, float H, unsigned stream, unsigned step, float &vx, float &vy,
                         float &vz, Tally &tl, int gl, int gshift) {
@@ -191,6 +194,7 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
     float vex = vx, vey = vy, vez = vz, te = 0.f;   // epoch start: velocity and time after the last accepted jump
     float t_run = 0.f;                              // time of the last proposal so far
     float Bv = 0.f, lam = 1.f, den = 1.f;
+    float ringS = S, ringM = c.SM;   // ring M is picked with probability ringM / ringS
     bool fresh = true;
     unsigned kb = 0, gblock = 0;
     while (__any_sync(full, !done)) {
@@ -198,8 +202,14 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
             const float tau = H - te;
             const float va = vex * ax + vey * ay + vez * az, v2 = vex * vex + vey * vey + vez * vez;
             Bv = sqrtf(v2 + tau * tau * a2 + 2.f * tau * fmaxf(va, 0.f));
-            lam = S * (beta * Bv + lam0);
-            den = bps ? Bv : fmaf(Bv, esb, kInvSqrt2Pi);
+            if (ADAPT) {   // sum over the listed pairs of lambda*_Y (R-19)
+                ringM = (float)c.NM * fmaf(beta * c.LM, Bv, lam0);
+                lam = ringM + (float)c.NL * fmaf(beta * c.LL, Bv, lam0);
+                ringS = lam;
+            } else {
+                lam = S * (beta * Bv + lam0);
+                den = bps ? Bv : fmaf(Bv, esb, kInvSqrt2Pi);
+            }
             fresh = false;
         }
         // lane gl draws Philox block kb + gl of the chain's stream: (E, ring, j, U) of proposal kb + gl (R-15)
@@ -218,11 +228,24 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
         tk += t_run;
         const bool alive = !done && tk <= H;   // the chain expires at the first proposal with t + T > delta/2
         const float U = u01(w[3]);
-        float goL = 0.f, nx = 0.f, ny = 0.f, nz = 0.f;
+        float g = 0.f, LY = 1.f, nx = 0.f, ny = 0.f, nz = 0.f;
         int tag = 0;
-        if (alive) propose_pair<LOG>(m, A.rowM, A.rowL, A.xs, A.orig, c, i, xi, w, goL, nx, ny, nz, tag);
+        if (alive) propose_pair<LOG>(m, A.rowM, A.rowL, A.xs, A.orig, c, ringS, ringM, i, xi, w, g, LY, nx, ny, nz, tag);
+        const float goL = g / LY;
         float p = 0.f, vn = 0.f;
         bool acc = false;
+        if (ADAPT) {
+            if (alive && g > 0.f) {
+                const float s = tk - te;
+                const float cx = fmaf(s, ax, vex), cy = fmaf(s, ay, vey), cz = fmaf(s, az, vez);  // the advanced v
+                vn = cx * nx + cy * ny + cz * nz;
+                const float eta = esb * g * vn, dena = fmaf(esb * LY, Bv, kInvSqrt2Pi);            // esb = eps0 sqrt(beta m)
+                if (LOG || U * dena <= (fmaxf(eta, 0.f) + kInvSqrt2Pi) * 1.0001f) {               // Theta <= eta_+ + 1/sqrt(2 pi)
+                    p = theta_of(eta) / dena;
+                    acc = U <= p;
+                }
+            }
+        } else
         // p <= |F_ij| / L_Y always (Theta(eta) <= eta_+ + 1/sqrt(2 pi), eta <= eps sqrt(beta m) B_v): most proposals
         // are rejected on that bound alone; p itself is evaluated when it can matter (or is logged)
         if (alive && goL > 0.f && (LOG || U <= goL * 1.0001f)) {
@@ -242,6 +265,7 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
         const int n_used = f >= 0 ? f + 1 : n_alive;
         const int fs = f >= 0 ? f : 0;
         const float tf = __shfl_sync(full, tk, fs, G), vnf = __shfl_sync(full, vn, fs, G);
+        const float gf = ADAPT ? __shfl_sync(full, g, fs, G) : 1.f;
         const float fnx = __shfl_sync(full, nx, fs, G), fny = __shfl_sync(full, ny, fs, G), fnz = __shfl_sync(full, nz, fs, G);
         const float t_last = __shfl_sync(full, tk, G - 1, G);
         if (done) continue;
@@ -250,10 +274,11 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
         float gt = 0.f;
         int att = 0;
         if (f >= 0) {   // kick (7) on the velocity at the time of proposal f; a new epoch starts there
-            if (!bps) gt = gtilde(esb * vnf, atom, step, stream + 16u, gblock, m, att);
+            const float eps_ij = ADAPT ? eps * gf : eps;   // eps(x) = eps0 |F_ij(x)|
+            if (!bps) gt = gtilde(eps_ij * sbm * vnf, atom, step, stream + 16u, gblock, m, att);
             const float s = tf - te;
             float cx = fmaf(s, ax, vex), cy = fmaf(s, ay, vey), cz = fmaf(s, az, vez);
-            jump_kick(eps, sbm, fnx, fny, fnz, gt, cx, cy, cz);
+            jump_kick(eps_ij, sbm, fnx, fny, fnz, gt, cx, cy, cz);
             vex = cx; vey = cy; vez = cz; te = tf; t_run = tf;
             fresh = true;
             if (lead) { tl.accepts++; tl.gt_attempts += att; }
@@ -334,7 +359,7 @@ __device__ inline double wrap1d(double x, double L) {
 
 // ---- the fused per-atom update: up to two velocity half-phases, then A O A + wrap ----------------------------
 // G lanes per atom (a power of two <= 32) share the atom's jump chains; lane 0 of the group does A-O-A and the stores.
-template <bool JUMPS, int G, bool LOG>
+template <bool JUMPS, int G, bool LOG, bool ADAPT>
 __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
     const unsigned full = 0xffffffffu;
     const int gt_id = blockIdx.x * blockDim.x + threadIdx.x;
@@ -386,7 +411,7 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
 #pragma unroll 1
             for (int slot = 0; slot < 3; ++slot) {
                 if (slot == 1) {
-                    if (P.coul) chain_C<G, LOG>(m, A, live, cc, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl, gl, gshift);
+                    if (P.coul) chain_C<G, LOG, ADAPT>(m, A, live, cc, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl, gl, gshift);
                     else if (P.use_grad) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
                 } else if (P.lj && live && (slot == 0) == (P.reverse != 0)) {
                     chain_J(m, A, NV, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
@@ -533,8 +558,13 @@ template <int G>
 static void update_dispatch(const Model &m, const UpdateArgs &A, cudaStream_t st) {
     const int B = 128;
     const unsigned grid = (unsigned)(((long long)m.n * G + B - 1) / B);
-    if (A.events) k_update<true, G, true><<<grid, B, 0, st>>>(m, A);
-    else k_update<true, G, false><<<grid, B, 0, st>>>(m, A);
+    if (m.eps_adaptive) {
+        if (A.events) k_update<true, G, true, true><<<grid, B, 0, st>>>(m, A);
+        else k_update<true, G, false, true><<<grid, B, 0, st>>>(m, A);
+    } else {
+        if (A.events) k_update<true, G, true, false><<<grid, B, 0, st>>>(m, A);
+        else k_update<true, G, false, false><<<grid, B, 0, st>>>(m, A);
+    }
 }
 // lanes per jump chain: as many as keep the whole grid resident at once (148 SMs x 6 CTAs of 128 threads, the
 // register-limited occupancy of k_update); JUMP_B200_LANES overrides (1, 4, 8, 16) for experiments
@@ -554,7 +584,7 @@ static int lanes_per_chain(int n) {
 void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st, int64_t *launches) {
     if (!jumps) {
         const int B = 128;
-        k_update<false, 1, false><<<(unsigned)((m.n + B - 1) / B), B, 0, st>>>(m, A);
+        k_update<false, 1, false, false><<<(unsigned)((m.n + B - 1) / B), B, 0, st>>>(m, A);
     } else {
         switch (lanes_per_chain(m.n)) {
             case 16: update_dispatch<16>(m, A, st); break;

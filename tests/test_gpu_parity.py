@@ -151,16 +151,18 @@ def test_forces_solute_config3(jb, jo):
 # ------------------------------------------------------------------------------------- jump chains
 # Philox keys chosen (scan of seeds 3000..3039 with the oracle alone) so that the oracle takes no fragile decision
 # (R-17) for 100 steps: the parity window is then long enough to mean something.
-@pytest.mark.parametrize("eps,seed", [(1.0, 3026), (0.3, 3011), (float("inf"), 3000)])
-def test_event_log_and_trajectory_cfg0(jb, jo, cfg0, eps, seed):
+@pytest.mark.parametrize("eps,seed,mode", [(1.0, 3026, 0), (0.3, 3011, 0), (float("inf"), 3000, 0), (2.0, 3009, 1)])
+def test_event_log_and_trajectory_cfg0(jb, jo, cfg0, eps, seed, mode):
     """a6-a8: every proposal of 10 JUMP steps (C', J', both halves) equals the oracle's; then the 100-step
-    trajectory stays within 1e-4 A on the window before the oracle's first fragile decision (R-17)."""
+    trajectory stays within 1e-4 A on the window before the oracle's first fragile decision (R-17).
+    mode 1: adaptive eps(x) = eps0 |F_ij(x)| (NEXT-1, R-19)."""
     sysd, run = cfg0
-    run = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG, eps_jump=eps, seed=seed)
+    run = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG, eps_jump=eps, eps_mode=mode, seed=seed)
     g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
     g.jump_step(10); g.sync(); o.jump_step(10)
     eg, eo = g.events(), o.events()
     assert len(eo) > 15000
+    assert mode == 0 or eo["accepted"].sum() > 3000       # the adaptive mechanism accepts about a quarter of its proposals
     check_events(eg, eo)
     assert set(np.unique(eo["stream"])) == {1, 2, 3, 4}
     g.clear_events(); o.clear_events()
@@ -232,11 +234,12 @@ def test_baoab_energy_conservation_gamma0(jb, cfg0):
     assert out[1] < 0.5 * out[0]              # second order: quartered, allow 2x
 
 
-@pytest.mark.parametrize("flags", [3, 3 | 8, 3 | 16, 3 | 8 | 16, 1])
-def test_respa_variants(jb, jo, cfg0, flags):
-    """a9: JUMP-RESPA (BASELINE variant and the paper's variant) and the BAOAB-RESPA comparator (R-12)."""
+@pytest.mark.parametrize("flags,mode", [(3, 0), (3 | 8, 0), (3 | 16, 0), (3 | 8 | 16, 0), (1, 0), (3, 1), (3 | 8, 1)])
+def test_respa_variants(jb, jo, cfg0, flags, mode):
+    """a9: JUMP-RESPA (BASELINE variant and the paper's variant) and the BAOAB-RESPA comparator (R-12);
+    mode 1: with the adaptive eps of R-19."""
     sysd, run = cfg0
-    r = dict(run, flags=flags | jb.F_EVENT_LOG)
+    r = dict(run, flags=flags | jb.F_EVENT_LOG, eps_mode=mode, eps_jump=2.0 if mode else run["eps_jump"])
     g, o = jb.JumpSim(sysd, **r), jo.Oracle(sysd, **r)
     g.jump_respa_step(3); g.sync(); o.jump_respa_step(3)
     assert g.step == 12 == o.step
@@ -289,7 +292,8 @@ def test_step_batching_is_invisible(jb, cfg0):
 # ------------------------------------------------------------------------------------- edge cases
 def test_bad_arguments_are_refused(jb, cfg0):
     sysd, run = cfg0
-    for bad in (dict(n_inner=3), dict(r_short=9.5), dict(r_long=9.5), dict(eps_jump=0.0), dict(eps_mode=1),
+    for bad in (dict(n_inner=3), dict(r_short=9.5), dict(r_long=9.5), dict(eps_jump=0.0), dict(eps_mode=2),
+                dict(eps_mode=1, eps_jump=float("inf")),
                 dict(r_switch=0.0), dict(dt_fs=0.0)):
         with pytest.raises(jb.JumpError):
             jb.JumpSim(sysd, **dict(run, **bad))
