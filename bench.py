@@ -165,7 +165,12 @@ def timed_blocks(torch, sim, stream, call, n_steps, block, flush):
     return sum(a.elapsed_time(b) for a, b in evs)
 
 
-def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, props, peaks):
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures of this command on the
+# configs[1] workload (profiles/r1_final_README.md); other workloads have no capture: null
+NCU_TRAFFIC_CFG1 = {"update": 9.67e6, "pair": 8.00e6, "build": 6.20e6}
+
+
+def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, props, peaks, traffic=None):
     """Per-kernel device times of K more steps (CUDA events on the streams the kernels are launched on, recorded by
     the library around each kernel group) against each kernel's roofline.  Returns (dominant line, other lines)."""
     with torch.cuda.stream(stream):
@@ -213,6 +218,10 @@ def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, pro
                   "algorithmic": "%.0f row entries x 4 B + %d atoms x 48 B" % (row_entries, n),
                   "avg_launch_us": 1e3 * build_ms, "share_of_step": share["build"]},
     }
+    for k, line in lines.items():
+        if traffic and k in traffic:
+            line["traffic"] = traffic[k]
+            line["traffic_source"] = "ncu --set full capture of k_%s, profiles/r1_final_dram_bytes.csv (bytes per launch)" % k
     share_note = "device time per kernel group / sum over groups; k_bonded runs on a side stream beside k_pair, so the groups overlap"
     dominant = max(("pair", "update", "build"), key=lambda k: share[k])
     roofline = dict(lines[dominant], kernel_ms_share=share, share_note=share_note)
@@ -316,7 +325,8 @@ def main():
     stats = sim.stats()
 
     # ---- per-kernel times of the same K steps (CUDA events on the launch stream, separate pass) --------------
-    roofline, roofline_other = kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, props, peaks)
+    roofline, roofline_other = kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, props, peaks,
+                                                traffic=NCU_TRAFFIC_CFG1 if (args.config == 1 and not respa) else None)
 
     # ---- same-GPU BAOAB with the unsplit r_long force (reported baseline) -------------------------------------
     with torch.cuda.stream(stream):
