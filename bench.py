@@ -240,6 +240,10 @@ def large_box_rooflines(torch, jb, wl, dev, stream, flush, props, peaks, config,
         sim.sync()
         ms = timed_blocks(torch, sim, stream, sim.jump_step, steps, BLOCK, flush)
         line, other = kernel_rooflines(torch, sim, stream, sim.jump_step, steps, BLOCK, flush, run, n, props, peaks)
+        n_in = run["n_inner"]
+        sim.jump_respa_step(5)
+        sim.sync()
+        ms_r = timed_blocks(torch, sim, stream, lambda b: sim.jump_respa_step(b // n_in), (steps // 20) * 20, 20, flush)
         sim.baoab_step(20)
         sim.sync()
         ms_b = timed_blocks(torch, sim, stream, sim.baoab_step, steps, BLOCK, flush)
@@ -251,6 +255,10 @@ def large_box_rooflines(torch, jb, wl, dev, stream, flush, props, peaks, config,
                         % (config, n, sysd["box"]),
             "steps": steps, "ms_per_step": ms / steps, "ns_per_day": ns_per_day(steps / (ms * 1e-3), run["dt_fs"]),
             "atom_steps_per_s": n * steps / (ms * 1e-3), "baoab_ms_per_step": ms_b / steps,
+            "jump_respa": {"n_inner": n_in, "ms_per_inner_step": ms_r / ((steps // 20) * 20),
+                           "ns_per_day": ns_per_day(((steps // 20) * 20) / (ms_r * 1e-3), run["dt_fs"]),
+                           "what": "JUMP-RESPA, inner %g fs (bonded + short-range), outer %g fs (jumps), configs[4]'s mode"
+                                   % (run["dt_fs"], n_in * run["dt_fs"])},
             "jump_vs_baoab": ms_b / ms, "error": err, "kernels": lines}
 
 
