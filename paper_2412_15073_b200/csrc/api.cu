@@ -38,6 +38,7 @@ struct jump_ctx {
     float4 *fnb, *fbond, *f0, *ftmp, *ftmp2;
 
     double *ke;
+    unsigned long long *pair_count;   // scratch of jump_count_pairs
     int *excl_ptr, *excl_idx;
     Topo topo;
     std::vector<void *> owned;  // everything to cudaFree
@@ -240,11 +241,14 @@ static int need_rows(jump_ctx *c, std::initializer_list<int> ks) {
 }
 static int need_row(jump_ctx *c, int k) { return need_rows(c, {k}); }
 
-static void pair(jump_ctx *c, int row, int wC, int wLJ, float4 *out, int accumulate, bool energy) {
-    if (need_row(c, row)) return;
+static int pair(jump_ctx *c, int row, int wC, int wLJ, float4 *out, int accumulate, bool energy) {
+    int r = need_row(c, row);
+    if (r) return r;
     prof_begin(c, PROF_PAIR);
-    launch_pair(c->m, c->rows[row], wC, wLJ, c->xs, c->lj, out, accumulate, energy, c->st, &c->launches);
+    r = launch_pair(c->m, c->rows[row], wC, wLJ, c->xs, c->lj, out, accumulate, energy, c->st, &c->launches);
     prof_end(c, PROF_PAIR);
+    if (r) { c->err = "no pair kernel for this (Coulomb, LJ) weight combination"; return JUMP_E_ARG; }
+    return 0;
 }
 static bool lj_jumps(const jump_ctx *c) { return (c->p.flags & JUMP_F_LJ_JUMPS) != 0; }
 static bool coul_jumps(const jump_ctx *c) { return (c->p.flags & JUMP_F_COUL_JUMPS) != 0; }
@@ -258,11 +262,13 @@ static int bonded(jump_ctx *c, const float4 *add, float4 *out_sum, float4 *out_b
 }
 // F0 = bonded + short non-bonded (R-13: the LJ tail stays in F0 when LJ jumps are off)
 static int compute_short_nb(jump_ctx *c, float4 *out, bool energy = false) {
-    if (lj_jumps(c)) pair(c, ROW_S, W_SHORT, W_SHORT, out, 0, energy);
+    int r;
+    if (lj_jumps(c)) r = pair(c, ROW_S, W_SHORT, W_SHORT, out, 0, energy);
     else {
-        pair(c, ROW_S, W_SHORT, W_FULL, out, 0, energy);
-        pair(c, ROW_W, W_NONE, W_FULL, out, 1, energy);
+        r = pair(c, ROW_S, W_SHORT, W_FULL, out, 0, energy);
+        if (!r) r = pair(c, ROW_W, W_NONE, W_FULL, out, 1, energy);
     }
+    if (r) return r;
     CK(cudaGetLastError());
     return 0;
 }
@@ -320,7 +326,7 @@ static int compute_f0_sum(jump_ctx *c) {
 static int compute_full_split(jump_ctx *c) {
     int r = bonded_fork(c);
     if (r) return r;
-    pair(c, ROW_F, W_FULL, W_FULL, c->ftmp2, 0, false);
+    if ((r = pair(c, ROW_F, W_FULL, W_FULL, c->ftmp2, 0, false))) return r;
     CK(cudaGetLastError());
     c->f0_valid = false;
     return bonded_join(c);
@@ -328,14 +334,15 @@ static int compute_full_split(jump_ctx *c) {
 static GradRef gr_full(const jump_ctx *c) { return gr(c->ftmp2, c->fbond); }
 static int compute_long(jump_ctx *c, float4 *out) {
     int wLJ = lj_jumps(c) ? W_LONG : W_NONE;
-    pair(c, ROW_M, W_LONG, wLJ, out, 0, false);
-    pair(c, ROW_L, W_LONG, wLJ, out, 1, false);
+    int r = pair(c, ROW_M, W_LONG, wLJ, out, 0, false);
+    if (!r) r = pair(c, ROW_L, W_LONG, wLJ, out, 1, false);
+    if (r) return r;
     CK(cudaGetLastError());
     return 0;
 }
 static int compute_full(jump_ctx *c, float4 *out, bool energy = false) {  // unsplit to r_long + bonded
-    int r;
-    pair(c, ROW_F, W_FULL, W_FULL, c->ftmp2, 0, energy);
+    int r = pair(c, ROW_F, W_FULL, W_FULL, c->ftmp2, 0, energy);
+    if (r) return r;
     CK(cudaGetLastError());
     return bonded(c, c->ftmp2, out, nullptr);
 }
@@ -463,9 +470,9 @@ extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
                 r = compute_long(c, fl);
                 if (r) return r;
                 if (paper) {  // + short non-bonded
-                    pair(c, ROW_S, W_SHORT, lj_jumps(c) ? W_SHORT : W_FULL, fl, 1, false);
-                    if (!lj_jumps(c))
-                        pair(c, ROW_W, W_NONE, W_FULL, fl, 1, false);
+                    r = pair(c, ROW_S, W_SHORT, lj_jumps(c) ? W_SHORT : W_FULL, fl, 1, false);
+                    if (!r && !lj_jumps(c)) r = pair(c, ROW_W, W_NONE, W_FULL, fl, 1, false);
+                    if (r) return r;
                     CK(cudaGetLastError());
                 }
                 outer[half] = ph_kick(0.5 * D);
@@ -678,6 +685,7 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     c->d_pos = d_pos; c->d_vel = d_vel;
     c->step = c->outer = c->rebuilds = c->launches = 0;
     c->sticky = 0;
+    c->pair_count = nullptr;
     c->f0_valid = false;
     c->prof = false;
     for (int k = 0; k < 4; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
@@ -840,11 +848,10 @@ extern "C" int jump_get_profile(jump_ctx *c, double ms[4], int64_t count[4]) {
 }
 extern "C" int jump_count_pairs(jump_ctx *c, int32_t which_row, double r_cut, int64_t *n_ordered) {
     if (!c || !n_ordered || which_row < 0 || which_row >= N_ROWS) return JUMP_E_ARG;
-    unsigned long long *d = nullptr;
     int r = need_row(c, which_row);
     if (r) return r;
-    r = dalloc(c, &d, 1);
-    if (r) return r;
+    if (!c->pair_count && (r = dalloc(c, &c->pair_count, 1))) return r;   // one counter, kept for the context's life
+    unsigned long long *d = c->pair_count;
     CK(cudaMemsetAsync(d, 0, sizeof(unsigned long long), c->st));
     launch_count_pairs(c->m, c->rows[which_row], c->xs, (float)(r_cut * r_cut), d, c->st, &c->launches);
     unsigned long long h = 0;
