@@ -366,3 +366,27 @@ def test_config2_sampled_forces_and_properties(jb, jo):
     assert st["error"] == 0 and st["max_p"] <= 1 + 1e-4 and st["max_g_over_L"] <= 1 + 1e-4
     per_atom_fs = st["proposals"] / (g.n * 20.0)
     assert 0.5 < per_atom_fs < 20.0
+
+
+def test_config4_one_million_atoms_properties(jb):
+    """BASELINE configs[4] (999 999 atoms, the largest size): no oracle run fits here, so properties that hold at
+    any size -- every row within capacity, the pair gradients of the short part sum to zero, thinning bounds hold
+    (p <= 1, |F_ij| <= L), proposals per atom in the range of the small boxes, bitwise determinism -- after JUMP
+    and JUMP-RESPA steps across a list rebuild (multi-block cell scan, two home cells per build CTA)."""
+    sysd, run = wl.make_config(4)
+    out = []
+    for rep in range(2):
+        g = jb.JumpSim(sysd, **run)
+        if rep == 0:
+            f = g.forces(4).cpu().numpy().astype(np.float64)
+            frms = np.sqrt((f ** 2).sum(1).mean())
+            assert np.abs(f.sum(0)).max() < 1e-4 * frms * np.sqrt(g.n)      # Newton's third law up to fp32 rounding
+        g.jump_step(12); g.jump_respa_step(2); g.sync()
+        st = g.stats()
+        assert st["error"] == 0 and st["rebuilds"] >= 2
+        assert st["max_p"] <= 1 + 1e-4 and st["max_g_over_L"] <= 1 + 1e-4
+        assert all(m <= c for m, c in zip(st["max_row"], st["cap_row"]) if c)
+        assert 2.0 < st["proposals"] / (g.n * 20.0) < 20.0
+        out.append((g.pos.cpu().numpy().copy(), g.vel.cpu().numpy().copy()))
+        g.close()
+    assert (out[0][0] == out[1][0]).all() and (out[0][1] == out[1][1]).all()
