@@ -129,13 +129,19 @@ __device__ inline float erfcx_poly(float x) {
 // coordinate differences (a - b of image_pair1): a plain fp32 r - r_lo carries an absolute error
 // of ~3e-7 A that chi'' u_C (~10 kcal/mol/A^2) turns into ~3e-6 per pair -- the largest error of the long
 // force and of the acceptance probabilities p (R-16, R-17).
+// EXACT = false (the pair kernel, whose output is a sum over ~100 pairs compared with the whole gradient): the same
+// ratio with r^2 - r_lo^2 in fp32, 6e-7 in u -- the fp64 conversions and FMAs were 15 % of that kernel's instructions.
+template <bool EXACT>
 __device__ inline float chi_zone(float ax, float ay, float az, float bx, float by, float bz, float r2, float r,
                                  const Model &m, float &dchi) {
     if (r2 <= m.rlo2) { dchi = 0.f; return 1.f; }
     if (r2 >= m.rc2) { dchi = 0.f; return 0.f; }
-    double dx = (double)ax - (double)bx, dy = (double)ay - (double)by, dz = (double)az - (double)bz;
-    double d2 = fma(dx, dx, fma(dy, dy, fma(dz, dz, -m.rlo2d)));
-    float u = __fdividef((float)d2 * m.inv_h, r + m.rlo);
+    float num;
+    if (EXACT) {
+        double dx = (double)ax - (double)bx, dy = (double)ay - (double)by, dz = (double)az - (double)bz;
+        num = (float)fma(dx, dx, fma(dy, dy, fma(dz, dz, -m.rlo2d)));
+    } else num = r2 - m.rlo2;
+    float u = __fdividef(num * m.inv_h, r + m.rlo);
     u = fminf(fmaxf(u, 0.f), 1.f);
     float omu = 1.f - u;
     dchi = -30.f * u * u * omu * omu * m.inv_h;

@@ -54,7 +54,7 @@ __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *_
         if (r2 >= cut2) continue;
         float rinv = rsqrtf(r2), r = r2 * rinv;
         float fr = 0.f, chi = 1.f, dchi = 0.f;
-        if (WC == W_SHORT || WC == W_LONG || WLJ == W_SHORT || WLJ == W_LONG) chi = chi_zone(ax, ay, az, bx, by, bz, r2, r, m, dchi);
+        if (WC == W_SHORT || WC == W_LONG || WLJ == W_SHORT || WLJ == W_LONG) chi = chi_zone<false>(ax, ay, az, bx, by, bz, r2, r, m, dchi);
         if (WC != W_NONE && r2 < cutC2) {
             float qq = qi * xj.w;
             float ex = expf(-m.alpha2 * r2), e = ex * erfcx_poly(m.alpha * r);

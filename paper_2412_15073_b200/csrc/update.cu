@@ -102,7 +102,7 @@ __device__ inline float fij_coul(const Model &m, const float4 &xi, const float4 
     float ex = expf(-m.alpha2 * r2), e = ex * erfcx_poly(m.alpha * r);
     float u = qq * e * rinv;
     float du = -(u + qq * kTwoOverSqrtPi * m.alpha * ex) * rinv;
-    float dchi, chi = chi_zone(ax, ay, az, bx, by, bz, r2, r, m, dchi);
+    float dchi, chi = chi_zone<true>(ax, ay, az, bx, by, bz, r2, r, m, dchi);
     return (1.f - chi) * du - dchi * u;
 }
 __device__ inline float fij_lj(const Model &m, const float4 &xi, const float4 &xj, float2 lji, float2 ljj, float &dx,
@@ -119,7 +119,7 @@ __device__ inline float fij_lj(const Model &m, const float4 &xi, const float4 &x
     float s = lji.x * ljj.x * rinv, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
     float e4 = lji.y * ljj.y;
     float u = e4 * (s12 - s6), du = e4 * (6.f * s6 - 12.f * s12) * rinv;
-    float dchi, chi = chi_zone(ax, ay, az, bx, by, bz, r2, r, m, dchi);
+    float dchi, chi = chi_zone<true>(ax, ay, az, bx, by, bz, r2, r, m, dchi);
     return (1.f - chi) * du - dchi * u;
 }
 
