@@ -57,6 +57,7 @@
 #define ORC_F_EVENT_LOG 4u
 #define ORC_F_RESPA_PAPER 8u
 #define ORC_F_RESPA_COMPARATOR 16u
+#define ORC_F_BJAOAJB 64u /* jump_step runs B J A O A J B instead of C'J' A O A J'C' */
 
 /* weight modes of a pair term */
 enum { W_NONE = 0, W_SHORT = 1, W_LONG = 2, W_FULL = 3 };
@@ -979,12 +980,24 @@ static void aoa_and_lists(orc_ctx *c) {
 /* ------------------------------------------------------------------ */
 /* C'J'AOAJ'C' */
 void orc_jump_step(orc_ctx *c, int nsteps) {
+    const double H = 0.5 * c->dt;
     for (int s = 0; s < nsteps; ++s) {
         int64_t st = c->step;
-        jump_phase(c, 0.5 * c->dt, c->f0, 1, 2, st, 0);
+        if (c->p.flags & ORC_F_BJAOAJB) {
+            /* B J A O A J B (NEXT-3): the kick by F0 apart from the jumps, which run on a piecewise
+             * constant velocity (W of P:L125) -- within (J) the Coulomb chains then the LJ chains, mirrored. */
+            phase_B(c, H, c->f0);
+            jump_phase(c, H, NULL, 1, 2, st, 0);
+            aoa_and_lists(c);
+            compute_f0(c);
+            jump_phase(c, H, NULL, 4, 3, st, 1);
+            phase_B(c, H, c->f0);
+            continue;
+        }
+        jump_phase(c, H, c->f0, 1, 2, st, 0);
         aoa_and_lists(c);
         compute_f0(c);
-        jump_phase(c, 0.5 * c->dt, c->f0, 4, 3, st, 1);
+        jump_phase(c, H, c->f0, 4, 3, st, 1);
     }
 }
 /* BAOAB with the unsplit force to r_long (P:L112-125 without J) */

@@ -17,6 +17,7 @@ _SRC = os.path.join(_HERE, "jump_oracle.c")
 _LIB = os.path.join(_HERE, "libjump_oracle.so")
 
 F_COUL_JUMPS, F_LJ_JUMPS, F_EVENT_LOG, F_RESPA_PAPER, F_RESPA_COMPARATOR = 1, 2, 4, 8, 16
+F_BJAOAJB = 64
 
 
 def build(force=False):

@@ -581,10 +581,12 @@ def test_jump_and_baoab_sample_the_same_measure(relaxed_small):
     sysd, _ = relaxed_small
     run = dict(r_short=4.0, r_long=6.0, r_mid=5.0, skin=1.0, nlist_every=10, dt_fs=1.0, gamma_per_ps=1.0, eps_jump=1.0, flags=3)
     out = {}
-    for name, seed in (("jump", 11), ("baoab", 12), ("adaptive", 13)):
+    for name, seed in (("jump", 11), ("baoab", 12), ("adaptive", 13), ("bjaoajb", 14)):
         kw = dict(run, seed=seed)
         if name == "adaptive":                                 # eps(x) = eps0 |F_ij(x)| (R-19)
             kw.update(eps_mode=1, eps_jump=0.5)
+        if name == "bjaoajb":                                  # B J A O A J B
+            kw.update(flags=3 | jo.F_BJAOAJB)
         o = jo.Oracle(sysd, **kw)
         step = o.baoab_step if name == "baoab" else o.jump_step
         step(1000)
@@ -602,6 +604,37 @@ def test_jump_and_baoab_sample_the_same_measure(relaxed_small):
     assert ob.agree(Tj, Tb, 4.0, slack=3.0), (Tj, Tb)        # K
     assert abs(Tj[0] - 300.0) < 20.0 and abs(Tb[0] - 300.0) < 20.0
     assert ob.agree(Uj, Ub, 4.0, slack=0.1), (Uj, Ub)        # kcal/mol per molecule
-    Ta, Ua = out["adaptive"]
-    assert ob.agree(Ta, Tb, 4.0, slack=3.0) and abs(Ta[0] - 300.0) < 20.0, (Ta, Tb)
-    assert ob.agree(Ua, Ub, 4.0, slack=0.1), (Ua, Ub)
+    for name in ("adaptive", "bjaoajb"):
+        Ta, Ua = out[name]
+        assert ob.agree(Ta, Tb, 4.0, slack=3.0) and abs(Ta[0] - 300.0) < 20.0, (name, Ta, Tb)
+        assert ob.agree(Ua, Ub, 4.0, slack=0.1), (name, Ua, Ub)
+
+
+def test_bjaoajb_scheme(relaxed_small):
+    """B J A O A J B: with no jump mechanism it IS BAOAB with F0 (bit for bit the same as the C'
+    scheme without jumps, whose event-free (C) is the same kick); with jumps the (J) parts run on a piecewise
+    constant velocity: the chains of a step see a = 0, so every chain's first bound is beta S |v| + S lam0 and
+    the events differ from the C'J'AOAJ'C' scheme's while the proposal rate stays the same to O(delta)."""
+    sysd, run = relaxed_small
+    kw = dict(run, dt_fs=1.0, gamma_per_ps=1.0, skin=1.0, nlist_every=10)
+    a, b = jo.Oracle(sysd, **dict(kw, flags=jo.F_BJAOAJB)), jo.Oracle(sysd, **dict(kw, flags=0))
+    a.jump_step(25); b.jump_step(25)
+    assert np.array_equal(a.pos, b.pos) and np.array_equal(a.vel, b.vel) and a.stats()["proposals"] == 0
+    a, b = jo.Oracle(sysd, **dict(kw, flags=3 | 4 | jo.F_BJAOAJB)), jo.Oracle(sysd, **dict(kw, flags=3 | 4))
+    a.jump_step(20); b.jump_step(20)
+    ea, eb = a.events(), b.events()
+    assert set(np.unique(ea["stream"])) == {1, 2, 3, 4}
+    assert len(ea) != len(eb) or not np.array_equal(ea["T"], eb["T"])
+    ra, rb = a.stats()["proposals"], b.stats()["proposals"]
+    assert abs(ra / rb - 1.0) < 0.05
+    assert a.stats()["max_p"] <= 1.0 and np.abs(a.pos - b.pos).max() > 1e-6
+    # one step by hand: B, J at frozen x with a = 0 (jump_half), A O A, J, B reproduce jump_step(1)
+    c = jo.Oracle(sysd, **dict(kw, flags=3 | jo.F_BJAOAJB, gamma_per_ps=0.0))
+    d = jo.Oracle(sysd, **dict(kw, flags=3, gamma_per_ps=0.0))
+    c.jump_step(1)
+    H = 0.5e-3
+    f0 = d.forces(0)
+    d.set_vel(d.vel - H * KCAL * f0 / sysd["mass"][:, None])
+    d.jump_half(H, with_accel=False, step=0)                 # opening C'J' streams (1, 2) with a = 0
+    x = d.pos + 2 * H * d.vel                                # A O A with gamma = 0
+    assert np.abs((c.pos - x + 6.0) % sysd["box"] - 6.0).max() < 1e-12
