@@ -36,6 +36,7 @@ extern "C" {
 #define JUMP_F_RESPA_PAPER 8u      /* RESPA: bonded inner, short non-bonded + jumps outer */
 #define JUMP_F_RESPA_COMPARATOR 16u /* jump_respa_step runs BAOAB-RESPA: outer kick by the long force */
 
+#define JUMP_F_BJAOAJB 64u         /* jump_step runs B J A O A J B instead of C'J' A O A J'C' */
 #define JUMP_F_STRICT_SKIN 32u      /* make a displacement beyond skin/2 between list builds an error (JUMP_E_SKIN) */
 
 typedef struct jump_ctx jump_ctx; /* opaque, owned by the library */

@@ -410,18 +410,22 @@ extern "C" int jump_step(jump_ctx *c, int32_t n_steps) {
     if (!c || n_steps < 0) return JUMP_E_ARG;
     if (n_steps == 0) return 0;
     const double H = 0.5 * c->dt;
+    const bool bj = (c->p.flags & JUMP_F_BJAOAJB) != 0;
     int r0 = ensure_f0(c);
     if (r0) return r0;
     for (int s = 0; s < n_steps; ++s) {
         int64_t st = c->step;
         Phase open = ph_jump(c, H, true, false, 1, 2, st);
         Phase close_prev = s > 0 ? ph_jump(c, H, true, true, 4, 3, st - 1) : ph_none();
+        if (bj) { open.bkick = 1; close_prev.bkick = 2; }   // B J A O A J B
         int r = run_update(c, close_prev, gr_f0(c), open, gr_f0(c), true);
         if (r) return r;
         r = compute_f0(c);
         if (r) return r;
     }
-    int r = run_update(c, ph_jump(c, H, true, true, 4, 3, c->step - 1), gr_f0(c), ph_none(), gr(nullptr), false);
+    Phase close_last = ph_jump(c, H, true, true, 4, 3, c->step - 1);
+    if (bj) close_last.bkick = 2;
+    int r = run_update(c, close_last, gr_f0(c), ph_none(), gr(nullptr), false);
     if (r) return r;
     return writeback(c);
 }

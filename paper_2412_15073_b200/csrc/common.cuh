@@ -170,6 +170,8 @@ struct Phase {      // one half-phase of velocity updates at frozen x
     float H;        // duration, ps
     int use_grad;   // acceleration a = -M^-1 (ga + gb) else 0
     int reverse;    // J' before C'
+    int bkick;      // kind 2 only: 0 = the chains run under the acceleration (step C'); 1 / 2 = B J / J B:
+                    // the kick H a apart, before / after chains on a piecewise constant velocity
     int coul, lj;   // which chains run (kind 2)
     int streamC, streamJ;
     unsigned int step;

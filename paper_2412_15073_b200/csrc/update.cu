@@ -407,16 +407,20 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
         if (P.kind == 1 || !JUMPS) {
             vx += P.H * ax; vy += P.H * ay; vz += P.H * az;
         } else {
+            // B J / J B: the kick apart, the chains on a piecewise constant velocity
+            const float cax = P.bkick ? 0.f : ax, cay = P.bkick ? 0.f : ay, caz = P.bkick ? 0.f : az;
+            if (P.bkick == 1) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
             // slots: J' if the phase is a closing one (J'C'), then C', then J' if it is an opening one (C'J')
 #pragma unroll 1
             for (int slot = 0; slot < 3; ++slot) {
                 if (slot == 1) {
-                    if (P.coul) chain_C<G, LOG, ADAPT>(m, A, live, cc, i, atom, xi, mi.y, ax, ay, az, P.H, P.streamC, P.step, vx, vy, vz, tl, gl, gshift);
-                    else if (P.use_grad) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
+                    if (P.coul) chain_C<G, LOG, ADAPT>(m, A, live, cc, i, atom, xi, mi.y, cax, cay, caz, P.H, P.streamC, P.step, vx, vy, vz, tl, gl, gshift);
+                    else if (P.use_grad) { vx += P.H * cax; vy += P.H * cay; vz += P.H * caz; }
                 } else if (P.lj && live && (slot == 0) == (P.reverse != 0)) {
                     chain_J(m, A, NV, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
                 }
             }
+            if (P.bkick == 2) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
         }
     }
     if (live) {

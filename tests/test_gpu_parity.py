@@ -184,6 +184,25 @@ def test_event_log_and_trajectory_cfg0(jb, jo, cfg0, eps, seed, mode):
         assert sg["gt_attempts"] == so["gt_attempts"] and sg["expiries"] == so["expiries"]
 
 
+def test_bjaoajb_scheme_matches_oracle(jb, jo, cfg0):
+    """NEXT-3: B J A O A J B as the scheme of jump_step -- event log and trajectory against the oracle,
+    and without any jump mechanism the scheme is bitwise the C' scheme without jumps (BAOAB with F0)."""
+    sysd, run = cfg0
+    r = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG | jb.F_BJAOAJB, seed=3026)
+    g, o = jb.JumpSim(sysd, **r), jo.Oracle(sysd, **r)
+    g.jump_step(10); g.sync(); o.jump_step(10)
+    assert len(o.events()) > 15000
+    check_events(g.events(), o.events())
+    g.clear_events(); o.clear_events()
+    g.jump_step(10); g.sync(); o.jump_step(10)
+    if not fragile(o):
+        assert pos_err(g, o, sysd["box"]) <= X_TOL
+        assert np.abs(g.vel.cpu().numpy() - o.vel).max() < 5e-3
+    a, b = jb.JumpSim(sysd, **dict(run, flags=jb.F_BJAOAJB)), jb.JumpSim(sysd, **dict(run, flags=0))
+    a.jump_step(25); b.jump_step(25); a.sync(); b.sync()
+    assert (a.pos == b.pos).all() and (a.vel == b.vel).all() and a.stats()["proposals"] == 0
+
+
 def test_jump_half_statistics_frozen_x(jb, jo, cfg0):
     """The C'/J' half-phase alone at frozen x, long duration (many events per atom), with and without drift."""
     sysd, run = cfg0
