@@ -116,6 +116,17 @@ int jump_clear_events(jump_ctx *c);
 /* Row which (0 short, 1 M, 2 L, 3 V) of original atom i as original indices in canonical order (R-10);
  * returns the row length (or a negative error); at most cap entries are written to host_out. */
 int jump_get_row(jump_ctx *c, int32_t which, int32_t atom, int32_t *host_out, int32_t cap);
+/* Observables on the device (the paper's evidence is of this kind).
+ * jump_get_images: periodic image counters (n x 3 int32, device, original order): the unwrapped position of atom i is
+ *   d_pos[i] + image[i] * box, continuous since jump_init (or the last jump_refresh, which resets the counters); each
+ *   counter holds +-511 box lengths.  Synchronises the stream.
+ * jump_rdf_accumulate: adds to d_hist[n_bins] (device, uint64, caller-owned and zeroed by the caller) the number of
+ *   unordered pairs of atoms (lj_only != 0: of LJ carriers, the water oxygens) whose minimum-image distance r at the
+ *   current positions is < r_max, in bin floor(r n_bins / r_max); r_max <= box/2, n_bins <= 2048.  Bonded exclusions
+ *   are not applied (a geometric histogram).  Asynchronous on the context's stream.  g(r) is
+ *   hist / (n_calls * 0.5 N (N-1) / V * shell volume). */
+int jump_get_images(jump_ctx *c, int32_t *d_img);
+int jump_rdf_accumulate(jump_ctx *c, int32_t lj_only, double r_max, int32_t n_bins, uint64_t *d_hist);
 /* Bounds as used (R-7): GM, GL, GV, qmax, eps_max, sig_min, sig_max, rM. */
 int jump_get_bounds(jump_ctx *c, double out[8]);
 /* Re-read d_pos / d_vel after the caller changed them: re-sort, rebuild rows, recompute F0. */

@@ -361,3 +361,18 @@ def gtilde_draw(eta, seed, atom, step=0):
 
 def num_threads():
     return int(lib().orc_num_threads())
+
+
+def pair_histogram(pos, box, r_max, n_bins):
+    """NEXT-4 oracle: number of unordered pairs of the given points whose minimum-image distance r (cubic periodic box,
+    P:L325) is < r_max, per bin floor(r n_bins / r_max) -- the plain definition, O(N^2), fp64.  g(r) follows by
+    dividing by 0.5 N (N-1) / V times the shell volumes (the radial distribution functions of P:L527-531)."""
+    x = np.asarray(pos, dtype=np.float64)
+    hist = np.zeros(n_bins, dtype=np.int64)
+    for i in range(len(x) - 1):
+        d = x[i + 1:] - x[i]
+        d -= box * np.round(d / box)
+        r = np.sqrt((d * d).sum(1))
+        b = np.floor(r[r < r_max] * (n_bins / r_max)).astype(np.int64)
+        hist += np.bincount(np.minimum(b, n_bins - 1), minlength=n_bins)
+    return hist

@@ -19,7 +19,7 @@ ERRORS = {-1: "bad argument", -2: "CUDA error", -3: "row/event overflow", -4: "t
           -5: "displacement beyond skin/2", -6: "non-finite state"}
 
 EXPORTS = ["jump_init", "jump_step", "baoab_step", "jump_respa_step", "jump_get_forces", "jump_get_energy",
-           "jump_get_stats", "jump_reset_stats", "jump_get_events", "jump_clear_events", "jump_get_row",
+           "jump_get_stats", "jump_reset_stats", "jump_get_events", "jump_clear_events", "jump_get_row", "jump_get_images", "jump_rdf_accumulate",
            "jump_get_bounds", "jump_refresh", "jump_half", "jump_sync", "jump_get_step", "jump_get_launches",
            "jump_last_error", "jump_free", "jump_set_profiling", "jump_get_profile", "jump_count_pairs"]
 
@@ -82,6 +82,8 @@ def lib():
         L.jump_clear_events.argtypes = [vp]
         L.jump_get_row.argtypes = [vp, i32, i32, C.POINTER(i32), i32]
         L.jump_get_bounds.argtypes = [vp, dp]
+        L.jump_get_images.argtypes = [vp, vp]
+        L.jump_rdf_accumulate.argtypes = [vp, i32, C.c_double, i32, vp]
         L.jump_refresh.argtypes = [vp]
         L.jump_half.argtypes = [vp, C.c_double, i32, i64]
         L.jump_sync.argtypes = [vp]
@@ -251,6 +253,22 @@ class JumpSim:
         out = (C.c_int32 * self.n)()
         m = self._check(self._L.jump_get_row(self._h, int(which), int(atom), out, self.n), "jump_get_row")
         return np.frombuffer(out, dtype=np.int32, count=m).copy()
+
+    def images(self):
+        """Periodic image counters (n x 3 int32 on the device): unwrapped position = pos + images * box."""
+        out = self._torch.empty((self.n, 3), dtype=self._torch.int32, device=self.device)
+        self._check(self._L.jump_get_images(self._h, C.c_void_p(out.data_ptr())), "jump_get_images")
+        return out
+
+    def pos_unwrapped(self):
+        box = self._torch.tensor([self.params.box[0], self.params.box[1], self.params.box[2]], dtype=self._torch.float64, device=self.device)
+        return self.pos.double() + self.images().double() * box
+
+    def rdf_accumulate(self, hist, r_max, lj_only=True):
+        """Add the pair-distance histogram of the current positions to hist (device int64 / uint64 tensor of n_bins)."""
+        assert hist.is_cuda and hist.element_size() == 8 and hist.is_contiguous()
+        self._check(self._L.jump_rdf_accumulate(self._h, int(bool(lj_only)), float(r_max), int(hist.numel()),
+                                                C.c_void_p(hist.data_ptr())), "jump_rdf_accumulate")
 
     def bounds(self):
         out = (C.c_double * 8)()

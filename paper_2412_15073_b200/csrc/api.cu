@@ -820,6 +820,22 @@ extern "C" int jump_get_row(jump_ctx *c, int32_t which, int32_t atom, int32_t *h
     for (int k = 0; k < cnt && k < cap; ++k) host_out[k] = orig[row[k]];
     return cnt;
 }
+extern "C" int jump_get_images(jump_ctx *c, int32_t *d_img) {
+    if (!c || !d_img) return JUMP_E_ARG;
+    launch_images(c->n, c->xl, c->orig, d_img, c->st, &c->launches);
+    CK(cudaGetLastError());
+    return poll_error(c);
+}
+extern "C" int jump_rdf_accumulate(jump_ctx *c, int32_t lj_only, double r_max, int32_t n_bins, uint64_t *d_hist) {
+    if (!c || !d_hist) return JUMP_E_ARG;
+    // The cell table of the last sort indexes the sorted array, and an atom has moved by at most about the skin
+    // since: the home cell of i is taken from its current position and the stencil reaches r_max + skin.
+    if (launch_rdf(c->m, c->g, lj_only != 0, r_max, r_max + c->p.skin, n_bins, c->cell_start, c->xs, c->lj,
+                   (unsigned long long *)d_hist, c->st, &c->launches))
+        return JUMP_E_ARG;
+    CK(cudaGetLastError());
+    return 0;
+}
 extern "C" int jump_get_bounds(jump_ctx *c, double out[8]) {
     if (!c || !out) return JUMP_E_ARG;
     out[0] = c->GM; out[1] = c->GL; out[2] = c->GV; out[3] = c->qmax;

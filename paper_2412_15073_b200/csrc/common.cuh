@@ -104,6 +104,16 @@ __device__ inline float min_image1(float xi, float xj, float L, float invL) {
     return a - b;
 }
 
+// Periodic image counters of an atom (NEXT-4: unwrapped trajectories for mean-square displacements): three
+// 10-bit fields biased by 512, carried in the spare .w of the position residual xl and moved with it by the sort.
+constexpr int kImgBias = 512;
+__host__ __device__ inline int img_pack(int ix, int iy, int iz) {
+    return ((ix + kImgBias) & 1023) | (((iy + kImgBias) & 1023) << 10) | (((iz + kImgBias) & 1023) << 20);
+}
+__host__ __device__ inline void img_unpack(int w, int &ix, int &iy, int &iz) {
+    ix = (w & 1023) - kImgBias; iy = ((w >> 10) & 1023) - kImgBias; iz = ((w >> 20) & 1023) - kImgBias;
+}
+
 // erfc(x) exp(x^2) for 0 <= x <= 4.3 (alpha r never exceeds 3.8 (1 + skin / r_long)): degree-8 polynomial in
 // t = 1 / (1 + x/2), a relative-weighted Chebyshev least-squares fit made for this file (max relative error
 // 6e-8 in exact arithmetic, 2.6e-7 evaluated in fp32 -- the accuracy of erfcf).  erfc(alpha r) is then

@@ -350,10 +350,13 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, int NV, int i, unsi
     }
 }
 
-__device__ inline double wrap1d(double x, double L) {
-    x -= L * floor(x / L);
-    if (x >= L) x -= L;
+__device__ inline double wrap1d(double x, double L, int &img) {   // img += the number of box lengths taken off
+    const double k = floor(x / L);
+    x -= L * k;
+    int ik = (int)k;
+    if (x >= L) { x -= L; ++ik; }
     if (x < 0.0) x = 0.0;
+    img += ik;
     return x;
 }
 
@@ -443,10 +446,13 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
             vy = A.c1 * vy + sc * (r1 * s1);
             vz = A.c1 * vz + sc * (r2 * c2);
             X += hdt * (double)vx; Y += hdt * (double)vy; Z += hdt * (double)vz;  // A
-            X = wrap1d(X, (double)m.box[0]); Y = wrap1d(Y, (double)m.box[1]); Z = wrap1d(Z, (double)m.box[2]);
+            int ix, iy, iz;
+            img_unpack(__float_as_int(xlo.w), ix, iy, iz);
+            X = wrap1d(X, (double)m.box[0], ix); Y = wrap1d(Y, (double)m.box[1], iy); Z = wrap1d(Z, (double)m.box[2], iz);
             const float x = (float)X, y = (float)Y, z = (float)Z;
             A.xs_out[i] = make_float4(x, y, z, xi.w);
-            A.xl[i] = make_float4((float)(X - (double)x), (float)(Y - (double)y), (float)(Z - (double)z), 0.f);
+            A.xl[i] = make_float4((float)(X - (double)x), (float)(Y - (double)y), (float)(Z - (double)z),
+                                  __int_as_float(img_pack(ix, iy, iz)));
             float4 xb = A.x_build[i];
             float ddx = min_image1(x, xb.x, m.box[0], m.inv_box[0]);
             float ddy = min_image1(y, xb.y, m.box[1], m.inv_box[1]);
@@ -525,7 +531,7 @@ __global__ void k_load(Model m, const float *__restrict__ pos, const float *__re
     float z = wrap1(pos[3 * i + 2], m.box[2], m.inv_box[2]);
     xs[i] = make_float4(x, y, z, charge[i]);
     vs[i] = make_float4(vel[3 * i], vel[3 * i + 1], vel[3 * i + 2], 0.f);
-    xl[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    xl[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(img_pack(0, 0, 0)));   // residual 0, image counters 0
     float e = eps[i];
     lj[i] = make_float2(e > 0.f ? (float)sqrt((double)sigma[i]) : 0.f, e > 0.f ? (float)(2.0 * sqrt((double)e)) : 0.f);
     double md = (double)mass[i];
@@ -545,8 +551,18 @@ __global__ void k_reload(Model m, const float *__restrict__ pos, const float *__
     x.y = wrap1(pos[3 * o + 1], m.box[1], m.inv_box[1]);
     x.z = wrap1(pos[3 * o + 2], m.box[2], m.inv_box[2]);
     xs[i] = x;
-    xl[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    xl[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(img_pack(0, 0, 0)));   // residual 0, image counters 0
     vs[i] = make_float4(vel[3 * o], vel[3 * o + 1], vel[3 * o + 2], 0.f);
+}
+
+// image counters (sorted) -> caller order, n x 3 int32
+__global__ void k_images(int n, const float4 *__restrict__ xl, const int *__restrict__ orig, int *__restrict__ out) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int ix, iy, iz;
+    img_unpack(__float_as_int(xl[i].w), ix, iy, iz);
+    int o = orig[i];
+    out[3 * o] = ix; out[3 * o + 1] = iy; out[3 * o + 2] = iz;
 }
 
 // kinetic energy per atom into out[i] (kcal/mol), sorted order
@@ -613,6 +629,10 @@ void launch_load(const Model &m, const float *pos, const float *vel, const float
 void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
                    float4 *xl, cudaStream_t st, int64_t *launches) {
     k_reload<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, orig, xs, vs, xl);
+    *launches += 1;
+}
+void launch_images(int n, const float4 *xl, const int *orig, int *out, cudaStream_t st, int64_t *launches) {
+    k_images<<<(n + 255) / 256, 256, 0, st>>>(n, xl, orig, out);
     *launches += 1;
 }
 void launch_kinetic(int n, const float4 *vs, const float2 *mi, double *out, cudaStream_t st, int64_t *launches) {

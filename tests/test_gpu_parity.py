@@ -409,3 +409,49 @@ def test_config4_one_million_atoms_properties(jb):
         out.append((g.pos.cpu().numpy().copy(), g.vel.cpu().numpy().copy()))
         g.close()
     assert (out[0][0] == out[1][0]).all() and (out[0][1] == out[1][1]).all()
+
+
+# ------------------------------------------------------------------------------------- NEXT-4: observables on the device
+def test_image_counters_give_continuous_unwrapped_positions(jb, jo, cfg0):
+    """Unwrapped positions pos + images * box: equal to the oracle's unwrapped trajectory on the parity window, and
+    continuous over a run long enough for many atoms to cross the box faces."""
+    sysd, run = cfg0
+    box = float(sysd["box"])
+    g, o = jb.JumpSim(sysd, **dict(run, seed=3026)), jo.Oracle(sysd, **dict(run, seed=3026))
+    g.jump_step(60); g.sync(); o.jump_step(60)
+    if not fragile(o):
+        assert np.abs(g.pos_unwrapped().cpu().numpy() - o.pos_unwrapped).max() <= X_TOL
+    prev = g.pos_unwrapped().cpu().numpy()
+    for _ in range(150):                                   # 3 ps, a check every 20 fs
+        g.jump_step(20)
+        cur = g.pos_unwrapped().cpu().numpy()
+        assert np.abs(cur - prev).max() < 2.0              # a missed or doubled image would be a jump of one box length
+        prev = cur
+    img = g.images().cpu().numpy()
+    assert (img != 0).any(1).sum() > 20                    # atoms did cross
+    w = g.pos.cpu().numpy().astype(np.float64)
+    assert (w >= 0).all() and (w < box).all()
+    g.refresh()
+    assert (g.images().cpu().numpy() == 0).all()           # jump_refresh restarts the counters
+
+
+@pytest.mark.parametrize("cfg,lj_only", [(0, True), (0, False), (1, True)])
+def test_rdf_histogram_matches_plain_definition(jb, jo, cfg, lj_only):
+    """jump_rdf_accumulate against the oracle's O(N^2) pair histogram of the same positions (integer counts; a pair
+    within fp32 rounding of a bin edge may fall on the other side of it)."""
+    import torch
+    sysd, run = wl.make_config(cfg)
+    g = jb.JumpSim(sysd, **run)
+    g.baoab_step(40); g.jump_step(27); g.sync()            # positions a few steps after a list rebuild
+    r_max, n_bins = 8.0, 160
+    hist = torch.zeros(n_bins, dtype=torch.int64, device=g.device)
+    g.rdf_accumulate(hist, r_max, lj_only=lj_only); g.sync()
+    x = g.pos.cpu().numpy().astype(np.float64)
+    sel = np.asarray(sysd["lj_eps"]) > 0 if lj_only else np.ones(g.n, bool)
+    ref = jo.pair_histogram(x[sel], float(sysd["box"]), r_max, n_bins)
+    got = hist.cpu().numpy()
+    assert abs(int(got.sum()) - int(ref.sum())) <= 2 and np.abs(got - ref).sum() <= 8
+    g.rdf_accumulate(hist, r_max, lj_only=lj_only); g.sync()
+    assert (hist.cpu().numpy() == 2 * got).all()           # accumulates
+    with pytest.raises(jb.JumpError):
+        g.rdf_accumulate(hist, 0.51 * float(sysd["box"]), lj_only=lj_only)

@@ -638,3 +638,21 @@ def test_bjaoajb_scheme(relaxed_small):
     d.jump_half(H, with_accel=False, step=0)                 # opening C'J' streams (1, 2) with a = 0
     x = d.pos + 2 * H * d.vel                                # A O A with gamma = 0
     assert np.abs((c.pos - x + 6.0) % sysd["box"] - 6.0).max() < 1e-12
+
+
+def test_pair_histogram_lattice_and_ideal_gas():
+    """NEXT-4 oracle pin: on a simple cubic lattice the neighbour shells are known in closed form (6 at a, 12 at
+    a sqrt 2, 8 at a sqrt 3, 6 at 2a per site, each pair once); for uniform random points g(r) = 1."""
+    n, a = 6, 2.0
+    g = np.stack(np.meshgrid(*[np.arange(n)] * 3, indexing="ij"), -1).reshape(-1, 3) * a
+    h = jo.pair_histogram(g, n * a, 4.1, 41)                      # bins of 0.1
+    N = n ** 3
+    expect = {20: 6 * N // 2, 28: 12 * N // 2, 34: 8 * N // 2, 40: 6 * N // 2}      # floor(r / 0.1)
+    for b in range(41):
+        assert h[b] == expect.get(b, 0), (b, h[b])
+    rng = np.random.default_rng(3)
+    box, M = 20.0, 3000
+    h = jo.pair_histogram(rng.uniform(0, box, size=(M, 3)), box, 8.0, 16)
+    edges = np.linspace(0, 8.0, 17)
+    ideal = 0.5 * M * (M - 1) / box ** 3 * 4 / 3 * np.pi * (edges[1:] ** 3 - edges[:-1] ** 3)
+    assert np.abs(h[2:] / ideal[2:] - 1).max() < 5 / np.sqrt(ideal[2:].min())
