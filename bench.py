@@ -366,7 +366,8 @@ def main():
     bytes_each_way = 2 * n * 3 * 4
     e2e = {"value": world * ns_per_day(e2e_steps / (ms_e_max * 1e-3), dt_fs), "unit": "ns/day",
            "h2d_bytes_per_step": bytes_each_way / block, "d2h_bytes_per_step": bytes_each_way / block,
-           "call": "JumpSim.run_host: pinned host (x, v) -> device, jump_refresh, %d steps, device -> host, per call" % block}
+           "call": "JumpSim.run_host: pinned host (x, v) -> device, jump_refresh_lazy (rows rebuilt only if an atom left its "
+                   "skin/2 ball), %d steps, device -> host, per call" % block}
 
     large = None
     if rank == 0 and world == 1 and args.large_config >= 0:

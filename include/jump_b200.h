@@ -131,6 +131,12 @@ int jump_rdf_accumulate(jump_ctx *c, int32_t lj_only, double r_max, int32_t n_bi
 int jump_get_bounds(jump_ctx *c, double out[8]);
 /* Re-read d_pos / d_vel after the caller changed them: re-sort, rebuild rows, recompute F0. */
 int jump_refresh(jump_ctx *c);
+/* The same for a caller that hands the state back after a few steps (host round trips): the rows are kept, and the
+ * sorted order with them, when no atom is farther than skin/2 from its position at the last list build -- they are
+ * still supersets of the pairs in range (R-10); otherwise re-sort and rebuild as jump_refresh does.  *rebuilt (may be
+ * NULL) receives 0 / 1.  The list-rebuild period of the step calls keeps counting.  F0 is recomputed; the image
+ * counters are reset.  Synchronises the stream once (the decision is taken on the host). */
+int jump_refresh_lazy(jump_ctx *c, int32_t *rebuilt);
 /* Run only the opening jump half-phase C'(H) [then J'(H)] at frozen x with stream ids 1, 2 (pins). */
 int jump_half(jump_ctx *c, double H_ps, int32_t with_accel, int64_t step);
 /* Wait for the stream; returns the sticky device error if any. */

@@ -20,7 +20,7 @@ ERRORS = {-1: "bad argument", -2: "CUDA error", -3: "row/event overflow", -4: "t
 
 EXPORTS = ["jump_init", "jump_step", "baoab_step", "jump_respa_step", "jump_get_forces", "jump_get_energy",
            "jump_get_stats", "jump_reset_stats", "jump_get_events", "jump_clear_events", "jump_get_row", "jump_get_images", "jump_rdf_accumulate",
-           "jump_get_bounds", "jump_refresh", "jump_half", "jump_sync", "jump_get_step", "jump_get_launches",
+           "jump_get_bounds", "jump_refresh", "jump_refresh_lazy", "jump_half", "jump_sync", "jump_get_step", "jump_get_launches",
            "jump_last_error", "jump_free", "jump_set_profiling", "jump_get_profile", "jump_count_pairs"]
 
 
@@ -85,6 +85,7 @@ def lib():
         L.jump_get_images.argtypes = [vp, vp]
         L.jump_rdf_accumulate.argtypes = [vp, i32, C.c_double, i32, vp]
         L.jump_refresh.argtypes = [vp]
+        L.jump_refresh_lazy.argtypes = [vp, C.POINTER(i32)]
         L.jump_half.argtypes = [vp, C.c_double, i32, i64]
         L.jump_sync.argtypes = [vp]
         L.jump_get_step.argtypes = [vp]
@@ -190,16 +191,23 @@ class JumpSim:
     def refresh(self):
         self._check(self._L.jump_refresh(self._h), "jump_refresh")
 
+    def refresh_lazy(self):
+        """Re-read pos / vel; rows are rebuilt only if an atom left the skin/2 ball of its build position.  -> rebuilt?"""
+        flag = C.c_int32(0)
+        self._check(self._L.jump_refresh_lazy(self._h, C.byref(flag)), "jump_refresh_lazy")
+        return bool(flag.value)
+
     def run_host(self, host_pos, host_vel, n_steps, mode="jump"):
-        """End-to-end call with HOST state: copy (x, v) from the (pinned) host tensors to the device, re-sort and
-        rebuild the rows at those positions, run n_steps (mode "jump": jump_step; "respa": jump_respa_step with
-        n_steps / n_inner outer steps; "baoab": baoab_step) and copy (x, v) back into the same host tensors.
-        Everything is enqueued on the context's stream; the caller synchronises it."""
+        """End-to-end call with HOST state: copy (x, v) from the (pinned) host tensors to the device, take them over
+        (jump_refresh_lazy: the rows are rebuilt at those positions unless every atom is still within skin/2 of where
+        the last build saw it), run n_steps (mode "jump": jump_step; "respa": jump_respa_step with n_steps / n_inner
+        outer steps; "baoab": baoab_step) and copy (x, v) back into the same host tensors.  The copies and kernels are
+        enqueued on the context's stream (jump_refresh_lazy synchronises it once); the caller synchronises at the end."""
         torch = self._torch
         with torch.cuda.stream(self.stream):
             self.pos.copy_(host_pos, non_blocking=True)
             self.vel.copy_(host_vel, non_blocking=True)
-            self.refresh()
+            self.refresh_lazy()
             if mode == "jump":
                 self.jump_step(n_steps)
             elif mode == "respa":

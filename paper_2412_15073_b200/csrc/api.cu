@@ -39,6 +39,7 @@ struct jump_ctx {
 
     double *ke;
     unsigned long long *pair_count;   // scratch of jump_count_pairs
+    int *moved_flag;                  // scratch of jump_refresh_lazy
     int *excl_ptr, *excl_idx;
     Topo topo;
     std::vector<void *> owned;  // everything to cudaFree
@@ -690,6 +691,7 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     c->step = c->outer = c->rebuilds = c->launches = 0;
     c->sticky = 0;
     c->pair_count = nullptr;
+    c->moved_flag = nullptr;
     c->f0_valid = false;
     c->prof = false;
     for (int k = 0; k < 4; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
@@ -844,12 +846,27 @@ extern "C" int jump_get_bounds(jump_ctx *c, double out[8]) {
 }
 extern "C" int jump_refresh(jump_ctx *c) {
     if (!c) return JUMP_E_ARG;
-    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, c->st, &c->launches);
+    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, nullptr, nullptr, c->st, &c->launches);
     CK(cudaGetLastError());
     int r = resort_and_build(c);
     if (r) return r;
     if ((r = compute_f0(c))) return r;
     return poll_error(c);
+}
+extern "C" int jump_refresh_lazy(jump_ctx *c, int32_t *rebuilt) {
+    if (!c) return JUMP_E_ARG;
+    int r;
+    if (!c->moved_flag && (r = dalloc(c, &c->moved_flag, 1))) return r;
+    CK(cudaMemsetAsync(c->moved_flag, 0, sizeof(int), c->st));
+    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, c->x_build, c->moved_flag, c->st, &c->launches);
+    CK(cudaGetLastError());
+    int moved = 0;
+    CK(cudaMemcpyAsync(&moved, c->moved_flag, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    if (moved && (r = resort_and_build(c))) return r;
+    if (rebuilt) *rebuilt = moved;
+    if ((r = compute_f0(c))) return r;
+    return 0;
 }
 
 // ---- measurement helpers (bench.py) ------------------------------------------------------------------------

@@ -58,7 +58,7 @@ void launch_load(const Model &m, const float *pos, const float *vel, const float
                  const float *sigma, const float *eps, double kT, float4 *xs, float4 *vs, float4 *xl, float2 *lj, float2 *mi, int *orig,
                  cudaStream_t st, int64_t *launches);
 void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
-                   float4 *xl, cudaStream_t st, int64_t *launches);
+                   float4 *xl, const float4 *x_build, int *moved, cudaStream_t st, int64_t *launches);
 int launch_rdf(const Model &m, const SortGrid &g, int lj_only, double r_max, double r_reach, int n_bins, const int *cell_start,
                const float4 *xs, const float2 *lj, unsigned long long *hist, cudaStream_t st, int64_t *launches);
 void launch_images(int n, const float4 *xl, const int *orig, int *out, cudaStream_t st, int64_t *launches);

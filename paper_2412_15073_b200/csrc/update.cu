@@ -540,9 +540,10 @@ __global__ void k_load(Model m, const float *__restrict__ pos, const float *__re
 }
 
 // re-read the caller's positions (wrapped) and velocities into the current sorted order
+// moved (may be NULL): set to 1 when some atom is farther than skin/2 from its position at the last list build
 __global__ void k_reload(Model m, const float *__restrict__ pos, const float *__restrict__ vel,
                          const int *__restrict__ orig, float4 *__restrict__ xs, float4 *__restrict__ vs,
-                         float4 *__restrict__ xl) {
+                         float4 *__restrict__ xl, const float4 *__restrict__ x_build, int *__restrict__ moved) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
     int o = orig[i];
@@ -550,6 +551,14 @@ __global__ void k_reload(Model m, const float *__restrict__ pos, const float *__
     x.x = wrap1(pos[3 * o], m.box[0], m.inv_box[0]);
     x.y = wrap1(pos[3 * o + 1], m.box[1], m.inv_box[1]);
     x.z = wrap1(pos[3 * o + 2], m.box[2], m.inv_box[2]);
+    if (moved) {
+        const float4 xb = x_build[i];
+        const float dx = min_image1(x.x, xb.x, m.box[0], m.inv_box[0]);
+        const float dy = min_image1(x.y, xb.y, m.box[1], m.inv_box[1]);
+        const float dz = min_image1(x.z, xb.z, m.box[2], m.inv_box[2]);
+        const float d2 = dx * dx + dy * dy + dz * dz;
+        if (!(d2 <= m.half_skin2)) *moved = 1;   // also when a position is not finite
+    }
     xs[i] = x;
     xl[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(img_pack(0, 0, 0)));   // residual 0, image counters 0
     vs[i] = make_float4(vel[3 * o], vel[3 * o + 1], vel[3 * o + 2], 0.f);
@@ -627,8 +636,8 @@ void launch_load(const Model &m, const float *pos, const float *vel, const float
     *launches += 1;
 }
 void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
-                   float4 *xl, cudaStream_t st, int64_t *launches) {
-    k_reload<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, orig, xs, vs, xl);
+                   float4 *xl, const float4 *x_build, int *moved, cudaStream_t st, int64_t *launches) {
+    k_reload<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, orig, xs, vs, xl, x_build, moved);
     *launches += 1;
 }
 void launch_images(int n, const float4 *xl, const int *orig, int *out, cudaStream_t st, int64_t *launches) {

@@ -286,6 +286,26 @@ def test_degenerate_no_jumps_is_baoab_with_short_forces(jb, jo, cfg0):
     assert g.stats()["proposals"] == 0
 
 
+def test_refresh_lazy_keeps_valid_rows_and_rebuilds_when_needed(jb, jo, cfg0):
+    """jump_refresh_lazy: unchanged positions keep the rows (no rebuild) and F0 equals the oracle's at those
+    positions; positions moved beyond skin/2 trigger the rebuild; either way the next steps run without a flag."""
+    sysd, run = cfg0
+    g = jb.JumpSim(sysd, **run)
+    g.jump_step(23); g.sync()
+    n0 = g.stats()["rebuilds"]
+    assert g.refresh_lazy() is False and g.stats()["rebuilds"] == n0
+    o = jo.Oracle(dict(sysd, pos=g.pos.cpu().numpy().astype(np.float64), vel=g.vel.cpu().numpy().astype(np.float64)), **run)
+    assert rel_force_err(g.forces(0).cpu().numpy(), o.forces(0)) <= F_TOL
+    g.jump_step(10); g.sync()
+    assert g.stats()["error"] == 0
+    g.pos[5, 0] += 0.8                                      # one atom pushed out of its skin/2 ball
+    assert g.refresh_lazy() is True and g.stats()["rebuilds"] == n0 + 2
+    o = jo.Oracle(dict(sysd, pos=g.pos.cpu().numpy().astype(np.float64), vel=g.vel.cpu().numpy().astype(np.float64)), **run)
+    assert rel_force_err(g.forces(0).cpu().numpy(), o.forces(0)) <= F_TOL
+    g.jump_step(10); g.sync()
+    assert g.stats()["error"] == 0
+
+
 def test_determinism_bitwise(jb, cfg0):
     """Same inputs and seed: same bits (counter-based RNG, no floating-point atomics, canonical rows)."""
     sysd, run = cfg0
