@@ -286,21 +286,39 @@ def test_degenerate_no_jumps_is_baoab_with_short_forces(jb, jo, cfg0):
     assert g.stats()["proposals"] == 0
 
 
+def _liquid_state(jo, sysd, run, n_steps=300):
+    """A liquid-like (not lattice) state made by the ORACLE (no test input ever comes from the CUDA path), fp32-exact."""
+    o = jo.Oracle(sysd, **run)
+    o.baoab_step(n_steps)
+    s2 = dict(sysd, pos=np.float32(o.pos).astype(np.float64), vel=np.float32(o.vel).astype(np.float64))
+    o.close()
+    return s2
+
+
 def test_refresh_lazy_keeps_valid_rows_and_rebuilds_when_needed(jb, jo, cfg0):
-    """jump_refresh_lazy: unchanged positions keep the rows (no rebuild) and F0 equals the oracle's at those
-    positions; positions moved beyond skin/2 trigger the rebuild; either way the next steps run without a flag."""
+    """jump_refresh_lazy: positions moved by less than skin/2 keep the rows (no rebuild, stale cell table) and F0
+    equals the oracle's at the new positions; one atom pushed beyond skin/2 triggers the rebuild; either way the next
+    steps run without an error flag."""
+    import torch
     sysd, run = cfg0
-    g = jb.JumpSim(sysd, **run)
-    g.jump_step(23); g.sync()
+    s2 = _liquid_state(jo, sysd, run)
+    g = jb.JumpSim(s2, **run)
     n0 = g.stats()["rebuilds"]
+    rng = np.random.default_rng(17)
+    pos2 = np.float32(s2["pos"] + rng.uniform(-0.25, 0.25, size=s2["pos"].shape)).astype(np.float64)   # |d| < 0.44 < skin/2
+    g.pos.copy_(torch.as_tensor(np.float32(pos2)))
     assert g.refresh_lazy() is False and g.stats()["rebuilds"] == n0
-    o = jo.Oracle(dict(sysd, pos=g.pos.cpu().numpy().astype(np.float64), vel=g.vel.cpu().numpy().astype(np.float64)), **run)
-    assert rel_force_err(g.forces(0).cpu().numpy(), o.forces(0)) <= F_TOL
+    o = jo.Oracle(dict(s2, pos=pos2), **run)
+    for which in (0, 2):
+        assert rel_force_err(g.forces(which).cpu().numpy(), o.forces(which)) <= F_TOL
     g.jump_step(10); g.sync()
     assert g.stats()["error"] == 0
-    g.pos[5, 0] += 0.8                                      # one atom pushed out of its skin/2 ball
-    assert g.refresh_lazy() is True and g.stats()["rebuilds"] == n0 + 2
-    o = jo.Oracle(dict(sysd, pos=g.pos.cpu().numpy().astype(np.float64), vel=g.vel.cpu().numpy().astype(np.float64)), **run)
+    pos3 = pos2.copy()
+    pos3[5, 0] += 0.8                                       # one atom pushed out of its skin/2 ball
+    g.pos.copy_(torch.as_tensor(np.float32(pos3)))
+    n1 = g.stats()["rebuilds"]
+    assert g.refresh_lazy() is True and g.stats()["rebuilds"] == n1 + 1
+    o = jo.Oracle(dict(s2, pos=np.float32(pos3).astype(np.float64)), **run)
     assert rel_force_err(g.forces(0).cpu().numpy(), o.forces(0)) <= F_TOL
     g.jump_step(10); g.sync()
     assert g.stats()["error"] == 0
@@ -458,23 +476,29 @@ def test_image_counters_give_continuous_unwrapped_positions(jb, jo, cfg0):
 @pytest.mark.parametrize("cfg,lj_only", [(0, True), (0, False), (1, True)])
 def test_rdf_histogram_matches_plain_definition(jb, jo, cfg, lj_only):
     """jump_rdf_accumulate against the oracle's O(N^2) pair histogram of the same positions (integer counts; a pair
-    within fp32 rounding of a bin edge may fall on the other side of it)."""
+    within fp32 rounding of a bin edge may fall on the other side of it).  The positions are a seeded perturbation of
+    the generator's, handed over by jump_refresh_lazy WITHOUT a rebuild: the cell table the kernel walks is stale by up
+    to skin/2 per atom, as it is between two rebuilds of a run."""
     import torch
     sysd, run = wl.make_config(cfg)
     g = jb.JumpSim(sysd, **run)
-    g.baoab_step(40); g.jump_step(27); g.sync()            # positions a few steps after a list rebuild
+    rng = np.random.default_rng(23)
+    pos2 = np.float32(sysd["pos"] + rng.uniform(-0.25, 0.25, size=sysd["pos"].shape))
+    g.pos.copy_(torch.as_tensor(pos2))
+    assert g.refresh_lazy() is False
+    box = float(sysd["box"])
+    x = np.mod(pos2.astype(np.float64), box)
     r_max, n_bins = 8.0, 160
     hist = torch.zeros(n_bins, dtype=torch.int64, device=g.device)
     g.rdf_accumulate(hist, r_max, lj_only=lj_only); g.sync()
-    x = g.pos.cpu().numpy().astype(np.float64)
     sel = np.asarray(sysd["lj_eps"]) > 0 if lj_only else np.ones(g.n, bool)
-    ref = jo.pair_histogram(x[sel], float(sysd["box"]), r_max, n_bins)
+    ref = jo.pair_histogram(x[sel], box, r_max, n_bins)
     got = hist.cpu().numpy()
     assert abs(int(got.sum()) - int(ref.sum())) <= 2 and np.abs(got - ref).sum() <= 8
     g.rdf_accumulate(hist, r_max, lj_only=lj_only); g.sync()
     assert (hist.cpu().numpy() == 2 * got).all()           # accumulates
     with pytest.raises(jb.JumpError):
-        g.rdf_accumulate(hist, 0.51 * float(sysd["box"]), lj_only=lj_only)
+        g.rdf_accumulate(hist, 0.51 * box, lj_only=lj_only)
 
 
 # ------------------------------------------------------------------------------------- orthorhombic boxes
