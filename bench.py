@@ -345,6 +345,25 @@ def main():
     baoab = {"ns_per_day": ns_per_day(Kb / (ms_b * 1e-3), dt_fs), "ms_per_step": ms_b / Kb, "steps": Kb,
              "force": "unsplit pair force to r_long = %.0f A" % run["r_long"]}
 
+    # ---- the paper's preferred setting, adaptive eps(x) = eps0 |F_ij(x)| (NEXT-1, R-19), same box ------
+    adaptive = None
+    if not respa:
+        with torch.cuda.stream(stream):
+            run_a = dict(run, eps_mode=1, eps_jump=2.0)
+            sim_a = jb.JumpSim(sysd, device=dev, stream=stream, **run_a)
+            sim_a.baoab_step(args.equil)
+            sim_a.jump_step(max(W, 50))
+            sim_a.sync()
+            sim_a.reset_stats()
+            Ka = min(K, 1000)
+            ms_a = timed_blocks(torch, sim_a, stream, sim_a.jump_step, Ka, block, flush)
+            st_a = sim_a.stats()
+            sim_a.close()
+        adaptive = {"eps0_A_mol_per_kcal": 2.0, "steps": Ka, "ms_per_step": ms_a / Ka,
+                    "ns_per_day": ns_per_day(Ka / (ms_a * 1e-3), dt_fs),
+                    "proposals_per_atom_step": st_a["proposals"] / (n * Ka), "accepts_per_atom_step": st_a["accepts"] / (n * Ka),
+                    "max_p": st_a["max_p"], "error": st_a["error"]}
+
     # ---- end to end through the public API with HOST buffers -------------------------------------------------
     with torch.cuda.stream(stream):
         Ke = min(K, 500)
@@ -398,6 +417,8 @@ def main():
                 "events": {"proposals_per_atom_step": stats["proposals"] / (n * (K + W)) if K + W else None,
                            "accepts_per_atom_step": stats["accepts"] / (n * (K + W)), "max_p": stats["max_p"],
                            "error": stats["error"]}}
+        if adaptive is not None:
+            line["jump_adaptive_eps"] = adaptive
         if large is not None:
             line["roofline_large_box"] = large
         if cpu is not None:
