@@ -9,6 +9,7 @@
 //     from uniformly, with their counts N_M(i), N_L(i), N_V(i)).
 #include <algorithm>
 #include <cmath>
+#include <type_traits>
 
 #include "launch.h"
 
@@ -360,72 +361,81 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                     rbase[k] = JB_ROW_ON(k) ? rows.r[k].idx + (size_t)i * rows.r[k].cap : nullptr;
                 }
                 const float e0 = stn.edge2[0], e1 = stn.edge2[1], e2 = stn.edge2[2], e3 = stn.edge2[3];
-                for (int q0 = 0; q0 < npad; q0 += 32) {
-                    const float4 xj = tile[q0 + lane];
-                    const int jraw = __float_as_int(xj.w);
-                    const int j = jraw & 0x7fffffff;
-                    float dx, dy, dz;
-                    if (FAST) { dx = xi - xj.x; dy = yi - xj.y; dz = zi - xj.z; }
-                    else {
-                        dx = min_image1(xi, xj.x, m.box[0], m.inv_box[0]);
-                        dy = min_image1(yi, xj.y, m.box[1], m.inv_box[1]);
-                        dz = min_image1(zi, xj.z, m.box[2], m.inv_box[2]);
-                    }
-                    const float r2 = dx * dx + dy * dy + dz * dz;
-                    bool valid = r2 < rmax2t;   // false for the NaN of a padding entry
-                    if (!__any_sync(full, valid)) continue;
-                    const bool nearby = valid && r2 <= exr2;
-                    if (__any_sync(full, nearby)) {   // the atom itself and excluded pairs are never listed (R-9)
-                        bool ex = (j == i) | (j == ex4[0]) | (j == ex4[1]) | (j == ex4[2]) | (j == ex4[3]);
-                        if (n_ex > 4) {
-                            for (int base = 0; base < n_ex; base += 32) {
-                                int mine = (base + lane < n_ex) ? sorted_of[excl_idx[ex_lo + base + lane]] : -1;
-                                int lim = min(32, n_ex - base);
-                                for (int e = 0; e < lim; ++e) ex |= (__shfl_sync(full, mine, e) == j);
+                // The scan is instantiated twice: an atom without LJ (two thirds of a water box) has no V / W row, and
+                // its copy of the loop carries no test, ballot or counter for them (MASK >= 0; a branch on this
+                // inside the unrolled row loop was measured slower than the work it skips).
+                auto scan = [&](auto lj_tag) {
+                    constexpr bool LJ_I = decltype(lj_tag)::value;
+#define JB_ROW_SCAN(k) (JB_ROW_ON(k) && (LJ_I || MASK < 0 || ((k) != ROW_V && (k) != ROW_W)))
+                    for (int q0 = 0; q0 < npad; q0 += 32) {
+                        const float4 xj = tile[q0 + lane];
+                        const int jraw = __float_as_int(xj.w);
+                        const int j = jraw & 0x7fffffff;
+                        float dx, dy, dz;
+                        if (FAST) { dx = xi - xj.x; dy = yi - xj.y; dz = zi - xj.z; }
+                        else {
+                            dx = min_image1(xi, xj.x, m.box[0], m.inv_box[0]);
+                            dy = min_image1(yi, xj.y, m.box[1], m.inv_box[1]);
+                            dz = min_image1(zi, xj.z, m.box[2], m.inv_box[2]);
+                        }
+                        const float r2 = dx * dx + dy * dy + dz * dz;
+                        bool valid = r2 < rmax2t;   // false for the NaN of a padding entry
+                        if (!__any_sync(full, valid)) continue;
+                        const bool nearby = valid && r2 <= exr2;
+                        if (__any_sync(full, nearby)) {   // the atom itself and excluded pairs are never listed (R-9)
+                            bool ex = (j == i) | (j == ex4[0]) | (j == ex4[1]) | (j == ex4[2]) | (j == ex4[3]);
+                            if (n_ex > 4) {
+                                for (int base = 0; base < n_ex; base += 32) {
+                                    int mine = (base + lane < n_ex) ? sorted_of[excl_idx[ex_lo + base + lane]] : -1;
+                                    int lim = min(32, n_ex - base);
+                                    for (int e = 0; e < lim; ++e) ex |= (__shfl_sync(full, mine, e) == j);
+                                }
+                            }
+                            valid = valid && !ex;
+                        }
+                        const bool ljp = LJ_I && jraw < 0;
+                        bool pass[N_ROWS];
+    #pragma unroll
+                        for (int k = 0; k < N_ROWS; ++k) {
+                            pass[k] = false;
+                            if (!JB_ROW_SCAN(k)) continue;
+                            const Row &R = rows.r[k];
+                            pass[k] = valid && (!R.lj_only || ljp) && r2 >= R.r2min && r2 < R.r2max;
+                        }
+                        const bool tie = valid && fminf(fminf(fabsf(r2 - e0), fabsf(r2 - e1)), fminf(fabsf(r2 - e2), fabsf(r2 - e3))) < BUILD_TIE;
+                        if (tie) {   // decide in fp64 from the full positions, like the oracle
+                            float4 hi_j = xs[j], li = xl[i], lo_j = xl[j];
+                            double d[3] = {((double)xi4.x + (double)li.x) - ((double)hi_j.x + (double)lo_j.x),
+                                           ((double)xi4.y + (double)li.y) - ((double)hi_j.y + (double)lo_j.y),
+                                           ((double)xi4.z + (double)li.z) - ((double)hi_j.z + (double)lo_j.z)};
+                            double r2d = 0.0;
+    #pragma unroll
+                            for (int k = 0; k < 3; ++k) {
+                                double L = (double)m.box[k];
+                                d[k] -= L * rint(d[k] / L);
+                                r2d += d[k] * d[k];
+                            }
+    #pragma unroll
+                            for (int k = 0; k < N_ROWS; ++k) {
+                                if (!JB_ROW_SCAN(k)) continue;
+                                const Row &R = rows.r[k];
+                                pass[k] = (!R.lj_only || ljp) && r2d >= R.r2min_d && r2d < R.r2max_d;
                             }
                         }
-                        valid = valid && !ex;
-                    }
-                    const bool ljp = lj_i && jraw < 0;
-                    bool pass[N_ROWS];
-#pragma unroll
-                    for (int k = 0; k < N_ROWS; ++k) {
-                        pass[k] = false;
-                        if (!JB_ROW_ON(k)) continue;
-                        const Row &R = rows.r[k];
-                        pass[k] = valid && (!R.lj_only || ljp) && r2 >= R.r2min && r2 < R.r2max;
-                    }
-                    const bool tie = valid && fminf(fminf(fabsf(r2 - e0), fabsf(r2 - e1)), fminf(fabsf(r2 - e2), fabsf(r2 - e3))) < BUILD_TIE;
-                    if (tie) {   // decide in fp64 from the full positions, like the oracle
-                        float4 hi_j = xs[j], li = xl[i], lo_j = xl[j];
-                        double d[3] = {((double)xi4.x + (double)li.x) - ((double)hi_j.x + (double)lo_j.x),
-                                       ((double)xi4.y + (double)li.y) - ((double)hi_j.y + (double)lo_j.y),
-                                       ((double)xi4.z + (double)li.z) - ((double)hi_j.z + (double)lo_j.z)};
-                        double r2d = 0.0;
-#pragma unroll
-                        for (int k = 0; k < 3; ++k) {
-                            double L = (double)m.box[k];
-                            d[k] -= L * rint(d[k] / L);
-                            r2d += d[k] * d[k];
-                        }
-#pragma unroll
+    #pragma unroll
                         for (int k = 0; k < N_ROWS; ++k) {
-                            if (!JB_ROW_ON(k)) continue;
-                            const Row &R = rows.r[k];
-                            pass[k] = (!R.lj_only || ljp) && r2d >= R.r2min_d && r2d < R.r2max_d;
+                            if (!JB_ROW_SCAN(k)) continue;
+                            const unsigned mask = __ballot_sync(full, pass[k]);
+                            if (pass[k]) {
+                                int pos = count[k] + __popc(mask & lt_mask);
+                                if (pos < rows.r[k].cap) rbase[k][pos] = j;
+                            }
+                            count[k] += __popc(mask);
                         }
                     }
-#pragma unroll
-                    for (int k = 0; k < N_ROWS; ++k) {
-                        if (!JB_ROW_ON(k)) continue;
-                        const unsigned mask = __ballot_sync(full, pass[k]);
-                        if (pass[k]) {
-                            int pos = count[k] + __popc(mask & lt_mask);
-                            if (pos < rows.r[k].cap) rbase[k][pos] = j;
-                        }
-                        count[k] += __popc(mask);
-                    }
-                }
+#undef JB_ROW_SCAN
+                };
+                if (lj_i) scan(std::true_type{}); else scan(std::false_type{});
                 if (c1 >= total) {   // last chunk: publish the counts
                     if (lane == 0) {
 #pragma unroll
