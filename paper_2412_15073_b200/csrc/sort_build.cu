@@ -175,6 +175,12 @@ __device__ inline float near_image1(float d, float L, float invL) {
     return fmaf(-L, t, d);
 }
 
+// *p = v under a predicate, as ONE predicated store (the compiler's branch around a conditional store costs a
+// convergence barrier pair and a jump per row and chunk in the row build's inner loop)
+__device__ __forceinline__ void store_if(bool ok, int *p, int v) {
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %0, 0;\n\t@q st.global.s32 [%1], %2;\n\t}" ::"r"((int)ok), "l"(p), "r"(v) : "memory");
+}
+
 // Row build, one CTA per cell of the contract grid (per CX consecutive cells along x when the grid is large).
 //  1. The candidate set of a cell is the same for all its atoms: the cells of a host-computed stencil (every cell
 //     whose extent comes within rmax of this cell), visited in ascending cell key, i.e. a list of contiguous runs
@@ -426,10 +432,8 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                         for (int k = 0; k < N_ROWS; ++k) {
                             if (!JB_ROW_SCAN(k)) continue;
                             const unsigned mask = __ballot_sync(full, pass[k]);
-                            if (pass[k]) {
-                                int pos = count[k] + __popc(mask & lt_mask);
-                                if (pos < rows.r[k].cap) rbase[k][pos] = j;
-                            }
+                            const int pos = count[k] + __popc(mask & lt_mask);
+                            store_if(pass[k] && pos < rows.r[k].cap, rbase[k] + pos, j);   // predicated, no branch
                             count[k] += __popc(mask);
                         }
                     }
