@@ -306,14 +306,17 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
             const int c1 = min(c0 + BUILD_CHUNK, total);
             const int npad = (c1 - c0 + 31) & ~31;
             __syncthreads();   // the previous chunk has been consumed (and s_count is zeroed)
-            {   // ---- stage [c0, c1): thread t takes the candidates c0 + t, + BUILD_THREADS, ...; its run is found by one
-                // bisection and then advanced linearly
-                int q = c0 + tid, r = 0;
-                if (q < c1) {
+            {   // ---- stage [c0, c1): each warp takes a contiguous quarter of the chunk, 32 consecutive candidates per
+                // iteration (coalesced loads); a lane's run is found by one bisection and then advanced linearly --
+                // by about one run per iteration, since consecutive iterations of a lane are 32 candidates apart
+                constexpr int PER_WARP = BUILD_CHUNK / BUILD_WARPS;
+                int q = c0 + warp * PER_WARP + lane, r = 0;
+                const int q_end = min(c0 + (warp + 1) * PER_WARP, c1);
+                if (q < q_end) {
                     int hi_r = nrun - 1;   // last run with run_pre[r] <= q
                     while (r < hi_r) { int mid = (r + hi_r + 1) >> 1; if (run_pre[mid] <= q) r = mid; else hi_r = mid - 1; }
                 }
-                for (; q < c1; q += BUILD_THREADS) {
+                for (; q < q_end; q += 32) {
                     while (run_pre[r + 1] <= q) ++r;
                     const int j = run_beg[r] + (q - run_pre[r]);
                     float4 x = xs[j];
