@@ -376,6 +376,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                 auto scan = [&](auto lj_tag) {
                     constexpr bool LJ_I = decltype(lj_tag)::value;
 #define JB_ROW_SCAN(k) (JB_ROW_ON(k) && (LJ_I || MASK < 0 || ((k) != ROW_V && (k) != ROW_W)))
+#define JB_LJ_ROW(k) (MASK >= 0 ? ((k) == ROW_V || (k) == ROW_W) : rows.r[k].lj_only != 0)   // V and W are the LJ-only rows
                     for (int q0 = 0; q0 < npad; q0 += 32) {
                         const float4 xj = tile[q0 + lane];
                         const int jraw = __float_as_int(xj.w);
@@ -409,7 +410,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                             pass[k] = false;
                             if (!JB_ROW_SCAN(k)) continue;
                             const Row &R = rows.r[k];
-                            pass[k] = valid && (!R.lj_only || ljp) && r2 >= R.r2min && r2 < R.r2max;
+                            pass[k] = valid && (!JB_LJ_ROW(k) || ljp) && r2 >= R.r2min && r2 < R.r2max;
                         }
                         const bool tie = valid && fminf(fminf(fabsf(r2 - e0), fabsf(r2 - e1)), fminf(fabsf(r2 - e2), fabsf(r2 - e3))) < BUILD_TIE;
                         if (tie) {   // decide in fp64 from the full positions, like the oracle
@@ -428,7 +429,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                             for (int k = 0; k < N_ROWS; ++k) {
                                 if (!JB_ROW_SCAN(k)) continue;
                                 const Row &R = rows.r[k];
-                                pass[k] = (!R.lj_only || ljp) && r2d >= R.r2min_d && r2d < R.r2max_d;
+                                pass[k] = (!JB_LJ_ROW(k) || ljp) && r2d >= R.r2min_d && r2d < R.r2max_d;
                             }
                         }
     #pragma unroll
@@ -441,6 +442,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                         }
                     }
 #undef JB_ROW_SCAN
+#undef JB_LJ_ROW
                 };
                 if (lj_i) scan(std::true_type{}); else scan(std::false_type{});
                 if (c1 >= total) {   // last chunk: publish the counts
