@@ -405,7 +405,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                         }
                         const bool ljp = LJ_I && jraw < 0;
                         bool pass[N_ROWS];
-    #pragma unroll
+#pragma unroll
                         for (int k = 0; k < N_ROWS; ++k) {
                             pass[k] = false;
                             if (!JB_ROW_SCAN(k)) continue;
@@ -419,20 +419,20 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                                            ((double)xi4.y + (double)li.y) - ((double)hi_j.y + (double)lo_j.y),
                                            ((double)xi4.z + (double)li.z) - ((double)hi_j.z + (double)lo_j.z)};
                             double r2d = 0.0;
-    #pragma unroll
+#pragma unroll
                             for (int k = 0; k < 3; ++k) {
                                 double L = (double)m.box[k];
                                 d[k] -= L * rint(d[k] / L);
                                 r2d += d[k] * d[k];
                             }
-    #pragma unroll
+#pragma unroll
                             for (int k = 0; k < N_ROWS; ++k) {
                                 if (!JB_ROW_SCAN(k)) continue;
                                 const Row &R = rows.r[k];
                                 pass[k] = (!JB_LJ_ROW(k) || ljp) && r2d >= R.r2min_d && r2d < R.r2max_d;
                             }
                         }
-    #pragma unroll
+#pragma unroll
                         for (int k = 0; k < N_ROWS; ++k) {
                             if (!JB_ROW_SCAN(k)) continue;
                             const unsigned mask = __ballot_sync(full, pass[k]);
