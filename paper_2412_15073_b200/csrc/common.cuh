@@ -144,8 +144,10 @@ __device__ inline float erfcx_poly(float x) {
 template <bool EXACT>
 __device__ inline float chi_zone(float ax, float ay, float az, float bx, float by, float bz, float r2, float r,
                                  const Model &m, float &dchi) {
-    if (r2 <= m.rlo2) { dchi = 0.f; return 1.f; }
-    if (r2 >= m.rc2) { dchi = 0.f; return 0.f; }
+    if (EXACT) {
+        if (r2 <= m.rlo2) { dchi = 0.f; return 1.f; }
+        if (r2 >= m.rc2) { dchi = 0.f; return 0.f; }
+    }   // (the fp32 form needs no branch: the clamp of u to [0, 1] gives chi = 1, 0 and chi' = 0 outside the zone)
     float num;
     if (EXACT) {
         double dx = (double)ax - (double)bx, dy = (double)ay - (double)by, dz = (double)az - (double)bz;

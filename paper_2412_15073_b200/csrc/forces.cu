@@ -32,6 +32,8 @@ __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *_
     const float cutC2 = (WC == W_SHORT) ? m.rc2 : m.rE2, cutL2 = (WLJ == W_SHORT) ? m.rc2 : m.rE2;
     const float cut2 = (WC == W_NONE) ? cutL2 : ((WLJ == W_NONE) ? cutC2 : fmaxf(cutC2, cutL2));
     const bool do_lj = (WLJ != W_NONE) && lji.y > 0.f;
+    // both terms end at the same cutoff: the per-term tests after the common one are dropped at compile time
+    constexpr bool SAME_CUT = WC == W_NONE || WLJ == W_NONE || ((WC == W_SHORT) == (WLJ == W_SHORT));
     const int cnt = row.cnt[i];
     const int *__restrict__ ridx = row.idx + (size_t)i * row.cap;
     float fx = 0.f, fy = 0.f, fz = 0.f, en = 0.f;
@@ -55,7 +57,7 @@ __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *_
         float rinv = rsqrtf(r2), r = r2 * rinv;
         float fr = 0.f, chi = 1.f, dchi = 0.f;
         if (WC == W_SHORT || WC == W_LONG || WLJ == W_SHORT || WLJ == W_LONG) chi = chi_zone<false>(ax, ay, az, bx, by, bz, r2, r, m, dchi);
-        if (WC != W_NONE && r2 < cutC2) {
+        if (WC != W_NONE && (SAME_CUT || r2 < cutC2)) {
             float qq = qi * xj.w;
             float ex = expf(-m.alpha2 * r2), e = ex * erfcx_poly(m.alpha * r);
             float u = qq * e * rinv;
@@ -63,7 +65,7 @@ __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *_
             fr += weighted_du<WC>(chi, dchi, u, du);
             if (ENERGY) en += weighted_u<WC>(chi, u);
         }
-        if (do_lj && r2 < cutL2) {
+        if (do_lj && (SAME_CUT || r2 < cutL2)) {
             float2 ljj = lj[j];
             if (ljj.y > 0.f) {
                 float s = lji.x * ljj.x * rinv, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
