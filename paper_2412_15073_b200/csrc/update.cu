@@ -350,12 +350,13 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, int NV, int i, unsi
     }
 }
 
-__device__ inline double wrap1d(double x, double L, int &img) {   // img += the number of box lengths taken off
-    const double k = floor(x / L);
+__device__ inline double wrap1d(double x, double L, double invL, int &img) {   // img += the number of box lengths taken off
+    const double k = floor(x * invL);   // (a product, not the 40-instruction fp64 division; off by one at most, fixed below)
     x -= L * k;
     int ik = (int)k;
     if (x >= L) { x -= L; ++ik; }
-    if (x < 0.0) x = 0.0;
+    if (x < 0.0) { x += L; --ik; }
+    if (x >= L || x < 0.0) x = 0.0;
     img += ik;
     return x;
 }
@@ -448,7 +449,9 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
             X += hdt * (double)vx; Y += hdt * (double)vy; Z += hdt * (double)vz;  // A
             int ix, iy, iz;
             img_unpack(__float_as_int(xlo.w), ix, iy, iz);
-            X = wrap1d(X, (double)m.box[0], ix); Y = wrap1d(Y, (double)m.box[1], iy); Z = wrap1d(Z, (double)m.box[2], iz);
+            X = wrap1d(X, (double)m.box[0], (double)m.inv_box[0], ix);
+            Y = wrap1d(Y, (double)m.box[1], (double)m.inv_box[1], iy);
+            Z = wrap1d(Z, (double)m.box[2], (double)m.inv_box[2], iz);
             const float x = (float)X, y = (float)Y, z = (float)Z;
             A.xs_out[i] = make_float4(x, y, z, xi.w);
             A.xl[i] = make_float4((float)(X - (double)x), (float)(Y - (double)y), (float)(Z - (double)z),
