@@ -215,7 +215,7 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
         // lane gl draws Philox block kb + gl of the chain's stream: (E, ring, j, U) of proposal kb + gl (R-15)
         uint32_t w[4];
         philox4x32_10(atom, step, stream, kb + (unsigned)gl, m.key0, m.key1, w);
-        const float T_ = done ? INFINITY : -logf(u01(w[0])) / lam;   // P:L379 (lam = 0: +inf)
+        const float T_ = done ? INFINITY : __fdividef(-logf(u01(w[0])), lam);   // P:L379 (lam = 0: +inf); 2-ulp division
         // time of my proposal: t_run + (T_0 + ... + T_gl), an inclusive scan over the group in log2 G shuffle steps
         // (the fp32 sum is associated differently from a sequential chain's: 1e-7 relative, far inside the
         // margins of R-17)
@@ -231,7 +231,7 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
         float g = 0.f, LY = 1.f, nx = 0.f, ny = 0.f, nz = 0.f;
         int tag = 0;
         if (alive) propose_pair<LOG>(m, A.rowM, A.rowL, A.xs, A.orig, c, ringS, ringM, i, xi, w, g, LY, nx, ny, nz, tag);
-        const float goL = g / LY;
+        const float goL = __fdividef(g, LY);
         float p = 0.f, vn = 0.f;
         bool acc = false;
         if (ADAPT) {
