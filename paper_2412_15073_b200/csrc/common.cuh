@@ -76,7 +76,8 @@ __host__ __device__ inline void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 }
 
 // uniform in (0,1) with 24 significant bits, exact in fp32 and fp64 (R-15)
-__device__ inline float u01(uint32_t w) { return ((float)(w >> 9) + 0.5f) * (1.0f / 8388608.0f); }
+// = ((w >> 9) + 0.5) 2^-23, built in the mantissa: (1 + k 2^-23) - (1 - 2^-24) is exact (an odd multiple of 2^-24)
+__device__ inline float u01(uint32_t w) { return __uint_as_float((w >> 9) | 0x3f800000u) - 0.99999994f; }
 
 __device__ inline float wrap1(float x, float L, float invL) {
     x -= L * floorf(x * invL);
