@@ -167,7 +167,7 @@ def timed_blocks(torch, sim, stream, call, n_steps, block, flush):
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures of this command on the
 # configs[1] workload (profiles/r1_final_README.md); other workloads have no capture: null
-NCU_TRAFFIC_CFG1 = {"update": 9.68e6, "pair": 8.00e6, "build": 6.03e6}
+NCU_TRAFFIC_CFG1 = {"update": 9.67e6, "pair": 7.99e6, "build": 6.16e6}
 
 
 def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, props, peaks, traffic=None):
