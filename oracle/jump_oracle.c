@@ -19,6 +19,8 @@
  *   - rejection sampler for G~
  *   - C'J'AOAJ'C' scheme
  *   - JUMP-RESPA / BAOAB-RESPA
+ *   - JUMP-RESPA1 / BAOAB-RESPA1 (three levels) with the reciprocal Ewald sum as the slow
+ *     many-body force F_{0,1}                      P:L145, P:L509-511, P:L325 (R-21)
  *
  * Parity pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer
  * vectors; closed forms of Theta and of the G~ CDF/mean; chi end conditions and
@@ -111,7 +113,11 @@ typedef struct {
     double *x_build;
     /* gradient pieces, kcal/mol/A */
     double *f_bond, *f_nb, *f0, *f_long;
-    int64_t step, outer;
+    int64_t step, outer, outer1;
+    /* reciprocal Ewald sum (R-21): half-space vectors n = (nx, ny, nz), k = 2 pi n / box */
+    int nk;
+    int *kn;
+    double *f_slow;
     /* log + stats */
     orc_event *ev;
     int64_t n_ev, cap_ev;
@@ -543,7 +549,9 @@ static void compute_full(orc_ctx *c, double *out) { /* BAOAB comparator: unsplit
     pairs_accumulate(c, W_FULL, W_FULL, 0, out);
 }
 
-/* which: 0 F0, 1 full, 2 long, 3 bonded, 4 short non-bonded; brute != 0 -> O(N^2) sweep */
+static double slow_accumulate(const orc_ctx *c, double *out);
+/* which: 0 F0, 1 full, 2 long, 3 bonded, 4 short non-bonded, 5 slow (reciprocal Ewald + exclusion correction, R-21);
+ * brute != 0 -> O(N^2) sweep */
 void orc_forces(orc_ctx *c, int which, int brute, double *out) {
     int wC, wLJ;
     memset(out, 0, sizeof(double) * 3 * c->n);
@@ -552,6 +560,7 @@ void orc_forces(orc_ctx *c, int which, int brute, double *out) {
     else if (which == 2) { long_modes(c, &wC, &wLJ); pairs_accumulate(c, wC, wLJ, brute, out); }
     else if (which == 3) bonded_accumulate(c, out);
     else if (which == 4) { f0_modes(c, &wC, &wLJ); pairs_accumulate(c, wC, wLJ, brute, out); }
+    else if (which == 5) slow_accumulate(c, out);
 }
 /* which as above; returns potential energy in kcal/mol */
 double orc_potential(orc_ctx *c, int which) {
@@ -563,6 +572,7 @@ double orc_potential(orc_ctx *c, int which) {
     else if (which == 2) { long_modes(c, &wC, &wLJ); e = pairs_accumulate(c, wC, wLJ, 0, tmp); }
     else if (which == 3) e = bonded_accumulate(c, tmp);
     else if (which == 4) { f0_modes(c, &wC, &wLJ); e = pairs_accumulate(c, wC, wLJ, 0, tmp); }
+    else if (which == 5) e = slow_accumulate(c, tmp);
     free(tmp);
     return e;
 }
@@ -976,6 +986,99 @@ static void aoa_and_lists(orc_ctx *c) {
 }
 
 /* ------------------------------------------------------------------ */
+/* Reciprocal part of the Ewald sum ("Ewald summation"; the paper's SPME is an FFT approximation of exactly */
+/* this sum and is out of scope: here the sum itself, as the slow many-body force F_{0,1} of P:L137-145, R-21).   */
+/*   U_rec  = (C / 2V) sum_{k != 0} (4 pi / k^2) exp(-k^2 / 4 alpha^2) |S(k)|^2,  S(k) = sum_j q_j exp(i k.x_j),   */
+/*            k = 2 pi (nx/Lx, ny/Ly, nz/Lz), all |k| <= k_cut; k and -k give the same term: sum over a half space. */
+/*   U_self = -C alpha / sqrt(pi) sum_i q_i^2 (constant)                                                           */
+/*   U_excl = -sum_{excluded pairs i<j} C q_i q_j erf(alpha r_ij) / r_ij: the reciprocal sum contains every pair,   */
+/*            also those that R-9 excludes from the direct sum; their smooth part is taken out again.               */
+/* ------------------------------------------------------------------ */
+void orc_ewald_setup(orc_ctx *c, double k_cut) {
+    free(c->kn); c->kn = NULL; c->nk = 0;
+    if (!(c->alpha > 0.0)) return;
+    if (!(k_cut > 0.0)) k_cut = 8.0 * c->alpha; /* exp(-k^2/4 alpha^2) = e^-16 = 1.1e-7, the size of erfc(3.8) (R-2) */
+    int nmax[3];
+    for (int d = 0; d < 3; ++d) nmax[d] = (int)floor(k_cut * c->p.box[d] / (2.0 * ORC_PI));
+    for (int pass = 0; pass < 2; ++pass) {
+        int cnt = 0;
+        for (int nx = 0; nx <= nmax[0]; ++nx)
+            for (int ny = (nx == 0 ? 0 : -nmax[1]); ny <= nmax[1]; ++ny)
+                for (int nz = ((nx == 0 && ny == 0) ? 1 : -nmax[2]); nz <= nmax[2]; ++nz) {
+                    double kx = 2.0 * ORC_PI * nx / c->p.box[0], ky = 2.0 * ORC_PI * ny / c->p.box[1], kz = 2.0 * ORC_PI * nz / c->p.box[2];
+                    if (kx * kx + ky * ky + kz * kz > k_cut * k_cut) continue;
+                    if (pass) { c->kn[3 * cnt] = nx; c->kn[3 * cnt + 1] = ny; c->kn[3 * cnt + 2] = nz; }
+                    ++cnt;
+                }
+        if (!pass) { c->nk = cnt; c->kn = malloc(sizeof(int) * 3 * (cnt > 0 ? cnt : 1)); }
+    }
+}
+int orc_ewald_nk(const orc_ctx *c) { return c->nk; }
+/* adds grad (U_rec + U_excl) to out (kcal/mol/A), returns U_rec + U_self + U_excl (kcal/mol) */
+static double slow_accumulate(const orc_ctx *c, double *out) {
+    const int n = c->n, nk = c->nk;
+    const double V = c->p.box[0] * c->p.box[1] * c->p.box[2];
+    double e = 0.0;
+    double *Sr = malloc(sizeof(double) * (nk > 0 ? nk : 1)), *Si = malloc(sizeof(double) * (nk > 0 ? nk : 1));
+#pragma omp parallel for schedule(static)
+    for (int m = 0; m < nk; ++m) {
+        const double kx = 2.0 * ORC_PI * c->kn[3 * m] / c->p.box[0], ky = 2.0 * ORC_PI * c->kn[3 * m + 1] / c->p.box[1],
+                     kz = 2.0 * ORC_PI * c->kn[3 * m + 2] / c->p.box[2];
+        double sr = 0.0, si = 0.0;
+        for (int j = 0; j < n; ++j) {
+            const double th = kx * c->x[3 * j] + ky * c->x[3 * j + 1] + kz * c->x[3 * j + 2];
+            sr += c->q[j] * cos(th); si += c->q[j] * sin(th);
+        }
+        Sr[m] = sr; Si[m] = si;
+    }
+    for (int m = 0; m < nk; ++m) {
+        const double kx = 2.0 * ORC_PI * c->kn[3 * m] / c->p.box[0], ky = 2.0 * ORC_PI * c->kn[3 * m + 1] / c->p.box[1],
+                     kz = 2.0 * ORC_PI * c->kn[3 * m + 2] / c->p.box[2];
+        const double k2 = kx * kx + ky * ky + kz * kz;
+        /* half space: twice the (1/2V) term */
+        e += (ORC_COULOMB / V) * (4.0 * ORC_PI / k2) * exp(-k2 / (4.0 * c->alpha * c->alpha)) * (Sr[m] * Sr[m] + Si[m] * Si[m]);
+    }
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < n; ++i) {
+        double g[3] = {0, 0, 0};
+        for (int m = 0; m < nk; ++m) {
+            const double kx = 2.0 * ORC_PI * c->kn[3 * m] / c->p.box[0], ky = 2.0 * ORC_PI * c->kn[3 * m + 1] / c->p.box[1],
+                         kz = 2.0 * ORC_PI * c->kn[3 * m + 2] / c->p.box[2];
+            const double k2 = kx * kx + ky * ky + kz * kz;
+            const double A = (ORC_COULOMB / V) * (4.0 * ORC_PI / k2) * exp(-k2 / (4.0 * c->alpha * c->alpha));
+            const double th = kx * c->x[3 * i] + ky * c->x[3 * i + 1] + kz * c->x[3 * i + 2];
+            /* d|S|^2/dx_i = 2 q_i k (S_i cos th - S_r sin th) */
+            const double t = 2.0 * A * c->q[i] * (Si[m] * cos(th) - Sr[m] * sin(th));
+            g[0] += t * kx; g[1] += t * ky; g[2] += t * kz;
+        }
+        for (int d = 0; d < 3; ++d) out[3 * i + d] += g[d];
+    }
+    free(Sr); free(Si);
+    if (nk > 0) {
+        for (int i = 0; i < n; ++i) e -= ORC_COULOMB * c->alpha / sqrt(ORC_PI) * c->q[i] * c->q[i];
+        if (c->excl_ptr)
+            for (int i = 0; i < n; ++i)
+                for (int t = c->excl_ptr[i]; t < c->excl_ptr[i + 1]; ++t) {
+                    const int j = c->excl_idx[t];
+                    if (j <= i) continue;
+                    double d[3];
+                    min_image(c, &c->x[3 * i], &c->x[3 * j], d);
+                    const double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]), qq = ORC_COULOMB * c->q[i] * c->q[j];
+                    const double ar = c->alpha * r;
+                    e -= qq * erf(ar) / r;
+                    /* d/dr [-qq erf(alpha r)/r] = -qq [ (2 alpha/sqrt pi) exp(-alpha^2 r^2) / r - erf(alpha r) / r^2 ] */
+                    const double du = -qq * (2.0 * c->alpha / sqrt(ORC_PI) * exp(-ar * ar) / r - erf(ar) / (r * r));
+                    for (int k = 0; k < 3; ++k) { out[3 * i + k] += du * d[k] / r; out[3 * j + k] -= du * d[k] / r; }
+                }
+    }
+    return e;
+}
+static void compute_slow(orc_ctx *c) {
+    memset(c->f_slow, 0, sizeof(double) * 3 * c->n);
+    slow_accumulate(c, c->f_slow);
+}
+
+/* ------------------------------------------------------------------ */
 /* public steps                                                        */
 /* ------------------------------------------------------------------ */
 /* C'J'AOAJ'C' */
@@ -1013,8 +1116,9 @@ void orc_baoab_step(orc_ctx *c, int nsteps) {
     free(f);
     compute_f0(c);
 }
-/* JUMP-RESPA / BAOAB-RESPA (R-12) */
-void orc_jump_respa_step(orc_ctx *c, int nouter) {
+/* JUMP-RESPA / BAOAB-RESPA (R-12).  long_in_outer: the comparator's kick carries the long pair gradient
+ * (two-level BAOAB-RESPA); 0 when a third level carries it (BAOAB-RESPA1). */
+static void respa_outer_steps(orc_ctx *c, int nouter, int long_in_outer) {
     const int n = c->p.n_inner;
     const double D = n * c->dt;
     const int paper = (c->p.flags & ORC_F_RESPA_PAPER) != 0, cmp = (c->p.flags & ORC_F_RESPA_COMPARATOR) != 0;
@@ -1032,8 +1136,8 @@ void orc_jump_respa_step(orc_ctx *c, int nouter) {
                 if (paper) compute_f0(c); /* short non-bonded at the new x for the closing outer phase */
             }
             if (cmp) {
-                compute_long(c);
-                for (int k = 0; k < 3 * c->n; ++k) fout[k] = c->f_long[k] + (paper ? c->f_nb[k] : 0.0);
+                if (long_in_outer) compute_long(c);
+                for (int k = 0; k < 3 * c->n; ++k) fout[k] = (long_in_outer ? c->f_long[k] : 0.0) + (paper ? c->f_nb[k] : 0.0);
                 phase_B(c, 0.5 * D, fout);
             } else {
                 const double *grad = paper ? c->f_nb : NULL;
@@ -1044,6 +1148,34 @@ void orc_jump_respa_step(orc_ctx *c, int nouter) {
         c->outer++;
     }
     free(fout);
+}
+void orc_jump_respa_step(orc_ctx *c, int nouter) { respa_outer_steps(c, nouter, 1); }
+
+/* JUMP-RESPA1 / BAOAB-RESPA1 ("can itself be iterated"; R-21): three levels delta, kappa = m delta
+ * (m = n_inner), Delta = n_mid kappa.  delta: intramolecular; kappa: short-range non-bonded and the jumps -- the
+ * "paper" placement of the two-level driver above; Delta: the slow many-body force F_{0,1} = grad(U_rec + U_excl),
+ *   v <- v - (Delta/2) M^-1 F_{0,1}(x);  n_mid x [middle step of size kappa];  v <- v - (Delta/2) M^-1 F_{0,1}(x).
+ * Comparator (ORC_F_RESPA_COMPARATOR): the long pair gradient rides with F_{0,1} in the outermost kick
+ * and the middle level kicks with the short non-bonded gradient only. */
+void orc_jump_respa1_step(orc_ctx *c, int nouter, int n_mid) {
+    const int cmp = (c->p.flags & ORC_F_RESPA_COMPARATOR) != 0;
+    const uint32_t keep = c->p.flags;
+    const double D = (double)n_mid * c->p.n_inner * c->dt;
+    if (!c->f_slow) c->f_slow = calloc(3 * c->n, sizeof(double));
+    double *fo = malloc(sizeof(double) * 3 * c->n);
+    c->p.flags |= ORC_F_RESPA_PAPER;
+    for (int o = 0; o < nouter; ++o) {
+        for (int half = 0; half < 2; ++half) {
+            if (half == 1) respa_outer_steps(c, n_mid, 0);
+            compute_slow(c);
+            if (cmp) compute_long(c);
+            for (int k = 0; k < 3 * c->n; ++k) fo[k] = c->f_slow[k] + (cmp ? c->f_long[k] : 0.0);
+            phase_B(c, 0.5 * D, fo);
+        }
+        c->outer1++;
+    }
+    c->p.flags = keep;
+    free(fo);
 }
 
 /* ------------------------------------------------------------------ */
@@ -1110,7 +1242,7 @@ void orc_free(orc_ctx *c) {
     free(c->bij); free(c->bk); free(c->br0); free(c->aijk); free(c->ak); free(c->at0);
     free(c->excl_ptr); free(c->excl_idx); free(c->sbm); free(c->x_build);
     free(c->ptrM); free(c->idxM); free(c->ptrL); free(c->idxL); free(c->ptrV); free(c->idxV);
-    free(c->f_bond); free(c->f_nb); free(c->f0); free(c->f_long); free(c->ev);
+    free(c->f_bond); free(c->f_nb); free(c->f0); free(c->f_long); free(c->ev); free(c->kn); free(c->f_slow);
     free(c);
 }
 /* which: 0 wrapped x, 1 v, 2 unwrapped x */

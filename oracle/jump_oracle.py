@@ -104,6 +104,10 @@ def lib():
         L.orc_set_eps.argtypes = [C.c_void_p, C.c_double]
         L.orc_scale_bounds.argtypes = [C.c_void_p, C.c_double]
         L.orc_jump_half.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_int64]
+        L.orc_ewald_setup.argtypes = [C.c_void_p, C.c_double]
+        L.orc_ewald_nk.argtypes = [C.c_void_p]
+        L.orc_ewald_nk.restype = C.c_int
+        L.orc_jump_respa1_step.argtypes = [C.c_void_p, C.c_int, C.c_int]
         L.orc_fij.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_int, dp]
         L.orc_fij.restype = C.c_double
         L.orc_num_threads.restype = C.c_int
@@ -194,6 +198,15 @@ class Oracle:
 
     def jump_respa_step(self, n=1):
         lib().orc_jump_respa_step(self._h, int(n))
+
+    def ewald_setup(self, k_cut=0.0):
+        """Reciprocal vectors |k| <= k_cut (default 8 alpha) of the slow force of JUMP-RESPA1 (R-21); returns their number."""
+        lib().orc_ewald_setup(self._h, float(k_cut))
+        return lib().orc_ewald_nk(self._h)
+
+    def jump_respa1_step(self, n=1, n_mid=3):
+        """Three-level JUMP-RESPA1 / BAOAB-RESPA1: Delta = n_mid * n_inner * dt."""
+        lib().orc_jump_respa1_step(self._h, int(n), int(n_mid))
 
     def jump_half(self, H_ps, with_accel=True, step=0):
         lib().orc_jump_half(self._h, float(H_ps), int(bool(with_accel)), int(step))

@@ -656,3 +656,104 @@ def test_pair_histogram_lattice_and_ideal_gas():
     edges = np.linspace(0, 8.0, 17)
     ideal = 0.5 * M * (M - 1) / box ** 3 * 4 / 3 * np.pi * (edges[1:] ** 3 - edges[:-1] ** 3)
     assert np.abs(h[2:] / ideal[2:] - 1).max() < 5 / np.sqrt(ideal[2:].min())
+
+
+# ---------------------------------------------------------------- NEXT-2: reciprocal Ewald sum as F_{0,1}, JUMP-RESPA1 (R-21)
+def _rock_salt(cells=2, d=1.0):
+    """(2 cells)^3 rock-salt lattice of unit charges, nearest-neighbour distance d."""
+    m = 2 * cells
+    g = np.array([(i, j, k) for i in range(m) for j in range(m) for k in range(m)])
+    n = len(g)
+    z = np.zeros(0)
+    return dict(n_atoms=n, box=m * d, pos=(g + 0.25) * d, vel=np.zeros((n, 3)), mass=np.full(n, 20.0),
+                charge=np.where(g.sum(1) % 2 == 0, 1.0, -1.0), lj_sigma=np.ones(n), lj_eps=np.zeros(n),
+                bond_ij=np.zeros((0, 2), dtype=np.int32), bond_k=z, bond_r0=z,
+                angle_ijk=np.zeros((0, 3), dtype=np.int32), angle_k=z, angle_t0=z,
+                excl_ptr=np.zeros(n + 1, dtype=np.int32), excl_idx=np.zeros(0, dtype=np.int32))
+
+
+def test_ewald_sum_gives_the_madelung_constant_of_rock_salt():
+    """Direct part (erfc, minimum image to r_long) + reciprocal part + self term of the Ewald sum of a
+    rock-salt lattice = -M C q^2 / d per ion pair with the textbook Madelung constant M = 1.7475645946: pins the
+    prefactor, the half-space sum, the k-vectors and the alpha convention of the slow force against the direct one."""
+    sysd = _rock_salt()
+    n = sysd["n_atoms"]
+    o = jo.Oracle(sysd, r_short=1.2, r_long=2.0, r_switch=0.2, r_mid=1.6, skin=0.0, flags=0)   # alpha = 3.8 / r_long
+    nk = o.ewald_setup(12.0 * 1.9)        # e^{-36}: the reciprocal tail is far below the erfc(3.8) = 8e-8 of the direct one
+    assert nk > 1000
+    e = o.potential(1) + o.potential(5)
+    assert abs(e / (-(n / 2) * COUL * 1.7475645946331822) - 1.0) < 2e-7
+    f = o.forces(5)
+    assert np.abs(f).max() < 1e-9 * COUL          # every ion is a centre of symmetry
+
+
+def test_slow_force_is_the_gradient_of_reciprocal_plus_exclusion_energy(cfg0):
+    """Finite differences of U_rec + U_excl (R-21) on the 648-atom water box; sum of the gradient = 0 (translation
+    invariance); the exclusion correction alone against its closed form -C q_i q_j erf(alpha r)/r on one molecule."""
+    sysd, run = cfg0
+    o = jo.Oracle(sysd, **run)
+    assert o.ewald_setup(5.0 * 3.8 / 9.0) > 100    # a short k list keeps the test fast; the identity holds for any list
+    g = o.forces(5)
+    assert np.abs(g.sum(0)).max() < 1e-9 * np.abs(g).max() * len(g)
+    x0 = o.pos
+    h = 1e-5
+    for (i, k) in ((0, 0), (1, 2), (5, 1), (301, 0)):
+        xp, xm = x0.copy(), x0.copy()
+        xp[i, k] += h; xm[i, k] -= h
+        o.set_state(pos=xp, rebuild=False); ep = o.potential(5)
+        o.set_state(pos=xm, rebuild=False); em = o.potential(5)
+        assert abs((ep - em) / (2 * h) - g[i, k]) < 1e-6 * max(1.0, abs(g[i, k]))
+    # one water molecule alone, no reciprocal vectors at all (k_cut below 2 pi / box): only the exclusion correction is left
+    one = dict(sysd, n_atoms=3, **{k: sysd[k][:3] for k in ("pos", "vel", "mass", "charge", "lj_sigma", "lj_eps")},
+               bond_ij=sysd["bond_ij"][:2], bond_k=sysd["bond_k"][:2], bond_r0=sysd["bond_r0"][:2],
+               angle_ijk=sysd["angle_ijk"][:1], angle_k=sysd["angle_k"][:1], angle_t0=sysd["angle_t0"][:1],
+               excl_ptr=sysd["excl_ptr"][:4], excl_idx=sysd["excl_idx"][:sysd["excl_ptr"][3]])
+    assert np.all(one["excl_idx"] < 3)
+    o1 = jo.Oracle(one, **run)
+    assert o1.ewald_setup(0.9 * 2 * math.pi / sysd["box"]) == 0
+    assert o1.potential(5) == 0.0                                    # no reciprocal vector: the slow force is switched off
+    assert o1.ewald_setup(1.01 * 2 * math.pi / sysd["box"]) == 3     # the three shortest half-space vectors
+    alpha = 3.8 / run["r_long"]
+    q, x = one["charge"], one["pos"]
+    excl = sum(-COUL * q[i] * q[j] * special.erf(alpha * np.linalg.norm(x[i] - x[j])) / np.linalg.norm(x[i] - x[j])
+               for i, j in ((0, 1), (0, 2), (1, 2)))
+    self_e = -COUL * alpha / math.sqrt(math.pi) * (q ** 2).sum()
+    V = sysd["box"] ** 3
+    rec = 0.0
+    for d in range(3):
+        k = 2 * math.pi / sysd["box"]
+        S = (q * np.exp(1j * k * x[:, d])).sum()
+        rec += COUL / V * 4 * math.pi / k ** 2 * math.exp(-k ** 2 / (4 * alpha ** 2)) * abs(S) ** 2
+    assert abs(o1.potential(5) - (excl + self_e + rec)) < 1e-10 * abs(excl)
+
+
+def test_respa1_reductions_and_energy_conservation(relaxed_small):
+    """JUMP-RESPA1 (R-21).  (i) Without charges the slow force vanishes and the three-level scheme is
+    the two-level one (R-12, paper placement) run n_mid times, bit for bit.  (ii) BAOAB-RESPA1 (comparator) at gamma = 0
+    conserves K + U_direct + U_rec + U_excl with an error of second order in the time steps."""
+    sysd, run = relaxed_small
+    neutral = dict(sysd, charge=np.zeros_like(sysd["charge"]))
+    a = jo.Oracle(neutral, **dict(run, flags=2, n_inner=2))
+    b = jo.Oracle(neutral, **dict(run, flags=2 | 8, n_inner=2))
+    assert a.ewald_setup() > 0
+    a.jump_respa1_step(2, 3); b.jump_respa_step(6)
+    assert np.array_equal(a.pos, b.pos) and np.array_equal(a.vel, b.vel)
+    drift = []
+    for dt in (0.25, 0.125):
+        o = jo.Oracle(sysd, **dict(run, dt_fs=dt, gamma_per_ps=0.0, flags=16, n_inner=2))
+        o.ewald_setup()
+        e = []
+        for _ in range(int(20 / (4 * dt))):
+            o.jump_respa1_step(1, 2)
+            e.append(o.kinetic() + o.potential(1) + o.potential(5))
+        drift.append(np.std(e))
+    assert drift[0] < 0.05 * 192 * KB * 300
+    assert 2.5 < drift[0] / drift[1] < 6.5
+    # the jumps of the middle level: proposals per unit time do not depend on how the levels are split (P:L507, L511)
+    rate = []
+    for n_inner, n_mid in ((2, 2), (4, 1)):
+        o = jo.Oracle(sysd, **dict(run, flags=1, n_inner=n_inner))
+        o.ewald_setup(3.0 * 3.8 / run["r_long"])
+        o.jump_respa1_step(40 // (n_inner * n_mid), n_mid)
+        rate.append(o.stats()["proposals"] / 40.0)
+    assert abs(rate[0] / rate[1] - 1.0) < 0.1
