@@ -103,8 +103,23 @@ int baoab_step(jump_ctx *c, int32_t n_steps);
 /* n_outer outer steps of JUMP-RESPA, or BAOAB-RESPA with JUMP_F_RESPA_COMPARATOR (R-12). */
 int jump_respa_step(jump_ctx *c, int32_t n_outer);
 
+/* NEXT-2 (R-21): the reciprocal part of the Ewald sum as the slow many-body force
+ * F_{0,1} = grad(U_rec + U_excl), U_rec = (C/2V) sum_{k != 0, |k| <= k_cut} (4 pi/k^2) exp(-k^2/4 alpha^2) |S(k)|^2,
+ * U_excl = -sum_{excluded pairs} C q_i q_j erf(alpha r)/r.  jump_ewald_setup builds the half-space k list on the host
+ * (k_cut in 1/A; <= 0: 8 alpha), uploads it and allocates the scratch; *n_k (host, may be NULL) receives the number of
+ * vectors.  Needs ewald_alpha != 0; at most 511 vectors per dimension (JUMP_E_ARG otherwise).  Synchronises. */
+int jump_ewald_setup(jump_ctx *c, double k_cut, int32_t *n_k);
+/* n_outer outer steps of the three-level JUMP-RESPA1: delta = dt_fs (bonded), kappa = n_inner delta
+ * (short non-bonded + the jumps), Delta = n_mid kappa (kick by F_{0,1} on both sides); with JUMP_F_RESPA_COMPARATOR
+ * BAOAB-RESPA1: the middle level kicks with the short non-bonded gradient, the long pair gradient rides with F_{0,1}
+ * (P:L511).  n_mid >= 1.  Asynchronous; JUMP_E_ARG before jump_ewald_setup. */
+int jump_respa1_step(jump_ctx *c, int32_t n_outer, int32_t n_mid);
+/* U_rec + U_self + U_excl at the current positions, kcal/mol (host double); 0 with no reciprocal vector.  Synchronises. */
+int jump_get_slow_energy(jump_ctx *c, double *e_slow);
+
 /* Gradient pieces at the current positions, original atom order, kcal/mol/A, into d_out (n x 3).
- * which: 0 F0 (bonded + short non-bonded), 1 full (unsplit to r_long), 2 long, 3 bonded, 4 short non-bonded. */
+ * which: 0 F0 (bonded + short non-bonded), 1 full (unsplit to r_long), 2 long, 3 bonded, 4 short non-bonded,
+ * 5 slow (reciprocal Ewald + exclusion correction, after jump_ewald_setup). */
 int jump_get_forces(jump_ctx *c, int32_t which, float *d_out);
 /* Kinetic energy and the full unsplit potential to r_long, kcal/mol (host doubles). */
 int jump_get_energy(jump_ctx *c, double *e_kin, double *e_pot_full);

@@ -21,7 +21,8 @@ ERRORS = {-1: "bad argument", -2: "CUDA error", -3: "row/event overflow", -4: "t
 EXPORTS = ["jump_init", "jump_step", "baoab_step", "jump_respa_step", "jump_get_forces", "jump_get_energy",
            "jump_get_stats", "jump_reset_stats", "jump_get_events", "jump_clear_events", "jump_get_row", "jump_get_images", "jump_rdf_accumulate",
            "jump_get_bounds", "jump_refresh", "jump_refresh_lazy", "jump_half", "jump_sync", "jump_get_step", "jump_get_launches",
-           "jump_last_error", "jump_free", "jump_set_profiling", "jump_get_profile", "jump_count_pairs"]
+           "jump_last_error", "jump_free", "jump_set_profiling", "jump_get_profile", "jump_count_pairs",
+           "jump_ewald_setup", "jump_respa1_step", "jump_get_slow_energy"]
 
 
 class jump_params(C.Structure):
@@ -74,6 +75,9 @@ def lib():
         L.jump_step.argtypes = [vp, i32]
         L.baoab_step.argtypes = [vp, i32]
         L.jump_respa_step.argtypes = [vp, i32]
+        L.jump_ewald_setup.argtypes = [vp, C.c_double, C.POINTER(C.c_int32)]
+        L.jump_respa1_step.argtypes = [vp, i32, i32]
+        L.jump_get_slow_energy.argtypes = [vp, C.POINTER(C.c_double)]
         L.jump_get_forces.argtypes = [vp, i32, vp]
         L.jump_get_energy.argtypes = [vp, dp, dp]
         L.jump_get_stats.argtypes = [vp, C.POINTER(jump_stats)]
@@ -181,6 +185,20 @@ class JumpSim:
 
     def jump_respa_step(self, n=1):
         self._check(self._L.jump_respa_step(self._h, int(n)), "jump_respa_step")
+
+    def ewald_setup(self, k_cut=0.0):
+        """Reciprocal vectors |k| <= k_cut (default 8 alpha) of the slow force of JUMP-RESPA1; returns their number."""
+        nk = C.c_int32(0)
+        self._check(self._L.jump_ewald_setup(self._h, float(k_cut), C.byref(nk)), "jump_ewald_setup")
+        return int(nk.value)
+
+    def jump_respa1_step(self, n=1, n_mid=3):
+        self._check(self._L.jump_respa1_step(self._h, int(n), int(n_mid)), "jump_respa1_step")
+
+    def slow_energy(self):
+        e = C.c_double(0.0)
+        self._check(self._L.jump_get_slow_energy(self._h, C.byref(e)), "jump_get_slow_energy")
+        return float(e.value)
 
     def jump_half(self, H_ps, with_accel=True, step=0):
         self._check(self._L.jump_half(self._h, float(H_ps), int(bool(with_accel)), int(step)), "jump_half")

@@ -36,6 +36,13 @@ struct jump_ctx {
     bool row_used[N_ROWS];   // read since the last sort: rebuilt eagerly at the next one (others lazily, on demand)
     bool f0_valid;           // c->f0 / fnb / fbond hold F0 at the current positions
     float4 *fnb, *fbond, *f0, *ftmp, *ftmp2;
+    // reciprocal Ewald sum, the slow force of JUMP-RESPA1 (R-21): set up by jump_ewald_setup
+    EwaldArgs ew;
+    float4 *fslow;
+    double *ew_sum;
+    double q2sum;            // sum of q_i^2 (self term)
+    bool slow_valid;         // fslow holds grad(U_rec + U_excl) at the current positions, in the current sorted order
+    int64_t outer1;
 
     double *ke;
     unsigned long long *pair_count;   // scratch of jump_count_pairs
@@ -224,6 +231,7 @@ static int resort_and_build(jump_ctx *c) {
     bool want[N_ROWS];
     for (int k = 0; k < N_ROWS; ++k) { c->row_fresh[k] = false; want[k] = c->row_used[k]; c->row_used[k] = false; }
     c->rebuilds++;
+    c->slow_valid = false;   // (sorted order changed)
     return build_rows(c, want);
 }
 
@@ -385,6 +393,7 @@ static int run_update(jump_ctx *c, const Phase &p0, GradRef g0, const Phase &p1,
     if (aoa) {
         std::swap(c->xs, c->xs_nxt);
         c->f0_valid = false;
+        c->slow_valid = false;
         c->step++;
         if (c->p.nlist_every > 0 && c->step % c->p.nlist_every == 0) return resort_and_build(c);
     }
@@ -448,11 +457,13 @@ extern "C" int baoab_step(jump_ctx *c, int32_t n_steps) {
     return writeback(c);  // F0 is recomputed on demand (f0_valid)
 }
 
-extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
-    if (!c || n_outer < 0) return JUMP_E_ARG;
+// n_outer outer steps of the two-level scheme (R-12).  long_in_outer: the comparator's kick carries the long pair
+// gradient (two-level BAOAB-RESPA); false when a third level carries it (BAOAB-RESPA1).  paper: bonded inner,
+// short non-bonded (+ jumps) outer.
+static int respa_outer_steps(jump_ctx *c, int n_outer, bool paper, bool long_in_outer) {
     const int n = c->p.n_inner;
     const double D = n * c->dt, H = 0.5 * c->dt;
-    const bool paper = (c->p.flags & JUMP_F_RESPA_PAPER) != 0, cmp = (c->p.flags & JUMP_F_RESPA_COMPARATOR) != 0;
+    const bool cmp = (c->p.flags & JUMP_F_RESPA_COMPARATOR) != 0;
     int r = ensure_f0(c);
     if (r) return r;
     for (int o = 0; o < n_outer; ++o) {
@@ -472,15 +483,20 @@ extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
             }
             if (cmp) {  // BAOAB-RESPA: v <- v - (Delta/2) M^-1 F_long
                 float4 *fl = half == 0 ? c->ftmp : c->ftmp2;
-                r = compute_long(c, fl);
-                if (r) return r;
+                int acc = 0;
+                if (long_in_outer) {
+                    r = compute_long(c, fl);
+                    if (r) return r;
+                    acc = 1;
+                }
                 if (paper) {  // + short non-bonded
-                    r = pair(c, ROW_S, W_SHORT, lj_jumps(c) ? W_SHORT : W_FULL, fl, 1, false);
+                    r = pair(c, ROW_S, W_SHORT, lj_jumps(c) ? W_SHORT : W_FULL, fl, acc, false);
                     if (!r && !lj_jumps(c)) r = pair(c, ROW_W, W_NONE, W_FULL, fl, 1, false);
                     if (r) return r;
                     CK(cudaGetLastError());
+                    acc = 1;
                 }
-                outer[half] = ph_kick(0.5 * D);
+                outer[half] = acc ? ph_kick(0.5 * D) : ph_none();
                 gout[half] = gr(fl);
             } else {
                 gout[half] = gr(paper ? c->fnb : nullptr);
@@ -493,7 +509,113 @@ extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
         if (r) return r;
         c->outer++;
     }
+    return 0;
+}
+extern "C" int jump_respa_step(jump_ctx *c, int32_t n_outer) {
+    if (!c || n_outer < 0) return JUMP_E_ARG;
+    int r = respa_outer_steps(c, n_outer, (c->p.flags & JUMP_F_RESPA_PAPER) != 0, true);
+    if (r) return r;
     return writeback(c);
+}
+
+// ---- NEXT-2: reciprocal Ewald sum as the slow force, three-level JUMP-RESPA1 (R-21) ---------------------------
+extern "C" int jump_ewald_setup(jump_ctx *c, double k_cut, int32_t *n_k) {
+    if (!c) return JUMP_E_ARG;
+    if (!(c->alpha > 0.0)) { c->err = "the reciprocal sum needs ewald_alpha > 0"; return JUMP_E_ARG; }
+    if (!(k_cut > 0.0)) k_cut = 8.0 * c->alpha;   // exp(-k^2/4 alpha^2) = e^-16 = 1.1e-7, the size of erfc(3.8) (R-2)
+    const double two_pi = 6.283185307179586476925;
+    const double V = c->p.box[0] * c->p.box[1] * c->p.box[2];
+    int nmax[3];
+    for (int d = 0; d < 3; ++d) {
+        nmax[d] = (int)std::floor(k_cut * c->p.box[d] / two_pi);
+        if (nmax[d] > 511) { c->err = "k_cut needs more than 511 reciprocal vectors per dimension"; return JUMP_E_ARG; }
+    }
+    std::vector<int> kp;
+    std::vector<double> cA;
+    for (int nx = 0; nx <= nmax[0]; ++nx)
+        for (int ny = (nx == 0 ? 0 : -nmax[1]); ny <= nmax[1]; ++ny)
+            for (int nz = ((nx == 0 && ny == 0) ? 1 : -nmax[2]); nz <= nmax[2]; ++nz) {
+                const double kx = two_pi * nx / c->p.box[0], ky = two_pi * ny / c->p.box[1], kz = two_pi * nz / c->p.box[2];
+                const double k2 = kx * kx + ky * ky + kz * kz;
+                if (k2 > k_cut * k_cut) continue;
+                kp.push_back(ewald_pack(nx, ny, nz));
+                cA.push_back((kCoulomb / V) * (4.0 * 3.14159265358979323846 / k2) * std::exp(-k2 / (4.0 * c->alpha * c->alpha)));
+            }
+    EwaldArgs e;
+    memset(&e, 0, sizeof e);
+    e.nk = (int)kp.size();
+    e.nch = std::max(1, std::min(16, c->n / 512));   // atom chunks of the structure-factor pass (more CTAs, fixed order)
+    e.alpha = c->alpha;
+    int r;
+    int *dk = nullptr;
+    double *dA = nullptr;
+    if ((r = dupload(c, &dk, kp)) || (r = dupload(c, &dA, cA))) return r;
+    e.kpack = dk; e.coefA = dA;
+    if ((r = dalloc(c, &e.part, (size_t)e.nch * e.nk)) || (r = dalloc(c, &e.W, (size_t)e.nk)) || (r = dalloc(c, &e.ek, (size_t)e.nk)))
+        return r;
+    if (!c->fslow && (r = dalloc(c, &c->fslow, (size_t)c->n))) return r;
+    if (!c->ew_sum && (r = dalloc(c, &c->ew_sum, 1))) return r;
+    std::vector<float4> hx;
+    if ((r = ddownload(c, hx, (const float4 *)c->xs, c->n))) return r;
+    c->q2sum = 0.0;
+    for (const float4 &v : hx) c->q2sum += (double)v.w * (double)v.w;
+    c->ew = e;
+    c->slow_valid = false;
+    if (n_k) *n_k = e.nk;
+    return 0;
+}
+static int compute_slow(jump_ctx *c) {
+    if (c->slow_valid) return 0;
+    if (c->ew.nk <= 0) {
+        if (!c->fslow) { c->err = "jump_ewald_setup has not been called"; return JUMP_E_ARG; }
+        CK(cudaMemsetAsync(c->fslow, 0, sizeof(float4) * c->n, c->st));   // no reciprocal vector: the slow force is off
+    } else {
+        launch_rec_force(c->m, c->ew, c->xs, c->xl, c->orig, c->sorted_of, c->excl_ptr, c->excl_idx, c->fslow, c->st, &c->launches);
+    }
+    CK(cudaGetLastError());
+    c->slow_valid = true;
+    return 0;
+}
+// Three levels delta, kappa = n_inner delta, Delta = n_mid kappa: the two-level scheme in its paper
+// placement between kicks by the slow gradient; comparator: the long pair gradient rides with it.
+extern "C" int jump_respa1_step(jump_ctx *c, int32_t n_outer, int32_t n_mid) {
+    if (!c || n_outer < 0 || n_mid < 1) return JUMP_E_ARG;
+    if (!c->fslow) { c->err = "jump_ewald_setup has not been called"; return JUMP_E_ARG; }
+    const bool cmp = (c->p.flags & JUMP_F_RESPA_COMPARATOR) != 0;
+    const double D = (double)n_mid * c->p.n_inner * c->dt;
+    int r = ensure_f0(c);
+    if (r) return r;
+    for (int o = 0; o < n_outer; ++o) {
+        for (int half = 0; half < 2; ++half) {
+            if (half == 1 && (r = respa_outer_steps(c, n_mid, true, false))) return r;
+            if ((r = compute_slow(c))) return r;
+            const float4 *fl = nullptr;
+            if (cmp) {
+                if ((r = compute_long(c, c->ftmp))) return r;
+                fl = c->ftmp;
+            }
+            if ((r = run_update(c, ph_kick(0.5 * D), gr(c->fslow, fl), ph_none(), gr(nullptr), false))) return r;
+        }
+        c->outer1++;
+    }
+    return writeback(c);
+}
+// U_rec + U_self + U_excl at the current positions, kcal/mol (0 when no reciprocal vector is set up)
+extern "C" int jump_get_slow_energy(jump_ctx *c, double *e_slow) {
+    if (!c || !e_slow) return JUMP_E_ARG;
+    *e_slow = 0.0;
+    if (c->ew.nk <= 0) return 0;
+    int r;
+    c->slow_valid = false;
+    if ((r = compute_slow(c))) return r;
+    launch_rec_energy(c->ew, c->ew_sum, c->st, &c->launches);
+    std::vector<double> h1;
+    std::vector<float4> hf;
+    if ((r = ddownload(c, h1, (const double *)c->ew_sum, 1)) || (r = ddownload(c, hf, (const float4 *)c->fslow, c->n))) return r;
+    double s = h1[0] - kCoulomb * c->alpha / std::sqrt(3.14159265358979323846) * c->q2sum;
+    for (const float4 &v : hf) s += (double)v.w;
+    *e_slow = s;
+    return poll_error(c);
 }
 
 extern "C" int jump_half(jump_ctx *c, double H_ps, int32_t with_accel, int64_t step) {
@@ -693,6 +815,9 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     c->pair_count = nullptr;
     c->moved_flag = nullptr;
     c->f0_valid = false;
+    c->slow_valid = false;
+    memset(&c->ew, 0, sizeof c->ew);
+    c->fslow = nullptr; c->ew_sum = nullptr; c->q2sum = 0.0; c->outer1 = 0;
     c->prof = false;
     for (int k = 0; k < 4; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     int r = init_impl(c, p, d_mass, d_charge, d_lj_sigma, d_lj_eps, n_bonds, d_bond_ij, d_bond_k, d_bond_r0, n_angles,
@@ -728,6 +853,7 @@ extern "C" int jump_get_forces(jump_ctx *c, int32_t which, float *d_out) {
         case 2: r = compute_long(c, c->ftmp); src = c->ftmp; break;
         case 3: r = bonded(c, nullptr, nullptr, c->fbond); src = c->fbond; break;
         case 4: r = compute_short_nb(c, c->fnb); src = c->fnb; break;
+        case 5: c->slow_valid = false; r = compute_slow(c); src = c->fslow; break;
         default: return JUMP_E_ARG;
     }
     if (r) return r;
@@ -863,6 +989,7 @@ extern "C" int jump_refresh_lazy(jump_ctx *c, int32_t *rebuilt) {
     int moved = 0;
     CK(cudaMemcpyAsync(&moved, c->moved_flag, sizeof(int), cudaMemcpyDeviceToHost, c->st));
     CK(cudaStreamSynchronize(c->st));
+    c->slow_valid = false;
     if (moved && (r = resort_and_build(c))) return r;
     if (rebuilt) *rebuilt = moved;
     if ((r = compute_f0(c))) return r;

@@ -38,6 +38,16 @@ struct UpdateArgs {
     long long event_cap;
 };
 
+struct EwaldArgs {   // reciprocal Ewald sum (ewald.cu, R-21)
+    int nk, nch;             // half-space k-vectors, atom chunks of the structure-factor pass
+    double alpha;
+    const int *kpack;        // [nk] packed (nx, ny, nz)
+    const double *coefA;     // [nk] A_k = (C/V)(4 pi/k^2) exp(-k^2/4 alpha^2), fp64 from the host
+    double2 *part;           // [nch][nk] structure-factor partials
+    double2 *W;              // [nk] 2 A_k S(k)
+    double *ek;              // [nk] A_k |S(k)|^2
+};
+
 void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches);
 void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS], float rmax_all, const int *cell_start,
                        const float4 *xs, const float4 *xl, const float2 *lj, const int *orig, const int *sorted_of,
@@ -63,5 +73,10 @@ int launch_rdf(const Model &m, const SortGrid &g, int lj_only, double r_max, dou
                const float4 *xs, const float2 *lj, unsigned long long *hist, cudaStream_t st, int64_t *launches);
 void launch_images(int n, const float4 *xl, const int *orig, int *out, cudaStream_t st, int64_t *launches);
 void launch_kinetic(int n, const float4 *vs, const float2 *mi, double *out, cudaStream_t st, int64_t *launches);
+void launch_rec_force(const Model &m, const EwaldArgs &e, const float4 *xs, const float4 *xl, const int *orig,
+                      const int *sorted_of, const int *excl_ptr, const int *excl_idx, float4 *out, cudaStream_t st,
+                      int64_t *launches);
+void launch_rec_energy(const EwaldArgs &e, double *out, cudaStream_t st, int64_t *launches);
+int ewald_pack(int nx, int ny, int nz);
 
 }  // namespace jb

@@ -527,3 +527,70 @@ def test_orthorhombic_box(jb, jo, case):
         d -= box * np.round(d / box)
         assert np.abs(d).max() <= X_TOL
     assert g.stats()["error"] == 0
+
+
+# ------------------------------------------------------------------------------------- NEXT-2: slow force, JUMP-RESPA1
+@pytest.mark.parametrize("cfg", [0, 3])
+def test_slow_force_reciprocal_ewald(jb, jo, cfg):
+    """R-21: grad(U_rec + U_excl) and the energy U_rec + U_self + U_excl against the oracle's plain double sum: 648-atom
+    water box with the default k_cut = 8 alpha (2 000 vectors, several tiles and a ragged tail in both passes), and the
+    23 558-atom solute box (heterogeneous charges, chain exclusions, 16 atom chunks) with a shorter list."""
+    sysd, run = wl.make_config(cfg)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    k_cut = 0.0 if cfg == 0 else 4.0 * 3.8 / run["r_long"]
+    nk = g.ewald_setup(k_cut)
+    assert nk == o.ewald_setup(k_cut) and nk > 1000
+    fo = o.forces(5)
+    err = rel_force_err(g.forces(5).cpu().numpy(), fo)
+    assert err <= F_TOL, err
+    assert g.slow_energy() == pytest.approx(o.potential(5), rel=2e-6)
+    if cfg == 0:   # after dynamics (sorted order changed, residuals xl non-zero)
+        g.jump_step(25); g.sync(); o.jump_step(25)
+        if not fragile(o):
+            assert rel_force_err(g.forces(5).cpu().numpy(), o.forces(5)) <= F_TOL
+
+
+@pytest.mark.parametrize("flags,n_inner,n_mid", [(3, 2, 3), (3 | 16, 2, 3), (1, 2, 2)])
+def test_respa1_three_levels(jb, jo, cfg0, flags, n_inner, n_mid):
+    """JUMP-RESPA1 (1 : 2 : 6 fs as in the paper's Table 2) and the BAOAB-RESPA1 comparator: event log
+    of the middle-level jumps and the trajectory against the oracle."""
+    sysd, run = cfg0
+    r = dict(run, flags=flags | jb.F_EVENT_LOG, n_inner=n_inner)
+    g, o = jb.JumpSim(sysd, **r), jo.Oracle(sysd, **r)
+    assert g.ewald_setup() == o.ewald_setup()
+    n_out = 3
+    g.jump_respa1_step(n_out, n_mid); g.sync(); o.jump_respa1_step(n_out, n_mid)
+    assert g.step == n_out * n_mid * n_inner == o.step
+    eg, eo = g.events(), o.events()
+    if flags & 16:
+        assert len(eg) == 0 == len(eo)
+    elif fragile(o):
+        keep_g, keep_o = eg["step"] < 2, eo["step"] < 2
+        check_events(eg[keep_g], eo[keep_o])
+        return
+    else:
+        check_events(eg, eo)
+        assert len(eo) > 1000
+    assert pos_err(g, o, sysd["box"]) <= X_TOL
+    assert np.abs(g.vel.cpu().numpy() - o.vel).max() < 5e-3
+
+
+def test_respa1_needs_setup_and_conserves_energy(jb, cfg0):
+    """jump_respa1_step before jump_ewald_setup is refused; BAOAB-RESPA1 at gamma = 0 conserves K + U_direct + U_rec +
+    U_excl to second order in the time steps (a wrong sign or factor of the slow kick would show as a drift)."""
+    sysd, run = cfg0
+    g = jb.JumpSim(sysd, **dict(run, flags=16, n_inner=2))
+    with pytest.raises(RuntimeError):
+        g.jump_respa1_step(1, 2)
+    out = []
+    for dt in (0.5, 0.25):
+        g = jb.JumpSim(sysd, **dict(run, flags=16, n_inner=2, dt_fs=dt, gamma_per_ps=0.0))
+        g.ewald_setup()
+        e = []
+        for _ in range(int(30 / (4 * dt))):
+            g.jump_respa1_step(1, 2)
+            ek, ep = g.energy()
+            e.append(ek + ep + g.slow_energy())
+        out.append(np.std(e))
+    assert out[0] < 0.02 * 648 * 0.6
+    assert out[1] < 0.5 * out[0]
