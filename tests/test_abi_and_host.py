@@ -23,7 +23,7 @@ def binding():
 def declared_symbols():
     txt = open(HEADER).read()
     txt = re.sub(r"/\*.*?\*/", "", txt, flags=re.S)
-    return sorted(set(re.findall(r"\b(jump_[a-z_]+|baoab_step)\s*\(", txt)))
+    return sorted(set(re.findall(r"\b(jump_[a-z0-9_]+|baoab_step)\s*\(", txt)))
 
 
 def test_library_exports_every_declared_symbol(binding):
