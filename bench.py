@@ -364,6 +364,40 @@ def main():
                     "proposals_per_atom_step": st_a["proposals"] / (n * Ka), "accepts_per_atom_step": st_a["accepts"] / (n * Ka),
                     "max_p": st_a["max_p"], "error": st_a["error"]}
 
+    # ---- NEXT-2: three-level JUMP-RESPA1 1:2:6 fs (the paper's Table 2 setting) against BAOAB-RESPA1 1:2:6, the
+    # reciprocal Ewald sum as the slow force (R-21), same box --------------------------------------------
+    respa1 = None
+    if not respa and rank == 0:
+        respa1 = {"levels_fs": [dt_fs, 2 * dt_fs, 6 * dt_fs],
+                  "what": "delta: bonded; kappa = 2 delta: short non-bonded + jumps (JUMP) or kick (BAOAB); Delta = 3 kappa: "
+                          "reciprocal Ewald sum + exclusion correction (+ long pair gradient for BAOAB-RESPA1, P:L511)"}
+        for name, fl in (("jump_respa1", 3 | 8), ("baoab_respa1", 3 | 8 | 16)):
+            with torch.cuda.stream(stream):
+                sim_r = jb.JumpSim(sysd, device=dev, stream=stream, **dict(run, flags=fl, n_inner=2))
+                sim_r.baoab_step(args.equil)
+                nk = sim_r.ewald_setup()
+                sim_r.jump_respa1_step(10, 3)
+                sim_r.sync()
+                Kr = max(min(K, 600) // 6, 1)
+                ms_r = timed_blocks(torch, sim_r, stream, lambda b: sim_r.jump_respa1_step(b, 3), Kr, 2, flush)
+                if name == "jump_respa1":   # the slow force alone (three kernels), per evaluation
+                    sim_r.forces(5)
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(stream)
+                    for _ in range(10):
+                        sim_r.forces(5)
+                    e1.record(stream)
+                    stream.synchronize()
+                    ms_s = e0.elapsed_time(e1) / 10
+                    respa1["slow_force"] = {"n_k": nk, "ms_per_evaluation": ms_s,
+                                            "terms_per_s": 2.0 * nk * n / (ms_s * 1e-3),
+                                            "what": "S(k) pass + force pass, n_k half-space vectors x n atoms x 2 sincos terms"}
+                err_r = sim_r.stats()["error"]
+                sim_r.close()
+            respa1[name] = {"ms_per_outer_step": ms_r / Kr, "ns_per_day": ns_per_day(Kr / (ms_r * 1e-3), 6 * dt_fs),
+                            "outer_steps": Kr, "error": err_r}
+        respa1["jump_vs_baoab"] = respa1["baoab_respa1"]["ms_per_outer_step"] / respa1["jump_respa1"]["ms_per_outer_step"]
+
     # ---- end to end through the public API with HOST buffers -------------------------------------------------
     with torch.cuda.stream(stream):
         Ke = min(K, 500)
@@ -419,6 +453,8 @@ def main():
                            "error": stats["error"]}}
         if adaptive is not None:
             line["jump_adaptive_eps"] = adaptive
+        if respa1 is not None:
+            line["jump_respa1"] = respa1
         if large is not None:
             line["roofline_large_box"] = large
         if cpu is not None:
