@@ -8,10 +8,15 @@
 //   d U_rec / d x_i = sum_half 2 A_k q_i k (Im S cos(k.x_i) - Re S sin(k.x_i)),  A_k = (C/V)(4 pi/k^2) exp(-k^2/4 alpha^2).
 //
 // The paper's SPME is an FFT approximation of this sum; the sum itself is evaluated here (O(N n_k): two passes of
-// independent sincos terms, ALU-bound, no tensor-core shape).  The phase k.x / 2 pi = n.(x/L) is formed in fp64 from
-// x = xs + xl and reduced to [-1/2, 1/2] before the fp32 sincospi: |n.(x/L)| reaches 30 and an fp32 phase would
-// carry 2e-6 cycles of error.  No floating-point atomics: structure-factor partials per atom chunk are written out
-// and added in a fixed order, the force of an atom is one warp's shuffle reduction -- bitwise deterministic.
+// independent sincos terms, ALU-bound, no tensor-core shape).  The phase k.x / 2 pi = n.(x/L) is formed in 32-bit
+// FIXED POINT: the scaled coordinate x/L in [0, 1) (from the fp64 position xs + xl) becomes an unsigned integer with
+// 2^32 = one cycle, and n.(x/L) mod 1 is then three wrapping integer multiply-adds -- the reduction to one period is
+// free and exact, the phase error is |n| 2^-33 <= 4e-9 cycles, and the fp64 multiply-adds, rint and the five 64-bit
+// conversions per term (a 16-per-clock pipe) of an fp64 phase are gone: that form of the loops ran 1.5 times slower.  The sines
+// and cosines are polynomials on [-pi/4, pi/4] after an integer quadrant reduction: fp64 in the structure-factor pass
+// (S(k) is the small remainder of N cancelling charges), fp32 in the force pass.
+// No floating-point atomics: structure-factor partials per atom chunk are written out and added in a fixed order, the
+// force of an atom is one warp's shuffle reduction -- bitwise deterministic.
 #include "launch.h"
 
 namespace jb {
@@ -23,17 +28,60 @@ __host__ __device__ inline int ew_pack(int nx, int ny, int nz) {
 __device__ inline void ew_unpack(int w, int &nx, int &ny, int &nz) {
     nx = (w & 1023) - EW_BIAS; ny = ((w >> 10) & 1023) - EW_BIAS; nz = ((w >> 20) & 1023) - EW_BIAS;
 }
-// cos and sin of 2 pi t for an fp64 phase t in cycles: fp32 sincospi of the reduced phase rounded to fp32, then one
-// first-order step over what the rounding dropped (up to 3e-8 cycles = 2e-7 in the sine: per-atom sums of thousands
-// of such terms cancel to a small force, and that error alone used the whole 1e-5 budget of R-16)
-__device__ inline void phase_sincos(double t, float &s, float &c) {
-    t -= rint(t);
-    const float tf = (float)t;
-    const float d = 6.2831853f * (float)(t - (double)tf);
-    float s0, c0;
-    sincospif(2.f * tf, &s0, &c0);
-    s = fmaf(d, c0, s0);
-    c = fmaf(-d, s0, c0);
+// scaled coordinate in [0, 1) -> 32-bit fixed point (wraps: 1.0 -> 0)
+__device__ inline unsigned fix_cycle(double s) { return (unsigned)(__double2ull_rn(s * 4294967296.0) & 0xffffffffull); }
+// cos and sin of 2 pi p / 2^32 for an integer phase p, with the whole range reduction in integers: q = nearest
+// quarter cycle, r = p - q 2^30 in [-2^29, 2^29) i.e. theta = 2 pi r / 2^32 in [-pi/4, pi/4); least-squares
+// polynomials in theta^2 made for this file (sin to 1e-8, cos to 2e-10 in exact arithmetic); the int -> fp32
+// conversion rounds r to 24 bits, at most 4.7e-8 rad.  fp32: the force pass.  (sincospif cost 35 instructions, this
+// costs 22: that pass is bound by instruction issue.)
+__device__ inline void phase_sincos(unsigned p, float &s, float &c) {
+    const unsigned q = (p + 0x20000000u) >> 30;
+    const int r = (int)(p - (q << 30));
+    const float th = 1.4629180792671596e-9f * (float)r;   // 2 pi / 2^32
+    const float t = th * th;
+    float sp = fmaf(t, -1.958794891834259e-4f, 8.332748897373676e-3f);
+    sp = fmaf(t, sp, -0.166666641831398f);
+    const float sn = fmaf(th * t, sp, th);
+    float cp = fmaf(t, 2.4463912268402055e-5f, -1.388759003020823e-3f);
+    cp = fmaf(t, cp, 4.166664928197861e-2f);
+    cp = fmaf(t, cp, -0.5f);
+    const float cs = fmaf(t, cp, 1.f);
+    // angle = q pi/2 + theta
+    const float a = (q & 1u) ? cs : sn, b = (q & 1u) ? sn : cs;
+    s = (q & 2u) ? -a : a;
+    c = ((q + 1u) & 2u) ? -b : b;
+}
+// The same in fp64 (Taylor polynomials to theta^11 / theta^12: 7e-12 on [-pi/4, pi/4]; r converts exactly), for the
+// structure-factor pass: in a liquid of neutral molecules S(k) at small k is what is left of N cancelling charges
+// (|S| ~ 1e-2 sqrt(N) |q| where A_k is largest), so the 6e-8 rounding of an fp32 cosine per atom came back as 3e-6 in
+// S(k) and 7e-6 in every force -- the sines and cosines of this pass need more than fp32 holds.
+__device__ inline void phase_sincos_d(unsigned p, double &s, double &c) {
+    const unsigned q = (p + 0x20000000u) >> 30;
+    const int r = (int)(p - (q << 30));
+    const double th = 1.4629180792671596e-9 * (double)r;   // 2 pi / 2^32
+    const double t = th * th;
+    double sp = fma(t, -2.505210838544172e-8, 2.755731922398589e-6);   // -1/11!, 1/9!
+    sp = fma(t, sp, -1.984126984126984e-4);                            // -1/7!
+    sp = fma(t, sp, 8.333333333333333e-3);                             //  1/5!
+    sp = fma(t, sp, -1.666666666666667e-1);                            // -1/3!
+    const double sn = fma(th * t, sp, th);
+    double cp = fma(t, 2.087675698786810e-9, -2.755731922398589e-7);   //  1/12!, -1/10!
+    cp = fma(t, cp, 2.480158730158730e-5);                             //  1/8!
+    cp = fma(t, cp, -1.388888888888889e-3);                            // -1/6!
+    cp = fma(t, cp, 4.166666666666667e-2);                             //  1/4!
+    cp = fma(t, cp, -0.5);
+    const double cs = fma(t, cp, 1.0);
+    const double a = (q & 1u) ? cs : sn, b = (q & 1u) ? sn : cs;
+    s = (q & 2u) ? -a : a;
+    c = ((q + 1u) & 2u) ? -b : b;
+}
+
+// running sum with a compensation term (Kahan)
+__device__ inline void ksum(float x, float &sum, float &comp) {
+    const float y = x - comp, t = sum + y;
+    comp = (t - sum) - y;
+    sum = t;
 }
 
 constexpr int SF_THREADS = 128;   // k-vectors per CTA of the structure-factor pass
@@ -44,34 +92,36 @@ constexpr int SF_TILE = 128;      // atoms staged per pass
 __global__ void __launch_bounds__(SF_THREADS) k_sfac_partial(int n, int nk, int chunk, double ibx, double iby, double ibz,
                                                            const float4 *__restrict__ xs, const float4 *__restrict__ xl,
                                                            const int *__restrict__ kpack, double2 *__restrict__ part) {
-    __shared__ double4 tile[SF_TILE];
+    __shared__ uint4 tile[SF_TILE];   // (fixed-point x/Lx, y/Ly, z/Lz, -)
+    __shared__ double tile_q[SF_TILE];
     const int k = blockIdx.x * SF_THREADS + threadIdx.x;
     int nx = 0, ny = 0, nz = 0;
     if (k < nk) ew_unpack(kpack[k], nx, ny, nz);
-    const double dnx = (double)nx, dny = (double)ny, dnz = (double)nz;
     const int a0 = blockIdx.y * chunk, a1 = min(a0 + chunk, n);
     double sr = 0.0, si = 0.0;
     for (int b = a0; b < a1; b += SF_TILE) {
         __syncthreads();
         for (int t = threadIdx.x; t < SF_TILE; t += SF_THREADS) {
             const int j = b + t;
-            double4 e = make_double4(0.0, 0.0, 0.0, 0.0);
+            uint4 e = make_uint4(0u, 0u, 0u, 0u);
+            double q = 0.0;   // charge 0: no contribution
             if (j < a1) {
                 const float4 h = xs[j], l = xl[j];
-                e = make_double4(((double)h.x + (double)l.x) * ibx, ((double)h.y + (double)l.y) * iby,
-                                 ((double)h.z + (double)l.z) * ibz, (double)h.w);
+                e = make_uint4(fix_cycle(((double)h.x + (double)l.x) * ibx), fix_cycle(((double)h.y + (double)l.y) * iby),
+                               fix_cycle(((double)h.z + (double)l.z) * ibz), 0u);
+                q = (double)h.w;
             }
-            tile[t] = e;
+            tile[t] = e; tile_q[t] = q;
         }
         __syncthreads();
-        const int lim = min(SF_TILE, a1 - b);
 #pragma unroll 4
-        for (int t = 0; t < lim; ++t) {
-            const double4 e = tile[t];
-            float s, c;
-            phase_sincos(fma(dnx, e.x, fma(dny, e.y, dnz * e.z)), s, c);
-            sr = fma(e.w, (double)c, sr);
-            si = fma(e.w, (double)s, si);
+        for (int t = 0; t < SF_TILE; ++t) {
+            const uint4 e = tile[t];
+            double s, c;
+            phase_sincos_d((unsigned)nx * e.x + (unsigned)ny * e.y + (unsigned)nz * e.z, s, c);
+            const double q = tile_q[t];
+            sr = fma(q, c, sr);
+            si = fma(q, s, si);
         }
     }
     if (k < nk) part[(size_t)blockIdx.y * nk + k] = make_double2(sr, si);
@@ -99,8 +149,11 @@ __global__ void __launch_bounds__(RF_THREADS) k_rec_force(Model m, int nk, doubl
                                                          const int *__restrict__ orig, const int *__restrict__ sorted_of,
                                                          const int *__restrict__ excl_ptr, const int *__restrict__ excl_idx,
                                                          float4 *__restrict__ out) {
-    __shared__ int s_k[RF_TILE];
-    __shared__ double2 s_w[RF_TILE];
+    // a staged k-vector: (nx, ny, nz, bits of W.x) as integers for the phase and (nx, ny, nz, W.y) as floats for the
+    // products -- no conversion in the loop.  fp32 sines, products and compensated fp32 sums are enough HERE (1e-7 of
+    // the force, measured): unlike S(k), an atom's sum over k is not the small remainder of a cancellation.
+    __shared__ int4 s_k[RF_TILE];
+    __shared__ float4 s_f[RF_TILE];
     const unsigned full = 0xffffffffu;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int i = blockIdx.x * (RF_THREADS / 32) + warp;
@@ -110,30 +163,32 @@ __global__ void __launch_bounds__(RF_THREADS) k_rec_force(Model m, int nk, doubl
         const float4 h = xs[i], l = xl[i];
         X = (double)h.x + (double)l.x; Y = (double)h.y + (double)l.y; Z = (double)h.z + (double)l.z; q = (double)h.w;
     }
-    const double sx = X * ibx, sy = Y * iby, sz = Z * ibz;
-    double gx = 0.0, gy = 0.0, gz = 0.0;   // sum of term * n per dimension
+    const unsigned ux = fix_cycle(X * ibx), uy = fix_cycle(Y * iby), uz = fix_cycle(Z * ibz);
+    float fx = 0.f, fy = 0.f, fz = 0.f, cx = 0.f, cy = 0.f, cz = 0.f;   // sum of term * n per dimension, compensated
     double ew = 0.0;                        // this atom's half of its exclusion-correction energies
     for (int b = 0; b < nk; b += RF_TILE) {
         __syncthreads();
         for (int t = threadIdx.x; t < RF_TILE; t += RF_THREADS) {
-            const bool in = b + t < nk;
-            s_k[t] = in ? kpack[b + t] : ew_pack(0, 0, 0);
-            s_w[t] = in ? W[b + t] : make_double2(0.0, 0.0);
+            int nx = 0, ny = 0, nz = 0;
+            double2 w = make_double2(0.0, 0.0);
+            if (b + t < nk) { ew_unpack(kpack[b + t], nx, ny, nz); w = W[b + t]; }
+            s_k[t] = make_int4(nx, ny, nz, __float_as_int((float)w.x));
+            s_f[t] = make_float4((float)nx, (float)ny, (float)nz, (float)w.y);
         }
         __syncthreads();
         if (!live) continue;
         const int lim = min(RF_TILE, nk - b);
 #pragma unroll 2
         for (int t = lane; t < lim; t += 32) {
-            int nx, ny, nz;
-            ew_unpack(s_k[t], nx, ny, nz);
-            const double2 w = s_w[t];
+            const int4 kn = s_k[t];
+            const float4 kf = s_f[t];
             float s, c;
-            phase_sincos(fma((double)nx, sx, fma((double)ny, sy, (double)nz * sz)), s, c);
-            const double term = w.y * (double)c - w.x * (double)s;   // 2 A_k (Im S cos - Re S sin)
-            gx = fma(term, (double)nx, gx); gy = fma(term, (double)ny, gy); gz = fma(term, (double)nz, gz);
+            phase_sincos((unsigned)kn.x * ux + (unsigned)kn.y * uy + (unsigned)kn.z * uz, s, c);
+            const float term = fmaf(kf.w, c, -__int_as_float(kn.w) * s);   // 2 A_k (Im S cos - Re S sin)
+            ksum(term * kf.x, fx, cx); ksum(term * kf.y, fy, cy); ksum(term * kf.z, fz, cz);
         }
     }
+    double gx = (double)fx - (double)cx, gy = (double)fy - (double)cy, gz = (double)fz - (double)cz;
     const double two_pi = 6.283185307179586476925;
     gx *= q * two_pi * ibx; gy *= q * two_pi * iby; gz *= q * two_pi * ibz;   // k = 2 pi n / L
     // exclusion correction: lane l takes the l-th, l+32-th ... excluded partner of the atom
