@@ -30,7 +30,9 @@
  * energy conservation / reversibility; 2-body Boltzmann histogram; degenerate
  * cases.  "Parity unpinned" by the paper (fixed by DESIGN.md readings only):
  * the formula of chi, the bound recipe L, r_M, the list policy (skin, order),
- * the G~ proposal details, the Philox stream layout.
+ * the G~ proposal details, the Philox stream layout, k_cut of the reciprocal sum and
+ * the outermost step ratio of RESPA1 (R-21).  The reciprocal sum itself is pinned (Madelung
+ * constant of rock salt, finite differences, a closed form on one molecule).
  *
  * Sign convention (R-4): every "F" here is a GRADIENT piece (grad U = sum F),
  * physical force = -F, exactly as in the paper.
