@@ -141,6 +141,12 @@ int jump_get_row(jump_ctx *c, int32_t which, int32_t atom, int32_t *host_out, in
  *   are not applied (a geometric histogram).  Asynchronous on the context's stream.  g(r) is
  *   hist / (n_calls * 0.5 N (N-1) / V * shell volume). */
 int jump_get_images(jump_ctx *c, int32_t *d_img);
+/* Velocity autocorrelation (the velocity spectra of P:L529-531, L583-589 are its cosine transform).  jump_vacf_mark
+ * stores the current velocities, by original atom index, as the time origin (asynchronous).  jump_vacf_dot writes
+ * *c_out = (1/N_sel) sum_{i in sel} v_i(origin) . v_i(now) in (A/ps)^2 (host double), sel = all atoms or (lj_only != 0) the LJ
+ * carriers; fp64 sums in a fixed order.  Synchronises; JUMP_E_ARG before a mark. */
+int jump_vacf_mark(jump_ctx *c);
+int jump_vacf_dot(jump_ctx *c, int32_t lj_only, double *c_out);
 int jump_rdf_accumulate(jump_ctx *c, int32_t lj_only, double r_max, int32_t n_bins, uint64_t *d_hist);
 /* Bounds as used (R-7): GM, GL, GV, qmax, eps_max, sig_min, sig_max, rM. */
 int jump_get_bounds(jump_ctx *c, double out[8]);

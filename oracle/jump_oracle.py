@@ -389,3 +389,22 @@ def pair_histogram(pos, box, r_max, n_bins):
         b = np.floor(r[r < r_max] * (n_bins / r_max)).astype(np.int64)
         hist += np.bincount(np.minimum(b, n_bins - 1), minlength=n_bins)
     return hist
+
+
+def velocity_autocorrelation(v_origin, v_now, select=None):
+    """NEXT-4 oracle: C = (1/N_sel) sum_{i in sel} v_i(t0) . v_i(t0 + tau), (A/ps)^2 -- the plain definition of the
+    velocity autocorrelation behind the spectra of P:L529-531, L583-589, fp64."""
+    a, b = np.asarray(v_origin, dtype=np.float64), np.asarray(v_now, dtype=np.float64)
+    if select is not None:
+        a, b = a[select], b[select]
+    return float((a * b).sum(1).mean())
+
+
+def vacf_spectrum(c, dt_ps, omegas):
+    """I(omega) = dt [C(0)/2 + sum_{k>=1} C(k dt) cos(omega k dt) w_k] with a Hann window w_k = cos^2(pi k / 2K) over the K
+    lags given: the windowed cosine transform of the autocorrelation (the velocity spectra of P:L529-531), fp64."""
+    c = np.asarray(c, dtype=np.float64)
+    k = np.arange(len(c))
+    w = np.cos(0.5 * np.pi * k / len(c)) ** 2
+    w[0] = 0.5
+    return np.array([dt_ps * float((c * w * np.cos(om * k * dt_ps)).sum()) for om in np.atleast_1d(omegas)])

@@ -22,7 +22,7 @@ EXPORTS = ["jump_init", "jump_step", "baoab_step", "jump_respa_step", "jump_get_
            "jump_get_stats", "jump_reset_stats", "jump_get_events", "jump_clear_events", "jump_get_row", "jump_get_images", "jump_rdf_accumulate",
            "jump_get_bounds", "jump_refresh", "jump_refresh_lazy", "jump_half", "jump_sync", "jump_get_step", "jump_get_launches",
            "jump_last_error", "jump_free", "jump_set_profiling", "jump_get_profile", "jump_count_pairs",
-           "jump_ewald_setup", "jump_respa1_step", "jump_get_slow_energy"]
+           "jump_ewald_setup", "jump_respa1_step", "jump_get_slow_energy", "jump_vacf_mark", "jump_vacf_dot"]
 
 
 class jump_params(C.Structure):
@@ -78,6 +78,8 @@ def lib():
         L.jump_ewald_setup.argtypes = [vp, C.c_double, C.POINTER(C.c_int32)]
         L.jump_respa1_step.argtypes = [vp, i32, i32]
         L.jump_get_slow_energy.argtypes = [vp, C.POINTER(C.c_double)]
+        L.jump_vacf_mark.argtypes = [vp]
+        L.jump_vacf_dot.argtypes = [vp, i32, C.POINTER(C.c_double)]
         L.jump_get_forces.argtypes = [vp, i32, vp]
         L.jump_get_energy.argtypes = [vp, dp, dp]
         L.jump_get_stats.argtypes = [vp, C.POINTER(jump_stats)]
@@ -194,6 +196,15 @@ class JumpSim:
 
     def jump_respa1_step(self, n=1, n_mid=3):
         self._check(self._L.jump_respa1_step(self._h, int(n), int(n_mid)), "jump_respa1_step")
+
+    def vacf_mark(self):
+        self._check(self._L.jump_vacf_mark(self._h), "jump_vacf_mark")
+
+    def vacf_dot(self, lj_only=False):
+        """(1/N_sel) sum v_i(mark) . v_i(now), (A/ps)^2."""
+        c = C.c_double(0.0)
+        self._check(self._L.jump_vacf_dot(self._h, int(bool(lj_only)), C.byref(c)), "jump_vacf_dot")
+        return float(c.value)
 
     def slow_energy(self):
         e = C.c_double(0.0)

@@ -41,6 +41,8 @@ struct jump_ctx {
     float4 *fslow;
     double *ew_sum;
     double q2sum;            // sum of q_i^2 (self term)
+    float4 *vacf_v0;         // velocities at the time origin of the autocorrelation, by original atom index
+    double2 *vacf_part;
     bool slow_valid;         // fslow holds grad(U_rec + U_excl) at the current positions, in the current sorted order
     int64_t outer1;
 
@@ -817,6 +819,7 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     c->f0_valid = false;
     c->slow_valid = false;
     memset(&c->ew, 0, sizeof c->ew);
+    c->vacf_v0 = nullptr; c->vacf_part = nullptr;
     c->fslow = nullptr; c->ew_sum = nullptr; c->q2sum = 0.0; c->outer1 = 0;
     c->prof = false;
     for (int k = 0; k < 4; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
@@ -962,6 +965,26 @@ extern "C" int jump_rdf_accumulate(jump_ctx *c, int32_t lj_only, double r_max, i
                    (unsigned long long *)d_hist, c->st, &c->launches))
         return JUMP_E_ARG;
     CK(cudaGetLastError());
+    return 0;
+}
+extern "C" int jump_vacf_mark(jump_ctx *c) {
+    if (!c) return JUMP_E_ARG;
+    int r;
+    if (!c->vacf_v0 && ((r = dalloc(c, &c->vacf_v0, (size_t)c->n)) || (r = dalloc(c, &c->vacf_part, (size_t)(c->n + 255) / 256 + 1)))) return r;
+    launch_vacf_mark(c->n, c->vs, c->orig, c->vacf_v0, c->st, &c->launches);
+    CK(cudaGetLastError());
+    return 0;
+}
+extern "C" int jump_vacf_dot(jump_ctx *c, int32_t lj_only, double *c_out) {
+    if (!c || !c_out) return JUMP_E_ARG;
+    if (!c->vacf_v0) { c->err = "jump_vacf_mark has not been called"; return JUMP_E_ARG; }
+    const size_t nb = (size_t)(c->n + 255) / 256;
+    launch_vacf_dot(c->n, lj_only != 0, c->vs, c->vacf_v0, c->orig, c->lj, c->vacf_part, c->vacf_part + nb, c->st, &c->launches);
+    CK(cudaGetLastError());
+    std::vector<double2> h;
+    int r = ddownload(c, h, (const double2 *)(c->vacf_part + nb), 1);
+    if (r) return r;
+    *c_out = h[0].y > 0.0 ? h[0].x / h[0].y : 0.0;
     return 0;
 }
 extern "C" int jump_get_bounds(jump_ctx *c, double out[8]) {

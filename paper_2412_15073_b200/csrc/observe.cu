@@ -1,5 +1,5 @@
 // observe.cu -- observables computed on the device from the sorted state: radial distribution
-// histograms.  (Image counters for unwrapped trajectories live in update.cu / common.cuh.)
+// histograms, velocity autocorrelation.  (Image counters for unwrapped trajectories live in update.cu / common.cuh.)
 // The paper's evidence that JUMP samples mu and keeps the dynamics is of this kind: radial distribution functions and
 // diffusion constants.
 #include "launch.h"
@@ -56,6 +56,56 @@ __global__ void __launch_bounds__(256) k_rdf(Model m, SortGrid g, int reach0, in
     __syncthreads();
     for (int b = threadIdx.x; b < n_bins; b += blockDim.x)
         if (s_hist[b]) atomicAdd(&hist[b], (unsigned long long)s_hist[b]);
+}
+
+// Velocity autocorrelation (velocity spectra): the velocities at the time origin are kept by
+// ORIGINAL atom index (the sort permutes atoms between two reads); C = (1/N_sel) sum v_i(origin) . v_i(now).
+__global__ void k_vacf_mark(int n, const float4 *__restrict__ vs, const int *__restrict__ orig, float4 *__restrict__ v0) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) v0[orig[i]] = vs[i];
+}
+// per-CTA partial sums in fp64, in a fixed order (shared-memory tree): (sum of dots, number of selected atoms)
+__global__ void __launch_bounds__(256) k_vacf_dot(int n, int lj_only, const float4 *__restrict__ vs, const float4 *__restrict__ v0,
+                                                  const int *__restrict__ orig, const float2 *__restrict__ lj,
+                                                  double2 *__restrict__ part) {
+    __shared__ double s_d[256], s_c[256];
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    double d = 0.0, cnt = 0.0;
+    if (i < n && (!lj_only || lj[i].y > 0.f)) {
+        const float4 a = v0[orig[i]], b = vs[i];
+        d = (double)a.x * (double)b.x + (double)a.y * (double)b.y + (double)a.z * (double)b.z;
+        cnt = 1.0;
+    }
+    s_d[threadIdx.x] = d; s_c[threadIdx.x] = cnt;
+    __syncthreads();
+    for (int off = 128; off > 0; off >>= 1) {
+        if (threadIdx.x < off) { s_d[threadIdx.x] += s_d[threadIdx.x + off]; s_c[threadIdx.x] += s_c[threadIdx.x + off]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) part[blockIdx.x] = make_double2(s_d[0], s_c[0]);
+}
+__global__ void k_vacf_final(int nb, const double2 *__restrict__ part, double2 *__restrict__ out) {
+    __shared__ double s_d[256], s_c[256];
+    double d = 0.0, c = 0.0;
+    for (int t = threadIdx.x; t < nb; t += 256) { d += part[t].x; c += part[t].y; }
+    s_d[threadIdx.x] = d; s_c[threadIdx.x] = c;
+    __syncthreads();
+    for (int off = 128; off > 0; off >>= 1) {
+        if (threadIdx.x < off) { s_d[threadIdx.x] += s_d[threadIdx.x + off]; s_c[threadIdx.x] += s_c[threadIdx.x + off]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = make_double2(s_d[0], s_c[0]);
+}
+void launch_vacf_mark(int n, const float4 *vs, const int *orig, float4 *v0, cudaStream_t st, int64_t *launches) {
+    k_vacf_mark<<<(n + 255) / 256, 256, 0, st>>>(n, vs, orig, v0);
+    *launches += 1;
+}
+void launch_vacf_dot(int n, int lj_only, const float4 *vs, const float4 *v0, const int *orig, const float2 *lj, double2 *part,
+                     double2 *out, cudaStream_t st, int64_t *launches) {
+    const int nb = (n + 255) / 256;
+    k_vacf_dot<<<nb, 256, 0, st>>>(n, lj_only, vs, v0, orig, lj, part);
+    k_vacf_final<<<1, 256, 0, st>>>(nb, part, out);
+    *launches += 2;
 }
 
 int launch_rdf(const Model &m, const SortGrid &g, int lj_only, double r_max, double r_reach, int n_bins, const int *cell_start,

@@ -594,3 +594,26 @@ def test_respa1_needs_setup_and_conserves_energy(jb, cfg0):
         out.append(np.std(e))
     assert out[0] < 0.02 * 648 * 0.6
     assert out[1] < 0.5 * out[0]
+
+
+def test_velocity_autocorrelation_on_the_device(jb, jo, cfg0):
+    """NEXT-4: jump_vacf_mark / jump_vacf_dot against the plain definition (oracle.velocity_autocorrelation) on the
+    oracle's own velocities of the same seeded run: exact at lag 0 (the generator's fp32 velocities), then along 40 JUMP
+    steps -- across a re-sort, which permutes the atoms -- to the accuracy the trajectories agree to (R-16)."""
+    sysd, run = cfg0
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    with pytest.raises(RuntimeError):
+        g.vacf_dot()
+    g.vacf_mark()
+    v0 = o.vel
+    oxy = sysd["lj_eps"] > 0
+    assert g.vacf_dot() == pytest.approx(jo.velocity_autocorrelation(v0, v0), rel=1e-12)
+    assert g.vacf_dot(lj_only=True) == pytest.approx(jo.velocity_autocorrelation(v0, v0, oxy), rel=1e-12)
+    c0 = jo.velocity_autocorrelation(v0, v0)
+    for _ in range(4):
+        g.jump_step(10); g.sync(); o.jump_step(10)
+        if fragile(o):
+            break
+        assert abs(g.vacf_dot() - jo.velocity_autocorrelation(v0, o.vel)) < 2e-4 * c0
+        assert abs(g.vacf_dot(lj_only=True) - jo.velocity_autocorrelation(v0, o.vel, oxy)) < 2e-4 * c0
+    assert o.step >= 10

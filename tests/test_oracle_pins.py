@@ -757,3 +757,34 @@ def test_respa1_reductions_and_energy_conservation(relaxed_small):
         o.jump_respa1_step(40 // (n_inner * n_mid), n_mid)
         rate.append(o.stats()["proposals"] / 40.0)
     assert abs(rate[0] / rate[1] - 1.0) < 0.1
+
+
+# ---------------------------------------------------------------- NEXT-4: velocity autocorrelation and its spectrum
+def test_vacf_of_the_O_step_is_exponential_and_its_spectrum_lorentzian():
+    """Free particles under the O part alone are an exact Ornstein-Uhlenbeck process: C(tau) = (3 k_B T / m)
+    exp(-gamma tau); the windowed cosine transform of exp(-gamma tau) is the Lorentzian gamma / (gamma^2 + omega^2)."""
+    sysd = _ideal_gas(n=6000, seed=3)
+    rng = np.random.default_rng(11)
+    sysd = dict(sysd, vel=rng.normal(size=(6000, 3)) * np.sqrt(KB * 300 * KCAL / sysd["mass"])[:, None])
+    gamma, dt = 5.0, 2.0e-3
+    o = jo.Oracle(sysd, r_short=4.0, r_long=6.0, r_mid=5.0, skin=0.5, nlist_every=50, dt_fs=dt * 1e3, gamma_per_ps=gamma,
+                  flags=0, seed=9)
+    heavy = sysd["mass"] == 16.0
+    v0 = o.vel
+    c = [jo.velocity_autocorrelation(v0, v0, heavy)]
+    for _ in range(60):
+        o.baoab_step(5)
+        c.append(jo.velocity_autocorrelation(v0, o.vel, heavy))
+    c = np.array(c)
+    tau = np.arange(61) * 5 * dt
+    c0 = 3 * KB * 300 * KCAL / 16.0
+    assert abs(c[0] / c0 - 1) < 0.05
+    assert np.abs(c / c[0] - np.exp(-gamma * tau)).max() < 0.05          # 3000 atoms: 1/sqrt(9000) = 0.01 per point
+    # the transform on an exact exponential
+    tt = np.arange(4000) * 1e-3
+    om = np.array([0.0, 2.0, 5.0, 12.0])
+    spec = jo.vacf_spectrum(np.exp(-gamma * tt), 1e-3, om)
+    assert np.abs(spec / (gamma / (gamma ** 2 + om ** 2)) - 1).max() < 0.02
+    # one harmonic mode shows up as a line at its frequency
+    line = jo.vacf_spectrum(np.cos(7.0 * tt), 1e-3, np.linspace(0.0, 14.0, 57))
+    assert abs(np.linspace(0.0, 14.0, 57)[np.argmax(line)] - 7.0) < 0.3
