@@ -555,6 +555,20 @@ extern "C" int jump_ewald_setup(jump_ctx *c, double k_cut, int32_t *n_k) {
     e.kpack = dk; e.coefA = dA;
     if ((r = dalloc(c, &e.part, (size_t)e.nch * e.nk)) || (r = dalloc(c, &e.W, (size_t)e.nk)) || (r = dalloc(c, &e.ek, (size_t)e.nk)))
         return r;
+    // factorised phase tables for the structure-factor pass when a tile of them fits the shared memory;
+    // JUMP_B200_EWALD_DIRECT=1 forces the direct form
+    int used[3] = {0, 0, 0};
+    for (size_t t = 0; t < kp.size(); ++t) {
+        const int w = kp[t];
+        const int nn[3] = {(w & 1023) - 512, ((w >> 10) & 1023) - 512, ((w >> 20) & 1023) - 512};
+        for (int d = 0; d < 3; ++d) used[d] = std::max(used[d], std::abs(nn[d]));
+    }
+    for (int d = 0; d < 3; ++d) e.nmax[d] = used[d];
+    const int E = used[0] + used[1] + used[2] + 3;
+    const char *direct = getenv("JUMP_B200_EWALD_DIRECT");
+    if (e.nk > 0 && E <= ewald_table_entries_max() && !(direct && atoi(direct) != 0)) {
+        if ((r = dalloc(c, &e.tabD, (size_t)E * c->n))) return r;
+    }
     if (!c->fslow && (r = dalloc(c, &c->fslow, (size_t)c->n))) return r;
     if (!c->ew_sum && (r = dalloc(c, &c->ew_sum, 1))) return r;
     std::vector<float4> hx;

@@ -220,6 +220,64 @@ __global__ void __launch_bounds__(RF_THREADS) k_rec_force(Model m, int nk, doubl
     if (live && lane == 0) out[i] = make_float4((float)gx, (float)gy, (float)gz, (float)ew);
 }
 
+// ---- factorised form of the structure-factor pass: exp(i k.x_j) = Ex_j[nx] Ey_j[ny] Ez_j[nz] -----------------------
+// Per atom and dimension the phase factors exp(2 pi i a x_j / L), a = 0 .. n_max (negative a: the conjugate), are
+// tabulated once per evaluation in fp64 (E = n_max,x + n_max,y + n_max,z + 3 entries per atom: 63 on the 49 A box
+// against the 16 493 terms they replace), the charge folded into Ex, entry-major [E][n] so that a tile of atoms loads
+// coalesced; a term is then two complex products (10 fp64 operations instead of 14 and the integer reduction).  It is
+// bound by the three 16-byte shared-memory reads per term (12 wavefronts per warp and term).  The same form of the
+// force pass (fp32 tables, one atom's table per warp) was measured slower than the direct fp32 polynomial (381 against
+// 370 us) and is not kept.
+__global__ void k_ew_tables(int n, int E, int ex, int ey, double ibx, double iby, double ibz,
+                            const float4 *__restrict__ xs, const float4 *__restrict__ xl, double2 *__restrict__ tabD) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= (long long)n * E) return;
+    const int e = (int)(g / n), i = (int)(g - (long long)e * n);   // consecutive threads: consecutive atoms of one entry
+    const float4 h = xs[i], l = xl[i];
+    const int dim = e < ex ? 0 : (e < ex + ey ? 1 : 2);
+    const int a = e - (dim == 0 ? 0 : (dim == 1 ? ex : ex + ey));
+    const double xd = dim == 0 ? ((double)h.x + (double)l.x) * ibx
+                               : (dim == 1 ? ((double)h.y + (double)l.y) * iby : ((double)h.z + (double)l.z) * ibz);
+    double sn, cs;
+    phase_sincos_d((unsigned)a * fix_cycle(xd), sn, cs);
+    const double q = dim == 0 ? (double)h.w : 1.0;
+    tabD[(size_t)e * n + i] = make_double2(q * cs, q * sn);
+}
+
+constexpr int SF2_THREADS = 512;   // k-vectors per CTA (the tables of an atom tile are staged once per CTA)
+constexpr int SF2_TA = 16;         // atoms per staged tile: E x 16 double2 <= 48 KB for E <= 192
+constexpr int SF2_EMAX = 192;
+
+__global__ void __launch_bounds__(SF2_THREADS) k_sfac_partial_tab(int n, int nk, int chunk, int E, int ex, int ey,
+                                                                const double2 *__restrict__ tabD,
+                                                                const int *__restrict__ kpack, double2 *__restrict__ part) {
+    extern __shared__ double2 s_tab[];   // [SF2_TA][E]: the threads of a warp differ in nz mostly -- consecutive entries
+    const int k = blockIdx.x * SF2_THREADS + threadIdx.x;
+    int nx = 0, ny = 0, nz = 0;
+    if (k < nk) ew_unpack(kpack[k], nx, ny, nz);
+    const int ox = nx, oy = ex + abs(ny), oz = ex + ey + abs(nz);
+    const double sy = ny < 0 ? -1.0 : 1.0, sz = nz < 0 ? -1.0 : 1.0;   // negative n: the conjugate entry
+    const int a0 = blockIdx.y * chunk, a1 = min(a0 + chunk, n);
+    double sr = 0.0, si = 0.0;
+    for (int b = a0; b < a1; b += SF2_TA) {
+        __syncthreads();
+        for (int t = threadIdx.x; t < E * SF2_TA; t += SF2_THREADS) {
+            const int e = t / SF2_TA, j = b + (t - e * SF2_TA);
+            s_tab[(t - e * SF2_TA) * E + e] = j < a1 ? tabD[(size_t)e * n + j] : make_double2(0.0, 0.0);   // (q = 0 in Ex: no contribution)
+        }
+        __syncthreads();
+#pragma unroll 4
+        for (int t = 0; t < SF2_TA; ++t) {
+            const double2 a = s_tab[t * E + ox], bb = s_tab[t * E + oy], c = s_tab[t * E + oz];
+            const double by = sy * bb.y, cy = sz * c.y;
+            const double pr = fma(a.x, bb.x, -a.y * by), pi = fma(a.x, by, a.y * bb.x);
+            sr = fma(pr, c.x, fma(-pi, cy, sr));
+            si = fma(pr, cy, fma(pi, c.x, si));
+        }
+    }
+    if (k < nk) part[(size_t)blockIdx.y * nk + k] = make_double2(sr, si);
+}
+
 // sum of n doubles by one CTA in a fixed order (energy diagnostics)
 __global__ void k_sum_doubles(int n, const double *__restrict__ in, double *__restrict__ out) {
     __shared__ double s[256];
@@ -239,6 +297,18 @@ void launch_rec_force(const Model &m, const EwaldArgs &e, const float4 *xs, cons
                       int64_t *launches) {
     const double ibx = 1.0 / (double)m.box[0], iby = 1.0 / (double)m.box[1], ibz = 1.0 / (double)m.box[2];
     const int chunk = (m.n + e.nch - 1) / e.nch;
+    if (e.tabD) {   // factorised structure-factor pass (the tables fit): see k_ew_tables
+        const int ex = e.nmax[0] + 1, ey = e.nmax[1] + 1, E = ex + ey + e.nmax[2] + 1;
+        const long long tot = (long long)m.n * E;
+        k_ew_tables<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(m.n, E, ex, ey, ibx, iby, ibz, xs, xl, e.tabD);
+        dim3 g1((unsigned)((e.nk + SF2_THREADS - 1) / SF2_THREADS), (unsigned)e.nch);
+        k_sfac_partial_tab<<<g1, SF2_THREADS, (size_t)E * SF2_TA * sizeof(double2), st>>>(m.n, e.nk, chunk, E, ex, ey, e.tabD, e.kpack, e.part);
+        k_sfac_reduce<<<(e.nk + 255) / 256, 256, 0, st>>>(e.nk, e.nch, e.part, e.coefA, e.W, e.ek);
+        k_rec_force<<<(m.n + RF_THREADS / 32 - 1) / (RF_THREADS / 32), RF_THREADS, 0, st>>>(m, e.nk, ibx, iby, ibz, e.alpha, xs, xl, e.kpack,
+                                                                                             e.W, orig, sorted_of, excl_ptr, excl_idx, out);
+        *launches += 4;
+        return;
+    }
     dim3 g1((unsigned)((e.nk + SF_THREADS - 1) / SF_THREADS), (unsigned)e.nch);
     k_sfac_partial<<<g1, SF_THREADS, 0, st>>>(m.n, e.nk, chunk, ibx, iby, ibz, xs, xl, e.kpack, e.part);
     k_sfac_reduce<<<(e.nk + 255) / 256, 256, 0, st>>>(e.nk, e.nch, e.part, e.coefA, e.W, e.ek);
@@ -246,6 +316,7 @@ void launch_rec_force(const Model &m, const EwaldArgs &e, const float4 *xs, cons
                                                                                          e.W, orig, sorted_of, excl_ptr, excl_idx, out);
     *launches += 3;
 }
+int ewald_table_entries_max() { return SF2_EMAX; }
 void launch_rec_energy(const EwaldArgs &e, double *out, cudaStream_t st, int64_t *launches) {
     k_sum_doubles<<<1, 256, 0, st>>>(e.nk, e.ek, out);
     *launches += 1;

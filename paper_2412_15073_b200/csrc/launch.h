@@ -46,6 +46,8 @@ struct EwaldArgs {   // reciprocal Ewald sum (ewald.cu, R-21)
     double2 *part;           // [nch][nk] structure-factor partials
     double2 *W;              // [nk] 2 A_k S(k)
     double *ek;              // [nk] A_k |S(k)|^2
+    int nmax[3];             // largest |n| per dimension
+    double2 *tabD;           // [E][n] fp64 phase-factor tables (NULL: direct sines and cosines), E = sum (nmax + 1)
 };
 
 void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches);
@@ -81,5 +83,6 @@ void launch_rec_force(const Model &m, const EwaldArgs &e, const float4 *xs, cons
                       int64_t *launches);
 void launch_rec_energy(const EwaldArgs &e, double *out, cudaStream_t st, int64_t *launches);
 int ewald_pack(int nx, int ny, int nz);
+int ewald_table_entries_max();
 
 }  // namespace jb
