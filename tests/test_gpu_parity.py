@@ -617,3 +617,27 @@ def test_velocity_autocorrelation_on_the_device(jb, jo, cfg0):
         assert abs(g.vacf_dot() - jo.velocity_autocorrelation(v0, o.vel)) < 2e-4 * c0
         assert abs(g.vacf_dot(lj_only=True) - jo.velocity_autocorrelation(v0, o.vel, oxy)) < 2e-4 * c0
     assert o.step >= 10
+
+
+@pytest.mark.parametrize("direct", [False, True])
+def test_slow_force_orthorhombic_box_and_both_kernel_forms(jb, jo, direct, monkeypatch):
+    """R-21 on a box with three different edges (different n_max per dimension: the table offsets of the factorised
+    structure-factor pass) and through both forms of that pass (JUMP_B200_EWALD_DIRECT=1: direct sines and cosines);
+    a k list of 3 vectors (shorter than a tile) and an empty one."""
+    if direct:
+        monkeypatch.setenv("JUMP_B200_EWALD_DIRECT", "1")
+    sysd = wl.small_water(5, seed=13)
+    box = np.array([16.0, 18.5, 21.0])
+    run = dict(wl.make_config(0)[1], r_short=4.0, r_long=7.5, r_mid=5.5, seed=9)
+    sysd = dict(sysd, box=box)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    for k_cut in (0.0, 1.05 * 2 * np.pi / 16.0, 0.1):
+        nk = g.ewald_setup(k_cut)
+        assert nk == o.ewald_setup(k_cut)
+        fo = o.forces(5)
+        fg = g.forces(5).cpu().numpy().astype(np.float64)
+        if nk == 0:
+            assert np.abs(fg).max() == 0.0 and np.abs(fo).max() == 0.0 and g.slow_energy() == 0.0
+        else:
+            assert rel_force_err(fg, fo) <= F_TOL, (k_cut, rel_force_err(fg, fo))
+            assert g.slow_energy() == pytest.approx(o.potential(5), rel=2e-6)
