@@ -119,3 +119,30 @@ def test_jump_baoab_energy_gap_is_time_step_bias(jb):
     print("gap", gap)
     assert gap[1.0][0] > 3 * gap[1.0][1]                                  # the gap at 1 fs is real ...
     assert gap[0.5][0] < 0.5 * gap[1.0][0] + 3 * gap[0.5][1]              # ... and of second order in delta
+
+
+def test_respa1_energy_gap_is_time_step_bias(jb):
+    """NEXT-2 (R-21): three-level JUMP-RESPA1 against BAOAB-RESPA1 under the full Ewald potential U_direct + U_rec +
+    U_self + U_excl.  Both sample the same measure up to a second-order bias in the time steps: the gap
+    between their mean potential energies, 0.16 kcal/mol per molecule at 1:2:4 fs, must fall about fourfold when every
+    level is halved (0.5:1:2 fs) -- a wrong slow kick or a wrong placement of the jumps in the levels would not."""
+    sysd, run = wl.make_config(0)
+    nmol = sysd["n_atoms"] // 3
+    gap = {}
+    for dt in (1.0, 0.5):
+        U = {}
+        for name, flags in (("jump", 3), ("baoab", 3 | 16)):
+            g = jb.JumpSim(sysd, **dict(run, flags=flags, n_inner=2, dt_fs=dt, seed=run["seed"] + 21))
+            assert g.ewald_setup() > 1000
+            g.baoab_step(int(3000 / dt)); g.jump_respa1_step(int(3000 / (4 * dt)), 2)
+            u = []
+            for _ in range(1500):
+                g.jump_respa1_step(int(round(24 / (4 * dt))), 2)
+                u.append((g.energy()[1] + g.slow_energy()) / nmol)
+            assert g.stats()["error"] == 0
+            U[name] = ob.block_mean_se(u)
+            g.close()
+        gap[dt] = (U["jump"][0] - U["baoab"][0], float(np.hypot(U["jump"][1], U["baoab"][1])))
+    print("respa1 gap", gap)
+    assert gap[1.0][0] > 3 * gap[1.0][1]
+    assert gap[0.5][0] < 0.5 * gap[1.0][0] + 3 * gap[0.5][1]
