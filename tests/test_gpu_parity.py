@@ -550,12 +550,13 @@ def test_slow_force_reciprocal_ewald(jb, jo, cfg):
             assert rel_force_err(g.forces(5).cpu().numpy(), o.forces(5)) <= F_TOL
 
 
-@pytest.mark.parametrize("flags,n_inner,n_mid", [(3, 2, 3), (3 | 16, 2, 3), (1, 2, 2)])
-def test_respa1_three_levels(jb, jo, cfg0, flags, n_inner, n_mid):
+@pytest.mark.parametrize("flags,n_inner,n_mid,mode", [(3, 2, 3, 0), (3 | 16, 2, 3, 0), (1, 2, 2, 0), (3, 2, 3, 1), (3, 4, 1, 0)])
+def test_respa1_three_levels(jb, jo, cfg0, flags, n_inner, n_mid, mode):
     """JUMP-RESPA1 (1 : 2 : 6 fs as in the paper's Table 2) and the BAOAB-RESPA1 comparator: event log
-    of the middle-level jumps and the trajectory against the oracle."""
+    of the middle-level jumps and the trajectory against the oracle; mode 1: with the adaptive eps of R-19 (the paper's
+    setting for these runs); n_mid = 1: the slow kick around every middle step."""
     sysd, run = cfg0
-    r = dict(run, flags=flags | jb.F_EVENT_LOG, n_inner=n_inner)
+    r = dict(run, flags=flags | jb.F_EVENT_LOG, n_inner=n_inner, eps_mode=mode, eps_jump=2.0 if mode else run["eps_jump"])
     g, o = jb.JumpSim(sysd, **r), jo.Oracle(sysd, **r)
     assert g.ewald_setup() == o.ewald_setup()
     n_out = 3
