@@ -681,10 +681,23 @@ def test_ewald_sum_gives_the_madelung_constant_of_rock_salt():
     o = jo.Oracle(sysd, r_short=1.2, r_long=2.0, r_switch=0.2, r_mid=1.6, skin=0.0, flags=0)   # alpha = 3.8 / r_long
     nk = o.ewald_setup(12.0 * 1.9)        # e^{-36}: the reciprocal tail is far below the erfc(3.8) = 8e-8 of the direct one
     assert nk > 1000
+    M = {l.split()[0]: float(l.split()[1]) for l in open(os.path.join(GOLD, "madelung_constants.txt")) if l[0] != "#"}
     e = o.potential(1) + o.potential(5)
-    assert abs(e / (-(n / 2) * COUL * 1.7475645946331822) - 1.0) < 2e-7
+    assert abs(e / (-(n / 2) * COUL * M["rocksalt"]) - 1.0) < 2e-7
     f = o.forces(5)
     assert np.abs(f).max() < 1e-9 * COUL          # every ion is a centre of symmetry
+    # caesium chloride: two interpenetrating simple-cubic lattices, nearest-neighbour distance sqrt(3)/2 of the cube edge
+    a, m = 2.0 / math.sqrt(3.0), 4
+    g = np.array([(i, j, k) for i in range(m) for j in range(m) for k in range(m)], dtype=np.float64)
+    pos = np.vstack([g * a + 0.1, (g + 0.5) * a + 0.1])
+    nn = len(pos)
+    cs = dict(sysd, n_atoms=nn, box=m * a, pos=pos, vel=np.zeros((nn, 3)), mass=np.full(nn, 20.0),
+              charge=np.r_[np.ones(nn // 2), -np.ones(nn // 2)], lj_sigma=np.ones(nn), lj_eps=np.zeros(nn),
+              excl_ptr=np.zeros(nn + 1, dtype=np.int32))
+    o2 = jo.Oracle(cs, r_short=1.2, r_long=0.5 * m * a, r_switch=0.2, r_mid=1.6, skin=0.0, flags=0)
+    assert o2.ewald_setup(12.0 * 3.8 / (0.5 * m * a)) > 1000
+    e2 = o2.potential(1) + o2.potential(5)
+    assert abs(e2 / (-(nn / 2) * COUL * M["cscl"]) - 1.0) < 2e-7     # nearest-neighbour distance = 1
 
 
 def test_slow_force_is_the_gradient_of_reciprocal_plus_exclusion_energy(cfg0):
