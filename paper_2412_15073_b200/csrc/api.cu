@@ -553,8 +553,7 @@ extern "C" int jump_ewald_setup(jump_ctx *c, double k_cut, int32_t *n_k) {
     double *dA = nullptr;
     if ((r = dupload(c, &dk, kp)) || (r = dupload(c, &dA, cA))) return r;
     e.kpack = dk; e.coefA = dA;
-    if ((r = dalloc(c, &e.part, (size_t)e.nch * e.nk)) || (r = dalloc(c, &e.W, (size_t)e.nk)) || (r = dalloc(c, &e.ek, (size_t)e.nk)))
-        return r;
+    if ((r = dalloc(c, &e.W, (size_t)e.nk)) || (r = dalloc(c, &e.ek, (size_t)e.nk))) return r;
     // factorised phase tables for the structure-factor pass when a tile of them fits the shared memory;
     // JUMP_B200_EWALD_DIRECT=1 forces the direct form
     int used[3] = {0, 0, 0};
@@ -568,7 +567,40 @@ extern "C" int jump_ewald_setup(jump_ctx *c, double k_cut, int32_t *n_k) {
     const char *direct = getenv("JUMP_B200_EWALD_DIRECT");
     if (e.nk > 0 && E <= ewald_table_entries_max() && !(direct && atoi(direct) != 0)) {
         if ((r = dalloc(c, &e.tabD, (size_t)E * c->n))) return r;
+        // tiles of the register-blocked pass (JUMP_B200_EWALD_BLOCKED=0: one term per thread instead)
+        const char *blk = getenv("JUMP_B200_EWALD_BLOCKED");
+        if (!(blk && atoi(blk) == 0)) {
+            const int Y = 2 * used[1] + 1, Z = 2 * used[2] + 1;
+            std::vector<int> cube((size_t)(used[0] + 1) * Y * Z, -1), tiles;
+            for (size_t t = 0; t < kp.size(); ++t) {
+                const int w = kp[t];
+                const int nx = (w & 1023) - 512, ny = ((w >> 10) & 1023) - 512, nz = ((w >> 20) & 1023) - 512;
+                cube[((size_t)nx * Y + (ny + used[1])) * Z + (nz + used[2])] = (int)t;
+            }
+            for (int nx = 0; nx <= used[0]; ++nx)
+                for (int ny0 = -used[1]; ny0 <= used[1]; ny0 += 4)
+                    for (int nz0 = -used[2]; nz0 <= used[2]; nz0 += 4) {
+                        bool any = false;
+                        for (int u = 0; u < 4 && !any; ++u)
+                            for (int v = 0; v < 4 && !any; ++v) {
+                                const int ny = ny0 + u, nz = nz0 + v;
+                                if (ny <= used[1] && nz <= used[2]) any = cube[((size_t)nx * Y + (ny + used[1])) * Z + (nz + used[2])] >= 0;
+                            }
+                        if (any) tiles.push_back(ewald_pack(nx, ny0, nz0));
+                    }
+            int *dt = nullptr, *dc = nullptr;
+            if ((r = dupload(c, &dt, tiles)) || (r = dupload(c, &dc, cube))) return r;
+            e.tiles = dt; e.cube2k = dc; e.ntile = (int)tiles.size();
+            if ((r = dalloc(c, &e.Wt, (size_t)16 * e.ntile)) || (r = dalloc(c, &e.tabF, (size_t)E * c->n))) return r;
+            // fewer threads than k-vectors: atom chunks fill the GPU -- one wave of CTAs (4 per SM at 128 registers)
+            int dev = 0, sms = 148;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            const int nblk = (e.ntile + 127) / 128;
+            e.nch = std::max(1, std::min(std::max(1, c->n / 64), (4 * sms) / std::max(nblk, 1)));
+        }
     }
+    if ((r = dalloc(c, &e.part, (size_t)e.nch * e.nk))) return r;   // (after the pass and its number of atom chunks are chosen)
     if (!c->fslow && (r = dalloc(c, &c->fslow, (size_t)c->n))) return r;
     if (!c->ew_sum && (r = dalloc(c, &c->ew_sum, 1))) return r;
     std::vector<float4> hx;

@@ -229,7 +229,8 @@ __global__ void __launch_bounds__(RF_THREADS) k_rec_force(Model m, int nk, doubl
 // force pass (fp32 tables, one atom's table per warp) was measured slower than the direct fp32 polynomial (381 against
 // 370 us) and is not kept.
 __global__ void k_ew_tables(int n, int E, int ex, int ey, double ibx, double iby, double ibz,
-                            const float4 *__restrict__ xs, const float4 *__restrict__ xl, double2 *__restrict__ tabD) {
+                            const float4 *__restrict__ xs, const float4 *__restrict__ xl, double2 *__restrict__ tabD,
+                            float2 *__restrict__ tabF) {
     const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (g >= (long long)n * E) return;
     const int e = (int)(g / n), i = (int)(g - (long long)e * n);   // consecutive threads: consecutive atoms of one entry
@@ -240,6 +241,7 @@ __global__ void k_ew_tables(int n, int E, int ex, int ey, double ibx, double iby
                                : (dim == 1 ? ((double)h.y + (double)l.y) * iby : ((double)h.z + (double)l.z) * ibz);
     double sn, cs;
     phase_sincos_d((unsigned)a * fix_cycle(xd), sn, cs);
+    if (tabF) tabF[(size_t)i * E + e] = make_float2((float)cs, (float)sn);   // atom-major, without the charge: the force pass
     const double q = dim == 0 ? (double)h.w : 1.0;
     tabD[(size_t)e * n + i] = make_double2(q * cs, q * sn);
 }
@@ -278,6 +280,197 @@ __global__ void __launch_bounds__(SF2_THREADS) k_sfac_partial_tab(int n, int nk,
     if (k < nk) part[(size_t)blockIdx.y * nk + k] = make_double2(sr, si);
 }
 
+// Register-blocked form of the factorised pass: a thread owns a 4 x 4 tile of the (ny, nz) plane at one nx -- 16 complex
+// accumulators -- so that per atom 9 table reads (Ex, 4 Ey, 4 Ez) feed 88 fp64 operations instead of 3 reads per 10:
+// the one-term-per-thread form above is bound by its shared-memory reads.  The host lists the tiles that hold at
+// least one k-vector of the sphere (tiles[]) and maps every cube position to its place in the k list (cube2k, -1
+// outside the sphere); entries of a tile outside the sphere are computed and dropped.
+constexpr int SB_THREADS = 128;
+constexpr int SB_TA = 16;
+
+__global__ void __launch_bounds__(SB_THREADS) k_sfac_partial_blk(int n, int nk, int chunk, int E, int ex, int ey, int ntile,
+                                                               int nmy, int nmz, const double2 *__restrict__ tabD,
+                                                               const int *__restrict__ tiles, const int *__restrict__ cube2k,
+                                                               double2 *__restrict__ part) {
+    extern __shared__ double2 s_tab[];   // [SB_TA][E]
+    const int tl = blockIdx.x * SB_THREADS + threadIdx.x;
+    int nx = 0, ny0 = 0, nz0 = 0;
+    if (tl < ntile) ew_unpack(tiles[tl], nx, ny0, nz0);
+    int oy[4], oz[4];
+    double sy[4], sz[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+        const int ny = min(ny0 + u, nmy), nz = min(nz0 + u, nmz);   // (clamped entries are dropped at the end)
+        oy[u] = ex + abs(ny); sy[u] = ny < 0 ? -1.0 : 1.0;
+        oz[u] = ex + ey + abs(nz); sz[u] = nz < 0 ? -1.0 : 1.0;
+    }
+    double ar[4][4], ai[4][4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+        for (int w = 0; w < 4; ++w) { ar[u][w] = 0.0; ai[u][w] = 0.0; }
+    const int a0 = blockIdx.y * chunk, a1 = min(a0 + chunk, n);
+    for (int b = a0; b < a1; b += SB_TA) {
+        __syncthreads();
+        for (int t = threadIdx.x; t < E * SB_TA; t += SB_THREADS) {
+            const int e = t / SB_TA, j = b + (t - e * SB_TA);
+            s_tab[(t - e * SB_TA) * E + e] = j < a1 ? tabD[(size_t)e * n + j] : make_double2(0.0, 0.0);
+        }
+        __syncthreads();
+#pragma unroll 1
+        for (int t = 0; t < SB_TA; ++t) {
+            const double2 *row = s_tab + t * E;
+            const double2 a = row[nx];
+            double pr[4], pi[4], cr[4], ci[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const double2 bb = row[oy[u]];
+                const double by = sy[u] * bb.y;
+                pr[u] = fma(a.x, bb.x, -a.y * by); pi[u] = fma(a.x, by, a.y * bb.x);
+                const double2 c = row[oz[u]];
+                cr[u] = c.x; ci[u] = sz[u] * c.y;
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int w = 0; w < 4; ++w) {
+                    ar[u][w] = fma(pr[u], cr[w], fma(-pi[u], ci[w], ar[u][w]));
+                    ai[u][w] = fma(pr[u], ci[w], fma(pi[u], cr[w], ai[u][w]));
+                }
+        }
+    }
+    if (tl < ntile) {
+        const int Y = 2 * nmy + 1, Z = 2 * nmz + 1;
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int w = 0; w < 4; ++w) {
+                const int ny = ny0 + u, nz = nz0 + w;
+                if (ny > nmy || nz > nmz) continue;
+                const int k = cube2k[((size_t)nx * Y + (ny + nmy)) * Z + (nz + nmz)];
+                if (k >= 0) part[(size_t)blockIdx.y * nk + k] = make_double2(ar[u][w], ai[u][w]);
+            }
+    }
+}
+
+// Register-blocked force pass over the same 4 x 4 tiles: W = 2 A_k S(k) is laid out per tile (entry-major [16][ntile],
+// 0 outside the sphere) by k_w_tiles; one warp per atom, its fp32 phase-factor table in shared memory, lanes stride
+// over the tiles: 9 table reads and 16 W reads feed 16 terms (the one-term-per-lane polynomial form: 52 instructions
+// per term).  Sums: fp32 inside a tile (4 terms per accumulator), fp64 across tiles.
+constexpr int FB_TT = 64;      // tiles staged per pass
+constexpr int FB_EMAX = 192;
+
+__global__ void k_w_tiles(int ntile, int nmy, int nmz, const int *__restrict__ tiles, const int *__restrict__ cube2k,
+                          const double2 *__restrict__ W, float2 *__restrict__ Wt) {
+    const int g = blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= 16 * ntile) return;
+    const int e = g / ntile, tl = g - e * ntile, u = e >> 2, w = e & 3;
+    int nx, ny0, nz0;
+    ew_unpack(tiles[tl], nx, ny0, nz0);
+    const int ny = ny0 + u, nz = nz0 + w;
+    float2 v = make_float2(0.f, 0.f);
+    if (ny <= nmy && nz <= nmz) {
+        const int Y = 2 * nmy + 1, Z = 2 * nmz + 1;
+        const int k = cube2k[((size_t)nx * Y + (ny + nmy)) * Z + (nz + nmz)];
+        if (k >= 0) { const double2 ww = W[k]; v = make_float2((float)ww.x, (float)ww.y); }
+    }
+    Wt[g] = v;
+}
+
+__global__ void __launch_bounds__(RF_THREADS) k_rec_force_blk(Model m, int ntile, int E, int ex, int ey, int nmy, int nmz,
+                                                             double ibx, double iby, double ibz, double alpha,
+                                                             const float4 *__restrict__ xs, const float4 *__restrict__ xl,
+                                                             const float2 *__restrict__ tabF, const int *__restrict__ tiles,
+                                                             const float2 *__restrict__ Wt, const int *__restrict__ orig,
+                                                             const int *__restrict__ sorted_of, const int *__restrict__ excl_ptr,
+                                                             const int *__restrict__ excl_idx, float4 *__restrict__ out) {
+    __shared__ int s_tile[FB_TT];
+    __shared__ float2 s_w[16][FB_TT];
+    __shared__ float2 s_t[RF_THREADS / 32][FB_EMAX];
+    const unsigned full = 0xffffffffu;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int i = blockIdx.x * (RF_THREADS / 32) + warp;
+    const bool live = i < m.n;
+    double X = 0.0, Y = 0.0, Z = 0.0, q = 0.0;
+    if (live) {
+        const float4 h = xs[i], l = xl[i];
+        X = (double)h.x + (double)l.x; Y = (double)h.y + (double)l.y; Z = (double)h.z + (double)l.z; q = (double)h.w;
+        for (int e = lane; e < E; e += 32) s_t[warp][e] = tabF[(size_t)i * E + e];
+    }
+    const float2 *tb = s_t[warp];
+    double gx = 0.0, gy = 0.0, gz = 0.0;   // sum of term * n per dimension
+    double ew = 0.0;                        // this atom's half of its exclusion-correction energies
+    for (int b = 0; b < ntile; b += FB_TT) {
+        __syncthreads();
+        const int cnt = min(FB_TT, ntile - b);
+        for (int t = threadIdx.x; t < FB_TT; t += RF_THREADS) s_tile[t] = t < cnt ? tiles[b + t] : ew_pack(0, 0, 0);
+        for (int t = threadIdx.x; t < 16 * FB_TT; t += RF_THREADS) {
+            const int e = t / FB_TT, tl = t - e * FB_TT;
+            s_w[e][tl] = tl < cnt ? Wt[(size_t)e * ntile + b + tl] : make_float2(0.f, 0.f);
+        }
+        __syncthreads();
+        if (!live) continue;
+        for (int tl = lane; tl < cnt; tl += 32) {
+            int nx, ny0, nz0;
+            ew_unpack(s_tile[tl], nx, ny0, nz0);
+            const float2 a = tb[nx];
+            float pr[4], pi[4], cr[4], ci[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int ny = min(ny0 + u, nmy), nz = min(nz0 + u, nmz);   // (clamped entries carry W = 0)
+                float2 bb = tb[ex + abs(ny)];
+                if (ny < 0) bb.y = -bb.y;
+                pr[u] = fmaf(a.x, bb.x, -a.y * bb.y); pi[u] = fmaf(a.x, bb.y, a.y * bb.x);
+                const float2 c = tb[ex + ey + abs(nz)];
+                cr[u] = c.x; ci[u] = nz < 0 ? -c.y : c.y;
+            }
+            float Tz = 0.f, Ty = 0.f, Tx = 0.f;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                float T = 0.f;
+#pragma unroll
+                for (int w = 0; w < 4; ++w) {
+                    const float2 ww = s_w[u * 4 + w][tl];
+                    const float cs = fmaf(pr[u], cr[w], -pi[u] * ci[w]), sn = fmaf(pr[u], ci[w], pi[u] * cr[w]);   // cos, sin of k.x_i
+                    const float term = fmaf(ww.y, cs, -ww.x * sn);   // 2 A_k (Im S cos - Re S sin)
+                    T += term;
+                    Tz = fmaf(term, (float)(nz0 + w), Tz);
+                }
+                Tx += T;
+                Ty = fmaf(T, (float)(ny0 + u), Ty);
+            }
+            gx = fma((double)Tx, (double)nx, gx); gy += (double)Ty; gz += (double)Tz;
+        }
+    }
+    const double two_pi = 6.283185307179586476925;
+    gx *= q * two_pi * ibx; gy *= q * two_pi * iby; gz *= q * two_pi * ibz;   // k = 2 pi n / L
+    if (live && excl_ptr) {
+        const int o = orig[i], lo = excl_ptr[o], n_ex = excl_ptr[o + 1] - lo;
+        for (int e = lane; e < n_ex; e += 32) {
+            const int j = sorted_of[excl_idx[lo + e]];
+            const float4 h = xs[j], l = xl[j];
+            double d[3] = {X - ((double)h.x + (double)l.x), Y - ((double)h.y + (double)l.y), Z - ((double)h.z + (double)l.z)};
+            double r2 = 0.0;
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                const double L = (double)m.box[k];
+                d[k] -= L * rint(d[k] / L);
+                r2 += d[k] * d[k];
+            }
+            const double r = sqrt(r2), ar = alpha * r, qq = kCoulomb * q * (double)h.w;
+            const double du = -qq * (1.1283791670955126 * alpha * exp(-ar * ar) / r - erf(ar) / r2);
+            gx += du * d[0] / r; gy += du * d[1] / r; gz += du * d[2] / r;
+            ew -= 0.5 * qq * erf(ar) / r;
+        }
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        gx += __shfl_xor_sync(full, gx, off); gy += __shfl_xor_sync(full, gy, off); gz += __shfl_xor_sync(full, gz, off);
+        ew += __shfl_xor_sync(full, ew, off);
+    }
+    if (live && lane == 0) out[i] = make_float4((float)gx, (float)gy, (float)gz, (float)ew);
+}
+
 // sum of n doubles by one CTA in a fixed order (energy diagnostics)
 __global__ void k_sum_doubles(int n, const double *__restrict__ in, double *__restrict__ out) {
     __shared__ double s[256];
@@ -300,12 +493,26 @@ void launch_rec_force(const Model &m, const EwaldArgs &e, const float4 *xs, cons
     if (e.tabD) {   // factorised structure-factor pass (the tables fit): see k_ew_tables
         const int ex = e.nmax[0] + 1, ey = e.nmax[1] + 1, E = ex + ey + e.nmax[2] + 1;
         const long long tot = (long long)m.n * E;
-        k_ew_tables<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(m.n, E, ex, ey, ibx, iby, ibz, xs, xl, e.tabD);
-        dim3 g1((unsigned)((e.nk + SF2_THREADS - 1) / SF2_THREADS), (unsigned)e.nch);
-        k_sfac_partial_tab<<<g1, SF2_THREADS, (size_t)E * SF2_TA * sizeof(double2), st>>>(m.n, e.nk, chunk, E, ex, ey, e.tabD, e.kpack, e.part);
+        k_ew_tables<<<(unsigned)((tot + 255) / 256), 256, 0, st>>>(m.n, E, ex, ey, ibx, iby, ibz, xs, xl, e.tabD, e.tabF);
+        if (e.ntile > 0) {
+            dim3 g1((unsigned)((e.ntile + SB_THREADS - 1) / SB_THREADS), (unsigned)e.nch);
+            k_sfac_partial_blk<<<g1, SB_THREADS, (size_t)E * SB_TA * sizeof(double2), st>>>(m.n, e.nk, chunk, E, ex, ey, e.ntile, e.nmax[1],
+                                                                                          e.nmax[2], e.tabD, e.tiles, e.cube2k, e.part);
+        } else {
+            dim3 g1((unsigned)((e.nk + SF2_THREADS - 1) / SF2_THREADS), (unsigned)e.nch);
+            k_sfac_partial_tab<<<g1, SF2_THREADS, (size_t)E * SF2_TA * sizeof(double2), st>>>(m.n, e.nk, chunk, E, ex, ey, e.tabD, e.kpack, e.part);
+        }
         k_sfac_reduce<<<(e.nk + 255) / 256, 256, 0, st>>>(e.nk, e.nch, e.part, e.coefA, e.W, e.ek);
-        k_rec_force<<<(m.n + RF_THREADS / 32 - 1) / (RF_THREADS / 32), RF_THREADS, 0, st>>>(m, e.nk, ibx, iby, ibz, e.alpha, xs, xl, e.kpack,
-                                                                                             e.W, orig, sorted_of, excl_ptr, excl_idx, out);
+        if (e.ntile > 0 && e.tabF) {
+            k_w_tiles<<<(16 * e.ntile + 255) / 256, 256, 0, st>>>(e.ntile, e.nmax[1], e.nmax[2], e.tiles, e.cube2k, e.W, e.Wt);
+            k_rec_force_blk<<<(m.n + RF_THREADS / 32 - 1) / (RF_THREADS / 32), RF_THREADS, 0, st>>>(
+                m, e.ntile, E, ex, ey, e.nmax[1], e.nmax[2], ibx, iby, ibz, e.alpha, xs, xl, e.tabF, e.tiles, e.Wt, orig, sorted_of,
+                excl_ptr, excl_idx, out);
+            *launches += 1;
+        } else {
+            k_rec_force<<<(m.n + RF_THREADS / 32 - 1) / (RF_THREADS / 32), RF_THREADS, 0, st>>>(m, e.nk, ibx, iby, ibz, e.alpha, xs, xl, e.kpack,
+                                                                                                 e.W, orig, sorted_of, excl_ptr, excl_idx, out);
+        }
         *launches += 4;
         return;
     }

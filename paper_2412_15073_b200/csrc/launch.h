@@ -47,6 +47,11 @@ struct EwaldArgs {   // reciprocal Ewald sum (ewald.cu, R-21)
     double2 *W;              // [nk] 2 A_k S(k)
     double *ek;              // [nk] A_k |S(k)|^2
     int nmax[3];             // largest |n| per dimension
+    int ntile;               // register-blocked structure-factor pass: 4 x 4 (ny, nz) tiles holding a k-vector (0: not used)
+    const int *tiles;        // [ntile] packed (nx, ny0, nz0)
+    const int *cube2k;       // [(nmax_x + 1)(2 nmax_y + 1)(2 nmax_z + 1)] cube position -> index in the k list, -1 outside
+    float2 *Wt;              // [16][ntile] W in tile order (register-blocked force pass)
+    float2 *tabF;            // [n][E] fp32 phase-factor tables (register-blocked force pass)
     double2 *tabD;           // [E][n] fp64 phase-factor tables (NULL: direct sines and cosines), E = sum (nmax + 1)
 };
 
