@@ -389,17 +389,18 @@ def main():
                     e1.record(stream)
                     stream.synchronize()
                     ms_s = e0.elapsed_time(e1) / 10
-                    # algorithmic work of a term: 3 integer multiply-adds (phase), 4 integer ops
-                    # (quadrant), 1 conversion, 15 for the two polynomials and the quadrant selects, 2 (structure
-                    # factor) or 8 (force: term, three products, three sums) multiply-adds: 25 and 31, 28 on average
+                    # algorithmic work per (atom, k-vector) pair in the factorised form: structure
+                    # factor 5 fp64 multiply-adds (one complex multiply-accumulate + the amortised Ex Ey product), force 9
+                    # fp32 ones (phase product 4, term 2, sums 2, amortised 1); an fp64 multiply-add takes two slots of
+                    # the FP32-pipe peak it is reported against (the fp64 pipe runs at half rate): 19 slots x 2 flop
                     peak_tf = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-                    ach_tf = 2.0 * nk * n * 28 * 2 / (ms_s * 1e-3) / 1e12
+                    ach_tf = 1.0 * nk * n * 19 * 2 / (ms_s * 1e-3) / 1e12
                     respa1["slow_force"] = {"n_k": nk, "ms_per_evaluation": ms_s,
                                             "terms_per_s": 2.0 * nk * n / (ms_s * 1e-3),
-                                            "what": "S(k) pass + force pass, n_k half-space vectors x n atoms x 2 sincos terms",
+                                            "what": "S(k) pass + force pass, n_k half-space vectors x n atoms x 2 terms",
                                             "roofline": {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
                                                          "frac": ach_tf / peak_tf, "traffic": None,
-                                                         "algorithmic": "%d terms x 28 FP32/INT-pipe instructions x 2 flop" % (2 * nk * n),
+                                                         "algorithmic": "%d (atom, k) pairs x (5 fp64 x 2 + 9 fp32) multiply-add slots x 2 flop" % (nk * n),
                                                          "peak_source": "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (sm_max_mhz)" % (props.multi_processor_count, peaks["sm_max_mhz"])}}
                 err_r = sim_r.stats()["error"]
                 sim_r.close()
