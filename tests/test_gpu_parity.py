@@ -620,13 +620,16 @@ def test_velocity_autocorrelation_on_the_device(jb, jo, cfg0):
     assert o.step >= 10
 
 
-@pytest.mark.parametrize("direct", [False, True])
-def test_slow_force_orthorhombic_box_and_both_kernel_forms(jb, jo, direct, monkeypatch):
-    """R-21 on a box with three different edges (different n_max per dimension: the table offsets of the factorised
-    structure-factor pass) and through both forms of that pass (JUMP_B200_EWALD_DIRECT=1: direct sines and cosines);
-    a k list of 3 vectors (shorter than a tile) and an empty one."""
-    if direct:
+@pytest.mark.parametrize("form", ["blocked", "tables", "direct"])
+def test_slow_force_orthorhombic_box_and_both_kernel_forms(jb, jo, form, monkeypatch):
+    """R-21 on a box with three different edges (different n_max per dimension: the table offsets and the tile grid of
+    the factorised passes) and through every form of the two passes: register-blocked over 4 x 4 tiles (the default),
+    one term per thread on the phase-factor tables (JUMP_B200_EWALD_BLOCKED=0), direct sines and cosines
+    (JUMP_B200_EWALD_DIRECT=1); a k list of 3 vectors (shorter than a tile) and an empty one."""
+    if form == "direct":
         monkeypatch.setenv("JUMP_B200_EWALD_DIRECT", "1")
+    if form == "tables":
+        monkeypatch.setenv("JUMP_B200_EWALD_BLOCKED", "0")
     sysd = wl.small_water(5, seed=13)
     box = np.array([16.0, 18.5, 21.0])
     run = dict(wl.make_config(0)[1], r_short=4.0, r_long=7.5, r_mid=5.5, seed=9)
