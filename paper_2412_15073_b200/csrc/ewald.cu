@@ -357,7 +357,7 @@ __global__ void __launch_bounds__(SB_THREADS) k_sfac_partial_blk(int n, int nk, 
 // 0 outside the sphere) by k_w_tiles; one warp per atom, its fp32 phase-factor table in shared memory, lanes stride
 // over the tiles: 9 table reads and 16 W reads feed 16 terms (the one-term-per-lane polynomial form: 52 instructions
 // per term).  Sums: fp32 inside a tile (4 terms per accumulator), fp64 across tiles.
-constexpr int FB_TT = 64;      // tiles staged per pass
+constexpr int FB_TT = 256;     // tiles staged per pass
 constexpr int FB_EMAX = 192;
 
 __global__ void k_w_tiles(int ntile, int nmy, int nmz, const int *__restrict__ tiles, const int *__restrict__ cube2k,
