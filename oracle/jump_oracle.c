@@ -22,17 +22,26 @@
  *   - JUMP-RESPA1 / BAOAB-RESPA1 (three levels) with the reciprocal Ewald sum as the slow
  *     many-body force F_{0,1}                      P:L145, P:L509-511, P:L325 (R-21)
  *
- * Parity pins (tests/test_oracle_*.py, -m "not gpu"): Philox known-answer
+ * Parity pins (tests/test_oracle_pins.py, -m "not gpu"): Philox known-answer
  * vectors; closed forms of Theta and of the G~ CDF/mean; chi end conditions and
  * short+long = unsplit; finite differences of U; brute-force O(N^2) sums;
  * stationarity identity of (6),(7); eps=inf == BPS; eps->0 mean drift == -F/m;
- * thinning invariance under inflated bounds; OU stationary variance; BAOAB
- * energy conservation / reversibility; 2-body Boltzmann histogram; degenerate
- * cases.  "Parity unpinned" by the paper (fixed by DESIGN.md readings only):
- * the formula of chi, the bound recipe L, r_M, the list policy (skin, order),
- * the G~ proposal details, the Philox stream layout, k_cut of the reciprocal sum and
- * the outermost step ratio of RESPA1 (R-21).  The reciprocal sum itself is pinned (Madelung
- * constant of rock salt, finite differences, a closed form on one molecule).
+ * thinning invariance under inflated bounds, under the two list policies and under
+ * the two forms of the bound of Algorithm 4 (R-11); OU stationary variance; BAOAB
+ * energy conservation / reversibility; 2-body Boltzmann histogram (with and without
+ * acceleration); rows and cell universe against an independent restatement of their
+ * rules; LJ bound over a range of sigma; degenerate cases.
+ * "Parity unpinned" by the paper (fixed by DESIGN.md readings only):
+ * the formula of chi, the bound recipe L, r_A and r_M, the list policy (skin, order,
+ * cell universe), the G~ proposal details, the Philox stream layout, k_cut of the
+ * reciprocal sum and the outermost step ratio of RESPA1 (R-21).  The reciprocal sum
+ * itself is pinned (Madelung constants, finite differences, a closed form on one molecule).
+ *
+ * List policies (orc_params.list_policy): 1 = R-10c, the contract of the CUDA path: rings
+ * [r_c-h, r_A), [r_A, r_M), [r_M, r_long) by CURRENT distance, candidates from two
+ * skin-padded rows and from the cell universe; 0 = R-10 (round 1): rows M, L, V with ring
+ * membership by build-time distance.  Both are exact (thinning); the pins run
+ * both and compare their accepted jumps.
  *
  * Sign convention (R-4): every "F" here is a GRADIENT piece (grad U = sum F),
  * physical force = -F, exactly as in the paper.
@@ -69,12 +78,15 @@ enum { W_NONE = 0, W_SHORT = 1, W_LONG = 2, W_FULL = 3 };
 typedef struct {
     int32_t n_atoms, n_inner, eps_mode;
     uint32_t flags;
-    int32_t nlist_every, pad0;
+    int32_t nlist_every;
+    int32_t list_policy; /* 0: R-10 (ring rows M, L, V, ring membership by build-time distance); 1: R-10c (rings by
+                            current distance, row M, cell universe for the rings L and V) */
     uint64_t seed;
     double box[3];
     double r_short, r_switch, r_mid, r_long, ewald_alpha;
     double dt_fs, gamma_per_ps, temperature_K;
     double eps_jump, skin, cell_edge;
+    double r_mid_in; /* R-10c: r_A, inner ring edge (rings [r_c-h, r_A), [r_A, r_M), [r_M, r_long)); <= 0: r_short */
 } orc_params;
 
 typedef struct {
@@ -106,10 +118,18 @@ typedef struct {
     double *bk, *br0, *ak, *at0;
     int *excl_ptr, *excl_idx;
     /* derived */
-    double kT, beta, dt, alpha, rc, h, rM, rE, skin;
+    double kT, beta, dt, alpha, rc, h, rA, rM, rE, skin;
     double *sbm; /* sqrt(beta m_i) in ps/A */
-    double qmax, GM, GL, GV, eps_max, sig_min, sig_max;
+    double qmax, eps_max, sig_min, sig_max;
+    double GM, GL, G3;   /* sup of the long Coulomb gradient per unit charges over ring 1, 2, 3 (R-7; G3: R-10c only) */
+    double GV, GV2, GV3; /* the same for the long LJ gradient with 4 eps = 1 (R-10: GV alone, over the whole shell) */
     int gnx, gny, gnz; /* contract grid for the canonical row order */
+    int policy;        /* list policy (orc_params.list_policy) */
+    int bound_every;   /* R-11: 1 = B_v and lambda-bar re-evaluated at every proposal, as Algorithm 4 prints them */
+    /* R-10c cell universe, built at x_build: atoms of every contract cell (ascending index) and the cell of every atom */
+    int *cell_ptr, *cell_atoms, *home, *uni_cnt;
+    int uR[3];         /* reach of the universe stencil in cells, per dimension */
+    double ureach;     /* r_long + skin */
     /* rows (CSR) built at x_build */
     int *ptrM, *idxM, *ptrL, *idxL, *ptrV, *idxV;
     double *x_build;
@@ -661,31 +681,111 @@ static void compute_bounds(orc_ctx *c) {
     }
     if (c->eps_max == 0.0) { c->sig_min = 0.0; c->sig_max = 0.0; }
     double lo = c->rc - c->h;
-    c->GM = sup_coul(c, lo, dmin(c->rM + c->skin, c->rE));
-    c->GL = sup_coul(c, dmax(c->rM - c->skin, lo), c->rE);
-    c->GV = sup_lj(c, lo, c->rE);
+    c->G3 = c->GV2 = c->GV3 = 0.0;
+    if (c->policy == 1) { /* R-10c: a ring holds the pairs whose CURRENT distance lies in it */
+        const double eA = dmin(dmax(c->rA, lo), c->rE), eM = dmin(dmax(c->rM, eA), c->rE);
+        c->GM = sup_coul(c, lo, eA); c->GL = sup_coul(c, eA, eM); c->G3 = sup_coul(c, eM, c->rE);
+        /* LJ jumps: the same three rings (the ring technique of P:L422-431 applied to Algorithm 5: beyond the
+         * switching zone the long LJ gradient falls off like r^-7) */
+        c->GV = sup_lj(c, lo, eA); c->GV2 = sup_lj(c, eA, eM); c->GV3 = sup_lj(c, eM, c->rE);
+    } else {              /* R-10: rings by build-time distance, reached up to one skin beyond their edges */
+        c->GM = sup_coul(c, lo, dmin(c->rM + c->skin, c->rE));
+        c->GL = sup_coul(c, dmax(c->rM - c->skin, lo), c->rE);
+        c->GV = sup_lj(c, lo, c->rE);
+    }
 }
-/* per-atom bounds, uniform in j */
-static double LM_of(const orc_ctx *c, int i) { return fabs(c->q[i]) * c->qmax * c->GM; }
-static double LL_of(const orc_ctx *c, int i) { return fabs(c->q[i]) * c->qmax * c->GL; }
-static double LV_of(const orc_ctx *c, int i) { return 4.0 * sqrt(c->eps[i] * c->eps_max) * c->GV; }
 
-void orc_get_bounds(const orc_ctx *c, double out[8]) {
+/* GM, GL, GV: rings 1, 2 (Coulomb) and the LJ bound of R-10 / of ring 1; G3, GV2, GV3: R-10c only */
+void orc_get_bounds(const orc_ctx *c, double out[12]) {
     out[0] = c->GM; out[1] = c->GL; out[2] = c->GV; out[3] = c->qmax;
     out[4] = c->eps_max; out[5] = c->sig_min; out[6] = c->sig_max; out[7] = c->rM;
+    out[8] = c->G3; out[9] = c->GV2; out[10] = c->GV3; out[11] = c->rA;
 }
 
 /* ------------------------------------------------------------------ */
 /* ring rows (R-10)                                         */
 /* ------------------------------------------------------------------ */
+/* ---- R-10c: the cell universe of the rings L and V -------------------------------------------------------- */
+/* The contract grid has gn cells per edge (cell of an atom = floor(x gn / box), key = (cz ny + cy) nx + cx).  The
+ * universe U(h) of a home cell h = (cx, cy, cz) is the set of atoms that sat, at the last list build, in a cell
+ * (x, y, z) with cyclic offsets a = |z - cz|, b = |y - cy|, e = |x - cx| such that
+ *     a <= R_z,  b <= R_y,  rem = reach^2 - (max(a-1,0) w_z)^2 - (max(b-1,0) w_y)^2 > 0,
+ *     e <= min(R_x, floor(sqrt(rem) / w_x) + 1),         reach = r_long + skin, w = box / gn, R = ceil(reach / w):
+ * every cell some point of which lies within reach of some point of h (and a few more).  Order: ascending cell
+ * key, ascending atom index within a cell.  Any pair closer than r_long now was closer than r_long + skin at the
+ * build (no atom moves more than skin/2 between builds), so its partner is in U: a superset to draw from
+ * uniformly; entries that carry no force at the moment (too far, too close, excluded, the atom itself)
+ * are proposals with rate 0, which thinning allows. */
+static int cyc_abs(int v, int c0, int n) {
+    int o = ((v - c0) % n + n) % n;
+    return o < n - o ? o : n - o;
+}
+static int uni_xreach(const orc_ctx *c, int a, int b) {
+    const double wz = c->p.box[2] / c->gnz, wy = c->p.box[1] / c->gny, wx = c->p.box[0] / c->gnx;
+    if (a > c->uR[2] || b > c->uR[1]) return -1;
+    const double gz = (a > 1 ? a - 1 : 0) * wz, gy = (b > 1 ? b - 1 : 0) * wy;
+    const double rem = c->ureach * c->ureach - gz * gz - gy * gy;
+    if (!(rem > 0.0)) return -1;
+    int v = (int)floor(sqrt(rem) / wx) + 1;
+    return v < c->uR[0] ? v : c->uR[0];
+}
+/* k >= 0: the k-th atom of U(h) (or -1 if k >= |U(h)|); k < 0: |U(h)| */
+static int universe_walk(const orc_ctx *c, int h, int k) {
+    const int nx = c->gnx, ny = c->gny, nz = c->gnz;
+    const int cx = h % nx, cy = (h / nx) % ny, cz = h / (nx * ny);
+    int seen = 0;
+    for (int z = 0; z < nz; ++z) {
+        const int a = cyc_abs(z, cz, nz);
+        if (a > c->uR[2]) continue;
+        for (int y = 0; y < ny; ++y) {
+            const int b = cyc_abs(y, cy, ny);
+            const int xm = uni_xreach(c, a, b);
+            if (xm < 0) continue;
+            for (int x = 0; x < nx; ++x) {
+                if (cyc_abs(x, cx, nx) > xm) continue;
+                const int key = (z * ny + y) * nx + x, cnt = c->cell_ptr[key + 1] - c->cell_ptr[key];
+                if (k >= 0 && k < seen + cnt) return c->cell_atoms[c->cell_ptr[key] + (k - seen)];
+                seen += cnt;
+            }
+        }
+    }
+    return k >= 0 ? -1 : seen;
+}
+static void rebuild_universe(orc_ctx *c) {
+    const int n = c->n, ncell = c->gnx * c->gny * c->gnz;
+    free(c->cell_ptr); free(c->cell_atoms); free(c->home); free(c->uni_cnt);
+    c->cell_ptr = calloc(ncell + 1, sizeof(int));
+    c->cell_atoms = malloc(sizeof(int) * n);
+    c->home = malloc(sizeof(int) * n);
+    c->uni_cnt = malloc(sizeof(int) * ncell);
+    for (int i = 0; i < n; ++i) { c->home[i] = contract_key(c, &c->x[3 * i]); c->cell_ptr[c->home[i] + 1]++; }
+    for (int k = 0; k < ncell; ++k) c->cell_ptr[k + 1] += c->cell_ptr[k];
+    int *fill = malloc(sizeof(int) * ncell);
+    memcpy(fill, c->cell_ptr, sizeof(int) * ncell);
+    for (int i = 0; i < n; ++i) c->cell_atoms[fill[c->home[i]]++] = i; /* ascending i within a cell */
+    free(fill);
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int h = 0; h < ncell; ++h) c->uni_cnt[h] = (c->cell_ptr[h + 1] > c->cell_ptr[h]) ? universe_walk(c, h, -1) : 0;
+}
+static int universe_count(const orc_ctx *c, int i) { return c->uni_cnt[c->home[i]]; }
+
 static void rebuild_rows(orc_ctx *c) {
     free(c->ptrM); free(c->idxM); free(c->ptrL); free(c->idxL); free(c->ptrV); free(c->idxV);
+    c->ptrL = c->idxL = c->ptrV = c->idxV = NULL;
     double s = c->skin, lo = c->rc - c->h - s;
     if (lo < 0.0) lo = 0.0;
     double em = 1e300;
-    neighbor_csr_audit(c, c->x, lo, c->rM, 0, 0, &c->ptrM, &c->idxM, &em);
-    neighbor_csr_audit(c, c->x, dmax(c->rM, lo), c->rE + s, 0, 0, &c->ptrL, &c->idxL, &em);
-    neighbor_csr_audit(c, c->x, lo, c->rE + s, 1, 0, &c->ptrV, &c->idxV, &em);
+    if (c->policy == 1) {
+        /* R-10c: row A lists every pair that can be closer than r_A before the next build, row B every pair that can
+         * be in [r_A, r_M) (they overlap by one skin on each side of r_A); ring 3 draws from the cell universe */
+        neighbor_csr_audit(c, c->x, lo, c->rA + s, 0, 0, &c->ptrM, &c->idxM, &em);                     /* row A */
+        neighbor_csr_audit(c, c->x, dmax(c->rA - s, lo), c->rM + s, 0, 0, &c->ptrL, &c->idxL, &em);   /* row B */
+        rebuild_universe(c);
+    } else {
+        neighbor_csr_audit(c, c->x, lo, c->rM, 0, 0, &c->ptrM, &c->idxM, &em);
+        neighbor_csr_audit(c, c->x, dmax(c->rM, lo), c->rE + s, 0, 0, &c->ptrL, &c->idxL, &em);
+        neighbor_csr_audit(c, c->x, lo, c->rE + s, 1, 0, &c->ptrV, &c->idxV, &em);
+    }
     {   /* contract-grid cell faces (the row order depends on the cell of every atom, R-10) */
         int nn[3] = {c->gnx, c->gny, c->gnz};
         for (int i = 0; i < c->n; ++i)
@@ -709,15 +809,20 @@ static void check_displacement(orc_ctx *c) {
     }
     if (mx > c->st.max_disp) c->st.max_disp = mx;
 }
+/* R-10: rows M, L, V.  R-10c: row A, row B, the cell universe of the atom's home cell */
 void orc_get_row_counts(const orc_ctx *c, int *nM, int *nL, int *nV) {
     for (int i = 0; i < c->n; ++i) {
         nM[i] = c->ptrM[i + 1] - c->ptrM[i];
         nL[i] = c->ptrL[i + 1] - c->ptrL[i];
-        nV[i] = c->ptrV[i + 1] - c->ptrV[i];
+        nV[i] = c->policy == 1 ? universe_count(c, i) : c->ptrV[i + 1] - c->ptrV[i];
     }
 }
-/* which: 0 M, 1 L, 2 V */
 int orc_get_row(const orc_ctx *c, int which, int i, int *out, int cap) {
+    if (c->policy == 1 && which == 2) {
+        int m = universe_count(c, i);
+        for (int k = 0; k < m && k < cap; ++k) out[k] = universe_walk(c, c->home[i], k);
+        return m;
+    }
     const int *ptr = which == 0 ? c->ptrM : (which == 1 ? c->ptrL : c->ptrV);
     const int *idx = which == 0 ? c->idxM : (which == 1 ? c->idxL : c->idxV);
     int m = ptr[i + 1] - ptr[i];
@@ -763,31 +868,79 @@ void orc_reset_stats(orc_ctx *c) {
 }
 
 /* ------------------------------------------------------------------ */
-/* Step (C'): Algorithm 4 with the ring technique (R-11)               */
-/* P:L352-420.  Position x frozen; one chain per atom.     */
+/* Jump chains: Algorithm 4 with the ring technique (step C', R-11;    */
+/* P:L352-420) and Algorithm 5 (step J', BPS on the long   */
+/* LJ part, R-14).  Position x frozen; one chain per atom. */
 /* ------------------------------------------------------------------ */
-static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int stream, int64_t step,
-                         int64_t *n_prop, int64_t *n_acc, int64_t *n_gt, int64_t *n_exp, double *max_p, double *max_gl) {
+/* One ring of one atom: a set one can draw from uniformly, its size and the bound on |F_ij| over it. */
+typedef struct {
+    int kind;        /* where the candidates come from: 0 row M, 1 row L, 2 row V, 3 the cell universe (R-10c) */
+    int n;           /* number of candidates, N_Y(i) */
+    double L;        /* L_{Y,i} */
+    double rlo, rhi; /* R-10c: the pair carries its force through this ring while rlo <= r < rhi (current distance);
+                        rlo < 0 (R-10): ring membership is list membership */
+} orc_ring;
+
+/* the rings of atom i for the Coulomb (lj = 0) or the LJ (lj = 1) jumps; returns their number */
+static int rings_of(const orc_ctx *c, int i, int lj, orc_ring R[3]) {
+    const double cq = fabs(c->q[i]) * c->qmax, ce = 4.0 * sqrt(c->eps[i] * c->eps_max); /* uniform in j: P:L346, L369, L455 */
+    const int nA = c->ptrM[i + 1] - c->ptrM[i];
+    if (c->policy == 1) { /* R-10c: A = [r_c - h, r_A), B = [r_A, r_M) from the rows, L = [r_M, r_long) from the universe */
+        const int nB = c->ptrL[i + 1] - c->ptrL[i], nU = universe_count(c, i);
+        R[0] = (orc_ring){0, nA, lj ? ce * c->GV : cq * c->GM, c->rc - c->h, c->rA};
+        R[1] = (orc_ring){1, nB, lj ? ce * c->GV2 : cq * c->GL, c->rA, c->rM};
+        R[2] = (orc_ring){3, nU, lj ? ce * c->GV3 : cq * c->G3, c->rM, c->rE};
+        return 3;
+    }
+    if (lj) { R[0] = (orc_ring){2, c->ptrV[i + 1] - c->ptrV[i], ce * c->GV, -1.0, 0.0}; return 1; }
+    R[0] = (orc_ring){0, nA, cq * c->GM, -1.0, 0.0};
+    R[1] = (orc_ring){1, c->ptrL[i + 1] - c->ptrL[i], cq * c->GL, -1.0, 0.0};
+    return 2;
+}
+static int ring_candidate(const orc_ctx *c, int i, const orc_ring *R, int k) {
+    switch (R->kind) {
+        case 0: return c->idxM[c->ptrM[i] + k];
+        case 1: return c->idxL[c->ptrL[i] + k];
+        case 2: return c->idxV[c->ptrV[i] + k];
+        default: return universe_walk(c, c->home[i], k);
+    }
+}
+
+/* lj = 0: step (C') for atom i, general mechanism (6),(7) with eps (or BPS, eps = inf), acceleration a between
+ * proposals.  lj = 1: step (J'), BPS (4),(5) on the long LJ part, a = 0 (the caller passes zeros): the same loop
+ * with the constant bound beta |v| sum N_Y L_Y (|v| is preserved by reflections), so that the number of
+ * proposals is Poisson as Algorithm 5 asks (R-14).
+ * Draws of a proposal, from one Philox block (R-15): E, ring, k, U; G~ attempts draw from stream + 16. */
+static void chain_atom(orc_ctx *c, int i, int lj, double H, const double a[3], int stream, int64_t step,
+                       int64_t *n_prop, int64_t *n_acc, int64_t *n_gt, int64_t *n_exp, double *max_p, double *max_gl) {
+    if (lj && !(c->eps[i] > 0.0)) return; /* no LJ on this atom: no chain */
     double *v = &c->v[3 * i];
-    const double eps = c->p.eps_jump, sbm = c->sbm[i], beta = c->beta;
+    const double eps = lj ? INFINITY : c->p.eps_jump, sbm = c->sbm[i], beta = c->beta;
     const int bps = isinf(eps);
     /* R-19 (NEXT-1): eps_mode 1 = adaptive eps(x) = eps0 |F_ij(x)|, eps0 = eps_jump.  With
      * g = |F_ij| <= L_Y, eta = eps0 g sqrt(beta m)(v.n) and Theta(eta) <= eta_+ + 1/sqrt(2 pi) the pair rate
      * lambda_ij = sqrt(beta) Theta(eta) / (eps0 sqrt(m)) (P:L340 with eps = eps0 g) is bounded, uniformly in j, by
      * lambda*_Y = beta L_Y B_v + (1/eps0) sqrt(beta / (2 pi m)); p = lambda_ij / lambda*_Y. */
     const int adaptive = c->p.eps_mode == 1 && !bps;
-    const int NM = c->ptrM[i + 1] - c->ptrM[i], NL = c->ptrL[i + 1] - c->ptrL[i];
-    const double LM = LM_of(c, i), LL = LL_of(c, i);
-    const double SM = (double)NM * LM, S = SM + (double)NL * LL;
+    orc_ring R[3];
+    const int nr = rings_of(c, i, lj, R);
+    double S = 0.0; /* sum_Y N_Y L_Y */
+    int ntot = 0;
+    for (int y = 0; y < nr; ++y) { S += (double)R[y].n * R[y].L; ntot += R[y].n; }
+    if (lj && !(S > 0.0)) return; /* (J') without a partner: nothing to log, as under Algorithm 5 with N = 0 */
     double t = 0.0;
     uint32_t block = 0;  /* proposal k of the chain draws Philox block k of its stream ...                     */
     uint32_t gblock = 0; /* ... and the G~ attempts draw blocks 0, 1, ... of stream + 16 (R-15)                 */
     uint32_t w[4];
-    /* R-11: the bound is "re-evaluated after each jump": B_v bounds |v_i| on the whole of [t, delta/2]
-     * (P:L373), so it and lambda-bar are evaluated at t = 0 and after every ACCEPTED jump and held in between. */
+    /* R-11: Algorithm 4 prints B_v and lambda-bar inside the loop, i.e. re-evaluated at every proposal;
+     * P:L161 says local bounds "need to be re-evaluated after each jump".  B_v bounds |v_i| on the whole of
+     * [t, delta/2] and between two accepted jumps v_i only drifts with a_i, so the bound evaluated at t = 0
+     * or after an ACCEPTED jump stays valid until the next accepted jump: by default (bound_every = 0) it is held in
+     * between ("epoch" form: looser, hence a few more proposals, the same law by P:L157); bound_every = 1 is the
+     * literal per-proposal form (orc_set_bound_mode; tests/test_oracle_pins.py compares the two). */
     int fresh = 1;
     double Bv = 0.0, lam = 0.0;
-    double ringM = SM, ringS = S; /* ring M is picked with probability ringM / ringS */
+    double wgt[3] = {0.0, 0.0, 0.0}; /* ring Y is picked with probability wgt[Y] / sum wgt */
     const double lam0 = bps ? 0.0 : (1.0 / eps) * beta * ORC_INV_SQRT_2PI / sbm; /* (1/eps) sqrt(beta/(2 pi m)) */
     const double a2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
     for (int iter = 0;; ++iter) {
@@ -796,16 +949,18 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
         ev.step = (int32_t)step; ev.stream = stream; ev.atom = i; ev.iter = iter; ev.ring = -1; ev.j = -1;
         double mg = 1e300;
         double tau = H - t;
-        if (fresh) {
+        if (fresh || c->bound_every) {
             double va = v[0] * a[0] + v[1] * a[1] + v[2] * a[2];
             double v2 = v[0] * v[0] + v[1] * v[1] + v[2] * v[2];
             Bv = sqrt(v2 + tau * tau * a2 + 2.0 * tau * (va > 0.0 ? va : 0.0)); /* P:L373 */
-            if (!(S > 0.0)) lam = 0.0; /* no partner, or an uncharged atom: no mechanism */
-            else if (adaptive) {        /* sum over the listed pairs of lambda*_Y (R-19) */
-                ringM = (double)NM * (beta * LM * Bv + lam0);
-                lam = ringM + (double)NL * (beta * LL * Bv + lam0);
-                ringS = lam;
-            } else lam = S * (beta * Bv + lam0); /* P:L374 */
+            lam = 0.0;
+            for (int y = 0; y < nr; ++y) {
+                if (!(S > 0.0)) wgt[y] = 0.0; /* no partner, or an uncharged atom: no mechanism */
+                else if (adaptive) wgt[y] = (double)R[y].n * (beta * R[y].L * Bv + lam0); /* sum of lambda*_Y (R-19) */
+                else wgt[y] = (double)R[y].n * R[y].L;
+                lam += wgt[y];
+            }
+            if (!adaptive) lam *= beta * Bv + lam0; /* P:L374; (J'): beta |v| sum N_Y L_Y, P:L457, L476 */
             fresh = 0;
         }
         chain_block(c, i, step, stream, block++, w);
@@ -822,29 +977,45 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
         }
         t += T; /* P:L388-390 */
         v[0] += T * a[0]; v[1] += T * a[1]; v[2] += T * a[2];
-        /* ring pick, P:L426-428 */
-        double ur = orc_u01(w[1]);
-        int ring;
-        if (NM > 0 && NL > 0) mg = upd(mg, ur - ringM / ringS);
-        ring = (ur * ringS < ringM) ? 0 : 1;
-        if (ring == 0 && NM == 0) ring = 1;
-        if (ring == 1 && NL == 0) ring = 0;
-        int cnt = ring == 0 ? NM : NL;
-        int k = (int)(((uint64_t)w[2] * (uint64_t)cnt) >> 32);
-        int j = ring == 0 ? c->idxM[c->ptrM[i] + k] : c->idxL[c->ptrL[i] + k];
-        double LY = ring == 0 ? LM : LL;
+        /* ring pick, P:L426-428: the first ring whose cumulated weight exceeds ur * (sum of weights) */
+        double ur = orc_u01(w[1]), wsum = 0.0, cum = 0.0;
+        for (int y = 0; y < nr; ++y) wsum += wgt[y];
+        int ring = 0;
+        for (int y = 0; y < nr; ++y) {
+            cum += wgt[y];
+            ring = y;
+            if (y < nr - 1 && wgt[y] > 0.0) mg = upd(mg, ur - cum / wsum);
+            if (ur * wsum < cum) break;
+        }
+        while (R[ring].n == 0 && ring > 0) --ring; /* (rounding at the upper end: fall back to a ring that has entries) */
+        while (R[ring].n == 0 && ring < nr - 1) ++ring;
+        int k = (int)(((uint64_t)w[2] * (uint64_t)R[ring].n) >> 32);
+        int j = ring_candidate(c, i, &R[ring], k);
+        double LY = R[ring].L;
         double U = orc_u01(w[3]);
-        ev.ring = ring; ev.j = j; ev.U = U;
+        ev.ring = (lj ? 4 : 0) + ring; ev.j = j; ev.U = U;
         (*n_prop)++;
         double F[3];
-        double g = fij_coul(c, i, j, F);
+        double g = 0.0;
+        if (R[ring].rlo < 0.0) g = lj ? fij_lj(c, i, j, F) : fij_coul(c, i, j, F); /* R-10 */
+        else if (j != i && !(R[ring].kind == 3 && is_excluded(c, i, j))) {
+            /* R-10c: the pair carries its force through the ring its CURRENT distance lies in (P:L424); drawn
+             * through another ring it has rate 0 -- every pair is counted exactly once.  The universe also holds
+             * the atom itself and its excluded partners: rate 0 (the rows never list them, R-9). */
+            double d[3];
+            min_image(c, &c->x[3 * i], &c->x[3 * j], d);
+            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            mg = upd(mg, r - R[ring].rlo);
+            mg = upd(mg, r - R[ring].rhi);
+            if (r >= R[ring].rlo && r < R[ring].rhi) g = lj ? fij_lj(c, i, j, F) : fij_coul(c, i, j, F);
+        }
         if (g > 0.0) {
             if (g / LY > *max_gl) *max_gl = g / LY;
             double n[3] = {F[0] / g, F[1] / g, F[2] / g};
             double vn = v[0] * n[0] + v[1] * n[1] + v[2] * n[2];
             double p;
             const double eps_ij = adaptive ? eps * g : eps; /* P:L100: eps(x) = eps0 |F_ij(x)| */
-            if (bps) p = (vn > 0.0 ? vn : 0.0) * g / (LY * Bv);
+            if (bps) p = (vn > 0.0 ? vn : 0.0) * g / (LY * Bv); /* (4) over the bound; (J'): P:L486 with B_v = |v| */
             else if (adaptive) p = orc_theta(eps_ij * sbm * vn) / (eps * sbm * LY * Bv + ORC_INV_SQRT_2PI); /* R-19 */
             else p = g * orc_theta(eps * sbm * vn) / (LY * (Bv * eps * sbm + ORC_INV_SQRT_2PI)); /* P:L397 + sqrt(beta) */
             ev.p = p;
@@ -854,7 +1025,7 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
                 double gt = 0.0;
                 int att = 0;
                 if (!bps) gt = orc_gtilde(c, eps_ij * sbm * vn, i, step, stream + 16, &gblock, &att, &mg);
-                orc_jump_kick(eps_ij, sbm, n, gt, v); /* P:L406 */
+                orc_jump_kick(eps_ij, sbm, n, gt, v); /* P:L406; eps = inf: reflection (5) */
                 ev.accepted = 1; ev.gt = gt; ev.n_gt = att;
                 (*n_acc)++;
                 (*n_gt) += att;
@@ -864,56 +1035,7 @@ static void chain_C_atom(orc_ctx *c, int i, double H, const double a[3], int str
         ev.margin = mg;
         log_event(c, &ev);
     }
-}
-
-/* Step (J'): Algorithm 5 (BPS on the long LJ part), exponential clock (R-14). P:L466-505 */
-static void chain_J_atom(orc_ctx *c, int i, double H, int stream, int64_t step,
-                         int64_t *n_prop, int64_t *n_acc, int64_t *n_exp, double *max_p, double *max_gl) {
-    const int NV = c->ptrV[i + 1] - c->ptrV[i];
-    if (!(c->eps[i] > 0.0) || NV == 0) return;
-    double *v = &c->v[3 * i];
-    const double L = LV_of(c, i);
-    double t = 0.0;
-    uint32_t block = 0;
-    uint32_t w[4];
-    for (int iter = 0;; ++iter) {
-        orc_event ev;
-        memset(&ev, 0, sizeof ev);
-        ev.step = (int32_t)step; ev.stream = stream; ev.atom = i; ev.iter = iter; ev.ring = -1; ev.j = -1;
-        double mg = 1e300;
-        double vv = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
-        double lam = (double)NV * c->beta * vv * L;
-        chain_block(c, i, step, stream, block++, w);
-        double E = -log(orc_u01(w[0]));
-        double T = lam > 0.0 ? E / lam : INFINITY;
-        ev.T = T;
-        if (isfinite(T)) mg = upd(mg, (t + T - H) / H);
-        if (t + T > H) { ev.margin = mg; (*n_exp)++; log_event(c, &ev); break; }
-        t += T;
-        int k = (int)(((uint64_t)w[1] * (uint64_t)NV) >> 32);
-        int j = c->idxV[c->ptrV[i] + k];
-        double U = orc_u01(w[2]);
-        ev.ring = 2; ev.j = j; ev.U = U;
-        (*n_prop)++;
-        double F[3];
-        double g = fij_lj(c, i, j, F);
-        if (g > 0.0) {
-            if (g / L > *max_gl) *max_gl = g / L;
-            double vF = v[0] * F[0] + v[1] * F[1] + v[2] * F[2];
-            double p = (vF > 0.0 ? vF : 0.0) / (vv * L);
-            ev.p = p;
-            if (p > *max_p) *max_p = p;
-            mg = upd(mg, U - p);
-            if (U <= p) { /* reflection (5) */
-                double n[3] = {F[0] / g, F[1] / g, F[2] / g};
-                orc_jump_kick(INFINITY, c->sbm[i], n, 0.0, v);
-                ev.accepted = 1;
-                (*n_acc)++;
-            }
-        }
-        ev.margin = mg;
-        log_event(c, &ev);
-    }
+    (void)ntot;
 }
 
 /* C over all atoms; acc_src: gradient array giving a = -M^-1 F (NULL -> a = 0) */
@@ -925,17 +1047,18 @@ static void phase_C(orc_ctx *c, double H, const double *grad, int stream, int64_
         double a[3] = {0, 0, 0};
         if (grad)
             for (int k = 0; k < 3; ++k) a[k] = -(ORC_KCAL / c->m[i]) * grad[3 * i + k]; /* P:L364 */
-        chain_C_atom(c, i, H, a, stream, step, &np, &nacc, &ngt, &nexp, &mp, &mgl);
+        chain_atom(c, i, 0, H, a, stream, step, &np, &nacc, &ngt, &nexp, &mp, &mgl);
     }
     c->st.proposals += np; c->st.accepts += nacc; c->st.gt_attempts += ngt; c->st.expiries += nexp;
     if (mp > c->st.max_p) c->st.max_p = mp;
     if (mgl > c->st.max_g_over_L) c->st.max_g_over_L = mgl;
 }
 static void phase_J(orc_ctx *c, double H, int stream, int64_t step) {
-    int64_t np = 0, nacc = 0, nexp = 0;
+    int64_t np = 0, nacc = 0, ngt = 0, nexp = 0;
     double mp = 0.0, mgl = 0.0;
-#pragma omp parallel for schedule(dynamic, 64) reduction(+ : np, nacc, nexp) reduction(max : mp, mgl)
-    for (int i = 0; i < c->n; ++i) chain_J_atom(c, i, H, stream, step, &np, &nacc, &nexp, &mp, &mgl);
+    const double zero[3] = {0.0, 0.0, 0.0};
+#pragma omp parallel for schedule(dynamic, 64) reduction(+ : np, nacc, ngt, nexp) reduction(max : mp, mgl)
+    for (int i = 0; i < c->n; ++i) chain_atom(c, i, 1, H, zero, stream, step, &np, &nacc, &ngt, &nexp, &mp, &mgl);
     c->st.proposals += np; c->st.accepts += nacc; c->st.expiries += nexp;
     if (mp > c->st.max_p) c->st.max_p = mp;
     if (mgl > c->st.max_g_over_L) c->st.max_g_over_L = mgl;
@@ -1220,12 +1343,21 @@ orc_ctx *orc_create(const orc_params *p, const double *pos, const double *vel, c
     c->alpha = p->ewald_alpha < 0.0 ? 3.8 / p->r_long : p->ewald_alpha; /* R-2 */
     /* r_mid <= 0: no ring, M is empty and L covers the whole shell */
     c->rM = p->r_mid > 0.0 ? p->r_mid : dmax(c->rc - c->h - c->skin, 0.0);
+    c->rA = p->r_mid_in > 0.0 ? p->r_mid_in : c->rc; /* R-10c: ring A = the switching zone by default */
+    if (c->rA > c->rM) c->rA = c->rM;
     c->sbm = malloc(sizeof(double) * n);
     for (int i = 0; i < n; ++i) c->sbm[i] = sqrt(c->m[i] / (c->kT * ORC_KCAL));
     double edge = p->cell_edge > 0.0 ? p->cell_edge : (p->r_long + p->skin) / 4.0;
     c->gnx = (int)floor(p->box[0] / edge); if (c->gnx < 1) c->gnx = 1;
     c->gny = (int)floor(p->box[1] / edge); if (c->gny < 1) c->gny = 1;
     c->gnz = (int)floor(p->box[2] / edge); if (c->gnz < 1) c->gnz = 1;
+    c->policy = p->list_policy == 1 ? 1 : 0;
+    if (c->policy == 1 && !(p->r_mid > 0.0)) c->rM = c->rA; /* no ring split asked for: rings A and the universe */
+    c->ureach = p->r_long + p->skin;
+    {
+        int nn[3] = {c->gnx, c->gny, c->gnz};
+        for (int k = 0; k < 3; ++k) c->uR[k] = (int)ceil(c->ureach / (p->box[k] / nn[k]));
+    }
     c->x_build = malloc(sizeof(double) * 3 * n);
     c->f_bond = calloc(3 * n, sizeof(double));
     c->f_nb = calloc(3 * n, sizeof(double));
@@ -1245,6 +1377,7 @@ void orc_free(orc_ctx *c) {
     free(c->excl_ptr); free(c->excl_idx); free(c->sbm); free(c->x_build);
     free(c->ptrM); free(c->idxM); free(c->ptrL); free(c->idxL); free(c->ptrV); free(c->idxV);
     free(c->f_bond); free(c->f_nb); free(c->f0); free(c->f_long); free(c->ev); free(c->kn); free(c->f_slow);
+    free(c->cell_ptr); free(c->cell_atoms); free(c->home); free(c->uni_cnt);
     free(c);
 }
 /* which: 0 wrapped x, 1 v, 2 unwrapped x */
@@ -1261,7 +1394,9 @@ void orc_set_state(orc_ctx *c, const double *x, const double *v, int rebuild) {
 }
 int64_t orc_get_step(const orc_ctx *c) { return c->step; }
 void orc_set_eps(orc_ctx *c, double eps) { c->p.eps_jump = eps; }
-void orc_scale_bounds(orc_ctx *c, double f) { c->GM *= f; c->GL *= f; c->GV *= f; } /* thinning-invariance pin */
+/* R-11: 0 = bound held between accepted jumps (default), 1 = re-evaluated at every proposal (Algorithm 4 as printed) */
+void orc_set_bound_mode(orc_ctx *c, int every_proposal) { c->bound_every = every_proposal ? 1 : 0; }
+void orc_scale_bounds(orc_ctx *c, double f) { c->GM *= f; c->GL *= f; c->G3 *= f; c->GV *= f; c->GV2 *= f; c->GV3 *= f; } /* thinning-invariance pin */
 int orc_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -34,12 +34,12 @@ def build(force=False):
 class Params(C.Structure):
     _fields_ = [
         ("n_atoms", C.c_int32), ("n_inner", C.c_int32), ("eps_mode", C.c_int32), ("flags", C.c_uint32),
-        ("nlist_every", C.c_int32), ("pad0", C.c_int32), ("seed", C.c_uint64),
+        ("nlist_every", C.c_int32), ("list_policy", C.c_int32), ("seed", C.c_uint64),
         ("box", C.c_double * 3),
         ("r_short", C.c_double), ("r_switch", C.c_double), ("r_mid", C.c_double), ("r_long", C.c_double),
         ("ewald_alpha", C.c_double),
         ("dt_fs", C.c_double), ("gamma_per_ps", C.c_double), ("temperature_K", C.c_double),
-        ("eps_jump", C.c_double), ("skin", C.c_double), ("cell_edge", C.c_double),
+        ("eps_jump", C.c_double), ("skin", C.c_double), ("cell_edge", C.c_double), ("r_mid_in", C.c_double),
     ]
 
 
@@ -103,6 +103,7 @@ def lib():
         L.orc_get_step.restype = C.c_int64
         L.orc_set_eps.argtypes = [C.c_void_p, C.c_double]
         L.orc_scale_bounds.argtypes = [C.c_void_p, C.c_double]
+        L.orc_set_bound_mode.argtypes = [C.c_void_p, C.c_int]
         L.orc_jump_half.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_int64]
         L.orc_ewald_setup.argtypes = [C.c_void_p, C.c_double]
         L.orc_ewald_nk.argtypes = [C.c_void_p]
@@ -143,17 +144,19 @@ def _ip(a):
 
 def make_params(n_atoms, box, r_short, r_long, r_switch=0.5, r_mid=None, ewald_alpha=-1.0, dt_fs=1.0,
                 gamma_per_ps=1.0, temperature_K=300.0, n_inner=4, eps_jump=1.0, eps_mode=0,
-                flags=F_COUL_JUMPS | F_LJ_JUMPS, skin=1.0, nlist_every=10, seed=0, cell_edge=0.0, **_ignored):
+                flags=F_COUL_JUMPS | F_LJ_JUMPS, skin=1.0, nlist_every=10, seed=0, cell_edge=0.0, list_policy=1,
+                r_mid_in=0.0, **_ignored):
+    """list_policy 1 (default, the contract of the CUDA path): DESIGN.md R-10c; 0: the ring rows of R-10."""
     p = Params()
     p.n_atoms, p.n_inner, p.eps_mode, p.flags = int(n_atoms), int(n_inner), int(eps_mode), int(flags)
-    p.nlist_every, p.seed = int(nlist_every), int(seed)
+    p.nlist_every, p.seed, p.list_policy = int(nlist_every), int(seed), int(list_policy)
     b = np.broadcast_to(np.asarray(box, dtype=np.float64), (3,))
     p.box[0], p.box[1], p.box[2] = float(b[0]), float(b[1]), float(b[2])
     p.r_short, p.r_switch, p.r_long = float(r_short), float(r_switch), float(r_long)
     p.r_mid = float(r_short + 2.0 if r_mid is None else r_mid)
     p.ewald_alpha = float(ewald_alpha)
     p.dt_fs, p.gamma_per_ps, p.temperature_K = float(dt_fs), float(gamma_per_ps), float(temperature_K)
-    p.eps_jump, p.skin, p.cell_edge = float(eps_jump), float(skin), float(cell_edge)
+    p.eps_jump, p.skin, p.cell_edge, p.r_mid_in = float(eps_jump), float(skin), float(cell_edge), float(r_mid_in)
     return p
 
 
@@ -278,9 +281,9 @@ class Oracle:
         lib().orc_reset_stats(self._h)
 
     def bounds(self):
-        out = np.empty(8, dtype=np.float64)
+        out = np.empty(12, dtype=np.float64)
         lib().orc_get_bounds(self._h, _dp(out))
-        return dict(zip(["GM", "GL", "GV", "qmax", "eps_max", "sig_min", "sig_max", "rM"], out.tolist()))
+        return dict(zip(["GM", "GL", "GV", "qmax", "eps_max", "sig_min", "sig_max", "rM", "G3", "GV2", "GV3", "rA"], out.tolist()))
 
     def row_counts(self):
         a = [np.empty(self.n, dtype=np.int32) for _ in range(3)]
@@ -310,6 +313,10 @@ class Oracle:
 
     def scale_bounds(self, f):
         lib().orc_scale_bounds(self._h, float(f))
+
+    def set_bound_mode(self, every_proposal):
+        """R-11: False = bound held between accepted jumps (default); True = Algorithm 4 as printed (every proposal)."""
+        lib().orc_set_bound_mode(self._h, int(bool(every_proposal)))
 
 
 # --- stand-alone functions used by the pins ---------------------------------

@@ -291,16 +291,19 @@ def test_neighbor_search_matches_brute_force(cfg0):
         assert np.array_equal(p1, p2) and np.array_equal(i1, i2)
 
 
+def _contract_keys(x, box, edge):
+    ng = np.maximum(1, np.floor(np.broadcast_to(box, (3,)) / edge).astype(int))
+    cell = np.minimum(np.floor(x * (ng / box)).astype(int), ng - 1)
+    return ng, cell, (cell[:, 2] * ng[1] + cell[:, 1]) * ng[0] + cell[:, 0]
+
+
 def test_ring_rows_contract(cfg0):
-    """R-10: M = [rc-h-s, rM), L = [rM, rlong+s), V = LJ pairs of the shell; ascending (cell key, index)."""
+    """R-10 (list_policy 0): M = [rc-h-s, rM), L = [rM, rlong+s), V = LJ pairs of the shell; ascending (cell key, index)."""
     sysd, run = cfg0
-    o = jo.Oracle(sysd, **run)
+    o = jo.Oracle(sysd, **dict(run, list_policy=0))
     x = sysd["pos"]; L = sysd["box"]; n = o.n
     rc, h, s, rM, rl = run["r_short"], run["r_switch"], run["skin"], run["r_mid"], run["r_long"]
-    edge = (rl + s) / 4
-    ng = max(1, int(math.floor(L / edge)))
-    cell = np.minimum(np.floor(x * (ng / L)).astype(int), ng - 1)
-    key = (cell[:, 2] * ng + cell[:, 1]) * ng + cell[:, 0]
+    _, _, key = _contract_keys(x, L, (rl + s) / 4)
     d = x[:, None, :] - x[None, :, :]
     d -= L * np.round(d / L)
     r = np.sqrt((d ** 2).sum(-1))
@@ -320,25 +323,178 @@ def test_ring_rows_contract(cfg0):
     assert nV[1::3].max() == 0 and nV[::3].min() > 0     # LJ rows on oxygens only
 
 
-def test_bounds_dominate_every_listed_pair(cfg0):
+@pytest.mark.parametrize("case", ["cfg0", "wide", "ortho"])
+def test_rows_and_cell_universe_contract(cfg0, case):
+    """R-10c (list_policy 1, the contract of the CUDA path): row A = [rc-h-s, rA+s), row B = [rA-s, rM+s) by build-time
+    distance, excluded pairs never listed, ascending (cell key, index); ring 3 draws from the cell universe of the
+    atom's home cell: the atoms of every contract cell within reach r_long + s of the home cell by the rule typed out
+    below (an independent restatement), ascending (cell key, index), the atom itself and its excluded partners
+    included.  And the property the thinning needs: every pair closer than r_long + s is in the universe."""
     sysd, run = cfg0
-    o = jo.Oracle(sysd, **run)
+    if case == "wide":       # a box several stencils wide: the universe is a proper subset of the box
+        sysd = wl.small_water(7, seed=4)                 # 1029 atoms, 31.3 A
+        run = dict(run, r_short=4.0, r_long=5.5, r_mid=5.0, r_mid_in=4.25, skin=0.5, cell_edge=2.0)
+    if case == "ortho":
+        sysd = dict(wl.small_water(5, seed=13), box=np.array([16.0, 18.5, 21.0]))
+        run = dict(run, r_short=4.0, r_long=7.5, r_mid=5.5, r_mid_in=4.5)
+    o = jo.Oracle(sysd, **dict(run, list_policy=1))
+    x = np.mod(sysd["pos"], sysd["box"]); n = o.n
+    box = np.broadcast_to(np.asarray(sysd["box"], float), (3,))
+    rc, h, s, rM, rl = run["r_short"], run["r_switch"], run["skin"], run["r_mid"], run["r_long"]
+    rA = run.get("r_mid_in", 0.0) or rc
+    edge = run.get("cell_edge", 0.0) or (rl + s) / 4
+    ng, cell, key = _contract_keys(x, box, edge)
+    d = x[:, None, :] - x[None, :, :]
+    d -= box * np.round(d / box)
+    r = np.sqrt((d ** 2).sum(-1))
+    nA, nB, nU = o.row_counts()
+    w = box / ng
+    reach = rl + s
+    R = np.ceil(reach / w).astype(int)
+
+    def cyc(a, b, m):
+        o_ = (a - b) % m
+        return min(o_, m - o_)
+
+    def in_universe(ci, cj):
+        a, b, e = cyc(cj[2], ci[2], ng[2]), cyc(cj[1], ci[1], ng[1]), cyc(cj[0], ci[0], ng[0])
+        if a > R[2] or b > R[1]:
+            return False
+        rem = reach ** 2 - (max(a - 1, 0) * w[2]) ** 2 - (max(b - 1, 0) * w[1]) ** 2
+        return rem > 0 and e <= min(R[0], int(math.floor(math.sqrt(rem) / w[0])) + 1)
+
+    lo = max(rc - h - s, 0.0)
+    for i in (0, 1, 2, 100, 331, n - 1):
+        excl = set(sysd["excl_idx"][sysd["excl_ptr"][i]:sysd["excl_ptr"][i + 1]].tolist()) | {i}
+        for which, lo_, hi_ in ((0, lo, rA + s), (1, max(rA - s, lo), rM + s)):
+            want = [j for j in range(n) if j not in excl and lo_ <= r[i, j] < hi_]
+            want.sort(key=lambda j: (key[j], j))
+            assert o.row(which, i).tolist() == want
+        want = [j for j in range(n) if in_universe(cell[i], cell[j])]
+        want.sort(key=lambda j: (key[j], j))
+        got = o.row(2, i).tolist()
+        assert got == want and len(got) == nU[i]
+        assert set(np.nonzero(r[i] < reach)[0].tolist()) <= set(got)       # superset of everything within reach
+    if case == "wide":
+        assert nU.max() < n                                                 # a proper subset
+
+
+@pytest.mark.parametrize("policy", [0, 1])
+def test_list_policies_give_the_same_accepted_jumps(relaxed_small, policy):
+    """R-10 and R-10c list the candidate pairs differently (rows by build-time distance / rings by current distance with
+    the cell universe) and so propose differently, but thinning makes the ACCEPTED jumps of every pair the same Poisson
+    process: accepted events per chain and the mean kick agree between the two policies (frozen x, many
+    replicas of one half-step), for the Coulomb and the LJ mechanism.  Run for policy 1 against the reference policy 0."""
+    if policy == 0:
+        pytest.skip("reference arm")
+    sysd, kw = _frozen(relaxed_small, flags=1 | 2 | 4, eps_jump=1.0, skin=0.5, nlist_every=10 ** 9)
+    res = []
+    R = 1200
+    for pol in (0, 1):
+        o = jo.Oracle(sysd, **dict(kw, list_policy=pol))
+        v0 = o.vel
+        dv = np.zeros_like(v0)
+        accC = accJ = 0
+        for rep in range(R):
+            o.set_vel(v0)
+            o.clear_events()
+            o.jump_half(4e-3, with_accel=False, step=rep + 50000 * pol)
+            ev = o.events()
+            accC += int(((ev["accepted"] == 1) & (ev["stream"] == 1)).sum())
+            accJ += int(((ev["accepted"] == 1) & (ev["stream"] == 2)).sum())
+            dv += o.vel - v0
+        st = o.stats()
+        assert st["max_p"] <= 1.0 and st["max_g_over_L"] <= 1.0
+        res.append((st["proposals"] / R, accC / R, accJ / R, dv / R))
+    (p0, c0, j0, d0), (p1, c1, j1, d1) = res
+    assert abs(c1 / c0 - 1.0) < 5 * math.sqrt(2 / (c0 * R)) and c0 * R > 3000
+    assert abs(j1 / j0 - 1.0) < 5 * math.sqrt(2 / (j0 * R)) and j0 * R > 100
+    o = jo.Oracle(sysd, **kw)
+    pred = -4e-3 * KCAL * o.forces(2) / sysd["mass"][:, None]
+    proj = [(d * pred).sum() / (pred * pred).sum() for d in (d0, d1)]
+    assert abs(proj[0] - proj[1]) < 0.3 and min(proj) > 0.3
+
+
+@pytest.mark.parametrize("policy", [0, 1])
+def test_bounds_dominate_every_listed_pair(cfg0, policy):
+    sysd, run = cfg0
+    o = jo.Oracle(sysd, **dict(run, list_policy=policy))
     b = o.bounds()
     q = sysd["charge"]
     rng = np.random.default_rng(3)
     worst = 0.0
+    x = sysd["pos"]; L = sysd["box"]
+    rc, h = run["r_short"], run["r_switch"]
+    edges = (rc - h, b["rA"], b["rM"], run["r_long"])
     for i in rng.choice(o.n, size=40, replace=False):
-        for which, G in ((0, b["GM"]), (1, b["GL"])):
+        if policy == 0:
+            for which, G in ((0, b["GM"]), (1, b["GL"])):
+                for j in o.row(which, int(i)):
+                    g, _ = o.fij(0, int(i), int(j))
+                    worst = max(worst, g / (abs(q[i]) * b["qmax"] * G))
+            for j in o.row(2, int(i)):
+                g, _ = o.fij(1, int(i), int(j))
+                worst = max(worst, g / (4 * math.sqrt(sysd["lj_eps"][i] * b["eps_max"]) * b["GV"]))
+            continue
+        # R-10c: a candidate carries its force through the ring its CURRENT distance lies in
+        for which, G, GV in ((0, b["GM"], b["GV"]), (1, b["GL"], b["GV2"]), (2, b["G3"], b["GV3"])):
             for j in o.row(which, int(i)):
+                if j == i:
+                    continue
+                d = x[i] - x[j]; d -= L * np.round(d / L)
+                r = math.sqrt((d * d).sum())
+                if not (edges[which] <= r < edges[which + 1]):
+                    continue
                 g, _ = o.fij(0, int(i), int(j))
-                Lb = abs(q[i]) * b["qmax"] * G
-                worst = max(worst, g / Lb)
-        for j in o.row(2, int(i)):
-            g, _ = o.fij(1, int(i), int(j))
-            worst = max(worst, g / (4 * math.sqrt(sysd["lj_eps"][i] * b["eps_max"]) * b["GV"]))
+                worst = max(worst, g / (abs(q[i]) * b["qmax"] * G))
+                if sysd["lj_eps"][i] * sysd["lj_eps"][j] > 0:
+                    g, _ = o.fij(1, int(i), int(j))
+                    worst = max(worst, g / (4 * math.sqrt(sysd["lj_eps"][i] * b["eps_max"]) * GV))
     assert 0.5 < worst <= 1.0
     # values quoted in SURVEY R-7 for the (5, 9, 3.8/9) shape
     assert abs(b["GM"] - 0.993) < 2e-3
+
+
+def test_lj_bound_covers_a_range_of_sigma():
+    """sup_lj sweeps sigma_ij over [sigma_min, sigma_max] (R-7; inside the switching zone (1-chi) u' and
+    -chi' u have opposite signs, so the sup over sigma is not at an end of the range by construction).  Two LJ species
+    with sigma 3.0 and 4.0 A and different eps, both policies: over every listed pair (each ring under R-10c) the long
+    LJ gradient stays below the bound, and the bound is not slack (max g / L > 0.5)."""
+    rng = np.random.default_rng(12)
+    n, box = 600, 26.0
+    side = 9
+    sites = np.array([(i, j, k) for i in range(side) for j in range(side) for k in range(side)])[rng.permutation(side ** 3)[:n]]
+    pos = (sites + 0.5) * (box / side) + rng.uniform(-0.5, 0.5, size=(n, 3))
+    z = np.zeros(0)
+    sp = rng.integers(0, 2, size=n)
+    sysd = dict(n_atoms=n, box=box, pos=np.mod(pos, box), vel=np.zeros((n, 3)), mass=np.full(n, 12.0), charge=np.zeros(n),
+                lj_sigma=np.where(sp == 0, 3.0, 4.0), lj_eps=np.where(sp == 0, 0.05, 0.2),
+                bond_ij=np.zeros((0, 2), dtype=np.int32), bond_k=z, bond_r0=z,
+                angle_ijk=np.zeros((0, 3), dtype=np.int32), angle_k=z, angle_t0=z,
+                excl_ptr=np.zeros(n + 1, dtype=np.int32), excl_idx=np.zeros(0, dtype=np.int32))
+    for policy in (0, 1):
+        o = jo.Oracle(sysd, r_short=5.0, r_long=9.0, r_mid=7.0, r_mid_in=5.25, skin=1.0, flags=2, list_policy=policy)
+        b = o.bounds()
+        assert b["sig_min"] == 3.0 and b["sig_max"] == 4.0 and b["eps_max"] == pytest.approx(0.2)
+        x = np.mod(sysd["pos"], box)
+        edges = (4.5, b["rA"], b["rM"], 9.0)
+        worst = [0.0, 0.0, 0.0]
+        for i in range(0, n, 7):
+            for which, GV in ((2, b["GV"]),) if policy == 0 else ((0, b["GV"]), (1, b["GV2"]), (2, b["GV3"])):
+                for j in o.row(which, i):
+                    if j == i:
+                        continue
+                    d = x[i] - x[j]; d -= box * np.round(d / box)
+                    r = math.sqrt((d * d).sum())
+                    if policy == 1 and not (edges[which] <= r < edges[which + 1]):
+                        continue
+                    g, _ = o.fij(1, i, int(j))
+                    k = 0 if policy == 0 else which
+                    worst[k] = max(worst[k], g / (4 * math.sqrt(sysd["lj_eps"][i] * b["eps_max"]) * GV))
+        assert max(worst) <= 1.0, worst
+        assert worst[0] > 0.5, worst
+        if policy == 1:
+            assert worst[1] > 0.3 and worst[2] > 0.3, worst
 
 
 # ---------------------------------------------------------------- integrator pieces
@@ -534,27 +690,58 @@ def test_thinning_is_invariant_under_looser_bounds(relaxed_small, mode):
     assert abs(proj[0] - proj[1]) < 0.5 and min(proj) > 0.3   # noisy: the sharp check is the accept count
 
 
-def test_proposal_counts_are_poisson_for_bps(relaxed_small):
-    # Alg. 5 / P:L161: with |v| frozen the number of proposals of a chain is Poisson(N beta |v| L H)
-    sysd, kw = _frozen(relaxed_small, flags=2 | 4)
+@pytest.mark.parametrize("policy", [0, 1])
+def test_proposal_counts_are_poisson_for_bps(relaxed_small, policy):
+    # Alg. 5 / P:L161: with |v| frozen the number of proposals of a chain is Poisson(beta |v| H sum_Y N_Y L_Y)
+    # (one ring V under R-10, the three rings of R-10c)
+    sysd, kw = _frozen(relaxed_small, flags=2 | 4, list_policy=policy)
     o = jo.Oracle(sysd, **kw)
     b = o.bounds()
-    nV = o.row_counts()[2]
+    n0, n1, n2 = o.row_counts()
     v0 = o.vel
     H = 2e-3
     i = 0
-    lam = nV[i] * (1 / (KB * 300)) * np.linalg.norm(v0[i]) * 4 * math.sqrt(sysd["lj_eps"][i] * b["eps_max"]) * b["GV"]
+    NG = n2[i] * b["GV"] if policy == 0 else n0[i] * b["GV"] + n1[i] * b["GV2"] + n2[i] * b["GV3"]
+    lam = NG * (1 / (KB * 300)) * np.linalg.norm(v0[i]) * 4 * math.sqrt(sysd["lj_eps"][i] * b["eps_max"])
     counts = []
     for rep in range(400):
         o.clear_events()
         o.set_state(vel=v0, rebuild=False)
         o.jump_half(H, with_accel=False, step=rep)
         ev = o.events()
-        counts.append(int(((ev["atom"] == i) & (ev["ring"] == 2)).sum()))
+        counts.append(int(((ev["atom"] == i) & (ev["ring"] >= 4)).sum()))
     counts = np.array(counts)
     mu = lam * H
     assert abs(counts.mean() - mu) < 5 * math.sqrt(mu / len(counts))
     assert abs(counts.var() / mu - 1) < 0.3
+
+
+def test_bound_held_between_accepted_jumps_is_algorithm_4(relaxed_small):
+    """R-11: Algorithm 4 prints B_v and lambda-bar at every proposal; the oracle's default holds the bound
+    evaluated at t = 0 / after an accepted jump until the next accepted jump ("re-evaluated after each jump").
+    Both are valid bounds on [t, delta/2], so by P:L157 the accepted jumps have the same law and only the number of
+    proposals differs: accepted events per chain and the mean velocity change agree between the two forms (frozen x,
+    acceleration on, a half-step long enough for several events per chain), the held bound proposes a little more."""
+    sysd, kw = _frozen(relaxed_small, flags=1, eps_jump=1.0)
+    res = []
+    R = 1500
+    for every in (False, True):
+        o = jo.Oracle(sysd, **kw)
+        o.set_bound_mode(every)
+        v0 = o.vel
+        dv = np.zeros_like(v0)
+        for rep in range(R):
+            o.set_vel(v0)
+            o.jump_half(5e-3, with_accel=True, step=rep + 200000 * int(every))
+            dv += o.vel - v0
+        st = o.stats()
+        assert st["max_p"] <= 1.0
+        res.append((st["proposals"] / R, st["accepts"] / R, dv / R))
+    (p_held, a_held, d_held), (p_every, a_every, d_every) = res
+    assert a_held * R > 5000
+    assert abs(a_every / a_held - 1.0) < 5 * math.sqrt(2 / (a_held * R))
+    assert 1.0 <= p_held / p_every < 1.5                      # looser bound: more proposals, never fewer
+    assert np.abs(d_held - d_every).max() < 6 * np.abs(d_held).std() / math.sqrt(R) + 0.05 * np.abs(d_held).max()
 
 
 def test_respa_proposals_per_time_independent_of_outer_step(relaxed_small):
@@ -608,6 +795,81 @@ def test_jump_and_baoab_sample_the_same_measure(relaxed_small):
         Ta, Ua = out[name]
         assert ob.agree(Ta, Tb, 4.0, slack=3.0) and abs(Ta[0] - 300.0) < 20.0, (name, Ta, Tb)
         assert ob.agree(Ua, Ub, 4.0, slack=0.1), (name, Ua, Ub)
+
+
+@pytest.mark.parametrize("variant", ["accel", "jumps_only"])
+def test_two_body_boltzmann_histogram(variant):
+    """SURVEY C.6 "2-body toy"; invariance of mu.  One fixed charge (mass 1e8) and 24 light mobile charges that
+    interact with it only (all mobile-mobile pairs are on the exclusion list): 24 copies of a two-body problem whose
+    stationary law is known in closed form -- the distance r to the fixed charge has density ~ r^2 exp(-beta U(r)) on
+    r <= box/2, U = u(r) - u(r_long) below r_long and 0 beyond (forces are truncated at r_long).  The whole
+    C' machinery (clock, ring pick, candidate draw, rate (6), bound, acceptance, G~, kick (7), the drift of v under a
+    before eta is formed) has to be right for the histogram of a long JUMP run to match it.
+      accel:      Coulomb r_c = 5 A: short part in F0, rings [4.5, 7) by jumps; an LJ term (LJ jumps off, so it stays in
+                  F0, R-13) accelerates the atoms everywhere in the rings (a != 0 while jumps happen);
+      jumps_only: r_c = 1 A, no LJ: F0 = 0 wherever an atom ever is (a = 0), every force acts through jumps.
+    Block averages over 20 blocks give the error bars; the laws without the jumped part are rejected by far."""
+    rng = np.random.default_rng(1)
+    box, nmob, q, al = 16.0, 24, 0.3, 0.25
+    n = nmob + 1
+    pos = np.zeros((n, 3)); pos[0] = [8.0, 8.0, 8.0]
+    pos[1:] = rng.uniform(0, box, size=(nmob, 3))
+    near = np.linalg.norm(pos[1:] - pos[0], axis=1) < 3.0
+    pos[1:][near] += 4.0
+    mass = np.r_[1e8, np.full(nmob, 1.0)]
+    lj_eps, lj_sig = np.zeros(n), np.ones(n)
+    if variant == "accel":
+        lj_eps[:] = 1.0; lj_sig[:] = 3.5
+    vel = rng.normal(size=(n, 3)) * np.sqrt(KB * 300 * KCAL / mass)[:, None]
+    lists = [[]] + [[j for j in range(1, n) if j != i] for i in range(1, n)]
+    ptr = np.zeros(n + 1, np.int32); ptr[1:] = np.cumsum([len(l) for l in lists])
+    z = np.zeros(0)
+    sysd = dict(n_atoms=n, box=box, pos=np.mod(pos, box), vel=vel, mass=mass, charge=np.full(n, q), lj_sigma=lj_sig,
+                lj_eps=lj_eps, bond_ij=np.zeros((0, 2), np.int32), bond_k=z, bond_r0=z,
+                angle_ijk=np.zeros((0, 3), np.int32), angle_k=z, angle_t0=z, excl_ptr=ptr,
+                excl_idx=np.array([j for l in lists for j in l], np.int32))
+    kw = dict(r_short=5.0, r_switch=0.5, r_mid_in=5.25, r_mid=6.0, r_long=7.0) if variant == "accel" else \
+        dict(r_short=1.0, r_switch=0.5, r_mid_in=3.0, r_mid=5.0, r_long=7.0)
+    o = jo.Oracle(sysd, ewald_alpha=al, dt_fs=2.0, gamma_per_ps=2.0, flags=1, eps_jump=1.0, skin=1.0, nlist_every=2, seed=1, **kw)
+    o.jump_step(2000)
+    nb, K, per = 11, 20, 4000
+    edges = np.linspace(2.5, 8.0, nb + 1)
+    H = np.zeros((K, nb))
+    for k in range(K):
+        for _ in range(per // 10):
+            o.jump_step(10)
+            d = o.pos[1:] - o.pos[0]
+            d -= box * np.round(d / box)
+            H[k] += np.histogram(np.linalg.norm(d, axis=1), bins=edges)[0]
+    st = o.stats()
+    assert st["max_p"] <= 1.0 and st["max_g_over_L"] <= 1.0 and st["accepts"] > 2000 and st["max_disp"] < 0.5
+    beta = 1.0 / (KB * 300)
+
+    def law(u_of_r):                               # bin probabilities of r^2 exp(-beta U), U shifted to 0 at r_long
+        rr = np.linspace(2.5, 8.0, 110001)
+        w = rr * rr * np.exp(-beta * np.where(rr < 7.0, u_of_r(rr) - u_of_r(7.0), 0.0))
+        cdf = np.concatenate([[0.0], np.cumsum(0.5 * (w[1:] + w[:-1]) * np.diff(rr))])
+        p = np.diff(np.interp(edges, rr, cdf))
+        return p / p.sum()
+
+    u_c = lambda r: 332.063713 * q * q * special.erfc(al * r) / r
+    u_lj = lambda r: 4.0 * ((3.5 / r) ** 12 - (3.5 / r) ** 6) if variant == "accel" else 0.0 * r
+    full = law(lambda r: u_c(r) + u_lj(r))
+    P = H / H.sum(1, keepdims=True)
+    m, se = P.mean(0), P.std(0, ddof=1) / math.sqrt(K)
+    ok = full > 0.02                               # bins that are populated
+    assert ok.sum() >= 7 and (se[ok] / full[ok]).max() < 0.06
+    zs = (m[ok] - full[ok]) / se[ok]
+    assert np.abs(zs).max() < 4.0, zs
+    # the same run rejects the law without the part of U the jumps carry (their force replaced by nothing)
+    def u_without_jumps(r):
+        chi = np.array([jo.chi(x, kw["r_short"], 0.5)[0] for x in np.atleast_1d(r)])
+        return chi * u_c(r) + u_lj(r)
+    rr = np.linspace(2.5, 8.0, 2201)
+    w = rr * rr * np.exp(-beta * (u_without_jumps(rr) - u_without_jumps(np.array([7.999]))[0]))
+    cdf = np.concatenate([[0.0], np.cumsum(0.5 * (w[1:] + w[:-1]) * np.diff(rr))])
+    alt = np.diff(np.interp(edges, rr, cdf)); alt /= alt.sum()
+    assert (((m[ok] - alt[ok]) / se[ok]) ** 2).sum() > 150.0
 
 
 def test_bjaoajb_scheme(relaxed_small):
