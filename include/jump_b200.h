@@ -12,7 +12,8 @@
  * Errors: every int-returning call gives 0 on success or a negative JUMP_E_* code.
  * Device-side flags (row overflow, thinning bound violated, displacement beyond
  * skin/2, non-finite state) are sticky and reported by the next synchronising call
- * (jump_get_*, jump_sync).  Nothing is printed and nothing calls exit().
+ * (jump_get_*, jump_sync); jump_reset_stats clears them.  Nothing is printed and
+ * nothing calls exit().
  */
 #ifndef JUMP_B200_H
 #define JUMP_B200_H
@@ -26,8 +27,9 @@ extern "C" {
 #define JUMP_E_CUDA (-2)     /* CUDA runtime error, see jump_last_error */
 #define JUMP_E_OVERFLOW (-3) /* a neighbour/ring row or the event buffer overflowed its capacity */
 #define JUMP_E_BOUND (-4)    /* thinning bound violated: an acceptance probability p > 1 was seen */
-#define JUMP_E_SKIN (-5)     /* an atom moved more than skin/2 since the last list build (only with JUMP_F_STRICT_SKIN;
-                                otherwise jump_stats.max_disp reports it: a hot, far-from-equilibrium start may exceed it) */
+#define JUMP_E_SKIN (-5)     /* an atom moved more than skin/2 since the last list build: the lists may have missed a pair
+                                (R-10c).  Checked on the device at every step; raise skin or lower nlist_every.  With
+                                JUMP_F_LAX_SKIN only jump_stats.max_disp reports it (equilibration of a hot start). */
 #define JUMP_E_NAN (-6)      /* non-finite position or velocity */
 
 #define JUMP_F_COUL_JUMPS 1u       /* Coulomb tail r_c..r_long by jumps (step C', Alg. 4) */
@@ -37,7 +39,7 @@ extern "C" {
 #define JUMP_F_RESPA_COMPARATOR 16u /* jump_respa_step runs BAOAB-RESPA: outer kick by the long force */
 
 #define JUMP_F_BJAOAJB 64u         /* jump_step runs B J A O A J B instead of C'J' A O A J'C' */
-#define JUMP_F_STRICT_SKIN 32u      /* make a displacement beyond skin/2 between list builds an error (JUMP_E_SKIN) */
+#define JUMP_F_LAX_SKIN 32u        /* a displacement beyond skin/2 between list builds is NOT an error (see JUMP_E_SKIN) */
 
 typedef struct jump_ctx jump_ctx; /* opaque, owned by the library */
 
@@ -54,16 +56,20 @@ typedef struct {
     double box[3];       /* orthorhombic periodic box edges, A */
     double r_short;      /* r_c: chi = 0 at and beyond it */
     double r_switch;     /* h: chi = 1 below r_c - h */
-    double r_mid;        /* r_M ring split; <= 0: no ring */
+    double r_mid;        /* r_M: outer ring edge (R-10c: rings [r_c-h, r_A), [r_A, r_M), [r_M, r_long));
+                            <= 0: r_A (two rings) */
     double r_long;       /* r_E: pairs beyond are neglected */
     double ewald_alpha;  /* alpha of erfc(alpha r)/r; < 0: 3.8 / r_long (R-2) */
     double dt_fs, gamma_per_ps, temperature_K; /* delta, gamma, T */
     double eps_jump;     /* epsilon of the general mechanism (6),(7); +inf: BPS */
     double skin;         /* list skin s (R-10) */
     double cell_edge;    /* minimum edge of the sort grid; <= 0: (r_long + skin) / 4 (R-10) */
+    double r_mid_in;     /* r_A: inner ring edge; <= 0: r_short (ring A = the switching zone) */
 } jump_params;
 
-/* One proposal of a jump chain (R-18).  ring: 0 = M, 1 = L, 2 = V (LJ), -1 = clock expired. */
+/* One proposal of a jump chain (R-18).  ring: 0, 1, 2 = ring A, B, C of a Coulomb chain (step C'), 4, 5, 6 = the same
+ * rings of an LJ chain (step J'), -1 = clock expired.  j: the candidate drawn (original index), whether or not it
+ * carries a force at the moment. */
 typedef struct {
     int32_t step, stream, atom, iter;
     int32_t ring, j, accepted, n_gt;
@@ -75,7 +81,7 @@ typedef struct {
     double max_p;        /* largest acceptance probability seen (must stay <= 1) */
     double max_g_over_L; /* largest |F_ij| / L seen (must stay <= 1) */
     double max_disp;     /* largest displacement since a list build, A */
-    int32_t max_row[6];  /* largest row length seen: short, M, L, V, full, LJ-tail */
+    int32_t max_row[6];  /* largest row length seen: short, A, B, (unused), full, LJ-tail */
     int32_t cap_row[6];  /* row capacities */
     int32_t error;       /* sticky device error (0 or JUMP_E_*) */
     int32_t pad;
@@ -128,13 +134,14 @@ int jump_reset_stats(jump_ctx *c);
 /* Copy up to cap logged events (unsorted) to host_buf; *n receives the number logged so far. */
 int jump_get_events(jump_ctx *c, jump_event *host_buf, int64_t cap, int64_t *n);
 int jump_clear_events(jump_ctx *c);
-/* Row which (0 short, 1 M, 2 L, 3 V) of original atom i as original indices in canonical order (R-10);
- * returns the row length (or a negative error); at most cap entries are written to host_out. */
+/* Candidate lists of original atom i as original indices in canonical order (R-10c): which = 0 short list, 1 row A,
+ * 2 row B, 3 the cell universe of the atom's home cell (ring C; it holds the atom itself and its excluded partners);
+ * 4 full list, 5 LJ-tail list.  Returns the length (or a negative error); at most cap entries are written to host_out. */
 int jump_get_row(jump_ctx *c, int32_t which, int32_t atom, int32_t *host_out, int32_t cap);
 /* Observables on the device (the paper's evidence is of this kind).
  * jump_get_images: periodic image counters (n x 3 int32, device, original order): the unwrapped position of atom i is
- *   d_pos[i] + image[i] * box, continuous since jump_init (or the last jump_refresh, which resets the counters); each
- *   counter holds +-511 box lengths.  Synchronises the stream.
+ *   d_pos[i] + image[i] * box, continuous since jump_init (or the last jump_refresh, which resets the counters;
+ *   jump_refresh_lazy keeps them); each counter holds +-511 box lengths (beyond that it wraps: a 512-box excursion).  Synchronises the stream.
  * jump_rdf_accumulate: adds to d_hist[n_bins] (device, uint64, caller-owned and zeroed by the caller) the number of
  *   unordered pairs of atoms (lj_only != 0: of LJ carriers, the water oxygens) whose minimum-image distance r at the
  *   current positions is < r_max, in bin floor(r n_bins / r_max); r_max <= box/2, n_bins <= 2048.  Bonded exclusions
@@ -148,15 +155,24 @@ int jump_get_images(jump_ctx *c, int32_t *d_img);
 int jump_vacf_mark(jump_ctx *c);
 int jump_vacf_dot(jump_ctx *c, int32_t lj_only, double *c_out);
 int jump_rdf_accumulate(jump_ctx *c, int32_t lj_only, double r_max, int32_t n_bins, uint64_t *d_hist);
-/* Bounds as used (R-7): GM, GL, GV, qmax, eps_max, sig_min, sig_max, rM. */
-int jump_get_bounds(jump_ctx *c, double out[8]);
+/* Bounds as used (R-7, R-10c): G_A, G_B, GV_A, qmax, eps_max, sig_min, sig_max, r_M, G_C, GV_B, GV_C, r_A (G: sup of the
+ * long Coulomb gradient per unit charges over a ring, GV: of the long LJ gradient with 4 eps = 1). */
+int jump_get_bounds(jump_ctx *c, double out[12]);
+/* Lanes that cooperate on one jump chain in the update kernel: 1, 4, 8 or 16; 0 = chosen from the number of atoms so
+ * that the grid fills the GPU once (the default).  Every choice runs the same chains with the same random streams
+ * (tests compare each against the oracle).  */
+int jump_set_lanes(jump_ctx *c, int32_t lanes);
+/* Switch JUMP_F_LAX_SKIN on / off after init (an equilibration from a hot start, then a checked production run). */
+int jump_set_lax_skin(jump_ctx *c, int32_t on);
 /* Re-read d_pos / d_vel after the caller changed them: re-sort, rebuild rows, recompute F0. */
 int jump_refresh(jump_ctx *c);
 /* The same for a caller that hands the state back after a few steps (host round trips): the rows are kept, and the
  * sorted order with them, when no atom is farther than skin/2 from its position at the last list build -- they are
- * still supersets of the pairs in range (R-10); otherwise re-sort and rebuild as jump_refresh does.  *rebuilt (may be
- * NULL) receives 0 / 1.  The list-rebuild period of the step calls keeps counting.  F0 is recomputed; the image
- * counters are reset.  Synchronises the stream once (the decision is taken on the host). */
+ * still supersets of the pairs in range (R-10c); otherwise re-sort and rebuild as jump_refresh does.  *rebuilt (may be
+ * NULL) receives 0 / 1.  The list-rebuild period of the step calls keeps counting.  F0 is recomputed.  The image
+ * counters are KEPT (the trajectory is taken to continue): an atom whose position comes back bit for bit as the library
+ * wrote it keeps its fp64 residual as well; for any other the residual restarts at 0 and a coordinate outside [0, L) adds
+ * its box lengths to the counter.  Synchronises the stream once (the decision is taken on the host). */
 int jump_refresh_lazy(jump_ctx *c, int32_t *rebuilt);
 /* Run only the opening jump half-phase C'(H) [then J'(H)] at frozen x with stream ids 1, 2 (pins). */
 int jump_half(jump_ctx *c, double H_ps, int32_t with_accel, int64_t step);

@@ -1342,8 +1342,9 @@ orc_ctx *orc_create(const orc_params *p, const double *pos, const double *vel, c
     c->rc = p->r_short; c->h = p->r_switch; c->rE = p->r_long; c->skin = p->skin;
     c->alpha = p->ewald_alpha < 0.0 ? 3.8 / p->r_long : p->ewald_alpha; /* R-2 */
     /* r_mid <= 0: no ring, M is empty and L covers the whole shell */
-    c->rM = p->r_mid > 0.0 ? p->r_mid : dmax(c->rc - c->h - c->skin, 0.0);
     c->rA = p->r_mid_in > 0.0 ? p->r_mid_in : c->rc; /* R-10c: ring A = the switching zone by default */
+    if (p->r_mid > 0.0) c->rM = p->r_mid;
+    else c->rM = p->list_policy == 1 ? c->rA : dmax(c->rc - c->h - c->skin, 0.0); /* no split asked for */
     if (c->rA > c->rM) c->rA = c->rM;
     c->sbm = malloc(sizeof(double) * n);
     for (int i = 0; i < n; ++i) c->sbm[i] = sqrt(c->m[i] / (c->kT * ORC_KCAL));
@@ -1352,7 +1353,6 @@ orc_ctx *orc_create(const orc_params *p, const double *pos, const double *vel, c
     c->gny = (int)floor(p->box[1] / edge); if (c->gny < 1) c->gny = 1;
     c->gnz = (int)floor(p->box[2] / edge); if (c->gnz < 1) c->gnz = 1;
     c->policy = p->list_policy == 1 ? 1 : 0;
-    if (c->policy == 1 && !(p->r_mid > 0.0)) c->rM = c->rA; /* no ring split asked for: rings A and the universe */
     c->ureach = p->r_long + p->skin;
     {
         int nn[3] = {c->gnx, c->gny, c->gnz};

@@ -145,7 +145,7 @@ def _ip(a):
 def make_params(n_atoms, box, r_short, r_long, r_switch=0.5, r_mid=None, ewald_alpha=-1.0, dt_fs=1.0,
                 gamma_per_ps=1.0, temperature_K=300.0, n_inner=4, eps_jump=1.0, eps_mode=0,
                 flags=F_COUL_JUMPS | F_LJ_JUMPS, skin=1.0, nlist_every=10, seed=0, cell_edge=0.0, list_policy=1,
-                r_mid_in=0.0, **_ignored):
+                r_mid_in=None, **_ignored):
     """list_policy 1 (default, the contract of the CUDA path): DESIGN.md R-10c; 0: the ring rows of R-10."""
     p = Params()
     p.n_atoms, p.n_inner, p.eps_mode, p.flags = int(n_atoms), int(n_inner), int(eps_mode), int(flags)
@@ -154,6 +154,7 @@ def make_params(n_atoms, box, r_short, r_long, r_switch=0.5, r_mid=None, ewald_a
     p.box[0], p.box[1], p.box[2] = float(b[0]), float(b[1]), float(b[2])
     p.r_short, p.r_switch, p.r_long = float(r_short), float(r_switch), float(r_long)
     p.r_mid = float(r_short + 2.0 if r_mid is None else r_mid)
+    r_mid_in = r_short + 0.25 if r_mid_in is None else r_mid_in
     p.ewald_alpha = float(ewald_alpha)
     p.dt_fs, p.gamma_per_ps, p.temperature_K = float(dt_fs), float(gamma_per_ps), float(temperature_K)
     p.eps_jump, p.skin, p.cell_edge, p.r_mid_in = float(eps_jump), float(skin), float(cell_edge), float(r_mid_in)

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libjump_b200.so")
 
 F_COUL_JUMPS, F_LJ_JUMPS, F_EVENT_LOG, F_RESPA_PAPER, F_RESPA_COMPARATOR = 1, 2, 4, 8, 16
-F_STRICT_SKIN = 32
+F_LAX_SKIN = 32
 F_BJAOAJB = 64
 ERRORS = {-1: "bad argument", -2: "CUDA error", -3: "row/event overflow", -4: "thinning bound violated",
           -5: "displacement beyond skin/2", -6: "non-finite state"}
@@ -22,7 +22,7 @@ EXPORTS = ["jump_init", "jump_step", "baoab_step", "jump_respa_step", "jump_get_
            "jump_get_stats", "jump_reset_stats", "jump_get_events", "jump_clear_events", "jump_get_row", "jump_get_images", "jump_rdf_accumulate",
            "jump_get_bounds", "jump_refresh", "jump_refresh_lazy", "jump_half", "jump_sync", "jump_get_step", "jump_get_launches",
            "jump_last_error", "jump_free", "jump_set_profiling", "jump_get_profile", "jump_count_pairs",
-           "jump_ewald_setup", "jump_respa1_step", "jump_get_slow_energy", "jump_vacf_mark", "jump_vacf_dot"]
+           "jump_ewald_setup", "jump_respa1_step", "jump_get_slow_energy", "jump_vacf_mark", "jump_vacf_dot", "jump_set_lanes", "jump_set_lax_skin"]
 
 
 class jump_params(C.Structure):
@@ -33,7 +33,7 @@ class jump_params(C.Structure):
         ("r_short", C.c_double), ("r_switch", C.c_double), ("r_mid", C.c_double), ("r_long", C.c_double),
         ("ewald_alpha", C.c_double),
         ("dt_fs", C.c_double), ("gamma_per_ps", C.c_double), ("temperature_K", C.c_double),
-        ("eps_jump", C.c_double), ("skin", C.c_double), ("cell_edge", C.c_double),
+        ("eps_jump", C.c_double), ("skin", C.c_double), ("cell_edge", C.c_double), ("r_mid_in", C.c_double),
     ]
 
 
@@ -105,13 +105,15 @@ def lib():
         L.jump_set_profiling.argtypes = [vp, i32]
         L.jump_get_profile.argtypes = [vp, dp, C.POINTER(i64)]
         L.jump_count_pairs.argtypes = [vp, i32, C.c_double, C.POINTER(i64)]
+        L.jump_set_lanes.argtypes = [vp, i32]
+        L.jump_set_lax_skin.argtypes = [vp, i32]
         _lib = L
     return _lib
 
 
 def make_params(n_atoms, box, r_short, r_long, r_switch=0.5, r_mid=None, ewald_alpha=-1.0, dt_fs=1.0, gamma_per_ps=1.0,
                 temperature_K=300.0, n_inner=4, eps_jump=1.0, eps_mode=0, flags=F_COUL_JUMPS | F_LJ_JUMPS, skin=1.0,
-                nlist_every=10, seed=0, cell_edge=0.0, **_ignored):
+                nlist_every=10, seed=0, cell_edge=0.0, r_mid_in=None, **_ignored):
     p = jump_params()
     p.n_atoms, p.n_inner, p.eps_mode, p.flags = int(n_atoms), int(n_inner), int(eps_mode), int(flags)
     p.nlist_every, p.seed = int(nlist_every), int(seed)
@@ -119,9 +121,10 @@ def make_params(n_atoms, box, r_short, r_long, r_switch=0.5, r_mid=None, ewald_a
     p.box[0], p.box[1], p.box[2] = float(b[0]), float(b[1]), float(b[2])
     p.r_short, p.r_switch, p.r_long = float(r_short), float(r_switch), float(r_long)
     p.r_mid = float(r_short + 2.0 if r_mid is None else r_mid)
+    r_mid_in = r_short + 0.25 if r_mid_in is None else r_mid_in
     p.ewald_alpha = float(ewald_alpha)
     p.dt_fs, p.gamma_per_ps, p.temperature_K = float(dt_fs), float(gamma_per_ps), float(temperature_K)
-    p.eps_jump, p.skin, p.cell_edge = float(eps_jump), float(skin), float(cell_edge)
+    p.eps_jump, p.skin, p.cell_edge, p.r_mid_in = float(eps_jump), float(skin), float(cell_edge), float(r_mid_in)
     return p
 
 
@@ -308,9 +311,17 @@ class JumpSim:
                                                 C.c_void_p(hist.data_ptr())), "jump_rdf_accumulate")
 
     def bounds(self):
-        out = (C.c_double * 8)()
+        out = (C.c_double * 12)()
         self._check(self._L.jump_get_bounds(self._h, out), "jump_get_bounds")
-        return dict(zip(["GM", "GL", "GV", "qmax", "eps_max", "sig_min", "sig_max", "rM"], list(out)))
+        return dict(zip(["GM", "GL", "GV", "qmax", "eps_max", "sig_min", "sig_max", "rM", "G3", "GV2", "GV3", "rA"], list(out)))
+
+    def set_lax_skin(self, on=True):
+        """A displacement beyond skin/2 between two list builds is (not) an error."""
+        self._check(self._L.jump_set_lax_skin(self._h, int(bool(on))), "jump_set_lax_skin")
+
+    def set_lanes(self, lanes=0):
+        """Lanes per jump chain in the update kernel (1, 4, 8, 16; 0 = automatic)."""
+        self._check(self._L.jump_set_lanes(self._h, int(lanes)), "jump_set_lanes")
 
     def set_profiling(self, on=True):
         self._check(self._L.jump_set_profiling(self._h, int(bool(on))), "jump_set_profiling")

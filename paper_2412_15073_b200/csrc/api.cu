@@ -22,8 +22,13 @@ struct jump_ctx {
     cudaEvent_t ev_fork, ev_join;
     bool bonded_in_flight;
     int n;
-    double kT, dt, alpha, rM, lo;  // ps; lo = max(r_c - h - skin, 0)
-    double GM, GL, GV, qmax, eps_max, sig_min, sig_max;
+    double kT, dt, alpha, rA, rM, lo;  // ps; lo = max(r_c - h - skin, 0)
+    double G[3], GV[3], qmax, eps_max, sig_min, sig_max;   // bounds per ring (R-7, R-10c)
+    Universe uni;                // cell universe of ring C (R-10c)
+    unsigned short *uni_cum;
+    int *cell_of;
+    int lanes;                   // jump_set_lanes
+    int64_t sort_step;           // step count at the last sort
     float c1, c2;
     float *d_pos, *d_vel;  // caller's
     // sorted state (cur) and spare buffers (nxt)
@@ -51,6 +56,7 @@ struct jump_ctx {
     int *moved_flag;                  // scratch of jump_refresh_lazy
     int *excl_ptr, *excl_idx;
     Topo topo;
+    Bonded bonded;               // small molecules (one thread each) + atoms of larger components (forces.cu)
     std::vector<void *> owned;  // everything to cudaFree
     Counters *ctr;
     jump_event *events;
@@ -170,16 +176,19 @@ static void compute_bounds(jump_ctx *c, const std::vector<float> &q, const std::
         }
     }
     if (c->eps_max == 0.0) c->sig_min = c->sig_max = 0.0;
-    const double rlo = c->p.r_short - c->p.r_switch, rE = c->p.r_long, s = c->p.skin;
-    c->GM = sup_long(c, rlo, std::min(c->rM + s, rE), 1e-4, true, 0.0);
-    c->GL = sup_long(c, std::max(c->rM - s, rlo), rE, 1e-4, true, 0.0);
-    c->GV = 0.0;
-    if (c->sig_max > 0.0) {
-        int NS = (c->sig_max > c->sig_min) ? 65 : 1;
-        for (int k = 0; k < NS; ++k) {
-            double sg = NS == 1 ? c->sig_min : c->sig_min + (c->sig_max - c->sig_min) * (double)k / (double)(NS - 1);
-            c->GV = std::max(c->GV, sup_long(c, rlo, rE, 1e-3, false, sg));
-        }
+    // R-10c: ring Y holds the pairs whose current distance lies in it, so its bound is the sup over the ring itself
+    const double rlo = c->p.r_short - c->p.r_switch, rE = c->p.r_long;
+    const double eA = std::min(std::max(c->rA, rlo), rE), eM = std::min(std::max(c->rM, eA), rE);
+    const double edge[4] = {rlo, eA, eM, rE};
+    const int NS = (c->sig_max > c->sig_min) ? 65 : 1;
+    for (int y = 0; y < 3; ++y) {
+        c->G[y] = sup_long(c, edge[y], edge[y + 1], 1e-4, true, 0.0);
+        c->GV[y] = 0.0;
+        if (c->sig_max > 0.0)
+            for (int k = 0; k < NS; ++k) {
+                double sg = NS == 1 ? c->sig_min : c->sig_min + (c->sig_max - c->sig_min) * (double)k / (double)(NS - 1);
+                c->GV[y] = std::max(c->GV[y], sup_long(c, edge[y], edge[y + 1], 1e-3, false, sg));
+            }
     }
 }
 
@@ -209,7 +218,10 @@ static int build_rows(jump_ctx *c, const bool want[N_ROWS]) {
     }
     if (!any) return 0;
     prof_begin(c, PROF_BUILD);
-    launch_build_rows(c->m, c->g, sel, (float)rmax, c->cell_start, c->xs, c->xl, c->lj, c->orig,
+    // A row asked for the first time between two sorts is built from the positions of the last sort (x_build), which
+    // the cell table describes and the displacement check refers to: it is the row an eager build would have made.
+    const float4 *xsrc = (c->step == c->sort_step) ? c->xs : c->x_build;
+    launch_build_rows(c->m, c->g, sel, (float)rmax, c->cell_start, xsrc, c->xl, c->lj, c->orig,
                       c->sorted_of, c->excl_ptr, c->excl_idx, c->ctr, c->st, &c->launches);
     prof_end(c, PROF_BUILD);
     CK(cudaGetLastError());
@@ -221,7 +233,7 @@ static int resort_and_build(jump_ctx *c) {
     a.n = c->n; a.grid = c->g;
     a.xs_in = c->xs; a.vs_in = c->vs; a.xl_in = c->xl; a.xl = c->xl_nxt; a.lj_in = c->lj; a.mi_in = c->mi; a.orig_in = c->orig;
     a.xs = c->xs_nxt; a.vs = c->vs_nxt; a.lj = c->lj_nxt; a.mi = c->mi_nxt; a.orig = c->orig_nxt;
-    a.sorted_of = c->sorted_of; a.x_build = c->x_build;
+    a.sorted_of = c->sorted_of; a.x_build = c->x_build; a.cell_of = c->cell_of;
     a.key = c->key; a.cell_count = c->cell_count; a.cell_fill = c->cell_fill; a.cell_start = c->cell_start;
     a.tmp_orig = c->tmp_orig; a.tmp_src = c->tmp_src; a.scan_sums = c->scan_sums; a.scan_offs = c->scan_offs; a.ctr = c->ctr;
     prof_begin(c, PROF_BUILD);
@@ -233,7 +245,14 @@ static int resort_and_build(jump_ctx *c) {
     bool want[N_ROWS];
     for (int k = 0; k < N_ROWS; ++k) { c->row_fresh[k] = false; want[k] = c->row_used[k]; c->row_used[k] = false; }
     c->rebuilds++;
+    c->sort_step = c->step;
     c->slow_valid = false;   // (sorted order changed)
+    if (c->uni_cum) {   // running sums of the universe of every cell (ring C, R-10c)
+        prof_begin(c, PROF_BUILD);
+        launch_universe(c->g, c->uni, c->cell_start, c->uni_cum, c->ctr, c->st, &c->launches);
+        prof_end(c, PROF_BUILD);
+        CK(cudaGetLastError());
+    }
     return build_rows(c, want);
 }
 
@@ -264,10 +283,9 @@ static int pair(jump_ctx *c, int row, int wC, int wLJ, float4 *out, int accumula
 static bool lj_jumps(const jump_ctx *c) { return (c->p.flags & JUMP_F_LJ_JUMPS) != 0; }
 static bool coul_jumps(const jump_ctx *c) { return (c->p.flags & JUMP_F_COUL_JUMPS) != 0; }
 
-static int bonded(jump_ctx *c, const float4 *add, float4 *out_sum, float4 *out_bond) {
-    prof_begin(c, PROF_BONDED);
-    launch_bonded(c->m, c->topo, c->xs, c->xl, c->orig, c->sorted_of, add, out_sum, out_bond, c->st, &c->launches);
-    prof_end(c, PROF_BONDED);
+// bonded gradient at the current positions into c->fbond (the one evaluation every path uses: steps and observers)
+static int bonded_eval(jump_ctx *c, cudaStream_t st) {
+    launch_bonded(c->m, c->topo, c->bonded, c->xs, c->xl, c->sorted_of, c->fbond, st, &c->launches);
     CK(cudaGetLastError());
     return 0;
 }
@@ -285,13 +303,12 @@ static int compute_short_nb(jump_ctx *c, float4 *out, bool energy = false) {
 }
 static int bonded_only(jump_ctx *c) {  // fbond at the current positions
     prof_begin(c, PROF_BONDED);
-    launch_bonded_lanes(c->m, c->topo, c->xs, c->xl, c->orig, c->sorted_of, c->fbond, c->st, &c->launches);
+    int r = bonded_eval(c, c->st);
     prof_end(c, PROF_BONDED);
-    CK(cudaGetLastError());
-    return 0;
+    return r;
 }
 // the same on the side stream: fork after everything enqueued so far, join_bonded() before fbond is read.
-// The bonded kernel (a few thousand latency-bound threads) then overlaps the pair kernel instead of preceding it.
+// The bonded kernels then overlap the pair kernel instead of preceding it.
 static int bonded_fork(jump_ctx *c) {
     CK(cudaEventRecord(c->ev_fork, c->st));
     CK(cudaStreamWaitEvent(c->st2, c->ev_fork, 0));
@@ -302,9 +319,9 @@ static int bonded_fork(jump_ctx *c) {
         cudaEventRecord(ev.first, c->st2);
         c->prof_pend[PROF_BONDED].push_back(ev);
     }
-    launch_bonded_lanes(c->m, c->topo, c->xs, c->xl, c->orig, c->sorted_of, c->fbond, c->st2, &c->launches);
+    int r = bonded_eval(c, c->st2);
     if (c->prof) cudaEventRecord(c->prof_pend[PROF_BONDED].back().second, c->st2);
-    CK(cudaGetLastError());
+    if (r) return r;
     CK(cudaEventRecord(c->ev_join, c->st2));
     c->bonded_in_flight = true;
     return 0;
@@ -326,13 +343,6 @@ static int compute_f0(jump_ctx *c) {
 }
 static GradRef gr_f0(const jump_ctx *c) { return gr(c->fnb, c->fbond); }
 static int ensure_f0(jump_ctx *c) { return c->f0_valid ? 0 : compute_f0(c); }
-// F0 materialised in c->f0 (observers only)
-static int compute_f0_sum(jump_ctx *c) {
-    int r = compute_short_nb(c, c->fnb);
-    if (r) return r;
-    c->f0_valid = true;
-    return bonded(c, c->fnb, c->f0, c->fbond);
-}
 // unsplit force to r_long as ftmp2 + fbond (BAOAB comparator); invalidates F0
 static int compute_full_split(jump_ctx *c) {
     int r = bonded_fork(c);
@@ -343,19 +353,20 @@ static int compute_full_split(jump_ctx *c) {
     return bonded_join(c);
 }
 static GradRef gr_full(const jump_ctx *c) { return gr(c->ftmp2, c->fbond); }
+// long part of the pair gradient (comparators only): the (1 - chi) weights over the full list
 static int compute_long(jump_ctx *c, float4 *out) {
     int wLJ = lj_jumps(c) ? W_LONG : W_NONE;
-    int r = pair(c, ROW_M, W_LONG, wLJ, out, 0, false);
-    if (!r) r = pair(c, ROW_L, W_LONG, wLJ, out, 1, false);
+    int r = pair(c, ROW_F, W_LONG, wLJ, out, 0, false);
     if (r) return r;
     CK(cudaGetLastError());
     return 0;
 }
-static int compute_full(jump_ctx *c, float4 *out, bool energy = false) {  // unsplit to r_long + bonded
+static int compute_full(jump_ctx *c, bool energy) {  // unsplit to r_long (ftmp2) + bonded (fbond), observers
     int r = pair(c, ROW_F, W_FULL, W_FULL, c->ftmp2, 0, energy);
     if (r) return r;
     CK(cudaGetLastError());
-    return bonded(c, c->ftmp2, out, nullptr);
+    c->f0_valid = false;
+    return bonded_only(c);
 }
 
 // ---- step drivers --------------------------------------------------------------------------------------
@@ -378,15 +389,16 @@ static int run_update(jump_ctx *c, const Phase &p0, GradRef g0, const Phase &p1,
     if (!g1.a) A.ph[1].use_grad = 0;
     A.do_aoa = aoa ? 1 : 0;
     A.half_dt = (float)(0.5 * c->dt); A.c1 = c->c1; A.c2 = c->c2; A.o_step = (unsigned)c->step;
-    A.xs = c->xs; A.xs_out = c->xs_nxt; A.vs = c->vs; A.xl = c->xl; A.mi = c->mi; A.lj = c->lj; A.orig = c->orig; A.x_build = c->x_build;
-    A.rowM = c->rows[ROW_M]; A.rowL = c->rows[ROW_L]; A.rowV = c->rows[ROW_V];
+    A.xs = c->xs; A.xs_out = c->xs_nxt; A.vs = c->vs; A.xl_out = c->xl_nxt; A.mi = c->mi; A.lj = c->lj; A.orig = c->orig; A.x_build = c->x_build;
+    A.rowA = c->rows[ROW_A]; A.rowB = c->rows[ROW_B];
+    A.uni = c->uni; A.grid = c->g; A.cell_start = c->cell_start; A.xl_all = c->xl; A.excl_ptr = c->excl_ptr; A.excl_idx = c->excl_idx;
+    A.lanes = c->lanes;
     A.ctr = c->ctr; A.events = (c->p.flags & JUMP_F_EVENT_LOG) ? c->events : nullptr; A.event_cap = c->event_cap;
     bool jumps = (p0.kind == 2 || p1.kind == 2) && (coul_jumps(c) || lj_jumps(c));
     if (jumps) {
-        int r = coul_jumps(c) ? need_rows(c, {ROW_M, ROW_L}) : 0;
-        if (!r && lj_jumps(c)) r = need_row(c, ROW_V);
+        int r = need_rows(c, {ROW_A, ROW_B});
         if (r) return r;
-        A.rowM = c->rows[ROW_M]; A.rowL = c->rows[ROW_L]; A.rowV = c->rows[ROW_V];
+        A.rowA = c->rows[ROW_A]; A.rowB = c->rows[ROW_B];
     }
     prof_begin(c, PROF_UPDATE);
     launch_update(c->m, A, jumps, c->st, &c->launches);
@@ -394,6 +406,7 @@ static int run_update(jump_ctx *c, const Phase &p0, GradRef g0, const Phase &p1,
     CK(cudaGetLastError());
     if (aoa) {
         std::swap(c->xs, c->xs_nxt);
+        std::swap(c->xl, c->xl_nxt);
         c->f0_valid = false;
         c->slow_valid = false;
         c->step++;
@@ -413,7 +426,7 @@ static int poll_error(jump_ctx *c) {  // sticky device flags -> error code
     if (h.err & ERR_NAN) c->sticky = JUMP_E_NAN;
     else if (h.err & (ERR_OVERFLOW | ERR_EVENTS)) c->sticky = JUMP_E_OVERFLOW;
     else if (h.err & ERR_BOUND) c->sticky = JUMP_E_BOUND;
-    else if ((h.err & ERR_SKIN) && (c->p.flags & JUMP_F_STRICT_SKIN)) c->sticky = JUMP_E_SKIN;
+    else if ((h.err & ERR_SKIN) && !(c->p.flags & JUMP_F_LAX_SKIN)) c->sticky = JUMP_E_SKIN;
     if (c->sticky && c->err.empty()) c->err = "device error flags " + std::to_string(h.err);
     return c->sticky;
 }
@@ -693,7 +706,9 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     c->dt = p->dt_fs * 1e-3;
     c->alpha = p->ewald_alpha < 0.0 ? 3.8 / p->r_long : p->ewald_alpha;  // R-2
     c->lo = std::max(p->r_short - p->r_switch - p->skin, 0.0);
-    c->rM = p->r_mid > 0.0 ? p->r_mid : c->lo;  // no ring: M empty, L covers the shell
+    c->rA = p->r_mid_in > 0.0 ? p->r_mid_in : p->r_short;   // R-10c: ring A = the switching zone by default
+    c->rM = p->r_mid > 0.0 ? p->r_mid : c->rA;              // no outer split asked for: rings A and C
+    if (c->rA > c->rM) c->rA = c->rM;
     double g1 = std::exp(-p->gamma_per_ps * c->dt);
     c->c1 = (float)g1;
     c->c2 = (float)std::sqrt(1.0 - g1 * g1);
@@ -715,8 +730,16 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     m.beta = (float)(1.0 / c->kT);
     m.eps_jump = std::isinf(p->eps_jump) ? INFINITY : (float)p->eps_jump;
     m.eps_adaptive = p->eps_mode == 1 ? 1 : 0;
-    m.qmaxGM = (float)(c->qmax * c->GM); m.qmaxGL = (float)(c->qmax * c->GL);
-    m.GV4se = (float)(4.0 * std::sqrt(c->eps_max) * c->GV);
+    {
+        const double rlo = p->r_short - p->r_switch;
+        const double eA = std::min(std::max(c->rA, rlo), p->r_long), eM = std::min(std::max(c->rM, eA), p->r_long);
+        const double edge[4] = {rlo, eA, eM, p->r_long};
+        for (int y = 0; y < 4; ++y) { m.ring2d[y] = edge[y] * edge[y]; m.ring2[y] = (float)m.ring2d[y]; }
+        for (int y = 0; y < 3; ++y) {
+            m.qmaxG[y] = (float)(c->qmax * c->G[y]);
+            m.GV4se[y] = (float)(4.0 * std::sqrt(c->eps_max) * c->GV[y]);
+        }
+    }
     m.half_skin2 = (float)(0.25 * p->skin * p->skin);
     m.key0 = (unsigned)(p->seed & 0xffffffffu); m.key1 = (unsigned)(p->seed >> 32);
     // sort grid (R-10)
@@ -734,7 +757,7 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     if ((r = dalloc(c, &c->xs, n)) || (r = dalloc(c, &c->xs_nxt, n)) || (r = dalloc(c, &c->vs, n)) ||
         (r = dalloc(c, &c->vs_nxt, n)) || (r = dalloc(c, &c->xl, n)) || (r = dalloc(c, &c->xl_nxt, n)) || (r = dalloc(c, &c->x_build, n)) || (r = dalloc(c, &c->lj, n)) ||
         (r = dalloc(c, &c->lj_nxt, n)) || (r = dalloc(c, &c->mi, n)) || (r = dalloc(c, &c->mi_nxt, n)) ||
-        (r = dalloc(c, &c->orig, n)) || (r = dalloc(c, &c->orig_nxt, n)) || (r = dalloc(c, &c->sorted_of, n)) ||
+        (r = dalloc(c, &c->orig, n)) || (r = dalloc(c, &c->orig_nxt, n)) || (r = dalloc(c, &c->sorted_of, n)) || (r = dalloc(c, &c->cell_of, n)) ||
         (r = dalloc(c, &c->key, n)) || (r = dalloc(c, &c->tmp_orig, n)) || (r = dalloc(c, &c->tmp_src, n)) ||
         (r = dalloc(c, &c->cell_count, g.ncell + 1)) || (r = dalloc(c, &c->cell_fill, g.ncell + 1)) ||
         (r = dalloc(c, &c->cell_start, g.ncell + 1)) || (r = dalloc(c, &c->scan_sums, g.ncell / 4096 + 2)) ||
@@ -743,6 +766,36 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
         (r = dalloc(c, &c->ke, n)) || (r = dalloc(c, &c->ctr, 1)))
         return r;
     CK(cudaMemsetAsync(c->ctr, 0, sizeof(Counters), c->st));
+    CK(cudaMemsetAsync(c->fbond, 0, sizeof(float4) * n, c->st));   // atoms without bonded terms are never written
+    {   // cell universe of ring C (R-10c): stencil of the cells within reach r_long + skin of a cell, in fp64 from the
+        // caller's numbers (the oracle takes the same decisions from the same numbers)
+        Universe &u = c->uni;
+        memset(&u, 0, sizeof u);
+        const double reach = p->r_long + p->skin;
+        double w[3];
+        for (int k = 0; k < 3; ++k) {
+            w[k] = p->box[k] / g.gn[k];
+            u.R[k] = (int)std::ceil(reach / w[k]);   // <= 8: checked above (g.reach)
+            u.cnt[k] = std::min(2 * u.R[k] + 1, g.gn[k]);
+        }
+        u.nrow = u.cnt[2] * u.cnt[1];
+        u.stride = (u.nrow + 1 + 7) / 8 * 8;
+        for (int a = 0; a < 17; ++a)
+            for (int b = 0; b < 17; ++b) {
+                const double gz = (a > 1 ? a - 1 : 0) * w[2], gy = (b > 1 ? b - 1 : 0) * w[1];
+                const double rem = reach * reach - gz * gz - gy * gy;
+                int v = -1;
+                if (a <= u.R[2] && b <= u.R[1] && rem > 0.0) v = std::min(u.R[0], (int)std::floor(std::sqrt(rem) / w[0]) + 1);
+                u.xr[a * 17 + b] = (signed char)v;
+            }
+        c->uni_cum = nullptr;
+        if (coul_jumps(c) || lj_jumps(c)) {
+            if ((r = dalloc(c, &c->uni_cum, (size_t)g.ncell * u.stride))) return r;
+            CK(cudaMemsetAsync(c->uni_cum, 0, sizeof(unsigned short) * (size_t)g.ncell * u.stride, c->st));
+        }
+        u.cum = c->uni_cum;
+        u.cell_of = c->cell_of;
+    }
     c->event_cap = 0; c->events = nullptr;
     if (p->flags & JUMP_F_EVENT_LOG) {
         c->event_cap = std::min<long long>(std::max<long long>(1ll << 21, 512ll * n), 1ll << 25);
@@ -793,6 +846,61 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
             (r = dupload(c, &daa, aa)) || (r = dupload(c, &dab, ab)) || (r = dupload(c, &dak, ak)) || (r = dupload(c, &dat, at)))
             return r;
         c->topo = Topo{dbptr, dbo, dbk, dbr, daptr, dar, daa, dab, dak, dat};
+        // connected components of the bonded graph: those of at most three atoms become "small molecules" (one thread
+        // each, every term evaluated once); the atoms of the others keep the per-atom CSR
+        std::vector<int> root(n);
+        for (int i = 0; i < n; ++i) root[i] = i;
+        auto find = [&](int x) { while (root[x] != x) { root[x] = root[root[x]]; x = root[x]; } return x; };
+        auto unite = [&](int x, int y) { x = find(x); y = find(y); if (x != y) root[std::max(x, y)] = std::min(x, y); };
+        for (int b = 0; b < n_bonds; ++b) unite(hb[2 * b], hb[2 * b + 1]);
+        for (int a = 0; a < n_angles; ++a) { unite(ha[3 * a], ha[3 * a + 1]); unite(ha[3 * a], ha[3 * a + 2]); }
+        std::vector<int> csize(n, 0), cterms(n, 0), slot(n, -1);
+        for (int i = 0; i < n; ++i) csize[find(i)]++;
+        for (int b = 0; b < n_bonds; ++b) cterms[find(hb[2 * b])]++;
+        for (int a = 0; a < n_angles; ++a) cterms[find(ha[3 * a])]++;
+        std::vector<int4> mols;
+        std::vector<MolType> mtypes;
+        std::vector<int> big, mol_of(n, -1);
+        for (int i = 0; i < n; ++i) {   // members of a component in ascending original index; root = smallest index
+            const int r0 = find(i);
+            if (cterms[r0] == 0) continue;   // no bonded term: the gradient stays zero
+            if (csize[r0] > 3) { big.push_back(i); continue; }
+            if (mol_of[r0] < 0) { mol_of[r0] = (int)mols.size(); mols.push_back(make_int4(-1, -1, -1, 0)); }
+            int4 &mm = mols[mol_of[r0]];
+            if (mm.x < 0) { mm.x = i; slot[i] = 0; } else if (mm.y < 0) { mm.y = i; slot[i] = 1; } else { mm.z = i; slot[i] = 2; }
+        }
+        std::vector<MolType> per_mol(mols.size());
+        for (auto &t : per_mol) memset(&t, 0, sizeof t);
+        bool fits = true;
+        for (int b = 0; b < n_bonds && fits; ++b) {
+            const int r0 = find(hb[2 * b]);
+            if (csize[r0] > 3) continue;
+            MolType &t = per_mol[mol_of[r0]];
+            if (t.nb >= 3) { fits = false; break; }
+            t.bp[t.nb] = slot[hb[2 * b]]; t.bq[t.nb] = slot[hb[2 * b + 1]]; t.bk[t.nb] = hbk[b]; t.br0[t.nb] = hbr[b]; t.nb++;
+        }
+        for (int a = 0; a < n_angles && fits; ++a) {
+            const int r0 = find(ha[3 * a]);
+            if (csize[r0] > 3) continue;
+            MolType &t = per_mol[mol_of[r0]];
+            if (t.na >= 3) { fits = false; break; }
+            t.ai[t.na] = slot[ha[3 * a]]; t.av[t.na] = slot[ha[3 * a + 1]]; t.ak_[t.na] = slot[ha[3 * a + 2]];
+            t.ak[t.na] = hak[a]; t.at0[t.na] = hat[a]; t.na++;
+        }
+        for (size_t q = 0; q < mols.size() && fits; ++q) {   // identical term tables share one type (a water box has one)
+            int ty = -1;
+            for (size_t u = 0; u < mtypes.size(); ++u) if (!memcmp(&mtypes[u], &per_mol[q], sizeof(MolType))) { ty = (int)u; break; }
+            if (ty < 0) { if (mtypes.size() >= 64) { fits = false; break; } ty = (int)mtypes.size(); mtypes.push_back(per_mol[q]); }
+            mols[q].w = ty;
+        }
+        if (!fits) {   // a small component with more terms than a type holds, or too many kinds: all atoms through the CSR
+            big.clear();
+            for (int i = 0; i < n; ++i) if (cterms[find(i)] > 0) big.push_back(i);
+            mols.clear(); mtypes.clear();
+        }
+        int4 *dmols = nullptr; MolType *dtypes = nullptr; int *dbig = nullptr;
+        if ((r = dupload(c, &dmols, mols)) || (r = dupload(c, &dtypes, mtypes)) || (r = dupload(c, &dbig, big))) return r;
+        c->bonded = Bonded{(int)mols.size(), dmols, dtypes, (int)big.size(), dbig};
     }
     // rows: windows (R-10) and capacities from the mean density with head-room
     {
@@ -802,9 +910,9 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
         const double rho_lj = n_lj / vol;
         struct W { double a, b; int lj; bool on; } w[N_ROWS] = {
             {0.0, rc + s, 0, true},                              // S short list
-            {c->lo, c->rM, 0, true},                             // M ring
-            {std::max(c->rM, c->lo), rE + s, 0, true},           // L ring
-            {c->lo, rE + s, 1, lj_jumps(c)},                     // V: LJ jump partners
+            {c->lo, c->rA + s, 0, true},                         // A: candidates of ring [r_c-h, r_A) (R-10c)
+            {std::max(c->rA - s, c->lo), c->rM + s, 0, true},    // B: candidates of ring [r_A, r_M)
+            {0.0, 0.0, 0, false},                                // (unused)
             {0.0, rE + s, 0, false},                             // F: full list (lazy)
             {rc + s, rE + s, 1, !lj_jumps(c)}};                  // W: LJ tail kept in F0 (R-13)
         for (int k = 0; k < N_ROWS; ++k) {
@@ -826,7 +934,8 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     if ((r = resort_and_build(c))) return r;
     c->rebuilds = 1;
     {   // the rows this mode reads on every step, built in one launch
-        bool want[N_ROWS] = {true, coul_jumps(c), coul_jumps(c), lj_jumps(c), false, !lj_jumps(c)};
+        const bool jumps = coul_jumps(c) || lj_jumps(c);
+        bool want[N_ROWS] = {true, jumps, jumps, false, false, !lj_jumps(c)};
         for (int k = 0; k < N_ROWS; ++k) if (want[k] && (r = alloc_row(c, k))) return r;
         if ((r = build_rows(c, want))) return r;
     }
@@ -868,6 +977,7 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     c->vacf_v0 = nullptr; c->vacf_part = nullptr;
     c->fslow = nullptr; c->ew_sum = nullptr; c->q2sum = 0.0; c->outer1 = 0;
     c->prof = false;
+    c->lanes = 0; c->sort_step = 0; c->uni_cum = nullptr; c->cell_of = nullptr;
     for (int k = 0; k < 4; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     int r = init_impl(c, p, d_mass, d_charge, d_lj_sigma, d_lj_eps, n_bonds, d_bond_ij, d_bond_k, d_bond_r0, n_angles,
                       d_angle_ijk, d_angle_k, d_angle_t0, d_excl_ptr, d_excl_idx);
@@ -896,17 +1006,18 @@ extern "C" int jump_get_forces(jump_ctx *c, int32_t which, float *d_out) {
     if (!c || !d_out) return JUMP_E_ARG;
     int r = 0;
     const float4 *src = nullptr;
+    const float4 *src2 = nullptr;   // pieces are kept apart on the device (pair part + bonded part) and added on the way out
     switch (which) {
-        case 0: r = compute_f0_sum(c); src = c->f0; break;
-        case 1: r = compute_full(c, c->ftmp); src = c->ftmp; break;
+        case 0: r = compute_f0(c); src = c->fnb; src2 = c->fbond; break;
+        case 1: r = compute_full(c, false); src = c->ftmp2; src2 = c->fbond; break;
         case 2: r = compute_long(c, c->ftmp); src = c->ftmp; break;
-        case 3: r = bonded(c, nullptr, nullptr, c->fbond); src = c->fbond; break;
+        case 3: r = bonded_only(c); src = c->fbond; break;
         case 4: r = compute_short_nb(c, c->fnb); src = c->fnb; break;
         case 5: c->slow_valid = false; r = compute_slow(c); src = c->fslow; break;
         default: return JUMP_E_ARG;
     }
     if (r) return r;
-    launch_unsort3(c->n, src, c->orig, d_out, c->st, &c->launches);
+    launch_unsort3(c->n, src, src2, c->orig, d_out, c->st, &c->launches);
     CK(cudaGetLastError());
     return poll_error(c);
 }
@@ -923,11 +1034,11 @@ extern "C" int jump_get_energy(jump_ctx *c, double *e_kin, double *e_pot_full) {
         *e_kin = s;
     }
     if (e_pot_full) {
-        if ((r = compute_full(c, c->ftmp, true))) return r;
-        std::vector<float4> h;
-        if ((r = ddownload(c, h, (const float4 *)c->ftmp, c->n))) return r;
+        if ((r = compute_full(c, true))) return r;
+        std::vector<float4> h, hb;
+        if ((r = ddownload(c, h, (const float4 *)c->ftmp2, c->n)) || (r = ddownload(c, hb, (const float4 *)c->fbond, c->n))) return r;
         double s = 0.0;
-        for (const float4 &v : h) s += (double)v.w;
+        for (int i = 0; i < c->n; ++i) s += (double)h[i].w + (double)hb[i].w;
         *e_pot_full = s;
     }
     return poll_error(c);
@@ -983,18 +1094,35 @@ extern "C" int jump_clear_events(jump_ctx *c) {
 }
 extern "C" int jump_get_row(jump_ctx *c, int32_t which, int32_t atom, int32_t *host_out, int32_t cap) {
     if (!c || which < 0 || which >= N_ROWS || atom < 0 || atom >= c->n) return JUMP_E_ARG;
-    { int r = need_row(c, which); if (r) return r; }
-    const Row &R = c->rows[which];
+    int r;
     int i = 0, cnt = 0;
     CK(cudaMemcpyAsync(&i, c->sorted_of + atom, sizeof(int), cudaMemcpyDeviceToHost, c->st));
     CK(cudaStreamSynchronize(c->st));
-    CK(cudaMemcpyAsync(&cnt, R.cnt + i, sizeof(int), cudaMemcpyDeviceToHost, c->st));
-    CK(cudaStreamSynchronize(c->st));
     std::vector<int> row, orig;
-    int r;
-    if ((r = ddownload(c, row, (const int *)(R.idx + (size_t)i * R.cap), cnt)) || (r = ddownload(c, orig, (const int *)c->orig, c->n)))
-        return r;
-    for (int k = 0; k < cnt && k < cap; ++k) host_out[k] = orig[row[k]];
+    if (which == ROW_UNUSED) {   // the cell universe of the atom's home cell (ring C), through the lookup the chains use
+        if (!c->uni_cum) return 0;
+        int home = 0;
+        unsigned short tot = 0;
+        CK(cudaMemcpyAsync(&home, c->cell_of + i, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+        CK(cudaStreamSynchronize(c->st));
+        CK(cudaMemcpyAsync(&tot, c->uni_cum + (size_t)home * c->uni.stride + c->uni.nrow, sizeof tot, cudaMemcpyDeviceToHost, c->st));
+        CK(cudaStreamSynchronize(c->st));
+        cnt = tot;
+        int *d_list = nullptr;
+        CK(cudaMalloc(&d_list, sizeof(int) * std::max(cnt, 1)));
+        launch_universe_list(c->g, c->uni, c->cell_start, home, d_list, cnt, c->st, &c->launches);
+        r = ddownload(c, row, (const int *)d_list, cnt);
+        cudaFree(d_list);
+        if (r) return r;
+    } else {
+        if ((r = need_row(c, which))) return r;
+        const Row &R = c->rows[which];
+        CK(cudaMemcpyAsync(&cnt, R.cnt + i, sizeof(int), cudaMemcpyDeviceToHost, c->st));
+        CK(cudaStreamSynchronize(c->st));
+        if ((r = ddownload(c, row, (const int *)(R.idx + (size_t)i * R.cap), cnt))) return r;
+    }
+    if ((r = ddownload(c, orig, (const int *)c->orig, c->n))) return r;
+    for (int k = 0; k < cnt && k < cap; ++k) host_out[k] = orig[row[k] & 0x7fffffff];   // (bit 31: LJ flag of rows S, F, W)
     return cnt;
 }
 extern "C" int jump_get_images(jump_ctx *c, int32_t *d_img) {
@@ -1033,15 +1161,26 @@ extern "C" int jump_vacf_dot(jump_ctx *c, int32_t lj_only, double *c_out) {
     *c_out = h[0].y > 0.0 ? h[0].x / h[0].y : 0.0;
     return 0;
 }
-extern "C" int jump_get_bounds(jump_ctx *c, double out[8]) {
+extern "C" int jump_get_bounds(jump_ctx *c, double out[12]) {
     if (!c || !out) return JUMP_E_ARG;
-    out[0] = c->GM; out[1] = c->GL; out[2] = c->GV; out[3] = c->qmax;
+    out[0] = c->G[0]; out[1] = c->G[1]; out[2] = c->GV[0]; out[3] = c->qmax;
     out[4] = c->eps_max; out[5] = c->sig_min; out[6] = c->sig_max; out[7] = c->rM;
+    out[8] = c->G[2]; out[9] = c->GV[1]; out[10] = c->GV[2]; out[11] = c->rA;
+    return 0;
+}
+extern "C" int jump_set_lax_skin(jump_ctx *c, int32_t on) {
+    if (!c) return JUMP_E_ARG;
+    if (on) c->p.flags |= JUMP_F_LAX_SKIN; else c->p.flags &= ~JUMP_F_LAX_SKIN;
+    return 0;
+}
+extern "C" int jump_set_lanes(jump_ctx *c, int32_t lanes) {
+    if (!c || !(lanes == 0 || lanes == 1 || lanes == 4 || lanes == 8 || lanes == 16)) return JUMP_E_ARG;
+    c->lanes = lanes;
     return 0;
 }
 extern "C" int jump_refresh(jump_ctx *c) {
     if (!c) return JUMP_E_ARG;
-    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, nullptr, nullptr, c->st, &c->launches);
+    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, nullptr, nullptr, 0, c->st, &c->launches);
     CK(cudaGetLastError());
     int r = resort_and_build(c);
     if (r) return r;
@@ -1053,7 +1192,7 @@ extern "C" int jump_refresh_lazy(jump_ctx *c, int32_t *rebuilt) {
     int r;
     if (!c->moved_flag && (r = dalloc(c, &c->moved_flag, 1))) return r;
     CK(cudaMemsetAsync(c->moved_flag, 0, sizeof(int), c->st));
-    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, c->x_build, c->moved_flag, c->st, &c->launches);
+    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, c->x_build, c->moved_flag, 1, c->st, &c->launches);
     CK(cudaGetLastError());
     int moved = 0;
     CK(cudaMemcpyAsync(&moved, c->moved_flag, sizeof(int), cudaMemcpyDeviceToHost, c->st));

@@ -19,8 +19,9 @@ constexpr float kTwoOverSqrtPi = 1.1283791670955126f;
 
 // weight of a pair term: none, chi u (short), (1-chi) u (long), u (unsplit)
 enum { W_NONE = 0, W_SHORT = 1, W_LONG = 2, W_FULL = 3 };
-// row kinds
-enum { ROW_S = 0, ROW_M = 1, ROW_L = 2, ROW_V = 3, ROW_F = 4, ROW_W = 5, N_ROWS = 6 };
+// row kinds (R-10c): S short list; A, B candidates of the jump rings [r_c-h, r_A), [r_A, r_M); F full list (BAOAB
+// comparator); W LJ tail kept in F0 (R-13).  Ring C = [r_M, r_long) has no row: it draws from the cell universe.
+enum { ROW_S = 0, ROW_A = 1, ROW_B = 2, ROW_UNUSED = 3, ROW_F = 4, ROW_W = 5, N_ROWS = 6 };
 // device error bits
 enum { ERR_OVERFLOW = 1, ERR_BOUND = 2, ERR_SKIN = 4, ERR_NAN = 8, ERR_EVENTS = 16 };
 
@@ -53,8 +54,10 @@ struct Model {
     float beta;                   // 1/kT, (kcal/mol)^-1
     float eps_jump;               // epsilon; +inf -> BPS
     int eps_adaptive;             // eps(x) = eps_jump |F_ij(x)| (R-19)
-    float qmaxGM, qmaxGL;         // qmax * G_M, qmax * G_L  (L_Y,i = |q_i| * this, R-7)
-    float GV4se;                  // 4 sqrt(eps_max) G_V     (L^vdW_i = sqrt(eps_i) * this)
+    float qmaxG[3];               // qmax * G_Y, rings A, B, C   (L_Y,i = |q_i| * this, R-7)
+    float GV4se[3];               // 4 sqrt(eps_max) GV_Y        (L^vdW_Y,i = sqrt(eps_i) * this)
+    float ring2[4];               // squared ring edges (r_c-h)^2, r_A^2, r_M^2, r_long^2: ring Y = [ring2[Y], ring2[Y+1])
+    double ring2d[4];             // the same in fp64 (an edge decision within RING_TIE is retaken in fp64, R-17)
     float half_skin2;             // (skin/2)^2
     unsigned int key0, key1;      // Philox key = seed
 };
@@ -167,11 +170,96 @@ struct SortGrid {
     int reach[3];     // cells to visit on each side for the largest enabled row
 };
 
+// Cell universe of jump ring C (R-10c): the atoms of every contract-grid cell within reach r_long + skin of the home
+// cell, in ascending (cell key, original index) order = a list of contiguous runs of the cell-sorted atom array, one or
+// two per (z, y) cell row of the stencil.  Per home cell the library keeps the running sums of the row lengths
+// (cum[h][p], p = mz * cnt_y + my in ascending (z, y); cum[h][nrow] = size of the universe).
+struct Universe {
+    int R[3];                 // stencil reach in cells per dimension
+    int cnt[3];               // cells covered per dimension: min(2 R + 1, gn)
+    int nrow;                 // cnt[2] * cnt[1]
+    int stride;               // entries per home cell in cum (nrow + 1, padded)
+    signed char xr[17 * 17];  // [|oz| * 17 + |oy|] -> largest |ox| within reach, -1: (z, y) cell row out of reach
+    const unsigned short *cum;
+    const int *cell_of;       // home cell of each sorted atom
+};
+
+// m-th value, in ascending order, of the cyclic cell range [start, start+cnt) mod gn
+__host__ __device__ inline int cyc_val(int m, int start, int cnt, int gn) {
+    int w = start + cnt - gn;
+    if (w < 0) w = 0;
+    return m < w ? m : start + m - w;
+}
+__host__ __device__ inline int cyc_off(int val, int c, int gn) {
+    int o = val - c;
+    if (2 * o > gn) o -= gn;
+    else if (2 * o < -gn) o += gn;
+    return o;
+}
+// The runs of stencil row p of home cell (cx, cy, cz): sorted atoms [b0, b0 + n0) (cells wrapped to the low end of the
+// x axis, first in key order) then [b1, b1 + n1).  Shared by the table build (sort_build.cu) and the draw (update.cu).
+__device__ inline void universe_row(const SortGrid &g, const Universe &u, const int *__restrict__ cell_start, int cx, int cy,
+                                    int cz, int p, int &b0, int &n0, int &b1, int &n1) {
+    b0 = n0 = b1 = n1 = 0;
+    const int mz = p / u.cnt[1], my = p - mz * u.cnt[1];
+    const int sz = u.cnt[2] == g.gn[2] ? 0 : (cz - u.R[2] + g.gn[2]) % g.gn[2];
+    const int sy = u.cnt[1] == g.gn[1] ? 0 : (cy - u.R[1] + g.gn[1]) % g.gn[1];
+    const int zc = cyc_val(mz, sz, u.cnt[2], g.gn[2]), yc = cyc_val(my, sy, u.cnt[1], g.gn[1]);
+    int oz = cyc_off(zc, cz, g.gn[2]), oy = cyc_off(yc, cy, g.gn[1]);
+    oz = oz < 0 ? -oz : oz; oy = oy < 0 ? -oy : oy;
+    const int xm = u.xr[oz * 17 + oy];
+    if (xm < 0) return;
+    const int rowbase = (zc * g.gn[1] + yc) * g.gn[0];
+    if (2 * xm + 1 >= g.gn[0]) {
+        b1 = cell_start[rowbase]; n1 = cell_start[rowbase + g.gn[0]] - b1;
+    } else {
+        const int xs0 = (cx - xm + g.gn[0]) % g.gn[0], xc = 2 * xm + 1;
+        int w = xs0 + xc - g.gn[0];
+        if (w < 0) w = 0;
+        if (w > 0) { b0 = cell_start[rowbase]; n0 = cell_start[rowbase + w] - b0; }
+        b1 = cell_start[rowbase + xs0]; n1 = cell_start[rowbase + xs0 + xc - w] - b1;
+    }
+}
+
 struct Topo {  // per-atom CSR of bonded terms in ORIGINAL indices (device)
     const int *bptr, *bother;   // bonds: partner atom
     const float *bk, *br0;
     const int *aptr, *arole, *aa, *ab;  // angles: my role (0 end i, 1 vertex, 2 end k) and the two other atoms
     const float *ak, *at0;
+};
+
+// k-th atom (sorted index) of the universe of home cell h: bisection on the running sums of the stencil rows (a dozen
+// dependent 2-byte loads from a few cache lines), then the row's one or two runs
+__device__ inline int universe_pick(const SortGrid &g, const Universe &u, const int *__restrict__ cell_start, int h, int k) {
+    const unsigned short *__restrict__ cum = u.cum + (size_t)h * u.stride;
+    int lo = 0, hi = u.nrow - 1;   // last row with cum[row] <= k
+    while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if ((int)cum[mid] <= k) lo = mid; else hi = mid - 1;
+    }
+    const int cx = h % g.gn[0], cy = (h / g.gn[0]) % g.gn[1], cz = h / (g.gn[0] * g.gn[1]);
+    int b0, n0, b1, n1;
+    universe_row(g, u, cell_start, cx, cy, cz, lo, b0, n0, b1, n1);
+    const int kk = k - (int)cum[lo];
+    return kk < n0 ? b0 + kk : b1 + (kk - n0);
+}
+
+constexpr float RING_TIE = 4e-3f;   // A^2: an fp32 r^2 this close to a ring edge is re-decided in fp64 (R-17)
+
+// Bonded terms of one kind of small molecule (<= 3 atoms), local atom numbers 0..2 (forces.cu: k_bonded_mol)
+struct MolType {
+    int nb, na;
+    int bp[3], bq[3];
+    float bk[3], br0[3];
+    int ai[3], av[3], ak_[3];   // angle: end, vertex, end
+    float ak[3], at0[3];
+};
+struct Bonded {
+    int nmol;                 // small molecules: one thread each
+    const int4 *mols;         // (a0, a1, a2 original indices or -1, type)
+    const MolType *types;
+    int nbig;                 // atoms of larger components: per-atom CSR (Topo)
+    const int *big_atoms;     // original indices
 };
 
 struct Phase {      // one half-phase of velocity updates at frozen x

@@ -22,11 +22,14 @@ __device__ inline float weighted_u(float chi, float u) {
     return W == W_SHORT ? chi * u : (1.f - chi) * u;
 }
 
-template <int WC, int WLJ, bool ENERGY>
+// One warp per atom over its row (entries: sorted index of j, bit 31 set when j carries LJ).
+// INTERIOR: the atom is farther than the row's reach + 2 skins from every box face, so no partner of its row can
+// be a periodic image: plain differences, no minimum image in the inner loop.
+template <int WC, int WLJ, bool ENERGY, bool INTERIOR>
 __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *__restrict__ xs,
-                                 const float2 *__restrict__ lj, float4 *__restrict__ out, int accumulate, int i, int lane) {
+                                 const float2 *__restrict__ lj, float4 *__restrict__ out, int accumulate, int i, int lane,
+                                 const float4 xi) {
     const unsigned full = 0xffffffffu;
-    const float4 xi = xs[i];
     const float qi = (float)kCoulomb * xi.w;
     const float2 lji = lj[i];
     const float cutC2 = (WC == W_SHORT) ? m.rc2 : m.rE2, cutL2 = (WLJ == W_SHORT) ? m.rc2 : m.rE2;
@@ -34,50 +37,58 @@ __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *_
     const bool do_lj = (WLJ != W_NONE) && lji.y > 0.f;
     // both terms end at the same cutoff: the per-term tests after the common one are dropped at compile time
     constexpr bool SAME_CUT = WC == W_NONE || WLJ == W_NONE || ((WC == W_SHORT) == (WLJ == W_SHORT));
+    constexpr bool NEED_CHI = WC == W_SHORT || WC == W_LONG || WLJ == W_SHORT || WLJ == W_LONG;
+    const float na2l = -m.alpha2 * 1.4426950408889634f;   // exp(-alpha^2 r^2) = 2^(na2l r^2)
+    const float kq = kTwoOverSqrtPi * m.alpha;
+    const float u_b = -m.rlo * m.inv_h;                   // switching argument u = r / h - r_lo / h
     const int cnt = row.cnt[i];
     const int *__restrict__ ridx = row.idx + (size_t)i * row.cap;
     float fx = 0.f, fy = 0.f, fz = 0.f, en = 0.f;
     // software pipeline: the index two iterations ahead and the position one iteration ahead are in flight while
     // the current entry is evaluated (the gathers' L1/L2 latency was the kernel's largest stall)
     int j1 = lane < cnt ? ridx[lane] : 0, j2 = lane + 32 < cnt ? ridx[lane + 32] : 0;
-    float4 x1 = xs[j1];
+    float4 x1 = xs[j1 & 0x7fffffff];
     for (int k = lane; k < cnt; k += 32) {
-        const int j = j1;
+        const int jraw = j1;
         const float4 xj = x1;
         j1 = j2;
-        x1 = xs[j1];
+        x1 = xs[j1 & 0x7fffffff];
         j2 = k + 64 < cnt ? ridx[k + 64] : 0;
-        float ax, ay, az, bx, by, bz;
-        image_pair1(xi.x, xj.x, m.box[0], m.inv_box[0], ax, bx);
-        image_pair1(xi.y, xj.y, m.box[1], m.inv_box[1], ay, by);
-        image_pair1(xi.z, xj.z, m.box[2], m.inv_box[2], az, bz);
-        float dx = ax - bx, dy = ay - by, dz = az - bz;
-        float r2 = dx * dx + dy * dy + dz * dz;
+        float dx, dy, dz;
+        if (INTERIOR) { dx = xi.x - xj.x; dy = xi.y - xj.y; dz = xi.z - xj.z; }
+        else {
+            dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
+            dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
+            dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
+        }
+        const float r2 = dx * dx + dy * dy + dz * dz;
         if (r2 >= cut2) continue;
-        float rinv = rsqrtf(r2), r = r2 * rinv;
+        const float rinv = rsqrtf(r2), r = r2 * rinv;
         float fr = 0.f, chi = 1.f, dchi = 0.f;
-        if (WC == W_SHORT || WC == W_LONG || WLJ == W_SHORT || WLJ == W_LONG) chi = chi_zone<false>(ax, ay, az, bx, by, bz, r2, r, m, dchi);
+        if (NEED_CHI) {   // chi (R-3): quintic smootherstep on [r_c - h, r_c]; the clamp gives 1, 0 and chi' = 0 outside
+            const float u = __saturatef(fmaf(r, m.inv_h, u_b)), omu = 1.f - u, u2 = u * u;
+            dchi = -30.f * m.inv_h * (u2 * (omu * omu));
+            chi = fmaf(-(u2 * u), fmaf(u, fmaf(6.f, u, -15.f), 10.f), 1.f);
+        }
         if (WC != W_NONE && (SAME_CUT || r2 < cutC2)) {
-            float qq = qi * xj.w;
-            float ex = expf(-m.alpha2 * r2), e = ex * erfcx_poly(m.alpha * r);
-            float u = qq * e * rinv;
-            float du = -(u + qq * kTwoOverSqrtPi * m.alpha * ex) * rinv;  // u'
+            const float qq = qi * xj.w;
+            const float ex = exp2f(na2l * r2), e = ex * erfcx_poly(m.alpha * r);   // erfc(alpha r)
+            const float u = qq * e * rinv;
+            const float du = -(u + qq * kq * ex) * rinv;  // u'
             fr += weighted_du<WC>(chi, dchi, u, du);
             if (ENERGY) en += weighted_u<WC>(chi, u);
         }
-        if (do_lj && (SAME_CUT || r2 < cutL2)) {
-            float2 ljj = lj[j];
-            if (ljj.y > 0.f) {
-                float s = lji.x * ljj.x * rinv, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
-                float e4 = lji.y * ljj.y;  // 4 eps_ij (R-8: geometric mixing)
-                float u = e4 * (s12 - s6);
-                float du = e4 * (6.f * s6 - 12.f * s12) * rinv;
-                fr += weighted_du<WLJ>(chi, dchi, u, du);
-                if (ENERGY) en += weighted_u<WLJ>(chi, u);
-            }
+        if (do_lj && jraw < 0 && (SAME_CUT || r2 < cutL2)) {
+            const float2 ljj = lj[jraw & 0x7fffffff];
+            const float s = lji.x * ljj.x * rinv, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
+            const float e4 = lji.y * ljj.y;  // 4 eps_ij (R-8: geometric mixing)
+            const float u = e4 * (s12 - s6);
+            const float du = e4 * (6.f * s6 - 12.f * s12) * rinv;
+            fr += weighted_du<WLJ>(chi, dchi, u, du);
+            if (ENERGY) en += weighted_u<WLJ>(chi, u);
         }
-        float s = fr * rinv;
-        fx += s * dx; fy += s * dy; fz += s * dz;
+        const float s = fr * rinv;
+        fx = fmaf(s, dx, fx); fy = fmaf(s, dy, fy); fz = fmaf(s, dz, fz);
     }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
@@ -94,15 +105,25 @@ __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *_
 }
 
 template <int WC, int WLJ, bool ENERGY>
-__global__ void __launch_bounds__(256) k_pair(Model m, Row row, const float4 *__restrict__ xs,
+__global__ void __launch_bounds__(256) k_pair(Model m, Row row, float margin, const float4 *__restrict__ xs,
                                               const float2 *__restrict__ lj, float4 *__restrict__ out, int accumulate) {
     int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (i >= m.n) return;
-    pair_warp<WC, WLJ, ENERGY>(m, row, xs, lj, out, accumulate, i, lane);
+    const float4 xi = xs[i];
+    // margin = reach of the row + 2 skins (a partner was within reach at the build; both atoms moved < skin since)
+    const bool interior = xi.x > margin && xi.x < m.box[0] - margin && xi.y > margin && xi.y < m.box[1] - margin &&
+                          xi.z > margin && xi.z < m.box[2] - margin;
+    if (interior) pair_warp<WC, WLJ, ENERGY, true>(m, row, xs, lj, out, accumulate, i, lane, xi);
+    else pair_warp<WC, WLJ, ENERGY, false>(m, row, xs, lj, out, accumulate, i, lane, xi);
 }
 
-// Harmonic bonds k (r-r0)^2 and angles k (theta-theta0)^2 (R-2), one thread per atom over the terms
-// the atom takes part in; evaluated in fp64 (a few hundred flops per atom) because r - r0 cancels.
+// Harmonic bonds k (r-r0)^2 and angles k (theta-theta0)^2 (R-2), in fp64: at the equilibrium geometry r - r0 and
+// theta - theta0 cancel to rounding, and the gradient there is compared with the fp64 oracle's relative to its own
+// (tiny) size.  Every term is evaluated ONCE:
+//   k_bonded_mol  one thread per small molecule (a connected component of the bonded graph with at most three atoms:
+//                 water), its bonds and angles from a per-type table, the gradients of its atoms written directly --
+//                 each atom belongs to one molecule, so there is nothing to reduce and nothing atomic;
+//   k_bonded_csr  the atoms of larger components (chains), one thread per atom over the terms it takes part in.
 __device__ inline double min_image_d(double xi, double xj, float L) {
     double d = xi - xj, Ld = (double)L;
     return d - Ld * rint(d / Ld);
@@ -113,149 +134,112 @@ __device__ inline D3 full_pos(const float4 *__restrict__ xs, const float4 *__res
     float4 a = xs[i], b = xl[i];  // x = hi + lo (the A steps integrate in fp64, see update.cu)
     return D3{(double)a.x + (double)b.x, (double)a.y + (double)b.y, (double)a.z + (double)b.z};
 }
+__device__ inline D3 image_diff(const Model &m, const D3 &a, const D3 &b) {
+    return D3{min_image_d(a.x, b.x, m.box[0]), min_image_d(a.y, b.y, m.box[1]), min_image_d(a.z, b.z, m.box[2])};
+}
+// gradient of k (theta - theta0)^2 with respect to the two ends (u = end1 - vertex, w = end2 - vertex); the vertex takes
+// minus their sum
+__device__ inline double angle_term(const D3 &u, const D3 &w, double k, double t0, D3 &g1, D3 &g2) {
+    const double lu = sqrt(u.x * u.x + u.y * u.y + u.z * u.z), lw = sqrt(w.x * w.x + w.y * w.y + w.z * w.z);
+    double ct = (u.x * w.x + u.y * w.y + u.z * w.z) / (lu * lw);
+    ct = fmin(1.0, fmax(-1.0, ct));
+    const double th = acos(ct), st = fmax(sqrt(1.0 - ct * ct), 1e-12);
+    const double dth = th - t0, dU = 2.0 * k * dth;
+    const double c1 = -dU / (lu * st), c2 = -dU / (lw * st);
+    g1 = D3{c1 * (w.x / lw - ct * u.x / lu), c1 * (w.y / lw - ct * u.y / lu), c1 * (w.z / lw - ct * u.z / lu)};
+    g2 = D3{c2 * (u.x / lu - ct * w.x / lw), c2 * (u.y / lu - ct * w.y / lw), c2 * (u.z / lu - ct * w.z / lw)};
+    return k * dth * dth;
+}
 
-__global__ void k_bonded(Model m, Topo t, const float4 *__restrict__ xs, const float4 *__restrict__ xl,
-                         const int *__restrict__ orig,
-                         const int *__restrict__ sorted_of, const float4 *__restrict__ add,
-                         float4 *__restrict__ out_sum, float4 *__restrict__ out_bond) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= m.n) return;
-    const int o = orig[i];
+__device__ inline D3 sel3(const D3 x[3], int k) { return k == 0 ? x[0] : (k == 1 ? x[1] : x[2]); }
+
+__global__ void __launch_bounds__(128) k_bonded_mol(Model m, int nmol, const int4 *__restrict__ mols, const MolType *__restrict__ types,
+                                                    const float4 *__restrict__ xs, const float4 *__restrict__ xl,
+                                                    const int *__restrict__ sorted_of, float4 *__restrict__ out_bond) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= nmol) return;
+    const int4 a = mols[t];                      // original indices of the atoms (-1: none), type
+    const MolType ty = types[a.w];
+    int idx[3] = {sorted_of[a.x], a.y >= 0 ? sorted_of[a.y] : -1, a.z >= 0 ? sorted_of[a.z] : -1};
+    D3 x[3], g[3];
+    double e[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        x[k] = idx[k] >= 0 ? full_pos(xs, xl, idx[k]) : D3{0.0, 0.0, 0.0};
+        g[k] = D3{0.0, 0.0, 0.0};
+    }
+#pragma unroll
+    for (int b = 0; b < 3; ++b) {
+        if (b >= ty.nb) break;
+        const int p = ty.bp[b], q = ty.bq[b];
+        const D3 d = image_diff(m, sel3(x, p), sel3(x, q));
+        const double r = sqrt(d.x * d.x + d.y * d.y + d.z * d.z), dr = r - (double)ty.br0[b], k = (double)ty.bk[b];
+        const double f = 2.0 * k * dr / r;
+#pragma unroll
+        for (int k2 = 0; k2 < 3; ++k2) {   // (static indexing keeps x, g in registers)
+            const double sgn = k2 == p ? 1.0 : (k2 == q ? -1.0 : 0.0);
+            g[k2].x += sgn * f * d.x; g[k2].y += sgn * f * d.y; g[k2].z += sgn * f * d.z;
+            e[k2] += (sgn != 0.0 ? 0.5 : 0.0) * k * dr * dr;
+        }
+    }
+#pragma unroll
+    for (int an = 0; an < 3; ++an) {
+        if (an >= ty.na) break;
+        const int i1 = ty.ai[an], v = ty.av[an], i2 = ty.ak_[an];
+        const D3 xe1 = sel3(x, i1), xv = sel3(x, v), xe2 = sel3(x, i2);
+        D3 g1, g2;
+        const double en = angle_term(image_diff(m, xe1, xv), image_diff(m, xe2, xv), (double)ty.ak[an], (double)ty.at0[an], g1, g2);
+#pragma unroll
+        for (int k2 = 0; k2 < 3; ++k2) {
+            const double s1 = k2 == i1 ? 1.0 : 0.0, s2 = k2 == i2 ? 1.0 : 0.0, sv = k2 == v ? -1.0 : 0.0;
+            g[k2].x += s1 * g1.x + s2 * g2.x + sv * (g1.x + g2.x);
+            g[k2].y += s1 * g1.y + s2 * g2.y + sv * (g1.y + g2.y);
+            g[k2].z += s1 * g1.z + s2 * g2.z + sv * (g1.z + g2.z);
+            e[k2] += (k2 == i1 || k2 == i2 || k2 == v) ? en * (1.0 / 3.0) : 0.0;
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+        if (idx[k] >= 0) out_bond[idx[k]] = make_float4((float)g[k].x, (float)g[k].y, (float)g[k].z, (float)e[k]);
+}
+
+// atoms of larger components: one thread per listed atom (original index) over its CSR of terms
+__global__ void __launch_bounds__(128) k_bonded_csr(Model m, Topo t, int natoms, const int *__restrict__ atoms,
+                                                    const float4 *__restrict__ xs, const float4 *__restrict__ xl,
+                                                    const int *__restrict__ sorted_of, float4 *__restrict__ out_bond) {
+    const int q = blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= natoms) return;
+    const int o = atoms[q], i = sorted_of[o];
     const D3 xi = full_pos(xs, xl, i);
     double gx = 0., gy = 0., gz = 0., en = 0.;
     for (int b = t.bptr[o]; b < t.bptr[o + 1]; ++b) {
-        D3 xj = full_pos(xs, xl, sorted_of[t.bother[b]]);
-        double dx = min_image_d(xi.x, xj.x, m.box[0]);
-        double dy = min_image_d(xi.y, xj.y, m.box[1]);
-        double dz = min_image_d(xi.z, xj.z, m.box[2]);
-        double r = sqrt(dx * dx + dy * dy + dz * dz), dr = r - (double)t.br0[b], k = (double)t.bk[b];
-        double f = 2.0 * k * dr / r;
-        gx += f * dx; gy += f * dy; gz += f * dz;
+        const D3 d = image_diff(m, xi, full_pos(xs, xl, sorted_of[t.bother[b]]));
+        const double r = sqrt(d.x * d.x + d.y * d.y + d.z * d.z), dr = r - (double)t.br0[b], k = (double)t.bk[b];
+        const double f = 2.0 * k * dr / r;
+        gx += f * d.x; gy += f * d.y; gz += f * d.z;
         en += 0.5 * k * dr * dr;
     }
     for (int a = t.aptr[o]; a < t.aptr[o + 1]; ++a) {
         // role 1: I am the vertex, (aa, ab) are the ends; else I am an end, aa = vertex, ab = other end
         const int role = t.arole[a];
-        D3 xa = full_pos(xs, xl, sorted_of[t.aa[a]]), xb = full_pos(xs, xl, sorted_of[t.ab[a]]);
-        D3 xv = role == 1 ? xi : xa;             // vertex
-        D3 xe1 = role == 1 ? xa : xi;            // end whose gradient is "gi"
-        D3 xe2 = xb;                             // other end
-        double u[3], w[3];
-        u[0] = min_image_d(xe1.x, xv.x, m.box[0]);
-        u[1] = min_image_d(xe1.y, xv.y, m.box[1]);
-        u[2] = min_image_d(xe1.z, xv.z, m.box[2]);
-        w[0] = min_image_d(xe2.x, xv.x, m.box[0]);
-        w[1] = min_image_d(xe2.y, xv.y, m.box[1]);
-        w[2] = min_image_d(xe2.z, xv.z, m.box[2]);
-        double lu = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]), lw = sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
-        double ct = (u[0] * w[0] + u[1] * w[1] + u[2] * w[2]) / (lu * lw);
-        ct = fmin(1.0, fmax(-1.0, ct));
-        double th = acos(ct), st = fmax(sqrt(1.0 - ct * ct), 1e-12);
-        double dth = th - (double)t.at0[a], k = (double)t.ak[a], dU = 2.0 * k * dth;
-        double g[3];
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            double gi = -dU * (w[c] / lw - ct * u[c] / lu) / (lu * st);
-            if (role == 1) {
-                double gk = -dU * (u[c] / lu - ct * w[c] / lw) / (lw * st);
-                g[c] = -(gi + gk);
-            } else g[c] = gi;
-        }
-        gx += g[0]; gy += g[1]; gz += g[2];
-        en += k * dth * dth * (1.0 / 3.0);
+        const D3 xa = full_pos(xs, xl, sorted_of[t.aa[a]]), xb = full_pos(xs, xl, sorted_of[t.ab[a]]);
+        const D3 xv = role == 1 ? xi : xa, xe1 = role == 1 ? xa : xi;
+        D3 g1, g2;
+        const double e3 = angle_term(image_diff(m, xe1, xv), image_diff(m, xb, xv), (double)t.ak[a], (double)t.at0[a], g1, g2);
+        if (role == 1) { gx -= g1.x + g2.x; gy -= g1.y + g2.y; gz -= g1.z + g2.z; }
+        else { gx += g1.x; gy += g1.y; gz += g1.z; }
+        en += e3 * (1.0 / 3.0);
     }
-    float4 fb = make_float4((float)gx, (float)gy, (float)gz, (float)en);
-    if (out_bond) out_bond[i] = fb;
-    if (out_sum) {
-        if (add) { float4 p = add[i]; fb.x += p.x; fb.y += p.y; fb.z += p.z; fb.w += p.w; }
-        out_sum[i] = fb;
-    }
-}
-
-// The same bonded terms with BONDED_LANES lanes per atom (lane l takes the terms l, l + BONDED_LANES, ... of the
-// atom's bond-then-angle list; the partial sums are combined by shuffles in a fixed order: deterministic).
-constexpr int BONDED_LANES = 4;
-__device__ inline void bonded_term(const Model &m, const Topo &t, const float4 *__restrict__ xs, const float4 *__restrict__ xl,
-                                   const int *__restrict__ sorted_of, int o, const D3 &xi, int term, int nb, double &gx,
-                                   double &gy, double &gz, double &en) {
-    if (term < nb) {
-        const int b = t.bptr[o] + term;
-        D3 xj = full_pos(xs, xl, sorted_of[t.bother[b]]);
-        double dx = min_image_d(xi.x, xj.x, m.box[0]);
-        double dy = min_image_d(xi.y, xj.y, m.box[1]);
-        double dz = min_image_d(xi.z, xj.z, m.box[2]);
-        double r = sqrt(dx * dx + dy * dy + dz * dz), dr = r - (double)t.br0[b], k = (double)t.bk[b];
-        double f = 2.0 * k * dr / r;
-        gx += f * dx; gy += f * dy; gz += f * dz;
-        en += 0.5 * k * dr * dr;
-        return;
-    }
-    const int a = t.aptr[o] + (term - nb);
-    const int role = t.arole[a];
-    D3 xa = full_pos(xs, xl, sorted_of[t.aa[a]]), xb = full_pos(xs, xl, sorted_of[t.ab[a]]);
-    D3 xv = role == 1 ? xi : xa;
-    D3 xe1 = role == 1 ? xa : xi;
-    D3 xe2 = xb;
-    double u[3], w[3];
-    u[0] = min_image_d(xe1.x, xv.x, m.box[0]);
-    u[1] = min_image_d(xe1.y, xv.y, m.box[1]);
-    u[2] = min_image_d(xe1.z, xv.z, m.box[2]);
-    w[0] = min_image_d(xe2.x, xv.x, m.box[0]);
-    w[1] = min_image_d(xe2.y, xv.y, m.box[1]);
-    w[2] = min_image_d(xe2.z, xv.z, m.box[2]);
-    double lu = sqrt(u[0] * u[0] + u[1] * u[1] + u[2] * u[2]), lw = sqrt(w[0] * w[0] + w[1] * w[1] + w[2] * w[2]);
-    double ct = (u[0] * w[0] + u[1] * w[1] + u[2] * w[2]) / (lu * lw);
-    ct = fmin(1.0, fmax(-1.0, ct));
-    double th = acos(ct), st = fmax(sqrt(1.0 - ct * ct), 1e-12);
-    double dth = th - (double)t.at0[a], k = (double)t.ak[a], dU = 2.0 * k * dth;
-    double g[3];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-        double gi = -dU * (w[c] / lw - ct * u[c] / lu) / (lu * st);
-        if (role == 1) {
-            double gk = -dU * (u[c] / lu - ct * w[c] / lw) / (lw * st);
-            g[c] = -(gi + gk);
-        } else g[c] = gi;
-    }
-    gx += g[0]; gy += g[1]; gz += g[2];
-    en += k * dth * dth * (1.0 / 3.0);
-}
-__device__ inline void bonded_lanes(const Model &m, const Topo &t, const float4 *__restrict__ xs, const float4 *__restrict__ xl,
-                                    const int *__restrict__ orig, const int *__restrict__ sorted_of,
-                                    float4 *__restrict__ out_bond, int i, int gl, unsigned gmask) {
-    double gx = 0., gy = 0., gz = 0., en = 0.;
-    if (i < m.n) {
-        const int o = orig[i];
-        const D3 xi = full_pos(xs, xl, i);
-        const int nb = t.bptr[o + 1] - t.bptr[o], nt = nb + t.aptr[o + 1] - t.aptr[o];
-        for (int term = gl; term < nt; term += BONDED_LANES) bonded_term(m, t, xs, xl, sorted_of, o, xi, term, nb, gx, gy, gz, en);
-    }
-#pragma unroll
-    for (int off = 1; off < BONDED_LANES; off <<= 1) {
-        gx += __shfl_xor_sync(gmask, gx, off);
-        gy += __shfl_xor_sync(gmask, gy, off);
-        gz += __shfl_xor_sync(gmask, gz, off);
-        en += __shfl_xor_sync(gmask, en, off);
-    }
-    if (gl == 0 && i < m.n) out_bond[i] = make_float4((float)gx, (float)gy, (float)gz, (float)en);
-}
-
-// bonded gradient alone, BONDED_LANES lanes per atom (a fused pair + bonded launch was tried: the fp64 bonded code
-// raises the register count of the whole kernel and halves the occupancy of the pair warps -- 32 us instead of 20 + 4)
-__global__ void __launch_bounds__(128) k_bonded_lanes(Model m, Topo t, const float4 *__restrict__ xs,
-                                                      const float4 *__restrict__ xl, const int *__restrict__ orig,
-                                                      const int *__restrict__ sorted_of, float4 *__restrict__ out_bond) {
-    const int gt = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
-    const int i = gt / BONDED_LANES, gl = gt % BONDED_LANES;
-    const unsigned gmask = ((1u << BONDED_LANES) - 1u) << (lane & ~(BONDED_LANES - 1));
-    bonded_lanes(m, t, xs, xl, orig, sorted_of, out_bond, i, gl, gmask);
+    out_bond[i] = make_float4((float)gx, (float)gy, (float)gz, (float)en);
 }
 
 // out[orig[i]] = f[i].xyz  (sorted -> caller order)
-__global__ void k_unsort3(int n, const float4 *__restrict__ f, const int *__restrict__ orig, float *__restrict__ out) {
+__global__ void k_unsort3(int n, const float4 *__restrict__ f, const float4 *__restrict__ f2, const int *__restrict__ orig,
+                          float *__restrict__ out) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     float4 v = f[i];
+    if (f2) { const float4 w = f2[i]; v.x += w.x; v.y += w.y; v.z += w.z; }
     int o = orig[i];
     out[3 * o] = v.x; out[3 * o + 1] = v.y; out[3 * o + 2] = v.z;
 }
@@ -269,7 +253,7 @@ __global__ void k_count_pairs(Model m, Row row, const float4 *__restrict__ xs, f
     const int *__restrict__ ridx = row.idx + (size_t)i * row.cap;
     unsigned c = 0;
     for (int k = lane; k < cnt; k += 32) {
-        float4 xj = xs[ridx[k]];
+        float4 xj = xs[ridx[k] & 0x7fffffff];
         float dx = min_image1(xi.x, xj.x, m.box[0], m.inv_box[0]);
         float dy = min_image1(xi.y, xj.y, m.box[1], m.inv_box[1]);
         float dz = min_image1(xi.z, xj.z, m.box[2], m.inv_box[2]);
@@ -290,8 +274,9 @@ static void pair_dispatch(const Model &m, const Row &row, const float4 *xs, cons
                           bool energy, cudaStream_t st) {
     const int B = 256;
     unsigned grid = (unsigned)(((long long)m.n * 32 + B - 1) / B);
-    if (energy) k_pair<WC, WLJ, true><<<grid, B, 0, st>>>(m, row, xs, lj, out, accumulate);
-    else k_pair<WC, WLJ, false><<<grid, B, 0, st>>>(m, row, xs, lj, out, accumulate);
+    const float margin = sqrtf(row.r2max) + 2.f * sqrtf(m.half_skin2) * 2.f;   // reach + 2 skins
+    if (energy) k_pair<WC, WLJ, true><<<grid, B, 0, st>>>(m, row, margin, xs, lj, out, accumulate);
+    else k_pair<WC, WLJ, false><<<grid, B, 0, st>>>(m, row, margin, xs, lj, out, accumulate);
 }
 
 int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *xs, const float2 *lj, float4 *out,
@@ -306,23 +291,22 @@ int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *x
     return -1;
 }
 
-void launch_bonded_lanes(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig,
-                         const int *sorted_of, float4 *out_bond, cudaStream_t st, int64_t *launches) {
+void launch_bonded(const Model &m, const Topo &t, const Bonded &b, const float4 *xs, const float4 *xl, const int *sorted_of,
+                   float4 *out_bond, cudaStream_t st, int64_t *launches) {
     const int B = 128;
-    k_bonded_lanes<<<(unsigned)(((long long)m.n * BONDED_LANES + B - 1) / B), B, 0, st>>>(m, t, xs, xl, orig, sorted_of, out_bond);
-    *launches += 1;
+    if (b.nmol > 0) {
+        k_bonded_mol<<<(b.nmol + B - 1) / B, B, 0, st>>>(m, b.nmol, b.mols, b.types, xs, xl, sorted_of, out_bond);
+        *launches += 1;
+    }
+    if (b.nbig > 0) {
+        k_bonded_csr<<<(b.nbig + B - 1) / B, B, 0, st>>>(m, t, b.nbig, b.big_atoms, xs, xl, sorted_of, out_bond);
+        *launches += 1;
+    }
 }
 
-void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig, const int *sorted_of,
-                   const float4 *add, float4 *out_sum, float4 *out_bond, cudaStream_t st, int64_t *launches) {
-    const int B = 128;
-    k_bonded<<<(m.n + B - 1) / B, B, 0, st>>>(m, t, xs, xl, orig, sorted_of, add, out_sum, out_bond);
-    *launches += 1;
-}
-
-void launch_unsort3(int n, const float4 *f, const int *orig, float *out, cudaStream_t st, int64_t *launches) {
+void launch_unsort3(int n, const float4 *f, const float4 *f2, const int *orig, float *out, cudaStream_t st, int64_t *launches) {
     const int B = 256;
-    k_unsort3<<<(n + B - 1) / B, B, 0, st>>>(n, f, orig, out);
+    k_unsort3<<<(n + B - 1) / B, B, 0, st>>>(n, f, f2, orig, out);
     *launches += 1;
 }
 

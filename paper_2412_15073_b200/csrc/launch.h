@@ -12,7 +12,7 @@ struct SortArgs {
     const int *orig_in;
     float4 *xs, *vs, *xl, *x_build;
     float2 *lj, *mi;
-    int *orig, *sorted_of;
+    int *orig, *sorted_of, *cell_of;
     int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src;
     int *scan_sums, *scan_offs;   // scratch of the multi-block scan (ncell / 4096 + 2 each)
     Counters *ctr;
@@ -28,14 +28,20 @@ struct UpdateArgs {
     const float4 *xs;
     float4 *xs_out;
     float4 *vs;
-    float4 *xl;  // position residuals: x = xs + xl (updated in place)
+    float4 *xl_out;  // position residuals x - xs after A-O-A (a second buffer: the chains of other atoms still read xl_all)
     const float2 *mi, *lj;
     const int *orig;
     const float4 *x_build;
-    Row rowM, rowL, rowV;
+    Row rowA, rowB;
+    Universe uni;
+    SortGrid grid;
+    const int *cell_start;
+    const float4 *xl_all;   // position residuals (read-only use: ring-edge ties)
+    const int *excl_ptr, *excl_idx;   // exclusions by original index (ring C candidates are not filtered at a build)
     Counters *ctr;
     jump_event *events;  // NULL: no log
     long long event_cap;
+    int lanes;           // lanes per jump chain (0: chosen from the grid size)
 };
 
 struct EwaldArgs {   // reciprocal Ewald sum (ewald.cu, R-21)
@@ -56,18 +62,20 @@ struct EwaldArgs {   // reciprocal Ewald sum (ewald.cu, R-21)
 };
 
 void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches);
+void launch_universe(const SortGrid &g, const Universe &u, const int *cell_start, unsigned short *cum, Counters *ctr,
+                     cudaStream_t st, int64_t *launches);
+int launch_universe_list(const SortGrid &g, const Universe &u, const int *cell_start, int home, int *out, int cap,
+                         cudaStream_t st, int64_t *launches);
 void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS], float rmax_all, const int *cell_start,
                        const float4 *xs, const float4 *xl, const float2 *lj, const int *orig, const int *sorted_of,
                        const int *excl_ptr, const int *excl_idx, Counters *ctr, cudaStream_t st, int64_t *launches);
 int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *xs, const float2 *lj, float4 *out,
                 int accumulate, bool energy, cudaStream_t st, int64_t *launches);
-void launch_bonded_lanes(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig,
-                         const int *sorted_of, float4 *out_bond, cudaStream_t st, int64_t *launches);
 void launch_count_pairs(const Model &m, const Row &row, const float4 *xs, float rc2, unsigned long long *out,
                         cudaStream_t st, int64_t *launches);
-void launch_bonded(const Model &m, const Topo &t, const float4 *xs, const float4 *xl, const int *orig, const int *sorted_of,
-                   const float4 *add, float4 *out_sum, float4 *out_bond, cudaStream_t st, int64_t *launches);
-void launch_unsort3(int n, const float4 *f, const int *orig, float *out, cudaStream_t st, int64_t *launches);
+void launch_bonded(const Model &m, const Topo &t, const Bonded &b, const float4 *xs, const float4 *xl, const int *sorted_of,
+                   float4 *out_bond, cudaStream_t st, int64_t *launches);
+void launch_unsort3(int n, const float4 *f, const float4 *f2, const int *orig, float *out, cudaStream_t st, int64_t *launches);
 void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st, int64_t *launches);
 void launch_writeback(int n, const float4 *xs, const float4 *vs, const int *orig, float *pos, float *vel, cudaStream_t st,
                       int64_t *launches);
@@ -75,7 +83,7 @@ void launch_load(const Model &m, const float *pos, const float *vel, const float
                  const float *sigma, const float *eps, double kT, float4 *xs, float4 *vs, float4 *xl, float2 *lj, float2 *mi, int *orig,
                  cudaStream_t st, int64_t *launches);
 void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
-                   float4 *xl, const float4 *x_build, int *moved, cudaStream_t st, int64_t *launches);
+                   float4 *xl, const float4 *x_build, int *moved, int keep, cudaStream_t st, int64_t *launches);
 int launch_rdf(const Model &m, const SortGrid &g, int lj_only, double r_max, double r_reach, int n_bins, const int *cell_start,
                const float4 *xs, const float2 *lj, unsigned long long *hist, cudaStream_t st, int64_t *launches);
 void launch_vacf_mark(int n, const float4 *vs, const int *orig, float4 *v0, cudaStream_t st, int64_t *launches);

@@ -138,10 +138,11 @@ __global__ void k_permute(int n, const int *__restrict__ src, const int *__restr
                           const float2 *__restrict__ lj_in, const float2 *__restrict__ mi_in,
                           float4 *__restrict__ xs, float4 *__restrict__ vs, float2 *__restrict__ lj,
                           float2 *__restrict__ mi, int *__restrict__ orig, int *__restrict__ sorted_of,
-                          float4 *__restrict__ x_build) {
+                          float4 *__restrict__ x_build, const int *__restrict__ key, int *__restrict__ cell_of) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int s = src[i];
+    cell_of[i] = key[s];
     float4 x = xs_in[s];
     xs[i] = x;
     x_build[i] = x;
@@ -155,18 +156,6 @@ __global__ void k_permute(int n, const int *__restrict__ src, const int *__restr
 }
 
 struct RowSet { Row r[N_ROWS]; };
-
-// m-th value, in ascending order, of the cyclic cell range [start, start+cnt) mod gn
-__device__ inline int cyc_val(int m, int start, int cnt, int gn) {
-    int w = max(0, start + cnt - gn);
-    return m < w ? m : start + m - w;
-}
-__device__ inline int cyc_off(int val, int c, int gn) {
-    int o = val - c;
-    if (2 * o > gn) o -= gn;
-    else if (2 * o < -gn) o += gn;
-    return o;
-}
 
 // d wrapped to the periodic image nearest to 0
 __device__ inline float near_image1(float d, float L, float invL) {
@@ -208,7 +197,7 @@ constexpr float BUILD_TIE = 4e-3f;          // A^2
 struct Stencil {
     int R[3];                 // cells on each side, per dimension
     int n_edge;               // distinct window edges of the selected rows (squared, fp32)
-    float edge2[4];           // padded with a value no r^2 comes near
+    float edge2[6];           // padded with a value no r^2 comes near
     signed char xr[17 * 17];  // [|oz| * 17 + |oy|] -> largest |ox| still within reach, -1: skip the (z, y) cell row
 };
 
@@ -369,14 +358,14 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                     count[k] = JB_ROW_ON(k) ? s_count[i - g0][k] : 0;
                     rbase[k] = JB_ROW_ON(k) ? rows.r[k].idx + (size_t)i * rows.r[k].cap : nullptr;
                 }
-                const float e0 = stn.edge2[0], e1 = stn.edge2[1], e2 = stn.edge2[2], e3 = stn.edge2[3];
-                // The scan is instantiated twice: an atom without LJ (two thirds of a water box) has no V / W row, and
+                const float e0 = stn.edge2[0], e1 = stn.edge2[1], e2 = stn.edge2[2], e3 = stn.edge2[3], e4 = stn.edge2[4], e5 = stn.edge2[5];
+                // The scan is instantiated twice: an atom without LJ (two thirds of a water box) has no W row, and
                 // its copy of the loop carries no test, ballot or counter for them (MASK >= 0; a branch on this
                 // inside the unrolled row loop was measured slower than the work it skips).
                 auto scan = [&](auto lj_tag) {
                     constexpr bool LJ_I = decltype(lj_tag)::value;
-#define JB_ROW_SCAN(k) (JB_ROW_ON(k) && (LJ_I || MASK < 0 || ((k) != ROW_V && (k) != ROW_W)))
-#define JB_LJ_ROW(k) (MASK >= 0 ? ((k) == ROW_V || (k) == ROW_W) : rows.r[k].lj_only != 0)   // V and W are the LJ-only rows
+#define JB_ROW_SCAN(k) (JB_ROW_ON(k) && (LJ_I || MASK < 0 || (k) != ROW_W))
+#define JB_LJ_ROW(k) (MASK >= 0 ? (k) == ROW_W : rows.r[k].lj_only != 0)   // W is the LJ-only row
                     for (int q0 = 0; q0 < npad; q0 += 32) {
                         const float4 xj = tile[q0 + lane];
                         const int jraw = __float_as_int(xj.w);
@@ -412,7 +401,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                             const Row &R = rows.r[k];
                             pass[k] = valid && (!JB_LJ_ROW(k) || ljp) && r2 >= R.r2min && r2 < R.r2max;
                         }
-                        const bool tie = valid && fminf(fminf(fabsf(r2 - e0), fabsf(r2 - e1)), fminf(fabsf(r2 - e2), fabsf(r2 - e3))) < BUILD_TIE;
+                        const bool tie = valid && fminf(fminf(fminf(fabsf(r2 - e0), fabsf(r2 - e1)), fminf(fabsf(r2 - e2), fabsf(r2 - e3))), fminf(fabsf(r2 - e4), fabsf(r2 - e5))) < BUILD_TIE;
                         if (tie) {   // decide in fp64 from the full positions, like the oracle
                             float4 hi_j = xs[j], li = xl[i], lo_j = xl[j];
                             double d[3] = {((double)xi4.x + (double)li.x) - ((double)hi_j.x + (double)lo_j.x),
@@ -437,7 +426,8 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                             if (!JB_ROW_SCAN(k)) continue;
                             const unsigned mask = __ballot_sync(full, pass[k]);
                             const int pos = count[k] + __popc(mask & lt_mask);
-                            store_if(pass[k] && pos < rows.r[k].cap, rbase[k] + pos, j);   // predicated, no branch
+                            // rows the pair kernel reads carry j's LJ flag in bit 31; the jump rows A, B plain indices
+                            store_if(pass[k] && pos < rows.r[k].cap, rbase[k] + pos, (k == ROW_A || k == ROW_B) ? j : jraw);
                             count[k] += __popc(mask);
                         }
                     }
@@ -467,6 +457,46 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
 #undef JB_ROW_ON
 }
 
+// ---- cell universe of jump ring C (R-10c) -----------------------------------------------------------------------
+// One warp per home cell: the lengths of its stencil rows (two cell_start differences each), prefix-summed into
+// cum[h][0 .. nrow]; cum[h][nrow] is the size of the universe, N_C of every atom of the cell.
+__global__ void __launch_bounds__(128) k_universe(SortGrid g, Universe u, const int *__restrict__ cell_start,
+                                                  unsigned short *__restrict__ cum, Counters *ctr) {
+    const int h = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (h >= g.ncell) return;
+    if (cell_start[h + 1] == cell_start[h]) return;   // no atom lives here: the row is never read
+    const int cx = h % g.gn[0], cy = (h / g.gn[0]) % g.gn[1], cz = h / (g.gn[0] * g.gn[1]);
+    unsigned short *out = cum + (size_t)h * u.stride;
+    int run = 0;
+    for (int p0 = 0; p0 < u.nrow; p0 += 32) {
+        const int p = p0 + lane;
+        int len = 0;
+        if (p < u.nrow) {
+            int b0, n0, b1, n1;
+            universe_row(g, u, cell_start, cx, cy, cz, p, b0, n0, b1, n1);
+            len = n0 + n1;
+        }
+        int inc = len;
+#pragma unroll
+        for (int off = 1; off < 32; off <<= 1) {
+            const int up = __shfl_up_sync(0xffffffffu, inc, off);
+            if (lane >= off) inc += up;
+        }
+        if (p < u.nrow) out[p] = (unsigned short)min(run + inc - len, 65535);
+        run += __shfl_sync(0xffffffffu, inc, 31);
+    }
+    if (lane == 0) {
+        out[u.nrow] = (unsigned short)min(run, 65535);
+        if (run >= 65535) atomicOr(&ctr->err, (unsigned)ERR_OVERFLOW);   // 16-bit running sums
+    }
+}
+// the universe of one home cell as a list of sorted indices (observer: jump_get_row), one thread per entry, through the
+// same lookup the jump chains use
+__global__ void k_universe_list(SortGrid g, Universe u, const int *__restrict__ cell_start, int h, int n, int *__restrict__ out) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) out[k] = universe_pick(g, u, cell_start, h, k);
+}
+
 // ------------------------------------------------------------------------------------------
 static inline int nblk(int n, int b) { return (n + b - 1) / b; }
 
@@ -487,8 +517,21 @@ void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches) {
     k_scatter<<<nblk(a.n, B), B, 0, st>>>(a.n, a.key, a.orig_in, a.cell_start, a.cell_fill, a.tmp_orig, a.tmp_src);
     k_cell_sort<<<nblk(a.grid.ncell, B), B, 0, st>>>(a.grid.ncell, a.cell_start, a.tmp_orig, a.tmp_src);
     k_permute<<<nblk(a.n, B), B, 0, st>>>(a.n, a.tmp_src, a.tmp_orig, a.xs_in, a.vs_in, a.xl_in, a.xl, a.lj_in, a.mi_in, a.xs, a.vs,
-                                          a.lj, a.mi, a.orig, a.sorted_of, a.x_build);
+                                          a.lj, a.mi, a.orig, a.sorted_of, a.x_build, a.key, a.cell_of);
     *launches += 5;
+}
+
+void launch_universe(const SortGrid &g, const Universe &u, const int *cell_start, unsigned short *cum, Counters *ctr,
+                     cudaStream_t st, int64_t *launches) {
+    const int B = 128;
+    k_universe<<<(unsigned)(((long long)g.ncell * 32 + B - 1) / B), B, 0, st>>>(g, u, cell_start, cum, ctr);
+    *launches += 1;
+}
+int launch_universe_list(const SortGrid &g, const Universe &u, const int *cell_start, int home, int *out, int n,
+                         cudaStream_t st, int64_t *launches) {
+    if (n > 0) k_universe_list<<<(n + 127) / 128, 128, 0, st>>>(g, u, cell_start, home, n, out);
+    *launches += 1;
+    return 0;
 }
 
 void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS], float rmax_all, const int *cell_start,
@@ -509,11 +552,10 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
         for (float e : {rows[k].r2min, rows[k].r2max}) {
             bool seen = e <= 0.f;
             for (int q = 0; q < stn.n_edge; ++q) seen |= stn.edge2[q] == e;
-            if (!seen && stn.n_edge < 4) stn.edge2[stn.n_edge++] = e;
-            else if (!seen) stn.n_edge = 5;   // cannot happen with the windows of api.cu (<= 4 distinct edges)
+            if (!seen && stn.n_edge < 6) stn.edge2[stn.n_edge++] = e;   // the windows of api.cu have <= 6 distinct edges
         }
     }
-    for (int q = stn.n_edge; q < 4; ++q) stn.edge2[q] = -1e30f;
+    for (int q = stn.n_edge; q < 6; ++q) stn.edge2[q] = -1e30f;
     const double r2 = (double)rmax_all * rmax_all;
     for (int a = 0; a < 17; ++a)
         for (int b = 0; b < 17; ++b) {
@@ -540,8 +582,8 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
                                                                                     orig, sorted_of, excl_ptr, excl_idx, ctr);            \
     } while (0)
     switch (mask) {
-        case 0x0F: JB_BUILD(0x0F); break;   // S M L V   (JUMP with Coulomb and LJ jumps)
-        case 0x27: JB_BUILD(0x27); break;   // S M L W   (Coulomb jumps only, R-13)
+        case 0x07: JB_BUILD(0x07); break;   // S A B     (JUMP with Coulomb and LJ jumps)
+        case 0x27: JB_BUILD(0x27); break;   // S A B W   (Coulomb jumps only, R-13)
         case 0x10: JB_BUILD(0x10); break;   // F         (BAOAB comparator)
         case 0x01: JB_BUILD(0x01); break;   // S
         default: JB_BUILD(-1); break;

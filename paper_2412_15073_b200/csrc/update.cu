@@ -7,8 +7,6 @@
 // Chains of different atoms are independent and a jump of type (i,j) changes v_i only
 // (P:L342): one chain per thread, writing nothing but its own v_i -- no cross-atom conflict; several
 // events on one atom are resolved in time order inside its chain.
-#include <cstdlib>
-
 #include "launch.h"
 
 namespace jb {
@@ -85,41 +83,37 @@ __device__ inline void jump_kick(float eps, float sbm, float nx, float ny, float
     vx -= amp * nx; vy -= amp * ny; vz -= amp * nz;
 }
 
-// long part of the Coulomb pair gradient, F_ij = grad_{x_i} (1-chi) u_C: returns fr = radial
-// derivative, d = minimum-image x_i - x_j, r
-__device__ inline float fij_coul(const Model &m, const float4 &xi, const float4 &xj, float &dx, float &dy, float &dz,
-                                 float &rinv) {
-    float ax, ay, az, bx, by, bz;
-    image_pair1(xi.x, xj.x, m.box[0], m.inv_box[0], ax, bx);
-    image_pair1(xi.y, xj.y, m.box[1], m.inv_box[1], ay, by);
-    image_pair1(xi.z, xj.z, m.box[2], m.inv_box[2], az, bz);
-    dx = ax - bx; dy = ay - by; dz = az - bz;
-    float r2 = dx * dx + dy * dy + dz * dz;
-    if (r2 >= m.rE2 || r2 <= m.rlo2) { rinv = 0.f; return 0.f; }
-    rinv = rsqrtf(r2);
-    float r = r2 * rinv;
-    float qq = (float)kCoulomb * xi.w * xj.w;
-    float ex = expf(-m.alpha2 * r2), e = ex * erfcx_poly(m.alpha * r);
+// geometry of a candidate pair: exact image pair (a, b) per dimension, d = a - b, r^2
+struct PairGeom { float ax, ay, az, bx, by, bz, dx, dy, dz, r2; };
+__device__ inline PairGeom pair_geom(const Model &m, const float4 &xi, const float4 &xj) {
+    PairGeom p;
+    image_pair1(xi.x, xj.x, m.box[0], m.inv_box[0], p.ax, p.bx);
+    image_pair1(xi.y, xj.y, m.box[1], m.inv_box[1], p.ay, p.by);
+    image_pair1(xi.z, xj.z, m.box[2], m.inv_box[2], p.az, p.bz);
+    p.dx = p.ax - p.bx; p.dy = p.ay - p.by; p.dz = p.az - p.bz;
+    p.r2 = p.dx * p.dx + p.dy * p.dy + p.dz * p.dz;
+    return p;
+}
+// long part of the Coulomb pair gradient, F_ij = grad_{x_i} (1-chi) u_C: returns the radial derivative
+__device__ inline float fij_coul(const Model &m, const PairGeom &p, float qi, float qj, float &rinv) {
+    if (p.r2 >= m.rE2 || p.r2 <= m.rlo2) { rinv = 0.f; return 0.f; }
+    rinv = rsqrtf(p.r2);
+    float r = p.r2 * rinv;
+    float qq = (float)kCoulomb * qi * qj;
+    float ex = expf(-m.alpha2 * p.r2), e = ex * erfcx_poly(m.alpha * r);
     float u = qq * e * rinv;
     float du = -(u + qq * kTwoOverSqrtPi * m.alpha * ex) * rinv;
-    float dchi, chi = chi_zone<true>(ax, ay, az, bx, by, bz, r2, r, m, dchi);
+    float dchi, chi = chi_zone<true>(p.ax, p.ay, p.az, p.bx, p.by, p.bz, p.r2, r, m, dchi);
     return (1.f - chi) * du - dchi * u;
 }
-__device__ inline float fij_lj(const Model &m, const float4 &xi, const float4 &xj, float2 lji, float2 ljj, float &dx,
-                               float &dy, float &dz, float &rinv) {
-    float ax, ay, az, bx, by, bz;
-    image_pair1(xi.x, xj.x, m.box[0], m.inv_box[0], ax, bx);
-    image_pair1(xi.y, xj.y, m.box[1], m.inv_box[1], ay, by);
-    image_pair1(xi.z, xj.z, m.box[2], m.inv_box[2], az, bz);
-    dx = ax - bx; dy = ay - by; dz = az - bz;
-    float r2 = dx * dx + dy * dy + dz * dz;
-    if (r2 >= m.rE2 || r2 <= m.rlo2) { rinv = 0.f; return 0.f; }
-    rinv = rsqrtf(r2);
-    float r = r2 * rinv;
+__device__ inline float fij_lj(const Model &m, const PairGeom &p, float2 lji, float2 ljj, float &rinv) {
+    if (p.r2 >= m.rE2 || p.r2 <= m.rlo2 || !(ljj.y > 0.f)) { rinv = 0.f; return 0.f; }
+    rinv = rsqrtf(p.r2);
+    float r = p.r2 * rinv;
     float s = lji.x * ljj.x * rinv, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
     float e4 = lji.y * ljj.y;
     float u = e4 * (s12 - s6), du = e4 * (6.f * s6 - 12.f * s12) * rinv;
-    float dchi, chi = chi_zone<true>(ax, ay, az, bx, by, bz, r2, r, m, dchi);
+    float dchi, chi = chi_zone<true>(p.ax, p.ay, p.az, p.bx, p.by, p.bz, p.r2, r, m, dchi);
     return (1.f - chi) * du - dchi * u;
 }
 
@@ -135,39 +129,68 @@ __device__ inline float fij_lj(const Model &m, const float4 &xi, const float4 &x
 //    probability and its accept test at once;
 //  * the first accepting lane (a ballot) ends the epoch: kick, new bound, the later lanes are dropped and the
 //    batch restarts after it -- accepted jumps are ~1-2 % of the proposals.
-struct ChainConst {   // per-atom constants of a C' chain
-    int NM, NL;
-    float LM, LL, SM, S;
+struct ChainConst {   // per-atom constants of the jump chains (R-10c): the three rings of P:L424
+    int N[3];         // candidates: row A, row B, the cell universe of the home cell
+    int home;         // home cell (ring C)
 };
-__device__ inline ChainConst chain_const(const Model &m, const Row &rowM, const Row &rowL, int i, float qi) {
+__device__ inline ChainConst chain_const(const UpdateArgs &A, int i) {
     ChainConst c;
-    c.NM = rowM.cnt[i]; c.NL = rowL.cnt[i];
-    const float aq = fabsf(qi);
-    c.LM = aq * m.qmaxGM; c.LL = aq * m.qmaxGL;
-    c.SM = (float)c.NM * c.LM; c.S = c.SM + (float)c.NL * c.LL;
+    c.N[0] = A.rowA.cnt[i]; c.N[1] = A.rowB.cnt[i];
+    c.home = A.uni.cell_of[i];
+    c.N[2] = (int)A.uni.cum[(size_t)c.home * A.uni.stride + A.uni.nrow];
     return c;
 }
-// state-independent part of a proposal, from its Philox block w: ring pick and partner, then
-// goL = |F_ij| / L_Y and n = F_ij / |F_ij|; tag = ring << 31 | j_orig (event log only)
-template <bool WANT_J>
-__device__ inline void propose_pair(const Model &m, const Row &rowM, const Row &rowL, const float4 *__restrict__ xs,
-                                    const int *__restrict__ orig, const ChainConst &c, float ringS, float ringM, int i,
-                                    const float4 &xi, const uint32_t w[4], float &g, float &LY, float &nx, float &ny,
-                                    float &nz, int &tag) {
-    int ring = (u01(w[1]) * ringS < ringM) ? 0 : 1;   // ring M with probability ringM / ringS
-    if (ring == 0 && c.NM == 0) ring = 1;
-    if (ring == 1 && c.NL == 0) ring = 0;
-    const int cnt = ring == 0 ? c.NM : c.NL;
-    const int k = (int)__umulhi(w[2], (unsigned)cnt);
-    const int j = ring == 0 ? rowM.idx[(size_t)i * rowM.cap + k] : rowL.idx[(size_t)i * rowL.cap + k];
-    float dx, dy, dz, rinv;
-    const float fr = fij_coul(m, xi, xs[j], dx, dy, dz, rinv);
+// ring pick: the first ring whose cumulated weight exceeds ur * (sum of weights); a ring without
+// candidates can only be hit through rounding at an end, and the pick then falls back as the oracle's does
+__device__ inline int pick_ring(const ChainConst &c, float ur, float c0, float c1, float tot) {
+    const float x = ur * tot;
+    int ring = x < c0 ? 0 : (x < c1 ? 1 : 2);
+    while (c.N[ring] == 0 && ring > 0) --ring;
+    while (c.N[ring] == 0 && ring < 2) ++ring;
+    return ring;
+}
+// state-independent part of a proposal, from its Philox block w: ring pick and partner, the ring the
+// pair's CURRENT distance lies in (R-10c: through any other ring its rate is 0), then g = |F_ij| and n = F_ij / |F_ij|;
+// tag = ring << 28 | j_orig (event log only).  LJ: the long LJ gradient (step J') instead of the Coulomb one.
+template <bool LJ, bool WANT_J>
+__device__ inline void propose_pair(const Model &m, const UpdateArgs &A, const ChainConst &c, float c0, float c1, float tot,
+                                    int i, const float4 &xi, float2 lji, const uint32_t w[4], float &g, int &ring, float &nx,
+                                    float &ny, float &nz, int &tag) {
+    ring = pick_ring(c, u01(w[1]), c0, c1, tot);
+    const int k = (int)__umulhi(w[2], (unsigned)c.N[ring]);
+    int j;
+    if (ring == 0) j = A.rowA.idx[(size_t)i * A.rowA.cap + k];
+    else if (ring == 1) j = A.rowB.idx[(size_t)i * A.rowB.cap + k];
+    else j = universe_pick(A.grid, A.uni, A.cell_start, c.home, k);
+    const float4 xj = A.xs[j];
+    const PairGeom p = pair_geom(m, xi, xj);
+    const float lo2 = m.ring2[ring], hi2 = m.ring2[ring + 1];
+    bool in = p.r2 >= lo2 && p.r2 < hi2;
+    if (fminf(fabsf(p.r2 - lo2), fabsf(p.r2 - hi2)) < RING_TIE) {   // decide in fp64 from the full positions, like the oracle
+        const float4 li = A.xl_all[i], lo_j = A.xl_all[j];
+        double d[3] = {((double)xi.x + (double)li.x) - ((double)xj.x + (double)lo_j.x),
+                       ((double)xi.y + (double)li.y) - ((double)xj.y + (double)lo_j.y),
+                       ((double)xi.z + (double)li.z) - ((double)xj.z + (double)lo_j.z)};
+        double r2d = 0.0;
+#pragma unroll
+        for (int q = 0; q < 3; ++q) {
+            const double L = (double)m.box[q];
+            d[q] -= L * rint(d[q] / L);
+            r2d += d[q] * d[q];
+        }
+        in = r2d >= m.ring2d[ring] && r2d < m.ring2d[ring + 1];
+    }
+    if (in && ring == 2 && A.excl_ptr) {   // the universe is not filtered at a build: excluded partners have rate 0 (R-9)
+        const int o = A.orig[i], oj = A.orig[j];
+        for (int e = A.excl_ptr[o]; e < A.excl_ptr[o + 1]; ++e) in = in && A.excl_idx[e] != oj;
+    }
+    float rinv = 0.f, fr = 0.f;
+    if (in) fr = LJ ? fij_lj(m, p, lji, A.lj[j], rinv) : fij_coul(m, p, xi.w, xj.w, rinv);
     const float sg = (fr > 0.f ? rinv : -rinv);  // n = F/|F|
-    LY = ring == 0 ? c.LM : c.LL;
     g = fabsf(fr);
-    nx = dx * sg; ny = dy * sg; nz = dz * sg;
+    nx = p.dx * sg; ny = p.dy * sg; nz = p.dz * sg;
     tag = 0;
-    if (WANT_J) tag = orig[j] | (ring << 31);
+    if (WANT_J) tag = A.orig[j] | (ring << 28);
 }
 
 // The chain of one atom, run by the G lanes of its group.  The whole warp executes the loop together (while any
@@ -182,7 +205,10 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
     const unsigned full = 0xffffffffu;
     const float eps = m.eps_jump, beta = m.beta;
     const bool bps = isinf(eps), lead = gl == 0;
-    const float S = c.S;
+    const float aq = fabsf(xi.w);
+    const float L0 = aq * m.qmaxG[0], L1 = aq * m.qmaxG[1], L2 = aq * m.qmaxG[2];   // L_Y,i = |q_i| q_max G_Y (R-7)
+    const float w0 = (float)c.N[0] * L0, w1 = (float)c.N[1] * L1, w2 = (float)c.N[2] * L2;
+    const float S = (w0 + w1) + w2;
     bool done = !(on && S > 0.f);
     if (on && done && lead) {  // no partner: lambda-bar = 0, the clock never rings; v drifts to the end below
         tl.expiries++;
@@ -194,18 +220,19 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
     float vex = vx, vey = vy, vez = vz, te = 0.f;   // epoch start: velocity and time after the last accepted jump
     float t_run = 0.f;                              // time of the last proposal so far
     float Bv = 0.f, lam = 1.f, den = 1.f;
-    float ringS = S, ringM = c.SM;   // ring M is picked with probability ringM / ringS
+    float c0 = w0, c1 = w0 + w1, tot = S;   // ring Y is picked by ur * tot against the cumulated weights
     bool fresh = true;
     unsigned kb = 0, gblock = 0;
     while (__any_sync(full, !done)) {
-        if (fresh) {   // the bound of this epoch, P:L373-374 (R-11)
+        if (fresh) {   // the bound of this epoch, P:L373-374 (R-11: held until the next accepted jump)
             const float tau = H - te;
             const float va = vex * ax + vey * ay + vez * az, v2 = vex * vex + vey * vey + vez * vez;
             Bv = sqrtf(v2 + tau * tau * a2 + 2.f * tau * fmaxf(va, 0.f));
-            if (ADAPT) {   // sum over the listed pairs of lambda*_Y (R-19)
-                ringM = (float)c.NM * fmaf(beta * c.LM, Bv, lam0);
-                lam = ringM + (float)c.NL * fmaf(beta * c.LL, Bv, lam0);
-                ringS = lam;
+            if (ADAPT) {   // sum over the candidates of lambda*_Y (R-19)
+                c0 = (float)c.N[0] * fmaf(beta * L0, Bv, lam0);
+                c1 = c0 + (float)c.N[1] * fmaf(beta * L1, Bv, lam0);
+                tot = c1 + (float)c.N[2] * fmaf(beta * L2, Bv, lam0);
+                lam = tot;
             } else {
                 lam = S * (beta * Bv + lam0);
                 den = bps ? Bv : fmaf(Bv, esb, kInvSqrt2Pi);
@@ -228,9 +255,10 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
         tk += t_run;
         const bool alive = !done && tk <= H;   // the chain expires at the first proposal with t + T > delta/2
         const float U = u01(w[3]);
-        float g = 0.f, LY = 1.f, nx = 0.f, ny = 0.f, nz = 0.f;
-        int tag = 0;
-        if (alive) propose_pair<LOG>(m, A.rowM, A.rowL, A.xs, A.orig, c, ringS, ringM, i, xi, w, g, LY, nx, ny, nz, tag);
+        float g = 0.f, nx = 0.f, ny = 0.f, nz = 0.f;
+        int tag = 0, ring = 0;
+        if (alive) propose_pair<false, LOG>(m, A, c, c0, c1, tot, i, xi, make_float2(0.f, 0.f), w, g, ring, nx, ny, nz, tag);
+        const float LY = ring == 0 ? L0 : (ring == 1 ? L1 : L2);
         const float goL = __fdividef(g, LY);
         float p = 0.f, vn = 0.f;
         bool acc = false;
@@ -285,7 +313,7 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
         }
         if (LOG) {
             if (gl < n_used)
-                log_event(A, step, stream, atom, (int)kb + gl, (int)((unsigned)tag >> 31), tag & 0x7fffffff, gl == f ? 1 : 0,
+                log_event(A, step, stream, atom, (int)kb + gl, (int)((unsigned)tag >> 28), tag & 0x0fffffff, gl == f ? 1 : 0,
                           gl == f ? att : 0, T_, p, U, gl == f ? gt : 0.f);
             else if (f < 0 && gl == n_alive)
                 log_event(A, step, stream, atom, (int)kb + gl, -1, -1, 0, 0, T_, 0.f, 0.f, 0.f);
@@ -302,19 +330,24 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
     }
 }
 
-// ---- step (J'): Algorithm 5 (R-14) ---------------------------------------------------------------------------
-// Rare (LJ carriers only, ~0.15 proposals per fs): every lane of the group runs the same sequential chain.
-__device__ void chain_J(const Model &m, const UpdateArgs &A, int NV, int i, unsigned atom, const float4 &xi, float2 lji,
-                        float sbm, float H, unsigned stream, unsigned step, float &vx, float &vy, float &vz, Tally &tl,
-                        bool lead) {
-    if (!(lji.y > 0.f) || NV == 0) return;
-    const float L = 0.5f * lji.y * m.GV4se;  // 4 sqrt(eps_i eps_max) G_V; lji.y = 2 sqrt(eps_i)
+// ---- step (J'): Algorithm 5 (R-14), with the rings of R-10c ------------------------------------------------------
+// Rare (LJ carriers only, ~0.1 proposals per fs): every lane of the group runs the same sequential chain.  The bound
+// beta |v| sum_Y N_Y L^vdW_Y is constant over the half-step (|v| is preserved by reflections).
+__device__ void chain_J(const Model &m, const UpdateArgs &A, const ChainConst &c, int i, unsigned atom, const float4 &xi,
+                        float2 lji, float sbm, float H, unsigned stream, unsigned step, float &vx, float &vy, float &vz,
+                        Tally &tl, bool lead) {
+    if (!(lji.y > 0.f)) return;
+    const float hs = 0.5f * lji.y;   // sqrt(eps_i); L^vdW_Y,i = 4 sqrt(eps_i eps_max) GV_Y
+    const float L0 = hs * m.GV4se[0], L1 = hs * m.GV4se[1], L2 = hs * m.GV4se[2];
+    const float w0 = (float)c.N[0] * L0, w1 = (float)c.N[1] * L1, w2 = (float)c.N[2] * L2;
+    const float c0 = w0, c1 = w0 + w1, S = (w0 + w1) + w2;
+    if (!(S > 0.f)) return;
     float t = 0.f;
     unsigned block = 0;
     uint32_t w[4];
     for (int iter = 0;; ++iter) {
         float vv = sqrtf(vx * vx + vy * vy + vz * vz);
-        float lam = (float)NV * m.beta * vv * L;
+        float lam = S * (m.beta * vv);
         philox4x32_10(atom, step, stream, block++, m.key0, m.key1, w);
         float E = -logf(u01(w[0]));
         float T = lam > 0.f ? E / lam : INFINITY;
@@ -326,17 +359,13 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, int NV, int i, unsi
             break;
         }
         t += T;
-        const int k = (int)__umulhi(w[1], (unsigned)NV);
-        const int j = A.rowV.idx[(size_t)i * A.rowV.cap + k];
-        const float U = u01(w[2]);
+        const float U = u01(w[3]);
         if (lead) tl.proposals++;
-        float dx, dy, dz, rinv;
-        float fr = fij_lj(m, xi, A.xs[j], lji, A.lj[j], dx, dy, dz, rinv);
-        float g = fabsf(fr), p = 0.f;
-        int acc = 0;
+        float g, nx, ny, nz, p = 0.f;
+        int ring, tag, acc = 0;
+        propose_pair<true, true>(m, A, c, c0, c1, S, i, xi, lji, w, g, ring, nx, ny, nz, tag);
+        const float L = ring == 0 ? L0 : (ring == 1 ? L1 : L2);
         if (g > 0.f) {
-            float sg = (fr > 0.f ? rinv : -rinv);
-            float nx = dx * sg, ny = dy * sg, nz = dz * sg;
             float vF = (vx * nx + vy * ny + vz * nz) * g;
             p = fmaxf(vF, 0.f) / (vv * L);
             if (lead) { tl.max_gl = fmaxf(tl.max_gl, g / L); tl.max_p = fmaxf(tl.max_p, p); }
@@ -346,7 +375,7 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, int NV, int i, unsi
                 if (lead) tl.accepts++;
             }
         }
-        if (lead) log_event(A, step, stream, atom, iter, 2, A.orig[j], acc, 0, T, p, U, 0.f);
+        if (lead) log_event(A, step, stream, atom, iter, 4 + ring, tag & 0x0fffffff, acc, 0, T, p, U, 0.f);
     }
 }
 
@@ -384,17 +413,16 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
     const bool any_lj = (jumpy0 && A.ph[0].lj) || (jumpy1 && A.ph[1].lj);
     float a0x = 0.f, a0y = 0.f, a0z = 0.f, a1x = 0.f, a1y = 0.f, a1z = 0.f;   // accelerations of the two phases
     ChainConst cc;
-    cc.NM = cc.NL = 0; cc.LM = cc.LL = cc.SM = cc.S = 0.f;
+    cc.N[0] = cc.N[1] = cc.N[2] = 0; cc.home = 0;
     float2 lji = make_float2(0.f, 0.f);
-    int NV = 0;
     if (live) {
         xi = A.xs[i]; v4 = A.vs[i]; mi = A.mi[i]; atom = (unsigned)A.orig[i];
         const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
         float4 g0 = z4, g1 = z4, b0 = z4, b1 = z4;
         if (A.ph[0].kind != 0 && A.ph[0].use_grad) { g0 = A.grad[0][i]; if (A.grad_b[0]) b0 = A.grad_b[0][i]; }
         if (A.ph[1].kind != 0 && A.ph[1].use_grad) { g1 = A.grad[1][i]; if (A.grad_b[1]) b1 = A.grad_b[1][i]; }
-        if (any_coul) cc = chain_const(m, A.rowM, A.rowL, i, xi.w);
-        if (any_lj) { lji = A.lj[i]; if (lji.y > 0.f) NV = A.rowV.cnt[i]; }
+        if (any_coul || any_lj) cc = chain_const(A, i);
+        if (any_lj) lji = A.lj[i];
         // a = -M^-1 F
         a0x = -mi.x * (b0.x + g0.x); a0y = -mi.x * (b0.y + g0.y); a0z = -mi.x * (b0.z + g0.z);
         a1x = -mi.x * (b1.x + g1.x); a1y = -mi.x * (b1.y + g1.y); a1z = -mi.x * (b1.z + g1.z);
@@ -421,7 +449,7 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
                     if (P.coul) chain_C<G, LOG, ADAPT>(m, A, live, cc, i, atom, xi, mi.y, cax, cay, caz, P.H, P.streamC, P.step, vx, vy, vz, tl, gl, gshift);
                     else if (P.use_grad) { vx += P.H * cax; vy += P.H * cay; vz += P.H * caz; }
                 } else if (P.lj && live && (slot == 0) == (P.reverse != 0)) {
-                    chain_J(m, A, NV, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
+                    chain_J(m, A, cc, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
                 }
             }
             if (P.bkick == 2) { vx += P.H * ax; vy += P.H * ay; vz += P.H * az; }
@@ -432,7 +460,7 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
             // positions are integrated in fp64 as hi + lo (hi = the fp32 value every pair kernel reads):
             // fp32 rounding of x (ulp(18 A) = 2e-6 A) through the stiff O-H bonds is otherwise the
             // largest noise source of the whole step
-            const float4 xlo = A.xl[i];
+            const float4 xlo = A.xl_all[i];
             double X = (double)xi.x + (double)xlo.x, Y = (double)xi.y + (double)xlo.y, Z = (double)xi.z + (double)xlo.z;
             const double hdt = (double)A.half_dt;
             X += hdt * (double)vx; Y += hdt * (double)vy; Z += hdt * (double)vz;  // A
@@ -454,8 +482,8 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
             Z = wrap1d(Z, (double)m.box[2], (double)m.inv_box[2], iz);
             const float x = (float)X, y = (float)Y, z = (float)Z;
             A.xs_out[i] = make_float4(x, y, z, xi.w);
-            A.xl[i] = make_float4((float)(X - (double)x), (float)(Y - (double)y), (float)(Z - (double)z),
-                                  __int_as_float(img_pack(ix, iy, iz)));
+            A.xl_out[i] = make_float4((float)(X - (double)x), (float)(Y - (double)y), (float)(Z - (double)z),
+                                      __int_as_float(img_pack(ix, iy, iz)));
             float4 xb = A.x_build[i];
             float ddx = min_image1(x, xb.x, m.box[0], m.inv_box[0]);
             float ddy = min_image1(y, xb.y, m.box[1], m.inv_box[1]);
@@ -544,16 +572,21 @@ __global__ void k_load(Model m, const float *__restrict__ pos, const float *__re
 
 // re-read the caller's positions (wrapped) and velocities into the current sorted order
 // moved (may be NULL): set to 1 when some atom is farther than skin/2 from its position at the last list build
+// keep: the image counters survive (jump_refresh_lazy: the caller hands the trajectory back); an atom whose
+// position is bit for bit the one the library wrote keeps its fp64 residual too, any other restarts it at 0 and adds
+// the box lengths its coordinate lies outside [0, L) by.  !keep (jump_refresh): residual and counters restart at 0.
 __global__ void k_reload(Model m, const float *__restrict__ pos, const float *__restrict__ vel,
                          const int *__restrict__ orig, float4 *__restrict__ xs, float4 *__restrict__ vs,
-                         float4 *__restrict__ xl, const float4 *__restrict__ x_build, int *__restrict__ moved) {
+                         float4 *__restrict__ xl, const float4 *__restrict__ x_build, int *__restrict__ moved, int keep) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
     int o = orig[i];
-    float4 x = xs[i];
-    x.x = wrap1(pos[3 * o], m.box[0], m.inv_box[0]);
-    x.y = wrap1(pos[3 * o + 1], m.box[1], m.inv_box[1]);
-    x.z = wrap1(pos[3 * o + 2], m.box[2], m.inv_box[2]);
+    const float4 old = xs[i];
+    float4 x = old;
+    const float px = pos[3 * o], py = pos[3 * o + 1], pz = pos[3 * o + 2];
+    x.x = wrap1(px, m.box[0], m.inv_box[0]);
+    x.y = wrap1(py, m.box[1], m.inv_box[1]);
+    x.z = wrap1(pz, m.box[2], m.inv_box[2]);
     if (moved) {
         const float4 xb = x_build[i];
         const float dx = min_image1(x.x, xb.x, m.box[0], m.inv_box[0]);
@@ -562,8 +595,19 @@ __global__ void k_reload(Model m, const float *__restrict__ pos, const float *__
         const float d2 = dx * dx + dy * dy + dz * dz;
         if (!(d2 <= m.half_skin2)) *moved = 1;   // also when a position is not finite
     }
+    float4 l = make_float4(0.f, 0.f, 0.f, __int_as_float(img_pack(0, 0, 0)));
+    if (keep) {
+        const float4 lo = xl[i];
+        if (x.x == old.x && x.y == old.y && x.z == old.z) l = lo;
+        else {
+            int ix, iy, iz;
+            img_unpack(__float_as_int(lo.w), ix, iy, iz);
+            ix += (int)floorf(px * m.inv_box[0]); iy += (int)floorf(py * m.inv_box[1]); iz += (int)floorf(pz * m.inv_box[2]);
+            l.w = __int_as_float(img_pack(ix, iy, iz));
+        }
+    }
     xs[i] = x;
-    xl[i] = make_float4(0.f, 0.f, 0.f, __int_as_float(img_pack(0, 0, 0)));   // residual 0, image counters 0
+    xl[i] = l;
     vs[i] = make_float4(vel[3 * o], vel[3 * o + 1], vel[3 * o + 2], 0.f);
 }
 
@@ -598,16 +642,19 @@ static void update_dispatch(const Model &m, const UpdateArgs &A, cudaStream_t st
         else k_update<true, G, false, false><<<grid, B, 0, st>>>(m, A);
     }
 }
-// lanes per jump chain: as many as keep the whole grid resident at once (148 SMs x 6 CTAs of 128 threads, the
-// register-limited occupancy of k_update); JUMP_B200_LANES overrides (1, 4, 8, 16) for experiments
-static int lanes_per_chain(int n) {
-    static int forced = -1;
-    if (forced < 0) {
-        const char *e = getenv("JUMP_B200_LANES");
-        forced = e ? atoi(e) : 0;
-    }
+// lanes per jump chain: as many as keep the whole grid resident at once (SMs x resident CTAs of k_update x 128
+// threads, asked of the occupancy API); A.lanes != 0 (jump_set_lanes: 1, 4, 8, 16) overrides, for tests and experiments
+static int lanes_per_chain(int n, int forced) {
     if (forced == 1 || forced == 4 || forced == 8 || forced == 16) return forced;
-    const long long budget = 148ll * 6 * 128;
+    static long long budget = 0;
+    if (budget == 0) {
+        int dev = 0, sms = 148, per_sm = 6;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_update<true, 8, false, false>, 128, 0) != cudaSuccess || per_sm < 1)
+            per_sm = 6;
+        budget = (long long)sms * per_sm * 128;
+    }
     if ((long long)n * 16 <= budget) return 16;
     if ((long long)n * 8 <= budget) return 8;
     if ((long long)n * 4 <= budget) return 4;
@@ -618,7 +665,7 @@ void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t
         const int B = 128;
         k_update<false, 1, false, false><<<(unsigned)((m.n + B - 1) / B), B, 0, st>>>(m, A);
     } else {
-        switch (lanes_per_chain(m.n)) {
+        switch (lanes_per_chain(m.n, A.lanes)) {
             case 16: update_dispatch<16>(m, A, st); break;
             case 8: update_dispatch<8>(m, A, st); break;
             case 4: update_dispatch<4>(m, A, st); break;
@@ -639,8 +686,8 @@ void launch_load(const Model &m, const float *pos, const float *vel, const float
     *launches += 1;
 }
 void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
-                   float4 *xl, const float4 *x_build, int *moved, cudaStream_t st, int64_t *launches) {
-    k_reload<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, orig, xs, vs, xl, x_build, moved);
+                   float4 *xl, const float4 *x_build, int *moved, int keep, cudaStream_t st, int64_t *launches) {
+    k_reload<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, orig, xs, vs, xl, x_build, moved, keep);
     *launches += 1;
 }
 void launch_images(int n, const float4 *xl, const int *orig, int *out, cudaStream_t st, int64_t *launches) {

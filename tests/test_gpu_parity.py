@@ -54,19 +54,51 @@ def fragile(o):
     return st["min_margin"] < 1e-6 or st["min_list_margin"] < 2e-6
 
 
-def check_events(eg, eo):
+INT_FIELDS = ("step", "stream", "atom", "iter", "ring", "j", "accepted", "n_gt")
+
+
+def check_events(eg, eo, steps=1):
+    """R-18: integer fields bit-exact; U exact (R-15).  T = E / lambda-bar carries the relative error of B_v, i.e. of the
+    fp32 velocities, and p, G~ are smooth functions of positions (held in fp32 by the pair arithmetic: 1e-5 A at a
+    100 A box) and velocities: the two paths drift apart by fp32 rounding, about 1e-7 relative per step (measured:
+    1.3e-5 in T after 10 steps at 12 000 atoms, 2e-4 after 100 steps at 648; SURVEY R-18 guessed a flat 1e-5).  Asserted:
+    T to 5e-5 relative, p to 1e-4, G~ to 2e-4, each times the number of 10-step chunks elapsed."""
+    k = max(1, (steps + 9) // 10)
     assert len(eg) == len(eo)
-    for k in ("step", "stream", "atom", "iter", "ring", "j", "accepted", "n_gt"):
-        assert (eg[k] == eo[k]).all(), k
+    for f in INT_FIELDS:
+        assert (eg[f] == eo[f]).all(), f
     fin = np.isfinite(eo["T"])
     assert (np.isfinite(eg["T"]) == fin).all()
-    if fin.any():
-        assert np.abs(eg["T"][fin] / eo["T"][fin] - 1).max() < 1e-3
+    if fin.any():   # (a kick that nearly cancels v leaves a small |v| with a large RELATIVE error: the rare outliers)
+        rel = np.abs(eg["T"][fin] / eo["T"][fin] - 1)
+        assert np.quantile(rel, 0.999) < 5e-5 * k and rel.max() < 5e-3
     if len(eo) == 0:
         return
-    assert np.abs(eg["p"] - eo["p"]).max() < 1e-4
+    assert np.abs(eg["p"] - eo["p"]).max() < 1e-4 * k
     assert (eg["U"] == eo["U"].astype(np.float32)).all()       # uniforms are exact in fp32 (R-15)
-    assert np.abs(eg["gt"] - eo["gt"]).max() < 1e-3
+    assert np.abs(eg["gt"] - eo["gt"]).max() < 2e-4 * k
+
+
+def first_divergence(eg, eo):
+    """Index of the first logged event (canonical order) whose integer fields differ, None if the logs agree."""
+    m = min(len(eg), len(eo))
+    bad = np.zeros(m, bool)
+    for f in INT_FIELDS:
+        bad |= eg[f][:m] != eo[f][:m]
+    if bad.any():
+        return int(np.argmax(bad))
+    return None if len(eg) == len(eo) else m
+
+
+def divergence_is_a_close_call(eo, k, o, steps):
+    """R-17: the two paths may take a discontinuous decision differently only where it is a closer call than they
+    differ.  The oracle logs the margin of every decision of every chain iteration (and of the list builds): the
+    chain the first differing event belongs to, up to that event, or the lists of the chunk, must show a margin below
+    2e-6 times the steps elapsed (the paths drift apart by about 1e-7 per step, relative; 20 times that)."""
+    tol = 2e-6 * steps
+    e = eo[min(k, len(eo) - 1)]
+    chain = eo[(eo["step"] == e["step"]) & (eo["stream"] == e["stream"]) & (eo["atom"] == e["atom"]) & (eo["iter"] <= e["iter"])]
+    return (len(chain) and chain["margin"].min() < tol) or o.stats()["min_list_margin"] < tol
 
 
 # ------------------------------------------------------------------------------------- rows, bounds
@@ -80,7 +112,8 @@ def test_bounds_match(jb, jo, cfg0):
 
 @pytest.mark.parametrize("case", ["cfg0", "small5", "no_ring", "big_cells"])
 def test_rows_identical(jb, jo, cfg0, case):
-    """a1-a3: sort + row build.  Rows M, L, V must hold the same atoms in the same (canonical) order."""
+    """a1-a3: sort + row build + cell universe (R-10c).  Row A, row B and the universe of ring C must hold the same atoms
+    in the same (canonical) order as the oracle's."""
     if case == "cfg0":
         sysd, run = cfg0
     else:
@@ -149,46 +182,73 @@ def test_forces_solute_config3(jb, jo):
 
 
 # ------------------------------------------------------------------------------------- jump chains
-# Philox keys chosen (scan of seeds 3000..3039 with the oracle alone) so that the oracle takes no fragile decision
-# (R-17) for 100 steps: the parity window is then long enough to mean something.
-@pytest.mark.parametrize("eps,seed,mode", [(1.0, 3026, 0), (0.3, 3011, 0), (float("inf"), 3000, 0), (2.0, 3009, 1)])
-def test_event_log_and_trajectory_cfg0(jb, jo, cfg0, eps, seed, mode):
-    """a6-a8: every proposal of 10 JUMP steps (C', J', both halves) equals the oracle's; then the 100-step
-    trajectory stays within 1e-4 A on the window before the oracle's first fragile decision (R-17).
-    mode 1: adaptive eps(x) = eps0 |F_ij(x)| (NEXT-1, R-19)."""
-    sysd, run = cfg0
-    run = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG, eps_jump=eps, eps_mode=mode, seed=seed)
+# Philox keys: for each mechanism the three most robust seeds of 3000..3199 by the oracle's own audit of its decisions
+# (tests/golden/scan_parity_seeds.py, oracle only).  Over 100 steps a 648-atom box takes ~2e5 discontinuous decisions
+# and rebuilds its lists 25 times; the two paths drift apart by fp32 rounding (~1e-5 A after 100 steps), so on about
+# half of all seeds one decision is eventually a closer call than that and is (legitimately, R-17) taken differently.
+PARITY_SEEDS = {(1.0, 0): (3164, 3127, 3088), (0.3, 0): (3157, 3068, 3005), (float("inf"), 0): (3185, 3175, 3087),
+                (2.0, 1): (3115, 3157, 3038)}
+
+
+def run_parity_window(jb, jo, sysd, run, lanes, n_chunks=10):
+    """Both paths, 10 steps at a time with every proposal logged.  Returns the number of steps over which the event
+    logs were identical and the positions within X_TOL; a divergence must be a close call of the oracle's (R-17)."""
     g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
-    g.jump_step(10); g.sync(); o.jump_step(10)
-    eg, eo = g.events(), o.events()
-    assert len(eo) > 15000
-    assert mode == 0 or eo["accepted"].sum() > 3000       # the adaptive mechanism accepts about a quarter of its proposals
-    check_events(eg, eo)
-    assert set(np.unique(eo["stream"])) == {1, 2, 3, 4}
-    g.clear_events(); o.clear_events()
-    window = 10
-    for _ in range(9):
-        o.jump_step(10)
-        st = o.stats()
-        g.jump_step(10); g.sync()
-        if fragile(o):                    # a decision the fp32 path may legitimately take the other way
+    g.set_lanes(lanes)
+    window, n_ev, n_acc, rings = 0, 0, 0, set()
+    for chunk in range(n_chunks):
+        o.reset_stats()
+        g.jump_step(10); g.sync(); o.jump_step(10)
+        eg, eo = g.events(), o.events()
+        k = first_divergence(eg, eo)
+        if k is not None:
+            assert divergence_is_a_close_call(eo, k, o, window + 10), (window, k, eo[max(0, k - 2):k + 2], eg[max(0, k - 2):k + 2])
             break
-        window += 10
+        check_events(eg, eo, steps=window + 10)
         assert pos_err(g, o, sysd["box"]) <= X_TOL
+        window += 10
+        n_ev += len(eo); n_acc += int(eo["accepted"].sum()); rings |= set(np.unique(eo["ring"]).tolist())
         g.clear_events(); o.clear_events()
-    assert window >= 80
-    sg, so = g.stats(), o.stats()
+    sg = g.stats()
     assert sg["error"] == 0 and sg["max_p"] <= 1.0 + 1e-4 and sg["max_g_over_L"] <= 1.0 + 1e-4
-    if window == 100:
-        assert sg["proposals"] == so["proposals"] and sg["accepts"] == so["accepts"]
-        assert sg["gt_attempts"] == so["gt_attempts"] and sg["expiries"] == so["expiries"]
+    assert sg["max_disp"] < 0.5 * run["skin"]
+    if window == 10 * n_chunks:
+        assert np.abs(g.vel.cpu().numpy() - o.vel).max() < 5e-3
+    g.close(); o.close()
+    return window, n_ev, n_acc, rings
+
+
+@pytest.mark.parametrize("lanes", [0, 1, 4, 8, 16])
+@pytest.mark.parametrize("eps,mode", [(1.0, 0), (0.3, 0), (float("inf"), 0), (2.0, 1)])
+def test_event_log_and_trajectory_cfg0(jb, jo, cfg0, eps, mode, lanes):
+    """a6-a8: every proposal of 100 JUMP steps (C', J', both halves) equals the oracle's -- partner, ring, accept flag,
+    sampler attempts bit for bit, times and probabilities to fp32 rounding -- and the trajectory stays within 1e-4 A
+    over the 100 steps (BASELINE.json north_star), for every instantiation of the update kernel (lanes per chain 1, 4,
+    8, 16; 0 = the automatic choice, 16 at this size).  Every recorded seed is run; each must agree up to a decision
+    that the oracle itself marks as a close call, and at least one must go the whole 100 steps.
+    mode 1: adaptive eps(x) = eps0 |F_ij(x)| (NEXT-1, R-19)."""
+    if lanes not in (0, 1) and (eps, mode) != (1.0, 0):
+        pytest.skip("lane counts 4, 8, 16 are compared on one mechanism")
+    sysd, run = cfg0
+    best = 0
+    for seed in PARITY_SEEDS[(eps, mode)]:
+        r = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG, eps_jump=eps, eps_mode=mode, seed=seed)
+        window, n_ev, n_acc, rings = run_parity_window(jb, jo, sysd, r, lanes)
+        assert window >= 10
+        if window == 100:
+            assert n_ev > 150000 and rings == {-1, 0, 1, 2, 4, 5, 6}
+            assert mode == 0 or n_acc > 30000           # the adaptive mechanism accepts about a quarter of its proposals
+        best = max(best, window)
+        if best == 100:
+            break
+    assert best == 100
 
 
 def test_bjaoajb_scheme_matches_oracle(jb, jo, cfg0):
     """NEXT-3: B J A O A J B as the scheme of jump_step -- event log and trajectory against the oracle,
     and without any jump mechanism the scheme is bitwise the C' scheme without jumps (BAOAB with F0)."""
     sysd, run = cfg0
-    r = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG | jb.F_BJAOAJB, seed=3026)
+    r = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG | jb.F_BJAOAJB, seed=3137)   # scan_parity_seeds.py
     g, o = jb.JumpSim(sysd, **r), jo.Oracle(sysd, **r)
     g.jump_step(10); g.sync(); o.jump_step(10)
     assert len(o.events()) > 15000
@@ -305,13 +365,13 @@ def test_refresh_lazy_keeps_valid_rows_and_rebuilds_when_needed(jb, jo, cfg0):
     g = jb.JumpSim(s2, **run)
     n0 = g.stats()["rebuilds"]
     rng = np.random.default_rng(17)
-    pos2 = np.float32(s2["pos"] + rng.uniform(-0.25, 0.25, size=s2["pos"].shape)).astype(np.float64)   # |d| < 0.44 < skin/2
+    pos2 = np.float32(s2["pos"] + rng.uniform(-0.03, 0.03, size=s2["pos"].shape)).astype(np.float64)   # |d| < 0.06: room for 3 more steps below skin/2
     g.pos.copy_(torch.as_tensor(np.float32(pos2)))
     assert g.refresh_lazy() is False and g.stats()["rebuilds"] == n0
     o = jo.Oracle(dict(s2, pos=pos2), **run)
     for which in (0, 2):
         assert rel_force_err(g.forces(which).cpu().numpy(), o.forces(which)) <= F_TOL
-    g.jump_step(10); g.sync()
+    g.jump_step(3); g.sync()
     assert g.stats()["error"] == 0
     pos3 = pos2.copy()
     pos3[5, 0] += 0.8                                       # one atom pushed out of its skin/2 ball
@@ -449,6 +509,100 @@ def test_config4_one_million_atoms_properties(jb):
     assert (out[0][0] == out[1][0]).all() and (out[0][1] == out[1][1]).all()
 
 
+def test_config2_logged_step_single_lane_chains(jb, jo):
+    """BASELINE configs[2] (96 000 atoms), where the update kernel runs one lane per chain -- the instantiation the
+    large-box throughput is quoted on: every proposal of one logged JUMP step against the oracle's."""
+    sysd, run = wl.make_config(2)
+    run = dict(run, flags=3 | 4)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    g.jump_step(1); g.sync(); o.jump_step(1)
+    eo = o.events()
+    assert len(eo) > 500000 and set(np.unique(eo["ring"])) == {-1, 0, 1, 2, 4, 5, 6}
+    check_events(g.events(), eo)
+    assert pos_err(g, o, sysd["box"]) <= X_TOL
+    sg, so = g.stats(), o.stats()
+    assert sg["error"] == 0 and sg["proposals"] == so["proposals"] and sg["accepts"] == so["accepts"]
+
+
+def test_config3_solute_logged_steps(jb, jo):
+    """BASELINE configs[3] (chain beads with up to five bonded terms each, per-bead charges and LJ parameters): the
+    per-atom bonded kernel of the step path, the LJ bounds over a range of sigma, four lanes per chain.  The generator
+    leaves the chain on lattice sites with stretched bonds and overlapping beads (a far-from-equilibrium start: forces of
+    1e4 kcal/mol/A), so the steps are short (0.25 fs), the lists are rebuilt at every step and the skin check is off;
+    parity does not need an equilibrated system: bonded and F0 gradients, then every proposal of 4 logged JUMP steps."""
+    sysd, run = wl.make_config(3)
+    run = dict(run, flags=3 | 4 | jb.F_LAX_SKIN, nlist_every=1, dt_fs=0.25)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    for which in (3, 0):
+        err = rel_force_err(g.forces(which).cpu().numpy(), o.forces(which))
+        assert err <= F_TOL, (which, err)
+    done = 0
+    for _ in range(4):
+        g.jump_step(1); g.sync(); o.jump_step(1)
+        eg, eo = g.events(), o.events()
+        k = first_divergence(eg, eo)
+        if k is not None:                                           # ~1e6 decisions a step on this hot start
+            assert divergence_is_a_close_call(eo, k, o, 1)
+            break
+        check_events(eg, eo)
+        assert (eo["ring"] >= 4).sum() > 300                        # LJ chains of the beads and the oxygens
+        assert (eo["atom"] < 2500).sum() > 2500                     # chain beads
+        assert pos_err(g, o, sysd["box"]) <= X_TOL
+        g.clear_events(); o.clear_events()
+        done += 1
+    assert done >= 1
+    sg = g.stats()
+    assert sg["error"] == 0 and sg["max_p"] <= 1 + 1e-4 and sg["max_g_over_L"] <= 1 + 1e-4
+
+
+def test_lists_between_two_builds_against_brute_force(jb, jo, cfg0):
+    """Validity of the lists in the middle of a rebuild interval (step 3 of 4), against a brute-force O(N^2) search on
+    the CURRENT positions rather than against the oracle's own lists: the short list holds every pair closer than r_c,
+    rows A and B every pair of their ring, the cell universe every pair closer than r_long; the short-range gradient
+    equals the oracle's brute-force sum; a row asked for the first time between two builds (the full list, through
+    jump_get_forces(2) and jump_get_energy) gives the brute-force long gradient and energy."""
+    sysd, run = cfg0
+    s2 = _liquid_state(jo, sysd, run)
+    g, o = jb.JumpSim(s2, **run), jo.Oracle(s2, **run)
+    assert run["nlist_every"] == 4
+    g.jump_step(3); g.sync(); o.jump_step(3)
+    assert g.stats()["rebuilds"] == 1 and not fragile(o)
+    x = o.pos; L = sysd["box"]; n = g.n
+    d = x[:, None, :] - x[None, :, :]
+    d -= L * np.round(d / L)
+    r = np.sqrt((d ** 2).sum(-1))
+    b = g.bounds()
+    rlo, rA, rM, rc, rE = run["r_short"] - run["r_switch"], b["rA"], b["rM"], run["r_short"], run["r_long"]
+    eps_r = 1e-5                                            # the two trajectories differ by ~1e-7 A
+    for i in range(0, n, 9):
+        excl = set(s2["excl_idx"][s2["excl_ptr"][i]:s2["excl_ptr"][i + 1]].tolist()) | {i}
+        rows = {w: set(g.row(w, i).tolist()) for w in (0, 1, 2, 3)}
+        for w, lo_, hi_ in ((0, 0.0, rc), (1, rlo, rA), (2, rA, rM), (3, 0.0, rE)):
+            need = {j for j in range(n) if (w == 3 or j not in excl) and lo_ + eps_r <= r[i, j] < hi_ - eps_r}
+            assert need <= rows[w], (i, w, sorted(need - rows[w]))
+    assert rel_force_err(g.forces(4).cpu().numpy(), o.forces(4, brute=True)) <= 2 * F_TOL
+    assert rel_force_err(g.forces(2).cpu().numpy(), o.forces(2, brute=True)) <= 2 * F_TOL      # full list built just now
+    assert g.energy()[1] == pytest.approx(o.potential(1), rel=2e-5, abs=1e-3)
+    g.jump_step(5); g.sync()
+    assert g.stats()["error"] == 0
+
+
+def test_displacement_beyond_half_skin_is_an_error_unless_lax(jb, cfg0):
+    """List validity is checked on the device at every step (JUMP_E_SKIN): a rebuild period far too long for the skin is
+    refused at the next synchronising call; JUMP_F_LAX_SKIN / jump_set_lax_skin only report it."""
+    sysd, run = cfg0
+    g = jb.JumpSim(sysd, **dict(run, nlist_every=40))
+    g.jump_step(30)
+    with pytest.raises(jb.JumpError, match="-5"):
+        g.sync()
+    g = jb.JumpSim(sysd, **dict(run, nlist_every=40, flags=run["flags"] | jb.F_LAX_SKIN))
+    g.jump_step(30); g.sync()
+    assert g.stats()["max_disp"] > 0.5 * run["skin"] and g.stats()["error"] == 0
+    g.set_lax_skin(False)
+    with pytest.raises(jb.JumpError, match="-5"):
+        g.sync()
+
+
 # ------------------------------------------------------------------------------------- NEXT-4: observables on the device
 def test_image_counters_give_continuous_unwrapped_positions(jb, jo, cfg0):
     """Unwrapped positions pos + images * box: equal to the oracle's unwrapped trajectory on the parity window, and
@@ -469,6 +623,9 @@ def test_image_counters_give_continuous_unwrapped_positions(jb, jo, cfg0):
     assert (img != 0).any(1).sum() > 20                    # atoms did cross
     w = g.pos.cpu().numpy().astype(np.float64)
     assert (w >= 0).all() and (w < box).all()
+    assert g.refresh_lazy() in (False, True)               # the hand-back call keeps the trajectory: counters survive
+    assert (g.images().cpu().numpy() == img).all()
+    assert np.abs(g.pos_unwrapped().cpu().numpy() - prev).max() < 1e-5
     g.refresh()
     assert (g.images().cpu().numpy() == 0).all()           # jump_refresh restarts the counters
 
@@ -521,8 +678,13 @@ def test_orthorhombic_box(jb, jo, case):
     for which in (0, 1, 2):
         assert rel_force_err(g.forces(which).cpu().numpy(), o.forces(which)) <= F_TOL, which
     g.jump_step(10); g.sync(); o.jump_step(10)
-    check_events(g.events(), o.events())
-    if not fragile(o):
+    eg, eo = g.events(), o.events()
+    k = first_divergence(eg, eo)
+    if k is not None:
+        assert divergence_is_a_close_call(eo, k, o, 10)
+    else:
+        check_events(eg, eo)
+    if k is None and not fragile(o):
         d = g.pos.cpu().numpy().astype(np.float64) - o.pos
         d -= box * np.round(d / box)
         assert np.abs(d).max() <= X_TOL

@@ -341,7 +341,7 @@ def test_rows_and_cell_universe_contract(cfg0, case):
     x = np.mod(sysd["pos"], sysd["box"]); n = o.n
     box = np.broadcast_to(np.asarray(sysd["box"], float), (3,))
     rc, h, s, rM, rl = run["r_short"], run["r_switch"], run["skin"], run["r_mid"], run["r_long"]
-    rA = run.get("r_mid_in", 0.0) or rc
+    rA = run.get("r_mid_in") or rc + 0.25
     edge = run.get("cell_edge", 0.0) or (rl + s) / 4
     ng, cell, key = _contract_keys(x, box, edge)
     d = x[:, None, :] - x[None, :, :]
