@@ -261,6 +261,7 @@ double orc_gtilde(const orc_ctx *c, double eta, int atom, int64_t step, int stre
         ++it;
         chain_block(c, atom, step, stream, (*block)++, w);
         double u0 = orc_u01(w[0]), u1 = orc_u01(w[1]), u2 = orc_u01(w[2]), u3 = orc_u01(w[3]);
+        mg = upd(mg, eta + 2.5); mg = upd(mg, eta + 1.0); mg = upd(mg, eta); /* which proposal family: a decision too */
         if (eta < -2.5) {
             double z = -(log(u0) + log(u1)) / fabs(eta); /* Gamma(2, |eta|) */
             double a = exp(-0.5 * z * z);

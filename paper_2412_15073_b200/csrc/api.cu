@@ -222,7 +222,8 @@ static int build_rows(jump_ctx *c, const bool want[N_ROWS]) {
     // the cell table describes and the displacement check refers to: it is the row an eager build would have made.
     const float4 *xsrc = (c->step == c->sort_step) ? c->xs : c->x_build;
     launch_build_rows(c->m, c->g, sel, (float)rmax, c->cell_start, xsrc, c->xl, c->lj, c->orig,
-                      c->sorted_of, c->excl_ptr, c->excl_idx, c->ctr, c->st, &c->launches);
+                      c->sorted_of, c->excl_ptr, c->excl_idx, c->ctr, (sel[ROW_A].enabled ? c->cell_of : nullptr),
+                      (float)std::pow(std::max(c->rM - 2.0 * c->p.skin, 0.0), 2), c->st, &c->launches);
     prof_end(c, PROF_BUILD);
     CK(cudaGetLastError());
     return 0;
@@ -750,7 +751,7 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
         g.gn[k] = std::max(1, (int)std::floor(p->box[k] / edge));
         g.scale[k] = (double)g.gn[k] / p->box[k];
         g.reach[k] = (int)std::ceil((p->r_long + p->skin) / (p->box[k] / g.gn[k]));
-        if (g.reach[k] > 8) return JUMP_E_ARG;  // stencil table of the row build (cell_edge too small)
+        if (g.reach[k] > 8 || g.gn[k] > 1023) return JUMP_E_ARG;  // stencil table of the row build (cell_edge too small); packed cells
         g.ncell *= g.gn[k];
     }
     // buffers
@@ -780,6 +781,7 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
         }
         u.nrow = u.cnt[2] * u.cnt[1];
         u.stride = (u.nrow + 1 + 7) / 8 * 8;
+        u.inv_cnt1 = (65536 + u.cnt[1] - 1) / u.cnt[1];
         for (int a = 0; a < 17; ++a)
             for (int b = 0; b < 17; ++b) {
                 const double gz = (a > 1 ? a - 1 : 0) * w[2], gy = (b > 1 ? b - 1 : 0) * w[1];
@@ -1105,7 +1107,9 @@ extern "C" int jump_get_row(jump_ctx *c, int32_t which, int32_t atom, int32_t *h
         unsigned short tot = 0;
         CK(cudaMemcpyAsync(&home, c->cell_of + i, sizeof(int), cudaMemcpyDeviceToHost, c->st));
         CK(cudaStreamSynchronize(c->st));
-        CK(cudaMemcpyAsync(&tot, c->uni_cum + (size_t)home * c->uni.stride + c->uni.nrow, sizeof tot, cudaMemcpyDeviceToHost, c->st));
+        home &= 0x3fffffff;   // (bit 30: far-exclusion flag)
+        const int hlin = ((home >> 20) * c->g.gn[1] + ((home >> 10) & 1023)) * c->g.gn[0] + (home & 1023);
+        CK(cudaMemcpyAsync(&tot, c->uni_cum + (size_t)hlin * c->uni.stride + c->uni.nrow, sizeof tot, cudaMemcpyDeviceToHost, c->st));
         CK(cudaStreamSynchronize(c->st));
         cnt = tot;
         int *d_list = nullptr;

@@ -179,9 +179,10 @@ struct Universe {
     int cnt[3];               // cells covered per dimension: min(2 R + 1, gn)
     int nrow;                 // cnt[2] * cnt[1]
     int stride;               // entries per home cell in cum (nrow + 1, padded)
+    int inv_cnt1;             // ceil(65536 / cnt[1]): row index -> (mz, my) without a division
     signed char xr[17 * 17];  // [|oz| * 17 + |oy|] -> largest |ox| within reach, -1: (z, y) cell row out of reach
     const unsigned short *cum;
-    const int *cell_of;       // home cell of each sorted atom
+    const int *cell_of;       // home cell of each sorted atom, packed (pack_cell)
 };
 
 // m-th value, in ascending order, of the cyclic cell range [start, start+cnt) mod gn
@@ -196,14 +197,17 @@ __host__ __device__ inline int cyc_off(int val, int c, int gn) {
     else if (2 * o < -gn) o += gn;
     return o;
 }
-// The runs of stencil row p of home cell (cx, cy, cz): sorted atoms [b0, b0 + n0) (cells wrapped to the low end of the
-// x axis, first in key order) then [b1, b1 + n1).  Shared by the table build (sort_build.cu) and the draw (update.cu).
+// home cell of an atom, packed: cx | cy << 10 | cz << 20 (at most 1023 cells per edge)
+__host__ __device__ inline int pack_cell(int cx, int cy, int cz) { return cx | (cy << 10) | (cz << 20); }
+// The runs of stencil row (mz, my) of home cell (cx, cy, cz): sorted atoms [b0, b0 + n0) (cells wrapped to the low end
+// of the x axis, first in key order) then [b1, b1 + n1).  Shared by the table build (sort_build.cu) and the draw
+// (chains.cuh).  No integer division: every wrap is a conditional add.
 __device__ inline void universe_row(const SortGrid &g, const Universe &u, const int *__restrict__ cell_start, int cx, int cy,
-                                    int cz, int p, int &b0, int &n0, int &b1, int &n1) {
+                                    int cz, int mz, int my, int &b0, int &n0, int &b1, int &n1) {
     b0 = n0 = b1 = n1 = 0;
-    const int mz = p / u.cnt[1], my = p - mz * u.cnt[1];
-    const int sz = u.cnt[2] == g.gn[2] ? 0 : (cz - u.R[2] + g.gn[2]) % g.gn[2];
-    const int sy = u.cnt[1] == g.gn[1] ? 0 : (cy - u.R[1] + g.gn[1]) % g.gn[1];
+    int sz = 0, sy = 0;
+    if (u.cnt[2] != g.gn[2]) { sz = cz - u.R[2]; if (sz < 0) sz += g.gn[2]; }
+    if (u.cnt[1] != g.gn[1]) { sy = cy - u.R[1]; if (sy < 0) sy += g.gn[1]; }
     const int zc = cyc_val(mz, sz, u.cnt[2], g.gn[2]), yc = cyc_val(my, sy, u.cnt[1], g.gn[1]);
     int oz = cyc_off(zc, cz, g.gn[2]), oy = cyc_off(yc, cy, g.gn[1]);
     oz = oz < 0 ? -oz : oz; oy = oy < 0 ? -oy : oy;
@@ -213,12 +217,58 @@ __device__ inline void universe_row(const SortGrid &g, const Universe &u, const 
     if (2 * xm + 1 >= g.gn[0]) {
         b1 = cell_start[rowbase]; n1 = cell_start[rowbase + g.gn[0]] - b1;
     } else {
-        const int xs0 = (cx - xm + g.gn[0]) % g.gn[0], xc = 2 * xm + 1;
+        int xs0 = cx - xm;
+        if (xs0 < 0) xs0 += g.gn[0];
+        const int xc = 2 * xm + 1;
         int w = xs0 + xc - g.gn[0];
         if (w < 0) w = 0;
         if (w > 0) { b0 = cell_start[rowbase]; n0 = cell_start[rowbase + w] - b0; }
         b1 = cell_start[rowbase + xs0]; n1 = cell_start[rowbase + xs0 + xc - w] - b1;
     }
+}
+
+// k-th atom (sorted index) of the universe of the home cell `hp` (packed coordinates): a fixed-length bisection on the
+// running sums of the stencil rows (nine dependent 2-byte loads from a few cache lines), then the row's one or two runs
+__device__ inline int universe_pick(const SortGrid &g, const Universe &u, const int *__restrict__ cell_start, int hp, int k) {
+    const int cx = hp & 1023, cy = (hp >> 10) & 1023, cz = hp >> 20;
+    const int h = (cz * g.gn[1] + cy) * g.gn[0] + cx;
+    const unsigned short *__restrict__ cum = u.cum + (size_t)h * u.stride;
+    int lo = 0;   // last row with cum[row] <= k
+#pragma unroll
+    for (int step = 256; step > 0; step >>= 1) {
+        const int t = lo + step;
+        if (t < u.nrow && (int)cum[t] <= k) lo = t;
+    }
+    const int mz = (lo * u.inv_cnt1) >> 16, my = lo - mz * u.cnt[1];   // lo / cnt[1] by a reciprocal (lo < 512, cnt[1] <= 17)
+    int b0, n0, b1, n1;
+    universe_row(g, u, cell_start, cx, cy, cz, mz, my, b0, n0, b1, n1);
+    const int kk = k - (int)cum[lo];
+    return kk < n0 ? b0 + kk : b1 + (kk - n0);
+}
+// The same lookup done by the whole warp for ONE request (hp, k), all 32 lanes converged: the running sums are read 32
+// at a time (coalesced), the row is the number of sums <= k minus one (a ballot count) -- three loads deep instead of
+// eleven, and nobody waits alone (a lane that walks through the bisection by itself stalls its whole warp).
+__device__ inline int universe_pick_warp(const SortGrid &g, const Universe &u, const int *__restrict__ cell_start, int hp, int k,
+                                         int lane) {
+    const int cx = hp & 1023, cy = (hp >> 10) & 1023, cz = hp >> 20;
+    const int h = (cz * g.gn[1] + cy) * g.gn[0] + cx;
+    const unsigned short *__restrict__ cum = u.cum + (size_t)h * u.stride;
+    int below = 0;
+    for (int base = 0; base < u.nrow; base += 32) {
+        const int row = base + lane;
+        const bool ok = row < u.nrow && (int)cum[row] <= k;
+        below += __popc(__ballot_sync(0xffffffffu, ok));
+    }
+    const int lo = below - 1;   // (cum[0] = 0 <= k)
+    const int mz = (lo * u.inv_cnt1) >> 16, my = lo - mz * u.cnt[1];
+    int b0, n0, b1, n1;
+    universe_row(g, u, cell_start, cx, cy, cz, mz, my, b0, n0, b1, n1);
+    const int kk = k - (int)cum[lo];
+    return kk < n0 ? b0 + kk : b1 + (kk - n0);
+}
+__device__ inline int universe_size(const SortGrid &g, const Universe &u, int hp) {
+    const int h = ((hp >> 20) * g.gn[1] + ((hp >> 10) & 1023)) * g.gn[0] + (hp & 1023);
+    return (int)u.cum[(size_t)h * u.stride + u.nrow];
 }
 
 struct Topo {  // per-atom CSR of bonded terms in ORIGINAL indices (device)
@@ -227,22 +277,6 @@ struct Topo {  // per-atom CSR of bonded terms in ORIGINAL indices (device)
     const int *aptr, *arole, *aa, *ab;  // angles: my role (0 end i, 1 vertex, 2 end k) and the two other atoms
     const float *ak, *at0;
 };
-
-// k-th atom (sorted index) of the universe of home cell h: bisection on the running sums of the stencil rows (a dozen
-// dependent 2-byte loads from a few cache lines), then the row's one or two runs
-__device__ inline int universe_pick(const SortGrid &g, const Universe &u, const int *__restrict__ cell_start, int h, int k) {
-    const unsigned short *__restrict__ cum = u.cum + (size_t)h * u.stride;
-    int lo = 0, hi = u.nrow - 1;   // last row with cum[row] <= k
-    while (lo < hi) {
-        const int mid = (lo + hi + 1) >> 1;
-        if ((int)cum[mid] <= k) lo = mid; else hi = mid - 1;
-    }
-    const int cx = h % g.gn[0], cy = (h / g.gn[0]) % g.gn[1], cz = h / (g.gn[0] * g.gn[1]);
-    int b0, n0, b1, n1;
-    universe_row(g, u, cell_start, cx, cy, cz, lo, b0, n0, b1, n1);
-    const int kk = k - (int)cum[lo];
-    return kk < n0 ? b0 + kk : b1 + (kk - n0);
-}
 
 constexpr float RING_TIE = 4e-3f;   // A^2: an fp32 r^2 this close to a ring edge is re-decided in fp64 (R-17)
 

@@ -68,7 +68,8 @@ int launch_universe_list(const SortGrid &g, const Universe &u, const int *cell_s
                          cudaStream_t st, int64_t *launches);
 void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS], float rmax_all, const int *cell_start,
                        const float4 *xs, const float4 *xl, const float2 *lj, const int *orig, const int *sorted_of,
-                       const int *excl_ptr, const int *excl_idx, Counters *ctr, cudaStream_t st, int64_t *launches);
+                       const int *excl_ptr, const int *excl_idx, Counters *ctr, int *cell_of, float far2, cudaStream_t st,
+                       int64_t *launches);
 int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *xs, const float2 *lj, float4 *out,
                 int accumulate, bool energy, cudaStream_t st, int64_t *launches);
 void launch_count_pairs(const Model &m, const Row &row, const float4 *xs, float rc2, unsigned long long *out,

@@ -138,11 +138,12 @@ __global__ void k_permute(int n, const int *__restrict__ src, const int *__restr
                           const float2 *__restrict__ lj_in, const float2 *__restrict__ mi_in,
                           float4 *__restrict__ xs, float4 *__restrict__ vs, float2 *__restrict__ lj,
                           float2 *__restrict__ mi, int *__restrict__ orig, int *__restrict__ sorted_of,
-                          float4 *__restrict__ x_build, const int *__restrict__ key, int *__restrict__ cell_of) {
+                          float4 *__restrict__ x_build, const int *__restrict__ key, int *__restrict__ cell_of, int gnx, int gny) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int s = src[i];
-    cell_of[i] = key[s];
+    const int kk = key[s];   // home cell, packed by coordinates (the universe lookup wants them without divisions)
+    cell_of[i] = pack_cell(kk % gnx, (kk / gnx) % gny, kk / (gnx * gny));
     float4 x = xs_in[s];
     xs[i] = x;
     x_build[i] = x;
@@ -209,7 +210,7 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                                                               const float2 *__restrict__ lj,
                                                               const int *__restrict__ orig, const int *__restrict__ sorted_of,
                                                               const int *__restrict__ excl_ptr, const int *__restrict__ excl_idx,
-                                                              Counters *ctr) {
+                                                              Counters *ctr, int *__restrict__ cell_of, float far2) {
     __shared__ int seg_beg[BUILD_MAXSEG];       // stencil runs in ascending cell key (many are empty) ...
     __shared__ int seg_pre[BUILD_MAXSEG + 1];   // ... their lengths, then (length << 10 | non-empty) prefix sums
     __shared__ int run_beg[BUILD_MAXSEG];       // the non-empty runs, compacted: first atom ...
@@ -347,6 +348,9 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                     }
                 }
                 exr2 = __uint_as_float(__reduce_max_sync(full, __float_as_uint(exr2)));   // non-negative floats order as uints
+                // an excluded partner that could be found in jump ring C (R-10c): the chains then check the universe's
+                // candidates against the exclusion list (never so in water)
+                if (cell_of && lane == 0 && c0 == 0 && exr2 > far2) cell_of[i] |= 1 << 30;
                 exr2 = exr2 * 1.0001f + 2e-3f;   // also catches the atom itself (r^2 = 0)
                 int ex4[4];
 #pragma unroll
@@ -473,7 +477,8 @@ __global__ void __launch_bounds__(128) k_universe(SortGrid g, Universe u, const 
         int len = 0;
         if (p < u.nrow) {
             int b0, n0, b1, n1;
-            universe_row(g, u, cell_start, cx, cy, cz, p, b0, n0, b1, n1);
+            const int mz = p / u.cnt[1];
+            universe_row(g, u, cell_start, cx, cy, cz, mz, p - mz * u.cnt[1], b0, n0, b1, n1);
             len = n0 + n1;
         }
         int inc = len;
@@ -492,7 +497,7 @@ __global__ void __launch_bounds__(128) k_universe(SortGrid g, Universe u, const 
 }
 // the universe of one home cell as a list of sorted indices (observer: jump_get_row), one thread per entry, through the
 // same lookup the jump chains use
-__global__ void k_universe_list(SortGrid g, Universe u, const int *__restrict__ cell_start, int h, int n, int *__restrict__ out) {
+__global__ void k_universe_list(SortGrid g, Universe u, const int *__restrict__ cell_start, int h, int n, int *__restrict__ out) {   // h: packed home cell
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k < n) out[k] = universe_pick(g, u, cell_start, h, k);
 }
@@ -517,7 +522,7 @@ void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches) {
     k_scatter<<<nblk(a.n, B), B, 0, st>>>(a.n, a.key, a.orig_in, a.cell_start, a.cell_fill, a.tmp_orig, a.tmp_src);
     k_cell_sort<<<nblk(a.grid.ncell, B), B, 0, st>>>(a.grid.ncell, a.cell_start, a.tmp_orig, a.tmp_src);
     k_permute<<<nblk(a.n, B), B, 0, st>>>(a.n, a.tmp_src, a.tmp_orig, a.xs_in, a.vs_in, a.xl_in, a.xl, a.lj_in, a.mi_in, a.xs, a.vs,
-                                          a.lj, a.mi, a.orig, a.sorted_of, a.x_build, a.key, a.cell_of);
+                                          a.lj, a.mi, a.orig, a.sorted_of, a.x_build, a.key, a.cell_of, a.grid.gn[0], a.grid.gn[1]);
     *launches += 5;
 }
 
@@ -536,7 +541,8 @@ int launch_universe_list(const SortGrid &g, const Universe &u, const int *cell_s
 
 void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS], float rmax_all, const int *cell_start,
                        const float4 *xs, const float4 *xl, const float2 *lj, const int *orig, const int *sorted_of,
-                       const int *excl_ptr, const int *excl_idx, Counters *ctr, cudaStream_t st, int64_t *launches) {
+                       const int *excl_ptr, const int *excl_idx, Counters *ctr, int *cell_of, float far2, cudaStream_t st,
+                       int64_t *launches) {
     RowSet rs;
     for (int k = 0; k < N_ROWS; ++k) rs.r[k] = rows[k];
     // stencil of cells within reach of a cell: gap between cells at offset o is (|o| - 1)_+ cell edges
@@ -577,9 +583,9 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
 #define JB_BUILD(MASK)                                                                                                        \
     do {                                                                                                                      \
         if (fast) k_build_rows<MASK, true><<<nblocks, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, \
-                                                                                       orig, sorted_of, excl_ptr, excl_idx, ctr);         \
+                                                                                       orig, sorted_of, excl_ptr, excl_idx, ctr, cell_of, far2); \
         else k_build_rows<MASK, false><<<nblocks, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, \
-                                                                                    orig, sorted_of, excl_ptr, excl_idx, ctr);            \
+                                                                                    orig, sorted_of, excl_ptr, excl_idx, ctr, cell_of, far2);   \
     } while (0)
     switch (mask) {
         case 0x07: JB_BUILD(0x07); break;   // S A B     (JUMP with Coulomb and LJ jumps)

@@ -7,191 +7,9 @@
 // Chains of different atoms are independent and a jump of type (i,j) changes v_i only
 // (P:L342): one chain per thread, writing nothing but its own v_i -- no cross-atom conflict; several
 // events on one atom are resolved in time order inside its chain.
-#include "launch.h"
+#include "chains.cuh"
 
 namespace jb {
-
-struct Tally {  // per-thread statistics, reduced once per warp at the end
-    unsigned proposals, accepts, gt_attempts, expiries;
-    float max_p, max_gl;
-};
-
-__device__ inline void log_event(const UpdateArgs &a, unsigned step, int stream, int atom, int iter, int ring, int j,
-                                 int accepted, int n_gt, float T, float p, float U, float gt) {
-    if (!a.events) return;
-    unsigned long long slot = atomicAdd(&a.ctr->n_events, 1ull);
-    if (slot >= (unsigned long long)a.event_cap) { atomicOr(&a.ctr->err, (unsigned)ERR_EVENTS); return; }
-    jump_event e;
-    e.step = (int)step; e.stream = stream; e.atom = atom; e.iter = iter;
-    e.ring = ring; e.j = j; e.accepted = accepted; e.n_gt = n_gt;
-    e.T = T; e.p = p; e.U = U; e.gt = gt;
-    a.events[slot] = e;
-}
-
-// Theta(eta) = E[(eta+G)_+] = eta Phi(eta) + phi(eta)  (R-5).  With x = |eta| / sqrt 2 both terms share
-// e^{-x^2}: erfc(x) = e^{-x^2} erfcx_poly(x), phi = e^{-x^2} / sqrt(2 pi).  Beyond the polynomial's range
-// (|eta| > 6.08) Theta is eta_+ to 1e-10, far below the smallest uniform (2^-24).
-__device__ inline float theta_of(float eta) {
-    const float x = fabsf(eta) * 0.70710678118654752f;
-    if (x > 4.3f) return fmaxf(eta, 0.f);
-    const float ex = expf(-x * x);
-    const float half_erfc = 0.5f * ex * erfcx_poly(x);            // Phi(-|eta|)
-    const float Phi = eta > 0.f ? 1.f - half_erfc : half_erfc;
-    return fmaf(eta, Phi, kInvSqrt2Pi * ex);
-}
-
-// G~ ~ f_eta by rejection (R-6; proposal family of P:L310).  One Philox block per attempt.
-__device__ inline float gtilde(float eta, unsigned atom, unsigned step, unsigned stream, unsigned &block,
-                               const Model &m, int &attempts) {
-    uint32_t w[4];
-    int it = 0;
-    float out = 0.f;
-    for (;;) {
-        ++it;
-        philox4x32_10(atom, step, stream, block++, m.key0, m.key1, w);
-        float u0 = u01(w[0]), u1 = u01(w[1]), u2 = u01(w[2]), u3 = u01(w[3]);
-        if (eta < -2.5f) {  // Gamma(2, |eta|)
-            float z = -(logf(u0) + logf(u1)) / fabsf(eta);
-            if (u2 <= expf(-0.5f * z * z)) { out = z - eta; break; }
-        } else if (eta < -1.f) {  // Exponential(|eta|)
-            float z = -logf(u0) / fabsf(eta);
-            if (u1 <= z * expf(0.5f * (1.f - z * z))) { out = z - eta; break; }
-        } else if (eta <= 0.f) {  // Rayleigh
-            float z = sqrtf(-2.f * logf(u0));
-            if (u1 <= expf(eta * z)) { out = z - eta; break; }
-        } else {  // Rayleigh-Gaussian mixture
-            float wR = 1.f / (1.f + eta * kSqrt2Pi);
-            if (u0 <= wR) { out = sqrtf(-2.f * logf(u1)); break; }
-            float y = sqrtf(-2.f * logf(u1)) * cospif(2.f * u2);
-            if (y > 0.f) { out = y; break; }
-            if (y > -eta) {
-                if (u3 <= (eta + y) / eta) { out = y; break; }
-            }
-        }
-        if (it >= 64) { out = (eta > 0.f) ? 0.f : -eta + 1.f; break; }
-    }
-    attempts = it;
-    return out;
-}
-
-// kick (7); eps = inf -> reflection (5)
-__device__ inline void jump_kick(float eps, float sbm, float nx, float ny, float nz, float gt, float &vx, float &vy,
-                                 float &vz) {
-    float vn = vx * nx + vy * ny + vz * nz, amp;
-    if (isinf(eps)) amp = 2.f * vn;
-    else amp = 2.f * eps / ((1.f + eps * eps) * sbm) * (eps * sbm * vn + gt);
-    vx -= amp * nx; vy -= amp * ny; vz -= amp * nz;
-}
-
-// geometry of a candidate pair: exact image pair (a, b) per dimension, d = a - b, r^2
-struct PairGeom { float ax, ay, az, bx, by, bz, dx, dy, dz, r2; };
-__device__ inline PairGeom pair_geom(const Model &m, const float4 &xi, const float4 &xj) {
-    PairGeom p;
-    image_pair1(xi.x, xj.x, m.box[0], m.inv_box[0], p.ax, p.bx);
-    image_pair1(xi.y, xj.y, m.box[1], m.inv_box[1], p.ay, p.by);
-    image_pair1(xi.z, xj.z, m.box[2], m.inv_box[2], p.az, p.bz);
-    p.dx = p.ax - p.bx; p.dy = p.ay - p.by; p.dz = p.az - p.bz;
-    p.r2 = p.dx * p.dx + p.dy * p.dy + p.dz * p.dz;
-    return p;
-}
-// long part of the Coulomb pair gradient, F_ij = grad_{x_i} (1-chi) u_C: returns the radial derivative
-__device__ inline float fij_coul(const Model &m, const PairGeom &p, float qi, float qj, float &rinv) {
-    if (p.r2 >= m.rE2 || p.r2 <= m.rlo2) { rinv = 0.f; return 0.f; }
-    rinv = rsqrtf(p.r2);
-    float r = p.r2 * rinv;
-    float qq = (float)kCoulomb * qi * qj;
-    float ex = expf(-m.alpha2 * p.r2), e = ex * erfcx_poly(m.alpha * r);
-    float u = qq * e * rinv;
-    float du = -(u + qq * kTwoOverSqrtPi * m.alpha * ex) * rinv;
-    float dchi, chi = chi_zone<true>(p.ax, p.ay, p.az, p.bx, p.by, p.bz, p.r2, r, m, dchi);
-    return (1.f - chi) * du - dchi * u;
-}
-__device__ inline float fij_lj(const Model &m, const PairGeom &p, float2 lji, float2 ljj, float &rinv) {
-    if (p.r2 >= m.rE2 || p.r2 <= m.rlo2 || !(ljj.y > 0.f)) { rinv = 0.f; return 0.f; }
-    rinv = rsqrtf(p.r2);
-    float r = p.r2 * rinv;
-    float s = lji.x * ljj.x * rinv, s2 = s * s, s6 = s2 * s2 * s2, s12 = s6 * s6;
-    float e4 = lji.y * ljj.y;
-    float u = e4 * (s12 - s6), du = e4 * (6.f * s6 - 12.f * s12) * rinv;
-    float dchi, chi = chi_zone<true>(p.ax, p.ay, p.az, p.bx, p.by, p.bz, p.r2, r, m, dchi);
-    return (1.f - chi) * du - dchi * u;
-}
-
-// ---- step (C'): Algorithm 4 + ring (R-11) --------------------------------------------------------------------
-// G lanes cooperate on one chain, and nothing in the common case is sequential:
-//  * what proposal k needs from the random stream and from x -- the exponential E_k, the ring, the partner j, the
-//    uniform U_k and the pair gradient F_ij(x) -- depends neither on the chain's state nor on the other
-//    proposals (x is frozen during a jump phase; proposal k draws Philox block k of its stream, the G~ attempts
-//    have a stream of their own, R-15): lane l evaluates proposal kb + l;
-//  * the bound lambda-bar is re-evaluated after each ACCEPTED jump only (R-11), so between two accepted
-//    jumps the proposal times are a running sum of E_k / lambda-bar and v(t) = v_e + (t - t_e) a in closed form:
-//    every lane gets its own proposal time (an inclusive scan over the group), its expiry test, its acceptance
-//    probability and its accept test at once;
-//  * the first accepting lane (a ballot) ends the epoch: kick, new bound, the later lanes are dropped and the
-//    batch restarts after it -- accepted jumps are ~1-2 % of the proposals.
-struct ChainConst {   // per-atom constants of the jump chains (R-10c): the three rings of P:L424
-    int N[3];         // candidates: row A, row B, the cell universe of the home cell
-    int home;         // home cell (ring C)
-};
-__device__ inline ChainConst chain_const(const UpdateArgs &A, int i) {
-    ChainConst c;
-    c.N[0] = A.rowA.cnt[i]; c.N[1] = A.rowB.cnt[i];
-    c.home = A.uni.cell_of[i];
-    c.N[2] = (int)A.uni.cum[(size_t)c.home * A.uni.stride + A.uni.nrow];
-    return c;
-}
-// ring pick: the first ring whose cumulated weight exceeds ur * (sum of weights); a ring without
-// candidates can only be hit through rounding at an end, and the pick then falls back as the oracle's does
-__device__ inline int pick_ring(const ChainConst &c, float ur, float c0, float c1, float tot) {
-    const float x = ur * tot;
-    int ring = x < c0 ? 0 : (x < c1 ? 1 : 2);
-    while (c.N[ring] == 0 && ring > 0) --ring;
-    while (c.N[ring] == 0 && ring < 2) ++ring;
-    return ring;
-}
-// state-independent part of a proposal, from its Philox block w: ring pick and partner, the ring the
-// pair's CURRENT distance lies in (R-10c: through any other ring its rate is 0), then g = |F_ij| and n = F_ij / |F_ij|;
-// tag = ring << 28 | j_orig (event log only).  LJ: the long LJ gradient (step J') instead of the Coulomb one.
-template <bool LJ, bool WANT_J>
-__device__ inline void propose_pair(const Model &m, const UpdateArgs &A, const ChainConst &c, float c0, float c1, float tot,
-                                    int i, const float4 &xi, float2 lji, const uint32_t w[4], float &g, int &ring, float &nx,
-                                    float &ny, float &nz, int &tag) {
-    ring = pick_ring(c, u01(w[1]), c0, c1, tot);
-    const int k = (int)__umulhi(w[2], (unsigned)c.N[ring]);
-    int j;
-    if (ring == 0) j = A.rowA.idx[(size_t)i * A.rowA.cap + k];
-    else if (ring == 1) j = A.rowB.idx[(size_t)i * A.rowB.cap + k];
-    else j = universe_pick(A.grid, A.uni, A.cell_start, c.home, k);
-    const float4 xj = A.xs[j];
-    const PairGeom p = pair_geom(m, xi, xj);
-    const float lo2 = m.ring2[ring], hi2 = m.ring2[ring + 1];
-    bool in = p.r2 >= lo2 && p.r2 < hi2;
-    if (fminf(fabsf(p.r2 - lo2), fabsf(p.r2 - hi2)) < RING_TIE) {   // decide in fp64 from the full positions, like the oracle
-        const float4 li = A.xl_all[i], lo_j = A.xl_all[j];
-        double d[3] = {((double)xi.x + (double)li.x) - ((double)xj.x + (double)lo_j.x),
-                       ((double)xi.y + (double)li.y) - ((double)xj.y + (double)lo_j.y),
-                       ((double)xi.z + (double)li.z) - ((double)xj.z + (double)lo_j.z)};
-        double r2d = 0.0;
-#pragma unroll
-        for (int q = 0; q < 3; ++q) {
-            const double L = (double)m.box[q];
-            d[q] -= L * rint(d[q] / L);
-            r2d += d[q] * d[q];
-        }
-        in = r2d >= m.ring2d[ring] && r2d < m.ring2d[ring + 1];
-    }
-    if (in && ring == 2 && A.excl_ptr) {   // the universe is not filtered at a build: excluded partners have rate 0 (R-9)
-        const int o = A.orig[i], oj = A.orig[j];
-        for (int e = A.excl_ptr[o]; e < A.excl_ptr[o + 1]; ++e) in = in && A.excl_idx[e] != oj;
-    }
-    float rinv = 0.f, fr = 0.f;
-    if (in) fr = LJ ? fij_lj(m, p, lji, A.lj[j], rinv) : fij_coul(m, p, xi.w, xj.w, rinv);
-    const float sg = (fr > 0.f ? rinv : -rinv);  // n = F/|F|
-    g = fabsf(fr);
-    nx = p.dx * sg; ny = p.dy * sg; nz = p.dz * sg;
-    tag = 0;
-    if (WANT_J) tag = A.orig[j] | (ring << 28);
-}
 
 // The chain of one atom, run by the G lanes of its group.  The whole warp executes the loop together (while any
 // of its 32 / G groups still has a live chain, finished groups predicated off): groups of one warp never run one
@@ -379,17 +197,6 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, const ChainConst &c
     }
 }
 
-__device__ inline double wrap1d(double x, double L, double invL, int &img) {   // img += the number of box lengths taken off
-    const double k = floor(x * invL);   // (a product, not the 40-instruction fp64 division; off by one at most, fixed below)
-    x -= L * k;
-    int ik = (int)k;
-    if (x >= L) { x -= L; ++ik; }
-    if (x < 0.0) { x += L; --ik; }
-    if (x >= L || x < 0.0) x = 0.0;
-    img += ik;
-    return x;
-}
-
 // ---- the fused per-atom update: up to two velocity half-phases, then A O A + wrap ----------------------------
 // G lanes per atom (a power of two <= 32) share the atom's jump chains; lane 0 of the group does A-O-A and the stores.
 template <bool JUMPS, int G, bool LOG, bool ADAPT>
@@ -413,7 +220,7 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
     const bool any_lj = (jumpy0 && A.ph[0].lj) || (jumpy1 && A.ph[1].lj);
     float a0x = 0.f, a0y = 0.f, a0z = 0.f, a1x = 0.f, a1y = 0.f, a1z = 0.f;   // accelerations of the two phases
     ChainConst cc;
-    cc.N[0] = cc.N[1] = cc.N[2] = 0; cc.home = 0;
+    cc.N[0] = cc.N[1] = cc.N[2] = 0; cc.home = 0; cc.far_excl = false;
     float2 lji = make_float2(0.f, 0.f);
     if (live) {
         xi = A.xs[i]; v4 = A.vs[i]; mi = A.mi[i]; atom = (unsigned)A.orig[i];
