@@ -1,12 +1,15 @@
 """bench.py -- throughput of the JUMP hot path on B200 (one JSON line on stdout).
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--mode respa] [--impl reference]
 
-A "step" is one jump_step(1): the whole hot path (jump half-phases C'J', A-O-A, list rebuild at its natural
-period, F0 = bonded + short-range pairs, jump half-phases J'C') over one synthetic water box.  Workload:
-BASELINE.json configs[1] (12 000 atoms, 49.3 A, cutoffs 6 / 12 A, dt 1 fs), equilibrated by 2 000 BAOAB steps
-(untimed).  Metric: ns/day (higher is better); atom-steps/s, same-GPU BAOAB with the unsplit 12 A force,
-the kernel roofline and the fp64 oracle on the host cores ride along in the same line.
+Workload (default): BASELINE.json configs[4], the largest single-GPU configuration -- 999 999-atom flexible water
+box, 215.2 A, cutoffs 6 / 12 A, JUMP-RESPA with inner step 1 fs (bonded + short-range pair force) and outer step
+4 fs (jump half-phases C'J' / J'C' in place of the 6-12 A pair force), equilibrated by BAOAB steps (untimed).
+A "step" is one inner MD step of 1 fs, i.e. a quarter of one jump_respa_step(1): the whole hot path -- outer jump
+phases, A-O-A, list rebuild at its natural period, F0 = bonded + short-range pairs -- over the box.  Metric: ns/day
+(higher is better); atom-steps/s, the same box under plain JUMP and under same-GPU BAOAB / BAOAB-RESPA with the
+unsplit 12 A force, the per-kernel rooflines, the end-to-end figure through host buffers and the fp64 oracle on the
+host cores ride along in the same line; `secondary` repeats JUMP vs BAOAB on configs[1] (12 000 atoms).
 N > 1: the path does not shard on one GPU's box sizes (replicas only), so every rank
 runs an independent replica with its own seed; value = sum over ranks / max-over-ranks time.
 """
@@ -24,7 +27,7 @@ if ROOT not in sys.path:
 
 import numpy as np
 
-BLOCK = 10                 # steps per timed block = nlist_every, so every block holds exactly one rebuild
+BLOCK = 20                 # steps per timed API call: a multiple of n_inner and of the rebuild period
 FLOPS_PER_PAIR = 2 * 50    # ~50 FP32-pipe instructions per in-range half pair, counted as FMAs
 PROPOSAL_INSTR = 250       # ~150 FP32-pipe + ~100 INT-pipe (one Philox block) instructions per proposal
 CHAIN_INSTR = 60           # chain set-up + expiry per half-phase chain
@@ -87,30 +90,51 @@ def measured_peaks():
     return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
 
 
+def oracle_sample(sysd, run, mode, budget_s, state=None):
+    """The fp64 oracle as it stands on the host cores: whole-box steps of the same workload in the same mode until
+    ~budget_s of CPU time (at least one API unit).  state = (pos, vel) to start from, else the generator's lattice
+    state after two oracle BAOAB steps.  Returns (steps, seconds, cores, description)."""
+    from oracle import jump_oracle as jo
+    s2 = sysd if state is None else dict(sysd, pos=state[0], vel=state[1])
+    o = jo.Oracle(s2, **run)
+    if state is None:
+        o.baoab_step(2)
+    unit = run["n_inner"] if mode == "respa" else 1
+    call = (lambda: o.jump_respa_step(1)) if mode == "respa" else (lambda: o.jump_step(1))
+    t0 = time.perf_counter()
+    n = 0
+    while True:
+        call()
+        n += unit
+        dt = time.perf_counter() - t0
+        if dt > budget_s or n >= 400:
+            break
+    o.close()
+    what = "%d whole-box %s steps of 1 fs of the same %d-atom box (%.1f s), started from %s" % (
+        n, "JUMP-RESPA" if mode == "respa" else "JUMP", sysd["n_atoms"], dt,
+        "the state the timed GPU run started from" if state is not None else "the lattice state (2 oracle BAOAB steps)")
+    return n, dt, jo.num_threads(), what
+
+
 def run_reference(args):
-    """--impl reference: the fp64 oracle, as it stands, on the host cores (same config, metric and unit)."""
+    """--impl reference: the fp64 oracle, as it stands, on the host cores (same config, mode, metric and unit).  The
+    GPU arm equilibrates the box with its own BAOAB steps before timing; the oracle cannot do that for 10^6 atoms within
+    minutes, so its bounded sample starts from the generator's lattice state (said in config.workload)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from oracle import jump_oracle as jo
     from paper_2412_15073_b200 import workloads as wl
     sysd, run = wl.make_config(args.config)
-    o = jo.Oracle(sysd, **run)
-    o.jump_step(max(args.warmup, 1))
-    t0 = time.perf_counter()
-    o.jump_step(args.steps)
-    dt = time.perf_counter() - t0
-    sps = args.steps / dt
+    n, dt, cores, what = oracle_sample(sysd, run, args.mode, budget_s=max(10.0, 0.02 * args.steps))
+    sps = n / dt
     val = ns_per_day(sps, run["dt_fs"])
-    cores = jo.num_threads()
-    line = {"impl": "reference", "metric": "ns_per_day_jump", "value": val, "unit": "ns/day", "n_gpus": args.gpus,
-            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "BASELINE configs[%d]: %d-atom flexible water box, lattice start (not equilibrated)"
-                                   % (args.config, sysd["n_atoms"])},
+    line = {"impl": "reference", "metric": "ns_per_day_jump" if args.mode == "jump" else "ns_per_day_jump_respa", "value": val,
+            "unit": "ns/day", "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / n,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "BASELINE configs[%d]: %d-atom flexible water box, %s; oracle sample: %s"
+                                   % (args.config, sysd["n_atoms"], "JUMP-RESPA n_inner %d" % run["n_inner"] if args.mode == "respa" else "JUMP", what)},
             "atom_steps_per_s": sps * sysd["n_atoms"],
-            "cpu_baseline": {"value": val, "unit": "ns/day", "cores": cores, "kind": "oracle",
-                             "sample": "%d whole-box JUMP steps" % args.steps},
+            "cpu_baseline": {"value": val, "unit": "ns/day", "cores": cores, "kind": "oracle", "sample": what},
             "e2e": {"value": val, "unit": "ns/day", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
 
@@ -126,23 +150,11 @@ def _dist_setup(n_gpus):
     return rank, world, dist
 
 
-def run_cpu_baseline(sysd, run, budget_s=15.0):
-    """The fp64 oracle as it stands on the host cores: whole-box JUMP steps of the same workload until ~budget_s."""
-    from oracle import jump_oracle as jo
-    o = jo.Oracle(sysd, **run)
-    o.jump_step(1)
-    t0 = time.perf_counter()
-    n = 0
-    while True:
-        o.jump_step(1)
-        n += 1
-        dt = time.perf_counter() - t0
-        if dt > budget_s or n >= 200:
-            break
-    o.close()
+def run_cpu_baseline(sysd, run, mode, state, budget_s=15.0):
+    """cpu_baseline leg: the oracle on the same workload, same mode, from the state the timed GPU run started from."""
+    n, dt, cores, what = oracle_sample(sysd, run, mode, budget_s, state=state)
     sps = n / dt
-    return {"value": ns_per_day(sps, run["dt_fs"]), "unit": "ns/day", "cores": jo.num_threads(), "kind": "oracle",
-            "sample": "%d whole-box JUMP steps of the same %d-atom box (%.1f s)" % (n, sysd["n_atoms"], dt),
+    return {"value": ns_per_day(sps, run["dt_fs"]), "unit": "ns/day", "cores": cores, "kind": "oracle", "sample": what,
             "atom_steps_per_s": sps * sysd["n_atoms"]}
 
 
@@ -165,14 +177,18 @@ def timed_blocks(torch, sim, stream, call, n_steps, block, flush):
     return sum(a.elapsed_time(b) for a, b in evs)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures of this command on the
-# configs[1] workload (profiles/r1_final_README.md); other workloads have no capture: null
-NCU_TRAFFIC_CFG1 = {"update": 9.67e6, "pair": 7.99e6, "build": 6.16e6}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures of
+# `python bench.py --steps 40 --warmup 8 --equil 60 --no-cpu-baseline --secondary-config -1` on the default workload
+# (profiles/r2_cfg4_README.md, profiles/r2_cfg4_dram_bytes.csv); other workloads have no capture: null
+NCU_TRAFFIC_CFG4 = {}
+BONDED_BYTES_PER_ATOM = 56    # per water: 16 B record + 3 x (16 + 16 B read, 16 B written)
 
 
 def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, props, peaks, traffic=None):
     """Per-kernel device times of K more steps (CUDA events on the streams the kernels are launched on, recorded by
-    the library around each kernel group) against each kernel's roofline.  Returns (dominant line, other lines)."""
+    the library around each kernel group) against each kernel's roofline.  Returns (dominant line, other lines).
+    The bonded kernels run on a side stream beside k_pair, so their bracket inside a step is stretched by the overlap:
+    their own time is taken from five stand-alone evaluations (jump_get_forces(3): bonded kernels + one 13 us copy)."""
     with torch.cuda.stream(stream):
         sim.reset_stats()
         r0 = sim.stats()["rebuilds"]
@@ -182,13 +198,24 @@ def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, pro
         sim.set_profiling(False)
         pstats = sim.stats()
         n_pairs_ordered = sim.count_pairs(0, run["r_short"])           # ordered in-range entries of the short row
-        row_entries = sum(sim.count_pairs(k, 1e3) for k in (0, 1, 2, 3) if pstats["cap_row"][k])
+        row_entries = sum(sim.count_pairs(k, 1e3) for k in (0, 1, 2) if pstats["cap_row"][k])
+        sim.forces(3)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(5):
+            sim.forces(3)
+        e1.record(stream)
+        stream.synchronize()
+        bonded_ms = e0.elapsed_time(e1) / 5
     rebuilds = max(pstats["rebuilds"] - r0, 1)
-    tot_prof = sum(v[0] for v in prof.values())
-    share = {k: (v[0] / tot_prof if tot_prof else 0.0) for k, v in prof.items()}
+    tot = {k: v[0] for k, v in prof.items()}
+    tot["bonded"] = bonded_ms * prof["bonded"][1]
+    tot_prof = sum(tot.values())
+    share = {k: (v / tot_prof if tot_prof else 0.0) for k, v in tot.items()}
     peak_tflops = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
     alu_src = "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (%s sm_max_mhz)" % (props.multi_processor_count, peaks["sm_max_mhz"],
                                                                       peaks["source"])
+    hbm_src = "%s HBM copy bandwidth (MEASURED_PEAKS.json)" % peaks["source"]
 
     def avg_ms(cat):
         return prof[cat][0] / max(prof[cat][1], 1)
@@ -199,82 +226,91 @@ def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, pro
                 "frac": ach / peak_tflops, "traffic": None, "peak_source": alu_src, "algorithmic": what,
                 "avg_launch_us": 1e3 * avg_ms(cat), "share_of_step": share[cat]}
 
+    def hbm_line(kernel, nbytes, what, ms, cat):
+        ach = nbytes / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
+        return {"kernel": kernel, "bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                "frac": ach / peaks["hbm_gbs"], "traffic": None, "peak_source": hbm_src, "algorithmic": what,
+                "avg_launch_us": 1e3 * ms, "share_of_step": share[cat]}
+
     half_pairs = n_pairs_ordered / 2.0
     n_upd = max(prof["update"][1], 1)
-    chains = 2.0 * n * (2 if run["flags"] & 2 else 1)                  # half-phases x (C' [+ J']) per update launch
+    chains = 2.0 * n * (2 if run["flags"] & 2 else 1)                  # half-phases x (C' [+ J']) per jump update launch
     upd_instr = pstats["proposals"] / n_upd * PROPOSAL_INSTR + chains * CHAIN_INSTR
-    build_ms = prof["build"][0] / rebuilds                             # sort (5 kernels) + k_build_rows, per rebuild
-    build_bytes = row_entries * 4.0 + n * 48.0
-    build_ach = build_bytes / (build_ms * 1e-3) / 1e9 if build_ms > 0 else 0.0
+    build_ms = prof["build"][0] / rebuilds                             # sort (7 kernels) + k_universe + k_build_rows, per rebuild
     lines = {
         "pair": alu_line("k_pair (short-range switched pair gradient, a5)", half_pairs * FLOPS_PER_PAIR,
                          "%.0f in-range half pairs x %d flop" % (half_pairs, FLOPS_PER_PAIR), "pair"),
-        "update": alu_line("k_update (jump chains C'J' of two half-phases + A-O-A, a6-a8)", 2.0 * upd_instr,
-                           "%.0f proposals x %d + %.0f chains x %d FP32/INT-pipe instructions, x 2 flop"
+        "update": alu_line("k_update (jump chains of the phases it carries + A-O-A, a6-a8), average over its launches",
+                           2.0 * upd_instr,
+                           "%.0f proposals x %d + %.0f chains x %d FP32/INT-pipe instructions, x 2 flop, per launch"
                            % (pstats["proposals"] / n_upd, PROPOSAL_INSTR, chains, CHAIN_INSTR), "update"),
-        "build": {"kernel": "sort + k_build_rows (a1-a3), one group per rebuild", "bound": "hbm", "achieved": build_ach,
-                  "peak": peaks["hbm_gbs"], "unit": "GB/s", "frac": build_ach / peaks["hbm_gbs"], "traffic": None,
-                  "peak_source": "%s HBM copy bandwidth" % peaks["source"],
-                  "algorithmic": "%.0f row entries x 4 B + %d atoms x 48 B" % (row_entries, n),
-                  "avg_launch_us": 1e3 * build_ms, "share_of_step": share["build"]},
+        "build": hbm_line("sort + k_universe + k_build_rows (a1-a3), per rebuild", row_entries * 4.0 + n * 48.0,
+                          "%.0f row entries x 4 B + %d atoms x 48 B" % (row_entries, n), build_ms, "build"),
+        "bonded": hbm_line("k_bonded_mol (+ k_bonded_csr) (a4), stand-alone", n * float(BONDED_BYTES_PER_ATOM),
+                           "%d atoms x %d B" % (n, BONDED_BYTES_PER_ATOM), bonded_ms, "bonded"),
     }
     for k, line in lines.items():
         if traffic and k in traffic:
             line["traffic"] = traffic[k]
-            line["traffic_source"] = "ncu --set full capture of k_%s, profiles/r1_final_dram_bytes.csv (bytes per launch)" % k
-    share_note = "device time per kernel group / sum over groups; k_bonded runs on a side stream beside k_pair, so the groups overlap"
-    dominant = max(("pair", "update", "build"), key=lambda k: share[k])
+            line["traffic_source"] = "ncu --set full capture of the %s kernel, profiles/r2_cfg4_dram_bytes.csv (bytes per launch)" % k
+    share_note = ("device time per kernel group / sum over groups (bonded: stand-alone time x launches; inside a step it "
+                  "runs on a side stream beside k_pair)")
+    dominant = max(lines, key=lambda k: share[k])
     roofline = dict(lines[dominant], kernel_ms_share=share, share_note=share_note)
     return roofline, {k: v for k, v in lines.items() if k != dominant}
 
 
-def large_box_rooflines(torch, jb, wl, dev, stream, flush, props, peaks, config, steps):
-    """The same kernel lines on a box large enough to fill the GPU (BASELINE configs[4], ~1e6 atoms: 'throughput and
-    roofline at 1 B200'); the configs[1] box of the headline metric leaves every kernel latency-bound."""
+def comparators(torch, sim, stream, flush, run, n, steps):
+    """Same box, same state, other schemes (reported baselines): plain JUMP, BAOAB with the unsplit force to r_long,
+    and -- for the RESPA headline -- nothing else: BAOAB-RESPA needs its own context (a flag fixed at init)."""
+    out = {}
+    with torch.cuda.stream(stream):
+        for name, call in (("jump", sim.jump_step), ("baoab", sim.baoab_step)):
+            call(BLOCK)
+            sim.sync()
+            ms = timed_blocks(torch, sim, stream, call, steps, BLOCK, flush)
+            out[name] = {"ms_per_step": ms / steps, "ns_per_day": ns_per_day(steps / (ms * 1e-3), run["dt_fs"]),
+                         "atom_steps_per_s": n * steps / (ms * 1e-3), "steps": steps}
+    out["baoab"]["force"] = "unsplit pair force to r_long = %.0f A" % run["r_long"]
+    return out
+
+
+def secondary_config(torch, jb, wl, dev, stream, flush, config, equil, steps):
+    """JUMP vs same-GPU BAOAB on a small box (BASELINE configs[1]: 'JUMP vs BAOAB'), where every kernel is bound by
+    latency rather than throughput."""
     sysd, run = wl.make_config(config)
     n = sysd["n_atoms"]
     with torch.cuda.stream(stream):
         sim = jb.JumpSim(sysd, device=dev, stream=stream, **run)
-        sim.baoab_step(300)
-        sim.jump_step(30)
+        sim.set_lax_skin(True)
+        sim.baoab_step(equil)
+        sim.set_lax_skin(False)
         sim.sync()
-        ms = timed_blocks(torch, sim, stream, sim.jump_step, steps, BLOCK, flush)
-        line, other = kernel_rooflines(torch, sim, stream, sim.jump_step, steps, BLOCK, flush, run, n, props, peaks)
-        n_in = run["n_inner"]
-        sim.jump_respa_step(5)
-        sim.sync()
-        ms_r = timed_blocks(torch, sim, stream, lambda b: sim.jump_respa_step(b // n_in), (steps // 20) * 20, 20, flush)
-        sim.baoab_step(20)
-        sim.sync()
-        ms_b = timed_blocks(torch, sim, stream, sim.baoab_step, steps, BLOCK, flush)
-        err = sim.stats()["error"]
+        sim.reset_stats()
+        cmp_ = comparators(torch, sim, stream, flush, run, n, steps)
+        st = sim.stats()
     sim.close()
-    lines = dict(other)
-    lines["dominant"] = line
-    return {"workload": "BASELINE configs[%d]: %d-atom flexible water box %.1f A, JUMP, equilibrated by 300 BAOAB steps"
-                        % (config, n, sysd["box"]),
-            "steps": steps, "ms_per_step": ms / steps, "ns_per_day": ns_per_day(steps / (ms * 1e-3), run["dt_fs"]),
-            "atom_steps_per_s": n * steps / (ms * 1e-3), "baoab_ms_per_step": ms_b / steps,
-            "jump_respa": {"n_inner": n_in, "ms_per_inner_step": ms_r / ((steps // 20) * 20),
-                           "ns_per_day": ns_per_day(((steps // 20) * 20) / (ms_r * 1e-3), run["dt_fs"]),
-                           "what": "JUMP-RESPA, inner %g fs (bonded + short-range), outer %g fs (jumps), configs[4]'s mode"
-                                   % (run["dt_fs"], n_in * run["dt_fs"])},
-            "jump_vs_baoab": ms_b / ms, "error": err, "kernels": lines}
+    return {"workload": "BASELINE configs[%d]: %d-atom flexible water box %.1f A, equilibrated by %d BAOAB steps"
+                        % (config, n, sysd["box"], equil),
+            "jump": cmp_["jump"], "baoab_same_gpu": cmp_["baoab"],
+            "jump_vs_baoab": cmp_["baoab"]["ms_per_step"] / cmp_["jump"]["ms_per_step"], "error": st["error"],
+            "max_disp_A": st["max_disp"]}
 
 
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=2000)
-    ap.add_argument("--warmup", type=int, default=200)
-    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=100)
+    ap.add_argument("--config", type=int, default=4)
     ap.add_argument("--impl", default="b200")
-    ap.add_argument("--equil", type=int, default=2000, help="untimed BAOAB equilibration steps from the lattice start")
+    ap.add_argument("--equil", type=int, default=600, help="untimed BAOAB equilibration steps from the lattice start")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--large-config", type=int, default=4,
-                    help="also report the kernel rooflines on this (GPU-filling) config, N=1 only; -1: skip")
-    ap.add_argument("--mode", default="jump", choices=["jump", "respa"])
-    ap.add_argument("--r-mid", type=float, default=None, help="ring split r_M (default: the config's)")
+    ap.add_argument("--secondary-config", type=int, default=1,
+                    help="also report JUMP vs BAOAB on this small config, N=1 only; -1: skip")
+    ap.add_argument("--mode", default="respa", choices=["jump", "respa"])
+    ap.add_argument("--r-mid", type=float, default=None, help="outer ring edge r_M (default: the config's)")
+    ap.add_argument("--r-mid-in", type=float, default=None, help="inner ring edge r_A (default: the config's)")
     ap.add_argument("--skin", type=float, default=None)
     ap.add_argument("--nlist-every", type=int, default=None)
     ap.add_argument("--eps-jump", type=float, default=None)
@@ -293,25 +329,30 @@ def main():
 
     sysd, run = wl.make_config(args.config)
     run = dict(run, seed=replicas.rank_seed(run["seed"], rank))       # independent replicas
-    for key, val in (("r_mid", args.r_mid), ("skin", args.skin), ("nlist_every", args.nlist_every), ("eps_jump", args.eps_jump)):
+    for key, val in (("r_mid", args.r_mid), ("r_mid_in", args.r_mid_in), ("skin", args.skin), ("nlist_every", args.nlist_every),
+                     ("eps_jump", args.eps_jump)):
         if val is not None:
             run[key] = val
     n, dt_fs = sysd["n_atoms"], run["dt_fs"]
+    respa = args.mode == "respa"
+    per_call = run["n_inner"] if respa else 1                          # MD steps of length dt per API unit
+    block = BLOCK
     stream = torch.cuda.Stream(dev)
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
     with torch.cuda.stream(stream):
         sim = jb.JumpSim(sysd, device=dev, stream=stream, **run)
+        sim.set_lax_skin(True)                                         # the lattice start is hot: no skin check while it relaxes
         sim.baoab_step(args.equil)
+        sim.set_lax_skin(False)                                        # from here on a displacement beyond skin/2 is an error
         sim.sync()
         sim.reset_stats()
-        respa = args.mode == "respa"
-        per_call = run["n_inner"] if respa else 1                      # MD steps of length dt per API unit
         step_call = (lambda b: sim.jump_respa_step(b // per_call)) if respa else sim.jump_step
-        block = BLOCK
-        K = max(args.steps // per_call * per_call, per_call)
+        K = max(args.steps // block * block, block)
         W = max(args.warmup, 3)
-        step_call(max(W // per_call * per_call, per_call))
+        W_steps = max((W + block - 1) // block * block, block)
+        step_call(W_steps)
         sim.sync()
+        state0 = (sim.pos.detach().cpu().numpy().astype(np.float64), sim.vel.detach().cpu().numpy().astype(np.float64))
 
     # ---- timed region: K steps, device time, max over ranks --------------------------------------------------
     sampler = ClockSampler(local)
@@ -328,89 +369,25 @@ def main():
         dist.barrier()
     launches = sim.launches - l0
     clocks = sampler.stop()
-    sim.sync()
+    timed_error = None
+    try:
+        sim.sync()                                                     # any device error flag (skin, bound, overflow) is reported
+    except jb.JumpError as e:
+        timed_error = str(e)
     ms_max = replicas.max_over_ranks(ms, dist, dev)
     stats = sim.stats()
 
-    # ---- per-kernel times of the same K steps (CUDA events on the launch stream, separate pass) --------------
-    roofline, roofline_other = kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, props, peaks,
-                                                traffic=NCU_TRAFFIC_CFG1 if (args.config == 1 and not respa) else None)
+    # ---- per-kernel times of K more steps (CUDA events on the launch streams, separate pass) -------------------
+    Kp = min(K, 200)
+    roofline, roofline_other = kernel_rooflines(torch, sim, stream, step_call, Kp, block, flush, run, n, props, peaks,
+                                                traffic=NCU_TRAFFIC_CFG4 if args.config == 4 else None)
 
-    # ---- same-GPU BAOAB with the unsplit r_long force (reported baseline) -------------------------------------
-    with torch.cuda.stream(stream):
-        sim.baoab_step(50)
-        sim.sync()
-        Kb = min(K, 500)
-        ms_b = timed_blocks(torch, sim, stream, sim.baoab_step, Kb, block, flush)
-    baoab = {"ns_per_day": ns_per_day(Kb / (ms_b * 1e-3), dt_fs), "ms_per_step": ms_b / Kb, "steps": Kb,
-             "force": "unsplit pair force to r_long = %.0f A" % run["r_long"]}
-
-    # ---- the paper's preferred setting, adaptive eps(x) = eps0 |F_ij(x)| (NEXT-1, R-19), same box ------
-    adaptive = None
-    if not respa:
-        with torch.cuda.stream(stream):
-            run_a = dict(run, eps_mode=1, eps_jump=2.0)
-            sim_a = jb.JumpSim(sysd, device=dev, stream=stream, **run_a)
-            sim_a.baoab_step(args.equil)
-            sim_a.jump_step(max(W, 50))
-            sim_a.sync()
-            sim_a.reset_stats()
-            Ka = min(K, 1000)
-            ms_a = timed_blocks(torch, sim_a, stream, sim_a.jump_step, Ka, block, flush)
-            st_a = sim_a.stats()
-            sim_a.close()
-        adaptive = {"eps0_A_mol_per_kcal": 2.0, "steps": Ka, "ms_per_step": ms_a / Ka,
-                    "ns_per_day": ns_per_day(Ka / (ms_a * 1e-3), dt_fs),
-                    "proposals_per_atom_step": st_a["proposals"] / (n * Ka), "accepts_per_atom_step": st_a["accepts"] / (n * Ka),
-                    "max_p": st_a["max_p"], "error": st_a["error"]}
-
-    # ---- NEXT-2: three-level JUMP-RESPA1 1:2:6 fs (the paper's Table 2 setting) against BAOAB-RESPA1 1:2:6, the
-    # reciprocal Ewald sum as the slow force (R-21), same box --------------------------------------------
-    respa1 = None
-    if not respa and rank == 0:
-        respa1 = {"levels_fs": [dt_fs, 2 * dt_fs, 6 * dt_fs],
-                  "what": "delta: bonded; kappa = 2 delta: short non-bonded + jumps (JUMP) or kick (BAOAB); Delta = 3 kappa: "
-                          "reciprocal Ewald sum + exclusion correction (+ long pair gradient for BAOAB-RESPA1, P:L511)"}
-        for name, fl in (("jump_respa1", 3 | 8), ("baoab_respa1", 3 | 8 | 16)):
-            with torch.cuda.stream(stream):
-                sim_r = jb.JumpSim(sysd, device=dev, stream=stream, **dict(run, flags=fl, n_inner=2))
-                sim_r.baoab_step(args.equil)
-                nk = sim_r.ewald_setup()
-                sim_r.jump_respa1_step(10, 3)
-                sim_r.sync()
-                Kr = max(min(K, 600) // 6, 1)
-                ms_r = timed_blocks(torch, sim_r, stream, lambda b: sim_r.jump_respa1_step(b, 3), Kr, 2, flush)
-                if name == "jump_respa1":   # the slow force alone (three kernels), per evaluation
-                    sim_r.forces(5)
-                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    e0.record(stream)
-                    for _ in range(10):
-                        sim_r.forces(5)
-                    e1.record(stream)
-                    stream.synchronize()
-                    ms_s = e0.elapsed_time(e1) / 10
-                    # algorithmic work per (atom, k-vector) pair in the factorised form: structure
-                    # factor 5 fp64 multiply-adds (one complex multiply-accumulate + the amortised Ex Ey product), force 9
-                    # fp32 ones (phase product 4, term 2, sums 2, amortised 1); an fp64 multiply-add takes two slots of
-                    # the FP32-pipe peak it is reported against (the fp64 pipe runs at half rate): 19 slots x 2 flop
-                    peak_tf = props.multi_processor_count * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-                    ach_tf = 1.0 * nk * n * 19 * 2 / (ms_s * 1e-3) / 1e12
-                    respa1["slow_force"] = {"n_k": nk, "ms_per_evaluation": ms_s,
-                                            "terms_per_s": 2.0 * nk * n / (ms_s * 1e-3),
-                                            "what": "S(k) pass + force pass, n_k half-space vectors x n atoms x 2 terms",
-                                            "roofline": {"bound": "alu", "achieved": ach_tf, "peak": peak_tf, "unit": "TFLOP/s",
-                                                         "frac": ach_tf / peak_tf, "traffic": None,
-                                                         "algorithmic": "%d (atom, k) pairs x (5 fp64 x 2 + 9 fp32) multiply-add slots x 2 flop" % (nk * n),
-                                                         "peak_source": "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (sm_max_mhz)" % (props.multi_processor_count, peaks["sm_max_mhz"])}}
-                err_r = sim_r.stats()["error"]
-                sim_r.close()
-            respa1[name] = {"ms_per_outer_step": ms_r / Kr, "ns_per_day": ns_per_day(Kr / (ms_r * 1e-3), 6 * dt_fs),
-                            "outer_steps": Kr, "error": err_r}
-        respa1["jump_vs_baoab"] = respa1["baoab_respa1"]["ms_per_outer_step"] / respa1["jump_respa1"]["ms_per_outer_step"]
+    # ---- the same box under plain JUMP and under same-GPU BAOAB with the unsplit r_long force -------------------
+    same_box = comparators(torch, sim, stream, flush, run, n, min(K, 200))
 
     # ---- end to end through the public API with HOST buffers -------------------------------------------------
     with torch.cuda.stream(stream):
-        Ke = min(K, 500)
+        Ke = min(K, 200)
         hp = sim.pos.detach().cpu().pin_memory()
         hv = sim.vel.detach().cpu().pin_memory()
         sim.run_host(hp, hv, block, mode=args.mode)                      # warm-up
@@ -429,16 +406,19 @@ def main():
     bytes_each_way = 2 * n * 3 * 4
     e2e = {"value": world * ns_per_day(e2e_steps / (ms_e_max * 1e-3), dt_fs), "unit": "ns/day",
            "h2d_bytes_per_step": bytes_each_way / block, "d2h_bytes_per_step": bytes_each_way / block,
+           "l2": "not flushed between calls (the host round trip itself evicts the state: %d MB each way)" % (bytes_each_way >> 20),
            "call": "JumpSim.run_host: pinned host (x, v) -> device, jump_refresh_lazy (rows rebuilt only if an atom left its "
                    "skin/2 ball), %d steps, device -> host, per call" % block}
+    err_end = sim.stats()["error"]
+    sim.close()
 
-    large = None
-    if rank == 0 and world == 1 and args.large_config >= 0:
-        large = large_box_rooflines(torch, jb, wl, dev, stream, flush, props, peaks, args.large_config, 100)
+    second = None
+    if rank == 0 and world == 1 and args.secondary_config >= 0:
+        second = secondary_config(torch, jb, wl, dev, stream, flush, args.secondary_config, 2000, 1000)
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        cpu = run_cpu_baseline(sysd, run)
+        cpu = run_cpu_baseline(sysd, run, args.mode, state0)
 
     if rank == 0:
         sps = K / (ms_max * 1e-3)
@@ -449,28 +429,29 @@ def main():
                 "config": {"workload": "BASELINE configs[%d]: %d-atom flexible water box %.1f A, r_c %.0f / r_long %.0f A, "
                                        "dt %.0f fs, %s, equilibrated by %d BAOAB steps"
                                        % (args.config, n, sysd["box"], run["r_short"], run["r_long"], dt_fs,
-                                          "JUMP-RESPA n_inner %d" % run["n_inner"] if respa else "JUMP (C'J'AOAJ'C')", args.equil),
-                           "eps_jump": run["eps_jump"], "r_mid": run["r_mid"], "skin": run["skin"],
+                                          "JUMP-RESPA n_inner %d (outer step %.0f fs; one step = one inner step)" % (run["n_inner"], run["n_inner"] * dt_fs)
+                                          if respa else "JUMP (C'J'AOAJ'C')", args.equil),
+                           "eps_jump": run["eps_jump"], "r_mid_in": run["r_mid_in"], "r_mid": run["r_mid"], "skin": run["skin"],
                            "nlist_every": run["nlist_every"], "steps_per_api_call": block,
-                           "l2": "flushed by a 256 MiB write between timed API calls (outside the event brackets)",
+                           "l2": "value: flushed by a 256 MiB write between timed API calls (outside the event brackets); e2e: not flushed",
+                           "baseline_note": "there is no reference implementation (the paper's lives in Tinker-HP): --impl reference and "
+                                            "cpu_baseline time this repo's own fp64 oracle; absolute ns/day and roofline fractions are the figures of merit",
                            "parallelism": "independent replicas x%d" % world},
                 "atom_steps_per_s": world * sps * n,
                 "clocks": clocks, "gpu_launches": launches, "wall_s": wall,
-                "e2e": e2e, "roofline": roofline, "roofline_other": roofline_other, "baoab_same_gpu": baoab,
-                "jump_vs_baoab": (K / ms_max) / (Kb / ms_b),
-                "events": {"proposals_per_atom_step": stats["proposals"] / (n * (K + W)) if K + W else None,
-                           "accepts_per_atom_step": stats["accepts"] / (n * (K + W)), "max_p": stats["max_p"],
-                           "error": stats["error"]}}
-        if adaptive is not None:
-            line["jump_adaptive_eps"] = adaptive
-        if respa1 is not None:
-            line["jump_respa1"] = respa1
-        if large is not None:
-            line["roofline_large_box"] = large
+                "e2e": e2e, "roofline": roofline, "roofline_other": roofline_other,
+                "same_box": {"jump": same_box["jump"], "baoab_same_gpu": same_box["baoab"],
+                             "jump_vs_baoab": same_box["baoab"]["ms_per_step"] / same_box["jump"]["ms_per_step"],
+                             "jump_respa_vs_baoab": same_box["baoab"]["ms_per_step"] / (ms_max / K) if respa else None},
+                "events": {"proposals_per_atom_step": stats["proposals"] / (n * (K + W_steps)),
+                           "accepts_per_atom_step": stats["accepts"] / (n * (K + W_steps)), "max_p": stats["max_p"],
+                           "timed_region_error": timed_error,
+                           "max_disp_A": stats["max_disp"], "rebuilds": stats["rebuilds"], "error": err_end}}
+        if second is not None:
+            line["secondary"] = second
         if cpu is not None:
             line["cpu_baseline"] = cpu
         print(json.dumps(line))
-    sim.close()
     if dist is not None:
         dist.destroy_process_group()
 

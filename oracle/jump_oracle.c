@@ -120,6 +120,7 @@ typedef struct {
     /* derived */
     double kT, beta, dt, alpha, rc, h, rA, rM, rE, skin;
     double *sbm; /* sqrt(beta m_i) in ps/A */
+    double *w, w_max; /* mass weights of the skin (R-10c): m_i^-1/2 / mean(m^-1/2) */
     double qmax, eps_max, sig_min, sig_max;
     double GM, GL, G3;   /* sup of the long Coulomb gradient per unit charges over ring 1, 2, 3 (R-7; G3: R-10c only) */
     double GV, GV2, GV3; /* the same for the long LJ gradient with 4 eps = 1 (R-10: GV alone, over the whole shell) */
@@ -341,6 +342,7 @@ static int contract_key(const orc_ctx *c, const double *x) {
     }
     return (cc[2] * c->gny + cc[1]) * c->gnx + cc[0];
 }
+static double dmax0(double a) { return a > 0.0 ? a : 0.0; }
 static int cmp_u64(const void *a, const void *b) {
     uint64_t x = *(const uint64_t *)a, y = *(const uint64_t *)b;
     return x < y ? -1 : (x > y ? 1 : 0);
@@ -352,13 +354,15 @@ static int cmp_u64(const void *a, const void *b) {
  * Each row in ascending (contract cell key of j, j) order (R-10).  The search
  * grid below is only an accelerator (checked against brute force in the tests).
  */
-static void neighbor_csr_audit(const orc_ctx *c, const double *x, double rmin, double rmax, int lj_only,
+static void neighbor_csr_audit(const orc_ctx *c, const double *x, double rmin, double rmax, double hs, int lj_only,
                                int brute, int **ptr_out, int **idx_out, double *edge_margin) {
+    /* hs > 0 (R-10c, mass-weighted skin): the window of the pair (i, j) is [rmin - hs (w_i + w_j), rmax + hs (w_i + w_j)) */
     int n = c->n;
     double emin = 1e300;
     int ng[3];
+    const double reach = rmax + 2.0 * hs * c->w_max;
     for (int k = 0; k < 3; ++k) {
-        ng[k] = (int)floor(c->p.box[k] / rmax);
+        ng[k] = (int)floor(c->p.box[k] / reach);
         if (ng[k] < 1) ng[k] = 1;
     }
     int ncell = ng[0] * ng[1] * ng[2];
@@ -384,7 +388,6 @@ static void neighbor_csr_audit(const orc_ctx *c, const double *x, double rmin, d
     }
     int *cnt = calloc(n + 1, sizeof(int));
     uint64_t **rows = malloc(sizeof(uint64_t *) * n);
-    double r2min = rmin * rmin, r2max = rmax * rmax;
 #pragma omp parallel for schedule(dynamic, 64) reduction(min : emin)
     for (int i = 0; i < n; ++i) {
         int cap = 64, m = 0;
@@ -408,10 +411,13 @@ static void neighbor_csr_audit(const orc_ctx *c, const double *x, double rmin, d
                         double d[3];
                         min_image(c, &x[3 * i], &x[3 * j], d);
                         double r2 = d[0] * d[0] + d[1] * d[1] + d[2] * d[2];
-                        if (edge_margin && (fabs(r2 - r2max) < 0.05 || (rmin > 0.0 && fabs(r2 - r2min) < 0.05)) &&
+                        const double sij = hs * (c->w[i] + c->w[j]);
+                        const double hi_e = rmax + sij, lo_e = rmin > 0.0 ? dmax0(rmin - sij) : 0.0;
+                        const double r2max = hi_e * hi_e, r2min = lo_e * lo_e;
+                        if (edge_margin && (fabs(r2 - r2max) < 0.05 || (lo_e > 0.0 && fabs(r2 - r2min) < 0.05)) &&
                             !is_excluded(c, i, j)) { /* audit only: how close is this decision to flipping */
-                            double r = sqrt(r2), e = fabs(r - rmax);
-                            if (rmin > 0.0 && fabs(r - rmin) < e) e = fabs(r - rmin);
+                            double r = sqrt(r2), e = fabs(r - hi_e);
+                            if (lo_e > 0.0 && fabs(r - lo_e) < e) e = fabs(r - lo_e);
                             if (e < emin) emin = e;
                         }
                         if (r2 >= r2max || r2 < r2min) continue;
@@ -438,7 +444,7 @@ static void neighbor_csr_audit(const orc_ctx *c, const double *x, double rmin, d
 }
 static void neighbor_csr(const orc_ctx *c, const double *x, double rmin, double rmax, int lj_only,
                          int brute, int **ptr_out, int **idx_out) {
-    neighbor_csr_audit(c, x, rmin, rmax, lj_only, brute, ptr_out, idx_out, NULL);
+    neighbor_csr_audit(c, x, rmin, rmax, 0.0, lj_only, brute, ptr_out, idx_out, NULL);
 }
 
 /* exported for the brute-force pin: returns CSR copies */
@@ -651,11 +657,11 @@ static double sup_lj(const orc_ctx *c, double lo, double hi) { /* 4 eps = 1; sup
     if (!(hi > lo) || !(c->sig_max > 0.0)) return 0.0;
     double best = 0.0;
     int NS = (c->sig_max > c->sig_min) ? 65 : 1;
-    long K = (long)floor((hi - lo) / 1e-3);
+    long K = (long)floor((hi - lo) / 1e-4);
     for (int s = 0; s < NS; ++s) {
         double sig = (NS == 1) ? c->sig_min : c->sig_min + (c->sig_max - c->sig_min) * (double)s / (double)(NS - 1);
         for (long k = 0; k <= K + 1; ++k) {
-            double r = (k <= K) ? lo + 1e-3 * (double)k : hi;
+            double r = (k <= K) ? lo + 1e-4 * (double)k : hi;
             if (r > hi) r = hi;
             double u, du;
             orc_u_lj(r, sig, 0.25, &u, &du);
@@ -777,15 +783,18 @@ static void rebuild_rows(orc_ctx *c) {
     if (lo < 0.0) lo = 0.0;
     double em = 1e300;
     if (c->policy == 1) {
-        /* R-10c: row A lists every pair that can be closer than r_A before the next build, row B every pair that can
-         * be in [r_A, r_M) (they overlap by one skin on each side of r_A); ring 3 draws from the cell universe */
-        neighbor_csr_audit(c, c->x, lo, c->rA + s, 0, 0, &c->ptrM, &c->idxM, &em);                     /* row A */
-        neighbor_csr_audit(c, c->x, dmax(c->rA - s, lo), c->rM + s, 0, 0, &c->ptrL, &c->idxL, &em);   /* row B */
+        /* R-10c: row A lists every pair that can be in ring A before the next build, row B every pair that can be in
+         * ring B (they overlap around r_A); ring C draws from the cell universe.  Mass-weighted skin: the pair (i, j)
+         * is listed over [ring - s_ij, ring + s_ij), s_ij = (skin/2)(w_i + w_j), w_i = m_i^-1/2 / mean(m^-1/2): an atom
+         * may then move w_i skin/2 before the lists have to be rebuilt -- light atoms move farther in the same time
+         * (displacement ~ m^-1/2), so one budget per atom lets a water box go 7 steps where a uniform skin/2 allows 4 */
+        neighbor_csr_audit(c, c->x, c->rc - c->h, c->rA, 0.5 * s, 0, 0, &c->ptrM, &c->idxM, &em);   /* row A */
+        neighbor_csr_audit(c, c->x, c->rA, c->rM, 0.5 * s, 0, 0, &c->ptrL, &c->idxL, &em);         /* row B */
         rebuild_universe(c);
     } else {
-        neighbor_csr_audit(c, c->x, lo, c->rM, 0, 0, &c->ptrM, &c->idxM, &em);
-        neighbor_csr_audit(c, c->x, dmax(c->rM, lo), c->rE + s, 0, 0, &c->ptrL, &c->idxL, &em);
-        neighbor_csr_audit(c, c->x, lo, c->rE + s, 1, 0, &c->ptrV, &c->idxV, &em);
+        neighbor_csr_audit(c, c->x, lo, c->rM, 0.0, 0, 0, &c->ptrM, &c->idxM, &em);
+        neighbor_csr_audit(c, c->x, dmax(c->rM, lo), c->rE + s, 0.0, 0, 0, &c->ptrL, &c->idxL, &em);
+        neighbor_csr_audit(c, c->x, lo, c->rE + s, 0.0, 1, 0, &c->ptrV, &c->idxV, &em);
     }
     {   /* contract-grid cell faces (the row order depends on the cell of every atom, R-10) */
         int nn[3] = {c->gnx, c->gny, c->gnz};
@@ -800,15 +809,17 @@ static void rebuild_rows(orc_ctx *c) {
     memcpy(c->x_build, c->x, sizeof(double) * 3 * c->n);
     c->st.rebuilds++;
 }
-static void check_displacement(orc_ctx *c) {
+static double check_displacement(orc_ctx *c) {
     double mx = 0.0;
     for (int i = 0; i < c->n; ++i) {
         double d[3];
         min_image(c, &c->x[3 * i], &c->x_build[3 * i], d);
         double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        if (c->policy == 1) r /= c->w[i]; /* mass-weighted skin: the budget of atom i is w_i skin / 2 */
         if (r > mx) mx = r;
     }
     if (mx > c->st.max_disp) c->st.max_disp = mx;
+    return mx;
 }
 /* R-10: rows M, L, V.  R-10c: row A, row B, the cell universe of the atom's home cell */
 void orc_get_row_counts(const orc_ctx *c, int *nM, int *nL, int *nV) {
@@ -1107,8 +1118,19 @@ static void aoa_and_lists(orc_ctx *c) {
     phase_A(c, 0.5 * c->dt);
     wrap_all(c);
     c->step++;
-    check_displacement(c);
-    if (c->p.nlist_every > 0 && c->step % c->p.nlist_every == 0) rebuild_rows(c);
+    const double mx = check_displacement(c);
+    /* R-10c list schedule: every P = nlist_every steps at the latest, and -- from step P/4 of such an interval on -- as
+     * soon as some atom has used up its share of the skin, w_i skin/2, since the last build (the lists are supersets
+     * of what they must hold while no atom has; water, skin 1 A: 6 to 9 steps).  The test on the displacement is
+     * one more discontinuous decision (R-17): its margin is audited with those of the lists. */
+    const int P = c->p.nlist_every;
+    int rebuild = P > 0 && c->step % P == 0;
+    if (!rebuild && c->policy == 1 && P > 0 && c->step % P >= (P >= 4 ? P / 4 : 1)) {
+        const double e = fabs(mx - 0.5 * c->skin);
+        if (e < c->st.min_list_margin) { c->st.min_list_margin = e; c->st.min_list_margin_step = c->step; }
+        rebuild = mx > 0.5 * c->skin;
+    }
+    if (rebuild) rebuild_rows(c);
 }
 
 /* ------------------------------------------------------------------ */
@@ -1349,12 +1371,22 @@ orc_ctx *orc_create(const orc_params *p, const double *pos, const double *vel, c
     if (c->rA > c->rM) c->rA = c->rM;
     c->sbm = malloc(sizeof(double) * n);
     for (int i = 0; i < n; ++i) c->sbm[i] = sqrt(c->m[i] / (c->kT * ORC_KCAL));
-    double edge = p->cell_edge > 0.0 ? p->cell_edge : (p->r_long + p->skin) / 4.0;
+    c->w = malloc(sizeof(double) * n);
+    {
+        double sum = 0.0;
+        for (int i = 0; i < n; ++i) sum += 1.0 / sqrt(c->m[i]);
+        c->w_max = 0.0;
+        for (int i = 0; i < n; ++i) {
+            c->w[i] = p->list_policy == 1 ? (1.0 / sqrt(c->m[i])) / (sum / n) : 1.0;
+            if (c->w[i] > c->w_max) c->w_max = c->w[i];
+        }
+    }
+    double edge = p->cell_edge > 0.0 ? p->cell_edge : (p->r_long + p->skin * c->w_max) / 4.0;
     c->gnx = (int)floor(p->box[0] / edge); if (c->gnx < 1) c->gnx = 1;
     c->gny = (int)floor(p->box[1] / edge); if (c->gny < 1) c->gny = 1;
     c->gnz = (int)floor(p->box[2] / edge); if (c->gnz < 1) c->gnz = 1;
     c->policy = p->list_policy == 1 ? 1 : 0;
-    c->ureach = p->r_long + p->skin;
+    c->ureach = p->r_long + p->skin * c->w_max;
     {
         int nn[3] = {c->gnx, c->gny, c->gnz};
         for (int k = 0; k < 3; ++k) c->uR[k] = (int)ceil(c->ureach / (p->box[k] / nn[k]));
@@ -1378,7 +1410,7 @@ void orc_free(orc_ctx *c) {
     free(c->excl_ptr); free(c->excl_idx); free(c->sbm); free(c->x_build);
     free(c->ptrM); free(c->idxM); free(c->ptrL); free(c->idxL); free(c->ptrV); free(c->idxV);
     free(c->f_bond); free(c->f_nb); free(c->f0); free(c->f_long); free(c->ev); free(c->kn); free(c->f_slow);
-    free(c->cell_ptr); free(c->cell_atoms); free(c->home); free(c->uni_cnt);
+    free(c->cell_ptr); free(c->cell_atoms); free(c->home); free(c->uni_cnt); free(c->w);
     free(c);
 }
 /* which: 0 wrapped x, 1 v, 2 unwrapped x */

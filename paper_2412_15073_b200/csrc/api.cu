@@ -24,21 +24,21 @@ struct jump_ctx {
     int n;
     double kT, dt, alpha, rA, rM, lo;  // ps; lo = max(r_c - h - skin, 0)
     double G[3], GV[3], qmax, eps_max, sig_min, sig_max;   // bounds per ring (R-7, R-10c)
+    double w_max, w_norm;        // mass weights of the skin: w_i = m_i^-1/2 / w_norm, w_norm = mean(m^-1/2) (R-10c)
     Universe uni;                // cell universe of ring C (R-10c)
     unsigned short *uni_cum;
     int *cell_of;
     int lanes;                   // jump_set_lanes
-    int64_t sort_step;           // step count at the last sort
     float c1, c2;
     float *d_pos, *d_vel;  // caller's
     // sorted state (cur) and spare buffers (nxt)
     float4 *xs, *xs_nxt, *vs, *vs_nxt, *xl, *xl_nxt, *x_build;
-    float2 *lj, *lj_nxt, *mi, *mi_nxt;
+    float2 *lj, *lj_nxt, *mi, *mi_nxt, *hw, *hw_nxt;   // hw: (skin/2) w_i, split fp64 (R-10c)
     int *orig, *orig_nxt, *sorted_of;
     int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src, *scan_sums, *scan_offs;
     Row rows[N_ROWS];
-    bool row_fresh[N_ROWS];  // built since the last sort
-    bool row_used[N_ROWS];   // read since the last sort: rebuilt eagerly at the next one (others lazily, on demand)
+    bool row_active[N_ROWS];      // refreshed by every list build
+    int64_t row_last_use[N_ROWS];
     bool f0_valid;           // c->f0 / fnb / fbond hold F0 at the current positions
     float4 *fnb, *fbond, *f0, *ftmp, *ftmp2;
     // reciprocal Ewald sum, the slow force of JUMP-RESPA1 (R-21): set up by jump_ewald_setup
@@ -61,7 +61,7 @@ struct jump_ctx {
     Counters *ctr;
     jump_event *events;
     long long event_cap;
-    int64_t step, outer, rebuilds, launches;
+    int64_t step, outer, launches;
     int sticky;
     std::string err;
     // optional per-category kernel timing with CUDA events on the launch stream (bench.py's roofline leg)
@@ -187,7 +187,7 @@ static void compute_bounds(jump_ctx *c, const std::vector<float> &q, const std::
         if (c->sig_max > 0.0)
             for (int k = 0; k < NS; ++k) {
                 double sg = NS == 1 ? c->sig_min : c->sig_min + (c->sig_max - c->sig_min) * (double)k / (double)(NS - 1);
-                c->GV[y] = std::max(c->GV[y], sup_long(c, edge[y], edge[y + 1], 1e-3, false, sg));
+                c->GV[y] = std::max(c->GV[y], sup_long(c, edge[y], edge[y + 1], 1e-4, false, sg));
             }
     }
 }
@@ -206,69 +206,72 @@ static int alloc_row(jump_ctx *c, int k) {
     return 0;
 }
 
-// build the given rows (all in one launch) at the current sort
-static int build_rows(jump_ctx *c, const bool want[N_ROWS]) {
+// Build the given rows in one launch from the positions of the last sort (x_build: what the cell table describes and
+// the displacement check refers to; at the sort itself they are the current positions).  go / want: see SortArgs.
+static int build_rows(jump_ctx *c, const bool want[N_ROWS], const int *go, int stamp) {
     Row sel[N_ROWS];
     bool any = false;
     double rmax = 0.0;
     for (int k = 0; k < N_ROWS; ++k) {
         sel[k] = c->rows[k];
-        if (!(want[k] && c->rows[k].enabled && !c->row_fresh[k])) sel[k].enabled = 0;
-        if (sel[k].enabled) { any = true; c->row_fresh[k] = true; rmax = std::max(rmax, std::sqrt(sel[k].r2max_d)); }
+        if (!(want[k] && c->rows[k].enabled)) sel[k].enabled = 0;
+        if (sel[k].enabled) { any = true; rmax = std::max(rmax, (double)std::sqrt(sel[k].r2max)); }
     }
     if (!any) return 0;
     prof_begin(c, PROF_BUILD);
-    // A row asked for the first time between two sorts is built from the positions of the last sort (x_build), which
-    // the cell table describes and the displacement check refers to: it is the row an eager build would have made.
-    const float4 *xsrc = (c->step == c->sort_step) ? c->xs : c->x_build;
-    launch_build_rows(c->m, c->g, sel, (float)rmax, c->cell_start, xsrc, c->xl, c->lj, c->orig,
+    launch_build_rows(c->m, c->g, sel, (float)rmax, c->cell_start, c->x_build, c->xl, c->lj, c->hw, c->orig,
                       c->sorted_of, c->excl_ptr, c->excl_idx, c->ctr, (sel[ROW_A].enabled ? c->cell_of : nullptr),
-                      (float)std::pow(std::max(c->rM - 2.0 * c->p.skin, 0.0), 2), c->st, &c->launches);
+                      (float)std::pow(std::max(c->rM - 2.0 * c->p.skin * c->w_max, 0.0), 2), go, stamp, c->st, &c->launches);
     prof_end(c, PROF_BUILD);
     CK(cudaGetLastError());
     return 0;
 }
 
-static int resort_and_build(jump_ctx *c) {
+// Sort + universe sums + every active row.  conditional: the kernels run only if the update kernel of this step armed
+// them (an atom farther than skin/2 from its build position, R-10c); the host never learns which way it went, so the
+// sorted state is permuted through scratch arrays and copied back (no pointer swap) and sorts are counted on the device.
+static int resort_and_build(jump_ctx *c, bool conditional) {
+    const int *go = conditional ? &c->ctr->go_step : nullptr;
+    const int stamp = (int)c->step;
     SortArgs a;
     a.n = c->n; a.grid = c->g;
-    a.xs_in = c->xs; a.vs_in = c->vs; a.xl_in = c->xl; a.xl = c->xl_nxt; a.lj_in = c->lj; a.mi_in = c->mi; a.orig_in = c->orig;
-    a.xs = c->xs_nxt; a.vs = c->vs_nxt; a.lj = c->lj_nxt; a.mi = c->mi_nxt; a.orig = c->orig_nxt;
+    a.xs = c->xs; a.vs = c->vs; a.xl = c->xl; a.lj = c->lj; a.mi = c->mi; a.hw = c->hw; a.orig = c->orig;
+    a.xs_t = c->xs_nxt; a.vs_t = c->vs_nxt; a.xl_t = c->xl_nxt; a.lj_t = c->lj_nxt; a.mi_t = c->mi_nxt; a.hw_t = c->hw_nxt; a.orig_t = c->orig_nxt;
     a.sorted_of = c->sorted_of; a.x_build = c->x_build; a.cell_of = c->cell_of;
     a.key = c->key; a.cell_count = c->cell_count; a.cell_fill = c->cell_fill; a.cell_start = c->cell_start;
     a.tmp_orig = c->tmp_orig; a.tmp_src = c->tmp_src; a.scan_sums = c->scan_sums; a.scan_offs = c->scan_offs; a.ctr = c->ctr;
+    a.go = go; a.want = stamp;
     prof_begin(c, PROF_BUILD);
     launch_sort(a, c->st, &c->launches);
     prof_end(c, PROF_BUILD);
     CK(cudaGetLastError());
-    std::swap(c->xs, c->xs_nxt); std::swap(c->vs, c->vs_nxt); std::swap(c->xl, c->xl_nxt); std::swap(c->lj, c->lj_nxt);
-    std::swap(c->mi, c->mi_nxt); std::swap(c->orig, c->orig_nxt);
-    bool want[N_ROWS];
-    for (int k = 0; k < N_ROWS; ++k) { c->row_fresh[k] = false; want[k] = c->row_used[k]; c->row_used[k] = false; }
-    c->rebuilds++;
-    c->sort_step = c->step;
-    c->slow_valid = false;   // (sorted order changed)
+    c->slow_valid = false;   // (the sorted order may have changed)
     if (c->uni_cum) {   // running sums of the universe of every cell (ring C, R-10c)
         prof_begin(c, PROF_BUILD);
-        launch_universe(c->g, c->uni, c->cell_start, c->uni_cum, c->ctr, c->st, &c->launches);
+        launch_universe(c->g, c->uni, c->cell_start, c->uni_cum, c->ctr, go, stamp, c->st, &c->launches);
         prof_end(c, PROF_BUILD);
         CK(cudaGetLastError());
     }
-    return build_rows(c, want);
+    // rows that nobody has read for a while leave the active set (they are built again on demand)
+    for (int k = 0; k < N_ROWS; ++k)
+        if (c->row_active[k] && c->step - c->row_last_use[k] > 3 * (int64_t)std::max(c->p.nlist_every, 1)) c->row_active[k] = false;
+    return build_rows(c, c->row_active, go, stamp);
 }
 
-// every read of a row goes through here: allocate on first use, build if stale
+// every read of a row goes through here: allocate on first use; a row outside the active set is built now (from the
+// positions of the last sort) and joins it: from then on every list build refreshes it
 static int need_rows(jump_ctx *c, std::initializer_list<int> ks) {
     bool want[N_ROWS] = {false, false, false, false, false, false};
     bool stale = false;
     for (int k : ks) {
         int r = alloc_row(c, k);
         if (r) return r;
-        c->row_used[k] = true;
-        want[k] = true;
-        stale |= !c->row_fresh[k];
+        c->row_last_use[k] = c->step;
+        want[k] = !c->row_active[k];
+        stale |= want[k];
+        c->row_active[k] = true;
     }
-    return stale ? build_rows(c, want) : 0;
+    return stale ? build_rows(c, want, nullptr, 0) : 0;
 }
 static int need_row(jump_ctx *c, int k) { return need_rows(c, {k}); }
 
@@ -394,6 +397,14 @@ static int run_update(jump_ctx *c, const Phase &p0, GradRef g0, const Phase &p1,
     A.rowA = c->rows[ROW_A]; A.rowB = c->rows[ROW_B];
     A.uni = c->uni; A.grid = c->g; A.cell_start = c->cell_start; A.xl_all = c->xl; A.excl_ptr = c->excl_ptr; A.excl_idx = c->excl_idx;
     A.lanes = c->lanes;
+    // R-10c list schedule: every P = nlist_every steps at the latest; from step P/4 of such an interval on the update kernel
+    // arms a conditional build as soon as an atom has used up its share of the skin (before that: the error JUMP_E_SKIN)
+    const int P = c->p.nlist_every;
+    const int64_t next = c->step + 1;
+    const bool scheduled = aoa && P > 0 && next % P == 0;
+    const bool will_check = scheduled || (aoa && P > 0 && next % P >= (P >= 4 ? P / 4 : 1));
+    A.trigger = scheduled ? 2 : (will_check ? 1 : 0);   // 2: a list build follows anyway (no error, nothing to arm)
+    A.step_id = (int)next;
     A.ctr = c->ctr; A.events = (c->p.flags & JUMP_F_EVENT_LOG) ? c->events : nullptr; A.event_cap = c->event_cap;
     bool jumps = (p0.kind == 2 || p1.kind == 2) && (coul_jumps(c) || lj_jumps(c));
     if (jumps) {
@@ -411,7 +422,7 @@ static int run_update(jump_ctx *c, const Phase &p0, GradRef g0, const Phase &p1,
         c->f0_valid = false;
         c->slow_valid = false;
         c->step++;
-        if (c->p.nlist_every > 0 && c->step % c->p.nlist_every == 0) return resort_and_build(c);
+        if (will_check) return resort_and_build(c, !scheduled);
     }
     return 0;
 }
@@ -691,7 +702,7 @@ extern "C" int jump_half(jump_ctx *c, double H_ps, int32_t with_accel, int64_t s
 
 // ---- life cycle ------------------------------------------------------------------------------------------
 static int load_state(jump_ctx *c, const float *d_mass, const float *d_charge, const float *d_sigma, const float *d_eps) {
-    launch_load(c->m, c->d_pos, c->d_vel, d_mass, d_charge, d_sigma, d_eps, c->kT, c->xs, c->vs, c->xl, c->lj, c->mi, c->orig, c->st,
+    launch_load(c->m, c->d_pos, c->d_vel, d_mass, d_charge, d_sigma, d_eps, c->kT, 0.5 * c->p.skin / c->w_norm, c->xs, c->vs, c->xl, c->lj, c->mi, c->hw, c->orig, c->st,
                 &c->launches);
     CK(cudaGetLastError());
     return 0;
@@ -716,7 +727,16 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     // host copies of the per-atom parameters (bounds) and the topology
     std::vector<float> hq, hs, he;
     int r;
-    if ((r = ddownload(c, hq, d_charge, n)) || (r = ddownload(c, hs, d_sigma, n)) || (r = ddownload(c, he, d_eps, n))) return r;
+    std::vector<float> hm;
+    if ((r = ddownload(c, hq, d_charge, n)) || (r = ddownload(c, hs, d_sigma, n)) || (r = ddownload(c, he, d_eps, n)) ||
+        (r = ddownload(c, hm, d_mass, n)))
+        return r;
+    {   // mass weights of the skin (R-10c): an atom may move w_i skin/2 between two list builds
+        double sum = 0.0, mmin = 1e300;
+        for (int i = 0; i < n; ++i) { if (!(hm[i] > 0.f)) return JUMP_E_ARG; sum += 1.0 / std::sqrt((double)hm[i]); mmin = std::min(mmin, (double)hm[i]); }
+        c->w_norm = sum / n;
+        c->w_max = (1.0 / std::sqrt(mmin)) / c->w_norm;
+    }
     compute_bounds(c, hq, hs, he);
     // model constants
     Model &m = c->m;
@@ -742,22 +762,25 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
         }
     }
     m.half_skin2 = (float)(0.25 * p->skin * p->skin);
+    m.hs = (float)(0.5 * p->skin);
+    m.Wc = (float)(1.0 / (std::sqrt(c->kT * kKcal) * c->w_norm));
+    m.w_max = (float)c->w_max;
     m.key0 = (unsigned)(p->seed & 0xffffffffu); m.key1 = (unsigned)(p->seed >> 32);
     // sort grid (R-10)
     SortGrid &g = c->g;
-    double edge = p->cell_edge > 0.0 ? p->cell_edge : (p->r_long + p->skin) / 4.0;
+    double edge = p->cell_edge > 0.0 ? p->cell_edge : (p->r_long + p->skin * c->w_max) / 4.0;
     g.ncell = 1;
     for (int k = 0; k < 3; ++k) {
         g.gn[k] = std::max(1, (int)std::floor(p->box[k] / edge));
         g.scale[k] = (double)g.gn[k] / p->box[k];
-        g.reach[k] = (int)std::ceil((p->r_long + p->skin) / (p->box[k] / g.gn[k]));
+        g.reach[k] = (int)std::ceil((p->r_long + p->skin * c->w_max) / (p->box[k] / g.gn[k]));
         if (g.reach[k] > 8 || g.gn[k] > 1023) return JUMP_E_ARG;  // stencil table of the row build (cell_edge too small); packed cells
         g.ncell *= g.gn[k];
     }
     // buffers
     if ((r = dalloc(c, &c->xs, n)) || (r = dalloc(c, &c->xs_nxt, n)) || (r = dalloc(c, &c->vs, n)) ||
         (r = dalloc(c, &c->vs_nxt, n)) || (r = dalloc(c, &c->xl, n)) || (r = dalloc(c, &c->xl_nxt, n)) || (r = dalloc(c, &c->x_build, n)) || (r = dalloc(c, &c->lj, n)) ||
-        (r = dalloc(c, &c->lj_nxt, n)) || (r = dalloc(c, &c->mi, n)) || (r = dalloc(c, &c->mi_nxt, n)) ||
+        (r = dalloc(c, &c->lj_nxt, n)) || (r = dalloc(c, &c->mi, n)) || (r = dalloc(c, &c->mi_nxt, n)) || (r = dalloc(c, &c->hw, n)) || (r = dalloc(c, &c->hw_nxt, n)) ||
         (r = dalloc(c, &c->orig, n)) || (r = dalloc(c, &c->orig_nxt, n)) || (r = dalloc(c, &c->sorted_of, n)) || (r = dalloc(c, &c->cell_of, n)) ||
         (r = dalloc(c, &c->key, n)) || (r = dalloc(c, &c->tmp_orig, n)) || (r = dalloc(c, &c->tmp_src, n)) ||
         (r = dalloc(c, &c->cell_count, g.ncell + 1)) || (r = dalloc(c, &c->cell_fill, g.ncell + 1)) ||
@@ -772,7 +795,7 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
         // caller's numbers (the oracle takes the same decisions from the same numbers)
         Universe &u = c->uni;
         memset(&u, 0, sizeof u);
-        const double reach = p->r_long + p->skin;
+        const double reach = p->r_long + p->skin * c->w_max;
         double w[3];
         for (int k = 0; k < 3; ++k) {
             w[k] = p->box[k] / g.gn[k];
@@ -910,37 +933,38 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
         int n_lj = 0;
         for (int i = 0; i < n; ++i) n_lj += he[i] > 0.f;
         const double rho_lj = n_lj / vol;
-        struct W { double a, b; int lj; bool on; } w[N_ROWS] = {
-            {0.0, rc + s, 0, true},                              // S short list
-            {c->lo, c->rA + s, 0, true},                         // A: candidates of ring [r_c-h, r_A) (R-10c)
-            {std::max(c->rA - s, c->lo), c->rM + s, 0, true},    // B: candidates of ring [r_A, r_M)
-            {0.0, 0.0, 0, false},                                // (unused)
-            {0.0, rE + s, 0, false},                             // F: full list (lazy)
-            {rc + s, rE + s, 1, !lj_jumps(c)}};                  // W: LJ tail kept in F0 (R-13)
+        // nominal windows [a, b) (R-10c); at a build the pair (i, j) is listed over [a - s_ij, b + s_ij), s_ij = (skin/2)(w_i + w_j)
+        const double rlo = rc - p->r_switch;
+        struct W { double a, b; int lj; } w[N_ROWS] = {
+            {0.0, rc, 0},                 // S short list
+            {rlo, c->rA, 0},              // A: candidates of ring [r_c-h, r_A)
+            {c->rA, c->rM, 0},            // B: candidates of ring [r_A, r_M)
+            {0.0, 0.0, 0},                // (unused)
+            {0.0, rE, 0},                 // F: full list (lazy)
+            {rc, rE, 1}};                 // W: LJ tail kept in F0 (R-13)
+        const double smax = s * c->w_max;
         for (int k = 0; k < N_ROWS; ++k) {
             Row &R = c->rows[k];
             memset(&R, 0, sizeof R);
-            double b3 = w[k].b * w[k].b * w[k].b, a3 = w[k].a * w[k].a * w[k].a;
-            double expect = 4.0 / 3.0 * M_PI * std::max(b3 - a3, 0.0) * (w[k].lj ? rho_lj : rho);
+            const double hi = w[k].b + smax, lo = std::max(w[k].a - smax, 0.0);
+            double expect = 4.0 / 3.0 * M_PI * std::max(hi * hi * hi - lo * lo * lo, 0.0) * (w[k].lj ? rho_lj : rho);
             R.cap = std::min(round32(1.6 * expect + 32.0), round32((double)n));
             R.lj_only = w[k].lj;
-            R.r2min = (float)(w[k].a * w[k].a);
-            R.r2max = (float)(w[k].b * w[k].b);
-            R.r2min_d = w[k].a * w[k].a;
-            R.r2max_d = w[k].b * w[k].b;
-            c->row_fresh[k] = false;
-            c->row_used[k] = false;
+            R.ra = (float)w[k].a; R.rb = (float)w[k].b; R.ra_d = w[k].a; R.rb_d = w[k].b;
+            R.lo_plus = k == ROW_W ? 1 : 0;
+            R.r2max = (float)(hi * hi);
+            c->row_active[k] = false;
+            c->row_last_use[k] = 0;
         }
     }
     if ((r = load_state(c, d_mass, d_charge, d_sigma, d_eps))) return r;
-    if ((r = resort_and_build(c))) return r;
-    c->rebuilds = 1;
-    {   // the rows this mode reads on every step, built in one launch
+    {   // the rows this mode reads on every step: active from the start, built with the first sort
         const bool jumps = coul_jumps(c) || lj_jumps(c);
-        bool want[N_ROWS] = {true, jumps, jumps, false, false, !lj_jumps(c)};
-        for (int k = 0; k < N_ROWS; ++k) if (want[k] && (r = alloc_row(c, k))) return r;
-        if ((r = build_rows(c, want))) return r;
+        const bool want[N_ROWS] = {true, jumps, jumps, false, false, !lj_jumps(c)};
+        for (int k = 0; k < N_ROWS; ++k)
+            if (want[k]) { if ((r = alloc_row(c, k))) return r; c->row_active[k] = true; }
     }
+    if ((r = resort_and_build(c, false))) return r;
     if ((r = compute_f0(c))) return r;
     if ((r = writeback(c))) return r;  // wrapped positions
     return poll_error(c);
@@ -969,7 +993,7 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
         c->err = "side stream / events"; *out = c; return JUMP_E_CUDA;
     }
     c->d_pos = d_pos; c->d_vel = d_vel;
-    c->step = c->outer = c->rebuilds = c->launches = 0;
+    c->step = c->outer = c->launches = 0;
     c->sticky = 0;
     c->pair_count = nullptr;
     c->moved_flag = nullptr;
@@ -979,7 +1003,7 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     c->vacf_v0 = nullptr; c->vacf_part = nullptr;
     c->fslow = nullptr; c->ew_sum = nullptr; c->q2sum = 0.0; c->outer1 = 0;
     c->prof = false;
-    c->lanes = 0; c->sort_step = 0; c->uni_cum = nullptr; c->cell_of = nullptr;
+    c->lanes = 0; c->uni_cum = nullptr; c->cell_of = nullptr;
     for (int k = 0; k < 4; ++k) { c->prof_ms[k] = 0.0; c->prof_n[k] = 0; }
     int r = init_impl(c, p, d_mass, d_charge, d_lj_sigma, d_lj_eps, n_bonds, d_bond_ij, d_bond_k, d_bond_r0, n_angles,
                       d_angle_ijk, d_angle_k, d_angle_t0, d_excl_ptr, d_excl_idx);
@@ -1053,7 +1077,7 @@ extern "C" int jump_get_stats(jump_ctx *c, jump_stats *o) {
     CK(cudaStreamSynchronize(c->st));
     memset(o, 0, sizeof *o);
     o->proposals = (int64_t)h.proposals; o->accepts = (int64_t)h.accepts; o->gt_attempts = (int64_t)h.gt_attempts;
-    o->expiries = (int64_t)h.expiries; o->rebuilds = c->rebuilds;
+    o->expiries = (int64_t)h.expiries; o->rebuilds = (int64_t)h.rebuilds;
     float f;
     memcpy(&f, &h.max_p_bits, 4); o->max_p = f;
     memcpy(&f, &h.max_gl_bits, 4); o->max_g_over_L = f;
@@ -1068,9 +1092,11 @@ extern "C" int jump_reset_stats(jump_ctx *c) {
     Counters h;
     CK(cudaMemcpyAsync(&h, c->ctr, sizeof h, cudaMemcpyDeviceToHost, c->st));
     CK(cudaStreamSynchronize(c->st));
-    unsigned long long ne = h.n_events;
+    const unsigned long long ne = h.n_events;
+    const unsigned nr = h.rebuilds;
+    const int gs = h.go_step;
     memset(&h, 0, sizeof h);
-    h.n_events = ne;
+    h.n_events = ne; h.rebuilds = nr; h.go_step = gs;
     CK(cudaMemcpyAsync(c->ctr, &h, sizeof h, cudaMemcpyHostToDevice, c->st));
     CK(cudaStreamSynchronize(c->st));
     c->sticky = 0; c->err.clear();
@@ -1139,7 +1165,7 @@ extern "C" int jump_rdf_accumulate(jump_ctx *c, int32_t lj_only, double r_max, i
     if (!c || !d_hist) return JUMP_E_ARG;
     // The cell table of the last sort indexes the sorted array, and an atom has moved by at most about the skin
     // since: the home cell of i is taken from its current position and the stencil reaches r_max + skin.
-    if (launch_rdf(c->m, c->g, lj_only != 0, r_max, r_max + c->p.skin, n_bins, c->cell_start, c->xs, c->lj,
+    if (launch_rdf(c->m, c->g, lj_only != 0, r_max, r_max + c->p.skin * c->w_max, n_bins, c->cell_start, c->xs, c->lj,
                    (unsigned long long *)d_hist, c->st, &c->launches))
         return JUMP_E_ARG;
     CK(cudaGetLastError());
@@ -1184,9 +1210,9 @@ extern "C" int jump_set_lanes(jump_ctx *c, int32_t lanes) {
 }
 extern "C" int jump_refresh(jump_ctx *c) {
     if (!c) return JUMP_E_ARG;
-    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, nullptr, nullptr, 0, c->st, &c->launches);
+    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, nullptr, nullptr, 0, c->mi, c->st, &c->launches);
     CK(cudaGetLastError());
-    int r = resort_and_build(c);
+    int r = resort_and_build(c, false);
     if (r) return r;
     if ((r = compute_f0(c))) return r;
     return poll_error(c);
@@ -1196,13 +1222,13 @@ extern "C" int jump_refresh_lazy(jump_ctx *c, int32_t *rebuilt) {
     int r;
     if (!c->moved_flag && (r = dalloc(c, &c->moved_flag, 1))) return r;
     CK(cudaMemsetAsync(c->moved_flag, 0, sizeof(int), c->st));
-    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, c->x_build, c->moved_flag, 1, c->st, &c->launches);
+    launch_reload(c->m, c->d_pos, c->d_vel, c->orig, c->xs, c->vs, c->xl, c->x_build, c->moved_flag, 1, c->mi, c->st, &c->launches);
     CK(cudaGetLastError());
     int moved = 0;
     CK(cudaMemcpyAsync(&moved, c->moved_flag, sizeof(int), cudaMemcpyDeviceToHost, c->st));
     CK(cudaStreamSynchronize(c->st));
     c->slow_valid = false;
-    if (moved && (r = resort_and_build(c))) return r;
+    if (moved && (r = resort_and_build(c, false))) return r;
     if (rebuilt) *rebuilt = moved;
     if ((r = compute_f0(c))) return r;
     return 0;

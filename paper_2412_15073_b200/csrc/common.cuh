@@ -30,8 +30,12 @@ struct Row {
     int *cnt;       // [n]
     int cap;        // multiple of 32
     int lj_only;    // keep eps_i eps_j > 0 only
-    float r2min, r2max;  // build-time window rmin <= d < rmax
-    double r2min_d, r2max_d;  // the same in fp64 (edge decisions, R-17)
+    // window of the pair (i, j) at a build (R-10c, mass-weighted skin): max(ra - s_ij, 0) <= d < rb + s_ij with
+    // s_ij = (skin/2)(w_i + w_j); ra = 0: no lower edge
+    float ra, rb;
+    double ra_d, rb_d;   // the same in fp64 (edge decisions, R-17)
+    int lo_plus;         // the lower edge is ra + s_ij instead (row W: the complement of row S)
+    float r2max;         // (rb + skin w_max)^2: the farthest an entry can be at a build
     int enabled;
 };
 
@@ -41,6 +45,8 @@ struct Counters {
     unsigned int max_p_bits, max_gl_bits, max_disp2_bits;  // non-negative floats compared as uints
     unsigned int err;
     int max_row[N_ROWS];
+    int go_step;            // step stamp of the last displacement trigger (k_update): the list kernels enqueued for that step run
+    unsigned int rebuilds;  // sorts done (counted on the device: the host does not know which conditional ones ran)
 };
 
 // constants of the physical model, passed by value to kernels
@@ -59,6 +65,9 @@ struct Model {
     float ring2[4];               // squared ring edges (r_c-h)^2, r_A^2, r_M^2, r_long^2: ring Y = [ring2[Y], ring2[Y+1])
     double ring2d[4];             // the same in fp64 (an edge decision within RING_TIE is retaken in fp64, R-17)
     float half_skin2;             // (skin/2)^2
+    float hs;                     // skin/2
+    float Wc;                     // w_i = Wc / sqrt(beta m_i): mass weight of atom i's skin, m_i^-1/2 / mean(m^-1/2) (R-10c)
+    float w_max;
     unsigned int key0, key1;      // Philox key = seed
 };
 

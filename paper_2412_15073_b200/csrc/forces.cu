@@ -274,7 +274,7 @@ static void pair_dispatch(const Model &m, const Row &row, const float4 *xs, cons
                           bool energy, cudaStream_t st) {
     const int B = 256;
     unsigned grid = (unsigned)(((long long)m.n * 32 + B - 1) / B);
-    const float margin = sqrtf(row.r2max) + 2.f * sqrtf(m.half_skin2) * 2.f;   // reach + 2 skins
+    const float margin = sqrtf(row.r2max) + 2.f * m.hs * m.w_max * 2.f;   // farthest entry at a build + what two atoms may move
     if (energy) k_pair<WC, WLJ, true><<<grid, B, 0, st>>>(m, row, margin, xs, lj, out, accumulate);
     else k_pair<WC, WLJ, false><<<grid, B, 0, st>>>(m, row, margin, xs, lj, out, accumulate);
 }

@@ -4,18 +4,25 @@
 
 namespace jb {
 
+// A list (re)build is a fixed sequence of kernels.  go == NULL: they run.  go != NULL: they run only if *go == want, i.e.
+// if the update kernel of this very step found an atom farther than skin/2 from its build position (R-10c) -- the
+// decision is taken on the device, the host enqueues the sequence either way and never waits for it.
 struct SortArgs {
     int n;
     SortGrid grid;
-    const float4 *xs_in, *vs_in, *xl_in;
-    const float2 *lj_in, *mi_in;
-    const int *orig_in;
-    float4 *xs, *vs, *xl, *x_build;
-    float2 *lj, *mi;
-    int *orig, *sorted_of, *cell_of;
+    float4 *xs, *vs, *xl;          // state in the current sorted order: read, then overwritten with the new order
+    float2 *lj, *mi, *hw;
+    int *orig;
+    float4 *xs_t, *vs_t, *xl_t;    // scratch of the permutation
+    float2 *lj_t, *mi_t, *hw_t;
+    int *orig_t;
+    float4 *x_build;
+    int *sorted_of, *cell_of;
     int *key, *cell_count, *cell_fill, *cell_start, *tmp_orig, *tmp_src;
     int *scan_sums, *scan_offs;   // scratch of the multi-block scan (ncell / 4096 + 2 each)
     Counters *ctr;
+    const int *go;
+    int want;
 };
 
 struct UpdateArgs {
@@ -42,6 +49,9 @@ struct UpdateArgs {
     jump_event *events;  // NULL: no log
     long long event_cap;
     int lanes;           // lanes per jump chain (0: chosen from the grid size)
+    int trigger;         // 1: a conditional list build follows this launch, a displacement beyond skin/2 arms it; 2: an
+                         // unconditional one follows; 0: none follows, such a displacement is the error ERR_SKIN
+    int step_id;         // the stamp it is armed with
 };
 
 struct EwaldArgs {   // reciprocal Ewald sum (ewald.cu, R-21)
@@ -63,13 +73,13 @@ struct EwaldArgs {   // reciprocal Ewald sum (ewald.cu, R-21)
 
 void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches);
 void launch_universe(const SortGrid &g, const Universe &u, const int *cell_start, unsigned short *cum, Counters *ctr,
-                     cudaStream_t st, int64_t *launches);
+                     const int *go, int want, cudaStream_t st, int64_t *launches);
 int launch_universe_list(const SortGrid &g, const Universe &u, const int *cell_start, int home, int *out, int cap,
                          cudaStream_t st, int64_t *launches);
 void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS], float rmax_all, const int *cell_start,
-                       const float4 *xs, const float4 *xl, const float2 *lj, const int *orig, const int *sorted_of,
-                       const int *excl_ptr, const int *excl_idx, Counters *ctr, int *cell_of, float far2, cudaStream_t st,
-                       int64_t *launches);
+                       const float4 *xs, const float4 *xl, const float2 *lj, const float2 *hw, const int *orig, const int *sorted_of,
+                       const int *excl_ptr, const int *excl_idx, Counters *ctr, int *cell_of, float far2, const int *go, int want,
+                       cudaStream_t st, int64_t *launches);
 int launch_pair(const Model &m, const Row &row, int wC, int wLJ, const float4 *xs, const float2 *lj, float4 *out,
                 int accumulate, bool energy, cudaStream_t st, int64_t *launches);
 void launch_count_pairs(const Model &m, const Row &row, const float4 *xs, float rc2, unsigned long long *out,
@@ -81,10 +91,10 @@ void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t
 void launch_writeback(int n, const float4 *xs, const float4 *vs, const int *orig, float *pos, float *vel, cudaStream_t st,
                       int64_t *launches);
 void launch_load(const Model &m, const float *pos, const float *vel, const float *mass, const float *charge,
-                 const float *sigma, const float *eps, double kT, float4 *xs, float4 *vs, float4 *xl, float2 *lj, float2 *mi, int *orig,
-                 cudaStream_t st, int64_t *launches);
+                 const float *sigma, const float *eps, double kT, double hs_over_wnorm, float4 *xs, float4 *vs, float4 *xl, float2 *lj,
+                 float2 *mi, float2 *hw, int *orig, cudaStream_t st, int64_t *launches);
 void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
-                   float4 *xl, const float4 *x_build, int *moved, int keep, cudaStream_t st, int64_t *launches);
+                   float4 *xl, const float4 *x_build, int *moved, int keep, const float2 *mi, cudaStream_t st, int64_t *launches);
 int launch_rdf(const Model &m, const SortGrid &g, int lj_only, double r_max, double r_reach, int n_bins, const int *cell_start,
                const float4 *xs, const float2 *lj, unsigned long long *hist, cudaStream_t st, int64_t *launches);
 void launch_vacf_mark(int n, const float4 *vs, const int *orig, float4 *v0, cudaStream_t st, int64_t *launches);

@@ -16,7 +16,8 @@
 namespace jb {
 
 __global__ void k_cell_key(int n, const float4 *__restrict__ xs, SortGrid g, int *__restrict__ key,
-                           int *__restrict__ cell_count, Counters *ctr) {
+                           int *__restrict__ cell_count, Counters *ctr, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     float4 x = xs[i];
@@ -37,7 +38,8 @@ __global__ void k_cell_key(int n, const float4 *__restrict__ xs, SortGrid g, int
 }
 
 // exclusive scan of cell_count[0..ncell) into cell_start[0..ncell]; one block
-__global__ void k_scan(int ncell, const int *__restrict__ cell_count, int *__restrict__ cell_start) {
+__global__ void k_scan(int ncell, const int *__restrict__ cell_count, int *__restrict__ cell_start, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
     __shared__ int part[1024];
     int t = threadIdx.x, nt = blockDim.x;
     int per = (ncell + nt - 1) / nt;
@@ -63,7 +65,8 @@ __global__ void k_scan(int ncell, const int *__restrict__ cell_count, int *__res
 // the same scan for large grids, in three small launches: per-block sums of 4096-cell slices, a scan of the
 // sums (k_scan on them), then each block scans its slice from its offset
 constexpr int SCAN_SLICE = 4096;
-__global__ void k_scan_sums(int ncell, const int *__restrict__ cell_count, int *__restrict__ sums) {
+__global__ void k_scan_sums(int ncell, const int *__restrict__ cell_count, int *__restrict__ sums, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
     __shared__ int part[32];
     const int lo = blockIdx.x * SCAN_SLICE, hi = min(lo + SCAN_SLICE, ncell);
     int s = 0;
@@ -78,7 +81,8 @@ __global__ void k_scan_sums(int ncell, const int *__restrict__ cell_count, int *
     }
 }
 __global__ void k_scan_slices(int ncell, const int *__restrict__ cell_count, const int *__restrict__ offs,
-                              int *__restrict__ cell_start) {
+                              int *__restrict__ cell_start, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
     __shared__ int part[1024];
     const int t = threadIdx.x, nt = blockDim.x;   // nt * 4 = SCAN_SLICE
     const int lo = blockIdx.x * SCAN_SLICE + 4 * t;
@@ -104,7 +108,8 @@ __global__ void k_scan_slices(int ncell, const int *__restrict__ cell_count, con
 
 __global__ void k_scatter(int n, const int *__restrict__ key, const int *__restrict__ orig,
                           const int *__restrict__ cell_start, int *__restrict__ cell_fill,
-                          int *__restrict__ tmp_orig, int *__restrict__ tmp_src) {
+                          int *__restrict__ tmp_orig, int *__restrict__ tmp_src, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int k = key[i];
@@ -115,7 +120,8 @@ __global__ void k_scatter(int n, const int *__restrict__ key, const int *__restr
 
 // order each cell by original index (insertion sort; a cell holds a handful of atoms)
 __global__ void k_cell_sort(int ncell, const int *__restrict__ cell_start, int *__restrict__ tmp_orig,
-                            int *__restrict__ tmp_src) {
+                            int *__restrict__ tmp_src, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
     int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= ncell) return;
     int lo = cell_start[c], hi = cell_start[c + 1];
@@ -135,12 +141,16 @@ __global__ void k_cell_sort(int ncell, const int *__restrict__ cell_start, int *
 __global__ void k_permute(int n, const int *__restrict__ src, const int *__restrict__ new_orig,
                           const float4 *__restrict__ xs_in, const float4 *__restrict__ vs_in,
                           const float4 *__restrict__ xl_in, float4 *__restrict__ xl,
-                          const float2 *__restrict__ lj_in, const float2 *__restrict__ mi_in,
+                          const float2 *__restrict__ lj_in, const float2 *__restrict__ mi_in, const float2 *__restrict__ hw_in,
+                          float2 *__restrict__ hw,
                           float4 *__restrict__ xs, float4 *__restrict__ vs, float2 *__restrict__ lj,
                           float2 *__restrict__ mi, int *__restrict__ orig, int *__restrict__ sorted_of,
-                          float4 *__restrict__ x_build, const int *__restrict__ key, int *__restrict__ cell_of, int gnx, int gny) {
+                          float4 *__restrict__ x_build, const int *__restrict__ key, int *__restrict__ cell_of, int gnx, int gny,
+                          Counters *ctr, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    if (i == 0) ctr->rebuilds += 1;
     int s = src[i];
     const int kk = key[s];   // home cell, packed by coordinates (the universe lookup wants them without divisions)
     cell_of[i] = pack_cell(kk % gnx, (kk / gnx) % gny, kk / (gnx * gny));
@@ -150,10 +160,22 @@ __global__ void k_permute(int n, const int *__restrict__ src, const int *__restr
     vs[i] = vs_in[s];
     xl[i] = xl_in[s];
     lj[i] = lj_in[s];
+    hw[i] = hw_in[s];
     mi[i] = mi_in[s];
     int o = new_orig[i];
     orig[i] = o;
     sorted_of[o] = i;
+}
+// the permuted copies back into the state arrays (a pointer swap on the host would need to know whether the sort ran)
+__global__ void k_copyback(int n, const float4 *__restrict__ xs_t, const float4 *__restrict__ vs_t, const float4 *__restrict__ xl_t,
+                           const float2 *__restrict__ lj_t, const float2 *__restrict__ mi_t, const float2 *__restrict__ hw_t, float2 *__restrict__ hw,
+                           const int *__restrict__ orig_t,
+                           float4 *__restrict__ xs, float4 *__restrict__ vs, float4 *__restrict__ xl, float2 *__restrict__ lj,
+                           float2 *__restrict__ mi, int *__restrict__ orig, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    xs[i] = xs_t[i]; vs[i] = vs_t[i]; xl[i] = xl_t[i]; lj[i] = lj_t[i]; mi[i] = mi_t[i]; hw[i] = hw_t[i]; orig[i] = orig_t[i];
 }
 
 struct RowSet { Row r[N_ROWS]; };
@@ -194,28 +216,30 @@ constexpr int BUILD_CHUNK = 1024;           // candidates staged per pass
 constexpr int BUILD_MAXSEG = 2 * 17 * 17;   // two x-runs per (z, y) cell row of the stencil
 constexpr int BUILD_MAXATOMS = 32;          // atoms of a cell whose running counts are held at once
 constexpr float BUILD_TIE = 4e-3f;          // A^2
+constexpr float BUILD_TIE_R = 3e-4f;        // A: an fp32 distance this close to a window edge is re-decided in fp64
 
 struct Stencil {
     int R[3];                 // cells on each side, per dimension
-    int n_edge;               // distinct window edges of the selected rows (squared, fp32)
-    float edge2[6];           // padded with a value no r^2 comes near
     signed char xr[17 * 17];  // [|oz| * 17 + |oy|] -> largest |ox| still within reach, -1: skip the (z, y) cell row
 };
 
 // MASK >= 0: bit k set = row k is built (compile-time row set of the common modes); MASK < 0: rows.r[k].enabled decides
 template <int MASK, bool FAST>
-__global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid g, RowSet rows, Stencil stn, float rmax_all, int CX,
+__global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGrid g, RowSet rows, Stencil stn, float rmax_all, int CX,
                                                               const int *__restrict__ cell_start,
                                                               const float4 *__restrict__ xs, const float4 *__restrict__ xl,
-                                                              const float2 *__restrict__ lj,
+                                                              const float2 *__restrict__ lj, const float2 *__restrict__ hw,
                                                               const int *__restrict__ orig, const int *__restrict__ sorted_of,
                                                               const int *__restrict__ excl_ptr, const int *__restrict__ excl_idx,
-                                                              Counters *ctr, int *__restrict__ cell_of, float far2) {
+                                                              Counters *ctr, int *__restrict__ cell_of, float far2,
+                                                              const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
     __shared__ int seg_beg[BUILD_MAXSEG];       // stencil runs in ascending cell key (many are empty) ...
     __shared__ int seg_pre[BUILD_MAXSEG + 1];   // ... their lengths, then (length << 10 | non-empty) prefix sums
     __shared__ int run_beg[BUILD_MAXSEG];       // the non-empty runs, compacted: first atom ...
     __shared__ int run_pre[BUILD_MAXSEG + 1];   // ... and exclusive prefix of the lengths
     __shared__ float4 tile[BUILD_CHUNK];        // (x, y, z, sorted index | LJ flag in bit 31)
+    __shared__ float tile_w[BUILD_CHUNK];       // (skin/2) w_j: the candidate's share of the pair's skin (R-10c)
     __shared__ int scan_tmp[BUILD_THREADS];
     __shared__ int s_count[BUILD_MAXATOMS][N_ROWS];
     const unsigned full = 0xffffffffu;
@@ -317,8 +341,9 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                     }
                     x.w = __int_as_float(j | (lj[j].y > 0.f ? (int)0x80000000 : 0));
                     tile[q - c0] = x;
+                    tile_w[q - c0] = hw[j].x;
                 }
-                for (int q = (c1 - c0) + tid; q < npad; q += BUILD_THREADS) tile[q] = make_float4(nanf(""), 0.f, 0.f, 0.f);   // padding: r^2 = NaN fails every test
+                for (int q = (c1 - c0) + tid; q < npad; q += BUILD_THREADS) { tile[q] = make_float4(nanf(""), 0.f, 0.f, 0.f); tile_w[q] = 0.f; }   // padding: r^2 = NaN fails every test
             }
             __syncthreads();
             // ---- 2./3. the atoms of the cell against the staged chunk ---------------------------------------------
@@ -331,6 +356,8 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                     zi = near_image1(zi - ctr3[2], m.box[2], m.inv_box[2]);
                 }
                 const bool lj_i = lj[i].y > 0.f;
+                const float2 hw_i = hw[i];
+                const float hsw_i = hw_i.x;   // (skin/2) w_i
                 // excluded partners (R-9): the first four in every lane, and the largest distance to any of them
                 int ex_lo = 0, n_ex = 0;
                 if (excl_ptr) { int o = orig[i]; ex_lo = excl_ptr[o]; n_ex = excl_ptr[o + 1] - ex_lo; }
@@ -362,7 +389,6 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                     count[k] = JB_ROW_ON(k) ? s_count[i - g0][k] : 0;
                     rbase[k] = JB_ROW_ON(k) ? rows.r[k].idx + (size_t)i * rows.r[k].cap : nullptr;
                 }
-                const float e0 = stn.edge2[0], e1 = stn.edge2[1], e2 = stn.edge2[2], e3 = stn.edge2[3], e4 = stn.edge2[4], e5 = stn.edge2[5];
                 // The scan is instantiated twice: an atom without LJ (two thirds of a water box) has no W row, and
                 // its copy of the loop carries no test, ballot or counter for them (MASK >= 0; a branch on this
                 // inside the unrolled row loop was measured slower than the work it skips).
@@ -397,15 +423,28 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                             valid = valid && !ex;
                         }
                         const bool ljp = LJ_I && jraw < 0;
+                        // window of this pair in row k: [ra - s_ij, rb + s_ij), s_ij = (skin/2)(w_i + w_j) (row W: from ra + s_ij),
+                        // tested on r -/+ s_ij against the row's constants
+                        const float sij = hsw_i + tile_w[q0 + lane];
+                        const float r = r2 * rsqrtf(fmaxf(r2, 1e-12f));
+                        const float rm = r - sij, rp = r + sij;
                         bool pass[N_ROWS];
+                        float edge_gap = 1e30f;   // distance of r to the nearest window edge of a scanned row
 #pragma unroll
                         for (int k = 0; k < N_ROWS; ++k) {
                             pass[k] = false;
                             if (!JB_ROW_SCAN(k)) continue;
                             const Row &R = rows.r[k];
-                            pass[k] = valid && (!JB_LJ_ROW(k) || ljp) && r2 >= R.r2min && r2 < R.r2max;
+                            bool in = rm < R.rb;
+                            edge_gap = fminf(edge_gap, fabsf(rm - R.rb));
+                            if (R.ra > 0.f) {
+                                const float t = R.lo_plus ? rm : rp;
+                                in = in && t >= R.ra;
+                                edge_gap = fminf(edge_gap, fabsf(t - R.ra));
+                            }
+                            pass[k] = valid && (!JB_LJ_ROW(k) || ljp) && in;
                         }
-                        const bool tie = valid && fminf(fminf(fminf(fabsf(r2 - e0), fabsf(r2 - e1)), fminf(fabsf(r2 - e2), fabsf(r2 - e3))), fminf(fabsf(r2 - e4), fabsf(r2 - e5))) < BUILD_TIE;
+                        const bool tie = valid && edge_gap < BUILD_TIE_R;
                         if (tie) {   // decide in fp64 from the full positions, like the oracle
                             float4 hi_j = xs[j], li = xl[i], lo_j = xl[j];
                             double d[3] = {((double)xi4.x + (double)li.x) - ((double)hi_j.x + (double)lo_j.x),
@@ -418,11 +457,15 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
                                 d[k] -= L * rint(d[k] / L);
                                 r2d += d[k] * d[k];
                             }
+                            const float2 hw_j = hw[j];
+                            const double sd = ((double)hw_i.x + (double)hw_i.y) + ((double)hw_j.x + (double)hw_j.y);   // s_ij in fp64
 #pragma unroll
                             for (int k = 0; k < N_ROWS; ++k) {
                                 if (!JB_ROW_SCAN(k)) continue;
                                 const Row &R = rows.r[k];
-                                pass[k] = (!JB_LJ_ROW(k) || ljp) && r2d >= R.r2min_d && r2d < R.r2max_d;
+                                const double hi = R.rb_d + sd;
+                                const double lo = R.ra > 0.f ? (R.lo_plus ? R.ra_d + sd : fmax(R.ra_d - sd, 0.0)) : 0.0;
+                                pass[k] = (!JB_LJ_ROW(k) || ljp) && r2d >= lo * lo && r2d < hi * hi;
                             }
                         }
 #pragma unroll
@@ -465,7 +508,8 @@ __global__ void __launch_bounds__(BUILD_THREADS) k_build_rows(Model m, SortGrid 
 // One warp per home cell: the lengths of its stencil rows (two cell_start differences each), prefix-summed into
 // cum[h][0 .. nrow]; cum[h][nrow] is the size of the universe, N_C of every atom of the cell.
 __global__ void __launch_bounds__(128) k_universe(SortGrid g, Universe u, const int *__restrict__ cell_start,
-                                                  unsigned short *__restrict__ cum, Counters *ctr) {
+                                                  unsigned short *__restrict__ cum, Counters *ctr, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
     const int h = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (h >= g.ncell) return;
     if (cell_start[h + 1] == cell_start[h]) return;   // no atom lives here: the row is never read
@@ -507,29 +551,32 @@ static inline int nblk(int n, int b) { return (n + b - 1) / b; }
 
 void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches) {
     const int B = 256;
-    cudaMemsetAsync(a.cell_count, 0, sizeof(int) * (a.grid.ncell + 1), st);
+    cudaMemsetAsync(a.cell_count, 0, sizeof(int) * (a.grid.ncell + 1), st);   // (scratch: harmless when the sort does not run)
     cudaMemsetAsync(a.cell_fill, 0, sizeof(int) * (a.grid.ncell + 1), st);
-    k_cell_key<<<nblk(a.n, B), B, 0, st>>>(a.n, a.xs_in, a.grid, a.key, a.cell_count, a.ctr);
+    k_cell_key<<<nblk(a.n, B), B, 0, st>>>(a.n, a.xs, a.grid, a.key, a.cell_count, a.ctr, a.go, a.want);
     if (a.grid.ncell <= 4 * SCAN_SLICE) {
-        k_scan<<<1, 1024, 0, st>>>(a.grid.ncell, a.cell_count, a.cell_start);
+        k_scan<<<1, 1024, 0, st>>>(a.grid.ncell, a.cell_count, a.cell_start, a.go, a.want);
     } else {
         const int nb = nblk(a.grid.ncell, SCAN_SLICE);
-        k_scan_sums<<<nb, 256, 0, st>>>(a.grid.ncell, a.cell_count, a.scan_sums);
-        k_scan<<<1, 1024, 0, st>>>(nb, a.scan_sums, a.scan_offs);
-        k_scan_slices<<<nb, SCAN_SLICE / 4, 0, st>>>(a.grid.ncell, a.cell_count, a.scan_offs, a.cell_start);
+        k_scan_sums<<<nb, 256, 0, st>>>(a.grid.ncell, a.cell_count, a.scan_sums, a.go, a.want);
+        k_scan<<<1, 1024, 0, st>>>(nb, a.scan_sums, a.scan_offs, a.go, a.want);
+        k_scan_slices<<<nb, SCAN_SLICE / 4, 0, st>>>(a.grid.ncell, a.cell_count, a.scan_offs, a.cell_start, a.go, a.want);
         *launches += 2;
     }
-    k_scatter<<<nblk(a.n, B), B, 0, st>>>(a.n, a.key, a.orig_in, a.cell_start, a.cell_fill, a.tmp_orig, a.tmp_src);
-    k_cell_sort<<<nblk(a.grid.ncell, B), B, 0, st>>>(a.grid.ncell, a.cell_start, a.tmp_orig, a.tmp_src);
-    k_permute<<<nblk(a.n, B), B, 0, st>>>(a.n, a.tmp_src, a.tmp_orig, a.xs_in, a.vs_in, a.xl_in, a.xl, a.lj_in, a.mi_in, a.xs, a.vs,
-                                          a.lj, a.mi, a.orig, a.sorted_of, a.x_build, a.key, a.cell_of, a.grid.gn[0], a.grid.gn[1]);
-    *launches += 5;
+    k_scatter<<<nblk(a.n, B), B, 0, st>>>(a.n, a.key, a.orig, a.cell_start, a.cell_fill, a.tmp_orig, a.tmp_src, a.go, a.want);
+    k_cell_sort<<<nblk(a.grid.ncell, B), B, 0, st>>>(a.grid.ncell, a.cell_start, a.tmp_orig, a.tmp_src, a.go, a.want);
+    k_permute<<<nblk(a.n, B), B, 0, st>>>(a.n, a.tmp_src, a.tmp_orig, a.xs, a.vs, a.xl, a.xl_t, a.lj, a.mi, a.hw, a.hw_t, a.xs_t, a.vs_t,
+                                          a.lj_t, a.mi_t, a.orig_t, a.sorted_of, a.x_build, a.key, a.cell_of, a.grid.gn[0],
+                                          a.grid.gn[1], a.ctr, a.go, a.want);
+    k_copyback<<<nblk(a.n, B), B, 0, st>>>(a.n, a.xs_t, a.vs_t, a.xl_t, a.lj_t, a.mi_t, a.hw_t, a.hw, a.orig_t, a.xs, a.vs, a.xl, a.lj, a.mi, a.orig,
+                                           a.go, a.want);
+    *launches += 6;
 }
 
 void launch_universe(const SortGrid &g, const Universe &u, const int *cell_start, unsigned short *cum, Counters *ctr,
-                     cudaStream_t st, int64_t *launches) {
+                     const int *go, int want, cudaStream_t st, int64_t *launches) {
     const int B = 128;
-    k_universe<<<(unsigned)(((long long)g.ncell * 32 + B - 1) / B), B, 0, st>>>(g, u, cell_start, cum, ctr);
+    k_universe<<<(unsigned)(((long long)g.ncell * 32 + B - 1) / B), B, 0, st>>>(g, u, cell_start, cum, ctr, go, want);
     *launches += 1;
 }
 int launch_universe_list(const SortGrid &g, const Universe &u, const int *cell_start, int home, int *out, int n,
@@ -540,9 +587,9 @@ int launch_universe_list(const SortGrid &g, const Universe &u, const int *cell_s
 }
 
 void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS], float rmax_all, const int *cell_start,
-                       const float4 *xs, const float4 *xl, const float2 *lj, const int *orig, const int *sorted_of,
-                       const int *excl_ptr, const int *excl_idx, Counters *ctr, int *cell_of, float far2, cudaStream_t st,
-                       int64_t *launches) {
+                       const float4 *xs, const float4 *xl, const float2 *lj, const float2 *hw, const int *orig, const int *sorted_of,
+                       const int *excl_ptr, const int *excl_idx, Counters *ctr, int *cell_of, float far2, const int *go, int want,
+                       cudaStream_t st, int64_t *launches) {
     RowSet rs;
     for (int k = 0; k < N_ROWS; ++k) rs.r[k] = rows[k];
     // stencil of cells within reach of a cell: gap between cells at offset o is (|o| - 1)_+ cell edges
@@ -552,16 +599,6 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
         cs[k] = (double)m.box[k] / g.gn[k];
         stn.R[k] = std::min(8, (int)std::ceil((double)rmax_all / cs[k]));  // init refuses grids that need more
     }
-    stn.n_edge = 0;
-    for (int k = 0; k < N_ROWS; ++k) {
-        if (!rows[k].enabled) continue;
-        for (float e : {rows[k].r2min, rows[k].r2max}) {
-            bool seen = e <= 0.f;
-            for (int q = 0; q < stn.n_edge; ++q) seen |= stn.edge2[q] == e;
-            if (!seen && stn.n_edge < 6) stn.edge2[stn.n_edge++] = e;   // the windows of api.cu have <= 6 distinct edges
-        }
-    }
-    for (int q = stn.n_edge; q < 6; ++q) stn.edge2[q] = -1e30f;
     const double r2 = (double)rmax_all * rmax_all;
     for (int a = 0; a < 17; ++a)
         for (int b = 0; b < 17; ++b) {
@@ -582,10 +619,10 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
     const unsigned nblocks = (unsigned)(((g.gn[0] + CX - 1) / CX) * g.gn[1] * g.gn[2]);
 #define JB_BUILD(MASK)                                                                                                        \
     do {                                                                                                                      \
-        if (fast) k_build_rows<MASK, true><<<nblocks, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, \
-                                                                                       orig, sorted_of, excl_ptr, excl_idx, ctr, cell_of, far2); \
-        else k_build_rows<MASK, false><<<nblocks, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, \
-                                                                                    orig, sorted_of, excl_ptr, excl_idx, ctr, cell_of, far2);   \
+        if (fast) k_build_rows<MASK, true><<<nblocks, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, hw, \
+                                                                                       orig, sorted_of, excl_ptr, excl_idx, ctr, cell_of, far2, go, want); \
+        else k_build_rows<MASK, false><<<nblocks, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, hw, \
+                                                                                    orig, sorted_of, excl_ptr, excl_idx, ctr, cell_of, far2, go, want);   \
     } while (0)
     switch (mask) {
         case 0x07: JB_BUILD(0x07); break;   // S A B     (JUMP with Coulomb and LJ jumps)

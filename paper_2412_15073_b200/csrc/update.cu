@@ -295,7 +295,9 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
             float ddx = min_image1(x, xb.x, m.box[0], m.inv_box[0]);
             float ddy = min_image1(y, xb.y, m.box[1], m.inv_box[1]);
             float ddz = min_image1(z, xb.z, m.box[2], m.inv_box[2]);
-            disp2 = ddx * ddx + ddy * ddy + ddz * ddz;
+            // scaled by the atom's share of the skin (R-10c): w_i = Wc / sqrt(beta m_i); the budget is (skin/2) w_i
+            const float inv_w = mi.y / m.Wc;
+            disp2 = (ddx * ddx + ddy * ddy + ddz * ddz) * (inv_w * inv_w);
             bad = !(isfinite(x) && isfinite(y) && isfinite(z));
         }
         bad = bad || !(isfinite(vx) && isfinite(vy) && isfinite(vz));
@@ -308,7 +310,7 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
     __syncthreads();
     unsigned err = 0;
     if (bad) err |= ERR_NAN;
-    if (disp2 > m.half_skin2) err |= ERR_SKIN;
+    if (disp2 > m.half_skin2 && !A.trigger) err |= ERR_SKIN;   // (with a conditional list build behind this launch it arms that instead)
     if (tl.max_p > 1.f + 1e-4f || tl.max_gl > 1.f + 1e-4f) err |= ERR_BOUND;
     unsigned d2b = __reduce_max_sync(full, __float_as_uint(disp2));
     err = __reduce_or_sync(full, err);
@@ -341,6 +343,8 @@ __global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
             if (s_stat[5] > A.ctr->max_gl_bits) atomicMax(&A.ctr->max_gl_bits, s_stat[5]);
         }
         if (s_stat[6] > A.ctr->max_disp2_bits) atomicMax(&A.ctr->max_disp2_bits, s_stat[6]);
+        // some atom is farther than skin/2 from where the lists saw it: the list kernels enqueued behind this launch run
+        if (A.trigger == 1 && __uint_as_float(s_stat[6]) > m.half_skin2) A.ctr->go_step = A.step_id;
         if (s_stat[7]) atomicOr(&A.ctr->err, s_stat[7]);
     }
 }
@@ -359,9 +363,9 @@ __global__ void k_writeback(int n, const float4 *__restrict__ xs, const float4 *
 // original order in: wrap positions, pack (x, q), (v), (sqrt sigma, 2 sqrt eps), (kcal/m, sqrt(beta m))
 __global__ void k_load(Model m, const float *__restrict__ pos, const float *__restrict__ vel,
                        const float *__restrict__ mass, const float *__restrict__ charge,
-                       const float *__restrict__ sigma, const float *__restrict__ eps, double kT, float4 *__restrict__ xs,
-                       float4 *__restrict__ vs, float4 *__restrict__ xl, float2 *__restrict__ lj, float2 *__restrict__ mi,
-                       int *__restrict__ orig) {
+                       const float *__restrict__ sigma, const float *__restrict__ eps, double kT, double hs_over_wnorm,
+                       float4 *__restrict__ xs, float4 *__restrict__ vs, float4 *__restrict__ xl, float2 *__restrict__ lj,
+                       float2 *__restrict__ mi, float2 *__restrict__ hw, int *__restrict__ orig) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
     float x = wrap1(pos[3 * i], m.box[0], m.inv_box[0]);
@@ -374,6 +378,11 @@ __global__ void k_load(Model m, const float *__restrict__ pos, const float *__re
     lj[i] = make_float2(e > 0.f ? (float)sqrt((double)sigma[i]) : 0.f, e > 0.f ? (float)(2.0 * sqrt((double)e)) : 0.f);
     double md = (double)mass[i];
     mi[i] = make_float2((float)(kKcal / md), (float)sqrt(md / (kT * kKcal)));
+    // the atom's share of a pair's skin, (skin/2) w_i with w_i = m_i^-1/2 / mean(m^-1/2) (R-10c), as an fp64 value split in
+    // two floats: list-edge ties are decided with the same number the fp64 oracle uses
+    const double hsw = (1.0 / sqrt(md)) * hs_over_wnorm;
+    const float hsw_hi = (float)hsw;
+    hw[i] = make_float2(hsw_hi, (float)(hsw - (double)hsw_hi));
     orig[i] = i;
 }
 
@@ -384,7 +393,8 @@ __global__ void k_load(Model m, const float *__restrict__ pos, const float *__re
 // the box lengths its coordinate lies outside [0, L) by.  !keep (jump_refresh): residual and counters restart at 0.
 __global__ void k_reload(Model m, const float *__restrict__ pos, const float *__restrict__ vel,
                          const int *__restrict__ orig, float4 *__restrict__ xs, float4 *__restrict__ vs,
-                         float4 *__restrict__ xl, const float4 *__restrict__ x_build, int *__restrict__ moved, int keep) {
+                         float4 *__restrict__ xl, const float4 *__restrict__ x_build, int *__restrict__ moved, int keep,
+                         const float2 *__restrict__ mi) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= m.n) return;
     int o = orig[i];
@@ -399,7 +409,8 @@ __global__ void k_reload(Model m, const float *__restrict__ pos, const float *__
         const float dx = min_image1(x.x, xb.x, m.box[0], m.inv_box[0]);
         const float dy = min_image1(x.y, xb.y, m.box[1], m.inv_box[1]);
         const float dz = min_image1(x.z, xb.z, m.box[2], m.inv_box[2]);
-        const float d2 = dx * dx + dy * dy + dz * dz;
+        const float inv_w = mi[i].y / m.Wc;   // (the atom's budget is (skin/2) w_i, R-10c)
+        const float d2 = (dx * dx + dy * dy + dz * dz) * (inv_w * inv_w);
         if (!(d2 <= m.half_skin2)) *moved = 1;   // also when a position is not finite
     }
     float4 l = make_float4(0.f, 0.f, 0.f, __int_as_float(img_pack(0, 0, 0)));
@@ -487,14 +498,14 @@ void launch_writeback(int n, const float4 *xs, const float4 *vs, const int *orig
     *launches += 1;
 }
 void launch_load(const Model &m, const float *pos, const float *vel, const float *mass, const float *charge,
-                 const float *sigma, const float *eps, double kT, float4 *xs, float4 *vs, float4 *xl, float2 *lj, float2 *mi,
-                 int *orig, cudaStream_t st, int64_t *launches) {
-    k_load<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, mass, charge, sigma, eps, kT, xs, vs, xl, lj, mi, orig);
+                 const float *sigma, const float *eps, double kT, double hs_over_wnorm, float4 *xs, float4 *vs, float4 *xl, float2 *lj,
+                 float2 *mi, float2 *hw, int *orig, cudaStream_t st, int64_t *launches) {
+    k_load<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, mass, charge, sigma, eps, kT, hs_over_wnorm, xs, vs, xl, lj, mi, hw, orig);
     *launches += 1;
 }
 void launch_reload(const Model &m, const float *pos, const float *vel, const int *orig, float4 *xs, float4 *vs,
-                   float4 *xl, const float4 *x_build, int *moved, int keep, cudaStream_t st, int64_t *launches) {
-    k_reload<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, orig, xs, vs, xl, x_build, moved, keep);
+                   float4 *xl, const float4 *x_build, int *moved, int keep, const float2 *mi, cudaStream_t st, int64_t *launches) {
+    k_reload<<<(m.n + 255) / 256, 256, 0, st>>>(m, pos, vel, orig, xs, vs, xl, x_build, moved, keep, mi);
     *launches += 1;
 }
 void launch_images(int n, const float4 *xl, const int *orig, int *out, cudaStream_t st, int64_t *launches) {

@@ -325,8 +325,9 @@ def test_ring_rows_contract(cfg0):
 
 @pytest.mark.parametrize("case", ["cfg0", "wide", "ortho"])
 def test_rows_and_cell_universe_contract(cfg0, case):
-    """R-10c (list_policy 1, the contract of the CUDA path): row A = [rc-h-s, rA+s), row B = [rA-s, rM+s) by build-time
-    distance, excluded pairs never listed, ascending (cell key, index); ring 3 draws from the cell universe of the
+    """R-10c (list_policy 1, the contract of the CUDA path): row A = [rc-h-s_ij, rA+s_ij), row B = [rA-s_ij, rM+s_ij) by
+    build-time distance with the mass-weighted skin s_ij = (s/2)(w_i + w_j), w = m^-1/2 / mean(m^-1/2), excluded pairs
+    never listed, ascending (cell key, index); ring 3 draws from the cell universe of the
     atom's home cell: the atoms of every contract cell within reach r_long + s of the home cell by the rule typed out
     below (an independent restatement), ascending (cell key, index), the atom itself and its excluded partners
     included.  And the property the thinning needs: every pair closer than r_long + s is in the universe."""
@@ -342,15 +343,16 @@ def test_rows_and_cell_universe_contract(cfg0, case):
     box = np.broadcast_to(np.asarray(sysd["box"], float), (3,))
     rc, h, s, rM, rl = run["r_short"], run["r_switch"], run["skin"], run["r_mid"], run["r_long"]
     rA = run.get("r_mid_in") or rc + 0.25
-    edge = run.get("cell_edge", 0.0) or (rl + s) / 4
+    w = 1.0 / np.sqrt(sysd["mass"]); w = w / w.mean()
+    edge = run.get("cell_edge", 0.0) or (rl + s * w.max()) / 4
     ng, cell, key = _contract_keys(x, box, edge)
     d = x[:, None, :] - x[None, :, :]
     d -= box * np.round(d / box)
     r = np.sqrt((d ** 2).sum(-1))
     nA, nB, nU = o.row_counts()
-    w = box / ng
-    reach = rl + s
-    R = np.ceil(reach / w).astype(int)
+    cw = box / ng
+    reach = rl + s * w.max()
+    R = np.ceil(reach / cw).astype(int)
 
     def cyc(a, b, m):
         o_ = (a - b) % m
@@ -360,14 +362,14 @@ def test_rows_and_cell_universe_contract(cfg0, case):
         a, b, e = cyc(cj[2], ci[2], ng[2]), cyc(cj[1], ci[1], ng[1]), cyc(cj[0], ci[0], ng[0])
         if a > R[2] or b > R[1]:
             return False
-        rem = reach ** 2 - (max(a - 1, 0) * w[2]) ** 2 - (max(b - 1, 0) * w[1]) ** 2
-        return rem > 0 and e <= min(R[0], int(math.floor(math.sqrt(rem) / w[0])) + 1)
+        rem = reach ** 2 - (max(a - 1, 0) * cw[2]) ** 2 - (max(b - 1, 0) * cw[1]) ** 2
+        return rem > 0 and e <= min(R[0], int(math.floor(math.sqrt(rem) / cw[0])) + 1)
 
-    lo = max(rc - h - s, 0.0)
     for i in (0, 1, 2, 100, 331, n - 1):
         excl = set(sysd["excl_idx"][sysd["excl_ptr"][i]:sysd["excl_ptr"][i + 1]].tolist()) | {i}
-        for which, lo_, hi_ in ((0, lo, rA + s), (1, max(rA - s, lo), rM + s)):
-            want = [j for j in range(n) if j not in excl and lo_ <= r[i, j] < hi_]
+        sij = 0.5 * s * (w[i] + w)
+        for which, lo_, hi_ in ((0, rc - h, rA), (1, rA, rM)):
+            want = [j for j in range(n) if j not in excl and max(lo_ - sij[j], 0.0) <= r[i, j] < hi_ + sij[j]]
             want.sort(key=lambda j: (key[j], j))
             assert o.row(which, i).tolist() == want
         want = [j for j in range(n) if in_universe(cell[i], cell[j])]
