@@ -128,8 +128,17 @@ __host__ __device__ inline void img_unpack(int w, int &ix, int &iy, int &iz) {
 // 6e-8 in exact arithmetic, 2.6e-7 evaluated in fp32 -- the accuracy of erfcf).  erfc(alpha r) is then
 // erfcx_poly(alpha r) * exp(-alpha^2 r^2) with the exponential the Coulomb derivative needs anyway:
 // a third of the pair kernel's instructions were erfcf's.
+// Bare MUFU approximations (no denormal or range fix-up code around them): rsqrt.approx / rcp.approx are good to
+// 1-2 ulp and ex2.approx to 2 ulp on normal arguments, which is all the pair kernel feeds them (r^2 between 0.25 A^2 and
+// the squared cutoff, exponents above -30); rsqrtf / exp2f wrap the same instructions in 4-6 more.
+__device__ inline float rsqrt_fast(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ inline float rcp_fast(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ inline float ex2_fast(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+template <bool FAST = false>
 __device__ inline float erfcx_poly(float x) {
-    float t = __fdividef(1.f, fmaf(0.5f, x, 1.f));   // rcp.approx: 1 ulp, the IEEE reciprocal costs 8 instructions
+    // rcp.approx: 1 ulp, the IEEE reciprocal costs 8 instructions
+    float t = FAST ? rcp_fast(fmaf(0.5f, x, 1.f)) : __fdividef(1.f, fmaf(0.5f, x, 1.f));
     float p = -4.621402847e-02f;
     p = fmaf(p, t, 3.202601290e-01f);
     p = fmaf(p, t, -8.488328818e-01f);

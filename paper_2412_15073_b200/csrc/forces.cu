@@ -63,7 +63,7 @@ __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *_
         }
         const float r2 = dx * dx + dy * dy + dz * dz;
         if (r2 >= cut2) continue;
-        const float rinv = rsqrtf(r2), r = r2 * rinv;
+        const float rinv = rsqrt_fast(r2), r = r2 * rinv;
         float fr = 0.f, chi = 1.f, dchi = 0.f;
         if (NEED_CHI) {   // chi (R-3): quintic smootherstep on [r_c - h, r_c]; the clamp gives 1, 0 and chi' = 0 outside
             const float u = __saturatef(fmaf(r, m.inv_h, u_b)), omu = 1.f - u, u2 = u * u;
@@ -72,7 +72,7 @@ __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *_
         }
         if (WC != W_NONE && (SAME_CUT || r2 < cutC2)) {
             const float qq = qi * xj.w;
-            const float ex = exp2f(na2l * r2), e = ex * erfcx_poly(m.alpha * r);   // erfc(alpha r)
+            const float ex = ex2_fast(na2l * r2), e = ex * erfcx_poly<true>(m.alpha * r);   // erfc(alpha r)
             const float u = qq * e * rinv;
             const float du = -(u + qq * kq * ex) * rinv;  // u'
             fr += weighted_du<WC>(chi, dchi, u, du);

@@ -88,7 +88,9 @@ def test_long_run_averages_jump_vs_baoab_vs_oracle(jb, jo):
     # as extra friction, so the diffusion constant is NOT expected to agree (eps -> 0 recovers the
     # Hamiltonian kicks): both are checked for sanity only.
     assert abs(T["jump"][0] - 300.0) < 15.0 and abs(T["baoab"][0] - 300.0) < 15.0
-    assert ob.agree(U["jump"], U["baoab"], 4.0, slack=0.05), (U["jump"], U["baoab"])
+    # The mean potential energies differ by the two splittings' O(delta^2) biases: 0.13 - 0.17 kcal/mol per molecule at
+    # delta = 1 fs in repeated runs, 0.03 at 0.5 fs (the next test checks that order); the slack is that bias, not noise.
+    assert ob.agree(U["jump"], U["baoab"], 4.0, slack=0.2), (U["jump"], U["baoab"])
     sj, sb = res["jump"][1].std(), res["baoab"][1].std()          # width of the energy distribution (heat capacity)
     assert abs(sj / sb - 1.0) < 0.3, (sj, sb)
     assert gj.max() > 2.0 and 2.6 < r[gj.argmax()] < 3.0          # first O-O peak of liquid water
@@ -97,7 +99,7 @@ def test_long_run_averages_jump_vs_baoab_vs_oracle(jb, jo):
 
 
 def test_jump_baoab_energy_gap_is_time_step_bias(jb):
-    """The potential energy of JUMP sits about 0.1 kcal/mol per molecule above BAOAB's at delta = 1 fs (flexible O-H
+    """The potential energy of JUMP sits 0.13 - 0.17 kcal/mol per molecule above BAOAB's at delta = 1 fs (flexible O-H
     bonds: omega delta = 0.7; BAOAB's velocities at the kick points are colder than 300 K by (omega delta)^2 terms and
     the jumps resample velocity components at exactly 300 K there).  Both schemes are second order in delta (P:L125:
     "the discretization bias on the invariant measure is of order delta^2"), so the gap must shrink about fourfold at
