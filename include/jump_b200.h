@@ -157,6 +157,23 @@ int jump_get_images(jump_ctx *c, int32_t *d_img);
 int jump_vacf_mark(jump_ctx *c);
 int jump_vacf_dot(jump_ctx *c, int32_t lj_only, double *c_out);
 int jump_rdf_accumulate(jump_ctx *c, int32_t lj_only, double r_max, int32_t n_bins, uint64_t *d_hist);
+/* The same sum for callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * no context, no cudaMalloc / cudaFree, the per-CTA partial sums in a 256 KiB file-scope device array of the library
+ * (held by every GPU that loads the library until the process exits).
+ *   d_v_now, d_v_origin  DEVICE, n x 3 packed floats (the layout of d_vel), the same atom order in both
+ *   d_select             DEVICE, n int32 (non-zero = atom counts), or NULL = all atoms
+ *   d_out                DEVICE, 2 doubles: (1/N_sel) sum_{i in sel} v_i(origin) . v_i(now) (0 if N_sel = 0), and N_sel
+ *   stream               cudaStream_t the two kernels are enqueued on (asynchronous; nothing is synchronised)
+ * n > JUMP_VACF_STATIC_MAX_ATOMS, n <= 0 or a null array: JUMP_E_ARG, nothing launched; text in
+ * jump_vacf_static_last_error() (per host thread).  All calls on a device share the scratch array: calls that overlap
+ * on the GPU (different streams without a dependency) race; calls on one stream, or ordered by events, do not.  The
+ * array needs no clearing between calls.  jump_vacf_static_setup() takes the array's device address for the CURRENT
+ * device (once per device; the first jump_vacf_dot_static on a device does it too -- call it before a graph capture). */
+#define JUMP_VACF_STATIC_MAX_ATOMS 4194304
+int jump_vacf_static_setup(void);
+int jump_vacf_dot_static(int32_t n, const float *d_v_now, const float *d_v_origin, const int32_t *d_select, double *d_out,
+                         void *stream);
+const char *jump_vacf_static_last_error(void);
 /* Bounds as used (R-7, R-10c): G_A, G_B, GV_A, qmax, eps_max, sig_min, sig_max, r_M, G_C, GV_B, GV_C, r_A (G: sup of the
  * long Coulomb gradient per unit charges over a ring, GV: of the long LJ gradient with 4 eps = 1). */
 int jump_get_bounds(jump_ctx *c, double out[12]);

@@ -22,7 +22,8 @@ EXPORTS = ["jump_init", "jump_step", "baoab_step", "jump_respa_step", "jump_get_
            "jump_get_stats", "jump_reset_stats", "jump_get_events", "jump_clear_events", "jump_get_row", "jump_get_images", "jump_rdf_accumulate",
            "jump_get_bounds", "jump_refresh", "jump_refresh_lazy", "jump_half", "jump_sync", "jump_get_step", "jump_get_launches",
            "jump_last_error", "jump_free", "jump_set_profiling", "jump_get_profile", "jump_count_pairs",
-           "jump_ewald_setup", "jump_respa1_step", "jump_get_slow_energy", "jump_vacf_mark", "jump_vacf_dot", "jump_set_lanes", "jump_set_lax_skin"]
+           "jump_ewald_setup", "jump_respa1_step", "jump_get_slow_energy", "jump_vacf_mark", "jump_vacf_dot", "jump_set_lanes", "jump_set_lax_skin",
+           "jump_vacf_static_setup", "jump_vacf_dot_static", "jump_vacf_static_last_error"]
 
 
 class jump_params(C.Structure):
@@ -107,6 +108,10 @@ def lib():
         L.jump_count_pairs.argtypes = [vp, i32, C.c_double, C.POINTER(i64)]
         L.jump_set_lanes.argtypes = [vp, i32]
         L.jump_set_lax_skin.argtypes = [vp, i32]
+        L.jump_vacf_static_setup.argtypes = []
+        L.jump_vacf_dot_static.argtypes = [i32, vp, vp, vp, vp, vp]
+        L.jump_vacf_static_last_error.argtypes = []
+        L.jump_vacf_static_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -130,6 +135,31 @@ def make_params(n_atoms, box, r_short, r_long, r_switch=0.5, r_mid=None, ewald_a
 
 class JumpError(RuntimeError):
     pass
+
+
+VACF_STATIC_MAX_ATOMS = 4194304
+
+
+def vacf_dot_static(v_now, v_origin, out, select=None, stream=None):
+    """jump_vacf_dot_static: (1/N_sel) sum v_i(origin) . v_i(now) and N_sel into `out` (2 float64 on the device) with no
+    allocation by the library (scratch in a static device array; at most VACF_STATIC_MAX_ATOMS atoms).  v_now,
+    v_origin: contiguous (n, 3) float32 CUDA tensors; select: (n,) int32 or None.  Asynchronous on `stream`."""
+    import torch
+    for t in (v_now, v_origin):
+        assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.dim() == 2 and t.shape[1] == 3
+    assert v_now.shape == v_origin.shape and out.is_cuda and out.dtype == torch.float64 and out.numel() == 2 and out.is_contiguous()
+    if select is not None:
+        assert select.is_cuda and select.dtype == torch.int32 and select.is_contiguous() and select.numel() == v_now.shape[0]
+    st = stream if stream is not None else torch.cuda.current_stream(v_now.device)
+    L = lib()
+    with torch.cuda.device(v_now.device):
+        rc = L.jump_vacf_dot_static(int(v_now.shape[0]), C.c_void_p(v_now.data_ptr()), C.c_void_p(v_origin.data_ptr()),
+                                    C.c_void_p(select.data_ptr() if select is not None else 0), C.c_void_p(out.data_ptr()),
+                                    C.c_void_p(st.cuda_stream))
+    if rc < 0:
+        raise JumpError("jump_vacf_dot_static failed: %d (%s) %s" % (rc, ERRORS.get(rc, "?"),
+                                                                     (L.jump_vacf_static_last_error() or b"").decode()))
+    return out
 
 
 class JumpSim:

@@ -7,7 +7,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libjump_b200.so")
-SOURCES = ["api.cu", "sort_build.cu", "forces.cu", "update.cu", "observe.cu", "ewald.cu"]
+SOURCES = ["api.cu", "sort_build.cu", "forces.cu", "update.cu", "observe.cu", "ewald.cu", "vacf_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
