@@ -314,6 +314,7 @@ def main():
     ap.add_argument("--skin", type=float, default=None)
     ap.add_argument("--nlist-every", type=int, default=None)
     ap.add_argument("--eps-jump", type=float, default=None)
+    ap.add_argument("--cell-edge", type=float, default=None, help="edge of the contract grid's cells, A (default: the library's)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -330,7 +331,7 @@ def main():
     sysd, run = wl.make_config(args.config)
     run = dict(run, seed=replicas.rank_seed(run["seed"], rank))       # independent replicas
     for key, val in (("r_mid", args.r_mid), ("r_mid_in", args.r_mid_in), ("skin", args.skin), ("nlist_every", args.nlist_every),
-                     ("eps_jump", args.eps_jump)):
+                     ("eps_jump", args.eps_jump), ("cell_edge", args.cell_edge)):
         if val is not None:
             run[key] = val
     n, dt_fs = sysd["n_atoms"], run["dt_fs"]

@@ -47,7 +47,28 @@ struct Counters {
     int max_row[N_ROWS];
     int go_step;            // step stamp of the last displacement trigger (k_update): the list kernels enqueued for that step run
     unsigned int rebuilds;  // sorts done (counted on the device: the host does not know which conditional ones ran)
+    int work_next[2], work_done[2];   // work queues of the resident-grid kernels (0 row build, 1 universe): next item, CTAs finished; 0 at rest
 };
+
+// Resident grid with a work queue: the CTAs of a grid that just fills the GPU take item numbers from a counter until
+// they run out -- the load balance of one CTA per item without its launch cost, which for the list kernels is paid
+// at EVERY step (they are always enqueued and return at once unless the step's displacement trigger armed them; a
+// 131 072-CTA grid takes 70 us just to return).  The last CTA out puts the counters back to 0.
+__device__ inline int work_fetch(Counters *ctr, int which, int *s_item) {
+    __syncthreads();   // everybody has read the previous item (and is done with the shared memory of its work)
+    if (threadIdx.x == 0) *s_item = atomicAdd(&ctr->work_next[which], 1);
+    __syncthreads();
+    return *s_item;
+}
+__device__ inline void work_leave(Counters *ctr, int which) {
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(&ctr->work_done[which], 1) == (int)gridDim.x - 1) {
+            ctr->work_next[which] = 0;
+            ctr->work_done[which] = 0;
+        }
+    }
+}
 
 // constants of the physical model, passed by value to kernels
 struct Model {

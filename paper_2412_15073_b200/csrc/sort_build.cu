@@ -225,15 +225,13 @@ struct Stencil {
 
 // MASK >= 0: bit k set = row k is built (compile-time row set of the common modes); MASK < 0: rows.r[k].enabled decides
 template <int MASK, bool FAST>
-__global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGrid g, RowSet rows, Stencil stn, float rmax_all, int CX,
-                                                              const int *__restrict__ cell_start,
-                                                              const float4 *__restrict__ xs, const float4 *__restrict__ xl,
-                                                              const float2 *__restrict__ lj, const float2 *__restrict__ hw,
-                                                              const int *__restrict__ orig, const int *__restrict__ sorted_of,
-                                                              const int *__restrict__ excl_ptr, const int *__restrict__ excl_idx,
-                                                              Counters *ctr, int *__restrict__ cell_of, float far2,
-                                                              const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
+__device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid &g, const RowSet &rows, const Stencil &stn, float rmax_all,
+                                                 int CX, const int *__restrict__ cell_start, const float4 *__restrict__ xs,
+                                                 const float4 *__restrict__ xl, const float2 *__restrict__ lj,
+                                                 const float2 *__restrict__ hw, const int *__restrict__ orig,
+                                                 const int *__restrict__ sorted_of, const int *__restrict__ excl_ptr,
+                                                 const int *__restrict__ excl_idx, Counters *ctr, int *__restrict__ cell_of,
+                                                 float far2, const int bid) {
     __shared__ int seg_beg[BUILD_MAXSEG];       // stencil runs in ascending cell key (many are empty) ...
     __shared__ int seg_pre[BUILD_MAXSEG + 1];   // ... their lengths, then (length << 10 | non-empty) prefix sums
     __shared__ int run_beg[BUILD_MAXSEG];       // the non-empty runs, compacted: first atom ...
@@ -247,9 +245,9 @@ __global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGr
     // the CTA's home: CX consecutive cells along x (their atoms are contiguous in the sorted array)
     const int nbx = (g.gn[0] + CX - 1) / CX;
     int c3[3];
-    c3[0] = (blockIdx.x % nbx) * CX;
-    c3[1] = (blockIdx.x / nbx) % g.gn[1];
-    c3[2] = blockIdx.x / (nbx * g.gn[1]);
+    c3[0] = (bid % nbx) * CX;
+    c3[1] = (bid / nbx) % g.gn[1];
+    c3[2] = bid / (nbx * g.gn[1]);
     const int ncx = min(CX, g.gn[0] - c3[0]);
     const int cell0 = (c3[2] * g.gn[1] + c3[1]) * g.gn[0] + c3[0];
     const int a_beg = cell_start[cell0], a_end = cell_start[cell0 + ncx];
@@ -313,6 +311,20 @@ __global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGr
     const float rmax2t = rmax_all * rmax_all + BUILD_TIE;
     const unsigned lt_mask = (1u << lane) - 1u;
 #define JB_ROW_ON(k) (MASK >= 0 ? (((MASK) >> (k)) & 1) != 0 : rows.r[k].enabled != 0)
+    // window constants of the rows, read once (the compile-time row sets also know which rows have a lower edge: A, B, W;
+    // and that only W counts it from r - s_ij)
+#define JB_HAS_LO(k) (MASK >= 0 ? ((k) == ROW_A || (k) == ROW_B || (k) == ROW_W) : e_lo[k] > 0.f)
+#define JB_LO_PLUS(k) (MASK >= 0 ? (k) == ROW_W : rows.r[k].lo_plus != 0)
+    float e_hi[N_ROWS], e_lo[N_ROWS];
+    int e_cap[N_ROWS];
+#pragma unroll
+    for (int k = 0; k < N_ROWS; ++k) {
+        e_hi[k] = JB_ROW_ON(k) ? rows.r[k].rb : 0.f;
+        e_lo[k] = JB_ROW_ON(k) ? rows.r[k].ra : 0.f;
+        e_cap[k] = JB_ROW_ON(k) ? rows.r[k].cap : 0;
+    }
+    const float4 *const tile_l = tile + lane;   // this lane's column of the staged chunk
+    const float *const tile_wl = tile_w + lane;
     for (int g0 = a_beg; g0 < a_end; g0 += BUILD_MAXATOMS) {   // one pass unless a cell holds > BUILD_MAXATOMS atoms
         const int g1 = min(g0 + BUILD_MAXATOMS, a_end);
         for (int t = tid; t < BUILD_MAXATOMS * N_ROWS; t += BUILD_THREADS) (&s_count[0][0])[t] = 0;
@@ -397,7 +409,7 @@ __global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGr
 #define JB_ROW_SCAN(k) (JB_ROW_ON(k) && (LJ_I || MASK < 0 || (k) != ROW_W))
 #define JB_LJ_ROW(k) (MASK >= 0 ? (k) == ROW_W : rows.r[k].lj_only != 0)   // W is the LJ-only row
                     for (int q0 = 0; q0 < npad; q0 += 32) {
-                        const float4 xj = tile[q0 + lane];
+                        const float4 xj = tile_l[q0];
                         const int jraw = __float_as_int(xj.w);
                         const int j = jraw & 0x7fffffff;
                         float dx, dy, dz;
@@ -425,8 +437,8 @@ __global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGr
                         const bool ljp = LJ_I && jraw < 0;
                         // window of this pair in row k: [ra - s_ij, rb + s_ij), s_ij = (skin/2)(w_i + w_j) (row W: from ra + s_ij),
                         // tested on r -/+ s_ij against the row's constants
-                        const float sij = hsw_i + tile_w[q0 + lane];
-                        const float r = r2 * rsqrtf(fmaxf(r2, 1e-12f));
+                        const float sij = hsw_i + tile_wl[q0];
+                        const float r = r2 * rsqrt_fast(fmaxf(r2, 1e-12f));
                         const float rm = r - sij, rp = r + sij;
                         bool pass[N_ROWS];
                         float edge_gap = 1e30f;   // distance of r to the nearest window edge of a scanned row
@@ -434,13 +446,12 @@ __global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGr
                         for (int k = 0; k < N_ROWS; ++k) {
                             pass[k] = false;
                             if (!JB_ROW_SCAN(k)) continue;
-                            const Row &R = rows.r[k];
-                            bool in = rm < R.rb;
-                            edge_gap = fminf(edge_gap, fabsf(rm - R.rb));
-                            if (R.ra > 0.f) {
-                                const float t = R.lo_plus ? rm : rp;
-                                in = in && t >= R.ra;
-                                edge_gap = fminf(edge_gap, fabsf(t - R.ra));
+                            bool in = rm < e_hi[k];
+                            edge_gap = fminf(edge_gap, fabsf(rm - e_hi[k]));
+                            if (JB_HAS_LO(k)) {
+                                const float t = JB_LO_PLUS(k) ? rm : rp;
+                                in = in && t >= e_lo[k];
+                                edge_gap = fminf(edge_gap, fabsf(t - e_lo[k]));
                             }
                             pass[k] = valid && (!JB_LJ_ROW(k) || ljp) && in;
                         }
@@ -474,7 +485,7 @@ __global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGr
                             const unsigned mask = __ballot_sync(full, pass[k]);
                             const int pos = count[k] + __popc(mask & lt_mask);
                             // rows the pair kernel reads carry j's LJ flag in bit 31; the jump rows A, B plain indices
-                            store_if(pass[k] && pos < rows.r[k].cap, rbase[k] + pos, (k == ROW_A || k == ROW_B) ? j : jraw);
+                            store_if(pass[k] && pos < e_cap[k], rbase[k] + pos, (k == ROW_A || k == ROW_B) ? j : jraw);
                             count[k] += __popc(mask);
                         }
                     }
@@ -502,6 +513,29 @@ __global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGr
         __syncthreads();   // before s_count is zeroed for the next group of atoms
     }
 #undef JB_ROW_ON
+#undef JB_HAS_LO
+#undef JB_LO_PLUS
+}
+
+// resident grid over the nblocks home-cell groups (work queue 0 of the counters)
+template <int MASK, bool FAST>
+__global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGrid g, RowSet rows, Stencil stn, float rmax_all, int CX,
+                                                              const int *__restrict__ cell_start,
+                                                              const float4 *__restrict__ xs, const float4 *__restrict__ xl,
+                                                              const float2 *__restrict__ lj, const float2 *__restrict__ hw,
+                                                              const int *__restrict__ orig, const int *__restrict__ sorted_of,
+                                                              const int *__restrict__ excl_ptr, const int *__restrict__ excl_idx,
+                                                              Counters *ctr, int *__restrict__ cell_of, float far2,
+                                                              const int *__restrict__ go, int want, int nblocks) {
+    if (go && *go != want) return;
+    __shared__ int s_item;
+    for (;;) {
+        const int bid = work_fetch(ctr, 0, &s_item);
+        if (bid >= nblocks) break;
+        build_rows_block<MASK, FAST>(m, g, rows, stn, rmax_all, CX, cell_start, xs, xl, lj, hw, orig, sorted_of, excl_ptr, excl_idx,
+                                     ctr, cell_of, far2, bid);
+    }
+    work_leave(ctr, 0);
 }
 
 // ---- cell universe of jump ring C (R-10c) -----------------------------------------------------------------------
@@ -510,9 +544,10 @@ __global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGr
 __global__ void __launch_bounds__(128) k_universe(SortGrid g, Universe u, const int *__restrict__ cell_start,
                                                   unsigned short *__restrict__ cum, Counters *ctr, const int *__restrict__ go, int want) {
     if (go && *go != want) return;
-    const int h = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (h >= g.ncell) return;
-    if (cell_start[h + 1] == cell_start[h]) return;   // no atom lives here: the row is never read
+    const int lane = threadIdx.x & 31, nwarp = (gridDim.x * blockDim.x) >> 5;
+    // resident grid, the cells dealt round-robin to its warps (equal work per cell; see work_fetch for why not a CTA per item)
+    for (int h = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; h < g.ncell; h += nwarp) {
+    if (cell_start[h + 1] == cell_start[h]) continue;   // no atom lives here: the row is never read
     const int cx = h % g.gn[0], cy = (h / g.gn[0]) % g.gn[1], cz = h / (g.gn[0] * g.gn[1]);
     unsigned short *out = cum + (size_t)h * u.stride;
     int run = 0;
@@ -538,6 +573,7 @@ __global__ void __launch_bounds__(128) k_universe(SortGrid g, Universe u, const 
         out[u.nrow] = (unsigned short)min(run, 65535);
         if (run >= 65535) atomicOr(&ctr->err, (unsigned)ERR_OVERFLOW);   // 16-bit running sums
     }
+    }
 }
 // the universe of one home cell as a list of sorted indices (observer: jump_get_row), one thread per entry, through the
 // same lookup the jump chains use
@@ -548,6 +584,19 @@ __global__ void k_universe_list(SortGrid g, Universe u, const int *__restrict__ 
 
 // ------------------------------------------------------------------------------------------
 static inline int nblk(int n, int b) { return (n + b - 1) / b; }
+// CTAs of a grid that fills the current device once with per_sm CTAs on every SM
+static int resident_ctas(int per_sm) {
+    static int sms[64] = {0};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    dev = std::max(0, std::min(dev, 63));
+    if (!sms[dev]) {
+        int v = 0;
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) v = 148;
+        sms[dev] = v;
+    }
+    return sms[dev] * per_sm;
+}
 
 void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches) {
     const int B = 256;
@@ -576,7 +625,8 @@ void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches) {
 void launch_universe(const SortGrid &g, const Universe &u, const int *cell_start, unsigned short *cum, Counters *ctr,
                      const int *go, int want, cudaStream_t st, int64_t *launches) {
     const int B = 128;
-    k_universe<<<(unsigned)(((long long)g.ncell * 32 + B - 1) / B), B, 0, st>>>(g, u, cell_start, cum, ctr, go, want);
+    const long long need = ((long long)g.ncell * 32 + B - 1) / B;
+    k_universe<<<(unsigned)std::min<long long>(need, resident_ctas(16)), B, 0, st>>>(g, u, cell_start, cum, ctr, go, want);
     *launches += 1;
 }
 int launch_universe_list(const SortGrid &g, const Universe &u, const int *cell_start, int home, int *out, int n,
@@ -616,13 +666,14 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
     // FAST: staged coordinates relative to the cell centre, no minimum image in the inner loop (see k_build_rows)
     bool fast = true;
     for (int k = 0; k < 3; ++k) fast = fast && ((double)rmax_all + 0.5 * cs[k] * (k == 0 ? CX : 1) <= 0.5 * (double)m.box[k]) && m.box[k] <= 512.f;
-    const unsigned nblocks = (unsigned)(((g.gn[0] + CX - 1) / CX) * g.gn[1] * g.gn[2]);
+    const int nblocks = ((g.gn[0] + CX - 1) / CX) * g.gn[1] * g.gn[2];
+    const unsigned ngrid = (unsigned)std::min(nblocks, resident_ctas(7));
 #define JB_BUILD(MASK)                                                                                                        \
     do {                                                                                                                      \
-        if (fast) k_build_rows<MASK, true><<<nblocks, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, hw, \
-                                                                                       orig, sorted_of, excl_ptr, excl_idx, ctr, cell_of, far2, go, want); \
-        else k_build_rows<MASK, false><<<nblocks, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, hw, \
-                                                                                    orig, sorted_of, excl_ptr, excl_idx, ctr, cell_of, far2, go, want);   \
+        if (fast) k_build_rows<MASK, true><<<ngrid, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, hw, \
+                                                                                     orig, sorted_of, excl_ptr, excl_idx, ctr, cell_of, far2, go, want, nblocks); \
+        else k_build_rows<MASK, false><<<ngrid, BUILD_THREADS, 0, st>>>(m, g, rs, stn, rmax_all, CX, cell_start, xs, xl, lj, hw, \
+                                                                                  orig, sorted_of, excl_ptr, excl_idx, ctr, cell_of, far2, go, want, nblocks);   \
     } while (0)
     switch (mask) {
         case 0x07: JB_BUILD(0x07); break;   // S A B     (JUMP with Coulomb and LJ jumps)
