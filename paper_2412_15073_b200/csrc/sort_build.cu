@@ -211,7 +211,7 @@ __device__ __forceinline__ void store_if(bool ok, int *p, int v) {
 //     decision (R-17) and the fp32 value of r^2 (error < 1e-3 A^2) would flip it where the fp64 oracle does not.
 constexpr int BUILD_THREADS = 128;
 constexpr int BUILD_WARPS = BUILD_THREADS / 32;
-constexpr int BUILD_CX_MAX = 2;            // home cells per CTA (consecutive along x): 1 on small grids, more when the grid is large
+constexpr int BUILD_CX_MAX = 4;            // home cells per CTA (consecutive along x): 1 on small grids, more when the grid is large
 constexpr int BUILD_CHUNK = 1024;           // candidates staged per pass
 constexpr int BUILD_MAXSEG = 2 * 17 * 17;   // two x-runs per (z, y) cell row of the stencil
 constexpr int BUILD_MAXATOMS = 32;          // atoms of a cell whose running counts are held at once
@@ -240,6 +240,7 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
     __shared__ float tile_w[BUILD_CHUNK];       // (skin/2) w_j: the candidate's share of the pair's skin (R-10c)
     __shared__ int scan_tmp[BUILD_THREADS];
     __shared__ int s_count[BUILD_MAXATOMS][N_ROWS];
+    __shared__ int s_queue[BUILD_WARPS][64];    // per warp: slots of the candidates that passed the distance filter
     const unsigned full = 0xffffffffu;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // the CTA's home: CX consecutive cells along x (their atoms are contiguous in the sorted array)
@@ -324,7 +325,6 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
         e_cap[k] = JB_ROW_ON(k) ? rows.r[k].cap : 0;
     }
     const float4 *const tile_l = tile + lane;   // this lane's column of the staged chunk
-    const float *const tile_wl = tile_w + lane;
     for (int g0 = a_beg; g0 < a_end; g0 += BUILD_MAXATOMS) {   // one pass unless a cell holds > BUILD_MAXATOMS atoms
         const int g1 = min(g0 + BUILD_MAXATOMS, a_end);
         for (int t = tid; t < BUILD_MAXATOMS * N_ROWS; t += BUILD_THREADS) (&s_count[0][0])[t] = 0;
@@ -408,10 +408,15 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                     constexpr bool LJ_I = decltype(lj_tag)::value;
 #define JB_ROW_SCAN(k) (JB_ROW_ON(k) && (LJ_I || MASK < 0 || (k) != ROW_W))
 #define JB_LJ_ROW(k) (MASK >= 0 ? (k) == ROW_W : rows.r[k].lj_only != 0)   // W is the LJ-only row
-                    for (int q0 = 0; q0 < npad; q0 += 32) {
-                        const float4 xj = tile_l[q0];
-                        const int jraw = __float_as_int(xj.w);
-                        const int j = jraw & 0x7fffffff;
+                    // Two passes per 32 candidates.  Filter: distance only; the slots of the candidates within reach
+                    // of the largest window go, in order, to a 64-entry ring buffer of the warp.  Windows: whenever 32
+                    // are waiting they are taken off the buffer, one per lane -- every lane of the expensive part
+                    // (window tests, ties, ballot compaction) then carries a candidate that can be listed, where
+                    // the chunk itself has them in 4 lanes out of 10.  The buffer keeps the candidates' order, and so
+                    // do the rows.
+                    int *const que = s_queue[warp];
+                    int q_head = 0, q_n = 0;
+                    auto dist2 = [&](const float4 &xj) {
                         float dx, dy, dz;
                         if (FAST) { dx = xi - xj.x; dy = yi - xj.y; dz = zi - xj.z; }
                         else {
@@ -419,9 +424,16 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                             dy = min_image1(yi, xj.y, m.box[1], m.inv_box[1]);
                             dz = min_image1(zi, xj.z, m.box[2], m.inv_box[2]);
                         }
-                        const float r2 = dx * dx + dy * dy + dz * dz;
-                        bool valid = r2 < rmax2t;   // false for the NaN of a padding entry
-                        if (!__any_sync(full, valid)) continue;
+                        return dx * dx + dy * dy + dz * dz;
+                    };
+                    auto windows = [&](const int n_live) {
+                        __syncwarp();
+                        const int slot = lane < n_live ? que[(q_head + lane) & 63] : 0;
+                        const float4 xj = tile[slot];
+                        const int jraw = __float_as_int(xj.w);
+                        const int j = jraw & 0x7fffffff;
+                        const float r2 = dist2(xj);
+                        bool valid = lane < n_live;
                         const bool nearby = valid && r2 <= exr2;
                         if (__any_sync(full, nearby)) {   // the atom itself and excluded pairs are never listed (R-9)
                             bool ex = (j == i) | (j == ex4[0]) | (j == ex4[1]) | (j == ex4[2]) | (j == ex4[3]);
@@ -437,7 +449,7 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                         const bool ljp = LJ_I && jraw < 0;
                         // window of this pair in row k: [ra - s_ij, rb + s_ij), s_ij = (skin/2)(w_i + w_j) (row W: from ra + s_ij),
                         // tested on r -/+ s_ij against the row's constants
-                        const float sij = hsw_i + tile_wl[q0];
+                        const float sij = hsw_i + tile_w[slot];
                         const float r = r2 * rsqrt_fast(fmaxf(r2, 1e-12f));
                         const float rm = r - sij, rp = r + sij;
                         bool pass[N_ROWS];
@@ -488,7 +500,17 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                             store_if(pass[k] && pos < e_cap[k], rbase[k] + pos, (k == ROW_A || k == ROW_B) ? j : jraw);
                             count[k] += __popc(mask);
                         }
+                        __syncwarp();   // the slots just read may be written again
+                    };
+                    for (int q0 = 0; q0 < npad; q0 += 32) {
+                        const bool within = dist2(tile_l[q0]) < rmax2t;   // false for the NaN of a padding entry
+                        const unsigned wmask = __ballot_sync(full, within);
+                        if (wmask == 0u) continue;
+                        if (within) que[(q_head + q_n + __popc(wmask & lt_mask)) & 63] = q0 + lane;
+                        q_n += __popc(wmask);
+                        if (q_n >= 32) { windows(32); q_head = (q_head + 32) & 63; q_n -= 32; }
                     }
+                    if (q_n > 0) windows(q_n);
 #undef JB_ROW_SCAN
 #undef JB_LJ_ROW
                 };
@@ -662,7 +684,8 @@ void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS]
     for (int k = 0; k < N_ROWS; ++k) mask |= rows[k].enabled ? (1 << k) : 0;
     // home cells per CTA: staging is shared by more atoms and the warps are better balanced, as long as the grid
     // still gives every SM several waves of CTAs
-    const int CX = std::max(1, std::min(BUILD_CX_MAX, g.ncell / 4000));
+    // (measured on the 10^6-atom box: a home about 10 A long is best -- 5.6 ms per build against 6.0 at 7 A and 6.5 at 27 A)
+    const int CX = std::max(1, std::min(std::min(BUILD_CX_MAX, (int)(11.0 / cs[0])), g.ncell / 4000));
     // FAST: staged coordinates relative to the cell centre, no minimum image in the inner loop (see k_build_rows)
     bool fast = true;
     for (int k = 0; k < 3; ++k) fast = fast && ((double)rmax_all + 0.5 * cs[k] * (k == 0 ? CX : 1) <= 0.5 * (double)m.box[k]) && m.box[k] <= 512.f;

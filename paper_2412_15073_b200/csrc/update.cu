@@ -200,7 +200,7 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, const ChainConst &c
 // ---- the fused per-atom update: up to two velocity half-phases, then A O A + wrap ----------------------------
 // G lanes per atom (a power of two <= 32) share the atom's jump chains; lane 0 of the group does A-O-A and the stores.
 template <bool JUMPS, int G, bool LOG, bool ADAPT>
-__global__ void __launch_bounds__(128, 6) k_update(Model m, UpdateArgs A) {
+__global__ void __launch_bounds__(128, 8) k_update(Model m, UpdateArgs A) {
     const unsigned full = 0xffffffffu;
     const int gt_id = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gt_id / G, gl = gt_id % G;
