@@ -187,6 +187,20 @@ __device__ inline float near_image1(float d, float L, float invL) {
     return fmaf(-L, t, d);
 }
 
+// Shared-memory accesses of the filter loop through 32-bit shared-space addresses that the compiler must keep in
+// registers (JB_KEEP makes a value opaque): left to itself, under the 72-register cap of 7 CTAs per SM, it
+// recomputes lane, masks, the squared reach and the generic addresses of the tile and the queue in every iteration
+// -- 18 of the loop's 47 instructions.
+#define JB_KEEP(x) asm volatile("" : "+r"(x))
+#define JB_KEEPF(x) asm volatile("" : "+f"(x))
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ float4 lds128(unsigned a) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void sts32(unsigned a, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+
 // *p = v under a predicate, as ONE predicated store (the compiler's branch around a conditional store costs a
 // convergence barrier pair and a jump per row and chunk in the row build's inner loop)
 __device__ __forceinline__ void store_if(bool ok, int *p, int v) {
@@ -324,7 +338,12 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
         e_lo[k] = JB_ROW_ON(k) ? rows.r[k].ra : 0.f;
         e_cap[k] = JB_ROW_ON(k) ? rows.r[k].cap : 0;
     }
-    const float4 *const tile_l = tile + lane;   // this lane's column of the staged chunk
+    unsigned tile_a = smem_u32(tile) + 16u * (unsigned)lane;   // this lane's column of the staged chunk
+    unsigned que_a = smem_u32(s_queue[warp]);
+    unsigned lt_keep = lt_mask;
+    float reach2 = rmax2t;
+    int lane_keep = lane;
+    JB_KEEP(tile_a); JB_KEEP(que_a); JB_KEEP(lt_keep); JB_KEEPF(reach2); JB_KEEP(lane_keep);
     for (int g0 = a_beg; g0 < a_end; g0 += BUILD_MAXATOMS) {   // one pass unless a cell holds > BUILD_MAXATOMS atoms
         const int g1 = min(g0 + BUILD_MAXATOMS, a_end);
         for (int t = tid; t < BUILD_MAXATOMS * N_ROWS; t += BUILD_THREADS) (&s_count[0][0])[t] = 0;
@@ -367,6 +386,7 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                     yi = near_image1(yi - ctr3[1], m.box[1], m.inv_box[1]);
                     zi = near_image1(zi - ctr3[2], m.box[2], m.inv_box[2]);
                 }
+                JB_KEEPF(xi); JB_KEEPF(yi); JB_KEEPF(zi);   // (else recomputed from xs[i] in every iteration of the scan)
                 const bool lj_i = lj[i].y > 0.f;
                 const float2 hw_i = hw[i];
                 const float hsw_i = hw_i.x;   // (skin/2) w_i
@@ -503,10 +523,10 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                         __syncwarp();   // the slots just read may be written again
                     };
                     for (int q0 = 0; q0 < npad; q0 += 32) {
-                        const bool within = dist2(tile_l[q0]) < rmax2t;   // false for the NaN of a padding entry
+                        const bool within = dist2(lds128(tile_a + 16u * (unsigned)q0)) < reach2;   // false for the NaN of a padding entry
                         const unsigned wmask = __ballot_sync(full, within);
                         if (wmask == 0u) continue;
-                        if (within) que[(q_head + q_n + __popc(wmask & lt_mask)) & 63] = q0 + lane;
+                        if (within) sts32(que_a + 4u * (unsigned)((q_head + q_n + __popc(wmask & lt_keep)) & 63), q0 + lane_keep);
                         q_n += __popc(wmask);
                         if (q_n >= 32) { windows(32); q_head = (q_head + 32) & 63; q_n -= 32; }
                     }
