@@ -196,9 +196,10 @@ __device__ inline float near_image1(float d, float L, float invL) {
 __device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ float4 lds128(unsigned a) {
     float4 v;
-    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a) : "memory");
     return v;
 }
+__device__ __forceinline__ int lds32(unsigned a) { int v; asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
 __device__ __forceinline__ void sts32(unsigned a, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 
 // *p = v under a predicate, as ONE predicated store (the compiler's branch around a conditional store costs a
@@ -343,7 +344,8 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
     unsigned lt_keep = lt_mask;
     float reach2 = rmax2t;
     int lane_keep = lane;
-    JB_KEEP(tile_a); JB_KEEP(que_a); JB_KEEP(lt_keep); JB_KEEPF(reach2); JB_KEEP(lane_keep);
+    unsigned tilew_a = smem_u32(tile_w);
+    JB_KEEP(tile_a); JB_KEEP(que_a); JB_KEEP(lt_keep); JB_KEEPF(reach2); JB_KEEP(lane_keep); JB_KEEP(tilew_a);
     for (int g0 = a_beg; g0 < a_end; g0 += BUILD_MAXATOMS) {   // one pass unless a cell holds > BUILD_MAXATOMS atoms
         const int g1 = min(g0 + BUILD_MAXATOMS, a_end);
         for (int t = tid; t < BUILD_MAXATOMS * N_ROWS; t += BUILD_THREADS) (&s_count[0][0])[t] = 0;
@@ -434,7 +436,6 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                     // (window tests, ties, ballot compaction) then carries a candidate that can be listed, where
                     // the chunk itself has them in 4 lanes out of 10.  The buffer keeps the candidates' order, and so
                     // do the rows.
-                    int *const que = s_queue[warp];
                     int q_head = 0, q_n = 0;
                     auto dist2 = [&](const float4 &xj) {
                         float dx, dy, dz;
@@ -448,12 +449,12 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                     };
                     auto windows = [&](const int n_live) {
                         __syncwarp();
-                        const int slot = lane < n_live ? que[(q_head + lane) & 63] : 0;
-                        const float4 xj = tile[slot];
+                        const int slot = lane_keep < n_live ? lds32(que_a + 4u * (unsigned)((q_head + lane_keep) & 63)) : 0;
+                        const float4 xj = lds128(tile_a + 16u * (unsigned)(slot - lane_keep));
                         const int jraw = __float_as_int(xj.w);
                         const int j = jraw & 0x7fffffff;
                         const float r2 = dist2(xj);
-                        bool valid = lane < n_live;
+                        bool valid = lane_keep < n_live;
                         const bool nearby = valid && r2 <= exr2;
                         if (__any_sync(full, nearby)) {   // the atom itself and excluded pairs are never listed (R-9)
                             bool ex = (j == i) | (j == ex4[0]) | (j == ex4[1]) | (j == ex4[2]) | (j == ex4[3]);
@@ -469,7 +470,7 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                         const bool ljp = LJ_I && jraw < 0;
                         // window of this pair in row k: [ra - s_ij, rb + s_ij), s_ij = (skin/2)(w_i + w_j) (row W: from ra + s_ij),
                         // tested on r -/+ s_ij against the row's constants
-                        const float sij = hsw_i + tile_w[slot];
+                        const float sij = hsw_i + __int_as_float(lds32(tilew_a + 4u * (unsigned)slot));
                         const float r = r2 * rsqrt_fast(fmaxf(r2, 1e-12f));
                         const float rm = r - sij, rp = r + sij;
                         bool pass[N_ROWS];
