@@ -27,9 +27,9 @@ extern "C" {
 #define JUMP_E_CUDA (-2)     /* CUDA runtime error, see jump_last_error */
 #define JUMP_E_OVERFLOW (-3) /* a neighbour/ring row or the event buffer overflowed its capacity */
 #define JUMP_E_BOUND (-4)    /* thinning bound violated: an acceptance probability p > 1 was seen */
-#define JUMP_E_SKIN (-5)     /* an atom moved more than skin/2 since the last list build at a step where no list build could
-                                follow: the lists may have missed a pair (R-10c).  Checked on the device at every step;
-                                lower nlist_every or raise skin.  With JUMP_F_LAX_SKIN only jump_stats.max_disp reports it. */
+#define JUMP_E_SKIN (-5)     /* an atom moved more than its share of the skin within min(3, nlist_every/4) steps of a list
+                                build (or with nlist_every = 0): the lists may have missed a pair (R-10c).  Checked on the
+                                device at every step; raise skin.  With JUMP_F_LAX_SKIN only jump_stats.max_disp reports it. */
 #define JUMP_E_NAN (-6)      /* non-finite position or velocity */
 
 #define JUMP_F_COUL_JUMPS 1u       /* Coulomb tail r_c..r_long by jumps (step C', Alg. 4) */
@@ -50,9 +50,9 @@ typedef struct {
     int32_t eps_mode;    /* 0 = constant epsilon = eps_jump (Alg. 4); 1 = adaptive eps(x) = eps_jump |F_ij(x)| (
                             DESIGN.md R-19), eps_jump finite, in A mol/kcal */
     uint32_t flags;      /* JUMP_F_* */
-    int32_t nlist_every; /* P: all lists are rebuilt at every P-th step, and -- decided on the device, step by step -- at a
-                            step of the second half of such an interval as soon as an atom has moved more than skin/2
-                            since the last build (R-10c); 0: never after init */
+    int32_t nlist_every; /* P: all lists are rebuilt P steps after their last build at the latest, and -- decided on the
+                            device, step by step -- from min(3, P/4) steps after it on as soon as an atom has moved more
+                            than its share of the skin since then (R-10c); 0: never after init */
     int32_t pad0;
     uint64_t seed;       /* Philox4x32-10 key (R-15) */
     double box[3];       /* orthorhombic periodic box edges, A */

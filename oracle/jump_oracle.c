@@ -126,6 +126,7 @@ typedef struct {
     double GV, GV2, GV3; /* the same for the long LJ gradient with 4 eps = 1 (R-10: GV alone, over the whole shell) */
     int gnx, gny, gnz; /* contract grid for the canonical row order */
     int policy;        /* list policy (orc_params.list_policy) */
+    long long last_build; /* step count at the last list build (R-10c schedule) */
     int bound_every;   /* R-11: 1 = B_v and lambda-bar re-evaluated at every proposal, as Algorithm 4 prints them */
     /* R-10c cell universe, built at x_build: atoms of every contract cell (ascending index) and the cell of every atom */
     int *cell_ptr, *cell_atoms, *home, *uni_cnt;
@@ -777,6 +778,7 @@ static void rebuild_universe(orc_ctx *c) {
 static int universe_count(const orc_ctx *c, int i) { return c->uni_cnt[c->home[i]]; }
 
 static void rebuild_rows(orc_ctx *c) {
+    c->last_build = c->step;
     free(c->ptrM); free(c->idxM); free(c->ptrL); free(c->idxL); free(c->ptrV); free(c->idxV);
     c->ptrL = c->idxL = c->ptrV = c->idxV = NULL;
     double s = c->skin, lo = c->rc - c->h - s;
@@ -1119,13 +1121,15 @@ static void aoa_and_lists(orc_ctx *c) {
     wrap_all(c);
     c->step++;
     const double mx = check_displacement(c);
-    /* R-10c list schedule: every P = nlist_every steps at the latest, and -- from step P/4 of such an interval on -- as
-     * soon as some atom has used up its share of the skin, w_i skin/2, since the last build (the lists are supersets
+    /* R-10c list schedule, counted from the LAST build: P = nlist_every steps after it at the latest, and -- from
+     * Q = min(3, P/4) steps after it on -- as soon as some atom has used up its share of the skin, w_i skin/2 (the lists are supersets
      * of what they must hold while no atom has; water, skin 1 A: 6 to 9 steps).  The test on the displacement is
-     * one more discontinuous decision (R-17): its margin is audited with those of the lists. */
+     * one more discontinuous decision (R-17): its margin is audited with those of the lists.  (Round-1 policy 0:
+     * every P-th step, nothing else.) */
     const int P = c->p.nlist_every;
-    int rebuild = P > 0 && c->step % P == 0;
-    if (!rebuild && c->policy == 1 && P > 0 && c->step % P >= (P >= 4 ? P / 4 : 1)) {
+    const long long age = c->step - c->last_build;
+    int rebuild = P > 0 && (c->policy == 1 ? age >= P : c->step % P == 0);
+    if (!rebuild && c->policy == 1 && P > 0 && age >= (P >= 12 ? 3 : (P >= 4 ? P / 4 : 1))) {
         const double e = fabs(mx - 0.5 * c->skin);
         if (e < c->st.min_list_margin) { c->st.min_list_margin = e; c->st.min_list_margin_step = c->step; }
         rebuild = mx > 0.5 * c->skin;

@@ -254,7 +254,7 @@ static int resort_and_build(jump_ctx *c, bool conditional) {
     }
     // rows that nobody has read for a while leave the active set (they are built again on demand)
     for (int k = 0; k < N_ROWS; ++k)
-        if (c->row_active[k] && c->step - c->row_last_use[k] > 3 * (int64_t)std::max(c->p.nlist_every, 1)) c->row_active[k] = false;
+        if (c->row_active[k] && c->step - c->row_last_use[k] > 36) c->row_active[k] = false;
     return build_rows(c, c->row_active, go, stamp);
 }
 
@@ -397,14 +397,15 @@ static int run_update(jump_ctx *c, const Phase &p0, GradRef g0, const Phase &p1,
     A.rowA = c->rows[ROW_A]; A.rowB = c->rows[ROW_B];
     A.uni = c->uni; A.grid = c->g; A.cell_start = c->cell_start; A.xl_all = c->xl; A.excl_ptr = c->excl_ptr; A.excl_idx = c->excl_idx;
     A.lanes = c->lanes;
-    // R-10c list schedule: every P = nlist_every steps at the latest; from step P/4 of such an interval on the update kernel
-    // arms a conditional build as soon as an atom has used up its share of the skin (before that: the error JUMP_E_SKIN)
+    // R-10c list schedule, counted from the last build: P = nlist_every steps after it at the latest; from Q = min(3, P/4)
+    // steps after it on as soon as an atom has used up its share of the skin (before that: the error JUMP_E_SKIN).  The update kernel
+    // decides (only the device knows when the last build was); the list kernels are enqueued behind it at every step.
     const int P = c->p.nlist_every;
     const int64_t next = c->step + 1;
-    const bool scheduled = aoa && P > 0 && next % P == 0;
-    const bool will_check = scheduled || (aoa && P > 0 && next % P >= (P >= 4 ? P / 4 : 1));
-    A.trigger = scheduled ? 2 : (will_check ? 1 : 0);   // 2: a list build follows anyway (no error, nothing to arm)
+    const bool will_check = aoa && P > 0;
+    A.trigger = will_check ? 1 : 0;
     A.step_id = (int)next;
+    A.list_P = P; A.list_Q = P >= 12 ? 3 : (P >= 4 ? P / 4 : 1);
     A.ctr = c->ctr; A.events = (c->p.flags & JUMP_F_EVENT_LOG) ? c->events : nullptr; A.event_cap = c->event_cap;
     bool jumps = (p0.kind == 2 || p1.kind == 2) && (coul_jumps(c) || lj_jumps(c));
     if (jumps) {
@@ -422,7 +423,7 @@ static int run_update(jump_ctx *c, const Phase &p0, GradRef g0, const Phase &p1,
         c->f0_valid = false;
         c->slow_valid = false;
         c->step++;
-        if (will_check) return resort_and_build(c, !scheduled);
+        if (will_check) return resort_and_build(c, true);
     }
     return 0;
 }
@@ -1094,9 +1095,9 @@ extern "C" int jump_reset_stats(jump_ctx *c) {
     CK(cudaStreamSynchronize(c->st));
     const unsigned long long ne = h.n_events;
     const unsigned nr = h.rebuilds;
-    const int gs = h.go_step;
+    const int gs = h.go_step, lb = h.last_build;
     memset(&h, 0, sizeof h);
-    h.n_events = ne; h.rebuilds = nr; h.go_step = gs;
+    h.n_events = ne; h.rebuilds = nr; h.go_step = gs; h.last_build = lb;
     CK(cudaMemcpyAsync(c->ctr, &h, sizeof h, cudaMemcpyHostToDevice, c->st));
     CK(cudaStreamSynchronize(c->st));
     c->sticky = 0; c->err.clear();

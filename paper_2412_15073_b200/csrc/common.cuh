@@ -47,6 +47,7 @@ struct Counters {
     int max_row[N_ROWS];
     int go_step;            // step stamp of the last displacement trigger (k_update): the list kernels enqueued for that step run
     unsigned int rebuilds;  // sorts done (counted on the device: the host does not know which conditional ones ran)
+    int last_build;         // step count at the last sort + list build (the list schedule counts from it, R-10c)
     int work_next[2], work_done[2];   // work queues of the resident-grid kernels (0 row build, 1 universe): next item, CTAs finished; 0 at rest
 };
 

@@ -49,9 +49,11 @@ struct UpdateArgs {
     jump_event *events;  // NULL: no log
     long long event_cap;
     int lanes;           // lanes per jump chain (0: chosen from the grid size)
-    int trigger;         // 1: a conditional list build follows this launch, a displacement beyond skin/2 arms it; 2: an
-                         // unconditional one follows; 0: none follows, such a displacement is the error ERR_SKIN
+    int trigger;         // 1: a conditional list build follows this launch and this kernel decides whether it runs (R-10c:
+                         // list_P steps after the last build, or from list_Q steps after it on when an atom is beyond its share
+                         // of the skin); 0: none follows.  A displacement beyond skin/2 that arms nothing is the error ERR_SKIN
     int step_id;         // the stamp it is armed with
+    int list_P, list_Q;
 };
 
 struct EwaldArgs {   // reciprocal Ewald sum (ewald.cu, R-21)

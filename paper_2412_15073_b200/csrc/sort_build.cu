@@ -150,7 +150,7 @@ __global__ void k_permute(int n, const int *__restrict__ src, const int *__restr
     if (go && *go != want) return;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    if (i == 0) ctr->rebuilds += 1;
+    if (i == 0) { ctr->rebuilds += 1; ctr->last_build = want; }
     int s = src[i];
     const int kk = key[s];   // home cell, packed by coordinates (the universe lookup wants them without divisions)
     cell_of[i] = pack_cell(kk % gnx, (kk / gnx) % gny, kk / (gnx * gny));

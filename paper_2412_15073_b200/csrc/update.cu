@@ -310,7 +310,6 @@ __global__ void __launch_bounds__(128, 8) k_update(Model m, UpdateArgs A) {
     __syncthreads();
     unsigned err = 0;
     if (bad) err |= ERR_NAN;
-    if (disp2 > m.half_skin2 && !A.trigger) err |= ERR_SKIN;   // (with a conditional list build behind this launch it arms that instead)
     if (tl.max_p > 1.f + 1e-4f || tl.max_gl > 1.f + 1e-4f) err |= ERR_BOUND;
     unsigned d2b = __reduce_max_sync(full, __float_as_uint(disp2));
     err = __reduce_or_sync(full, err);
@@ -343,8 +342,13 @@ __global__ void __launch_bounds__(128, 8) k_update(Model m, UpdateArgs A) {
             if (s_stat[5] > A.ctr->max_gl_bits) atomicMax(&A.ctr->max_gl_bits, s_stat[5]);
         }
         if (s_stat[6] > A.ctr->max_disp2_bits) atomicMax(&A.ctr->max_disp2_bits, s_stat[6]);
-        // some atom is farther than skin/2 from where the lists saw it: the list kernels enqueued behind this launch run
-        if (A.trigger == 1 && __uint_as_float(s_stat[6]) > m.half_skin2) A.ctr->go_step = A.step_id;
+        // R-10c list schedule, decided here: the list kernels enqueued behind this launch run if the lists are list_P steps
+        // old, or (from list_Q steps on) if some atom of this CTA is farther than its share of the skin from where they
+        // saw it; such an atom with nothing to arm is an error
+        const bool over = __uint_as_float(s_stat[6]) > m.half_skin2;
+        const int age = A.trigger ? A.step_id - A.ctr->last_build : 0;
+        if (A.trigger && (age >= A.list_P || (over && age >= A.list_Q))) A.ctr->go_step = A.step_id;
+        else if (over) s_stat[7] |= ERR_SKIN;
         if (s_stat[7]) atomicOr(&A.ctr->err, s_stat[7]);
     }
 }

@@ -230,7 +230,7 @@ def make_config(k, temperature=300.0):
     run = dict(r_short=cfg["r_short"], r_long=cfg["r_long"], r_switch=0.5, r_mid=cfg["r_short"] + 2.0,
                r_mid_in=cfg["r_short"] + 0.25,
                ewald_alpha=-1.0, dt_fs=cfg["dt_fs"], gamma_per_ps=1.0, temperature_K=temperature,
-               n_inner=cfg["n_inner"], eps_jump=1.0, eps_mode=0, flags=3, skin=1.0, nlist_every=12,
+               n_inner=cfg["n_inner"], eps_jump=1.0, eps_mode=0, flags=3, skin=1.0, nlist_every=24,
                seed=3000 + k, cell_edge=0.0)
     return sysd, run
 
