@@ -11,15 +11,14 @@
 #include <cmath>
 #include <type_traits>
 
+#include <cooperative_groups.h>
 #include "launch.h"
 
 namespace jb {
 
-__global__ void k_cell_key(int n, const float4 *__restrict__ xs, SortGrid g, int *__restrict__ key,
-                           int *__restrict__ cell_count, Counters *ctr, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
+// The per-element bodies of the sort passes are device functions: the large-box path runs each pass as a kernel of its
+// own, the small-box path (k_sort_small) all of them in one CTA.
+__device__ __forceinline__ void cell_key_one(int i, const float4 *xs, const SortGrid &g, int *key, int *cell_count, Counters *ctr) {
     float4 x = xs[i];
     if (!(isfinite(x.x) && isfinite(x.y) && isfinite(x.z))) {
         atomicOr(&ctr->err, (unsigned)ERR_NAN);
@@ -36,11 +35,16 @@ __global__ void k_cell_key(int n, const float4 *__restrict__ xs, SortGrid g, int
     key[i] = k;
     atomicAdd(&cell_count[k], 1);
 }
-
-// exclusive scan of cell_count[0..ncell) into cell_start[0..ncell]; one block
-__global__ void k_scan(int ncell, const int *__restrict__ cell_count, int *__restrict__ cell_start, const int *__restrict__ go, int want) {
+__global__ void k_cell_key(int n, const float4 *__restrict__ xs, SortGrid g, int *__restrict__ key,
+                           int *__restrict__ cell_count, Counters *ctr, const int *__restrict__ go, int want) {
     if (go && *go != want) return;
-    __shared__ int part[1024];
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    cell_key_one(i, xs, g, key, cell_count, ctr);
+}
+
+// exclusive scan of cell_count[0..ncell) into cell_start[0..ncell]; one block (part: blockDim.x ints of shared memory)
+__device__ __forceinline__ void scan_block(int ncell, const int *cell_count, int *cell_start, int *part) {
     int t = threadIdx.x, nt = blockDim.x;
     int per = (ncell + nt - 1) / nt;
     int lo = min(t * per, ncell), hi = min(lo + per, ncell);
@@ -60,6 +64,11 @@ __global__ void k_scan(int ncell, const int *__restrict__ cell_count, int *__res
         run += cell_count[k];
     }
     if (t == nt - 1) cell_start[ncell] = part[t];
+}
+__global__ void k_scan(int ncell, const int *__restrict__ cell_count, int *__restrict__ cell_start, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
+    __shared__ int part[1024];
+    scan_block(ncell, cell_count, cell_start, part);
 }
 
 // the same scan for large grids, in three small launches: per-block sums of 4096-cell slices, a scan of the
@@ -106,24 +115,24 @@ __global__ void k_scan_slices(int ncell, const int *__restrict__ cell_count, con
     if (lo <= ncell - 1 && ncell - 1 < lo + 4) cell_start[ncell] = run;
 }
 
+__device__ __forceinline__ void scatter_one(int i, const int *key, const int *orig, const int *cell_start, int *cell_fill,
+                                            int *tmp_orig, int *tmp_src) {
+    int k = key[i];
+    int slot = cell_start[k] + atomicAdd(&cell_fill[k], 1);
+    tmp_orig[slot] = orig[i];
+    tmp_src[slot] = i;
+}
 __global__ void k_scatter(int n, const int *__restrict__ key, const int *__restrict__ orig,
                           const int *__restrict__ cell_start, int *__restrict__ cell_fill,
                           int *__restrict__ tmp_orig, int *__restrict__ tmp_src, const int *__restrict__ go, int want) {
     if (go && *go != want) return;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    int k = key[i];
-    int slot = cell_start[k] + atomicAdd(&cell_fill[k], 1);
-    tmp_orig[slot] = orig[i];
-    tmp_src[slot] = i;
+    scatter_one(i, key, orig, cell_start, cell_fill, tmp_orig, tmp_src);
 }
 
 // order each cell by original index (insertion sort; a cell holds a handful of atoms)
-__global__ void k_cell_sort(int ncell, const int *__restrict__ cell_start, int *__restrict__ tmp_orig,
-                            int *__restrict__ tmp_src, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= ncell) return;
+__device__ __forceinline__ void cell_sort_one(int c, const int *cell_start, int *tmp_orig, int *tmp_src) {
     int lo = cell_start[c], hi = cell_start[c + 1];
     for (int a = lo + 1; a < hi; ++a) {
         int ko = tmp_orig[a], ks = tmp_src[a];
@@ -136,6 +145,13 @@ __global__ void k_cell_sort(int ncell, const int *__restrict__ cell_start, int *
         tmp_orig[b + 1] = ko;
         tmp_src[b + 1] = ks;
     }
+}
+__global__ void k_cell_sort(int ncell, const int *__restrict__ cell_start, int *__restrict__ tmp_orig,
+                            int *__restrict__ tmp_src, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
+    int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncell) return;
+    cell_sort_one(c, cell_start, tmp_orig, tmp_src);
 }
 
 __global__ void k_permute(int n, const int *__restrict__ src, const int *__restrict__ new_orig,
@@ -584,13 +600,9 @@ __global__ void __launch_bounds__(BUILD_THREADS, 7) k_build_rows(Model m, SortGr
 // ---- cell universe of jump ring C (R-10c) -----------------------------------------------------------------------
 // One warp per home cell: the lengths of its stencil rows (two cell_start differences each), prefix-summed into
 // cum[h][0 .. nrow]; cum[h][nrow] is the size of the universe, N_C of every atom of the cell.
-__global__ void __launch_bounds__(128) k_universe(SortGrid g, Universe u, const int *__restrict__ cell_start,
-                                                  unsigned short *__restrict__ cum, Counters *ctr, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    const int lane = threadIdx.x & 31, nwarp = (gridDim.x * blockDim.x) >> 5;
-    // resident grid, the cells dealt round-robin to its warps (equal work per cell; see work_fetch for why not a CTA per item)
-    for (int h = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; h < g.ncell; h += nwarp) {
-    if (cell_start[h + 1] == cell_start[h]) continue;   // no atom lives here: the row is never read
+__device__ __forceinline__ void universe_cell(const SortGrid &g, const Universe &u, const int *cell_start, unsigned short *cum,
+                                              Counters *ctr, int h, int lane) {
+    if (cell_start[h + 1] == cell_start[h]) return;   // no atom lives here: the row is never read
     const int cx = h % g.gn[0], cy = (h / g.gn[0]) % g.gn[1], cz = h / (g.gn[0] * g.gn[1]);
     unsigned short *out = cum + (size_t)h * u.stride;
     int run = 0;
@@ -616,7 +628,13 @@ __global__ void __launch_bounds__(128) k_universe(SortGrid g, Universe u, const 
         out[u.nrow] = (unsigned short)min(run, 65535);
         if (run >= 65535) atomicOr(&ctr->err, (unsigned)ERR_OVERFLOW);   // 16-bit running sums
     }
-    }
+}
+__global__ void __launch_bounds__(128) k_universe(SortGrid g, Universe u, const int *__restrict__ cell_start,
+                                                  unsigned short *__restrict__ cum, Counters *ctr, const int *__restrict__ go, int want) {
+    if (go && *go != want) return;
+    const int lane = threadIdx.x & 31, nwarp = (gridDim.x * blockDim.x) >> 5;
+    // resident grid, the cells dealt round-robin to its warps (equal work per cell; see work_fetch for why not a CTA per item)
+    for (int h = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; h < g.ncell; h += nwarp) universe_cell(g, u, cell_start, cum, ctr, h, lane);
 }
 // the universe of one home cell as a list of sorted indices (observer: jump_get_row), one thread per entry, through the
 // same lookup the jump chains use
@@ -626,6 +644,50 @@ __global__ void k_universe_list(SortGrid g, Universe u, const int *__restrict__ 
 }
 
 // ------------------------------------------------------------------------------------------
+// Small boxes: the whole sort in ONE cooperative launch (zero the counts, keys, scan, scatter, per-cell order, permute,
+// copy back, the running sums of the cell universe, with grid-wide barriers between the passes).  On a 12 000-atom box
+// the step is a chain of launches of a few microseconds each, and the list kernels are enqueued at every step to return
+// at once on most of them: one such launch instead of nine (two memsets and seven kernels).  Plain pointers on purpose:
+// the passes read what earlier passes of the same kernel wrote, which the read-only data path would not see.
+constexpr int SORT_SMALL_THREADS = 512, SORT_SMALL_CTAS = 32;
+constexpr int SORT_SMALL_MAX_ATOMS = 32768, SORT_SMALL_MAX_CELLS = 16384;
+__global__ void __launch_bounds__(SORT_SMALL_THREADS) k_sort_small(SortArgs a, Universe u, unsigned short *cum) {
+    if (a.go && *a.go != a.want) return;   // (every CTA takes the same way: nobody is left waiting at a barrier)
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    __shared__ int part[SORT_SMALL_THREADS];
+    const int t = blockIdx.x * SORT_SMALL_THREADS + threadIdx.x, nt = gridDim.x * SORT_SMALL_THREADS, n = a.n, ncell = a.grid.ncell;
+    for (int c = t; c <= ncell; c += nt) { a.cell_count[c] = 0; a.cell_fill[c] = 0; }
+    grid.sync();
+    for (int i = t; i < n; i += nt) cell_key_one(i, a.xs, a.grid, a.key, a.cell_count, a.ctr);
+    grid.sync();
+    if (blockIdx.x == 0) scan_block(ncell, a.cell_count, a.cell_start, part);
+    grid.sync();
+    for (int i = t; i < n; i += nt) scatter_one(i, a.key, a.orig, a.cell_start, a.cell_fill, a.tmp_orig, a.tmp_src);
+    grid.sync();
+    for (int c = t; c < ncell; c += nt) cell_sort_one(c, a.cell_start, a.tmp_orig, a.tmp_src);
+    grid.sync();
+    if (t == 0) { a.ctr->rebuilds += 1; a.ctr->last_build = a.want; }
+    const int gnx = a.grid.gn[0], gny = a.grid.gn[1];
+    for (int i = t; i < n; i += nt) {
+        const int s = a.tmp_src[i], kk = a.key[s];
+        a.cell_of[i] = pack_cell(kk % gnx, (kk / gnx) % gny, kk / (gnx * gny));
+        const float4 x = a.xs[s];
+        a.xs_t[i] = x; a.x_build[i] = x;
+        a.vs_t[i] = a.vs[s]; a.xl_t[i] = a.xl[s]; a.lj_t[i] = a.lj[s]; a.hw_t[i] = a.hw[s]; a.mi_t[i] = a.mi[s];
+        const int o = a.tmp_orig[i];
+        a.orig_t[i] = o;
+        a.sorted_of[o] = i;
+    }
+    grid.sync();
+    for (int i = t; i < n; i += nt) {
+        a.xs[i] = a.xs_t[i]; a.vs[i] = a.vs_t[i]; a.xl[i] = a.xl_t[i]; a.lj[i] = a.lj_t[i]; a.mi[i] = a.mi_t[i]; a.hw[i] = a.hw_t[i];
+        a.orig[i] = a.orig_t[i];
+    }
+    if (!cum) return;
+    // running sums of the cell universe (k_universe's pass), one warp per home cell: reads cell_start only
+    for (int h = t >> 5; h < ncell; h += nt >> 5) universe_cell(a.grid, u, a.cell_start, cum, a.ctr, h, t & 31);
+}
+
 static inline int nblk(int n, int b) { return (n + b - 1) / b; }
 // CTAs of a grid that fills the current device once with per_sm CTAs on every SM
 static int resident_ctas(int per_sm) {
@@ -641,8 +703,18 @@ static int resident_ctas(int per_sm) {
     return sms[dev] * per_sm;
 }
 
-void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches) {
+// uni_cum != NULL: the running sums of the cell universe are wanted too; returns true if this call made them (small
+// boxes), false if launch_universe has to follow
+bool launch_sort(const SortArgs &a, const Universe &u, unsigned short *uni_cum, cudaStream_t st, int64_t *launches) {
     const int B = 256;
+    if (a.n <= SORT_SMALL_MAX_ATOMS && a.grid.ncell <= SORT_SMALL_MAX_CELLS) {
+        SortArgs aa = a;
+        Universe uu = u;
+        void *args[] = {(void *)&aa, (void *)&uu, (void *)&uni_cum};
+        cudaLaunchCooperativeKernel((const void *)k_sort_small, dim3(SORT_SMALL_CTAS), dim3(SORT_SMALL_THREADS), args, 0, st);
+        *launches += 1;
+        return true;
+    }
     cudaMemsetAsync(a.cell_count, 0, sizeof(int) * (a.grid.ncell + 1), st);   // (scratch: harmless when the sort does not run)
     cudaMemsetAsync(a.cell_fill, 0, sizeof(int) * (a.grid.ncell + 1), st);
     k_cell_key<<<nblk(a.n, B), B, 0, st>>>(a.n, a.xs, a.grid, a.key, a.cell_count, a.ctr, a.go, a.want);
@@ -663,6 +735,7 @@ void launch_sort(const SortArgs &a, cudaStream_t st, int64_t *launches) {
     k_copyback<<<nblk(a.n, B), B, 0, st>>>(a.n, a.xs_t, a.vs_t, a.xl_t, a.lj_t, a.mi_t, a.hw_t, a.hw, a.orig_t, a.xs, a.vs, a.xl, a.lj, a.mi, a.orig,
                                            a.go, a.want);
     *launches += 6;
+    return false;
 }
 
 void launch_universe(const SortGrid &g, const Universe &u, const int *cell_start, unsigned short *cum, Counters *ctr,
