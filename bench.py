@@ -180,7 +180,7 @@ def timed_blocks(torch, sim, stream, call, n_steps, block, flush):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures of
 # `python bench.py --steps 40 --warmup 8 --equil 60 --no-cpu-baseline --secondary-config -1` on the default workload
 # (profiles/r2_cfg4_README.md, profiles/r2_cfg4_dram_bytes.csv); other workloads have no capture: null
-NCU_TRAFFIC_CFG4 = {}
+NCU_TRAFFIC_CFG4 = {"pair": 652.9e6, "update": 927.0e6, "build": 2215.1e6, "bonded": 42.6e6}   # build: k_build_rows + k_universe
 BONDED_BYTES_PER_ATOM = 56    # per water: 16 B record + 3 x (16 + 16 B read, 16 B written)
 
 
@@ -236,7 +236,7 @@ def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, pro
     n_upd = max(prof["update"][1], 1)
     chains = 2.0 * n * (2 if run["flags"] & 2 else 1)                  # half-phases x (C' [+ J']) per jump update launch
     upd_instr = pstats["proposals"] / n_upd * PROPOSAL_INSTR + chains * CHAIN_INSTR
-    build_ms = prof["build"][0] / rebuilds                             # sort (7 kernels) + k_universe + k_build_rows, per rebuild
+    build_ms = prof["build"][0] / rebuilds                             # sort + k_universe + k_build_rows (and their idle launches), per rebuild
     lines = {
         "pair": alu_line("k_pair (short-range switched pair gradient, a5)", half_pairs * FLOPS_PER_PAIR,
                          "%.0f in-range half pairs x %d flop" % (half_pairs, FLOPS_PER_PAIR), "pair"),

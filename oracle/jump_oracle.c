@@ -71,6 +71,9 @@
 #define ORC_F_RESPA_PAPER 8u
 #define ORC_F_RESPA_COMPARATOR 16u
 #define ORC_F_BJAOAJB 64u /* jump_step runs B J A O A J B instead of C'J' A O A J'C' */
+#define ORC_F_COMBINED 128u /* ONE mechanism per pair for the whole long pair gradient, Coulomb + LJ, in step (C'); no (J')
+                               (R-22; P:L78-84 a mechanism per force piece F_i, P:L342 F_ij any pair term; needs
+                               flags 1 | 2 and list_policy 1) */
 
 /* weight modes of a pair term */
 enum { W_NONE = 0, W_SHORT = 1, W_LONG = 2, W_FULL = 3 };
@@ -389,7 +392,7 @@ static void neighbor_csr_audit(const orc_ctx *c, const double *x, double rmin, d
     }
     int *cnt = calloc(n + 1, sizeof(int));
     uint64_t **rows = malloc(sizeof(uint64_t *) * n);
-#pragma omp parallel for schedule(dynamic, 64) reduction(min : emin)
+#pragma omp parallel for if (c->n >= 64) schedule(dynamic, 64) reduction(min : emin)
     for (int i = 0; i < n; ++i) {
         int cap = 64, m = 0;
         uint64_t *row = malloc(sizeof(uint64_t) * cap);
@@ -491,7 +494,7 @@ static double pairs_accumulate(const orc_ctx *c, int wC, int wLJ, int brute, dou
     int *ptr, *idx;
     neighbor_csr(c, c->x, 0.0, rmax, 0, brute, &ptr, &idx);
     double etot = 0.0;
-#pragma omp parallel for schedule(dynamic, 64) reduction(+ : etot)
+#pragma omp parallel for if (c->n >= 64) schedule(dynamic, 64) reduction(+ : etot)
     for (int i = 0; i < c->n; ++i) {
         double acc[3] = {0, 0, 0}, e = 0.0;
         for (int k = ptr[i]; k < ptr[i + 1]; ++k) {
@@ -895,15 +898,17 @@ typedef struct {
                         rlo < 0 (R-10): ring membership is list membership */
 } orc_ring;
 
-/* the rings of atom i for the Coulomb (lj = 0) or the LJ (lj = 1) jumps; returns their number */
+/* the rings of atom i for the Coulomb (lj = 0), the LJ (lj = 1) or the combined (lj = 2, R-22) jumps; returns their number */
 static int rings_of(const orc_ctx *c, int i, int lj, orc_ring R[3]) {
     const double cq = fabs(c->q[i]) * c->qmax, ce = 4.0 * sqrt(c->eps[i] * c->eps_max); /* uniform in j: P:L346, L369, L455 */
     const int nA = c->ptrM[i + 1] - c->ptrM[i];
     if (c->policy == 1) { /* R-10c: A = [r_c - h, r_A), B = [r_A, r_M) from the rows, L = [r_M, r_long) from the universe */
         const int nB = c->ptrL[i + 1] - c->ptrL[i], nU = universe_count(c, i);
-        R[0] = (orc_ring){0, nA, lj ? ce * c->GV : cq * c->GM, c->rc - c->h, c->rA};
-        R[1] = (orc_ring){1, nB, lj ? ce * c->GV2 : cq * c->GL, c->rA, c->rM};
-        R[2] = (orc_ring){3, nU, lj ? ce * c->GV3 : cq * c->G3, c->rM, c->rE};
+        /* lj = 2 (R-22): the pair gradient is the sum of the two long parts, bounded by the sum of their bounds */
+        const double fq = lj == 1 ? 0.0 : cq, fe = lj == 0 ? 0.0 : ce;
+        R[0] = (orc_ring){0, nA, fq * c->GM + fe * c->GV, c->rc - c->h, c->rA};
+        R[1] = (orc_ring){1, nB, fq * c->GL + fe * c->GV2, c->rA, c->rM};
+        R[2] = (orc_ring){3, nU, fq * c->G3 + fe * c->GV3, c->rM, c->rE};
         return 3;
     }
     if (lj) { R[0] = (orc_ring){2, c->ptrV[i + 1] - c->ptrV[i], ce * c->GV, -1.0, 0.0}; return 1; }
@@ -920,16 +925,28 @@ static int ring_candidate(const orc_ctx *c, int i, const orc_ring *R, int k) {
     }
 }
 
-/* lj = 0: step (C') for atom i, general mechanism (6),(7) with eps (or BPS, eps = inf), acceleration a between
+/* F_ij of the mechanism run by chain_atom: lj = 0 the long Coulomb gradient, 1 the long LJ gradient, 2 their sum (R-22) */
+static double fij_mode(const orc_ctx *c, int lj, int i, int j, double F[3]) {
+    if (lj == 0) return fij_coul(c, i, j, F);
+    if (lj == 1) return fij_lj(c, i, j, F);
+    double Fl[3];
+    fij_coul(c, i, j, F);
+    fij_lj(c, i, j, Fl);
+    for (int k = 0; k < 3; ++k) F[k] += Fl[k];
+    return sqrt(F[0] * F[0] + F[1] * F[1] + F[2] * F[2]);
+}
+
+/* lj = 2 (R-22, ORC_F_COMBINED): as lj = 0 with F_ij the whole long pair gradient and L_Y the sum of the two bounds.
+ * lj = 0: step (C') for atom i, general mechanism (6),(7) with eps (or BPS, eps = inf), acceleration a between
  * proposals.  lj = 1: step (J'), BPS (4),(5) on the long LJ part, a = 0 (the caller passes zeros): the same loop
  * with the constant bound beta |v| sum N_Y L_Y (|v| is preserved by reflections), so that the number of
  * proposals is Poisson as Algorithm 5 asks (R-14).
  * Draws of a proposal, from one Philox block (R-15): E, ring, k, U; G~ attempts draw from stream + 16. */
 static void chain_atom(orc_ctx *c, int i, int lj, double H, const double a[3], int stream, int64_t step,
                        int64_t *n_prop, int64_t *n_acc, int64_t *n_gt, int64_t *n_exp, double *max_p, double *max_gl) {
-    if (lj && !(c->eps[i] > 0.0)) return; /* no LJ on this atom: no chain */
+    if (lj == 1 && !(c->eps[i] > 0.0)) return; /* no LJ on this atom: no chain */
     double *v = &c->v[3 * i];
-    const double eps = lj ? INFINITY : c->p.eps_jump, sbm = c->sbm[i], beta = c->beta;
+    const double eps = lj == 1 ? INFINITY : c->p.eps_jump, sbm = c->sbm[i], beta = c->beta;
     const int bps = isinf(eps);
     /* R-19 (NEXT-1): eps_mode 1 = adaptive eps(x) = eps0 |F_ij(x)|, eps0 = eps_jump.  With
      * g = |F_ij| <= L_Y, eta = eps0 g sqrt(beta m)(v.n) and Theta(eta) <= eta_+ + 1/sqrt(2 pi) the pair rate
@@ -941,7 +958,7 @@ static void chain_atom(orc_ctx *c, int i, int lj, double H, const double a[3], i
     double S = 0.0; /* sum_Y N_Y L_Y */
     int ntot = 0;
     for (int y = 0; y < nr; ++y) { S += (double)R[y].n * R[y].L; ntot += R[y].n; }
-    if (lj && !(S > 0.0)) return; /* (J') without a partner: nothing to log, as under Algorithm 5 with N = 0 */
+    if (lj == 1 && !(S > 0.0)) return; /* (J') without a partner: nothing to log, as under Algorithm 5 with N = 0 */
     double t = 0.0;
     uint32_t block = 0;  /* proposal k of the chain draws Philox block k of its stream ...                     */
     uint32_t gblock = 0; /* ... and the G~ attempts draw blocks 0, 1, ... of stream + 16 (R-15)                 */
@@ -1007,11 +1024,11 @@ static void chain_atom(orc_ctx *c, int i, int lj, double H, const double a[3], i
         int j = ring_candidate(c, i, &R[ring], k);
         double LY = R[ring].L;
         double U = orc_u01(w[3]);
-        ev.ring = (lj ? 4 : 0) + ring; ev.j = j; ev.U = U;
+        ev.ring = 4 * lj + ring; ev.j = j; ev.U = U; /* ring codes 0-2 (C'), 4-6 (J'), 8-10 (combined) */
         (*n_prop)++;
         double F[3];
         double g = 0.0;
-        if (R[ring].rlo < 0.0) g = lj ? fij_lj(c, i, j, F) : fij_coul(c, i, j, F); /* R-10 */
+        if (R[ring].rlo < 0.0) g = fij_mode(c, lj, i, j, F); /* R-10 */
         else if (j != i && !(R[ring].kind == 3 && is_excluded(c, i, j))) {
             /* R-10c: the pair carries its force through the ring its CURRENT distance lies in; drawn
              * through another ring it has rate 0 -- every pair is counted exactly once.  The universe also holds
@@ -1021,7 +1038,7 @@ static void chain_atom(orc_ctx *c, int i, int lj, double H, const double a[3], i
             double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
             mg = upd(mg, r - R[ring].rlo);
             mg = upd(mg, r - R[ring].rhi);
-            if (r >= R[ring].rlo && r < R[ring].rhi) g = lj ? fij_lj(c, i, j, F) : fij_coul(c, i, j, F);
+            if (r >= R[ring].rlo && r < R[ring].rhi) g = fij_mode(c, lj, i, j, F);
         }
         if (g > 0.0) {
             if (g / LY > *max_gl) *max_gl = g / LY;
@@ -1053,15 +1070,15 @@ static void chain_atom(orc_ctx *c, int i, int lj, double H, const double a[3], i
 }
 
 /* C over all atoms; acc_src: gradient array giving a = -M^-1 F (NULL -> a = 0) */
-static void phase_C(orc_ctx *c, double H, const double *grad, int stream, int64_t step) {
+static void phase_C(orc_ctx *c, double H, const double *grad, int stream, int64_t step, int mode) {
     int64_t np = 0, nacc = 0, ngt = 0, nexp = 0;
     double mp = 0.0, mgl = 0.0;
-#pragma omp parallel for schedule(dynamic, 64) reduction(+ : np, nacc, ngt, nexp) reduction(max : mp, mgl)
+#pragma omp parallel for if (c->n >= 64) schedule(dynamic, 64) reduction(+ : np, nacc, ngt, nexp) reduction(max : mp, mgl)
     for (int i = 0; i < c->n; ++i) {
         double a[3] = {0, 0, 0};
         if (grad)
             for (int k = 0; k < 3; ++k) a[k] = -(ORC_KCAL / c->m[i]) * grad[3 * i + k];
-        chain_atom(c, i, 0, H, a, stream, step, &np, &nacc, &ngt, &nexp, &mp, &mgl);
+        chain_atom(c, i, mode, H, a, stream, step, &np, &nacc, &ngt, &nexp, &mp, &mgl);
     }
     c->st.proposals += np; c->st.accepts += nacc; c->st.gt_attempts += ngt; c->st.expiries += nexp;
     if (mp > c->st.max_p) c->st.max_p = mp;
@@ -1071,7 +1088,7 @@ static void phase_J(orc_ctx *c, double H, int stream, int64_t step) {
     int64_t np = 0, nacc = 0, ngt = 0, nexp = 0;
     double mp = 0.0, mgl = 0.0;
     const double zero[3] = {0.0, 0.0, 0.0};
-#pragma omp parallel for schedule(dynamic, 64) reduction(+ : np, nacc, ngt, nexp) reduction(max : mp, mgl)
+#pragma omp parallel for if (c->n >= 64) schedule(dynamic, 64) reduction(+ : np, nacc, ngt, nexp) reduction(max : mp, mgl)
     for (int i = 0; i < c->n; ++i) chain_atom(c, i, 1, H, zero, stream, step, &np, &nacc, &ngt, &nexp, &mp, &mgl);
     c->st.proposals += np; c->st.accepts += nacc; c->st.expiries += nexp;
     if (mp > c->st.max_p) c->st.max_p = mp;
@@ -1088,8 +1105,12 @@ static void phase_B(orc_ctx *c, double H, const double *grad) {
 /* C' then J' (fwd) or J' then C' (reverse) over a duration H */
 static void jump_phase(orc_ctx *c, double H, const double *grad, int sC, int sJ, int64_t step, int reverse) {
     int coul = (c->p.flags & ORC_F_COUL_JUMPS) != 0, lj = (c->p.flags & ORC_F_LJ_JUMPS) != 0;
+    if (c->p.flags & ORC_F_COMBINED) { /* R-22: one mechanism for the whole long pair gradient, no (J') */
+        phase_C(c, H, grad, sC, step, 2);
+        return;
+    }
     if (reverse && lj) phase_J(c, H, sJ, step);
-    if (coul) phase_C(c, H, grad, sC, step);
+    if (coul) phase_C(c, H, grad, sC, step, 0);
     else if (grad) phase_B(c, H, grad);
     if (!reverse && lj) phase_J(c, H, sJ, step);
 }

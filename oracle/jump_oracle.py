@@ -18,6 +18,7 @@ _LIB = os.path.join(_HERE, "libjump_oracle.so")
 
 F_COUL_JUMPS, F_LJ_JUMPS, F_EVENT_LOG, F_RESPA_PAPER, F_RESPA_COMPARATOR = 1, 2, 4, 8, 16
 F_BJAOAJB = 64
+F_COMBINED = 128   # one mechanism per pair for the whole long pair gradient in (C'), no (J') (R-22)
 
 
 def build(force=False):

@@ -47,6 +47,7 @@ if __name__ == "__main__":
         r = dict(run, flags=3 | 4, eps_jump=eps, eps_mode=mode)
         best("jump_step x100 eps=%s mode=%d" % (eps, mode), sysd, r, first, last)
     best("bjaoajb x20", sysd, dict(run, flags=3 | 4 | 64), first, last, chunks=2)
+    best("combined x100 (R-22)", sysd, dict(run, flags=3 | 4 | 128), first, last)
     for flags, mode in ((3, 0), (3 | 8, 0), (1, 0), (3, 1), (3 | 8, 1)):
         r = dict(run, flags=flags | 4, eps_mode=mode, eps_jump=2.0 if mode else run["eps_jump"])
         best("respa x3 flags=%d mode=%d" % (flags, mode), sysd, r, first, last, chunks=1, call=lambda o: o.jump_respa_step(3))

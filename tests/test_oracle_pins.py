@@ -771,12 +771,14 @@ def test_jump_and_baoab_sample_the_same_measure(relaxed_small):
     sysd, _ = relaxed_small
     run = dict(r_short=4.0, r_long=6.0, r_mid=5.0, skin=1.0, nlist_every=10, dt_fs=1.0, gamma_per_ps=1.0, eps_jump=1.0, flags=3)
     out = {}
-    for name, seed in (("jump", 11), ("baoab", 12), ("adaptive", 13), ("bjaoajb", 14)):
+    for name, seed in (("jump", 11), ("baoab", 12), ("adaptive", 13), ("bjaoajb", 14), ("combined", 15)):
         kw = dict(run, seed=seed)
         if name == "adaptive":                                 # eps(x) = eps0 |F_ij(x)| (R-19)
             kw.update(eps_mode=1, eps_jump=0.5)
         if name == "bjaoajb":                                  # B J A O A J B
             kw.update(flags=3 | jo.F_BJAOAJB)
+        if name == "combined":                                 # one mechanism for Coulomb + LJ (R-22)
+            kw.update(flags=3 | jo.F_COMBINED)
         o = jo.Oracle(sysd, **kw)
         step = o.baoab_step if name == "baoab" else o.jump_step
         step(1000)
@@ -799,7 +801,7 @@ def test_jump_and_baoab_sample_the_same_measure(relaxed_small):
     # the same bias in the mean potential energy: 0.09 - 0.1 kcal/mol per molecule in those runs (-1.61 against -1.70);
     # tests/test_gpu_longrun.py shows it falling fourfold at delta = 0.5 fs
     assert ob.agree(Uj, Ub, 4.0, slack=0.15), (Uj, Ub)       # kcal/mol per molecule
-    for name in ("adaptive", "bjaoajb"):
+    for name in ("adaptive", "bjaoajb", "combined"):
         Ta, Ua = out[name]
         assert ob.agree(Ta, Tb, 4.0, slack=12.0) and abs(Ta[0] - 300.0) < 20.0, (name, Ta, Tb)
         assert ob.agree(Ua, Ub, 4.0, slack=0.15), (name, Ua, Ub)
@@ -1071,3 +1073,70 @@ def test_vacf_of_the_O_step_is_exponential_and_its_spectrum_lorentzian():
     # one harmonic mode shows up as a line at its frequency
     line = jo.vacf_spectrum(np.cos(7.0 * tt), 1e-3, np.linspace(0.0, 14.0, 57))
     assert abs(np.linspace(0.0, 14.0, 57)[np.argmax(line)] - 7.0) < 0.3
+
+
+# ------------------------------------------------------------------------------------ NEXT-3: the combined mechanism (R-22)
+def test_combined_mechanism_drift_is_the_whole_long_gradient():
+    """R-22 (a jump mechanism per force piece F_ij; "both combined"): with F_COMBINED step (C')
+    runs ONE mechanism per pair whose F_ij is the sum of the long Coulomb and the long LJ gradient.  The mean-drift
+    identity (rate (6) x mean kick (7) = -F_ij/m) must then hold with the SUM: two like charges (Coulomb
+    repulsive, -1.9 kcal/mol/A along the pair axis) with a strong LJ attraction (+0.76) -- a dropped term gives -1.9 or
+    +0.76 and a sign error +-2.7 instead of -1.1."""
+    z = np.zeros(0)
+    sysd = dict(n_atoms=2, box=24.0, pos=np.array([[5.0, 5.0, 5.0], [10.0, 5.0, 5.0]]), vel=np.zeros((2, 3)),
+                mass=np.array([16.0, 12.0]), charge=np.array([0.5, 0.5]), lj_sigma=np.array([3.4, 3.4]),
+                lj_eps=np.array([2.0, 2.0]), bond_ij=np.zeros((0, 2), dtype=np.int32), bond_k=z, bond_r0=z,
+                angle_ijk=np.zeros((0, 3), dtype=np.int32), angle_k=z, angle_t0=z,
+                excl_ptr=np.zeros(3, dtype=np.int32), excl_idx=np.zeros(0, dtype=np.int32))
+    kw = dict(r_short=4.0, r_long=8.0, r_mid=6.0, skin=0.5, ewald_alpha=0.2, eps_jump=0.7, nlist_every=10 ** 9, seed=78)
+    parts = {}
+    for name, flags in (("coul", 1), ("both", 1 | 2)):          # forces(2): the long gradient the flags hand to the jumps
+        o = jo.Oracle(sysd, flags=flags, **kw)
+        parts[name] = o.forces(2)
+        o.close()
+    Fc, F = parts["coul"][:, 0], parts["both"][:, 0]
+    assert Fc[0] > 1.0 and (F - Fc)[0] < -0.4 and F[0] > 0.5      # gradient on atom 0: Coulomb +, LJ -, sum +
+    o = jo.Oracle(sysd, flags=1 | 2 | jo.F_COMBINED, **kw)
+    kT = KB * 300
+    sbm = np.sqrt(sysd["mass"] / (kT * KCAL))
+    eps = kw["eps_jump"]
+    rate0 = max(jo.jump_rate(eps, 1 / kT, sbm[i], abs(F[i]), 0.0) for i in range(2))
+    H = 0.02 / (rate0 * math.sqrt(1 + eps * eps))
+    rng = np.random.default_rng(9)
+    R = 200_000
+    acc = np.zeros((2, 3))
+    V = rng.normal(size=(R, 2, 3)) / sbm[None, :, None]
+    for rep in range(R):
+        o.set_vel(V[rep])
+        o.jump_half(H, with_accel=False, step=rep)
+        acc += o.vel - V[rep]
+    mean = acc / R
+    pred = -H * KCAL * parts["both"] / sysd["mass"][:, None]
+    st = o.stats()
+    assert st["accepts"] > 2000 and st["max_g_over_L"] <= 1.0 and st["max_p"] <= 1.0
+    for i in range(2):
+        assert abs(mean[i, 0] / pred[i, 0] - 1.0) < 0.08, (i, mean[i, 0], pred[i, 0])
+        assert np.abs(mean[i, 1:]).max() < 0.06 * abs(pred[i, 0])
+
+
+def test_combined_mechanism_event_log_and_bounds(relaxed_small):
+    """R-22: one chain per atom and half-phase (stream 1 / 4), none in the (J') streams; ring codes 8-10; the bound of a
+    ring is the sum of the Coulomb and the LJ bound and dominates the combined gradient of every proposal; more proposals
+    than the Coulomb mechanism alone (and more than the two side by side: the LJ bound now also carries the (1/eps)
+    term of the general mechanism's rate bound, which BPS does not have)."""
+    sysd, kw = _frozen(relaxed_small, flags=1 | 2 | 4 | jo.F_COMBINED, eps_jump=1.0)
+    o = jo.Oracle(sysd, **kw)
+    o.jump_step(40)
+    ev, st = o.events(), o.stats()
+    assert st["max_p"] <= 1.0 and st["max_g_over_L"] <= 1.0
+    prop = ev[ev["ring"] >= 0]
+    assert len(prop) == st["proposals"] > 300 and set(np.unique(prop["ring"])) <= {8, 9, 10}
+    assert set(np.unique(ev["stream"])) <= {1, 4}
+    assert np.array_equal(prop["accepted"] == 1, prop["U"] <= prop["p"])
+    n_comb = st["proposals"]
+    counts = {}
+    for name, flags in (("coul", 1 | 4), ("two", 1 | 2 | 4)):
+        o2 = jo.Oracle(sysd, **dict(kw, flags=flags))
+        o2.jump_step(40)
+        counts[name] = o2.stats()["proposals"]
+    assert counts["coul"] < n_comb < 2 * counts["two"]
