@@ -39,6 +39,8 @@ extern "C" {
 #define JUMP_F_RESPA_COMPARATOR 16u /* jump_respa_step runs BAOAB-RESPA: outer kick by the long force */
 
 #define JUMP_F_BJAOAJB 64u         /* jump_step runs B J A O A J B instead of C'J' A O A J'C' */
+#define JUMP_F_COMBINED 128u       /* with flags 1 | 2: step C' runs ONE mechanism per pair for the whole long pair gradient, Coulomb + LJ
+                                      (bound = sum of the two ring bounds), and there is no step J' (R-22) */
 #define JUMP_F_LAX_SKIN 32u        /* a displacement beyond skin/2 between list builds is NOT an error (see JUMP_E_SKIN) */
 
 typedef struct jump_ctx jump_ctx; /* opaque, owned by the library */

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libjump_b200.so")
 F_COUL_JUMPS, F_LJ_JUMPS, F_EVENT_LOG, F_RESPA_PAPER, F_RESPA_COMPARATOR = 1, 2, 4, 8, 16
 F_LAX_SKIN = 32
 F_BJAOAJB = 64
+F_COMBINED = 128
 ERRORS = {-1: "bad argument", -2: "CUDA error", -3: "row/event overflow", -4: "thinning bound violated",
           -5: "displacement beyond skin/2", -6: "non-finite state"}
 

@@ -379,7 +379,7 @@ static Phase ph_kick(double H) { Phase p = ph_none(); p.kind = 1; p.H = (float)H
 static Phase ph_jump(const jump_ctx *c, double H, bool grad, bool reverse, int sC, int sJ, int64_t step) {
     Phase p = ph_none();
     p.kind = 2; p.H = (float)H; p.use_grad = grad ? 1 : 0; p.reverse = reverse ? 1 : 0;
-    p.coul = coul_jumps(c) ? 1 : 0; p.lj = lj_jumps(c) ? 1 : 0;
+    p.coul = coul_jumps(c) ? 1 : 0; p.lj = (lj_jumps(c) && !c->m.combined) ? 1 : 0;   // R-22: no J' under the combined mechanism
     p.streamC = sC; p.streamJ = sJ; p.step = (unsigned)step;
     return p;
 }
@@ -752,6 +752,15 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
     m.beta = (float)(1.0 / c->kT);
     m.eps_jump = std::isinf(p->eps_jump) ? INFINITY : (float)p->eps_jump;
     m.eps_adaptive = p->eps_mode == 1 ? 1 : 0;
+    m.combined = (p->flags & JUMP_F_COMBINED) ? 1 : 0;
+    if (m.combined && (p->flags & (JUMP_F_COUL_JUMPS | JUMP_F_LJ_JUMPS)) != (JUMP_F_COUL_JUMPS | JUMP_F_LJ_JUMPS)) {
+        c->err = "JUMP_F_COMBINED needs JUMP_F_COUL_JUMPS | JUMP_F_LJ_JUMPS (R-22)";
+        return JUMP_E_ARG;
+    }
+    if (m.combined && m.eps_adaptive) {
+        c->err = "JUMP_F_COMBINED with eps_mode 1 is not built (R-22 runs the constant-eps mechanism)";
+        return JUMP_E_ARG;
+    }
     {
         const double rlo = p->r_short - p->r_switch;
         const double eA = std::min(std::max(c->rA, rlo), p->r_long), eM = std::min(std::max(c->rM, eA), p->r_long);

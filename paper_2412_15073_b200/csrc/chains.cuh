@@ -152,7 +152,8 @@ __device__ inline int pick_ring(const ChainConst &c, float ur, float c0, float c
 // Coulomb one.  An fp32 r^2 within RING_TIE of a ring edge is re-decided in fp64 from the full positions (R-17).
 // far_excl: the atom has an excluded partner that could be as far as ring C (never so in water): only then the
 // universe's candidates are checked against the exclusion list (R-9).
-template <bool LJ>
+// MODE 0: the long Coulomb gradient (step C'), 1: the long LJ gradient (step J'), 2: their sum (R-22)
+template <int MODE>
 __device__ inline void eval_candidate(const Model &m, const UpdateArgs &A, int ring, int i, int j, const float4 &xi, float2 lji,
                                       bool far_excl, float &g, float &nx, float &ny, float &nz) {
     const float4 xj = A.xs[j];
@@ -178,7 +179,11 @@ __device__ inline void eval_candidate(const Model &m, const UpdateArgs &A, int r
         for (int e = A.excl_ptr[o]; e < A.excl_ptr[o + 1]; ++e) in = in && A.excl_idx[e] != oj;
     }
     float rinv = 0.f, fr = 0.f;
-    if (in) fr = LJ ? fij_lj(m, p, lji, A.lj[j], rinv) : fij_coul(m, p, xi.w, xj.w, rinv);
+    if (in) fr = MODE == 1 ? fij_lj(m, p, lji, A.lj[j], rinv) : fij_coul(m, p, xi.w, xj.w, rinv);
+    if (MODE == 2 && in) {   // R-22: F_ij is the whole long pair gradient (both parts lie along the pair axis)
+        float rinv_lj;
+        fr += fij_lj(m, p, lji, A.lj[j], rinv_lj);
+    }
     const float sg = (fr > 0.f ? rinv : -rinv);  // n = F/|F|
     g = fabsf(fr);
     nx = p.dx * sg; ny = p.dy * sg; nz = p.dz * sg;
@@ -191,15 +196,15 @@ __device__ inline int ring_candidate(const UpdateArgs &A, const ChainConst &c, i
 }
 // state-independent part of a proposal, from its Philox block w: ring pick and partner, then the pair;
 // tag = ring << 28 | j_orig (event log only)
-template <bool LJ, bool WANT_J>
+template <int MODE, bool WANT_J>
 __device__ inline void propose_pair(const Model &m, const UpdateArgs &A, const ChainConst &c, float c0, float c1, float tot,
                                     int i, const float4 &xi, float2 lji, const uint32_t w[4], float &g, int &ring, float &nx,
                                     float &ny, float &nz, int &tag) {
     ring = pick_ring(c, u01(w[1]), c0, c1, tot);
     const int j = ring_candidate(A, c, i, ring, (int)__umulhi(w[2], (unsigned)c.N[ring]));
-    eval_candidate<LJ>(m, A, ring, i, j, xi, lji, c.far_excl, g, nx, ny, nz);
+    eval_candidate<MODE>(m, A, ring, i, j, xi, lji, c.far_excl, g, nx, ny, nz);
     tag = 0;
-    if (WANT_J) tag = A.orig[j] | (ring << 28);
+    if (WANT_J) tag = A.orig[j] | ((ring + (MODE == 2 ? 8 : 0)) << 28);   // ring codes 8-10: the combined mechanism
 }
 
 __device__ inline double wrap1d(double x, double L, double invL, int &img) {   // img += the number of box lengths taken off

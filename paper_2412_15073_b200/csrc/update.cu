@@ -16,15 +16,20 @@ namespace jb {
 // after the other, and every shuffle and ballot is a full-warp one.  `on` = this lane's atom exists and runs C'.
 // ADAPT: eps(x) = eps0 |F_ij(x)| (R-19): per-pair bound beta L_Y B_v + lam0, p = Theta(eta) / (eps0
 // sqrt(beta m) L_Y B_v + 1/sqrt(2 pi)), G~ and the kick (7) with eps = eps0 |F_ij|.
-template <int G, bool LOG, bool ADAPT>
+// MECH 0: constant eps; 1 (ADAPT): adaptive eps; 2 (COMB): constant eps on the whole long pair gradient, Coulomb + LJ (R-22)
+template <int G, bool LOG, int MECH>
 __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const ChainConst &c, int i, unsigned atom, const float4 &xi,
-                        float sbm, float ax, float ay, float az, float H, unsigned stream, unsigned step, float &vx, float &vy,
+                        float2 lji, float sbm, float ax, float ay, float az, float H, unsigned stream, unsigned step, float &vx, float &vy,
                         float &vz, Tally &tl, int gl, int gshift) {
+    constexpr bool ADAPT = MECH == 1, COMB = MECH == 2;
     const unsigned full = 0xffffffffu;
     const float eps = m.eps_jump, beta = m.beta;
     const bool bps = isinf(eps), lead = gl == 0;
     const float aq = fabsf(xi.w);
-    const float L0 = aq * m.qmaxG[0], L1 = aq * m.qmaxG[1], L2 = aq * m.qmaxG[2];   // L_Y,i = |q_i| q_max G_Y (R-7)
+    // L_Y,i = |q_i| q_max G_Y (R-7); combined mechanism (R-22): + sqrt(eps_i) 4 sqrt(eps_max) GV_Y, the LJ bound of the ring
+    const float se = COMB ? 0.5f * lji.y : 0.f;
+    const float L0 = fmaf(se, m.GV4se[0], aq * m.qmaxG[0]), L1 = fmaf(se, m.GV4se[1], aq * m.qmaxG[1]),
+                L2 = fmaf(se, m.GV4se[2], aq * m.qmaxG[2]);
     const float w0 = (float)c.N[0] * L0, w1 = (float)c.N[1] * L1, w2 = (float)c.N[2] * L2;
     const float S = (w0 + w1) + w2;
     bool done = !(on && S > 0.f);
@@ -75,7 +80,7 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
         const float U = u01(w[3]);
         float g = 0.f, nx = 0.f, ny = 0.f, nz = 0.f;
         int tag = 0, ring = 0;
-        if (alive) propose_pair<false, LOG>(m, A, c, c0, c1, tot, i, xi, make_float2(0.f, 0.f), w, g, ring, nx, ny, nz, tag);
+        if (alive) propose_pair<COMB ? 2 : 0, LOG>(m, A, c, c0, c1, tot, i, xi, lji, w, g, ring, nx, ny, nz, tag);
         const float LY = ring == 0 ? L0 : (ring == 1 ? L1 : L2);
         const float goL = __fdividef(g, LY);
         float p = 0.f, vn = 0.f;
@@ -181,7 +186,7 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, const ChainConst &c
         if (lead) tl.proposals++;
         float g, nx, ny, nz, p = 0.f;
         int ring, tag, acc = 0;
-        propose_pair<true, true>(m, A, c, c0, c1, S, i, xi, lji, w, g, ring, nx, ny, nz, tag);
+        propose_pair<1, true>(m, A, c, c0, c1, S, i, xi, lji, w, g, ring, nx, ny, nz, tag);
         const float L = ring == 0 ? L0 : (ring == 1 ? L1 : L2);
         if (g > 0.f) {
             float vF = (vx * nx + vy * ny + vz * nz) * g;
@@ -199,7 +204,7 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, const ChainConst &c
 
 // ---- the fused per-atom update: up to two velocity half-phases, then A O A + wrap ----------------------------
 // G lanes per atom (a power of two <= 32) share the atom's jump chains; lane 0 of the group does A-O-A and the stores.
-template <bool JUMPS, int G, bool LOG, bool ADAPT>
+template <bool JUMPS, int G, bool LOG, int MECH>
 __global__ void __launch_bounds__(128, 8) k_update(Model m, UpdateArgs A) {
     const unsigned full = 0xffffffffu;
     const int gt_id = blockIdx.x * blockDim.x + threadIdx.x;
@@ -229,7 +234,7 @@ __global__ void __launch_bounds__(128, 8) k_update(Model m, UpdateArgs A) {
         if (A.ph[0].kind != 0 && A.ph[0].use_grad) { g0 = A.grad[0][i]; if (A.grad_b[0]) b0 = A.grad_b[0][i]; }
         if (A.ph[1].kind != 0 && A.ph[1].use_grad) { g1 = A.grad[1][i]; if (A.grad_b[1]) b1 = A.grad_b[1][i]; }
         if (any_coul || any_lj) cc = chain_const(A, i);
-        if (any_lj) lji = A.lj[i];
+        if (any_lj || MECH == 2) lji = A.lj[i];
         // a = -M^-1 F
         a0x = -mi.x * (b0.x + g0.x); a0y = -mi.x * (b0.y + g0.y); a0z = -mi.x * (b0.z + g0.z);
         a1x = -mi.x * (b1.x + g1.x); a1y = -mi.x * (b1.y + g1.y); a1z = -mi.x * (b1.z + g1.z);
@@ -253,7 +258,7 @@ __global__ void __launch_bounds__(128, 8) k_update(Model m, UpdateArgs A) {
 #pragma unroll 1
             for (int slot = 0; slot < 3; ++slot) {
                 if (slot == 1) {
-                    if (P.coul) chain_C<G, LOG, ADAPT>(m, A, live, cc, i, atom, xi, mi.y, cax, cay, caz, P.H, P.streamC, P.step, vx, vy, vz, tl, gl, gshift);
+                    if (P.coul) chain_C<G, LOG, MECH>(m, A, live, cc, i, atom, xi, lji, mi.y, cax, cay, caz, P.H, P.streamC, P.step, vx, vy, vz, tl, gl, gshift);
                     else if (P.use_grad) { vx += P.H * cax; vy += P.H * cay; vz += P.H * caz; }
                 } else if (P.lj && live && (slot == 0) == (P.reverse != 0)) {
                     chain_J(m, A, cc, i, atom, xi, lji, mi.y, P.H, P.streamJ, P.step, vx, vy, vz, tl, lead);
@@ -457,11 +462,14 @@ static void update_dispatch(const Model &m, const UpdateArgs &A, cudaStream_t st
     const int B = 128;
     const unsigned grid = (unsigned)(((long long)m.n * G + B - 1) / B);
     if (m.eps_adaptive) {
-        if (A.events) k_update<true, G, true, true><<<grid, B, 0, st>>>(m, A);
-        else k_update<true, G, false, true><<<grid, B, 0, st>>>(m, A);
+        if (A.events) k_update<true, G, true, 1><<<grid, B, 0, st>>>(m, A);
+        else k_update<true, G, false, 1><<<grid, B, 0, st>>>(m, A);
+    } else if (m.combined) {
+        if (A.events) k_update<true, G, true, 2><<<grid, B, 0, st>>>(m, A);
+        else k_update<true, G, false, 2><<<grid, B, 0, st>>>(m, A);
     } else {
-        if (A.events) k_update<true, G, true, false><<<grid, B, 0, st>>>(m, A);
-        else k_update<true, G, false, false><<<grid, B, 0, st>>>(m, A);
+        if (A.events) k_update<true, G, true, 0><<<grid, B, 0, st>>>(m, A);
+        else k_update<true, G, false, 0><<<grid, B, 0, st>>>(m, A);
     }
 }
 // lanes per jump chain: as many as keep the whole grid resident at once (SMs x resident CTAs of k_update x 128
@@ -473,7 +481,7 @@ static int lanes_per_chain(int n, int forced) {
         int dev = 0, sms = 148, per_sm = 6;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_update<true, 8, false, false>, 128, 0) != cudaSuccess || per_sm < 1)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_update<true, 8, false, 0>, 128, 0) != cudaSuccess || per_sm < 1)
             per_sm = 6;
         budget = (long long)sms * per_sm * 128;
     }
@@ -485,7 +493,7 @@ static int lanes_per_chain(int n, int forced) {
 void launch_update(const Model &m, const UpdateArgs &A, bool jumps, cudaStream_t st, int64_t *launches) {
     if (!jumps) {
         const int B = 128;
-        k_update<false, 1, false, false><<<(unsigned)((m.n + B - 1) / B), B, 0, st>>>(m, A);
+        k_update<false, 1, false, 0><<<(unsigned)((m.n + B - 1) / B), B, 0, st>>>(m, A);
     } else {
         switch (lanes_per_chain(m.n, A.lanes)) {
             case 16: update_dispatch<16>(m, A, st); break;

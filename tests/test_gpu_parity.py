@@ -190,8 +190,9 @@ def test_forces_solute_config3(jb, jo):
 # (tests/golden/scan_parity_seeds.py, oracle only).  Over 100 steps a 648-atom box takes ~2e5 discontinuous decisions
 # and rebuilds its lists 25 times; the two paths drift apart by fp32 rounding (~1e-5 A after 100 steps), so on about
 # half of all seeds one decision is eventually a closer call than that and is (legitimately, R-17) taken differently.
-PARITY_SEEDS = {(1.0, 0): (3164, 3127, 3088), (0.3, 0): (3157, 3068, 3005), (float("inf"), 0): (3185, 3175, 3087),
-                (2.0, 1): (3115, 3157, 3038)}
+PARITY_SEEDS = {(1.0, 0): (3055, 3003, 3039), (0.3, 0): (3037, 3038, 3060), (float("inf"), 0): (3042, 3048, 3038),
+                (2.0, 1): (3115, 3157, 3038)}   # (adaptive: every seed scores ~1e-9, the scan cannot rank them; kept from the 3000..3199 scan)
+COMBINED_SEEDS = (3018, 3054, 3057)   # (scan of seeds 3000..3079 under the round-2 list contract)
 
 
 def run_parity_window(jb, jo, sysd, run, lanes, n_chunks=10):
@@ -253,7 +254,7 @@ def test_bjaoajb_scheme_matches_oracle(jb, jo, cfg0):
     """NEXT-3: B J A O A J B as the scheme of jump_step -- event log and trajectory against the oracle,
     and without any jump mechanism the scheme is bitwise the C' scheme without jumps (BAOAB with F0)."""
     sysd, run = cfg0
-    r = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG | jb.F_BJAOAJB, seed=3137)   # scan_parity_seeds.py
+    r = dict(run, flags=jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG | jb.F_BJAOAJB, seed=3065)   # scan_parity_seeds.py
     g, o = jb.JumpSim(sysd, **r), jo.Oracle(sysd, **r)
     g.jump_step(10); g.sync(); o.jump_step(10)
     assert len(o.events()) > 15000
@@ -266,6 +267,28 @@ def test_bjaoajb_scheme_matches_oracle(jb, jo, cfg0):
     a, b = jb.JumpSim(sysd, **dict(run, flags=jb.F_BJAOAJB)), jb.JumpSim(sysd, **dict(run, flags=0))
     a.jump_step(25); b.jump_step(25); a.sync(); b.sync()
     assert (a.pos == b.pos).all() and (a.vel == b.vel).all() and a.stats()["proposals"] == 0
+
+
+@pytest.mark.parametrize("lanes", [0, 1])
+def test_combined_mechanism_matches_oracle(jb, jo, cfg0, lanes):
+    """NEXT-3 (R-22): JUMP_F_COMBINED -- one mechanism per pair for the whole long pair gradient (Coulomb + LJ) in step C',
+    no step J': every proposal of up to 100 steps equals the oracle's (partner, ring code 8-10, accept flag, sampler
+    attempts), trajectory within 1e-4 A, up to a decision the oracle marks as a close call; and the flag is refused
+    without both jump flags."""
+    sysd, run = cfg0
+    flags = jb.F_COUL_JUMPS | jb.F_LJ_JUMPS | jb.F_EVENT_LOG | jb.F_COMBINED
+    best = 0
+    for seed in COMBINED_SEEDS:
+        window, n_ev, n_acc, rings = run_parity_window(jb, jo, sysd, dict(run, flags=flags, seed=seed), lanes)
+        assert window >= 10
+        if window >= 50:
+            assert rings == {-1, 8, 9, 10} and n_ev > 60000 and n_acc > 500
+        best = max(best, window)
+        if best == 100:
+            break
+    assert best >= 50
+    with pytest.raises(jb.JumpError, match="COMBINED"):
+        jb.JumpSim(sysd, **dict(run, flags=jb.F_COUL_JUMPS | jb.F_COMBINED))
 
 
 def test_jump_half_statistics_frozen_x(jb, jo, cfg0):
