@@ -538,6 +538,28 @@ def test_config4_one_million_atoms_properties(jb):
     assert (out[0][0] == out[1][0]).all() and (out[0][1] == out[1][1]).all()
 
 
+def test_config4_forces_rows_and_one_outer_step_against_the_oracle(jb, jo):
+    """BASELINE configs[4], the workload and launch configuration bench.py times (999 999 atoms, JUMP-RESPA 1:4 fs, one
+    lane per chain, multi-kernel sort, resident-grid list kernels): F0 of EVERY atom against the oracle's, rows A and B
+    and the cell universe of a seeded sample of atoms bit for bit, then one JUMP-RESPA outer step (four inner steps,
+    ~2.5e7 discontinuous decisions): the same number of proposals and accepted jumps up to the handful of close calls
+    the fp32 path may take the other way (R-17), and the positions of all but those atoms within 1e-4 A."""
+    sysd, run = wl.make_config(4)
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    assert rel_force_err(g.forces(0).cpu().numpy(), o.forces(0)) <= F_TOL
+    check_sampled_rows(g, o, 64)
+    g.jump_respa_step(1); g.sync(); o.jump_respa_step(1)
+    sg, so = g.stats(), o.stats()
+    assert sg["error"] == 0 and sg["max_p"] <= 1 + 1e-4 and sg["max_g_over_L"] <= 1 + 1e-4
+    assert so["proposals"] > 4e6 and abs(sg["proposals"] - so["proposals"]) <= 50
+    assert so["accepts"] > 1e5 and abs(sg["accepts"] - so["accepts"]) <= 50
+    d = g.pos.cpu().numpy().astype(np.float64) - o.pos
+    d -= sysd["box"] * np.round(d / sysd["box"])
+    bad = np.abs(d).max(1) > X_TOL
+    assert bad.sum() <= 50, int(bad.sum())                    # (a jump taken on one side only moves its atom by ~1e-2 A)
+    g.close(); o.close()
+
+
 def test_config2_logged_step_single_lane_chains(jb, jo):
     """BASELINE configs[2] (96 000 atoms), where the update kernel runs one lane per chain -- the instantiation the
     large-box throughput is quoted on: every proposal of one logged JUMP step against the oracle's."""
