@@ -217,6 +217,8 @@ __device__ __forceinline__ float4 lds128(unsigned a) {
 }
 __device__ __forceinline__ int lds32(unsigned a) { int v; asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
 __device__ __forceinline__ void sts32(unsigned a, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
+__device__ __forceinline__ int lds16(unsigned a) { unsigned short v; asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(a) : "memory"); return (int)v; }
+__device__ __forceinline__ void sts16(unsigned a, int v) { asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"((unsigned short)v) : "memory"); }
 
 // *p = v under a predicate, as ONE predicated store (the compiler's branch around a conditional store costs a
 // convergence barrier pair and a jump per row and chunk in the row build's inner loop)
@@ -271,7 +273,7 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
     __shared__ float tile_w[BUILD_CHUNK];       // (skin/2) w_j: the candidate's share of the pair's skin (R-10c)
     __shared__ int scan_tmp[BUILD_THREADS];
     __shared__ int s_count[BUILD_MAXATOMS][N_ROWS];
-    __shared__ int s_queue[BUILD_WARPS][64];    // per warp: slots of the candidates that passed the distance filter
+    __shared__ unsigned short s_queue[BUILD_WARPS][128];   // per warp: slots of the candidates that passed the distance filter
     const unsigned full = 0xffffffffu;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // the CTA's home: CX consecutive cells along x (their atoms are contiguous in the sorted array)
@@ -367,7 +369,7 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
         for (int t = tid; t < BUILD_MAXATOMS * N_ROWS; t += BUILD_THREADS) (&s_count[0][0])[t] = 0;
         for (int c0 = 0; c0 < total || c0 == 0; c0 += BUILD_CHUNK) {
             const int c1 = min(c0 + BUILD_CHUNK, total);
-            const int npad = (c1 - c0 + 31) & ~31;
+            const int npad = (c1 - c0 + 63) & ~63;   // (the filter takes two groups of 32 per iteration)
             __syncthreads();   // the previous chunk has been consumed (and s_count is zeroed)
             {   // ---- stage [c0, c1): each warp takes a contiguous quarter of the chunk, 32 consecutive candidates per
                 // iteration (coalesced loads); a lane's run is found by one bisection and then advanced linearly --
@@ -465,7 +467,7 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                     };
                     auto windows = [&](const int n_live) {
                         __syncwarp();
-                        const int slot = lane_keep < n_live ? lds32(que_a + 4u * (unsigned)((q_head + lane_keep) & 63)) : 0;
+                        const int slot = lane_keep < n_live ? lds16(que_a + 2u * (unsigned)((q_head + lane_keep) & 127)) : 0;
                         const float4 xj = lds128(tile_a + 16u * (unsigned)(slot - lane_keep));
                         const int jraw = __float_as_int(xj.w);
                         const int j = jraw & 0x7fffffff;
@@ -539,13 +541,16 @@ __device__ __forceinline__ void build_rows_block(const Model &m, const SortGrid 
                         }
                         __syncwarp();   // the slots just read may be written again
                     };
-                    for (int q0 = 0; q0 < npad; q0 += 32) {
-                        const bool within = dist2(lds128(tile_a + 16u * (unsigned)q0)) < reach2;   // false for the NaN of a padding entry
-                        const unsigned wmask = __ballot_sync(full, within);
-                        if (wmask == 0u) continue;
-                        if (within) sts32(que_a + 4u * (unsigned)((q_head + q_n + __popc(wmask & lt_keep)) & 63), q0 + lane_keep);
-                        q_n += __popc(wmask);
-                        if (q_n >= 32) { windows(32); q_head = (q_head + 32) & 63; q_n -= 32; }
+                    for (int q0 = 0; q0 < npad; q0 += 64) {   // two groups of 32 per iteration: half the loop and vote overhead
+                        const bool in_a = dist2(lds128(tile_a + 16u * (unsigned)q0)) < reach2;   // false for the NaN of a padding entry
+                        const bool in_b = dist2(lds128(tile_a + 16u * (unsigned)(q0 + 32))) < reach2;
+                        const unsigned ma = __ballot_sync(full, in_a), mb = __ballot_sync(full, in_b);
+                        if ((ma | mb) == 0u) continue;
+                        const int at = q_head + q_n;
+                        if (in_a) sts16(que_a + 2u * (unsigned)((at + __popc(ma & lt_keep)) & 127), q0 + lane_keep);
+                        if (in_b) sts16(que_a + 2u * (unsigned)((at + __popc(ma) + __popc(mb & lt_keep)) & 127), q0 + 32 + lane_keep);
+                        q_n += __popc(ma) + __popc(mb);   // at most 31 + 64 of the 128 entries
+                        while (q_n >= 32) { windows(32); q_head = (q_head + 32) & 127; q_n -= 32; }
                     }
                     if (q_n > 0) windows(q_n);
 #undef JB_ROW_SCAN
