@@ -138,13 +138,15 @@ __device__ inline ChainConst chain_const(const UpdateArgs &A, int i) {
     c.N[2] = universe_size(A.grid, A.uni, c.home);
     return c;
 }
+// N_Y by selects: an index computed at run time would put the three counts into local memory
+__device__ __forceinline__ int ring_count(const ChainConst &c, int ring) { return ring == 0 ? c.N[0] : (ring == 1 ? c.N[1] : c.N[2]); }
 // ring pick: the first ring whose cumulated weight exceeds ur * (sum of weights); a ring without
 // candidates can only be hit through rounding at an end, and the pick then falls back as the oracle's does
 __device__ inline int pick_ring(const ChainConst &c, float ur, float c0, float c1, float tot) {
     const float x = ur * tot;
     int ring = x < c0 ? 0 : (x < c1 ? 1 : 2);
-    while (c.N[ring] == 0 && ring > 0) --ring;
-    while (c.N[ring] == 0 && ring < 2) ++ring;
+    while (ring_count(c, ring) == 0 && ring > 0) --ring;
+    while (ring_count(c, ring) == 0 && ring < 2) ++ring;
     return ring;
 }
 // A candidate j of ring `ring` (R-10c): the ring the pair's CURRENT distance lies in carries its force, through any
@@ -201,7 +203,7 @@ __device__ inline void propose_pair(const Model &m, const UpdateArgs &A, const C
                                     int i, const float4 &xi, float2 lji, const uint32_t w[4], float &g, int &ring, float &nx,
                                     float &ny, float &nz, int &tag) {
     ring = pick_ring(c, u01(w[1]), c0, c1, tot);
-    const int j = ring_candidate(A, c, i, ring, (int)__umulhi(w[2], (unsigned)c.N[ring]));
+    const int j = ring_candidate(A, c, i, ring, (int)__umulhi(w[2], (unsigned)ring_count(c, ring)));
     eval_candidate<MODE>(m, A, ring, i, j, xi, lji, c.far_excl, g, nx, ny, nz);
     tag = 0;
     if (WANT_J) tag = A.orig[j] | ((ring + (MODE == 2 ? 8 : 0)) << 28);   // ring codes 8-10: the combined mechanism

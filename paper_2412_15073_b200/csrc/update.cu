@@ -109,16 +109,18 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
                 acc = U <= p;
             }
         }
-        const unsigned alive_m = (__ballot_sync(full, alive) >> gshift) & gbits;
-        const unsigned acc_m = (__ballot_sync(full, acc) >> gshift) & gbits;
+        // (G = 1: the group is the lane itself -- no ballots, no shuffles)
+        const unsigned alive_m = G == 1 ? (alive ? 1u : 0u) : ((__ballot_sync(full, alive) >> gshift) & gbits);
+        const unsigned acc_m = G == 1 ? (acc ? 1u : 0u) : ((__ballot_sync(full, acc) >> gshift) & gbits);
         const int n_alive = __popc(alive_m);
         const int f = acc_m ? __ffs(acc_m) - 1 : -1;   // first accepted proposal of the batch
         const int n_used = f >= 0 ? f + 1 : n_alive;
         const int fs = f >= 0 ? f : 0;
-        const float tf = __shfl_sync(full, tk, fs, G), vnf = __shfl_sync(full, vn, fs, G);
-        const float gf = ADAPT ? __shfl_sync(full, g, fs, G) : 1.f;
-        const float fnx = __shfl_sync(full, nx, fs, G), fny = __shfl_sync(full, ny, fs, G), fnz = __shfl_sync(full, nz, fs, G);
-        const float t_last = __shfl_sync(full, tk, G - 1, G);
+        const float tf = G == 1 ? tk : __shfl_sync(full, tk, fs, G), vnf = G == 1 ? vn : __shfl_sync(full, vn, fs, G);
+        const float gf = ADAPT ? (G == 1 ? g : __shfl_sync(full, g, fs, G)) : 1.f;
+        const float fnx = G == 1 ? nx : __shfl_sync(full, nx, fs, G), fny = G == 1 ? ny : __shfl_sync(full, ny, fs, G),
+                    fnz = G == 1 ? nz : __shfl_sync(full, nz, fs, G);
+        const float t_last = G == 1 ? tk : __shfl_sync(full, tk, G - 1, G);
         if (done) continue;
         if (gl < n_used) { tl.max_gl = fmaxf(tl.max_gl, goL); tl.max_p = fmaxf(tl.max_p, p); }
         if (lead) tl.proposals += (unsigned)n_used;
