@@ -24,6 +24,7 @@ struct jump_ctx {
     int n;
     double kT, dt, alpha, rA, rM, lo;  // ps; lo = max(r_c - h - skin, 0)
     double G[3], GV[3], qmax, eps_max, sig_min, sig_max;   // bounds per ring (R-7, R-10c)
+    double qmin_abs;
     double w_max, w_norm;        // mass weights of the skin: w_i = m_i^-1/2 / w_norm, w_norm = mean(m^-1/2) (R-10c)
     Universe uni;                // cell universe of ring C (R-10c)
     unsigned short *uni_cum;
@@ -166,9 +167,10 @@ static double sup_long(const jump_ctx *c, double lo, double hi, double step, boo
 }
 static void compute_bounds(jump_ctx *c, const std::vector<float> &q, const std::vector<float> &sig,
                            const std::vector<float> &eps) {
-    c->qmax = 0.0; c->eps_max = 0.0; c->sig_min = 1e300; c->sig_max = 0.0;
+    c->qmax = 0.0; c->eps_max = 0.0; c->sig_min = 1e300; c->sig_max = 0.0; c->qmin_abs = 1e300;
     for (int i = 0; i < c->n; ++i) {
         c->qmax = std::max(c->qmax, std::fabs((double)q[i]));
+        c->qmin_abs = std::min(c->qmin_abs, std::fabs((double)q[i]));
         if (eps[i] > 0.f) {
             c->eps_max = std::max(c->eps_max, (double)eps[i]);
             c->sig_min = std::min(c->sig_min, (double)sig[i]);
@@ -771,6 +773,7 @@ static int init_impl(jump_ctx *c, const jump_params *p, const float *d_mass, con
             m.GV4se[y] = (float)(4.0 * std::sqrt(c->eps_max) * c->GV[y]);
         }
     }
+    m.q_split = (float)(0.5 * (c->qmin_abs + c->qmax));
     m.half_skin2 = (float)(0.25 * p->skin * p->skin);
     m.hs = (float)(0.5 * p->skin);
     m.Wc = (float)(1.0 / (std::sqrt(c->kT * kKcal) * c->w_norm));

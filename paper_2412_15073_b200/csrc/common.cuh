@@ -83,6 +83,7 @@ struct Model {
     float eps_jump;               // epsilon; +inf -> BPS
     int eps_adaptive;             // eps(x) = eps_jump |F_ij(x)| (R-19)
     int combined;                 // step C' treats the whole long pair gradient, Coulomb + LJ, as one mechanism (R-22)
+    float q_split;                // (min |q| + max |q|) / 2: atoms above it run the long chains (k_update's lane order)
     float qmaxG[3];               // qmax * G_Y, rings A, B, C   (L_Y,i = |q_i| * this, R-7)
     float GV4se[3];               // 4 sqrt(eps_max) GV_Y        (L^vdW_Y,i = sqrt(eps_i) * this)
     float ring2[4];               // squared ring edges (r_c-h)^2, r_A^2, r_M^2, r_long^2: ring Y = [ring2[Y], ring2[Y+1])

@@ -210,8 +210,28 @@ template <bool JUMPS, int G, bool LOG, int MECH>
 __global__ void __launch_bounds__(128, 8) k_update(Model m, UpdateArgs A) {
     const unsigned full = 0xffffffffu;
     const int gt_id = blockIdx.x * blockDim.x + threadIdx.x;
-    const int i = gt_id / G, gl = gt_id % G;
+    int i = gt_id / G;
+    const int gl = gt_id % G;
     const int lane = threadIdx.x & 31, gshift = lane & ~(G - 1);
+    if (JUMPS && G == 1) {
+        // One chain per lane: a warp runs as long as its longest chain, and the chains of the strongly charged atoms
+        // (rate ~ |q_i|: the oxygens of water, which also run the J' chains) are about twice as long as the others'.
+        // The 128 atoms of the CTA are therefore dealt to its lanes with those atoms first (a stable partition): the
+        // warps become homogeneous, and the ones with the short chains finish early.
+        __shared__ int s_heavy[4];
+        __shared__ unsigned char s_perm[128];
+        const bool heavy = i < m.n && fabsf(A.xs[i].w) > m.q_split;
+        const unsigned hb = __ballot_sync(full, heavy);
+        const int wp = threadIdx.x >> 5;
+        if (lane == 0) s_heavy[wp] = __popc(hb);
+        __syncthreads();
+        int before = __popc(hb & ((1u << lane) - 1u)), total = 0;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) { const int hk = s_heavy[k]; before += k < wp ? hk : 0; total += hk; }
+        s_perm[heavy ? before : total + ((int)threadIdx.x - before)] = (unsigned char)threadIdx.x;
+        __syncthreads();
+        i = blockIdx.x * 128 + s_perm[threadIdx.x];
+    }
     const bool live = i < m.n, lead = gl == 0;
     Tally tl = {0u, 0u, 0u, 0u, 0.f, 0.f};
     float disp2 = 0.f;
