@@ -287,27 +287,6 @@ __device__ inline int universe_pick(const SortGrid &g, const Universe &u, const 
     const int kk = k - (int)cum[lo];
     return kk < n0 ? b0 + kk : b1 + (kk - n0);
 }
-// The same lookup done by the whole warp for ONE request (hp, k), all 32 lanes converged: the running sums are read 32
-// at a time (coalesced), the row is the number of sums <= k minus one (a ballot count) -- three loads deep instead of
-// eleven, and nobody waits alone (a lane that walks through the bisection by itself stalls its whole warp).
-__device__ inline int universe_pick_warp(const SortGrid &g, const Universe &u, const int *__restrict__ cell_start, int hp, int k,
-                                         int lane) {
-    const int cx = hp & 1023, cy = (hp >> 10) & 1023, cz = hp >> 20;
-    const int h = (cz * g.gn[1] + cy) * g.gn[0] + cx;
-    const unsigned short *__restrict__ cum = u.cum + (size_t)h * u.stride;
-    int below = 0;
-    for (int base = 0; base < u.nrow; base += 32) {
-        const int row = base + lane;
-        const bool ok = row < u.nrow && (int)cum[row] <= k;
-        below += __popc(__ballot_sync(0xffffffffu, ok));
-    }
-    const int lo = below - 1;   // (cum[0] = 0 <= k)
-    const int mz = (lo * u.inv_cnt1) >> 16, my = lo - mz * u.cnt[1];
-    int b0, n0, b1, n1;
-    universe_row(g, u, cell_start, cx, cy, cz, mz, my, b0, n0, b1, n1);
-    const int kk = k - (int)cum[lo];
-    return kk < n0 ? b0 + kk : b1 + (kk - n0);
-}
 __device__ inline int universe_size(const SortGrid &g, const Universe &u, int hp) {
     const int h = ((hp >> 20) * g.gn[1] + ((hp >> 10) & 1023)) * g.gn[0] + (hp & 1023);
     return (int)u.cum[(size_t)h * u.stride + u.nrow];
