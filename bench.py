@@ -315,6 +315,7 @@ def main():
     ap.add_argument("--nlist-every", type=int, default=None)
     ap.add_argument("--eps-jump", type=float, default=None)
     ap.add_argument("--cell-edge", type=float, default=None, help="edge of the contract grid's cells, A (default: the library's)")
+    ap.add_argument("--lanes", type=int, default=0, help="lanes per jump chain in k_update: 1, 4, 8, 16 (default 0: the library's choice)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
@@ -342,6 +343,8 @@ def main():
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
     with torch.cuda.stream(stream):
         sim = jb.JumpSim(sysd, device=dev, stream=stream, **run)
+        if args.lanes:
+            sim.set_lanes(args.lanes)
         sim.set_lax_skin(True)                                         # the lattice start is hot: no skin check while it relaxes
         sim.baoab_step(args.equil)
         sim.set_lax_skin(False)                                        # from here on a displacement beyond skin/2 is an error
