@@ -244,16 +244,10 @@ static int resort_and_build(jump_ctx *c, bool conditional) {
     a.tmp_orig = c->tmp_orig; a.tmp_src = c->tmp_src; a.scan_sums = c->scan_sums; a.scan_offs = c->scan_offs; a.ctr = c->ctr;
     a.go = go; a.want = stamp;
     prof_begin(c, PROF_BUILD);
-    const bool uni_done = launch_sort(a, c->uni, c->uni_cum, c->st, &c->launches);
+    launch_sort(a, c->uni, c->uni_cum, c->st, &c->launches);   // (with the running sums of the universe of every cell, ring C, R-10c)
     prof_end(c, PROF_BUILD);
     CK(cudaGetLastError());
     c->slow_valid = false;   // (the sorted order may have changed)
-    if (c->uni_cum && !uni_done) {   // running sums of the universe of every cell (ring C, R-10c)
-        prof_begin(c, PROF_BUILD);
-        launch_universe(c->g, c->uni, c->cell_start, c->uni_cum, c->ctr, go, stamp, c->st, &c->launches);
-        prof_end(c, PROF_BUILD);
-        CK(cudaGetLastError());
-    }
     // rows that nobody has read for a while leave the active set (they are built again on demand)
     for (int k = 0; k < N_ROWS; ++k)
         if (c->row_active[k] && c->step - c->row_last_use[k] > 36) c->row_active[k] = false;

@@ -73,9 +73,7 @@ struct EwaldArgs {   // reciprocal Ewald sum (ewald.cu, R-21)
     double2 *tabD;           // [E][n] fp64 phase-factor tables (NULL: direct sines and cosines), E = sum (nmax + 1)
 };
 
-bool launch_sort(const SortArgs &a, const Universe &u, unsigned short *uni_cum, cudaStream_t st, int64_t *launches);
-void launch_universe(const SortGrid &g, const Universe &u, const int *cell_start, unsigned short *cum, Counters *ctr,
-                     const int *go, int want, cudaStream_t st, int64_t *launches);
+void launch_sort(const SortArgs &a, const Universe &u, unsigned short *uni_cum, cudaStream_t st, int64_t *launches);
 int launch_universe_list(const SortGrid &g, const Universe &u, const int *cell_start, int home, int *out, int cap,
                          cudaStream_t st, int64_t *launches);
 void launch_build_rows(const Model &m, const SortGrid &g, const Row rows[N_ROWS], float rmax_all, const int *cell_start,

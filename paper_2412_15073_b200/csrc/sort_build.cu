@@ -16,8 +16,7 @@
 
 namespace jb {
 
-// The per-element bodies of the sort passes are device functions: the large-box path runs each pass as a kernel of its
-// own, the small-box path (k_sort_small) all of them in one CTA.
+// The per-element bodies of the sort passes (they are the passes of k_sort below).
 __device__ __forceinline__ void cell_key_one(int i, const float4 *xs, const SortGrid &g, int *key, int *cell_count, Counters *ctr) {
     float4 x = xs[i];
     if (!(isfinite(x.x) && isfinite(x.y) && isfinite(x.z))) {
@@ -35,14 +34,6 @@ __device__ __forceinline__ void cell_key_one(int i, const float4 *xs, const Sort
     key[i] = k;
     atomicAdd(&cell_count[k], 1);
 }
-__global__ void k_cell_key(int n, const float4 *__restrict__ xs, SortGrid g, int *__restrict__ key,
-                           int *__restrict__ cell_count, Counters *ctr, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    cell_key_one(i, xs, g, key, cell_count, ctr);
-}
-
 // exclusive scan of cell_count[0..ncell) into cell_start[0..ncell]; one block (part: blockDim.x ints of shared memory)
 __device__ __forceinline__ void scan_block(int ncell, const int *cell_count, int *cell_start, int *part) {
     int t = threadIdx.x, nt = blockDim.x;
@@ -65,55 +56,7 @@ __device__ __forceinline__ void scan_block(int ncell, const int *cell_count, int
     }
     if (t == nt - 1) cell_start[ncell] = part[t];
 }
-__global__ void k_scan(int ncell, const int *__restrict__ cell_count, int *__restrict__ cell_start, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    __shared__ int part[1024];
-    scan_block(ncell, cell_count, cell_start, part);
-}
-
-// the same scan for large grids, in three small launches: per-block sums of 4096-cell slices, a scan of the
-// sums (k_scan on them), then each block scans its slice from its offset
-constexpr int SCAN_SLICE = 4096;
-__global__ void k_scan_sums(int ncell, const int *__restrict__ cell_count, int *__restrict__ sums, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    __shared__ int part[32];
-    const int lo = blockIdx.x * SCAN_SLICE, hi = min(lo + SCAN_SLICE, ncell);
-    int s = 0;
-    for (int k = lo + threadIdx.x; k < hi; k += blockDim.x) s += cell_count[k];
-    s = __reduce_add_sync(0xffffffffu, s);
-    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        int v = threadIdx.x < (blockDim.x >> 5) ? part[threadIdx.x] : 0;
-        v = __reduce_add_sync(0xffffffffu, v);
-        if (threadIdx.x == 0) sums[blockIdx.x] = v;
-    }
-}
-__global__ void k_scan_slices(int ncell, const int *__restrict__ cell_count, const int *__restrict__ offs,
-                              int *__restrict__ cell_start, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    __shared__ int part[1024];
-    const int t = threadIdx.x, nt = blockDim.x;   // nt * 4 = SCAN_SLICE
-    const int lo = blockIdx.x * SCAN_SLICE + 4 * t;
-    int c[4], s = 0;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) { c[k] = lo + k < ncell ? cell_count[lo + k] : 0; s += c[k]; }
-    part[t] = s;
-    __syncthreads();
-    for (int off = 1; off < nt; off <<= 1) {
-        int v = (t >= off) ? part[t - off] : 0;
-        __syncthreads();
-        part[t] += v;
-        __syncthreads();
-    }
-    int run = offs[blockIdx.x] + part[t] - s;
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        if (lo + k < ncell) cell_start[lo + k] = run;
-        run += c[k];
-    }
-    if (lo <= ncell - 1 && ncell - 1 < lo + 4) cell_start[ncell] = run;
-}
+constexpr int SCAN_SLICE = 4096;   // cells per slice of the scan of large grids
 
 __device__ __forceinline__ void scatter_one(int i, const int *key, const int *orig, const int *cell_start, int *cell_fill,
                                             int *tmp_orig, int *tmp_src) {
@@ -122,15 +65,6 @@ __device__ __forceinline__ void scatter_one(int i, const int *key, const int *or
     tmp_orig[slot] = orig[i];
     tmp_src[slot] = i;
 }
-__global__ void k_scatter(int n, const int *__restrict__ key, const int *__restrict__ orig,
-                          const int *__restrict__ cell_start, int *__restrict__ cell_fill,
-                          int *__restrict__ tmp_orig, int *__restrict__ tmp_src, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    scatter_one(i, key, orig, cell_start, cell_fill, tmp_orig, tmp_src);
-}
-
 // order each cell by original index (insertion sort; a cell holds a handful of atoms)
 __device__ __forceinline__ void cell_sort_one(int c, const int *cell_start, int *tmp_orig, int *tmp_src) {
     int lo = cell_start[c], hi = cell_start[c + 1];
@@ -146,54 +80,6 @@ __device__ __forceinline__ void cell_sort_one(int c, const int *cell_start, int 
         tmp_src[b + 1] = ks;
     }
 }
-__global__ void k_cell_sort(int ncell, const int *__restrict__ cell_start, int *__restrict__ tmp_orig,
-                            int *__restrict__ tmp_src, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= ncell) return;
-    cell_sort_one(c, cell_start, tmp_orig, tmp_src);
-}
-
-__global__ void k_permute(int n, const int *__restrict__ src, const int *__restrict__ new_orig,
-                          const float4 *__restrict__ xs_in, const float4 *__restrict__ vs_in,
-                          const float4 *__restrict__ xl_in, float4 *__restrict__ xl,
-                          const float2 *__restrict__ lj_in, const float2 *__restrict__ mi_in, const float2 *__restrict__ hw_in,
-                          float2 *__restrict__ hw,
-                          float4 *__restrict__ xs, float4 *__restrict__ vs, float2 *__restrict__ lj,
-                          float2 *__restrict__ mi, int *__restrict__ orig, int *__restrict__ sorted_of,
-                          float4 *__restrict__ x_build, const int *__restrict__ key, int *__restrict__ cell_of, int gnx, int gny,
-                          Counters *ctr, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    if (i == 0) { ctr->rebuilds += 1; ctr->last_build = want; }
-    int s = src[i];
-    const int kk = key[s];   // home cell, packed by coordinates (the universe lookup wants them without divisions)
-    cell_of[i] = pack_cell(kk % gnx, (kk / gnx) % gny, kk / (gnx * gny));
-    float4 x = xs_in[s];
-    xs[i] = x;
-    x_build[i] = x;
-    vs[i] = vs_in[s];
-    xl[i] = xl_in[s];
-    lj[i] = lj_in[s];
-    hw[i] = hw_in[s];
-    mi[i] = mi_in[s];
-    int o = new_orig[i];
-    orig[i] = o;
-    sorted_of[o] = i;
-}
-// the permuted copies back into the state arrays (a pointer swap on the host would need to know whether the sort ran)
-__global__ void k_copyback(int n, const float4 *__restrict__ xs_t, const float4 *__restrict__ vs_t, const float4 *__restrict__ xl_t,
-                           const float2 *__restrict__ lj_t, const float2 *__restrict__ mi_t, const float2 *__restrict__ hw_t, float2 *__restrict__ hw,
-                           const int *__restrict__ orig_t,
-                           float4 *__restrict__ xs, float4 *__restrict__ vs, float4 *__restrict__ xl, float2 *__restrict__ lj,
-                           float2 *__restrict__ mi, int *__restrict__ orig, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    xs[i] = xs_t[i]; vs[i] = vs_t[i]; xl[i] = xl_t[i]; lj[i] = lj_t[i]; mi[i] = mi_t[i]; hw[i] = hw_t[i]; orig[i] = orig_t[i];
-}
-
 struct RowSet { Row r[N_ROWS]; };
 
 // d wrapped to the periodic image nearest to 0
@@ -634,38 +520,66 @@ __device__ __forceinline__ void universe_cell(const SortGrid &g, const Universe 
         if (run >= 65535) atomicOr(&ctr->err, (unsigned)ERR_OVERFLOW);   // 16-bit running sums
     }
 }
-__global__ void __launch_bounds__(128) k_universe(SortGrid g, Universe u, const int *__restrict__ cell_start,
-                                                  unsigned short *__restrict__ cum, Counters *ctr, const int *__restrict__ go, int want) {
-    if (go && *go != want) return;
-    const int lane = threadIdx.x & 31, nwarp = (gridDim.x * blockDim.x) >> 5;
-    // resident grid, the cells dealt round-robin to its warps (equal work per cell; see work_fetch for why not a CTA per item)
-    for (int h = (blockIdx.x * blockDim.x + threadIdx.x) >> 5; h < g.ncell; h += nwarp) universe_cell(g, u, cell_start, cum, ctr, h, lane);
-}
-// the universe of one home cell as a list of sorted indices (observer: jump_get_row), one thread per entry, through the
-// same lookup the jump chains use
 __global__ void k_universe_list(SortGrid g, Universe u, const int *__restrict__ cell_start, int h, int n, int *__restrict__ out) {   // h: packed home cell
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k < n) out[k] = universe_pick(g, u, cell_start, h, k);
 }
 
 // ------------------------------------------------------------------------------------------
-// Small boxes: the whole sort in ONE cooperative launch (zero the counts, keys, scan, scatter, per-cell order, permute,
-// copy back, the running sums of the cell universe, with grid-wide barriers between the passes).  On a 12 000-atom box
-// the step is a chain of launches of a few microseconds each, and the list kernels are enqueued at every step to return
-// at once on most of them: one such launch instead of nine (two memsets and seven kernels).  Plain pointers on purpose:
-// the passes read what earlier passes of the same kernel wrote, which the read-only data path would not see.
-constexpr int SORT_SMALL_THREADS = 512, SORT_SMALL_CTAS = 32;
-constexpr int SORT_SMALL_MAX_ATOMS = 32768, SORT_SMALL_MAX_CELLS = 16384;
-__global__ void __launch_bounds__(SORT_SMALL_THREADS) k_sort_small(SortArgs a, Universe u, unsigned short *cum) {
+// The whole sort in ONE cooperative launch: zero the counts, keys, scan, scatter, per-cell order, permute into scratch,
+// copy back (whether a conditional sort ran is known on the device only: no pointer swap), the running sums of the cell
+// universe -- with grid-wide barriers between the passes.  The list kernels are enqueued at every step to return at once
+// on most of them: one idle launch instead of eleven (two memsets and nine kernels) -- a quarter of the step on a
+// 12 000-atom box, half a percent at 10^6 atoms.  Plain pointers on purpose: the passes read what earlier passes of the
+// same kernel wrote, which the read-only data path would not see.
+constexpr int SORT_THREADS = 512;
+constexpr int SORT_SMALL_MAX_ATOMS = 32768, SORT_SMALL_CTAS = 32;   // small boxes: few CTAs, cheap barriers
+__global__ void __launch_bounds__(SORT_THREADS) k_sort(SortArgs a, Universe u, unsigned short *cum) {
     if (a.go && *a.go != a.want) return;   // (every CTA takes the same way: nobody is left waiting at a barrier)
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
-    __shared__ int part[SORT_SMALL_THREADS];
-    const int t = blockIdx.x * SORT_SMALL_THREADS + threadIdx.x, nt = gridDim.x * SORT_SMALL_THREADS, n = a.n, ncell = a.grid.ncell;
+    __shared__ int part[SORT_THREADS];
+    const int t = blockIdx.x * SORT_THREADS + threadIdx.x, nt = gridDim.x * SORT_THREADS, n = a.n, ncell = a.grid.ncell;
     for (int c = t; c <= ncell; c += nt) { a.cell_count[c] = 0; a.cell_fill[c] = 0; }
     grid.sync();
     for (int i = t; i < n; i += nt) cell_key_one(i, a.xs, a.grid, a.key, a.cell_count, a.ctr);
     grid.sync();
-    if (blockIdx.x == 0) scan_block(ncell, a.cell_count, a.cell_start, part);
+    if (ncell <= 4 * SCAN_SLICE) {
+        if (blockIdx.x == 0) scan_block(ncell, a.cell_count, a.cell_start, part);
+    } else {   // large grids: sums of 4096-cell slices, their scan by one CTA, then every slice from its offset
+        const int nslice = (ncell + SCAN_SLICE - 1) / SCAN_SLICE, tid = threadIdx.x;
+        constexpr int PER = SCAN_SLICE / SORT_THREADS;   // cells per thread and slice
+        for (int sl = blockIdx.x; sl < nslice; sl += gridDim.x) {
+            int sum = 0;
+            for (int k = 0; k < PER; ++k) { const int cc = sl * SCAN_SLICE + k * SORT_THREADS + tid; sum += cc < ncell ? a.cell_count[cc] : 0; }
+            __syncthreads();
+            part[tid] = sum;
+            __syncthreads();
+            for (int off = SORT_THREADS / 2; off > 0; off >>= 1) { if (tid < off) part[tid] += part[tid + off]; __syncthreads(); }
+            if (tid == 0) a.scan_sums[sl] = part[0];
+        }
+        grid.sync();
+        if (blockIdx.x == 0) scan_block(nslice, a.scan_sums, a.scan_offs, part);
+        grid.sync();
+        for (int sl = blockIdx.x; sl < nslice; sl += gridDim.x) {
+            const int lo = sl * SCAN_SLICE + PER * tid;
+            int cnt[PER], sum = 0;
+#pragma unroll
+            for (int k = 0; k < PER; ++k) { cnt[k] = lo + k < ncell ? a.cell_count[lo + k] : 0; sum += cnt[k]; }
+            __syncthreads();
+            part[tid] = sum;
+            __syncthreads();
+            for (int off = 1; off < SORT_THREADS; off <<= 1) {
+                const int v = tid >= off ? part[tid - off] : 0;
+                __syncthreads();
+                part[tid] += v;
+                __syncthreads();
+            }
+            int run = a.scan_offs[sl] + part[tid] - sum;
+#pragma unroll
+            for (int k = 0; k < PER; ++k) { if (lo + k < ncell) a.cell_start[lo + k] = run; run += cnt[k]; }
+            if (lo <= ncell - 1 && ncell - 1 < lo + PER) a.cell_start[ncell] = run;
+        }
+    }
     grid.sync();
     for (int i = t; i < n; i += nt) scatter_one(i, a.key, a.orig, a.cell_start, a.cell_fill, a.tmp_orig, a.tmp_src);
     grid.sync();
@@ -693,7 +607,6 @@ __global__ void __launch_bounds__(SORT_SMALL_THREADS) k_sort_small(SortArgs a, U
     for (int h = t >> 5; h < ncell; h += nt >> 5) universe_cell(a.grid, u, a.cell_start, cum, a.ctr, h, t & 31);
 }
 
-static inline int nblk(int n, int b) { return (n + b - 1) / b; }
 // CTAs of a grid that fills the current device once with per_sm CTAs on every SM
 static int resident_ctas(int per_sm) {
     static int sms[64] = {0};
@@ -708,46 +621,13 @@ static int resident_ctas(int per_sm) {
     return sms[dev] * per_sm;
 }
 
-// uni_cum != NULL: the running sums of the cell universe are wanted too; returns true if this call made them (small
-// boxes), false if launch_universe has to follow
-bool launch_sort(const SortArgs &a, const Universe &u, unsigned short *uni_cum, cudaStream_t st, int64_t *launches) {
-    const int B = 256;
-    if (a.n <= SORT_SMALL_MAX_ATOMS && a.grid.ncell <= SORT_SMALL_MAX_CELLS) {
-        SortArgs aa = a;
-        Universe uu = u;
-        void *args[] = {(void *)&aa, (void *)&uu, (void *)&uni_cum};
-        cudaLaunchCooperativeKernel((const void *)k_sort_small, dim3(SORT_SMALL_CTAS), dim3(SORT_SMALL_THREADS), args, 0, st);
-        *launches += 1;
-        return true;
-    }
-    cudaMemsetAsync(a.cell_count, 0, sizeof(int) * (a.grid.ncell + 1), st);   // (scratch: harmless when the sort does not run)
-    cudaMemsetAsync(a.cell_fill, 0, sizeof(int) * (a.grid.ncell + 1), st);
-    k_cell_key<<<nblk(a.n, B), B, 0, st>>>(a.n, a.xs, a.grid, a.key, a.cell_count, a.ctr, a.go, a.want);
-    if (a.grid.ncell <= 4 * SCAN_SLICE) {
-        k_scan<<<1, 1024, 0, st>>>(a.grid.ncell, a.cell_count, a.cell_start, a.go, a.want);
-    } else {
-        const int nb = nblk(a.grid.ncell, SCAN_SLICE);
-        k_scan_sums<<<nb, 256, 0, st>>>(a.grid.ncell, a.cell_count, a.scan_sums, a.go, a.want);
-        k_scan<<<1, 1024, 0, st>>>(nb, a.scan_sums, a.scan_offs, a.go, a.want);
-        k_scan_slices<<<nb, SCAN_SLICE / 4, 0, st>>>(a.grid.ncell, a.cell_count, a.scan_offs, a.cell_start, a.go, a.want);
-        *launches += 2;
-    }
-    k_scatter<<<nblk(a.n, B), B, 0, st>>>(a.n, a.key, a.orig, a.cell_start, a.cell_fill, a.tmp_orig, a.tmp_src, a.go, a.want);
-    k_cell_sort<<<nblk(a.grid.ncell, B), B, 0, st>>>(a.grid.ncell, a.cell_start, a.tmp_orig, a.tmp_src, a.go, a.want);
-    k_permute<<<nblk(a.n, B), B, 0, st>>>(a.n, a.tmp_src, a.tmp_orig, a.xs, a.vs, a.xl, a.xl_t, a.lj, a.mi, a.hw, a.hw_t, a.xs_t, a.vs_t,
-                                          a.lj_t, a.mi_t, a.orig_t, a.sorted_of, a.x_build, a.key, a.cell_of, a.grid.gn[0],
-                                          a.grid.gn[1], a.ctr, a.go, a.want);
-    k_copyback<<<nblk(a.n, B), B, 0, st>>>(a.n, a.xs_t, a.vs_t, a.xl_t, a.lj_t, a.mi_t, a.hw_t, a.hw, a.orig_t, a.xs, a.vs, a.xl, a.lj, a.mi, a.orig,
-                                           a.go, a.want);
-    *launches += 6;
-    return false;
-}
-
-void launch_universe(const SortGrid &g, const Universe &u, const int *cell_start, unsigned short *cum, Counters *ctr,
-                     const int *go, int want, cudaStream_t st, int64_t *launches) {
-    const int B = 128;
-    const long long need = ((long long)g.ncell * 32 + B - 1) / B;
-    k_universe<<<(unsigned)std::min<long long>(need, resident_ctas(16)), B, 0, st>>>(g, u, cell_start, cum, ctr, go, want);
+// uni_cum != NULL: the running sums of the cell universe are made too
+void launch_sort(const SortArgs &a, const Universe &u, unsigned short *uni_cum, cudaStream_t st, int64_t *launches) {
+    SortArgs aa = a;
+    Universe uu = u;
+    void *args[] = {(void *)&aa, (void *)&uu, (void *)&uni_cum};
+    const int ctas = a.n <= SORT_SMALL_MAX_ATOMS ? SORT_SMALL_CTAS : resident_ctas(2);
+    cudaLaunchCooperativeKernel((const void *)k_sort, dim3(ctas), dim3(SORT_THREADS), args, 0, st);
     *launches += 1;
 }
 int launch_universe_list(const SortGrid &g, const Universe &u, const int *cell_start, int home, int *out, int n,
