@@ -626,7 +626,7 @@ void launch_sort(const SortArgs &a, const Universe &u, unsigned short *uni_cum, 
     SortArgs aa = a;
     Universe uu = u;
     void *args[] = {(void *)&aa, (void *)&uu, (void *)&uni_cum};
-    const int ctas = a.n <= SORT_SMALL_MAX_ATOMS ? SORT_SMALL_CTAS : resident_ctas(2);
+    const int ctas = a.n <= SORT_SMALL_MAX_ATOMS ? SORT_SMALL_CTAS : resident_ctas(3);
     cudaLaunchCooperativeKernel((const void *)k_sort, dim3(ctas), dim3(SORT_THREADS), args, 0, st);
     *launches += 1;
 }
