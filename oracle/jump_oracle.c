@@ -57,6 +57,18 @@
 #ifdef _OPENMP
 #include <omp.h>
 #endif
+/* threads for the loops over n atoms: one per 256 atoms (a 192-atom box on 8 threads spent its
+ * time waiting at barriers -- minutes when the host was busy; nothing but the speed depends on it) */
+static int orc_threads(int n) {
+#ifdef _OPENMP
+    int t = n / 256, m = omp_get_max_threads();
+    if (t < 1) t = 1;
+    return t < m ? t : m;
+#else
+    (void)n;
+    return 1;
+#endif
+}
 
 #define ORC_KB 1.987204259e-3 /* kcal/mol/K */
 #define ORC_COULOMB 332.063713 /* kcal A / (mol e^2) */
@@ -392,7 +404,7 @@ static void neighbor_csr_audit(const orc_ctx *c, const double *x, double rmin, d
     }
     int *cnt = calloc(n + 1, sizeof(int));
     uint64_t **rows = malloc(sizeof(uint64_t *) * n);
-#pragma omp parallel for if (c->n >= 64) schedule(dynamic, 64) reduction(min : emin)
+#pragma omp parallel for num_threads(orc_threads(c->n)) schedule(dynamic, 64) reduction(min : emin)
     for (int i = 0; i < n; ++i) {
         int cap = 64, m = 0;
         uint64_t *row = malloc(sizeof(uint64_t) * cap);
@@ -494,7 +506,7 @@ static double pairs_accumulate(const orc_ctx *c, int wC, int wLJ, int brute, dou
     int *ptr, *idx;
     neighbor_csr(c, c->x, 0.0, rmax, 0, brute, &ptr, &idx);
     double etot = 0.0;
-#pragma omp parallel for if (c->n >= 64) schedule(dynamic, 64) reduction(+ : etot)
+#pragma omp parallel for num_threads(orc_threads(c->n)) schedule(dynamic, 64) reduction(+ : etot)
     for (int i = 0; i < c->n; ++i) {
         double acc[3] = {0, 0, 0}, e = 0.0;
         for (int k = ptr[i]; k < ptr[i + 1]; ++k) {
@@ -775,7 +787,7 @@ static void rebuild_universe(orc_ctx *c) {
     memcpy(fill, c->cell_ptr, sizeof(int) * ncell);
     for (int i = 0; i < n; ++i) c->cell_atoms[fill[c->home[i]]++] = i; /* ascending i within a cell */
     free(fill);
-#pragma omp parallel for schedule(dynamic, 64)
+#pragma omp parallel for num_threads(orc_threads(c->n)) schedule(dynamic, 64)
     for (int h = 0; h < ncell; ++h) c->uni_cnt[h] = (c->cell_ptr[h + 1] > c->cell_ptr[h]) ? universe_walk(c, h, -1) : 0;
 }
 static int universe_count(const orc_ctx *c, int i) { return c->uni_cnt[c->home[i]]; }
@@ -1073,7 +1085,7 @@ static void chain_atom(orc_ctx *c, int i, int lj, double H, const double a[3], i
 static void phase_C(orc_ctx *c, double H, const double *grad, int stream, int64_t step, int mode) {
     int64_t np = 0, nacc = 0, ngt = 0, nexp = 0;
     double mp = 0.0, mgl = 0.0;
-#pragma omp parallel for if (c->n >= 64) schedule(dynamic, 64) reduction(+ : np, nacc, ngt, nexp) reduction(max : mp, mgl)
+#pragma omp parallel for num_threads(orc_threads(c->n)) schedule(dynamic, 64) reduction(+ : np, nacc, ngt, nexp) reduction(max : mp, mgl)
     for (int i = 0; i < c->n; ++i) {
         double a[3] = {0, 0, 0};
         if (grad)
@@ -1088,7 +1100,7 @@ static void phase_J(orc_ctx *c, double H, int stream, int64_t step) {
     int64_t np = 0, nacc = 0, ngt = 0, nexp = 0;
     double mp = 0.0, mgl = 0.0;
     const double zero[3] = {0.0, 0.0, 0.0};
-#pragma omp parallel for if (c->n >= 64) schedule(dynamic, 64) reduction(+ : np, nacc, ngt, nexp) reduction(max : mp, mgl)
+#pragma omp parallel for num_threads(orc_threads(c->n)) schedule(dynamic, 64) reduction(+ : np, nacc, ngt, nexp) reduction(max : mp, mgl)
     for (int i = 0; i < c->n; ++i) chain_atom(c, i, 1, H, zero, stream, step, &np, &nacc, &ngt, &nexp, &mp, &mgl);
     c->st.proposals += np; c->st.accepts += nacc; c->st.expiries += nexp;
     if (mp > c->st.max_p) c->st.max_p = mp;
@@ -1193,7 +1205,7 @@ static double slow_accumulate(const orc_ctx *c, double *out) {
     const double V = c->p.box[0] * c->p.box[1] * c->p.box[2];
     double e = 0.0;
     double *Sr = malloc(sizeof(double) * (nk > 0 ? nk : 1)), *Si = malloc(sizeof(double) * (nk > 0 ? nk : 1));
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for num_threads(orc_threads(c->n)) schedule(static)
     for (int m = 0; m < nk; ++m) {
         const double kx = 2.0 * ORC_PI * c->kn[3 * m] / c->p.box[0], ky = 2.0 * ORC_PI * c->kn[3 * m + 1] / c->p.box[1],
                      kz = 2.0 * ORC_PI * c->kn[3 * m + 2] / c->p.box[2];
@@ -1211,7 +1223,7 @@ static double slow_accumulate(const orc_ctx *c, double *out) {
         /* half space: twice the (1/2V) term */
         e += (ORC_COULOMB / V) * (4.0 * ORC_PI / k2) * exp(-k2 / (4.0 * c->alpha * c->alpha)) * (Sr[m] * Sr[m] + Si[m] * Si[m]);
     }
-#pragma omp parallel for schedule(static)
+#pragma omp parallel for num_threads(orc_threads(c->n)) schedule(static)
     for (int i = 0; i < n; ++i) {
         double g[3] = {0, 0, 0};
         for (int m = 0; m < nk; ++m) {
