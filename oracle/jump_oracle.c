@@ -57,11 +57,11 @@
 #ifdef _OPENMP
 #include <omp.h>
 #endif
-/* threads for the loops over n atoms: one per 256 atoms (a 192-atom box on 8 threads spent its
+/* threads for the loops over n atoms: one per 128 atoms (a 192-atom box on 8 threads spent its
  * time waiting at barriers -- minutes when the host was busy; nothing but the speed depends on it) */
 static int orc_threads(int n) {
 #ifdef _OPENMP
-    int t = n / 256, m = omp_get_max_threads();
+    int t = n / 128, m = omp_get_max_threads();
     if (t < 1) t = 1;
     return t < m ? t : m;
 #else
