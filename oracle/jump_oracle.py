@@ -409,6 +409,15 @@ def velocity_autocorrelation(v_origin, v_now, select=None):
     return float((a * b).sum(1).mean())
 
 
+def mean_square_displacement(x_origin_unwrapped, x_now_unwrapped, select=None):
+    """NEXT-4 oracle: MSD = (1/N_sel) sum_{i in sel} |x_i(t0 + tau) - x_i(t0)|^2, A^2, on UNWRAPPED positions -- the plain
+    definition behind the diffusion constants D = lim MSD / (6 tau) of P:L527, L575-581, fp64."""
+    a, b = np.asarray(x_origin_unwrapped, dtype=np.float64), np.asarray(x_now_unwrapped, dtype=np.float64)
+    if select is not None:
+        a, b = a[select], b[select]
+    return float(((b - a) ** 2).sum(1).mean())
+
+
 def vacf_spectrum(c, dt_ps, omegas):
     """I(omega) = dt [C(0)/2 + sum_{k>=1} C(k dt) cos(omega k dt) w_k] with a Hann window w_k = cos^2(pi k / 2K) over the K
     lags given: the windowed cosine transform of the autocorrelation (the velocity spectra of P:L529-531), fp64."""

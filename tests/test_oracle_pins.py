@@ -1140,3 +1140,26 @@ def test_combined_mechanism_event_log_and_bounds(relaxed_small):
         o2.jump_step(40)
         counts[name] = o2.stats()["proposals"]
     assert counts["coul"] < n_comb < 2 * counts["two"]
+
+
+def test_mean_square_displacement_of_free_flight_is_v2_t2():
+    """NEXT-4: the mean-square displacement on unwrapped positions.  Non-interacting atoms (no charge, no LJ, no bonds)
+    without friction fly straight: MSD(t) = <|v|^2> t^2 exactly, also after every atom has left the periodic box several
+    times (on wrapped positions it would saturate at the box size); a subset selects."""
+    n = 96
+    rng = np.random.default_rng(31)
+    z = np.zeros(0)
+    box = 12.0
+    sysd = dict(n_atoms=n, box=box, pos=rng.uniform(0, box, (n, 3)), vel=rng.normal(size=(n, 3)) * 30.0,
+                mass=np.full(n, 12.0), charge=np.zeros(n), lj_sigma=np.ones(n), lj_eps=np.zeros(n),
+                bond_ij=np.zeros((0, 2), dtype=np.int32), bond_k=z, bond_r0=z, angle_ijk=np.zeros((0, 3), dtype=np.int32),
+                angle_k=z, angle_t0=z, excl_ptr=np.zeros(n + 1, dtype=np.int32), excl_idx=np.zeros(0, dtype=np.int32))
+    o = jo.Oracle(sysd, r_short=3.0, r_long=5.0, r_mid=4.0, skin=0.5, nlist_every=5, dt_fs=2.0, gamma_per_ps=0.0, flags=3, seed=3)
+    x0, v0 = o.pos_unwrapped, o.vel
+    o.jump_step(1000)                                   # 2 ps at 30 A/ps: 60 A, five box lengths
+    t = 2.0
+    sel = np.arange(n) % 3 == 0
+    assert np.abs(o.pos).max() <= box and np.abs(o.pos_unwrapped - x0).max() > 3 * box
+    assert jo.mean_square_displacement(x0, o.pos_unwrapped) == pytest.approx((v0 ** 2).sum(1).mean() * t * t, rel=1e-9)
+    assert jo.mean_square_displacement(x0, o.pos_unwrapped, sel) == pytest.approx((v0[sel] ** 2).sum(1).mean() * t * t, rel=1e-9)
+    assert jo.mean_square_displacement(x0, o.pos) < 3 * box * box < jo.mean_square_displacement(x0, o.pos_unwrapped)
