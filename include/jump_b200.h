@@ -158,6 +158,13 @@ int jump_get_images(jump_ctx *c, int32_t *d_img);
  * carriers; fp64 sums in a fixed order.  Synchronises; JUMP_E_ARG before a mark. */
 int jump_vacf_mark(jump_ctx *c);
 int jump_vacf_dot(jump_ctx *c, int32_t lj_only, double *c_out);
+/* Mean-square displacement (the diffusion constants of P:L527, L575-581 are its long-time slope / 6).  jump_msd_mark stores
+ * the current UNWRAPPED positions (d_pos + image counters x box, fp64), by original atom index, as the time origin
+ * (asynchronous).  jump_msd writes *msd_out = (1/N_sel) sum_{i in sel} |x_i(now) - x_i(origin)|^2 in A^2 (host double), sel
+ * as in jump_vacf_dot; fp64 sums in a fixed order.  Synchronises; JUMP_E_ARG before a mark.  A jump_refresh (not
+ * jump_refresh_lazy) resets the image counters and with them the continuity of the unwrapped positions. */
+int jump_msd_mark(jump_ctx *c);
+int jump_msd(jump_ctx *c, int32_t lj_only, double *msd_out);
 int jump_rdf_accumulate(jump_ctx *c, int32_t lj_only, double r_max, int32_t n_bins, uint64_t *d_hist);
 /* The same sum for callers that may not allocate (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
  * no context, no cudaMalloc / cudaFree, the per-CTA partial sums in a 256 KiB file-scope device array of the library

@@ -23,7 +23,7 @@ EXPORTS = ["jump_init", "jump_step", "baoab_step", "jump_respa_step", "jump_get_
            "jump_get_stats", "jump_reset_stats", "jump_get_events", "jump_clear_events", "jump_get_row", "jump_get_images", "jump_rdf_accumulate",
            "jump_get_bounds", "jump_refresh", "jump_refresh_lazy", "jump_half", "jump_sync", "jump_get_step", "jump_get_launches",
            "jump_last_error", "jump_free", "jump_set_profiling", "jump_get_profile", "jump_count_pairs",
-           "jump_ewald_setup", "jump_respa1_step", "jump_get_slow_energy", "jump_vacf_mark", "jump_vacf_dot", "jump_set_lanes", "jump_set_lax_skin",
+           "jump_ewald_setup", "jump_respa1_step", "jump_get_slow_energy", "jump_vacf_mark", "jump_vacf_dot", "jump_msd_mark", "jump_msd", "jump_set_lanes", "jump_set_lax_skin",
            "jump_vacf_static_setup", "jump_vacf_dot_static", "jump_vacf_static_last_error"]
 
 
@@ -80,6 +80,8 @@ def lib():
         L.jump_ewald_setup.argtypes = [vp, C.c_double, C.POINTER(C.c_int32)]
         L.jump_respa1_step.argtypes = [vp, i32, i32]
         L.jump_get_slow_energy.argtypes = [vp, C.POINTER(C.c_double)]
+        L.jump_msd_mark.argtypes = [vp]
+        L.jump_msd.argtypes = [vp, i32, C.POINTER(C.c_double)]
         L.jump_vacf_mark.argtypes = [vp]
         L.jump_vacf_dot.argtypes = [vp, i32, C.POINTER(C.c_double)]
         L.jump_get_forces.argtypes = [vp, i32, vp]
@@ -230,6 +232,15 @@ class JumpSim:
 
     def jump_respa1_step(self, n=1, n_mid=3):
         self._check(self._L.jump_respa1_step(self._h, int(n), int(n_mid)), "jump_respa1_step")
+
+    def msd_mark(self):
+        self._check(self._L.jump_msd_mark(self._h), "jump_msd_mark")
+
+    def msd(self, lj_only=False):
+        """(1/N_sel) sum |x_i(now) - x_i(mark)|^2 on unwrapped positions, A^2."""
+        out = C.c_double(0.0)
+        self._check(self._L.jump_msd(self._h, int(bool(lj_only)), C.byref(out)), "jump_msd")
+        return float(out.value)
 
     def vacf_mark(self):
         self._check(self._L.jump_vacf_mark(self._h), "jump_vacf_mark")

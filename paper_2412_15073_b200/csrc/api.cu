@@ -49,6 +49,8 @@ struct jump_ctx {
     double q2sum;            // sum of q_i^2 (self term)
     float4 *vacf_v0;         // velocities at the time origin of the autocorrelation, by original atom index
     double2 *vacf_part;
+    double *msd_x0;          // unwrapped positions at the time origin of the mean-square displacement, by original atom index
+    double2 *msd_part;
     bool slow_valid;         // fslow holds grad(U_rec + U_excl) at the current positions, in the current sorted order
     int64_t outer1;
 
@@ -1007,7 +1009,7 @@ extern "C" int jump_init(jump_ctx **out, const jump_params *p, float *d_pos, flo
     c->f0_valid = false;
     c->slow_valid = false;
     memset(&c->ew, 0, sizeof c->ew);
-    c->vacf_v0 = nullptr; c->vacf_part = nullptr;
+    c->vacf_v0 = nullptr; c->vacf_part = nullptr; c->msd_x0 = nullptr; c->msd_part = nullptr;
     c->fslow = nullptr; c->ew_sum = nullptr; c->q2sum = 0.0; c->outer1 = 0;
     c->prof = false;
     c->lanes = 0; c->uni_cum = nullptr; c->cell_of = nullptr;
@@ -1176,6 +1178,26 @@ extern "C" int jump_rdf_accumulate(jump_ctx *c, int32_t lj_only, double r_max, i
                    (unsigned long long *)d_hist, c->st, &c->launches))
         return JUMP_E_ARG;
     CK(cudaGetLastError());
+    return 0;
+}
+extern "C" int jump_msd_mark(jump_ctx *c) {
+    if (!c) return JUMP_E_ARG;
+    int r;
+    if (!c->msd_x0 && ((r = dalloc(c, &c->msd_x0, 3 * (size_t)c->n)) || (r = dalloc(c, &c->msd_part, (size_t)(c->n + 255) / 256 + 1)))) return r;
+    launch_msd_mark(c->m, c->xs, c->xl, c->orig, c->msd_x0, c->st, &c->launches);
+    CK(cudaGetLastError());
+    return 0;
+}
+extern "C" int jump_msd(jump_ctx *c, int32_t lj_only, double *msd_out) {
+    if (!c || !msd_out) return JUMP_E_ARG;
+    if (!c->msd_x0) { c->err = "jump_msd_mark has not been called"; return JUMP_E_ARG; }
+    const size_t nb = (size_t)(c->n + 255) / 256;
+    launch_msd_sum(c->m, lj_only != 0, c->xs, c->xl, c->orig, c->lj, c->msd_x0, c->msd_part, c->msd_part + nb, c->st, &c->launches);
+    CK(cudaGetLastError());
+    std::vector<double2> h;
+    int r = ddownload(c, h, (const double2 *)(c->msd_part + nb), 1);
+    if (r) return r;
+    *msd_out = h[0].y > 0.0 ? h[0].x / h[0].y : 0.0;
     return 0;
 }
 extern "C" int jump_vacf_mark(jump_ctx *c) {

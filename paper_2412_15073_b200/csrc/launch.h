@@ -97,6 +97,9 @@ void launch_reload(const Model &m, const float *pos, const float *vel, const int
                    float4 *xl, const float4 *x_build, int *moved, int keep, const float2 *mi, cudaStream_t st, int64_t *launches);
 int launch_rdf(const Model &m, const SortGrid &g, int lj_only, double r_max, double r_reach, int n_bins, const int *cell_start,
                const float4 *xs, const float2 *lj, unsigned long long *hist, cudaStream_t st, int64_t *launches);
+void launch_msd_mark(const Model &m, const float4 *xs, const float4 *xl, const int *orig, double *x0, cudaStream_t st, int64_t *launches);
+void launch_msd_sum(const Model &m, int lj_only, const float4 *xs, const float4 *xl, const int *orig, const float2 *lj, const double *x0,
+                    double2 *part, double2 *out, cudaStream_t st, int64_t *launches);
 void launch_vacf_mark(int n, const float4 *vs, const int *orig, float4 *v0, cudaStream_t st, int64_t *launches);
 void launch_vacf_dot(int n, int lj_only, const float4 *vs, const float4 *v0, const int *orig, const float2 *lj, double2 *part,
                      double2 *out, cudaStream_t st, int64_t *launches);

@@ -108,6 +108,60 @@ void launch_vacf_dot(int n, int lj_only, const float4 *vs, const float4 *v0, con
     *launches += 2;
 }
 
+// Mean-square displacement on unwrapped positions (the diffusion constants of P:L527, L575-581 are its slope / 6): the
+// unwrapped position x + image * box (fp64: hi + lo + image counters, see update.cu) at the time origin is kept by
+// ORIGINAL atom index; MSD = (1/N_sel) sum |x_i(now) - x_i(origin)|^2, per-CTA partial sums in a fixed order.
+__device__ inline void unwrapped(const Model &m, const float4 *__restrict__ xs, const float4 *__restrict__ xl, int i, double out[3]) {
+    const float4 a = xs[i], b = xl[i];
+    int ix, iy, iz;
+    img_unpack(__float_as_int(b.w), ix, iy, iz);
+    out[0] = (double)a.x + (double)b.x + (double)ix * (double)m.box[0];
+    out[1] = (double)a.y + (double)b.y + (double)iy * (double)m.box[1];
+    out[2] = (double)a.z + (double)b.z + (double)iz * (double)m.box[2];
+}
+__global__ void k_msd_mark(Model m, const float4 *__restrict__ xs, const float4 *__restrict__ xl, const int *__restrict__ orig,
+                           double *__restrict__ x0) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m.n) return;
+    double u[3];
+    unwrapped(m, xs, xl, i, u);
+    const size_t o = 3 * (size_t)orig[i];
+    x0[o] = u[0]; x0[o + 1] = u[1]; x0[o + 2] = u[2];
+}
+__global__ void __launch_bounds__(256) k_msd_sum(Model m, int lj_only, const float4 *__restrict__ xs, const float4 *__restrict__ xl,
+                                                 const int *__restrict__ orig, const float2 *__restrict__ lj,
+                                                 const double *__restrict__ x0, double2 *__restrict__ part) {
+    __shared__ double s_d[256], s_c[256];
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    double d = 0.0, cnt = 0.0;
+    if (i < m.n && (!lj_only || lj[i].y > 0.f)) {
+        double u[3];
+        unwrapped(m, xs, xl, i, u);
+        const size_t o = 3 * (size_t)orig[i];
+        const double dx = u[0] - x0[o], dy = u[1] - x0[o + 1], dz = u[2] - x0[o + 2];
+        d = dx * dx + dy * dy + dz * dz;
+        cnt = 1.0;
+    }
+    s_d[threadIdx.x] = d; s_c[threadIdx.x] = cnt;
+    __syncthreads();
+    for (int off = 128; off > 0; off >>= 1) {
+        if (threadIdx.x < off) { s_d[threadIdx.x] += s_d[threadIdx.x + off]; s_c[threadIdx.x] += s_c[threadIdx.x + off]; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) part[blockIdx.x] = make_double2(s_d[0], s_c[0]);
+}
+void launch_msd_mark(const Model &m, const float4 *xs, const float4 *xl, const int *orig, double *x0, cudaStream_t st, int64_t *launches) {
+    k_msd_mark<<<(m.n + 255) / 256, 256, 0, st>>>(m, xs, xl, orig, x0);
+    *launches += 1;
+}
+void launch_msd_sum(const Model &m, int lj_only, const float4 *xs, const float4 *xl, const int *orig, const float2 *lj, const double *x0,
+                    double2 *part, double2 *out, cudaStream_t st, int64_t *launches) {
+    const int nb = (m.n + 255) / 256;
+    k_msd_sum<<<nb, 256, 0, st>>>(m, lj_only, xs, xl, orig, lj, x0, part);
+    k_vacf_final<<<1, 256, 0, st>>>(nb, part, out);
+    *launches += 2;
+}
+
 int launch_rdf(const Model &m, const SortGrid &g, int lj_only, double r_max, double r_reach, int n_bins, const int *cell_start,
                const float4 *xs, const float2 *lj, unsigned long long *hist, cudaStream_t st, int64_t *launches) {
     if (n_bins <= 0 || n_bins > RDF_MAX_BINS || !(r_max > 0.0)) return -1;

@@ -835,6 +835,34 @@ def test_velocity_autocorrelation_on_the_device(jb, jo, cfg0):
     assert o.step >= 10
 
 
+def test_mean_square_displacement_on_the_device(jb, jo, cfg0):
+    """NEXT-4: jump_msd_mark / jump_msd against the plain definition (oracle.mean_square_displacement) on the oracle's own
+    unwrapped positions of the same seeded run, along 40 JUMP steps (across re-sorts) to the accuracy the trajectories
+    agree to; then over 3 ps, long enough for atoms to cross the box faces, against the same sum formed on the host from
+    d_pos and the image counters; the LJ-carrier subset selects the oxygens."""
+    sysd, run = cfg0
+    g, o = jb.JumpSim(sysd, **run), jo.Oracle(sysd, **run)
+    with pytest.raises(RuntimeError):
+        g.msd()
+    g.msd_mark()
+    x0, x0g = o.pos_unwrapped, g.pos_unwrapped().cpu().numpy()
+    oxy = sysd["lj_eps"] > 0
+    assert g.msd() == 0.0
+    for _ in range(4):
+        g.jump_step(10); g.sync(); o.jump_step(10)
+        if fragile(o):
+            break
+        want, want_o = jo.mean_square_displacement(x0, o.pos_unwrapped), jo.mean_square_displacement(x0, o.pos_unwrapped, oxy)
+        assert g.msd() == pytest.approx(want, rel=2e-3, abs=1e-7) and g.msd(lj_only=True) == pytest.approx(want_o, rel=2e-3, abs=1e-7)
+    assert o.step >= 10
+    g.jump_step(3000); g.sync()
+    xg = g.pos_unwrapped().cpu().numpy()
+    assert np.abs(g.images().cpu().numpy()).max() >= 1                      # somebody has left the box
+    assert g.msd() == pytest.approx(jo.mean_square_displacement(x0g, xg), rel=1e-5)
+    assert g.msd(lj_only=True) == pytest.approx(jo.mean_square_displacement(x0g, xg, oxy), rel=1e-5)
+    assert 0.5 < g.msd() < 50.0                                             # A^2 after 3 ps of liquid water
+
+
 @pytest.mark.parametrize("form", ["blocked", "tables", "direct"])
 def test_slow_force_orthorhombic_box_and_both_kernel_forms(jb, jo, form, monkeypatch):
     """R-21 on a box with three different edges (different n_max per dimension: the table offsets and the tile grid of
