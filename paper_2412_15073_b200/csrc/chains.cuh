@@ -9,7 +9,12 @@ namespace jb {
 struct Tally {  // per-thread statistics, reduced once per warp at the end
     unsigned proposals, accepts, gt_attempts, expiries;
     float max_p, max_gl;
+    unsigned runaway;   // a chain was cut at kMaxChain proposals (reported as ERR_NAN: the state has blown up)
 };
+// A chain draws a few proposals per half-phase; with a non-finite or exploded velocity the bound lambda-bar is infinite,
+// every waiting time is 0 and the clock never reaches the end of the phase: the chain is cut and the error flagged
+// instead of spinning on the device for ever.
+constexpr unsigned kMaxChain = 1u << 14;
 
 __device__ inline void log_event(const UpdateArgs &a, unsigned step, int stream, int atom, int iter, int ring, int j,
                                  int accepted, int n_gt, float T, float p, float U, float gt) {

@@ -143,6 +143,7 @@ __device__ void chain_C(const Model &m, const UpdateArgs &A, bool on, const Chai
             else if (f < 0 && gl == n_alive)
                 log_event(A, step, stream, atom, (int)kb + gl, -1, -1, 0, 0, T_, 0.f, 0.f, 0.f);
         }
+        if (kb > kMaxChain) { done = true; tl.runaway = 1u; }
         if (f >= 0) kb += (unsigned)(f + 1);
         else if (n_alive < G) {   // expired inside this batch
             done = true;
@@ -171,6 +172,7 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, const ChainConst &c
     unsigned block = 0;
     uint32_t w[4];
     for (int iter = 0;; ++iter) {
+        if ((unsigned)iter > kMaxChain) { tl.runaway = 1u; break; }
         float vv = sqrtf(vx * vx + vy * vy + vz * vz);
         float lam = S * (m.beta * vv);
         philox4x32_10(atom, step, stream, block++, m.key0, m.key1, w);
@@ -233,7 +235,7 @@ __global__ void __launch_bounds__(128, 8) k_update(Model m, UpdateArgs A) {
         i = blockIdx.x * 128 + s_perm[threadIdx.x];
     }
     const bool live = i < m.n, lead = gl == 0;
-    Tally tl = {0u, 0u, 0u, 0u, 0.f, 0.f};
+    Tally tl = {0u, 0u, 0u, 0u, 0.f, 0.f, 0u};
     float disp2 = 0.f;
     bool bad = false;
     float4 xi = make_float4(0.f, 0.f, 0.f, 0.f), v4 = xi;
@@ -336,7 +338,7 @@ __global__ void __launch_bounds__(128, 8) k_update(Model m, UpdateArgs A) {
     if (threadIdx.x < 8) s_stat[threadIdx.x] = 0u;
     __syncthreads();
     unsigned err = 0;
-    if (bad) err |= ERR_NAN;
+    if (bad || tl.runaway) err |= ERR_NAN;
     if (tl.max_p > 1.f + 1e-4f || tl.max_gl > 1.f + 1e-4f) err |= ERR_BOUND;
     unsigned d2b = __reduce_max_sync(full, __float_as_uint(disp2));
     err = __reduce_or_sync(full, err);

@@ -182,3 +182,36 @@ def test_config1_jump_vs_baoab_10000_steps(jb):
     # water at gamma = 1 / ps is about 1 ps), so each standard deviation is known to +-22 % and their ratio to +-31 % (one
     # sigma); repeated runs gave 0.57 and 0.69.  Checked as "the same order", three sigma.
     assert 0.4 < res["jump"][2] / res["baoab"][2] < 2.5
+
+
+def test_bounce_heats_where_jump_does_not(jb):
+    """NEXT-3 / P:L315-319: "the BPS electrostatic jumps can only be done on a very small range.  Jumping on a larger range
+    yields too many velocity bounces" -- BOUNCE (eps = inf, B J A O A J B) on the 5-9 A range at delta = 1 fs heats the
+    216-water box by hundreds of K within 400 steps and blows up; fusing the force and jump steps (C'J' A O A J'C' with
+    eps = inf) "stabilizes further": it heats several times more slowly; the general mechanism with eps = 1 stays
+    at the thermostat's temperature.  The blown-up run ends with a device error within seconds (chains are cut at 16 384
+    proposals: an exploded velocity makes every waiting time 0), not with a kernel that never returns."""
+    sysd, run = wl.make_config(0)
+    n = sysd["n_atoms"]
+    T = {}
+    for name, kw in (("bounce", dict(eps_jump=float("inf"), flags=3 | jb.F_BJAOAJB)), ("fused_inf", dict(eps_jump=float("inf"), flags=3)),
+                     ("jump", dict(eps_jump=1.0, flags=3))):
+        g = jb.JumpSim(sysd, **dict(run, seed=run["seed"] + 41, **kw))
+        g.set_lax_skin(True)
+        g.baoab_step(3000)                                   # the same equilibrated start for the three
+        g.jump_step(300)
+        t = []
+        for _ in range(5):
+            g.jump_step(20)
+            t.append(2.0 * g.energy()[0] / (3.0 * n * KB))
+        T[name] = float(np.mean(t))                          # kinetic temperature over steps 300-400
+        if name == "bounce":
+            with pytest.raises(jb.JumpError):                # non-finite state, row overflow or a bound violated: it blows up
+                for _ in range(40):
+                    g.jump_step(100); g.sync()
+        else:
+            assert g.stats()["error"] == 0
+        g.close()
+    print("bounce", T)
+    assert T["bounce"] > 420.0 and abs(T["jump"] - 300.0) < 25.0
+    assert T["jump"] + 20.0 < T["fused_inf"] < T["bounce"] - 40.0
