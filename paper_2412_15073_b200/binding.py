@@ -121,7 +121,7 @@ def lib():
 
 def make_params(n_atoms, box, r_short, r_long, r_switch=0.5, r_mid=None, ewald_alpha=-1.0, dt_fs=1.0, gamma_per_ps=1.0,
                 temperature_K=300.0, n_inner=4, eps_jump=1.0, eps_mode=0, flags=F_COUL_JUMPS | F_LJ_JUMPS, skin=1.0,
-                nlist_every=10, seed=0, cell_edge=0.0, r_mid_in=None, **_ignored):
+                nlist_every=24, seed=0, cell_edge=0.0, r_mid_in=None, **_ignored):
     p = jump_params()
     p.n_atoms, p.n_inner, p.eps_mode, p.flags = int(n_atoms), int(n_inner), int(eps_mode), int(flags)
     p.nlist_every, p.seed = int(nlist_every), int(seed)
