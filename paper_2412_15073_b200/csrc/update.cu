@@ -211,6 +211,9 @@ __device__ void chain_J(const Model &m, const UpdateArgs &A, const ChainConst &c
 template <bool JUMPS, int G, bool LOG, int MECH>
 __global__ void __launch_bounds__(128, 8) k_update(Model m, UpdateArgs A) {
     const unsigned full = 0xffffffffu;
+    // a non-finite or blown-up state was flagged by an earlier launch: it is reported at the next synchronising call, and
+    // until then the steps already enqueued do nothing (their chains would each run to the cut, 16 384 proposals)
+    if (A.ctr->err & (unsigned)ERR_NAN) return;
     const int gt_id = blockIdx.x * blockDim.x + threadIdx.x;
     int i = gt_id / G;
     const int gl = gt_id % G;
