@@ -215,3 +215,44 @@ def test_bounce_heats_where_jump_does_not(jb):
     print("bounce", T)
     assert T["bounce"] > 420.0 and abs(T["jump"] - 300.0) < 25.0
     assert T["jump"] + 20.0 < T["fused_inf"] < T["bounce"] - 40.0
+
+
+def test_config3_solute_jump_vs_baoab(jb):
+    """BASELINE configs[3] ("JUMP vs BAOAB", 2 500-bead charged chain in water, 23 558 atoms, delta = 1 fs).  The generator's
+    state (chain laid through lattice sites) is far from equilibrium and explodes at 1 fs, so both schemes start from the same
+    staged BAOAB relaxation on the device (0.05 fs at gamma = 200 / ps up to 1 fs at gamma = 1 / ps, 10 000 steps in all);
+    then 6 000 steps each: no device error with the skin check on, thinning bounds never violated (the chain's LJ
+    parameters span sigma in [3, 4] A: the sup over sigma of R-7), rows within capacity, both kinetic temperatures near
+    300 K and the potential energy per atom of JUMP within the second-order gap of BAOAB's."""
+    sysd, run = wl.make_config(3)
+    n = sysd["n_atoms"]
+    pos, vel = sysd["pos"], sysd["vel"]
+    for dt, gam, steps in ((0.05, 200.0, 2000), (0.2, 100.0, 2000), (0.5, 20.0, 2000), (1.0, 5.0, 2000), (1.0, 1.0, 2000)):
+        g = jb.JumpSim(dict(sysd, pos=pos, vel=vel), **dict(run, dt_fs=dt, gamma_per_ps=gam))
+        g.set_lax_skin(True)
+        g.baoab_step(steps); g.sync()
+        pos, vel = g.pos.cpu().numpy().astype(np.float64), g.vel.cpu().numpy().astype(np.float64)
+        g.close()
+    res = {}
+    for name in ("jump", "baoab"):
+        # nlist_every = 4: a rebuild may follow the previous one at once (Q = 1, R-10c).  The freely jointed chain has rare
+        # violent close contacts (a bead thrown at 100 A/ps, 20 thermal sigmas) that use up a bead's share of the skin within
+        # two steps; with the default period that is reported as JUMP_E_SKIN ("skin too small for this system")
+        g = jb.JumpSim(dict(sysd, pos=pos, vel=vel), **dict(run, seed=run["seed"] + 51, nlist_every=4))
+        step = g.jump_step if name == "jump" else g.baoab_step
+        step(2000); g.sync()
+        g.reset_stats()
+        T, U = [], []
+        for _ in range(200):
+            step(20)
+            ek, ep = g.energy()
+            T.append(2.0 * ek / (3.0 * n * KB)); U.append(ep / n)
+        st = g.stats()
+        assert st["error"] == 0 and st["max_p"] <= 1 + 1e-4 and st["max_g_over_L"] <= 1 + 1e-4
+        assert all(m <= c for m, c in zip(st["max_row"], st["cap_row"]) if c)
+        res[name] = (ob.block_mean_se(T), ob.block_mean_se(U))
+        g.close()
+    print("config3", res)
+    assert abs(res["jump"][0][0] - 300.0) < 12.0 and abs(res["baoab"][0][0] - 300.0) < 15.0
+    gap = res["jump"][1][0] - res["baoab"][1][0]                 # kcal/mol per ATOM here (a third of the per-molecule figure)
+    assert -0.03 < gap < 0.12, gap
