@@ -440,7 +440,7 @@ def main():
                                           "JUMP-RESPA n_inner %d (outer step %.0f fs; one step = one inner step)" % (run["n_inner"], run["n_inner"] * dt_fs)
                                           if respa else "JUMP (C'J'AOAJ'C')", args.equil),
                            "eps_jump": run["eps_jump"], "r_mid_in": run["r_mid_in"], "r_mid": run["r_mid"], "skin": run["skin"],
-                           "nlist_every": run["nlist_every"], "steps_per_api_call": block,
+                           "nlist_every": run["nlist_every"], "cell_edge": run.get("cell_edge", 0.0), "steps_per_api_call": block,
                            "l2": "value: flushed by a 256 MiB write between timed API calls (outside the event brackets); e2e: not flushed",
                            "baseline_note": "there is no reference implementation (the paper's lives in Tinker-HP): --impl reference and "
                                             "cpu_baseline time this repo's own fp64 oracle; absolute ns/day and roofline fractions are the figures of merit",
