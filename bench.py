@@ -236,7 +236,7 @@ def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, pro
     n_upd = max(prof["update"][1], 1)
     chains = 2.0 * n * (2 if run["flags"] & 2 else 1)                  # half-phases x (C' [+ J']) per jump update launch
     upd_instr = pstats["proposals"] / n_upd * PROPOSAL_INSTR + chains * CHAIN_INSTR
-    build_ms = prof["build"][0] / rebuilds                             # sort + k_universe + k_build_rows (and their idle launches), per rebuild
+    build_ms = prof["build"][0] / rebuilds                             # k_sort + k_build_rows (and their idle launches), per rebuild
     lines = {
         "pair": alu_line("k_pair (short-range switched pair gradient, a5)", half_pairs * FLOPS_PER_PAIR,
                          "%.0f in-range half pairs x %d flop" % (half_pairs, FLOPS_PER_PAIR), "pair"),
@@ -244,7 +244,7 @@ def kernel_rooflines(torch, sim, stream, step_call, K, block, flush, run, n, pro
                            2.0 * upd_instr,
                            "%.0f proposals x %d + %.0f chains x %d FP32/INT-pipe instructions, x 2 flop, per launch"
                            % (pstats["proposals"] / n_upd, PROPOSAL_INSTR, chains, CHAIN_INSTR), "update"),
-        "build": hbm_line("sort + k_universe + k_build_rows (a1-a3), per rebuild", row_entries * 4.0 + n * 48.0,
+        "build": hbm_line("k_sort + k_build_rows (a1-a3), per rebuild", row_entries * 4.0 + n * 48.0,
                           "%.0f row entries x 4 B + %d atoms x 48 B" % (row_entries, n), build_ms, "build"),
         "bonded": hbm_line("k_bonded_mol (+ k_bonded_csr) (a4), stand-alone", n * float(BONDED_BYTES_PER_ATOM),
                            "%d atoms x %d B" % (n, BONDED_BYTES_PER_ATOM), bonded_ms, "bonded"),

@@ -603,7 +603,7 @@ __global__ void __launch_bounds__(SORT_THREADS) k_sort(SortArgs a, Universe u, u
         a.orig[i] = a.orig_t[i];
     }
     if (!cum) return;
-    // running sums of the cell universe (k_universe's pass), one warp per home cell: reads cell_start only
+    // running sums of the cell universe (R-10c, ring C), one warp per home cell: reads cell_start only
     for (int h = t >> 5; h < ncell; h += nt >> 5) universe_cell(a.grid, u, a.cell_start, cum, a.ctr, h, t & 31);
 }
 
