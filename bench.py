@@ -355,6 +355,7 @@ def main():
         step_call(2 * block)
         sim.sync()
         sim.reset_stats()
+        rebuilds0 = sim.stats()["rebuilds"]                             # the sort counter runs on through reset_stats
         K = max(args.steps // block * block, block)
         W = max(args.warmup, 3)
         W_steps = max((W + block - 1) // block * block, block)
@@ -454,7 +455,8 @@ def main():
                 "events": {"proposals_per_atom_step": stats["proposals"] / (n * (K + W_steps)),
                            "accepts_per_atom_step": stats["accepts"] / (n * (K + W_steps)), "max_p": stats["max_p"],
                            "timed_region_error": timed_error,
-                           "max_disp_A": stats["max_disp"], "rebuilds": stats["rebuilds"], "error": err_end}}
+                           "max_disp_A": stats["max_disp"], "rebuilds": stats["rebuilds"] - rebuilds0,
+                           "steps_per_rebuild": (K + W_steps) / max(stats["rebuilds"] - rebuilds0, 1), "error": err_end}}
         if second is not None:
             line["secondary"] = second
         if cpu is not None:
