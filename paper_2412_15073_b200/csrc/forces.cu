@@ -22,6 +22,10 @@ __device__ inline float weighted_u(float chi, float u) {
     return W == W_SHORT ? chi * u : (1.f - chi) * u;
 }
 
+// CTAs of two warps: rows differ in length, and small CTAs leave an SM's slots sooner (256 threads: 630 us at 10^6
+// atoms, 128: 617, 64: 612)
+constexpr int PAIR_THREADS = 64;
+
 // One warp per atom over its row (entries: sorted index of j, bit 31 set when j carries LJ).
 // INTERIOR: the atom is farther than the row's reach + 2 skins from every box face, so no partner of its row can
 // be a periodic image: plain differences, no minimum image in the inner loop.
@@ -105,7 +109,7 @@ __device__ inline void pair_warp(const Model &m, const Row &row, const float4 *_
 }
 
 template <int WC, int WLJ, bool ENERGY>
-__global__ void __launch_bounds__(256) k_pair(Model m, Row row, float margin, const float4 *__restrict__ xs,
+__global__ void __launch_bounds__(PAIR_THREADS) k_pair(Model m, Row row, float margin, const float4 *__restrict__ xs,
                                               const float2 *__restrict__ lj, float4 *__restrict__ out, int accumulate) {
     int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (i >= m.n) return;
@@ -272,7 +276,7 @@ void launch_count_pairs(const Model &m, const Row &row, const float4 *xs, float 
 template <int WC, int WLJ>
 static void pair_dispatch(const Model &m, const Row &row, const float4 *xs, const float2 *lj, float4 *out, int accumulate,
                           bool energy, cudaStream_t st) {
-    const int B = 256;
+    const int B = PAIR_THREADS;
     unsigned grid = (unsigned)(((long long)m.n * 32 + B - 1) / B);
     const float margin = sqrtf(row.r2max) + 2.f * m.hs * m.w_max * 2.f;   // farthest entry at a build + what two atoms may move
     if (energy) k_pair<WC, WLJ, true><<<grid, B, 0, st>>>(m, row, margin, xs, lj, out, accumulate);
