@@ -180,7 +180,7 @@ def timed_blocks(torch, sim, stream, call, n_steps, block, flush):
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the `ncu --set full` captures of
 # `python bench.py --steps 40 --warmup 8 --equil 60 --no-cpu-baseline --secondary-config -1` on the default workload
 # (profiles/r2_cfg4_README.md, profiles/r2_cfg4_dram_bytes.csv); other workloads have no capture: null
-NCU_TRAFFIC_CFG4 = {"pair": 653.8e6, "update": 870.1e6, "build": 2584.0e6, "bonded": 41.8e6}   # build: k_build_rows + k_sort
+NCU_TRAFFIC_CFG4 = {"pair": 653.1e6, "update": 870.1e6, "build": 2584.0e6, "bonded": 41.8e6}   # build: k_build_rows + k_sort
 BONDED_BYTES_PER_ATOM = 56    # per water: 16 B record + 3 x (16 + 16 B read, 16 B written)
 
 
